@@ -1,0 +1,226 @@
+"""Seeded synthetic inputs shaped like the paper's workloads.
+
+This module holds NO arithmetic of the method (no f, no gradient, no GDA step): it only draws
+problem data and start points.  It is the one module that both the CPU oracle's tests and the CUDA
+path's tests/bench import, so that the two sides see identical arrays.
+
+Shapes follow BASELINE.json `configs` and SURVEY.md section 8(d):
+  cfg1  Max-Cut  G(20, p=0.5), unit weights, B=64           (brute-force checkable)
+  cfg2  Max-Cut  G(800, m=19176), unit weights, B=1024      (stands in for the 800-node Gset family)
+  cfg3  Max-Cut  G(20000, m=40000), weights +-1, B=256      (stands in for G81)
+  cfg4  dense QUBO n=4096, N(0,1) entries bf16-representable, B=4096
+  cfg5  weighted Max-3-SAT n=10000, m=42600, w in 1..10, B=512  (stands in for the 3-CNF set)
+Max-Cut is handed to the solvers in the paper's minimisation form F(x) = x^T W x - 1^T W x
+(PAPER.md:146, 604), i.e. Q = W (symmetric, both directions stored) and c = -W 1; cut(x) = -F(x).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Optional
+
+import numpy as np
+
+
+# --------------------------------------------------------------------------------------------
+# problem containers (plain arrays; host memory)
+# --------------------------------------------------------------------------------------------
+@dataclass
+class QuboCSR:
+    """F(x) = x^T Q x + c^T x, Q symmetric, given as CSR with both (i,j) and (j,i) stored."""
+    n: int
+    rowptr: np.ndarray  # int32 [n+1]
+    col: np.ndarray     # int32 [nnz]
+    val: np.ndarray     # float32 [nnz]
+    c: np.ndarray       # float32 [n]
+    edges: Optional[np.ndarray] = None  # int64 [m,2] (i<j) when the instance is a Max-Cut graph
+    edge_w: Optional[np.ndarray] = None  # float32 [m]
+
+
+@dataclass
+class QuboDense:
+    """F(x) = x^T Q x + c^T x, Q symmetric row-major [n,n] float32 (bf16-representable values)."""
+    n: int
+    Q: np.ndarray  # float32 [n,n]
+    c: np.ndarray  # float32 [n]
+
+
+@dataclass
+class MaxSat:
+    """F(x) = sum_j w_j [clause j unsatisfied]; lit = +-(var+1), DIMACS sign convention."""
+    n: int
+    m: int
+    cptr: np.ndarray  # int32 [m+1]
+    lit: np.ndarray   # int32 [L]
+    w: np.ndarray     # float32 [m]
+
+
+@dataclass
+class Hyper:
+    """(y-bar, alpha, beta, delta, g) and run lengths for one config (Table 6; R7)."""
+    lambda0: float
+    alpha: float
+    beta: float
+    delta: float = 1e-4
+    gfun: int = 0          # 0 quadratic x^2-x, 1 entropy
+    log_eps: float = 1e-6
+    iters: int = 1000
+    eval_every: int = 100
+    seed: int = 0
+
+
+@dataclass
+class Workload:
+    name: str
+    kind: str              # "qubo_csr" | "qubo_dense" | "maxsat"
+    problem: object
+    B: int
+    hyper: Hyper
+    x0_seed: int
+    note: str = ""
+    extra: dict = field(default_factory=dict)
+
+
+# --------------------------------------------------------------------------------------------
+# graph / matrix / formula generators
+# --------------------------------------------------------------------------------------------
+def edges_gnp(n: int, p: float, seed: int) -> np.ndarray:
+    """Erdos-Renyi G(n,p): one Bernoulli(p) draw per unordered pair, upper triangle, row-major."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    iu, ju = np.triu_indices(n, k=1)
+    keep = rng.random(iu.shape[0]) < p
+    return np.stack([iu[keep], ju[keep]], axis=1).astype(np.int64)
+
+
+def edges_gnm(n: int, m: int, seed: int) -> np.ndarray:
+    """G(n,m): m distinct unordered pairs i<j, uniform (oversample, dedupe, keep the first m)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    total = n * (n - 1) // 2
+    if m > total:
+        raise ValueError("m exceeds the number of pairs")
+    chosen = np.empty(0, dtype=np.int64)
+    while chosen.shape[0] < m:
+        a = rng.integers(0, n, size=2 * m + 16, dtype=np.int64)
+        b = rng.integers(0, n, size=2 * m + 16, dtype=np.int64)
+        ok = a != b
+        lo = np.minimum(a[ok], b[ok])
+        hi = np.maximum(a[ok], b[ok])
+        code = np.concatenate([chosen, lo * n + hi])
+        _, first = np.unique(code, return_index=True)
+        chosen = code[np.sort(first)]          # keep draw order, drop repeats
+    chosen = chosen[:m]
+    return np.stack([chosen // n, chosen % n], axis=1).astype(np.int64)
+
+
+def edge_weights(m: int, seed: int, kind: str) -> np.ndarray:
+    rng = np.random.Generator(np.random.PCG64(seed + 7919))
+    if kind == "unit":
+        return np.ones(m, dtype=np.float32)
+    if kind == "pm1":
+        return (2 * rng.integers(0, 2, size=m) - 1).astype(np.float32)
+    raise ValueError(kind)
+
+
+def maxcut_as_qubo(n: int, edges: np.ndarray, w: np.ndarray) -> QuboCSR:
+    """Q = W (symmetric CSR, zero diagonal, columns sorted), c = -W 1  (reading R8)."""
+    i = np.concatenate([edges[:, 0], edges[:, 1]])
+    j = np.concatenate([edges[:, 1], edges[:, 0]])
+    v = np.concatenate([w, w]).astype(np.float32)
+    order = np.lexsort((j, i))
+    i, j, v = i[order], j[order], v[order]
+    rowptr = np.zeros(n + 1, dtype=np.int64)
+    np.add.at(rowptr, i + 1, 1)
+    rowptr = np.cumsum(rowptr)
+    wdeg = np.zeros(n, dtype=np.float64)
+    np.add.at(wdeg, i, v.astype(np.float64))
+    return QuboCSR(n=n, rowptr=rowptr.astype(np.int32), col=j.astype(np.int32), val=v,
+                   c=(-wdeg).astype(np.float32), edges=edges, edge_w=w.astype(np.float32))
+
+
+def round_to_bf16(a: np.ndarray) -> np.ndarray:
+    """Round float32 values to the nearest bf16-representable value (ties to even), kept as float32."""
+    u = np.ascontiguousarray(a, dtype=np.float32).view(np.uint32).astype(np.uint64)
+    u = (u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000
+    return u.astype(np.uint32).view(np.float32).reshape(a.shape)
+
+
+def dense_qubo(n: int, seed: int) -> QuboDense:
+    """Q = triu(A,1) + triu(A,1)^T + diag(d), A,d ~ N(0,1), rounded to bf16 (reading R13); c ~ N(0,1)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    A = rng.standard_normal((n, n), dtype=np.float32)
+    d = rng.standard_normal(n, dtype=np.float32)
+    c = rng.standard_normal(n, dtype=np.float32)
+    U = np.triu(A, 1)
+    Q = U + U.T
+    Q[np.arange(n), np.arange(n)] = d
+    return QuboDense(n=n, Q=round_to_bf16(Q), c=c)
+
+
+def random_ksat(n: int, m: int, k: int, seed: int, wmax: int = 10) -> MaxSat:
+    """m clauses of k DISTINCT variables (uniform), uniform signs, integer weights uniform in 1..wmax."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    var = rng.integers(0, n, size=(m, k), dtype=np.int64)
+    while True:
+        s = np.sort(var, axis=1)
+        bad = np.nonzero((s[:, 1:] == s[:, :-1]).any(axis=1))[0]
+        if bad.size == 0:
+            break
+        var[bad] = rng.integers(0, n, size=(bad.size, k), dtype=np.int64)
+    sign = 2 * rng.integers(0, 2, size=(m, k), dtype=np.int64) - 1
+    w = rng.integers(1, wmax + 1, size=m).astype(np.float32)
+    lit = (sign * (var + 1)).astype(np.int32).reshape(-1)
+    cptr = (np.arange(m + 1, dtype=np.int64) * k).astype(np.int32)
+    return MaxSat(n=n, m=m, cptr=cptr, lit=lit, w=w)
+
+
+def x0_uniform(n: int, B: int, seed: int) -> np.ndarray:
+    """x0 ~ U[0,1)^(n x B), float32, layout [n][B]."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    return rng.random((n, B), dtype=np.float32)
+
+
+# --------------------------------------------------------------------------------------------
+# the five BASELINE.json configs (1-based like SURVEY.md section 8(d))
+# --------------------------------------------------------------------------------------------
+def config(idx: int, B: Optional[int] = None, n_scale: float = 1.0) -> Workload:
+    """Build config `idx` (1..5).  `B` overrides the restart count; `n_scale` shrinks n (and m)
+    proportionally for quick tests while keeping density / degree / clause ratio."""
+    if idx == 1:
+        n = 20
+        e = edges_gnp(n, 0.5, 101)
+        P = maxcut_as_qubo(n, e, edge_weights(e.shape[0], 101, "unit"))
+        return Workload("cfg1_maxcut_n20", "qubo_csr", P, B or 64,
+                        Hyper(6.0, 0.025, 0.025, 1e-4, 0, 1e-6, 1000, 50, 101), 1101,
+                        "Max-Cut G(20,0.5), unit weights; brute force 2^20")
+    if idx == 2:
+        n = max(8, int(round(800 * n_scale)))
+        m = int(round(19176 * n_scale * n_scale)) if n_scale != 1.0 else 19176
+        e = edges_gnm(n, m, 102)
+        P = maxcut_as_qubo(n, e, edge_weights(m, 102, "unit"))
+        return Workload("cfg2_maxcut_n800", "qubo_csr", P, B or 1024,
+                        Hyper(6.0, 0.008, 0.025, 1e-4, 0, 1e-6, 5000, 100, 102), 1102,
+                        "Max-Cut G(800,19176), unit weights; alpha per reading R7")
+    if idx == 3:
+        n = max(8, int(round(20000 * n_scale)))
+        m = 2 * n
+        e = edges_gnm(n, m, 103)
+        P = maxcut_as_qubo(n, e, edge_weights(m, 103, "pm1"))
+        return Workload("cfg3_maxcut_n20000", "qubo_csr", P, B or 256,
+                        Hyper(6.0, 0.025, 0.025, 1e-4, 0, 1e-6, 10000, 100, 103), 1103,
+                        "Max-Cut G(20000,40000), weights +-1")
+    if idx == 4:
+        n = max(128, int(round(4096 * n_scale)) // 128 * 128)
+        P = dense_qubo(n, 104)
+        s = 2.0 * np.sqrt(n)                      # spectral scale of the N(0,1) matrix (reading R7)
+        lam = 1.75 * s
+        return Workload("cfg4_dense_n4096", "qubo_dense", P, B or 4096,
+                        Hyper(float(lam), float(1.0 / (4.0 * (s + lam))), float(4.0 * lam / 1000.0),
+                              1e-4, 0, 1e-6, 2000, 100, 104), 1104,
+                        "dense QUBO N(0,1), bf16-representable Q")
+    if idx == 5:
+        n = max(8, int(round(10000 * n_scale)))
+        m = int(round(4.26 * n))
+        P = random_ksat(n, m, 3, 105)
+        return Workload("cfg5_max3sat_n10000", "maxsat", P, B or 512,
+                        Hyper(2.0, 0.01, 0.005, 1e-4, 1, 1e-6, 5000, 100, 105), 1105,
+                        "weighted Max-3-SAT ratio 4.26, w in 1..10, entropy g")
+    raise ValueError("config index must be 1..5")
