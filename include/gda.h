@@ -1,0 +1,146 @@
+/* include/gda.h -- C ABI of the B200-native GDA hot path of PDBO (arxiv 2509.21064).
+ *
+ * The library solves   min_{x in {0,1}^n} F(x)   (Eq. 1) by simultaneous projected
+ * gradient descent-ascent (Eq. 6) on the Lagrangian
+ *     L(x, y) = f(x) + sum_i y_i g(x_i)
+ * of the multilinear extension f of F (Def. 2.2, 69-73 Prop. 2.4), for B independent
+ * restarts at once, with periodic rounding, exact scoring and an arg-best over
+ * restarts.  The dual variable the paper calls y is `lambda` here.
+ *
+ * Conventions
+ *   - Plain C, no exceptions or aborts across the boundary; every entry point returns a gda_status and
+ *     leaves a thread-local message for gda_last_error().  `out` handles are NULL on failure.
+ *   - "HOST" / "DEVICE" says where a pointer must live.  The library never frees or keeps caller memory
+ *     (problem data is copied at create).
+ *   - Iterates are fp32, layout [n][B] row-major: element (variable i, restart b) at i*B + b, so the
+ *     restart index is contiguous.  B must be a positive multiple of 4 (128-bit vectors across restarts).
+ *   - gda_run / gda_grad / gda_score enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream) and return without synchronising; outputs are valid once the stream has
+ *     reached that point.  A handle must not be used from two streams or threads at the same time.
+ *   - All compute runs in CUDA kernels for sm_100a; there is no CPU fallback: without a usable device
+ *     every compute entry point fails with GDA_ERR_CUDA.
+ */
+#ifndef GDA_H_
+#define GDA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gda_problem gda_problem; /* opaque; owns the device copies of the problem and a workspace */
+
+typedef enum {
+    GDA_OK = 0,
+    GDA_ERR_INVALID_ARG = 1, /* null pointer, bad size, asymmetric Q, index out of range, bad parameter ... */
+    GDA_ERR_ALLOC = 2,       /* host or device allocation failed */
+    GDA_ERR_CUDA = 3,        /* a CUDA call or kernel launch failed (message has the CUDA error string) */
+    GDA_ERR_UNSUPPORTED = 4  /* valid request this build cannot serve (e.g. dense n not a multiple of 128) */
+} gda_status;
+
+/* binarity function g (default quadratic; entropy for Max-k-SAT, 580/592) */
+typedef enum {
+    GDA_G_QUADRATIC = 0, /* g(x) = x^2 - x,                     g'(x) = 2x - 1                      */
+    GDA_G_ENTROPY = 1    /* g(x) = x ln x + (1-x) ln(1-x), 0 at the ends; g'(x) = ln(xc) - ln(1-xc),
+                            xc = clip(x, log_eps, 1-log_eps)   (reading R4)               */
+} gda_gfun;
+
+#define GDA_DENSE_BF16 1 /* gda_create_qubo_dense flag: store Q in bf16, fp32 accumulate (tcgen05 path) */
+
+/* ---- problems ---------------------------------------------------------------------------------------
+ * QUBO: F(x) = x^T Q x + c^T x.  Q must be symmetric.  A non-zero diagonal is folded into
+ * the linear term, f(x) = sum_{i!=j} Q_ij x_i x_j + sum_i (Q_ii + c_i) x_i  (Prop. 2.4 with x_i^2 -> x_i;
+ * DESIGN.md reading R1).  Max-Cut with weight matrix W is Q = W, c = -W 1 and
+ * cut(x) = -F(x).
+ *
+ * gda_create_qubo_csr: HOST rowptr[n+1], col[nnz], val[nnz] (both (i,j) and (j,i) stored, any order within
+ *   a row, no duplicate (i,j)), HOST c[n] or NULL (= 0).
+ *   INVALID_ARG: n <= 0, null pointers, rowptr not non-decreasing from 0, column out of range, duplicate
+ *   entry, Q_ij != Q_ji, non-finite value. */
+gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, const int32_t* col, const float* val,
+                               const float* c, gda_problem** out);
+
+/* gda_create_qubo_dense: HOST Q row-major [n][n] (symmetric), HOST c[n] or NULL.  flags must contain
+ *   GDA_DENSE_BF16: Q is rounded to bf16 (lossless when Q is bf16-representable, reading R13)
+ *   and the gradient is a tcgen05 GEMM with fp32 accumulation.  UNSUPPORTED: n not a multiple of 128 or
+ *   flags without GDA_DENSE_BF16.  gda_run on a dense problem needs B to be a multiple of 128. */
+gda_status gda_create_qubo_dense(int32_t n, const float* Q, const float* c, int32_t flags, gda_problem** out);
+
+/* Weighted MaxSAT: F(x) = sum_j w_j [clause j unsatisfied] = sum_j w_j prod_{l in C_j} p_l(x)
+ * (weights: DESIGN.md reading R9).  HOST cptr[m+1], lit[cptr[m]] with
+ * lit = +(var+1) for a positive literal (p = 1 - x) and -(var+1) for a negated one (p = x), HOST w[m] or
+ * NULL (= all 1).  INVALID_ARG: empty clause, variable out of range, a variable repeated inside one clause
+ * (the product would not be the multilinear extension, reading R2), non-finite or negative weight. */
+gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cptr, const int32_t* lit, const float* w,
+                             gda_problem** out);
+
+void gda_destroy(gda_problem* p); /* NULL-safe; synchronises the device before freeing */
+
+/* ---- the run ----------------------------------------------------------------------------------------- */
+typedef struct {
+    float alpha;        /* primal step size > 0                                          */
+    float beta;         /* dual step size > 0                                          */
+    float delta;        /* perturbation band half-width in [0, 1/2); 0 disables (R3) */
+    float log_eps;      /* clamp for g' of the entropy g, in (0, 1/2) (R4); ignored for the quadratic g */
+    int32_t iters;      /* T_max >= 0: exactly this many GDA steps (R0)                                 */
+    int32_t eval_every; /* > 0: round + score every eval_every steps and after the last step (R5)       */
+    int32_t gfun;       /* gda_gfun                                                                     */
+    int32_t t0;         /* iteration index of x0 (only enters the exact-1/2 tie-break hash, R3)         */
+    uint64_t seed;      /* seed of that hash                                                            */
+} gda_params;
+
+/* Optional extra outputs of gda_run; every pointer is DEVICE memory and may be NULL. */
+typedef struct {
+    float* x_final;       /* [n][B] iterate x^T                                                         */
+    float* lambda_final;  /* [n][B] dual iterate y^T                                                    */
+    double* best_obj;     /* [1]    obj[best_restart]                                                   */
+    double* trace_best;   /* [trace_cap] min over restarts of the best objective after evaluation k     */
+    uint64_t* trace_ns;   /* [trace_cap] GPU globaltimer (ns) when evaluation k finished                */
+    int32_t trace_cap;    /* entries available in the two trace arrays (evaluations beyond it are dropped) */
+} gda_extra;
+
+/* Algorithm 1 (reconstructed in DESIGN.md reading R0) for B restarts.
+ *   x0          DEVICE fp32 [n][B], values in [0,1]           (x0 ~ U[0,1]^n)
+ *   lambda0     DEVICE fp32 [n][B] or NULL -> every entry = lambda0_scalar (y-bar)
+ *   x_bin       DEVICE uint8 [n][B]: per restart, the rounded point x_hat = [x > 1/2] with the best
+ *               objective seen at any evaluation (R5)
+ *   obj         DEVICE double [B]: F(x_bin[:,b]) -- exact integers when all coefficients are integers
+ *   best_restart DEVICE int32 [1]: argmin_b obj[b], ties -> lowest b (R6)
+ * INVALID_ARG: null required pointer, B <= 0 or B % 4 != 0, alpha/beta <= 0 or non-finite, delta outside
+ * [0, 1/2), eval_every <= 0, iters < 0, unknown gfun, log_eps outside (0, 1/2) with the entropy g.       */
+gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const float* lambda0, float lambda0_scalar,
+                   const gda_params* params, uint8_t* x_bin, double* obj, int32_t* best_restart,
+                   const gda_extra* extra, void* stream);
+
+/* Same run with HOST buffers (x0, lambda0, x_bin, obj, best_restart on the host; `extra` must be NULL):
+ * copies the inputs to the device, runs, copies the three results back and synchronises `stream`. */
+gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, const float* lambda0, float lambda0_scalar,
+                        const gda_params* params, uint8_t* x_bin, double* obj, int32_t* best_restart,
+                        void* stream);
+
+/* ---- single steps of the path, exposed for parity tests and profiling ---------------------------------
+ * gda_grad:  G = grad f(X), DEVICE fp32 [n][B] in and out (S1 sparse / S2 dense / S3 MaxSAT of DESIGN.md).
+ * gda_score: obj[b] = F(x_hat), x_hat = [X[:,b] > 1/2]; DEVICE fp32 X [n][B], DEVICE double obj[B] (S5). */
+gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float* G, void* stream);
+gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, void* stream);
+
+/* ---- queries ------------------------------------------------------------------------------------------ */
+typedef struct {
+    int32_t kind;        /* 0 sparse QUBO, 1 dense QUBO, 2 MaxSAT                                       */
+    int32_t n;
+    int64_t nnz;         /* off-diagonal non-zeros (sparse), n*n (dense), literals (MaxSAT)             */
+    int32_t m;           /* clauses (MaxSAT), else 0                                                    */
+    int32_t integral;    /* 1 when every coefficient is an integer: objectives are accumulated in int64 */
+    int64_t last_run_kernel_launches; /* kernels launched by the most recent gda_run on this handle     */
+    int64_t last_run_step_launches;   /* of those, launches of the per-step kernel                      */
+} gda_info;
+gda_status gda_get_info(const gda_problem* p, gda_info* info);
+
+const char* gda_last_error(void); /* thread-local message of the last non-OK status ("" if none) */
+const char* gda_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GDA_H_ */

@@ -1,0 +1,589 @@
+// gda_api.cu -- the C ABI of include/gda.h: validation and preprocessing at create, workspace,
+// CUDA-graph-captured run loop, host-buffer variant, single-step entry points.
+#include "gda_internal.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+int sparse_heavy_threshold();
+
+// ---------------------------------------------------------------------------------------------------
+// errors
+// ---------------------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+void gda_set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+extern "C" const char* gda_last_error(void) { return g_err; }
+extern "C" const char* gda_version(void) { return "gda-b200 0.1 (sm_100a)"; }
+
+#define GDA_REQUIRE(cond, ...)                 \
+    do {                                       \
+        if (!(cond)) {                         \
+            gda_set_error(__VA_ARGS__);        \
+            return GDA_ERR_INVALID_ARG;        \
+        }                                      \
+    } while (0)
+
+template <typename T>
+static gda_status upload(T** dptr, const std::vector<T>& h) {
+    *dptr = nullptr;
+    const size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(T);
+    if (cudaMalloc((void**)dptr, bytes) != cudaSuccess) {
+        gda_set_error("device allocation of %zu bytes failed: %s", bytes, cudaGetErrorString(cudaGetLastError()));
+        return GDA_ERR_ALLOC;
+    }
+    if (!h.empty()) GDA_CUDA_TRY(cudaMemcpy(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return GDA_OK;
+}
+
+static gda_status device_setup(gda_problem* p) {
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess || count == 0) {
+        gda_set_error("no usable CUDA device (%s); this library has no CPU fallback",
+                      e != cudaSuccess ? cudaGetErrorString(e) : "device count is 0");
+        cudaGetLastError();
+        return GDA_ERR_CUDA;
+    }
+    GDA_CUDA_TRY(cudaGetDevice(&p->device));
+    cudaDeviceProp prop;
+    GDA_CUDA_TRY(cudaGetDeviceProperties(&prop, p->device));
+    if (prop.major != 10) {
+        gda_set_error("device '%s' is sm_%d%d; this library is built for sm_100a (B200) only", prop.name,
+                      prop.major, prop.minor);
+        return GDA_ERR_UNSUPPORTED;
+    }
+    p->num_sms = prop.multiProcessorCount;
+    return GDA_OK;
+}
+
+static bool is_integer_valued(float v, float limit) { return std::isfinite(v) && v == std::nearbyint(v) && std::fabs(v) <= limit; }
+
+// ---------------------------------------------------------------------------------------------------
+// create: sparse QUBO
+// ---------------------------------------------------------------------------------------------------
+extern "C" gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, const int32_t* col, const float* val,
+                                          const float* c, gda_problem** out) {
+    if (out) *out = nullptr;
+    GDA_REQUIRE(out != nullptr, "gda_create_qubo_csr: out is NULL");
+    GDA_REQUIRE(n > 0, "gda_create_qubo_csr: n must be > 0 (got %d)", n);
+    GDA_REQUIRE(rowptr != nullptr, "gda_create_qubo_csr: rowptr is NULL");
+    GDA_REQUIRE(rowptr[0] == 0, "gda_create_qubo_csr: rowptr[0] must be 0");
+    for (int i = 0; i < n; ++i)
+        GDA_REQUIRE(rowptr[i + 1] >= rowptr[i], "gda_create_qubo_csr: rowptr decreases at row %d", i);
+    const int64_t nnz_in = rowptr[n];
+    GDA_REQUIRE(nnz_in == 0 || (col != nullptr && val != nullptr), "gda_create_qubo_csr: col/val is NULL");
+
+    // sort each row by column, check range / duplicates / finiteness
+    std::vector<std::pair<int32_t, float>> ent((size_t)nnz_in);
+    for (int i = 0; i < n; ++i) {
+        for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+            GDA_REQUIRE(col[k] >= 0 && col[k] < n, "gda_create_qubo_csr: column %d out of range in row %d", col[k], i);
+            GDA_REQUIRE(std::isfinite(val[k]), "gda_create_qubo_csr: non-finite value in row %d", i);
+            ent[k] = {col[k], val[k]};
+        }
+        std::sort(ent.begin() + rowptr[i], ent.begin() + rowptr[i + 1]);
+        for (int k = rowptr[i] + 1; k < rowptr[i + 1]; ++k)
+            GDA_REQUIRE(ent[k].first != ent[k - 1].first, "gda_create_qubo_csr: duplicate entry (%d,%d)", i, ent[k].first);
+    }
+    // symmetry: Q_ij == Q_ji exactly
+    for (int i = 0; i < n; ++i)
+        for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+            const int j = ent[k].first;
+            if (j == i) continue;
+            auto lo = ent.begin() + rowptr[j], hi = ent.begin() + rowptr[j + 1];
+            auto it = std::lower_bound(lo, hi, std::make_pair((int32_t)i, -INFINITY));
+            GDA_REQUIRE(it != hi && it->first == i && it->second == ent[k].second,
+                        "gda_create_qubo_csr: Q is not symmetric at (%d,%d)", i, j);
+        }
+    // fold the diagonal into the linear term (reading R1), double the off-diagonal (G = 2 Q_off x + c')
+    std::vector<int32_t> h_rowptr(n + 1, 0), h_col;
+    std::vector<float> h_val2, h_cp(n);
+    std::vector<int32_t> heavy, light;
+    h_col.reserve(nnz_in); h_val2.reserve(nnz_in);
+    bool integral = true;
+    int32_t max_deg = 0;
+    for (int i = 0; i < n; ++i) {
+        float cp = c ? c[i] : 0.0f;
+        GDA_REQUIRE(std::isfinite(cp), "gda_create_qubo_csr: non-finite c[%d]", i);
+        double abs_row = 0.0;
+        for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+            if (ent[k].first == i) { cp += ent[k].second; continue; }
+            h_col.push_back(ent[k].first);
+            h_val2.push_back(2.0f * ent[k].second);
+            integral = integral && is_integer_valued(ent[k].second, 1048576.0f);
+            abs_row += std::fabs(2.0 * ent[k].second);
+        }
+        h_cp[i] = cp;
+        integral = integral && is_integer_valued(cp, 1073741824.0f) && abs_row < 1073741824.0;
+        h_rowptr[i + 1] = (int32_t)h_col.size();
+        const int32_t deg = h_rowptr[i + 1] - h_rowptr[i];
+        max_deg = std::max(max_deg, deg);
+        (deg > sparse_heavy_threshold() ? heavy : light).push_back(i);
+    }
+
+    gda_problem* p = new (std::nothrow) gda_problem();
+    if (!p) { gda_set_error("host allocation failed"); return GDA_ERR_ALLOC; }
+    p->kind = GDA_KIND_SPARSE; p->n = n; p->nnz = (int64_t)h_col.size(); p->integral = integral ? 1 : 0;
+    p->max_deg = max_deg;
+    gda_status st = device_setup(p);
+    if (st == GDA_OK) st = upload(&p->d_rowptr, h_rowptr);
+    if (st == GDA_OK) st = upload(&p->d_col, h_col);
+    if (st == GDA_OK) st = upload(&p->d_val2, h_val2);
+    if (st == GDA_OK) st = upload(&p->d_cprime, h_cp);
+    if (st == GDA_OK && !heavy.empty()) {
+        p->n_heavy = (int32_t)heavy.size(); p->n_light = (int32_t)light.size();
+        st = upload(&p->d_heavy_rows, heavy);
+        if (st == GDA_OK) st = upload(&p->d_light_rows, light);
+    }
+    if (st != GDA_OK) { gda_destroy(p); return st; }
+    *out = p;
+    return GDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// create: dense QUBO (the heavy lifting is in gda_dense.cu)
+// ---------------------------------------------------------------------------------------------------
+extern "C" gda_status gda_create_qubo_dense(int32_t n, const float* Q, const float* c, int32_t flags,
+                                            gda_problem** out) {
+    if (out) *out = nullptr;
+    GDA_REQUIRE(out != nullptr, "gda_create_qubo_dense: out is NULL");
+    GDA_REQUIRE(n > 0, "gda_create_qubo_dense: n must be > 0 (got %d)", n);
+    GDA_REQUIRE(Q != nullptr, "gda_create_qubo_dense: Q is NULL");
+    if (!(flags & GDA_DENSE_BF16)) { gda_set_error("gda_create_qubo_dense: only GDA_DENSE_BF16 is implemented"); return GDA_ERR_UNSUPPORTED; }
+    if (n % 128 != 0) { gda_set_error("gda_create_qubo_dense: n must be a multiple of 128 (got %d)", n); return GDA_ERR_UNSUPPORTED; }
+    for (int i = 0; i < n; ++i) {
+        GDA_REQUIRE(!c || std::isfinite(c[i]), "gda_create_qubo_dense: non-finite c[%d]", i);
+        for (int j = i; j < n; ++j) {
+            const float a = Q[(size_t)i * n + j], b = Q[(size_t)j * n + i];
+            GDA_REQUIRE(std::isfinite(a), "gda_create_qubo_dense: non-finite Q[%d][%d]", i, j);
+            GDA_REQUIRE(a == b, "gda_create_qubo_dense: Q is not symmetric at (%d,%d)", i, j);
+        }
+    }
+    gda_problem* p = new (std::nothrow) gda_problem();
+    if (!p) { gda_set_error("host allocation failed"); return GDA_ERR_ALLOC; }
+    p->kind = GDA_KIND_DENSE; p->n = n; p->nnz = (int64_t)n * n; p->integral = 0;
+    gda_status st = device_setup(p);
+    if (st == GDA_OK) st = dense_prepare(p, Q, c);
+    if (st != GDA_OK) { gda_destroy(p); return st; }
+    *out = p;
+    return GDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// create: MaxSAT
+// ---------------------------------------------------------------------------------------------------
+extern "C" gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cptr, const int32_t* lit, const float* w,
+                                        gda_problem** out) {
+    if (out) *out = nullptr;
+    GDA_REQUIRE(out != nullptr, "gda_create_maxsat: out is NULL");
+    GDA_REQUIRE(n > 0 && m > 0, "gda_create_maxsat: n and m must be > 0 (got %d, %d)", n, m);
+    GDA_REQUIRE(cptr != nullptr && lit != nullptr, "gda_create_maxsat: cptr/lit is NULL");
+    GDA_REQUIRE(cptr[0] == 0, "gda_create_maxsat: cptr[0] must be 0");
+    int32_t kmax = 0;
+    bool integral = true;
+    std::vector<int32_t> occ(n + 1, 0), tmp;
+    for (int j = 0; j < m; ++j) {
+        const int k = cptr[j + 1] - cptr[j];
+        GDA_REQUIRE(k > 0, "gda_create_maxsat: clause %d is empty", j);
+        kmax = std::max(kmax, k);
+        tmp.clear();
+        for (int a = cptr[j]; a < cptr[j + 1]; ++a) {
+            const int l = lit[a];
+            const int v = (l > 0 ? l : -l) - 1;
+            GDA_REQUIRE(l != 0 && v < n, "gda_create_maxsat: literal %d of clause %d out of range", l, j);
+            tmp.push_back(v);
+            ++occ[v + 1];
+        }
+        std::sort(tmp.begin(), tmp.end());
+        for (size_t a = 1; a < tmp.size(); ++a)
+            GDA_REQUIRE(tmp[a] != tmp[a - 1], "gda_create_maxsat: variable %d repeated in clause %d", tmp[a], j);
+        const float wj = w ? w[j] : 1.0f;
+        GDA_REQUIRE(std::isfinite(wj) && wj >= 0.0f, "gda_create_maxsat: weight of clause %d is negative or non-finite", j);
+        integral = integral && is_integer_valued(wj, 1048576.0f);
+    }
+    if (kmax > 65) { gda_set_error("gda_create_maxsat: clauses longer than 65 literals are not supported (got %d)", kmax); return GDA_ERR_UNSUPPORTED; }
+    const int64_t L = cptr[m];
+    const int32_t kw = std::max(kmax - 1, 1);
+    for (int i = 0; i < n; ++i) occ[i + 1] += occ[i];
+    std::vector<int32_t> h_vptr(occ), next(occ.begin(), occ.end() - 1);
+    std::vector<float> h_coef((size_t)L), h_w(m);
+    std::vector<int32_t> h_others((size_t)L * kw, 0);
+    for (int j = 0; j < m; ++j) {
+        const float wj = w ? w[j] : 1.0f;
+        h_w[j] = wj;
+        for (int a = cptr[j]; a < cptr[j + 1]; ++a) {
+            const int l = lit[a];
+            const int v = (l > 0 ? l : -l) - 1;
+            const int s = next[v]++;
+            h_coef[s] = l > 0 ? -wj : wj;                    // d/dx of p: -1 for a positive literal, +1 for a negated one
+            int q = 0;
+            for (int b = cptr[j]; b < cptr[j + 1]; ++b)
+                if (b != a) h_others[(size_t)s * kw + q++] = lit[b];
+        }
+    }
+    gda_problem* p = new (std::nothrow) gda_problem();
+    if (!p) { gda_set_error("host allocation failed"); return GDA_ERR_ALLOC; }
+    p->kind = GDA_KIND_MAXSAT; p->n = n; p->m = m; p->nnz = L; p->integral = integral ? 1 : 0;
+    p->kw = kw; p->kmax = kmax;
+    gda_status st = device_setup(p);
+    if (st == GDA_OK) st = upload(&p->d_vptr, h_vptr);
+    if (st == GDA_OK) st = upload(&p->d_coef, h_coef);
+    if (st == GDA_OK) st = upload(&p->d_others, h_others);
+    if (st == GDA_OK) st = upload(&p->d_cptr, std::vector<int32_t>(cptr, cptr + m + 1));
+    if (st == GDA_OK) st = upload(&p->d_lit, std::vector<int32_t>(lit, lit + L));
+    if (st == GDA_OK) st = upload(&p->d_w, h_w);
+    if (st != GDA_OK) { gda_destroy(p); return st; }
+    *out = p;
+    return GDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// workspace / destroy
+// ---------------------------------------------------------------------------------------------------
+static void drop_graphs(gda_problem* p) {
+    for (auto& g : p->graphs) {
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+        if (g.graph) cudaGraphDestroy(g.graph);
+    }
+    p->graphs.clear();
+}
+
+static void free_workspace(gda_problem* p) {
+    Workspace& ws = p->ws;
+    drop_graphs(p);
+    cudaFree(ws.x[0]); cudaFree(ws.x[1]); cudaFree(ws.y); cudaFree(ws.x_bin); cudaFree(ws.best_obj);
+    cudaFree(ws.obj_now); cudaFree(ws.improved); cudaFree(ws.partial); cudaFree(ws.state);
+    cudaFree(ws.best_restart); cudaFree(ws.best_val); cudaFree(ws.trace_best); cudaFree(ws.trace_ns);
+    cudaFree(ws.zt[0]); cudaFree(ws.zt[1]); cudaFree(ws.gtmp);
+    if (ws.h_x0) cudaFreeHost(ws.h_x0);
+    if (ws.h_l0) cudaFreeHost(ws.h_l0);
+    ws = Workspace();
+}
+
+extern "C" void gda_destroy(gda_problem* p) {
+    if (!p) return;
+    cudaDeviceSynchronize();
+    free_workspace(p);
+    cudaFree(p->d_rowptr); cudaFree(p->d_col); cudaFree(p->d_val2); cudaFree(p->d_cprime);
+    cudaFree(p->d_heavy_rows); cudaFree(p->d_light_rows);
+    cudaFree(p->d_vptr); cudaFree(p->d_coef); cudaFree(p->d_others); cudaFree(p->d_cptr); cudaFree(p->d_lit); cudaFree(p->d_w);
+    dense_release(p);
+    if (p->own_stream) cudaStreamDestroy(p->own_stream);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
+    cudaGetLastError();
+    delete p;
+}
+
+static int32_t num_partials(const gda_problem* p, int32_t B) {
+    switch (p->kind) {
+        case GDA_KIND_SPARSE: return sparse_num_partials(p, B);
+        case GDA_KIND_MAXSAT: return maxsat_num_partials(p, B);
+        default: return dense_num_partials(p, B);
+    }
+}
+
+template <typename T>
+static gda_status dmalloc(T** ptr, size_t count) {
+    const size_t bytes = std::max<size_t>(count, 1) * sizeof(T);
+    if (cudaMalloc((void**)ptr, bytes) != cudaSuccess) {
+        *ptr = nullptr;
+        gda_set_error("device allocation of %zu bytes failed: %s", bytes, cudaGetErrorString(cudaGetLastError()));
+        return GDA_ERR_ALLOC;
+    }
+    return GDA_OK;
+}
+
+static const int32_t TRACE_CAP = 4096;
+
+static gda_status ensure_workspace(gda_problem* p, int32_t B) {
+    Workspace& ws = p->ws;
+    if (ws.B == B) return GDA_OK;
+    GDA_CUDA_TRY(cudaDeviceSynchronize());
+    free_workspace(p);
+    const size_t elems = (size_t)p->n * B;
+    gda_status st = GDA_OK;
+    if (p->kind != GDA_KIND_DENSE) {
+        if (st == GDA_OK) st = dmalloc(&ws.x[1], elems);
+    } else {
+        if (st == GDA_OK) st = dmalloc(&ws.zt[0], elems);
+        if (st == GDA_OK) st = dmalloc(&ws.zt[1], elems);
+    }
+    if (st == GDA_OK) st = dmalloc(&ws.x[0], elems);
+    if (st == GDA_OK) st = dmalloc(&ws.y, elems);
+    if (st == GDA_OK) st = dmalloc(&ws.x_bin, elems);
+    if (st == GDA_OK) st = dmalloc(&ws.best_obj, (size_t)B);
+    if (st == GDA_OK) st = dmalloc(&ws.obj_now, (size_t)B);
+    if (st == GDA_OK) st = dmalloc(&ws.improved, (size_t)B);
+    ws.n_part = num_partials(p, B);
+    if (st == GDA_OK) st = dmalloc((double**)&ws.partial, (size_t)ws.n_part * B);
+    if (st == GDA_OK) st = dmalloc(&ws.state, 1);
+    if (st == GDA_OK) st = dmalloc(&ws.best_restart, 1);
+    if (st == GDA_OK) st = dmalloc(&ws.best_val, 1);
+    ws.trace_cap = TRACE_CAP;
+    if (st == GDA_OK) st = dmalloc(&ws.trace_best, (size_t)TRACE_CAP);
+    if (st == GDA_OK) st = dmalloc(&ws.trace_ns, (size_t)TRACE_CAP);
+    if (st != GDA_OK) { free_workspace(p); return st; }
+    ws.B = B;
+    return GDA_OK;
+}
+
+// the caller's stream, or our own when the caller's cannot be captured (legacy default stream)
+static gda_status pick_stream(gda_problem* p, void* stream, cudaStream_t* user, cudaStream_t* exec) {
+    *user = (cudaStream_t)stream;
+    if (stream != nullptr && *user != cudaStreamLegacy) { *exec = *user; return GDA_OK; }
+    if (!p->own_stream) {
+        GDA_CUDA_TRY(cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking));
+        GDA_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
+        GDA_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming));
+    }
+    *exec = p->own_stream;
+    GDA_CUDA_TRY(cudaEventRecord(p->ev_fork, *user));
+    GDA_CUDA_TRY(cudaStreamWaitEvent(*exec, p->ev_fork, 0));
+    return GDA_OK;
+}
+
+static gda_status join_stream(gda_problem* p, cudaStream_t user, cudaStream_t exec) {
+    if (user == exec) return GDA_OK;
+    GDA_CUDA_TRY(cudaEventRecord(p->ev_join, exec));
+    GDA_CUDA_TRY(cudaStreamWaitEvent(user, p->ev_join, 0));
+    return GDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// one chunk = `len` GDA steps followed by one evaluation (round, score, best-so-far, commit)
+// ---------------------------------------------------------------------------------------------------
+static UpdParams make_upd(const gda_params& prm) {
+    UpdParams up;
+    up.alpha = prm.alpha; up.beta = prm.beta; up.delta = prm.delta; up.log_eps = prm.log_eps;
+    up.gfun = prm.gfun;
+    up.seed_mix = mix32((uint32_t)prm.seed ^ ((uint32_t)(prm.seed >> 32) * 0x9E3779B9u));
+    return up;
+}
+
+static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t parity, const gda_params& prm,
+                                cudaStream_t s, int64_t* launches, int64_t* step_launches) {
+    Workspace& ws = p->ws;
+    const UpdParams up = make_upd(prm);
+    int cur = parity;
+    for (int k = 0; k < len; ++k) {
+        int64_t before = *launches;
+        if (p->kind == GDA_KIND_SPARSE)
+            GDA_TRY(sparse_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, ws.state, (uint32_t)k, s, launches));
+        else if (p->kind == GDA_KIND_MAXSAT)
+            GDA_TRY(maxsat_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, ws.state, (uint32_t)k, s, launches));
+        else
+            GDA_TRY(dense_step(p, B, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, ws.state, (uint32_t)k, s, launches));
+        *step_launches += *launches - before;
+        cur ^= 1;
+    }
+    const float* xcur = (p->kind == GDA_KIND_DENSE) ? ws.x[0] : ws.x[cur];
+    int32_t n_part = 0;
+    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
+    else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
+    else GDA_TRY(dense_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
+    GDA_TRY(eval_finalize(p, B, ws.partial, n_part, ws.obj_now, ws.best_obj, ws.improved, ws.state, ws.trace_best,
+                          ws.trace_ns, ws.trace_cap, (uint32_t)len, s, launches));
+    GDA_TRY(eval_commit(p, B, xcur, ws.improved, ws.x_bin, s, launches));
+    return GDA_OK;
+}
+
+bool GraphKey::operator==(const GraphKey& o) const {
+    return B == o.B && len == o.len && parity == o.parity && with_eval == o.with_eval &&
+           prm.alpha == o.prm.alpha && prm.beta == o.prm.beta && prm.delta == o.prm.delta &&
+           prm.log_eps == o.prm.log_eps && prm.gfun == o.prm.gfun && prm.seed == o.prm.seed;
+}
+
+static bool graphs_disabled() {
+    const char* e = getenv("GDA_NO_GRAPH");
+    return e && e[0] && e[0] != '0';
+}
+
+static gda_status launch_chunk(gda_problem* p, int32_t B, int32_t len, int32_t parity, const gda_params& prm,
+                               cudaStream_t s) {
+    if (graphs_disabled() || len == 0) {
+        return enqueue_chunk(p, B, len, parity, prm, s, &p->last_launches, &p->last_step_launches);
+    }
+    GraphKey key;
+    key.B = B; key.len = len; key.parity = parity; key.with_eval = 1; key.prm = prm;
+    CachedGraph* hit = nullptr;
+    for (auto& g : p->graphs) if (g.key == key) { hit = &g; break; }
+    if (!hit) {
+        if (p->graphs.size() >= 8) drop_graphs(p);
+        CachedGraph g;
+        g.key = key;
+        GDA_CUDA_TRY(cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+        gda_status st = enqueue_chunk(p, B, len, parity, prm, s, &g.launches, &g.step_launches);
+        cudaError_t e = cudaStreamEndCapture(s, &g.graph);
+        if (st != GDA_OK) { if (g.graph) cudaGraphDestroy(g.graph); return st; }
+        if (e != cudaSuccess) { gda_set_error("cudaStreamEndCapture failed: %s", cudaGetErrorString(e)); return GDA_ERR_CUDA; }
+        e = cudaGraphInstantiate(&g.exec, g.graph, 0);
+        if (e != cudaSuccess) {
+            cudaGraphDestroy(g.graph);
+            gda_set_error("cudaGraphInstantiate failed: %s", cudaGetErrorString(e));
+            return GDA_ERR_CUDA;
+        }
+        p->graphs.push_back(g);
+        hit = &p->graphs.back();
+    }
+    GDA_CUDA_TRY(cudaGraphLaunch(hit->exec, s));
+    p->last_launches += hit->launches;
+    p->last_step_launches += hit->step_launches;
+    return GDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// gda_run
+// ---------------------------------------------------------------------------------------------------
+static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x0, const gda_params* prm,
+                                 const void* x_bin, const void* obj, const void* best_restart) {
+    GDA_REQUIRE(p != nullptr, "gda_run: problem is NULL");
+    GDA_REQUIRE(prm != nullptr, "gda_run: params is NULL");
+    GDA_REQUIRE(x0 != nullptr && x_bin != nullptr && obj != nullptr && best_restart != nullptr,
+                "gda_run: x0, x_bin, obj and best_restart are required");
+    GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_run: B must be a positive multiple of 4 (got %d)", B);
+    GDA_REQUIRE(std::isfinite(prm->alpha) && prm->alpha > 0.0f, "gda_run: alpha must be > 0");
+    GDA_REQUIRE(std::isfinite(prm->beta) && prm->beta > 0.0f, "gda_run: beta must be > 0");
+    GDA_REQUIRE(prm->delta >= 0.0f && prm->delta < 0.5f, "gda_run: delta must be in [0, 1/2)");
+    GDA_REQUIRE(prm->eval_every > 0, "gda_run: eval_every must be > 0");
+    GDA_REQUIRE(prm->iters >= 0, "gda_run: iters must be >= 0");
+    GDA_REQUIRE(prm->gfun == GDA_G_QUADRATIC || prm->gfun == GDA_G_ENTROPY, "gda_run: unknown gfun %d", prm->gfun);
+    if (prm->gfun == GDA_G_ENTROPY)
+        GDA_REQUIRE(prm->log_eps > 0.0f && prm->log_eps < 0.5f, "gda_run: log_eps must be in (0, 1/2) for the entropy g");
+    if (p->kind == GDA_KIND_DENSE && B % 128 != 0) {
+        gda_set_error("gda_run: the dense path needs B to be a multiple of 128 (got %d)", B);
+        return GDA_ERR_UNSUPPORTED;
+    }
+    return GDA_OK;
+}
+
+extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const float* lambda0, float lambda0_scalar,
+                              const gda_params* prm, uint8_t* x_bin, double* obj, int32_t* best_restart,
+                              const gda_extra* extra, void* stream) {
+    GDA_TRY(check_run_args(p, B, x0, prm, x_bin, obj, best_restart));
+    GDA_CUDA_TRY(cudaSetDevice(p->device));
+    GDA_TRY(ensure_workspace(p, B));
+    cudaStream_t user, s;
+    GDA_TRY(pick_stream(p, stream, &user, &s));
+    Workspace& ws = p->ws;
+    const size_t elems = (size_t)p->n * B;
+    p->last_launches = 0; p->last_step_launches = 0;
+
+    GDA_TRY(run_init(p, B, x0, lambda0, lambda0_scalar, (uint32_t)prm->t0, s, &p->last_launches));
+    int parity = 0;
+    if (p->kind == GDA_KIND_DENSE)
+        GDA_TRY(dense_make_operand(p, B, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
+    const int32_t full = prm->iters / prm->eval_every, rem = prm->iters % prm->eval_every;
+    for (int32_t c = 0; c < full; ++c) {
+        GDA_TRY(launch_chunk(p, B, prm->eval_every, parity, *prm, s));
+        parity ^= (prm->eval_every & 1);
+    }
+    if (rem > 0) { GDA_TRY(launch_chunk(p, B, rem, parity, *prm, s)); parity ^= (rem & 1); }
+    if (prm->iters == 0) GDA_TRY(launch_chunk(p, B, 0, parity, *prm, s));     // evaluate the start point
+    GDA_TRY(eval_argbest(B, ws.best_obj, ws.best_restart, ws.best_val, s, &p->last_launches));
+
+    const float* xfin = (p->kind == GDA_KIND_DENSE) ? ws.x[0] : ws.x[parity];
+    GDA_CUDA_TRY(cudaMemcpyAsync(x_bin, ws.x_bin, elems, cudaMemcpyDeviceToDevice, s));
+    GDA_CUDA_TRY(cudaMemcpyAsync(obj, ws.best_obj, (size_t)B * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    GDA_CUDA_TRY(cudaMemcpyAsync(best_restart, ws.best_restart, sizeof(int32_t), cudaMemcpyDeviceToDevice, s));
+    if (extra) {
+        if (extra->x_final) GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, xfin, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        if (extra->lambda_final) GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.y, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        if (extra->best_obj) GDA_CUDA_TRY(cudaMemcpyAsync(extra->best_obj, ws.best_val, sizeof(double), cudaMemcpyDeviceToDevice, s));
+        const int32_t n_eval = std::max(1, full + (rem > 0 ? 1 : 0));
+        const int32_t cnt = std::min(std::min(n_eval, extra->trace_cap), ws.trace_cap);
+        if (extra->trace_best && cnt > 0) GDA_CUDA_TRY(cudaMemcpyAsync(extra->trace_best, ws.trace_best, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToDevice, s));
+        if (extra->trace_ns && cnt > 0) GDA_CUDA_TRY(cudaMemcpyAsync(extra->trace_ns, ws.trace_ns, (size_t)cnt * sizeof(uint64_t), cudaMemcpyDeviceToDevice, s));
+    }
+    return join_stream(p, user, s);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// gda_run_host: same run, HOST buffers in and out (copies are part of the call)
+// ---------------------------------------------------------------------------------------------------
+extern "C" gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, const float* lambda0,
+                                   float lambda0_scalar, const gda_params* prm, uint8_t* x_bin, double* obj,
+                                   int32_t* best_restart, void* stream) {
+    GDA_TRY(check_run_args(p, B, x0, prm, x_bin, obj, best_restart));
+    GDA_CUDA_TRY(cudaSetDevice(p->device));
+    GDA_TRY(ensure_workspace(p, B));
+    cudaStream_t user, s;
+    GDA_TRY(pick_stream(p, stream, &user, &s));
+    Workspace& ws = p->ws;
+    const size_t elems = (size_t)p->n * B;
+    // device staging: x0 -> x[1] would be clobbered by the run, so stage in dedicated buffers
+    float* d_x0 = nullptr; float* d_l0 = nullptr; uint8_t* d_xb = nullptr; double* d_obj = nullptr; int32_t* d_best = nullptr;
+    gda_status st = dmalloc(&d_x0, elems);
+    if (st == GDA_OK && lambda0) st = dmalloc(&d_l0, elems);
+    if (st == GDA_OK) st = dmalloc(&d_xb, elems);
+    if (st == GDA_OK) st = dmalloc(&d_obj, (size_t)B);
+    if (st == GDA_OK) st = dmalloc(&d_best, 1);
+    cudaError_t e = cudaSuccess;
+    if (st == GDA_OK) {
+        e = cudaMemcpyAsync(d_x0, x0, elems * sizeof(float), cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess && lambda0) e = cudaMemcpyAsync(d_l0, lambda0, elems * sizeof(float), cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) st = gda_run(p, B, d_x0, d_l0, lambda0_scalar, prm, d_xb, d_obj, d_best, nullptr, s);
+        if (st == GDA_OK && e == cudaSuccess) e = cudaMemcpyAsync(x_bin, d_xb, elems, cudaMemcpyDeviceToHost, s);
+        if (st == GDA_OK && e == cudaSuccess) e = cudaMemcpyAsync(obj, d_obj, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, s);
+        if (st == GDA_OK && e == cudaSuccess) e = cudaMemcpyAsync(best_restart, d_best, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    }
+    cudaFree(d_x0); cudaFree(d_l0); cudaFree(d_xb); cudaFree(d_obj); cudaFree(d_best);
+    (void)ws;
+    if (st != GDA_OK) return st;
+    if (e != cudaSuccess) { gda_set_error("gda_run_host: %s", cudaGetErrorString(e)); return GDA_ERR_CUDA; }
+    return join_stream(p, user, s);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// single steps of the path: gradient (S1/S2/S3) and score (S5)
+// ---------------------------------------------------------------------------------------------------
+extern "C" gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float* G, void* stream) {
+    GDA_REQUIRE(p != nullptr && x != nullptr && G != nullptr, "gda_grad: null argument");
+    GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_grad: B must be a positive multiple of 4 (got %d)", B);
+    if (p->kind == GDA_KIND_DENSE && B % 128 != 0) { gda_set_error("gda_grad: the dense path needs B %% 128 == 0"); return GDA_ERR_UNSUPPORTED; }
+    GDA_CUDA_TRY(cudaSetDevice(p->device));
+    cudaStream_t user, s;
+    if (p->kind == GDA_KIND_DENSE) GDA_TRY(ensure_workspace(p, B));
+    GDA_TRY(pick_stream(p, stream, &user, &s));
+    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_grad(p, B, x, G, s));
+    else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_grad(p, B, x, G, s));
+    else GDA_TRY(dense_grad(p, B, x, G, s));
+    return join_stream(p, user, s);
+}
+
+extern "C" gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, void* stream) {
+    GDA_REQUIRE(p != nullptr && x != nullptr && obj != nullptr, "gda_score: null argument");
+    GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_score: B must be a positive multiple of 4 (got %d)", B);
+    if (p->kind == GDA_KIND_DENSE && B % 128 != 0) { gda_set_error("gda_score: the dense path needs B %% 128 == 0"); return GDA_ERR_UNSUPPORTED; }
+    GDA_CUDA_TRY(cudaSetDevice(p->device));
+    GDA_TRY(ensure_workspace(p, B));
+    cudaStream_t user, s;
+    GDA_TRY(pick_stream(p, stream, &user, &s));
+    int32_t n_part = 0;
+    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr));
+    else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr));
+    else GDA_TRY(dense_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr));
+    GDA_TRY(score_reduce(p, B, p->ws.partial, n_part, obj, s));
+    return join_stream(p, user, s);
+}
+
+extern "C" gda_status gda_get_info(const gda_problem* p, gda_info* info) {
+    GDA_REQUIRE(p != nullptr && info != nullptr, "gda_get_info: null argument");
+    info->kind = p->kind; info->n = p->n; info->nnz = p->nnz; info->m = p->m; info->integral = p->integral;
+    info->last_run_kernel_launches = p->last_launches;
+    info->last_run_step_launches = p->last_step_launches;
+    return GDA_OK;
+}

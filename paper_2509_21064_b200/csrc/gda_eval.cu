@@ -1,0 +1,179 @@
+// gda_eval.cu -- the evaluation tail shared by all three problem kinds (S5 bookkeeping, S6 arg-best):
+//   fixed-order reduction of the per-block partial objective sums, best-so-far per restart
+//   ("retaining the best solution"; reading R5), committing x_hat of improved restarts,
+//   the best-vs-time trace and the final argmin over restarts (reading R6).
+#include "gda_internal.cuh"
+
+#include <math_constants.h>
+
+namespace {
+
+constexpr int FIN_THREADS = 256;
+
+__device__ __forceinline__ uint64_t globaltimer_ns() {
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+// obj_now[b] = sum_p partial[p][b] in the fixed order p = 0..n_part-1 (deterministic); best-so-far update.
+// One block; thread 0 afterwards records the trace entry and advances the run state.
+template <bool INTEGRAL>
+__global__ void __launch_bounds__(FIN_THREADS)
+finalize_kernel(int B, const void* __restrict__ partial, int n_part, double* __restrict__ obj_now,
+                double* __restrict__ best_obj, int32_t* __restrict__ improved, RunState* st,
+                double* __restrict__ trace_best, uint64_t* __restrict__ trace_ns, int trace_cap,
+                uint32_t advance_t) {
+    using acc_t = typename std::conditional<INTEGRAL, long long, double>::type;
+    __shared__ double smin[FIN_THREADS / 32];
+    const acc_t* part = reinterpret_cast<const acc_t*>(partial);
+    double local_min = CUDART_INF;
+    for (int b = threadIdx.x; b < B; b += FIN_THREADS) {
+        acc_t s = 0;
+        for (int q = 0; q < n_part; ++q) s += part[(size_t)q * B + b];
+        const double v = (double)s;
+        if (obj_now) obj_now[b] = v;
+        if (best_obj) {
+            double best = best_obj[b];
+            const int imp = v < best;
+            if (imp) { best = v; best_obj[b] = v; }
+            improved[b] = imp;
+            local_min = fmin(local_min, best);
+        }
+    }
+    if (!st) return;
+    for (int o = 16; o > 0; o >>= 1) local_min = fmin(local_min, __shfl_xor_sync(0xffffffffu, local_min, o));
+    if ((threadIdx.x & 31) == 0) smin[threadIdx.x >> 5] = local_min;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double m = smin[0];
+        for (int w = 1; w < FIN_THREADS / 32; ++w) m = fmin(m, smin[w]);
+        const uint32_t k = st->n_eval;
+        if (trace_best && (int)k < trace_cap) { trace_best[k] = m; trace_ns[k] = globaltimer_ns(); }
+        st->n_eval = k + 1;
+        st->t += advance_t;
+    }
+}
+
+// x_bin[:, b] = [x[:, b] > 1/2] for every restart b whose objective improved at this evaluation
+__global__ void __launch_bounds__(256)
+commit_kernel(size_t n_vec, int B4, const float* __restrict__ x, const int32_t* __restrict__ improved,
+              uint8_t* __restrict__ x_bin) {
+    const size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= n_vec) return;
+    const int c4 = (int)(v % (size_t)B4);
+    const int4 imp = __ldg(reinterpret_cast<const int4*>(improved) + c4);
+    if (!(imp.x | imp.y | imp.z | imp.w)) return;
+    const float4 xv = ldg4(x + 4 * v);
+    uchar4 o = reinterpret_cast<uchar4*>(x_bin)[v];
+    if (imp.x) o.x = xv.x > 0.5f;
+    if (imp.y) o.y = xv.y > 0.5f;
+    if (imp.z) o.z = xv.z > 0.5f;
+    if (imp.w) o.w = xv.w > 0.5f;
+    reinterpret_cast<uchar4*>(x_bin)[v] = o;
+}
+
+// S6: argmin over restarts, ties -> lowest index; warp shuffles, then one warp over the per-warp winners
+__global__ void __launch_bounds__(256)
+argbest_kernel(int B, const double* __restrict__ obj, int32_t* __restrict__ best_restart,
+               double* __restrict__ best_val) {
+    __shared__ double sv[8];
+    __shared__ int si[8];
+    double v = CUDART_INF;
+    int idx = 0x7fffffff;
+    for (int b = threadIdx.x; b < B; b += blockDim.x) {
+        const double o = obj[b];
+        if (o < v || (o == v && b < idx)) { v = o; idx = b; }
+    }
+    for (int off = 16; off > 0; off >>= 1) {
+        const double ov = __shfl_xor_sync(0xffffffffu, v, off);
+        const int oi = __shfl_xor_sync(0xffffffffu, idx, off);
+        if (ov < v || (ov == v && oi < idx)) { v = ov; idx = oi; }
+    }
+    if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = v; si[threadIdx.x >> 5] = idx; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        v = threadIdx.x < 8 ? sv[threadIdx.x] : CUDART_INF;
+        idx = threadIdx.x < 8 ? si[threadIdx.x] : 0x7fffffff;
+        for (int off = 4; off > 0; off >>= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, v, off);
+            const int oi = __shfl_xor_sync(0xffffffffu, idx, off);
+            if (ov < v || (ov == v && oi < idx)) { v = ov; idx = oi; }
+        }
+        if (threadIdx.x == 0) {
+            *best_restart = (idx == 0x7fffffff) ? 0 : idx;      // all +inf / NaN: restart 0
+            if (best_val) *best_val = (idx == 0x7fffffff) ? obj[0] : v;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+fill_kernel(size_t n_vec, float4* __restrict__ dst, float v) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_vec) dst[i] = make_float4(v, v, v, v);
+}
+
+__global__ void __launch_bounds__(256)
+init_state_kernel(int B, double* __restrict__ best_obj, int32_t* __restrict__ improved, RunState* st, uint32_t t0) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < B) { best_obj[b] = CUDART_INF; improved[b] = 0; }
+    if (b == 0) { st->t = t0; st->n_eval = 0; }
+}
+
+}  // namespace
+
+gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0, float l0_scalar,
+                    uint32_t t0, cudaStream_t s, int64_t* launches) {
+    Workspace& ws = p->ws;
+    const size_t elems = (size_t)p->n * B;
+    GDA_CUDA_TRY(cudaMemcpyAsync(ws.x[0], x0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+    if (l0) {
+        GDA_CUDA_TRY(cudaMemcpyAsync(ws.y, l0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+    } else {
+        const size_t n_vec = elems / 4;
+        fill_kernel<<<(unsigned)((n_vec + 255) / 256), 256, 0, s>>>(n_vec, reinterpret_cast<float4*>(ws.y), l0_scalar);
+        if (launches) ++*launches;
+    }
+    GDA_CUDA_TRY(cudaMemsetAsync(ws.x_bin, 0, elems, s));
+    init_state_kernel<<<(B + 255) / 256, 256, 0, s>>>(B, ws.best_obj, ws.improved, ws.state, t0);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status eval_finalize(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj_now,
+                         double* best_obj, int32_t* improved, RunState* st, double* trace_best,
+                         uint64_t* trace_ns, int32_t trace_cap, uint32_t advance_t, cudaStream_t s,
+                         int64_t* launches) {
+    if (p->integral)
+        finalize_kernel<true><<<1, FIN_THREADS, 0, s>>>(B, partial, n_part, obj_now, best_obj, improved, st,
+                                                        trace_best, trace_ns, trace_cap, advance_t);
+    else
+        finalize_kernel<false><<<1, FIN_THREADS, 0, s>>>(B, partial, n_part, obj_now, best_obj, improved, st,
+                                                         trace_best, trace_ns, trace_cap, advance_t);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status score_reduce(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj,
+                        cudaStream_t s) {
+    return eval_finalize(p, B, partial, n_part, obj, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, s, nullptr);
+}
+
+gda_status eval_commit(gda_problem* p, int32_t B, const float* x, const int32_t* improved, uint8_t* x_bin,
+                       cudaStream_t s, int64_t* launches) {
+    const size_t n_vec = (size_t)p->n * B / 4;
+    commit_kernel<<<(unsigned)((n_vec + 255) / 256), 256, 0, s>>>(n_vec, B / 4, x, improved, x_bin);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status eval_argbest(int32_t B, const double* obj, int32_t* best_restart, double* best_val,
+                        cudaStream_t s, int64_t* launches) {
+    argbest_kernel<<<1, 256, 0, s>>>(B, obj, best_restart, best_val);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}

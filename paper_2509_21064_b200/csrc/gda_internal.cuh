@@ -1,0 +1,209 @@
+// gda_internal.cuh -- shared by the translation units of libgda_b200.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/gda.h"
+
+// ---------------------------------------------------------------------------------------------------
+// error plumbing
+// ---------------------------------------------------------------------------------------------------
+void gda_set_error(const char* fmt, ...);
+
+#define GDA_CUDA_TRY(expr)                                                                        \
+    do {                                                                                          \
+        cudaError_t e__ = (expr);                                                                 \
+        if (e__ != cudaSuccess) {                                                                 \
+            gda_set_error("%s:%d: %s failed: %s", __FILE__, __LINE__, #expr, cudaGetErrorString(e__)); \
+            return GDA_ERR_CUDA;                                                                  \
+        }                                                                                         \
+    } while (0)
+
+#define GDA_TRY(expr)                        \
+    do {                                     \
+        gda_status s__ = (expr);             \
+        if (s__ != GDA_OK) return s__;       \
+    } while (0)
+
+enum { GDA_KIND_SPARSE = 0, GDA_KIND_DENSE = 1, GDA_KIND_MAXSAT = 2 };
+
+// ---------------------------------------------------------------------------------------------------
+// update parameters handed to the kernels by value
+// ---------------------------------------------------------------------------------------------------
+struct UpdParams {
+    float alpha, beta, delta, log_eps;
+    uint32_t seed_mix;   // mix32(seed_lo ^ seed_hi * 0x9E3779B9)
+    int32_t gfun;
+};
+
+// device-side run state (lives in the workspace)
+struct RunState {
+    uint32_t t;          // iteration index of the iterate currently in x[cur]
+    uint32_t n_eval;     // evaluations done so far in this run
+};
+
+// ---------------------------------------------------------------------------------------------------
+// the opaque handle
+// ---------------------------------------------------------------------------------------------------
+struct Workspace {
+    int32_t B = 0;
+    float* x[2] = {nullptr, nullptr};   // [n][B] double buffer (Jacobi: every row reads all of x^t)
+    float* y = nullptr;                 // [n][B], updated in place
+    uint8_t* x_bin = nullptr;           // [n][B] best-so-far rounded point
+    double* best_obj = nullptr;         // [B]
+    double* obj_now = nullptr;          // [B]
+    int32_t* improved = nullptr;        // [B]
+    void* partial = nullptr;            // [n_part][B] int64 or double partial objective sums
+    int32_t n_part = 0;
+    RunState* state = nullptr;
+    int32_t* best_restart = nullptr;    // [1]
+    double* best_val = nullptr;         // [1]
+    double* trace_best = nullptr;       // internal trace buffers (copied out on request)
+    uint64_t* trace_ns = nullptr;
+    int32_t trace_cap = 0;
+    // dense path
+    __nv_bfloat16* zt[2] = {nullptr, nullptr};  // [B][n] bf16 GEMM operand (centred x - 1/2, or x_hat)
+    float* gtmp = nullptr;                      // [n][B] gradient scratch for gda_grad on the dense path
+    // host staging for gda_run_host
+    float* h_x0 = nullptr; float* h_l0 = nullptr;
+};
+
+struct GraphKey {
+    int32_t B = -1, len = 0, parity = 0, with_eval = 0;
+    gda_params prm{};
+    bool operator==(const GraphKey& o) const;
+};
+struct CachedGraph {
+    GraphKey key;
+    cudaGraphExec_t exec = nullptr;
+    cudaGraph_t graph = nullptr;
+    int64_t launches = 0, step_launches = 0;
+};
+
+struct gda_problem {
+    int32_t kind = 0;
+    int32_t n = 0;
+    int64_t nnz = 0;
+    int32_t m = 0;
+    int32_t integral = 0;
+    int device = 0;
+    int num_sms = 148;
+    // sparse QUBO: off-diagonal CSR with val2 = Q_ij + Q_ji (= 2 Q_ij), cprime = c + diag(Q)
+    int32_t* d_rowptr = nullptr; int32_t* d_col = nullptr; float* d_val2 = nullptr;
+    float* d_cprime = nullptr;           // also used by the dense path
+    int32_t* d_heavy_rows = nullptr; int32_t n_heavy = 0;   // rows handled by the row-split kernel
+    int32_t* d_light_rows = nullptr; int32_t n_light = 0;   // nullptr = all rows, in order
+    int32_t max_deg = 0;
+    // dense QUBO: Q_off in bf16 [n][n] (zero diagonal), r0 = Q_off 1 (row sums) for the centred operand
+    __nv_bfloat16* d_Qbf = nullptr; float* d_rowsum = nullptr;
+    void* tmap_Q = nullptr;              // CUtensorMap (128 B), host copy
+    // MaxSAT: per occurrence slot (variable-major): coef = w_j * s_ji, others[kw] signed literals (0 = pad)
+    int32_t* d_vptr = nullptr; float* d_coef = nullptr; int32_t* d_others = nullptr; int32_t kw = 0;
+    int32_t* d_cptr = nullptr; int32_t* d_lit = nullptr; float* d_w = nullptr; int32_t kmax = 0;
+    Workspace ws;
+    cudaStream_t own_stream = nullptr;   // used when the caller passes the legacy default stream (not capturable)
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    std::vector<CachedGraph> graphs;
+    int64_t last_launches = 0, last_step_launches = 0;
+};
+
+// ---------------------------------------------------------------------------------------------------
+// kernels' launchers, one translation unit per path.  Every launcher enqueues on `s` and returns the
+// number of kernels it launched through *launches (may be nullptr).
+// ---------------------------------------------------------------------------------------------------
+// sparse QUBO (gda_sparse.cu)
+gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
+                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
+gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);
+gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
+                                 cudaStream_t s, int64_t* launches);
+int32_t sparse_num_partials(const gda_problem* p, int32_t B);
+
+// MaxSAT (gda_maxsat.cu)
+gda_status maxsat_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
+                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
+gda_status maxsat_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);
+gda_status maxsat_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
+                                 cudaStream_t s, int64_t* launches);
+int32_t maxsat_num_partials(const gda_problem* p, int32_t B);
+
+// dense QUBO (gda_dense.cu)
+gda_status dense_prepare(gda_problem* p, const float* Q_host, const float* c_host);   // at create
+gda_status dense_make_operand(gda_problem* p, int32_t B, const float* x, __nv_bfloat16* zt, int hat,
+                              cudaStream_t s, int64_t* launches);
+gda_status dense_step(gda_problem* p, int32_t B, float* x, float* y, const __nv_bfloat16* zt_in,
+                      __nv_bfloat16* zt_out, const UpdParams& up, const RunState* st, uint32_t t_off,
+                      cudaStream_t s, int64_t* launches);
+gda_status dense_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);
+gda_status dense_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
+                                cudaStream_t s, int64_t* launches);
+int32_t dense_num_partials(const gda_problem* p, int32_t B);
+void dense_release(gda_problem* p);
+
+// shared evaluation tail (gda_eval.cu)
+gda_status eval_finalize(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj_now,
+                         double* best_obj, int32_t* improved, RunState* st, double* trace_best,
+                         uint64_t* trace_ns, int32_t trace_cap, uint32_t advance_t, cudaStream_t s,
+                         int64_t* launches);
+gda_status eval_commit(gda_problem* p, int32_t B, const float* x, const int32_t* improved, uint8_t* x_bin,
+                       cudaStream_t s, int64_t* launches);
+gda_status eval_argbest(int32_t B, const double* obj, int32_t* best_restart, double* best_val,
+                        cudaStream_t s, int64_t* launches);
+gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0, float l0_scalar,
+                    uint32_t t0, cudaStream_t s, int64_t* launches);
+gda_status score_reduce(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj,
+                        cudaStream_t s);
+
+// ---------------------------------------------------------------------------------------------------
+// device helpers: g, g', the fused update S4 (Eq. 6 + perturbation), the tie-break hash
+// ---------------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__host__ __device__ __forceinline__ uint32_t mix32(uint32_t h) {
+    h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
+    return h;
+}
+
+// s = +1 / -1 from (seed, t, i, b): DESIGN.md reading R3 (the oracle writes the same integer function out itself)
+__device__ __forceinline__ float side_from_hash(uint32_t seed_mix, uint32_t t, uint32_t i, uint32_t b) {
+    uint32_t h = mix32(seed_mix + t);
+    h = mix32(h + i);
+    h = mix32(h + b);
+    return (h & 1u) ? 1.0f : -1.0f;
+}
+
+__device__ __forceinline__ float xlogx_f(float u) { return u > 0.0f ? u * logf(u) : 0.0f; }
+
+// One element of S4: (x, y, G) at time t -> (x, y) at time t+1.   PAPER.md:136-142 (Eq. 6), 148, 732.
+template <int GFUN>
+__device__ __forceinline__ void gda_update(float x, float y, float G, const UpdParams& up, uint32_t t,
+                                           uint32_t i, uint32_t b, float& xn, float& yn) {
+    float gp, gv;
+    if (GFUN == GDA_G_QUADRATIC) {
+        gp = 2.0f * x - 1.0f;
+        gv = x * x - x;
+    } else {
+        const float xc = fminf(fmaxf(x, up.log_eps), 1.0f - up.log_eps);
+        const float l0 = logf(xc), l1 = logf(1.0f - xc);
+        gp = l0 - l1;
+        gv = (xc == x) ? (x * l0 + (1.0f - x) * l1) : (xlogx_f(x) + xlogx_f(1.0f - x));
+    }
+    float xt = x - up.alpha * (G + y * gp);
+    xt = fminf(fmaxf(xt, 0.0f), 1.0f);
+    yn = y + up.beta * gv;
+    if (up.delta > 0.0f && fabsf(x - 0.5f) < up.delta && fabsf(xt - 0.5f) < up.delta) {
+        float s;
+        if (xt > 0.5f) s = 1.0f; else if (xt < 0.5f) s = -1.0f;
+        else if (x > 0.5f) s = 1.0f; else if (x < 0.5f) s = -1.0f;
+        else s = side_from_hash(up.seed_mix, t, i, b);
+        xt = 0.5f + up.delta * s;
+        if (fabsf(xt - 0.5f) < up.delta)                       // rounding fell inside: one ulp away from 1/2
+            xt = __int_as_float(__float_as_int(xt) + (s > 0.0f ? 1 : -1));
+        }
+    xn = xt;
+}
+
+__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+#endif

@@ -1,0 +1,204 @@
+// gda_maxsat.cu -- S3 + S4 for weighted MaxSAT: per-clause literal products gathered back to variables
+// through a precomputed variable-to-clause CSC, fused with the GDA update; S5 scoring by clause.
+//
+//   f(x) = sum_j w_j prod_{l in C_j} p_l(x),  p = 1 - x (positive literal) or x (negated)
+//   G_i  = sum_{j : i in C_j} w_j s_ji prod_{l in C_j, l != i} p_l(x),  s = -1 / +1          (leave-one-out)
+//
+// Variable-major gather, no atomics: occurrence slot s of variable i holds coef = w_j s_ji and the kw =
+// kmax-1 OTHER literals of its clause (0-padded), so the leave-one-out product is recomputed from X
+// (L2-resident) instead of being stored per literal (that would add 2 x 4 x L x B bytes of HBM traffic).
+// With restarts across lanes ([n][B] layout) every product is lane-local; warp shuffles only broadcast
+// the slot records, which are fetched with one coalesced load per 32 slots.
+#include "gda_internal.cuh"
+
+namespace {
+
+constexpr int WARPS = 8;
+constexpr int THREADS = WARPS * 32;
+constexpr int SCORE_CLAUSES = 128;
+
+__device__ __forceinline__ float4 lit_term(int l, const float* __restrict__ x, int B, int c4) {
+    const int v = (l > 0 ? l : -l) - 1;
+    const float4 g = ldg4(x + (size_t)v * B + 4 * c4);
+    return l > 0 ? make_float4(1.0f - g.x, 1.0f - g.y, 1.0f - g.z, 1.0f - g.w) : g;
+}
+
+// KW > 0: compile-time number of "other" literals (3-SAT: 2), slot records broadcast by shuffle.
+// KW == 0: run-time kw, records read with broadcast loads.
+template <int KW>
+__device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, const int32_t* __restrict__ others,
+                                             int kw, int start, int end, const float* __restrict__ x, int B,
+                                             int c4, bool active, int lane) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (KW > 0) {
+        for (int base = start; base < end; base += 32) {
+            const int s = base + lane;
+            const float my_coef = (s < end) ? __ldg(coef + s) : 0.0f;
+            int my_o[KW > 0 ? KW : 1];
+#pragma unroll
+            for (int q = 0; q < KW; ++q) my_o[q] = (s < end) ? __ldg(others + (size_t)s * KW + q) : 0;
+            const int cnt = min(32, end - base);
+            for (int u = 0; u < cnt; ++u) {
+                const float cf = __shfl_sync(0xffffffffu, my_coef, u);
+                int l[KW > 0 ? KW : 1];
+#pragma unroll
+                for (int q = 0; q < KW; ++q) l[q] = __shfl_sync(0xffffffffu, my_o[q], u);
+                if (!active) continue;
+                float4 prod = make_float4(cf, cf, cf, cf);
+#pragma unroll
+                for (int q = 0; q < KW; ++q) {
+                    if (l[q] == 0) continue;
+                    const float4 t = lit_term(l[q], x, B, c4);
+                    prod.x *= t.x; prod.y *= t.y; prod.z *= t.z; prod.w *= t.w;
+                }
+                acc.x += prod.x; acc.y += prod.y; acc.z += prod.z; acc.w += prod.w;
+            }
+        }
+    } else {
+        if (!active) return acc;
+        for (int s = start; s < end; ++s) {
+            const float cf = __ldg(coef + s);
+            float4 prod = make_float4(cf, cf, cf, cf);
+            for (int q = 0; q < kw; ++q) {
+                const int l = __ldg(others + (size_t)s * kw + q);
+                if (l == 0) break;
+                const float4 t = lit_term(l, x, B, c4);
+                prod.x *= t.x; prod.y *= t.y; prod.z *= t.z; prod.w *= t.w;
+            }
+            acc.x += prod.x; acc.y += prod.y; acc.z += prod.z; acc.w += prod.w;
+        }
+    }
+    return acc;
+}
+
+// warp-per-(variable, 128-restart chunk).  MODE 0: fused step; MODE 1: write G only.
+template <int GFUN, int MODE, int KW>
+__global__ void __launch_bounds__(THREADS)
+maxsat_step_kernel(int n, int B, int chunks, const int32_t* __restrict__ vptr, const float* __restrict__ coef,
+                   const int32_t* __restrict__ others, int kw, const float* __restrict__ x,
+                   float* __restrict__ y, float* __restrict__ xn, UpdParams up,
+                   const RunState* __restrict__ st, uint32_t t_off) {
+    const int lane = threadIdx.x & 31;
+    const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
+    if (item >= (long long)n * chunks) return;
+    const int var = (int)(item / chunks);
+    const int chunk = (int)(item - (long long)var * chunks);
+    const int c4 = chunk * 32 + lane;
+    const bool active = 4 * c4 < B;
+    const int start = __ldg(vptr + var), end = __ldg(vptr + var + 1);
+    const float4 G = gather_var<KW>(coef, others, kw, start, end, x, B, c4, active, lane);
+    if (!active) return;
+    const size_t off = (size_t)var * B + 4 * c4;
+    if (MODE == 1) { *reinterpret_cast<float4*>(xn + off) = G; return; }
+    const uint32_t t = (st ? st->t : 0u) + t_off;
+    const float4 xv = ldg4(x + off);
+    const float4 yv = *reinterpret_cast<const float4*>(y + off);
+    float4 xo, yo;
+    const uint32_t b0 = 4u * (uint32_t)c4;
+    gda_update<GFUN>(xv.x, yv.x, G.x, up, t, (uint32_t)var, b0 + 0, xo.x, yo.x);
+    gda_update<GFUN>(xv.y, yv.y, G.y, up, t, (uint32_t)var, b0 + 1, xo.y, yo.y);
+    gda_update<GFUN>(xv.z, yv.z, G.z, up, t, (uint32_t)var, b0 + 2, xo.z, yo.z);
+    gda_update<GFUN>(xv.w, yv.w, G.w, up, t, (uint32_t)var, b0 + 3, xo.w, yo.w);
+    *reinterpret_cast<float4*>(xn + off) = xo;
+    *reinterpret_cast<float4*>(y + off) = yo;
+}
+
+// S5: partial[cb][b] = sum over the clauses of block cb of w_j [every literal of C_j false under x_hat]
+template <bool INTEGRAL>
+__global__ void __launch_bounds__(THREADS)
+maxsat_score(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __restrict__ lit,
+             const float* __restrict__ w, const float* __restrict__ x, void* __restrict__ partial) {
+    using acc_t = typename std::conditional<INTEGRAL, long long, double>::type;
+    __shared__ acc_t red[WARPS][32][4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c4 = blockIdx.y * 32 + lane;
+    const bool active = 4 * c4 < B;
+    acc_t acc[4] = {0, 0, 0, 0};
+    if (active) {
+        for (int r = warp; r < SCORE_CLAUSES; r += WARPS) {
+            const int j = blockIdx.x * SCORE_CLAUSES + r;
+            if (j >= m) break;
+            bool unsat[4] = {true, true, true, true};
+            for (int a = __ldg(cptr + j); a < __ldg(cptr + j + 1); ++a) {
+                const int l = __ldg(lit + a);
+                const int v = (l > 0 ? l : -l) - 1;
+                const float4 g = ldg4(x + (size_t)v * B + 4 * c4);
+                const bool h[4] = {g.x > 0.5f, g.y > 0.5f, g.z > 0.5f, g.w > 0.5f};
+#pragma unroll
+                for (int q = 0; q < 4; ++q) unsat[q] = unsat[q] && (l > 0 ? !h[q] : h[q]);   // literal false
+            }
+            const float wj = __ldg(w + j);
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (unsat[q]) acc[q] += INTEGRAL ? (acc_t)__float2int_rn(wj) : (acc_t)wj;
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) red[warp][lane][q] = acc[q];
+    __syncthreads();
+    if (warp == 0 && active) {
+        acc_t* out = reinterpret_cast<acc_t*>(partial) + (size_t)blockIdx.x * B + 4 * c4;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            acc_t t = red[0][lane][q];
+            for (int k = 1; k < WARPS; ++k) t += red[k][lane][q];
+            out[q] = t;
+        }
+    }
+}
+
+template <int GFUN, int MODE>
+void launch_kw(gda_problem* p, int32_t B, int chunks, unsigned grid, const float* x, float* y, float* xn,
+               const UpdParams& up, const RunState* st, uint32_t t_off, cudaStream_t s) {
+#define GDA_MS_ARGS p->n, B, chunks, p->d_vptr, p->d_coef, p->d_others, p->kw, x, y, xn, up, st, t_off
+    switch (p->kw) {
+        case 1: maxsat_step_kernel<GFUN, MODE, 1><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        case 2: maxsat_step_kernel<GFUN, MODE, 2><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        case 3: maxsat_step_kernel<GFUN, MODE, 3><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        case 4: maxsat_step_kernel<GFUN, MODE, 4><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        default: maxsat_step_kernel<GFUN, MODE, 0><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+    }
+#undef GDA_MS_ARGS
+}
+
+template <int MODE>
+gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
+                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+    const int chunks = (B / 4 + 31) / 32;
+    const long long items = (long long)p->n * chunks;
+    const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
+    if (up.gfun == GDA_G_QUADRATIC) launch_kw<GDA_G_QUADRATIC, MODE>(p, B, chunks, grid, x, y, xn, up, st, t_off, s);
+    else launch_kw<GDA_G_ENTROPY, MODE>(p, B, chunks, grid, x, y, xn, up, st, t_off, s);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+}  // namespace
+
+gda_status maxsat_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
+                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+    return launch_step<0>(p, B, x, y, xn, up, st, t_off, s, launches);
+}
+
+gda_status maxsat_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s) {
+    UpdParams up{};
+    up.gfun = GDA_G_QUADRATIC;
+    return launch_step<1>(p, B, x, nullptr, G, up, nullptr, 0, s, nullptr);
+}
+
+int32_t maxsat_num_partials(const gda_problem* p, int32_t) { return (p->m + SCORE_CLAUSES - 1) / SCORE_CLAUSES; }
+
+gda_status maxsat_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
+                                 cudaStream_t s, int64_t* launches) {
+    const int chunks = (B / 4 + 31) / 32;
+    dim3 grid((unsigned)maxsat_num_partials(p, B), (unsigned)chunks);
+    if (p->integral)
+        maxsat_score<true><<<grid, THREADS, 0, s>>>(p->m, B, p->d_cptr, p->d_lit, p->d_w, x, partial);
+    else
+        maxsat_score<false><<<grid, THREADS, 0, s>>>(p->m, B, p->d_cptr, p->d_lit, p->d_w, x, partial);
+    if (launches) ++*launches;
+    *n_part = (int32_t)grid.x;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}

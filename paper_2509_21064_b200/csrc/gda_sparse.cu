@@ -1,0 +1,252 @@
+// gda_sparse.cu -- S1 + S4 for sparse QUBO / Max-Cut: batched CSR SpMM gradient fused with the GDA update.
+//
+//   G = 2 Q_off X + c' 1^T            (multilinear extension of x^T Q x + c^T x)
+//   x+ = clip(x - alpha (G + y g'(x))),  y+ = y + beta g(x),  perturbation near 1/2
+//
+// Layout: X, Y are [n][B] fp32 with the restart index contiguous, so the gather of row j for 128
+// consecutive restarts is one coalesced 512-byte request (a float4 per lane).  One warp owns one
+// (row, 128-restart chunk) item: it loads the row's (col, val) pairs with one coalesced load and
+// broadcasts them by shuffle, gathers, and applies the fused update in registers -- G never goes to memory.
+// Rows with more than HEAVY_DEG non-zeros are split across the 8 warps of a block (row-split variant).
+#include "gda_internal.cuh"
+
+namespace {
+
+constexpr int WARPS = 8;
+constexpr int THREADS = WARPS * 32;
+constexpr int HEAVY_DEG = 256;     // rows above this use the row-split kernel
+constexpr int SCORE_ROWS = 64;     // rows per block in the scoring kernel
+
+__device__ __forceinline__ void fma4(float4& a, float v, const float4& g) {
+    a.x = fmaf(v, g.x, a.x); a.y = fmaf(v, g.y, a.y); a.z = fmaf(v, g.z, a.z); a.w = fmaf(v, g.w, a.w);
+}
+
+// sum_k val2[k] * X[col[k]][c4]  for k in [start, end): (col,val) fetched 32 at a time, one per lane
+__device__ __forceinline__ float4 gather_row(const int32_t* __restrict__ col, const float* __restrict__ val2,
+                                             int start, int end, const float* __restrict__ x, int B,
+                                             int c4, bool active, int lane) {
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int base = start; base < end; base += 32) {
+        const int k = base + lane;
+        const int my_c = (k < end) ? __ldg(col + k) : 0;
+        const float my_v = (k < end) ? __ldg(val2 + k) : 0.0f;
+        const int cnt = min(32, end - base);
+        int u = 0;
+        for (; u + 4 <= cnt; u += 4) {                       // 4 independent 512 B gathers in flight
+            int c[4]; float v[4]; float4 g[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { c[q] = __shfl_sync(0xffffffffu, my_c, u + q); v[q] = __shfl_sync(0xffffffffu, my_v, u + q); }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) g[q] = active ? ldg4(x + (size_t)c[q] * B + 4 * c4) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) fma4(acc, v[q], g[q]);
+        }
+        for (; u < cnt; ++u) {
+            const int c = __shfl_sync(0xffffffffu, my_c, u);
+            const float v = __shfl_sync(0xffffffffu, my_v, u);
+            if (active) fma4(acc, v, ldg4(x + (size_t)c * B + 4 * c4));
+        }
+    }
+    return acc;
+}
+
+template <int GFUN>
+__device__ __forceinline__ void update_store(int row, int c4, int B, float4 G, const float* __restrict__ x,
+                                             float* __restrict__ y, float* __restrict__ xn,
+                                             const UpdParams& up, uint32_t t) {
+    const size_t off = (size_t)row * B + 4 * c4;
+    const float4 xv = ldg4(x + off);
+    const float4 yv = *reinterpret_cast<const float4*>(y + off);
+    float4 xo, yo;
+    const uint32_t b0 = 4u * (uint32_t)c4;
+    gda_update<GFUN>(xv.x, yv.x, G.x, up, t, (uint32_t)row, b0 + 0, xo.x, yo.x);
+    gda_update<GFUN>(xv.y, yv.y, G.y, up, t, (uint32_t)row, b0 + 1, xo.y, yo.y);
+    gda_update<GFUN>(xv.z, yv.z, G.z, up, t, (uint32_t)row, b0 + 2, xo.z, yo.z);
+    gda_update<GFUN>(xv.w, yv.w, G.w, up, t, (uint32_t)row, b0 + 3, xo.w, yo.w);
+    *reinterpret_cast<float4*>(xn + off) = xo;
+    *reinterpret_cast<float4*>(y + off) = yo;
+}
+
+// warp-per-(row, chunk).  MODE 0: fused step, MODE 1: write G only (gda_grad).
+template <int GFUN, int MODE>
+__global__ void __launch_bounds__(THREADS)
+spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B, int chunks,
+               const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+               const float* __restrict__ val2, const float* __restrict__ cprime,
+               const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
+               UpdParams up, const RunState* __restrict__ st, uint32_t t_off) {
+    const int lane = threadIdx.x & 31;
+    const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
+    if (item >= (long long)n_rows * chunks) return;
+    const int ridx = (int)(item / chunks);
+    const int chunk = (int)(item - (long long)ridx * chunks);
+    const int row = row_list ? __ldg(row_list + ridx) : ridx;
+    const int c4 = chunk * 32 + lane;
+    const bool active = 4 * c4 < B;
+    const int start = __ldg(rowptr + row), end = __ldg(rowptr + row + 1);
+    float4 G = gather_row(col, val2, start, end, x, B, c4, active, lane);
+    const float cp = __ldg(cprime + row);
+    G.x += cp; G.y += cp; G.z += cp; G.w += cp;
+    if (!active) return;
+    if (MODE == 1) { *reinterpret_cast<float4*>(xn + (size_t)row * B + 4 * c4) = G; return; }
+    const uint32_t t = (st ? st->t : 0u) + t_off;
+    update_store<GFUN>(row, c4, B, G, x, y, xn, up, t);
+}
+
+// row-split: one block per (heavy row, chunk); the 8 warps take interleaved 32-entry slices of the row
+template <int GFUN, int MODE>
+__global__ void __launch_bounds__(THREADS)
+spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chunks,
+                const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                const float* __restrict__ val2, const float* __restrict__ cprime,
+                const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
+                UpdParams up, const RunState* __restrict__ st, uint32_t t_off) {
+    __shared__ float4 red[WARPS][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int ridx = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
+    const int row = __ldg(row_list + ridx);
+    const int c4 = chunk * 32 + lane;
+    const bool active = 4 * c4 < B;
+    const int start = __ldg(rowptr + row), end = __ldg(rowptr + row + 1);
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int base = start + 32 * warp; base < end; base += 32 * WARPS) {
+        const float4 part = gather_row(col, val2, base, min(base + 32, end), x, B, c4, active, lane);
+        acc.x += part.x; acc.y += part.y; acc.z += part.z; acc.w += part.w;
+    }
+    red[warp][lane] = acc;
+    __syncthreads();
+    if (warp != 0 || !active) return;
+    float4 G = red[0][lane];
+#pragma unroll
+    for (int w = 1; w < WARPS; ++w) { const float4 r = red[w][lane]; G.x += r.x; G.y += r.y; G.z += r.z; G.w += r.w; }
+    const float cp = __ldg(cprime + row);
+    G.x += cp; G.y += cp; G.z += cp; G.w += cp;
+    if (MODE == 1) { *reinterpret_cast<float4*>(xn + (size_t)row * B + 4 * c4) = G; return; }
+    const uint32_t t = (st ? st->t : 0u) + t_off;
+    update_store<GFUN>(row, c4, B, G, x, y, xn, up, t);
+}
+
+// S5 for sparse QUBO: partial[rb][b] = sum over the rows of block rb of x_hat_i ((Q_off x_hat)_i + c'_i)
+template <bool INTEGRAL>
+__global__ void __launch_bounds__(THREADS)
+spmm_score(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+           const float* __restrict__ val2, const float* __restrict__ cprime, const float* __restrict__ x,
+           void* __restrict__ partial) {
+    using acc_t = typename std::conditional<INTEGRAL, long long, double>::type;
+    __shared__ acc_t red[WARPS][32][4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c4 = blockIdx.y * 32 + lane;
+    const bool active = 4 * c4 < B;
+    const int row0 = blockIdx.x * SCORE_ROWS;
+    acc_t acc[4] = {0, 0, 0, 0};
+    for (int r = warp; r < SCORE_ROWS; r += WARPS) {
+        const int row = row0 + r;
+        if (row >= n) break;
+        const int start = __ldg(rowptr + row), end = __ldg(rowptr + row + 1);
+        float s[4] = {0.f, 0.f, 0.f, 0.f};                   // fp32 row sums of val2 * x_hat_j
+        int si[4] = {0, 0, 0, 0};
+        for (int base = start; base < end; base += 32) {
+            const int k = base + lane;
+            const int my_c = (k < end) ? __ldg(col + k) : 0;
+            const float my_v = (k < end) ? __ldg(val2 + k) : 0.0f;
+            const int cnt = min(32, end - base);
+            for (int u = 0; u < cnt; ++u) {
+                const int c = __shfl_sync(0xffffffffu, my_c, u);
+                const float v = __shfl_sync(0xffffffffu, my_v, u);
+                if (!active) continue;
+                const float4 g = ldg4(x + (size_t)c * B + 4 * c4);
+                if (INTEGRAL) {
+                    const int vi = __float2int_rn(v);
+                    si[0] += g.x > 0.5f ? vi : 0; si[1] += g.y > 0.5f ? vi : 0;
+                    si[2] += g.z > 0.5f ? vi : 0; si[3] += g.w > 0.5f ? vi : 0;
+                } else {
+                    s[0] += g.x > 0.5f ? v : 0.f; s[1] += g.y > 0.5f ? v : 0.f;
+                    s[2] += g.z > 0.5f ? v : 0.f; s[3] += g.w > 0.5f ? v : 0.f;
+                }
+            }
+        }
+        if (!active) continue;
+        const float4 xi = ldg4(x + (size_t)row * B + 4 * c4);
+        const float cp = __ldg(cprime + row);
+        const bool on[4] = {xi.x > 0.5f, xi.y > 0.5f, xi.z > 0.5f, xi.w > 0.5f};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (!on[q]) continue;
+            if (INTEGRAL) acc[q] += (long long)(si[q] / 2) + (long long)__float2int_rn(cp);  // val2 = 2 Q_ij: even
+            else acc[q] += 0.5 * (double)s[q] + (double)cp;
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) red[warp][lane][q] = acc[q];
+    __syncthreads();
+    if (warp == 0 && active) {
+        acc_t* out = reinterpret_cast<acc_t*>(partial) + (size_t)blockIdx.x * B + 4 * c4;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            acc_t t = red[0][lane][q];
+            for (int w = 1; w < WARPS; ++w) t += red[w][lane][q];
+            out[q] = t;
+        }
+    }
+}
+
+template <int MODE>
+gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
+                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+    const int chunks = (B / 4 + 31) / 32;
+    const int n_light = p->d_light_rows ? p->n_light : p->n;
+    if (n_light > 0) {
+        const long long items = (long long)n_light * chunks;
+        const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
+        if (up.gfun == GDA_G_QUADRATIC)
+            spmm_step_warp<GDA_G_QUADRATIC, MODE><<<grid, THREADS, 0, s>>>(n_light, p->d_light_rows, B, chunks, p->d_rowptr,
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off);
+        else
+            spmm_step_warp<GDA_G_ENTROPY, MODE><<<grid, THREADS, 0, s>>>(n_light, p->d_light_rows, B, chunks, p->d_rowptr,
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off);
+        if (launches) ++*launches;
+    }
+    if (p->n_heavy > 0) {
+        const unsigned grid = (unsigned)(p->n_heavy * chunks);
+        if (up.gfun == GDA_G_QUADRATIC)
+            spmm_step_split<GDA_G_QUADRATIC, MODE><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off);
+        else
+            spmm_step_split<GDA_G_ENTROPY, MODE><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off);
+        if (launches) ++*launches;
+    }
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+}  // namespace
+
+int sparse_heavy_threshold() { return HEAVY_DEG; }
+
+gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
+                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+    return launch_step<0>(p, B, x, y, xn, up, st, t_off, s, launches);
+}
+
+gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s) {
+    UpdParams up{};
+    up.gfun = GDA_G_QUADRATIC;
+    return launch_step<1>(p, B, x, nullptr, G, up, nullptr, 0, s, nullptr);
+}
+
+int32_t sparse_num_partials(const gda_problem* p, int32_t) { return (p->n + SCORE_ROWS - 1) / SCORE_ROWS; }
+
+gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
+                                 cudaStream_t s, int64_t* launches) {
+    const int chunks = (B / 4 + 31) / 32;
+    dim3 grid((unsigned)sparse_num_partials(p, B), (unsigned)chunks);
+    if (p->integral)
+        spmm_score<true><<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
+    else
+        spmm_score<false><<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
+    if (launches) ++*launches;
+    *n_part = (int32_t)grid.x;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
