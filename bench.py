@@ -1,0 +1,385 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the GDA hot path on synthetic BASELINE.json workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over the batch of B restarts: `eval_every` GDA iterations
+(gradient S1/S2/S3 + fused update S4, one kernel each) followed by one evaluation (round + exact score
+S5 + best-so-far), i.e. one CUDA-graph launch of the library; the arg-best S6 closes every call.
+metric = restart-iterations/s = B * eval_every * K / time.
+
+Timed region: K resumed gda_run calls of one step each, every one bracketed by CUDA events on the
+launching stream; the L2 is flushed (a 256 MiB write, not timed) between steps because the state of
+the sparse configs (61.5 MB) is smaller than the 126 MB L2.  `whole_run` repeats the measurement as ONE
+gda_run of K steps without flushes (the way a user runs it).  `e2e` is gda_run_host: pinned HOST
+buffers in, HOST results out, copies inside the timed region.
+
+Under torchrun (N > 1) every rank runs its own B restarts of the same instance (restarts are
+independent): weak scaling, no collective on the data path; the best objective is
+combined with one all-reduce(MIN) after the timed region.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_2509_21064_b200 import workloads as wl  # noqa: E402
+
+HEADLINE_CONFIG = 3   # BASELINE.json configs[2]: Max-Cut n=20000, B=256 -- the config the HBM target is quoted on
+
+
+def load_peaks():
+    f = ROOT / "MEASURED_PEAKS.json"
+    if f.exists():
+        d = json.loads(f.read_text())
+        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16_tflops=float(d["bf16_tflops"]),
+                    bf16_tflops_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), source="measured")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
+
+
+def algorithmic_work(w: wl.Workload):
+    """Per GDA step (one launch of the step kernel): algorithmic bytes / flops."""
+    P, B = w.problem, w.B
+    n = P.n
+    state = 16 * n * B                       # read x, y; write x, y (fp32)
+    if w.kind == "qubo_csr":
+        nnz = int(P.rowptr[-1])
+        return dict(bound="hbm", bytes=state + 8 * nnz + 4 * (n + 1) + 4 * n, flops=2 * nnz * B)
+    if w.kind == "maxsat":
+        L = int(P.lit.shape[0])
+        k = L // P.m
+        return dict(bound="hbm", bytes=state + 4 * (n + 1) + L * (4 + 4 * max(k - 1, 1)), flops=(k + 1) * L * B)
+    return dict(bound="tensor", bytes=state + 2 * 2 * n * B + 2 * n * n, flops=2 * n * n * B)
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu, self.rows, self.proc = gpu_index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.gpu)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+        sm, smax, reasons = [], 0.0, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1]))
+                smax = max(smax, float(r[2]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        busy = [v for v in sm if v > 0]
+        return dict(sm_mhz=statistics.median(busy) if busy else None, sm_max_mhz=smax or None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle arm (cpu_baseline leg and --impl reference): the ONLY place bench.py executes oracle/
+# ------------------------------------------------------------------------------------------------
+def oracle_problem(P):
+    from oracle import pdbo
+    if isinstance(P, wl.QuboCSR):
+        return pdbo.Problem.qubo_csr(P.n, P.rowptr, P.col, P.val, P.c)
+    if isinstance(P, wl.QuboDense):
+        return pdbo.Problem.qubo_dense(P.n, P.Q, P.c)
+    return pdbo.Problem.maxsat(P.n, P.m, P.cptr, P.lit, P.w)
+
+
+def oracle_kwargs(h, iters):
+    f = lambda v: float(np.float32(v))
+    return dict(alpha=f(h.alpha), beta=f(h.beta), delta=f(h.delta), gfun=h.gfun, log_eps=f(h.log_eps),
+                iters=iters, eval_every=h.eval_every, seed=h.seed)
+
+
+def oracle_sample_columns(w: wl.Workload, cores: int) -> int:
+    """Restart columns per oracle step: one per core, fewer for the dense config (n^2 work per column-step)."""
+    return max(1, min(w.B, cores if w.kind != "qubo_dense" else min(cores, 8)))
+
+
+def time_oracle(w: wl.Workload, budget_s: float):
+    """cpu_baseline: the oracle as it stands (fp64, OpenMP over restarts) on a bounded sample."""
+    from oracle import pdbo
+    pdbo.build()
+    cores = max(1, min(pdbo.max_threads(), os.cpu_count() or 1))
+    OP = oracle_problem(w.problem)
+    Bo = oracle_sample_columns(w, cores)
+    X0 = wl.x0_uniform(w.problem.n, w.B, w.x0_seed)[:, :Bo].copy()
+    h = w.hyper
+    it = 2 if w.kind == "qubo_dense" else 10
+    pdbo.run(OP, X0, float(np.float32(h.lambda0)), nthreads=cores, **oracle_kwargs(h, it))     # thread-pool warm-up
+    t0 = time.perf_counter()
+    pdbo.run(OP, X0, float(np.float32(h.lambda0)), nthreads=cores, **oracle_kwargs(h, it))
+    per_iter = (time.perf_counter() - t0) / it
+    iters = int(max(it, min(h.iters, budget_s / max(per_iter, 1e-9))))
+    mult = int(min(w.B // Bo, max(1.0, budget_s / max(iters * per_iter, 1e-9))))   # more columns if the budget allows
+    if mult > 1:
+        Bo *= mult
+        X0 = wl.x0_uniform(w.problem.n, w.B, w.x0_seed)[:, :Bo].copy()
+    t0 = time.perf_counter()
+    pdbo.run(OP, X0, float(np.float32(h.lambda0)), nthreads=cores, **oracle_kwargs(h, iters))
+    dt = time.perf_counter() - t0
+    return dict(value=Bo * iters / dt, unit="restart-iters/s", cores=cores, kind="oracle",
+                sample=f"{Bo} of {w.B} restarts x {iters} GDA iterations of {w.name}, fp64, gcc -O2 -fopenmp, {dt:.1f} s")
+
+
+def run_reference(args, w: wl.Workload):
+    """--impl reference: K steps of the oracle, each `eval_every` iterations + evaluation on a column sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import pdbo
+    pdbo.build()
+    cores = max(1, min(pdbo.max_threads(), os.cpu_count() or 1))
+    OP = oracle_problem(w.problem)
+    Bo = oracle_sample_columns(w, cores)
+    h = w.hyper
+    per_step = h.eval_every if w.kind != "qubo_dense" else max(1, h.eval_every // 50)
+    X = wl.x0_uniform(w.problem.n, w.B, w.x0_seed)[:, :Bo].copy().astype(np.float64)
+    Y = np.full_like(X, float(np.float32(h.lambda0)))
+    kw = oracle_kwargs(h, per_step)
+    kw["eval_every"] = per_step
+    t = 0
+    for _ in range(args.warmup):
+        r = pdbo.run(OP, X, Y, nthreads=cores, t0=t, **kw)
+        X, Y, t = r["x"], r["y"], t + per_step
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r = pdbo.run(OP, X, Y, nthreads=cores, t0=t, **kw)
+        X, Y, t = r["x"], r["y"], t + per_step
+    dt = time.perf_counter() - t0
+    value = Bo * per_step * args.steps / dt
+    sample = f"{Bo} of {w.B} restarts, {per_step} GDA iterations + 1 evaluation per step, fp64 oracle"
+    print(json.dumps({
+        "impl": "reference", "metric": "restart-iterations/s", "value": value, "unit": "restart-iters/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "n": w.problem.n, "B": w.B, "note": w.note},
+        "cpu_baseline": {"value": value, "unit": "restart-iters/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "restart-iters/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------
+def run_ours(args, w: wl.Workload):
+    import torch
+    import torch.distributed as dist
+    from paper_2509_21064_b200 import api, build
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus != world and world > 1:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    api.lib()
+
+    peaks = load_peaks()
+    h, B, n = w.hyper, w.B, w.problem.n
+    K, W = args.steps, max(args.warmup, 3)
+    P = api.create_from_workload(w.problem)
+    x0_host = torch.from_numpy(wl.x0_uniform(n, B, w.x0_seed + 7919 * rank)).pin_memory()   # each rank: its own restarts
+    x0 = x0_host.to(dev, non_blocking=True)
+    stream = torch.cuda.Stream(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    prm_step = api.params_from_hyper(h, iters=h.eval_every)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+
+    def sync_all():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    with torch.cuda.stream(stream):
+        # ---- warm-up: W steps (captures the CUDA graph, warms caches and clocks) ----
+        out = P.run(x0, h.lambda0, prm_step)
+        for _ in range(W - 1):
+            P.resume(prm_step, out)
+        sync_all()
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        # ---- timed: K steps, L2 flushed (untimed) between them ----
+        out = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=0))
+        launches = P.info().last_run_kernel_launches
+        sync_all()
+        wall0 = time.perf_counter()
+        for k in range(K):
+            flush.fill_(k & 0xFF)
+            ev[k][0].record(stream)
+            P.resume(prm_step, out)
+            ev[k][1].record(stream)
+            launches += P.info().last_run_kernel_launches
+        sync_all()
+        wall = time.perf_counter() - wall0
+        step_ms = [a.elapsed_time(b) for a, b in ev]
+        t_steps = sum(step_ms) / 1e3
+        best_flushed = float(out["obj"].min().item())
+
+        # ---- whole_run: one gda_run of K steps, no flush ----
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        prm_all = api.params_from_hyper(h, iters=h.eval_every * K)
+        sync_all()
+        e0.record(stream)
+        out = P.run(x0, h.lambda0, prm_all, trace_cap=min(K, 4096))
+        e1.record(stream)
+        sync_all()
+        t_whole = e0.elapsed_time(e1) / 1e3
+        whole_launches = P.info().last_run_kernel_launches
+        step_launches = P.info().last_run_step_launches
+
+        # ---- evaluation alone (one evaluation-only call), to isolate the step kernel's share ----
+        prm0 = api.params_from_hyper(h, iters=0)
+        P.resume(prm0, out)
+        sync_all()
+        e0.record(stream)
+        for _ in range(10):
+            P.resume(prm0, out)
+        e1.record(stream)
+        sync_all()
+        t_eval = e0.elapsed_time(e1) / 1e3 / 10
+        clocks = sampler.stop()
+
+        # ---- e2e: HOST buffers through gda_run_host (copies inside the timed region) ----
+        xb_host = torch.empty((n, B), dtype=torch.uint8).pin_memory()
+        obj_host = torch.empty(B, dtype=torch.float64).pin_memory()
+        best_host = torch.empty(1, dtype=torch.int32).pin_memory()
+        P.run_host_ptrs(B, x0_host.data_ptr(), h.lambda0, api.params_from_hyper(h, iters=h.eval_every),
+                        xb_host.data_ptr(), obj_host.data_ptr(), best_host.data_ptr(), stream.cuda_stream)
+        sync_all()
+        w0 = time.perf_counter()
+        e0.record(stream)
+        P.run_host_ptrs(B, x0_host.data_ptr(), h.lambda0, prm_all, xb_host.data_ptr(), obj_host.data_ptr(),
+                        best_host.data_ptr(), stream.cuda_stream)
+        e1.record(stream)
+        sync_all()
+        t_e2e = max(e0.elapsed_time(e1) / 1e3, 0.0)
+        t_e2e_wall = time.perf_counter() - w0
+
+    def max_over_ranks(v):
+        if world == 1:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    t_steps, t_whole, t_e2e, t_eval = map(max_over_ranks, (t_steps, t_whole, max(t_e2e, t_e2e_wall), t_eval))
+    best = float(out["obj"].min().item())
+    if world > 1:
+        tb = torch.tensor([best], dtype=torch.float64, device=dev)
+        dist.all_reduce(tb, op=dist.ReduceOp.MIN)           # the only exchange: arg-best across ranks
+        best = float(tb.item())
+
+    iters_per_step = h.eval_every
+    units = world * B * iters_per_step * K
+    work = algorithmic_work(w)
+    t_kernel = max((t_steps / K - t_eval), 1e-9) / iters_per_step        # avg duration of one step-kernel launch
+    if work["bound"] == "hbm":
+        achieved, peak, unit = work["bytes"] / t_kernel / 1e9, peaks["hbm_gbs"], "GB/s"
+    else:
+        achieved, peak, unit = work["flops"] / t_kernel / 1e12, peaks["bf16_tflops_sustained"], "TFLOP/s"
+    trace = None
+    if "trace_best" in out:
+        tb_, tn_ = out["trace_best"].cpu().numpy(), out["trace_ns"].cpu().numpy()
+        sel = sorted(set([0, len(tb_) // 4, len(tb_) // 2, len(tb_) - 1]))
+        trace = [{"ms": float((tn_[i] - tn_[0]) / 1e6 + t_whole * 1e3 / K), "best": float(tb_[i])} for i in sel]
+
+    if rank == 0:
+        cpu = time_oracle(w, args.cpu_budget) if world == 1 and not args.no_cpu_baseline else None
+        line = {
+            "metric": "restart-iterations/s", "value": units / t_steps, "unit": "restart-iters/s",
+            "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": 1e3 * t_steps / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if w.kind != "qubo_dense" else "bf16 x bf16 -> f32 (state f32)", "data": "synthetic",
+            "config": {"workload": w.name, "baseline_config_index": args.config, "kind": w.kind, "n": n, "B_per_gpu": B,
+                       "step": f"{iters_per_step} GDA iterations + 1 evaluation (one CUDA graph launch)",
+                       "hyper": {"lambda0": h.lambda0, "alpha": h.alpha, "beta": h.beta, "delta": h.delta, "gfun": h.gfun},
+                       "l2": "flushed between timed steps (256 MiB write, untimed)", "note": w.note},
+            "whole_run": {"value": units / t_whole, "unit": "restart-iters/s", "ms_total": 1e3 * t_whole,
+                          "iters": iters_per_step * K, "l2": "not flushed (one gda_run call)", "best_objective": best,
+                          "best_vs_time": trace},
+            "e2e": {"value": units / t_e2e, "unit": "restart-iters/s", "h2d_bytes_per_step": 4 * n * B / K,
+                    "d2h_bytes_per_step": (n * B + 8 * B + 4) / K, "ms_total": 1e3 * t_e2e,
+                    "note": "gda_run_host: one call of K steps; x0 H2D and x_bin/obj/best D2H once per call, amortised per step"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": work["bound"], "achieved": achieved, "peak": peak, "unit": unit,
+                         "frac": achieved / peak, "traffic": None, "peak_source": peaks["source"],
+                         "kernel": "step kernel (gradient + fused update)", "us_per_launch": t_kernel * 1e6,
+                         "algorithmic_bytes_per_launch": work["bytes"], "algorithmic_flops_per_launch": work["flops"],
+                         "eval_us": t_eval * 1e6},
+            "clocks": clocks,
+            "best_objective": best, "best_objective_flushed_run": best_flushed,
+        }
+        if cpu:
+            line["cpu_baseline"] = cpu
+        print(json.dumps(line))
+    P.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=HEADLINE_CONFIG, help="BASELINE.json config, 1-based")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--B", type=int, default=None)
+    args = ap.parse_args()
+    w = wl.config(args.config, B=args.B)
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()

@@ -101,7 +101,9 @@ typedef struct {
 } gda_extra;
 
 /* Algorithm 1 (reconstructed in DESIGN.md reading R0) for B restarts.
- *   x0          DEVICE fp32 [n][B], values in [0,1]           (x0 ~ U[0,1]^n)
+ *   x0          DEVICE fp32 [n][B], values in [0,1]           (x0 ~ U[0,1]^n); or NULL to RESUME:
+ *               continue from the iterates, duals, iteration counter and best-so-far that the previous
+ *               gda_run on this handle (same B) left in it -- lambda0 and params->t0 are then ignored
  *   lambda0     DEVICE fp32 [n][B] or NULL -> every entry = lambda0_scalar (y-bar)
  *   x_bin       DEVICE uint8 [n][B]: per restart, the rounded point x_hat = [x > 1/2] with the best
  *               objective seen at any evaluation (R5)

@@ -141,6 +141,7 @@ class Problem:
         assert x0.is_cuda and x0.dtype == torch.float32 and x0.is_contiguous() and x0.shape[0] == self.n
         n, B = x0.shape
         dev = x0.device
+        self._last = (n, B, dev)
         l_ptr, l_scalar = None, 0.0
         if isinstance(lambda0, torch.Tensor):
             assert lambda0.is_cuda and lambda0.dtype == torch.float32 and lambda0.is_contiguous() and lambda0.shape == x0.shape
@@ -163,6 +164,16 @@ class Problem:
         s = torch.cuda.current_stream(dev).cuda_stream if stream is None else stream
         _check(lib().gda_run(self._h, B, x0.data_ptr(), l_ptr, l_scalar, C.byref(params), out["x_bin"].data_ptr(),
                              out["obj"].data_ptr(), out["best_restart"].data_ptr(), C.byref(ex), s))
+        return out
+
+    def resume(self, params: Params, out: dict, stream=None):
+        """gda_run with x0 = NULL: continue the previous run on this handle for params.iters more steps,
+        writing into the tensors of `out` (a dict returned by run())."""
+        import torch
+        n, B, dev = self._last
+        s = torch.cuda.current_stream(dev).cuda_stream if stream is None else stream
+        _check(lib().gda_run(self._h, B, None, None, 0.0, C.byref(params), out["x_bin"].data_ptr(),
+                             out["obj"].data_ptr(), out["best_restart"].data_ptr(), None, s))
         return out
 
     def run_host(self, x0: np.ndarray, lambda0, params: Params, stream=None):

@@ -451,8 +451,10 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
                                  const void* x_bin, const void* obj, const void* best_restart) {
     GDA_REQUIRE(p != nullptr, "gda_run: problem is NULL");
     GDA_REQUIRE(prm != nullptr, "gda_run: params is NULL");
-    GDA_REQUIRE(x0 != nullptr && x_bin != nullptr && obj != nullptr && best_restart != nullptr,
-                "gda_run: x0, x_bin, obj and best_restart are required");
+    GDA_REQUIRE(x_bin != nullptr && obj != nullptr && best_restart != nullptr,
+                "gda_run: x_bin, obj and best_restart are required");
+    GDA_REQUIRE(x0 != nullptr || (p->ws.has_state && p->ws.B == B),
+                "gda_run: x0 is NULL but the handle holds no state of a previous run with B = %d to resume", B);
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_run: B must be a positive multiple of 4 (got %d)", B);
     GDA_REQUIRE(std::isfinite(prm->alpha) && prm->alpha > 0.0f, "gda_run: alpha must be > 0");
     GDA_REQUIRE(std::isfinite(prm->beta) && prm->beta > 0.0f, "gda_run: beta must be > 0");
@@ -481,10 +483,15 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
     const size_t elems = (size_t)p->n * B;
     p->last_launches = 0; p->last_step_launches = 0;
 
-    GDA_TRY(run_init(p, B, x0, lambda0, lambda0_scalar, (uint32_t)prm->t0, s, &p->last_launches));
     int parity = 0;
-    if (p->kind == GDA_KIND_DENSE)
-        GDA_TRY(dense_make_operand(p, B, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
+    if (x0) {
+        ws.has_state = false;
+        GDA_TRY(run_init(p, B, x0, lambda0, lambda0_scalar, (uint32_t)prm->t0, s, &p->last_launches));
+        if (p->kind == GDA_KIND_DENSE)
+            GDA_TRY(dense_make_operand(p, B, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
+    } else {
+        parity = ws.parity;      // resume: iterates, duals, best-so-far and the iteration counter stay as they are
+    }
     const int32_t full = prm->iters / prm->eval_every, rem = prm->iters % prm->eval_every;
     for (int32_t c = 0; c < full; ++c) {
         GDA_TRY(launch_chunk(p, B, prm->eval_every, parity, *prm, s));
@@ -494,6 +501,8 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
     if (prm->iters == 0) GDA_TRY(launch_chunk(p, B, 0, parity, *prm, s));     // evaluate the start point
     GDA_TRY(eval_argbest(B, ws.best_obj, ws.best_restart, ws.best_val, s, &p->last_launches));
 
+    ws.parity = parity;
+    ws.has_state = true;
     const float* xfin = (p->kind == GDA_KIND_DENSE) ? ws.x[0] : ws.x[parity];
     GDA_CUDA_TRY(cudaMemcpyAsync(x_bin, ws.x_bin, elems, cudaMemcpyDeviceToDevice, s));
     GDA_CUDA_TRY(cudaMemcpyAsync(obj, ws.best_obj, (size_t)B * sizeof(double), cudaMemcpyDeviceToDevice, s));
@@ -516,6 +525,7 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
 extern "C" gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, const float* lambda0,
                                    float lambda0_scalar, const gda_params* prm, uint8_t* x_bin, double* obj,
                                    int32_t* best_restart, void* stream) {
+    GDA_REQUIRE(x0 != nullptr, "gda_run_host: x0 is required");
     GDA_TRY(check_run_args(p, B, x0, prm, x_bin, obj, best_restart));
     GDA_CUDA_TRY(cudaSetDevice(p->device));
     GDA_TRY(ensure_workspace(p, B));

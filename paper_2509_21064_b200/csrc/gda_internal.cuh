@@ -50,6 +50,8 @@ struct RunState {
 // ---------------------------------------------------------------------------------------------------
 struct Workspace {
     int32_t B = 0;
+    int32_t parity = 0;                 // which x / zt buffer holds the current iterate
+    bool has_state = false;             // a previous gda_run left (x, y, best-so-far) here: x0 == NULL may resume
     float* x[2] = {nullptr, nullptr};   // [n][B] double buffer (Jacobi: every row reads all of x^t)
     float* y = nullptr;                 // [n][B], updated in place
     uint8_t* x_bin = nullptr;           // [n][B] best-so-far rounded point
@@ -185,10 +187,14 @@ __device__ __forceinline__ void gda_update(float x, float y, float G, const UpdP
         gp = 2.0f * x - 1.0f;
         gv = x * x - x;
     } else {
-        const float xc = fminf(fmaxf(x, up.log_eps), 1.0f - up.log_eps);
-        const float l0 = logf(xc), l1 = logf(1.0f - xc);
+        // g'(x) = ln(xc) - ln(1 - xc), xc = clip(x, eps, 1 - eps) (reading R4), evaluated as
+        // ln(clip(x)) - ln(clip(1 - x)): the same function, but 1 - x is exact in fp32 near x = 1
+        // whereas 1 - eps is not representable (1 - fl(1 - 1e-6) = 1.013e-6 would shift g' by 1.3e-2).
+        const float u = 1.0f - x, hi = 1.0f - up.log_eps;
+        const float a = fminf(fmaxf(x, up.log_eps), hi), b = fminf(fmaxf(u, up.log_eps), hi);
+        const float l0 = logf(a), l1 = logf(b);
         gp = l0 - l1;
-        gv = (xc == x) ? (x * l0 + (1.0f - x) * l1) : (xlogx_f(x) + xlogx_f(1.0f - x));
+        gv = (a == x && b == u) ? (x * l0 + u * l1) : (xlogx_f(x) + xlogx_f(u));
     }
     float xt = x - up.alpha * (G + y * gp);
     xt = fminf(fmaxf(xt, 0.0f), 1.0f);
