@@ -323,6 +323,10 @@ def run_ours(args, w: wl.Workload):
         achieved, peak, unit = work["bytes"] / t_kernel / 1e9, peaks["hbm_gbs"], "GB/s"
     else:
         achieved, peak, unit = work["flops"] / t_kernel / 1e12, peaks["bf16_tflops_sustained"], "TFLOP/s"
+    traffic = None
+    tf = ROOT / "profiles" / "ncu_traffic.json"
+    if tf.exists():
+        traffic = json.loads(tf.read_text()).get(w.name, {}).get("bytes")
     trace = None
     if "trace_best" in out:
         tb_, tn_ = out["trace_best"].cpu().numpy(), out["trace_ns"].cpu().numpy()
@@ -348,7 +352,7 @@ def run_ours(args, w: wl.Workload):
                     "note": "gda_run_host: one call of K steps; x0 H2D and x_bin/obj/best D2H once per call, amortised per step"},
             "gpu_launches": int(launches),
             "roofline": {"bound": work["bound"], "achieved": achieved, "peak": peak, "unit": unit,
-                         "frac": achieved / peak, "traffic": None, "peak_source": peaks["source"],
+                         "frac": achieved / peak, "traffic": traffic, "peak_source": peaks["source"],
                          "kernel": "step kernel (gradient + fused update)", "us_per_launch": t_kernel * 1e6,
                          "algorithmic_bytes_per_launch": work["bytes"], "algorithmic_flops_per_launch": work["flops"],
                          "eval_us": t_eval * 1e6},
