@@ -36,7 +36,7 @@ typedef enum {
     GDA_ERR_INVALID_ARG = 1, /* null pointer, bad size, asymmetric Q, index out of range, bad parameter ... */
     GDA_ERR_ALLOC = 2,       /* host or device allocation failed */
     GDA_ERR_CUDA = 3,        /* a CUDA call or kernel launch failed (message has the CUDA error string) */
-    GDA_ERR_UNSUPPORTED = 4  /* valid request this build cannot serve (e.g. dense n not a multiple of 128) */
+    GDA_ERR_UNSUPPORTED = 4  /* valid request this build cannot serve (e.g. dense n not a multiple of 256) */
 } gda_status;
 
 /* binarity function g (default quadratic; entropy for Max-k-SAT, 580/592) */
@@ -63,7 +63,7 @@ gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, const int32_t* 
 
 /* gda_create_qubo_dense: HOST Q row-major [n][n] (symmetric), HOST c[n] or NULL.  flags must contain
  *   GDA_DENSE_BF16: Q is rounded to bf16 (lossless when Q is bf16-representable, reading R13)
- *   and the gradient is a tcgen05 GEMM with fp32 accumulation.  UNSUPPORTED: n not a multiple of 128 or
+ *   and the gradient is a tcgen05 GEMM with fp32 accumulation.  UNSUPPORTED: n not a multiple of 256 or
  *   flags without GDA_DENSE_BF16.  gda_run on a dense problem needs B to be a multiple of 128. */
 gda_status gda_create_qubo_dense(int32_t n, const float* Q, const float* c, int32_t flags, gda_problem** out);
 

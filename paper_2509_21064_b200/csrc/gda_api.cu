@@ -162,7 +162,7 @@ extern "C" gda_status gda_create_qubo_dense(int32_t n, const float* Q, const flo
     GDA_REQUIRE(n > 0, "gda_create_qubo_dense: n must be > 0 (got %d)", n);
     GDA_REQUIRE(Q != nullptr, "gda_create_qubo_dense: Q is NULL");
     if (!(flags & GDA_DENSE_BF16)) { gda_set_error("gda_create_qubo_dense: only GDA_DENSE_BF16 is implemented"); return GDA_ERR_UNSUPPORTED; }
-    if (n % 128 != 0) { gda_set_error("gda_create_qubo_dense: n must be a multiple of 128 (got %d)", n); return GDA_ERR_UNSUPPORTED; }
+    if (n % 256 != 0) { gda_set_error("gda_create_qubo_dense: n must be a multiple of 256 (got %d)", n); return GDA_ERR_UNSUPPORTED; }
     for (int i = 0; i < n; ++i) {
         GDA_REQUIRE(!c || std::isfinite(c[i]), "gda_create_qubo_dense: non-finite c[%d]", i);
         for (int j = i; j < n; ++j) {
@@ -393,7 +393,7 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     int32_t n_part = 0;
     if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
     else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
-    else GDA_TRY(dense_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
+    else { ws.score_scratch = cur ^ 1; GDA_TRY(dense_score_partials(p, B, xcur, ws.partial, &n_part, s, launches)); }
     GDA_TRY(eval_finalize(p, B, ws.partial, n_part, ws.obj_now, ws.best_obj, ws.improved, ws.state, ws.trace_best,
                           ws.trace_ns, ws.trace_cap, (uint32_t)len, s, launches));
     GDA_TRY(eval_commit(p, B, xcur, ws.improved, ws.x_bin, s, launches));
@@ -585,7 +585,7 @@ extern "C" gda_status gda_score(gda_problem* p, int32_t B, const float* x, doubl
     int32_t n_part = 0;
     if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr));
     else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr));
-    else GDA_TRY(dense_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr));
+    else { p->ws.has_state = false; p->ws.score_scratch = 1; GDA_TRY(dense_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr)); }
     GDA_TRY(score_reduce(p, B, p->ws.partial, n_part, obj, s));
     return join_stream(p, user, s);
 }

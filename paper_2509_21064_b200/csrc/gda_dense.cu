@@ -1,12 +1,444 @@
-// gda_dense.cu -- S2 + S4 for dense QUBO (tcgen05 GEMM gradient).  Placeholder until the kernel lands.
+// gda_dense.cu -- S2 + S4 for dense QUBO: tcgen05 / TMA / TMEM GEMM gradient with the GDA update fused
+// into the epilogue.
+//
+//   G = 2 Q_off X + c' 1^T          (reading R1)
+// computed with the CENTRED bf16 operand z = x - 1/2 (reading R13):  G = 2 Q_off z + (Q_off 1 + c').
+//
+// GEMM shape (both operands K-major, the layout tcgen05 takes without transposition):
+//   D[b][i] = sum_k Zt[b][k] * Qoff[i][k]        M = restarts b, N = variables i, K = variables k
+//   A = Zt   bf16 [B][n]  (the transposed, centred copy of X; double-buffered: step t reads zt_in while
+//                          its epilogue writes zt_out for step t+1 -- Jacobi update, Eq. 6)
+//   B = Qoff bf16 [n][n]  (symmetric, zero diagonal)
+//   D fp32 in TMEM: lane = restart b (128 per tile), column = variable i (256 per tile), two accumulator
+//   stages (2 x 256 = 512 columns) so the epilogue of tile t overlaps the MMAs of tile t+1.
+// With lanes = restarts the epilogue's accesses to the fp32 state X, Y ([n][B]) are coalesced 128-byte
+// rows per warp, and each thread writes 64 contiguous bytes of the next bf16 operand.
+//
+// Warp roles (384 threads, one persistent CTA per SM): warp 0 TMA producer, warp 1 MMA issuer (one
+// elected thread), warp 2 TMEM allocator, warps 4-11 epilogue (two warpgroups, 128 columns each).
 #include "gda_internal.cuh"
 
-static gda_status nyi() { gda_set_error("dense path: not built yet"); return GDA_ERR_UNSUPPORTED; }
-gda_status dense_prepare(gda_problem*, const float*, const float*) { return nyi(); }
-gda_status dense_make_operand(gda_problem*, int32_t, const float*, __nv_bfloat16*, int, cudaStream_t, int64_t*) { return nyi(); }
-gda_status dense_step(gda_problem*, int32_t, float*, float*, const __nv_bfloat16*, __nv_bfloat16*, const UpdParams&,
-                      const RunState*, uint32_t, cudaStream_t, int64_t*) { return nyi(); }
-gda_status dense_grad(gda_problem*, int32_t, const float*, float*, cudaStream_t) { return nyi(); }
-gda_status dense_score_partials(gda_problem*, int32_t, const float*, void*, int32_t*, cudaStream_t, int64_t*) { return nyi(); }
-int32_t dense_num_partials(const gda_problem*, int32_t) { return 1; }
-void dense_release(gda_problem*) {}
+#include <cuda.h>
+#include <cmath>
+#include <vector>
+
+namespace {
+
+constexpr int BM = 128, BN = 256, BK = 64, STAGES = 4, UMMA_K = 16;
+constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int NUM_THREADS = 384, EPI_WARP0 = 4, EPI_WARPS = 8;
+constexpr int TMEM_COLS = 512;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024;     // tiles + barriers + alignment slack
+
+enum { MODE_STEP = 0, MODE_GRAD = 1, MODE_SCORE = 2 };
+
+// ---- PTX wrappers -------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.b32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+// try_wait suspends in hardware for a bounded time per call; a wait that never completes is a pipeline bug,
+// so trap instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    for (uint32_t spins = 0; !mbar_try_wait(bar, parity); ++spins)
+        if (spins > (1u << 26)) __trap();
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem], bf16 x bf16 -> fp32, issued by one thread
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// 32 lanes x 32 columns of fp32 accumulator -> 32 registers per thread (thread = lane, register = column)
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// K-major, 128-byte-swizzled shared-memory operand descriptor (rows of 64 bf16 = 128 B, 8-row groups 1024 B apart)
+__device__ __forceinline__ uint64_t make_sdesc(uint32_t smem_addr) {
+    uint64_t d = 0;
+    d |= (uint64_t)((smem_addr & 0x3FFFF) >> 4);          // [0,14)  start address / 16
+    d |= (uint64_t)1 << 16;                               // [16,30) leading byte offset (unused for swizzled K-major)
+    d |= (uint64_t)(1024 >> 4) << 32;                     // [32,46) stride byte offset: 8 rows x 128 B
+    d |= (uint64_t)1 << 46;                               // [46,48) descriptor version (sm_100)
+    d |= (uint64_t)2 << 61;                               // [61,64) layout: SWIZZLE_128B
+    return d;
+}
+// instruction descriptor, kind::f16: D fp32, A/B bf16, both K-major, N and M of the UMMA
+__host__ __device__ constexpr uint32_t make_idesc(int M, int N) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+// ---- the fused GEMM + update kernel ----------------------------------------------------------------------
+struct DenseArgs {
+    int n, B;
+    float* x;                    // [n][B] fp32 state, updated in place (each element is owned by one thread)
+    float* y;                    // [n][B]
+    __nv_bfloat16* zt_out;       // [B][n] centred bf16 operand of the NEXT step
+    const float* hvec;           // [n]  Q_off 1 + c'  (constant part of the gradient with the centred operand)
+    const float* cprime;         // [n]  c + diag(Q)
+    float* gout;                 // MODE_GRAD: [n][B] gradient
+    double* partial;             // MODE_SCORE: [n/128][B] partial objective sums
+    UpdParams up;
+    const RunState* st;
+    uint32_t t_off;
+};
+
+template <int MODE, int GFUN>
+__global__ void __launch_bounds__(NUM_THREADS, 1)
+dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
+                  const DenseArgs args) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;            // SWIZZLE_128B needs 1024 B alignment
+    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+    auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + s); };
+    auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + 2 + s); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
+    volatile uint32_t* tmem_slot_ptr =
+        reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int num_m = args.B / BM, num_n = args.n / BN, num_tiles = num_m * num_n, num_kb = args.n / BK;
+
+    if (warp == 0 && lane == 0) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_a) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_b) : "memory");
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), EPI_WARPS); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 2) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+                const int m_blk = tile % num_m, n_blk = tile / num_m;
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
+                    mbar_expect_tx(full_bar(stage), STAGE_BYTES);
+                    const uint32_t a_dst = smem_base + stage * STAGE_BYTES;
+                    tma_load_2d(a_dst, &tmap_a, full_bar(stage), kb * BK, m_blk * BM);
+                    tma_load_2d(a_dst + A_BYTES, &tmap_b, full_bar(stage), kb * BK, n_blk * BN);
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one thread) =====
+        if (lane == 0) {
+            constexpr uint32_t idesc = make_idesc(BM, BN);
+            int stage = 0; uint32_t phase = 0; int it = 0;
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
+                const int as = it & 1;
+                const uint32_t aphase = (uint32_t)(it >> 1) & 1u;
+                mbar_wait(tempty_bar(as), aphase ^ 1u);                           // epilogue has drained this accumulator
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
+                for (int kb = 0; kb < num_kb; ++kb) {
+                    mbar_wait(full_bar(stage), phase);                            // TMA bytes have landed
+                    tc_fence_after();
+                    const uint32_t a_addr = smem_base + stage * STAGE_BYTES;
+                    const uint64_t adesc = make_sdesc(a_addr), bdesc = make_sdesc(a_addr + A_BYTES);
+#pragma unroll
+                    for (int k = 0; k < BK / UMMA_K; ++k)                          // +32 B per K=16 slice inside the swizzle atom
+                        tc_mma(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)((kb | k) != 0));
+                    tc_commit(empty_bar(stage));                                   // frees the smem slot when the MMAs retire
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+                tc_commit(tfull_bar(as));                                          // accumulator complete -> epilogue
+            }
+        }
+    } else if (warp >= EPI_WARP0) {
+        // ===== epilogue: TMEM -> registers -> fused GDA update -> global =====
+        const int ew = warp - EPI_WARP0;
+        const int lane_grp = warp & 3;                      // TMEM lanes 32*lane_grp .. +31 are accessible to this warp
+        const int half = ew >> 2;                           // which 128 of the tile's 256 columns
+        const uint32_t t = (args.st ? args.st->t : 0u) + args.t_off;
+        int it = 0;
+        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
+            const int m_blk = tile % num_m, n_blk = tile / num_m;
+            const int as = it & 1;
+            const uint32_t aphase = (uint32_t)(it >> 1) & 1u;
+            const int b = m_blk * BM + lane_grp * 32 + lane;                      // restart owned by this thread
+            mbar_wait(tfull_bar(as), aphase);
+            tc_fence_after();
+            double score = 0.0;
+            for (int cb = 0; cb < 4; ++cb) {
+                const int col0 = half * 128 + cb * 32;
+                const int i0 = n_blk * BN + col0;
+                uint32_t acc[32];
+                tc_ld32(tmem_base + ((uint32_t)(lane_grp * 32) << 16) + (uint32_t)(as * BN + col0), acc);
+                if (MODE == MODE_STEP) {
+                    float xv[32], yv[32];
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        xv[j] = args.x[(size_t)(i0 + j) * args.B + b];
+                        yv[j] = args.y[(size_t)(i0 + j) * args.B + b];
+                    }
+                    tc_wait_ld();
+                    uint32_t packed[16];
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        const float G = fmaf(2.0f, __uint_as_float(acc[j]), __ldg(args.hvec + i0 + j));
+                        float xn, yn;
+                        gda_update<GFUN>(xv[j], yv[j], G, args.up, t, (uint32_t)(i0 + j), (uint32_t)b, xn, yn);
+                        args.x[(size_t)(i0 + j) * args.B + b] = xn;
+                        args.y[(size_t)(i0 + j) * args.B + b] = yn;
+                        const uint32_t zb = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(xn - 0.5f));
+                        if (j & 1) packed[j >> 1] |= zb << 16; else packed[j >> 1] = zb;
+                    }
+                    uint4* zdst = reinterpret_cast<uint4*>(args.zt_out + (size_t)b * args.n + i0);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        zdst[q] = make_uint4(packed[4 * q], packed[4 * q + 1], packed[4 * q + 2], packed[4 * q + 3]);
+                } else if (MODE == MODE_GRAD) {
+                    tc_wait_ld();
+#pragma unroll
+                    for (int j = 0; j < 32; ++j)
+                        args.gout[(size_t)(i0 + j) * args.B + b] = fmaf(2.0f, __uint_as_float(acc[j]), __ldg(args.hvec + i0 + j));
+                } else {
+                    float xv[32];
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) xv[j] = args.x[(size_t)(i0 + j) * args.B + b];
+                    tc_wait_ld();
+#pragma unroll
+                    for (int j = 0; j < 32; ++j)                                  // x_hat_i ((Q_off x_hat)_i + c'_i), fp32 row sums
+                        if (xv[j] > 0.5f) score += (double)__uint_as_float(acc[j]) + (double)__ldg(args.cprime + i0 + j);
+                }
+            }
+            if (MODE == MODE_SCORE) args.partial[(size_t)(n_blk * 2 + half) * args.B + b] = score;
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar(as));                           // 8 warps -> accumulator stage free
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    }
+}
+
+// fp32 X [n][B] -> bf16 operand [B][n]: centred (x - 1/2) for the step GEMM, or x_hat = [x > 1/2] for scoring
+template <int HAT>
+__global__ void __launch_bounds__(256)
+make_operand_kernel(int n, int B, const float* __restrict__ x, __nv_bfloat16* __restrict__ zt) {
+    __shared__ float tile[32][33];
+    const int i0 = blockIdx.x * 32, b0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int r = ty; r < 32; r += 8) tile[r][tx] = x[(size_t)(i0 + r) * B + b0 + tx];
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        const float v = tile[tx][r];
+        zt[(size_t)(b0 + r) * n + i0 + tx] = __float2bfloat16_rn(HAT ? (v > 0.5f ? 1.0f : 0.0f) : v - 0.5f);
+    }
+}
+
+// ---- host side ---------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+gda_status get_encoder(EncodeTiledFn* fn) {
+    static EncodeTiledFn cached = nullptr;
+    if (!cached) {
+        void* sym = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        GDA_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &q));
+        if (q != cudaDriverEntryPointSuccess || !sym) {
+            gda_set_error("cuTensorMapEncodeTiled is not available from this driver");
+            return GDA_ERR_CUDA;
+        }
+        cached = reinterpret_cast<EncodeTiledFn>(sym);
+    }
+    *fn = cached;
+    return GDA_OK;
+}
+
+// bf16 row-major [rows][cols] (cols contiguous = K), box = box_rows x 64 elements, 128-byte swizzle
+gda_status make_tmap(CUtensorMap* map, const void* base, uint64_t rows, uint64_t cols, uint32_t box_rows) {
+    EncodeTiledFn enc;
+    GDA_TRY(get_encoder(&enc));
+    const cuuint64_t dims[2] = {cols, rows};
+    const cuuint64_t strides[1] = {cols * sizeof(__nv_bfloat16)};
+    const cuuint32_t box[2] = {(cuuint32_t)BK, box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { gda_set_error("cuTensorMapEncodeTiled failed with CUresult %d", (int)r); return GDA_ERR_CUDA; }
+    return GDA_OK;
+}
+
+struct DenseHost {
+    CUtensorMap tmap_q;
+    CUtensorMap tmap_z[2];
+    const void* z_ptr[2] = {nullptr, nullptr};
+    int32_t z_B = 0;
+    bool attr_set = false;
+};
+
+template <int MODE, int GFUN>
+gda_status launch_gemm(gda_problem* p, const CUtensorMap& ta, const DenseArgs& a, cudaStream_t s) {
+    DenseHost* h = static_cast<DenseHost*>(p->tmap_Q);
+    auto kern = dense_gemm_kernel<MODE, GFUN>;
+    static bool configured = false;
+    if (!configured) {
+        GDA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        configured = true;
+    }
+    const int tiles = (a.B / BM) * (a.n / BN);
+    const int grid = tiles < p->num_sms ? tiles : p->num_sms;
+    kern<<<grid, NUM_THREADS, SMEM_BYTES, s>>>(ta, h->tmap_q, a);
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status z_maps(gda_problem* p, int32_t B, const __nv_bfloat16* zt, const CUtensorMap** out) {
+    DenseHost* h = static_cast<DenseHost*>(p->tmap_Q);
+    for (int k = 0; k < 2; ++k)
+        if (h->z_ptr[k] == zt && h->z_B == B) { *out = &h->tmap_z[k]; return GDA_OK; }
+    if (h->z_B != B) { h->z_ptr[0] = h->z_ptr[1] = nullptr; h->z_B = B; }
+    const int k = h->z_ptr[0] == nullptr ? 0 : 1;
+    GDA_TRY(make_tmap(&h->tmap_z[k], zt, (uint64_t)B, (uint64_t)p->n, BM));
+    h->z_ptr[k] = zt;
+    *out = &h->tmap_z[k];
+    return GDA_OK;
+}
+
+}  // namespace
+
+gda_status dense_prepare(gda_problem* p, const float* Q, const float* c) {
+    const int n = p->n;
+    if (n % BN != 0) { gda_set_error("dense path: n must be a multiple of %d (got %d)", BN, n); return GDA_ERR_UNSUPPORTED; }
+    std::vector<__nv_bfloat16> qb((size_t)n * n);
+    std::vector<float> hvec(n), cp(n);
+    for (int i = 0; i < n; ++i) {
+        double rs = 0.0;
+        for (int j = 0; j < n; ++j) {
+            const __nv_bfloat16 v = __float2bfloat16_rn(j == i ? 0.0f : Q[(size_t)i * n + j]);
+            qb[(size_t)i * n + j] = v;
+            rs += (double)__bfloat162float(v);
+        }
+        cp[i] = (c ? c[i] : 0.0f) + Q[(size_t)i * n + i];                // fold the diagonal (reading R1)
+        hvec[i] = (float)(rs + (double)cp[i]);                          // Q_off 1 + c'
+    }
+    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_Qbf, qb.size() * sizeof(__nv_bfloat16)));
+    GDA_CUDA_TRY(cudaMemcpy(p->d_Qbf, qb.data(), qb.size() * sizeof(__nv_bfloat16), cudaMemcpyHostToDevice));
+    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_rowsum, n * sizeof(float)));
+    GDA_CUDA_TRY(cudaMemcpy(p->d_rowsum, hvec.data(), n * sizeof(float), cudaMemcpyHostToDevice));
+    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_cprime, n * sizeof(float)));
+    GDA_CUDA_TRY(cudaMemcpy(p->d_cprime, cp.data(), n * sizeof(float), cudaMemcpyHostToDevice));
+    DenseHost* h = new DenseHost();
+    p->tmap_Q = h;
+    return make_tmap(&h->tmap_q, p->d_Qbf, (uint64_t)n, (uint64_t)n, BN);
+}
+
+void dense_release(gda_problem* p) {
+    cudaFree(p->d_Qbf); cudaFree(p->d_rowsum);
+    p->d_Qbf = nullptr; p->d_rowsum = nullptr;
+    delete static_cast<DenseHost*>(p->tmap_Q);
+    p->tmap_Q = nullptr;
+}
+
+gda_status dense_make_operand(gda_problem* p, int32_t B, const float* x, __nv_bfloat16* zt, int hat, cudaStream_t s,
+                              int64_t* launches) {
+    dim3 grid((unsigned)(p->n / 32), (unsigned)(B / 32));
+    if (hat) make_operand_kernel<1><<<grid, 256, 0, s>>>(p->n, B, x, zt);
+    else make_operand_kernel<0><<<grid, 256, 0, s>>>(p->n, B, x, zt);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status dense_step(gda_problem* p, int32_t B, float* x, float* y, const __nv_bfloat16* zt_in, __nv_bfloat16* zt_out,
+                      const UpdParams& up, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+    const CUtensorMap* ta;
+    GDA_TRY(z_maps(p, B, zt_in, &ta));
+    DenseArgs a{};
+    a.n = p->n; a.B = B; a.x = x; a.y = y; a.zt_out = zt_out; a.hvec = p->d_rowsum; a.cprime = p->d_cprime;
+    a.up = up; a.st = st; a.t_off = t_off;
+    if (launches) ++*launches;
+    if (up.gfun == GDA_G_QUADRATIC) return launch_gemm<MODE_STEP, GDA_G_QUADRATIC>(p, *ta, a, s);
+    return launch_gemm<MODE_STEP, GDA_G_ENTROPY>(p, *ta, a, s);
+}
+
+// gda_grad: operand from x (centred), GEMM, G written out.  Uses zt[0] of the workspace as scratch.
+gda_status dense_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s) {
+    Workspace& ws = p->ws;
+    ws.has_state = false;                                               // zt[0] is clobbered
+    GDA_TRY(dense_make_operand(p, B, x, ws.zt[0], 0, s, nullptr));
+    const CUtensorMap* ta;
+    GDA_TRY(z_maps(p, B, ws.zt[0], &ta));
+    DenseArgs a{};
+    a.n = p->n; a.B = B; a.hvec = p->d_rowsum; a.cprime = p->d_cprime; a.gout = G;
+    return launch_gemm<MODE_GRAD, GDA_G_QUADRATIC>(p, *ta, a, s);
+}
+
+int32_t dense_num_partials(const gda_problem* p, int32_t) { return p->n / 128; }
+
+// S5: x_hat operand (exact in bf16), GEMM, per-thread column sums.  Scratch: the zt buffer NOT holding the current operand.
+gda_status dense_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
+                                cudaStream_t s, int64_t* launches) {
+    Workspace& ws = p->ws;
+    __nv_bfloat16* scratch = ws.zt[ws.score_scratch];
+    GDA_TRY(dense_make_operand(p, B, x, scratch, 1, s, launches));
+    const CUtensorMap* ta;
+    GDA_TRY(z_maps(p, B, scratch, &ta));
+    DenseArgs a{};
+    a.n = p->n; a.B = B; a.x = const_cast<float*>(x); a.hvec = p->d_rowsum; a.cprime = p->d_cprime;
+    a.partial = static_cast<double*>(partial);
+    *n_part = dense_num_partials(p, B);
+    if (launches) ++*launches;
+    return launch_gemm<MODE_SCORE, GDA_G_QUADRATIC>(p, *ta, a, s);
+}

@@ -68,6 +68,7 @@ struct Workspace {
     int32_t trace_cap = 0;
     // dense path
     __nv_bfloat16* zt[2] = {nullptr, nullptr};  // [B][n] bf16 GEMM operand (centred x - 1/2, or x_hat)
+    int32_t score_scratch = 1;                  // which zt buffer dense scoring may clobber (the one not holding z^t)
     float* gtmp = nullptr;                      // [n][B] gradient scratch for gda_grad on the dense path
     // host staging for gda_run_host
     float* h_x0 = nullptr; float* h_l0 = nullptr;

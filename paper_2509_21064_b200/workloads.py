@@ -208,7 +208,7 @@ def config(idx: int, B: Optional[int] = None, n_scale: float = 1.0) -> Workload:
                         Hyper(6.0, 0.025, 0.025, 1e-4, 0, 1e-6, 10000, 100, 103), 1103,
                         "Max-Cut G(20000,40000), weights +-1")
     if idx == 4:
-        n = max(128, int(round(4096 * n_scale)) // 128 * 128)
+        n = max(256, int(round(4096 * n_scale)) // 256 * 256)
         P = dense_qubo(n, 104)
         s = 2.0 * np.sqrt(n)                      # spectral scale of the N(0,1) matrix (reading R7)
         lam = 1.75 * s

@@ -72,13 +72,13 @@ def test_invalid_arguments_are_rejected_before_the_device(L):
         api.Problem.create_maxsat(S.n, S.m, cptr, S.lit, S.w)
     assert e.value.status == 1
     Q = np.zeros((100, 100), dtype=np.float32)
-    with pytest.raises(api.GdaError) as e:                       # dense n must be a multiple of 128
+    with pytest.raises(api.GdaError) as e:                       # dense n must be a multiple of 256
         api.Problem.create_qubo_dense(100, Q, None)
     assert e.value.status == 4
-    Q = np.zeros((128, 128), dtype=np.float32)
+    Q = np.zeros((256, 256), dtype=np.float32)
     Q[0, 1] = 1.0
     with pytest.raises(api.GdaError) as e:
-        api.Problem.create_qubo_dense(128, Q, None)
+        api.Problem.create_qubo_dense(256, Q, None)
     assert e.value.status == 1
     h = C.c_void_p(123)
     assert L.gda_create_qubo_csr(4, None, None, None, None, C.byref(h)) == 1 and h.value is None   # out set to NULL

@@ -362,3 +362,90 @@ def test_run_arguments_are_validated(api):
     with pytest.raises(api.GdaError):
         P.run(dev(wl.x0_uniform(w.problem.n, 6, 1)), 6.0, api.params_from_hyper(w.hyper))     # B % 4 != 0
     P.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# dense QUBO: tcgen05 GEMM gradient (bf16 operands, fp32 accumulate) -- gradients within 1e-2 (north_star)
+# ------------------------------------------------------------------------------------------------
+TOL_GRAD_BF16 = 1e-2
+
+
+def dense_workloads():
+    return [wl.config(4, B=128, n_scale=0.0625), wl.config(4, B=384, n_scale=0.125), wl.config(4, B=256, n_scale=0.25)]
+
+
+DENSE = dense_workloads()
+
+
+def dense_F_tolerance(Pw, x_bin):
+    """rtol 1e-5 * sum |terms| (fp32 row sums accumulated in fp64)."""
+    xb = x_bin.astype(np.float64)
+    return 1e-5 * (xb.T @ np.abs(Pw.Q.astype(np.float64)) @ xb).diagonal().max() + 1e-3
+
+
+@pytest.mark.parametrize("w", DENSE, ids=lambda w: f"{w.name}_n{w.problem.n}_B{w.B}")
+def test_dense_gradient_and_score(api, oracle, w):
+    OP = oracle_problem(w.problem)
+    P = api.create_from_workload(w.problem)
+    n, B = w.problem.n, w.B
+    rng = np.random.default_rng(6)
+    X = rng.random((n, B), dtype=np.float32)
+    X[:, 0] = (X[:, 0] > 0.5)
+    X[:, 1] = 0.5
+    X[:, 2] = 0.5 + 1e-3 * (rng.random(n, dtype=np.float32) - 0.5)          # near 1/2: the centred operand keeps precision
+    Gref = oracle.grad(OP, X.astype(np.float64))
+    G = P.grad(dev(X)).cpu().numpy()
+    assert grad_rel_err(G, Gref) <= TOL_GRAD_BF16
+    assert np.abs(G[:, 0] - Gref[:, 0]).max() <= 1e-3 * np.abs(Gref[:, 0]).max()   # binary column: z = +-1/2 exact in bf16
+    obj = P.score(dev(X)).cpu().numpy()
+    xh = (X > 0.5).astype(np.uint8)
+    Fref = oracle.F_binary(OP, xh)
+    assert np.abs(obj - Fref).max() <= dense_F_tolerance(w.problem, xh)
+    assert P.info().integral == 0 and P.info().kind == 1
+    P.destroy()
+
+
+@pytest.mark.parametrize("w", DENSE[:2], ids=lambda w: f"{w.name}_n{w.problem.n}_B{w.B}")
+def test_dense_teacher_forced_steps(api, oracle, w):
+    OP = oracle_problem(w.problem)
+    P = api.create_from_workload(w.problem)
+    n, B, h = w.problem.n, w.B, w.hyper
+    x = dev(wl.x0_uniform(n, B, w.x0_seed))
+    lam = torch.full((n, B), h.lambda0, dtype=torch.float32, device="cuda")
+    t = 0
+    for hop in (0, 1, 50, 301):
+        if hop:
+            r = P.run(x, lam, api.params_from_hyper(h, iters=hop, eval_every=50, t0=t), want_final=True)
+            x, lam, t = r["x"], r["lam"], t + hop
+        r1 = P.run(x, lam, api.params_from_hyper(h, iters=1, eval_every=1, t0=t, delta=0.0), want_final=True)
+        xp, lp = x.cpu().numpy(), lam.cpu().numpy()
+        ref = oracle.run(OP, xp, lp, **okw(h, iters=1, eval_every=1, t0=t, delta=0.0))
+        Gref = oracle.grad(OP, xp.astype(np.float64))
+        # x+ = clip(x - alpha (G + y g')): a gradient error of 1e-2 ||G||inf moves x+ by at most alpha * that
+        tol_x = f32(h.alpha) * TOL_GRAD_BF16 * np.maximum(np.abs(Gref).max(axis=0), 1.0) + TOL_STEP
+        assert (np.abs(r1["x"].cpu().numpy() - ref["x"]).max(axis=0) <= tol_x).all(), t
+        yg = r1["lam"].cpu().numpy()
+        assert (np.abs(yg - ref["y"]) / np.maximum(1.0, np.abs(ref["y"]))).max() <= TOL_STEP     # dual step has no GEMM in it
+    P.destroy()
+
+
+@pytest.mark.parametrize("w", DENSE[:2], ids=lambda w: f"{w.name}_n{w.problem.n}_B{w.B}")
+def test_dense_full_run(api, oracle, w):
+    OP = oracle_problem(w.problem)
+    P = api.create_from_workload(w.problem)
+    n, B, h = w.problem.n, w.B, w.hyper
+    X0 = wl.x0_uniform(n, B, w.x0_seed)
+    iters = 1500
+    r = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=iters), want_final=True, trace_cap=32)
+    x_bin, obj = r["x_bin"].cpu().numpy(), r["obj"].cpu().numpy()
+    assert set(np.unique(x_bin)) <= {0, 1}
+    Fref = oracle.F_binary(OP, x_bin)
+    assert np.abs(obj - Fref).max() <= dense_F_tolerance(w.problem, x_bin)          # (a), fp64 with rtol on the dense path
+    best = int(r["best_restart"].item())
+    assert obj[best] == obj.min()
+    nb = min(B, 32)
+    ref = oracle.run(OP, X0[:, :nb].copy(), f32(h.lambda0), nthreads=8, **okw(h, iters=iters))
+    assert_statistics_close(obj[:nb], ref["obj"])
+    rnd = oracle.F_binary(OP, (np.random.default_rng(0).random((n, 64)) < 0.5).astype(np.uint8))
+    assert obj.max() < rnd.min()
+    P.destroy()
