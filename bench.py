@@ -202,7 +202,7 @@ def run_reference(args, w: wl.Workload):
 def run_ours(args, w: wl.Workload):
     import torch
     import torch.distributed as dist
-    from paper_2509_21064_b200 import api, build
+    from paper_2509_21064_b200 import api, build, multirank
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -223,7 +223,7 @@ def run_ours(args, w: wl.Workload):
     h, B, n = w.hyper, w.B, w.problem.n
     K, W = args.steps, max(args.warmup, 3)
     P = api.create_from_workload(w.problem)
-    x0_host = torch.from_numpy(wl.x0_uniform(n, B, w.x0_seed + 7919 * rank)).pin_memory()   # each rank: its own restarts
+    x0_host = torch.from_numpy(wl.x0_uniform(n, B, multirank.rank_x0_seed(w.x0_seed, rank))).pin_memory()   # each rank: its own restarts
     x0 = x0_host.to(dev, non_blocking=True)
     stream = torch.cuda.Stream(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -301,19 +301,10 @@ def run_ours(args, w: wl.Workload):
         t_e2e = max(e0.elapsed_time(e1) / 1e3, 0.0)
         t_e2e_wall = time.perf_counter() - w0
 
-    def max_over_ranks(v):
-        if world == 1:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
-    t_steps, t_whole, t_e2e, t_eval = map(max_over_ranks, (t_steps, t_whole, max(t_e2e, t_e2e_wall), t_eval))
-    best = float(out["obj"].min().item())
-    if world > 1:
-        tb = torch.tensor([best], dtype=torch.float64, device=dev)
-        dist.all_reduce(tb, op=dist.ReduceOp.MIN)           # the only exchange: arg-best across ranks
-        best = float(tb.item())
+    t_steps, t_whole, t_e2e, t_eval = (multirank.max_over_ranks(v, world, dev)
+                                       for v in (t_steps, t_whole, max(t_e2e, t_e2e_wall), t_eval))
+    best, best_rank, best_restart = multirank.combine_best(float(out["obj"].min().item()),
+                                                            int(out["best_restart"].item()), rank, world, dev)
 
     iters_per_step = h.eval_every
     units = world * B * iters_per_step * K
@@ -357,7 +348,7 @@ def run_ours(args, w: wl.Workload):
                          "algorithmic_bytes_per_launch": work["bytes"], "algorithmic_flops_per_launch": work["flops"],
                          "eval_us": t_eval * 1e6},
             "clocks": clocks,
-            "best_objective": best, "best_objective_flushed_run": best_flushed,
+            "best_objective": best, "best_rank": best_rank, "best_restart": best_restart, "best_objective_flushed_run": best_flushed,
         }
         if cpu:
             line["cpu_baseline"] = cpu
