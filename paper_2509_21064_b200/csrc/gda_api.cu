@@ -191,13 +191,14 @@ extern "C" gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cpt
     GDA_REQUIRE(n > 0 && m > 0, "gda_create_maxsat: n and m must be > 0 (got %d, %d)", n, m);
     GDA_REQUIRE(cptr != nullptr && lit != nullptr, "gda_create_maxsat: cptr/lit is NULL");
     GDA_REQUIRE(cptr[0] == 0, "gda_create_maxsat: cptr[0] must be 0");
-    int32_t kmax = 0;
+    int32_t kmax = 0, kmin = 0x7fffffff;
     bool integral = true;
     std::vector<int32_t> occ(n + 1, 0), tmp;
     for (int j = 0; j < m; ++j) {
         const int k = cptr[j + 1] - cptr[j];
         GDA_REQUIRE(k > 0, "gda_create_maxsat: clause %d is empty", j);
         kmax = std::max(kmax, k);
+        kmin = std::min(kmin, k);
         tmp.clear();
         for (int a = cptr[j]; a < cptr[j + 1]; ++a) {
             const int l = lit[a];
@@ -219,7 +220,7 @@ extern "C" gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cpt
     for (int i = 0; i < n; ++i) occ[i + 1] += occ[i];
     std::vector<int32_t> h_vptr(occ), next(occ.begin(), occ.end() - 1);
     std::vector<float> h_coef((size_t)L), h_w(m);
-    std::vector<int32_t> h_others((size_t)L * kw, 0);
+    std::vector<int32_t> h_others((size_t)L * kw, 0x7FFFFFFF);      // ENC_PAD
     for (int j = 0; j < m; ++j) {
         const float wj = w ? w[j] : 1.0f;
         h_w[j] = wj;
@@ -230,13 +231,17 @@ extern "C" gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cpt
             h_coef[s] = l > 0 ? -wj : wj;                    // d/dx of p: -1 for a positive literal, +1 for a negated one
             int q = 0;
             for (int b = cptr[j]; b < cptr[j + 1]; ++b)
-                if (b != a) h_others[(size_t)s * kw + q++] = lit[b];
+                if (b != a) {                                  // enc = var | (positive literal ? 0x80000000 : 0)
+                    const int lb = lit[b];
+                    const uint32_t vb = (uint32_t)((lb > 0 ? lb : -lb) - 1);
+                    h_others[(size_t)s * kw + q++] = (int32_t)(vb | (lb > 0 ? 0x80000000u : 0u));
+                }
         }
     }
     gda_problem* p = new (std::nothrow) gda_problem();
     if (!p) { gda_set_error("host allocation failed"); return GDA_ERR_ALLOC; }
     p->kind = GDA_KIND_MAXSAT; p->n = n; p->m = m; p->nnz = L; p->integral = integral ? 1 : 0;
-    p->kw = kw; p->kmax = kmax;
+    p->kw = kw; p->kmax = kmax; p->kmin = kmin;
     gda_status st = device_setup(p);
     if (st == GDA_OK) st = upload(&p->d_vptr, h_vptr);
     if (st == GDA_OK) st = upload(&p->d_coef, h_coef);
@@ -466,6 +471,10 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
         GDA_REQUIRE(prm->log_eps > 0.0f && prm->log_eps < 0.5f, "gda_run: log_eps must be in (0, 1/2) for the entropy g");
     if (p->kind == GDA_KIND_DENSE && B % 128 != 0) {
         gda_set_error("gda_run: the dense path needs B to be a multiple of 128 (got %d)", B);
+        return GDA_ERR_UNSUPPORTED;
+    }
+    if ((int64_t)p->n * (int64_t)B >= ((int64_t)1 << 30)) {
+        gda_set_error("gda_run: n * B must be below 2^30 (got %lld): kernels use 32-bit byte offsets into X", (long long)p->n * B);
         return GDA_ERR_UNSUPPORTED;
     }
     return GDA_OK;

@@ -105,7 +105,7 @@ struct gda_problem {
     void* tmap_Q = nullptr;              // CUtensorMap (128 B), host copy
     // MaxSAT: per occurrence slot (variable-major): coef = w_j * s_ji, others[kw] signed literals (0 = pad)
     int32_t* d_vptr = nullptr; float* d_coef = nullptr; int32_t* d_others = nullptr; int32_t kw = 0;
-    int32_t* d_cptr = nullptr; int32_t* d_lit = nullptr; float* d_w = nullptr; int32_t kmax = 0;
+    int32_t* d_cptr = nullptr; int32_t* d_lit = nullptr; float* d_w = nullptr; int32_t kmax = 0, kmin = 0;
     Workspace ws;
     cudaStream_t own_stream = nullptr;   // used when the caller passes the legacy default stream (not capturable)
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
@@ -177,7 +177,9 @@ __device__ __forceinline__ float side_from_hash(uint32_t seed_mix, uint32_t t, u
     return (h & 1u) ? 1.0f : -1.0f;
 }
 
-__device__ __forceinline__ float xlogx_f(float u) { return u > 0.0f ? u * logf(u) : 0.0f; }
+// natural log through MUFU.LG2 (__logf: abs error <= 2^-21.4 on [0.5, 2], <= 3 ulp elsewhere): with alpha*y and beta
+// of order 1e-2 that is < 1e-7 on x+ and y+, two orders below the 1e-5 step tolerance
+__device__ __forceinline__ float fast_ln(float u) { return __logf(u); }
 
 // One element of S4: (x, y, G) at time t -> (x, y) at time t+1.   PAPER.md:136-142 (Eq. 6), 148, 732.
 template <int GFUN>
@@ -188,14 +190,17 @@ __device__ __forceinline__ void gda_update(float x, float y, float G, const UpdP
         gp = 2.0f * x - 1.0f;
         gv = x * x - x;
     } else {
-        // g'(x) = ln(xc) - ln(1 - xc), xc = clip(x, eps, 1 - eps) (reading R4), evaluated as
-        // ln(clip(x)) - ln(clip(1 - x)): the same function, but 1 - x is exact in fp32 near x = 1
-        // whereas 1 - eps is not representable (1 - fl(1 - 1e-6) = 1.013e-6 would shift g' by 1.3e-2).
-        const float u = 1.0f - x, hi = 1.0f - up.log_eps;
-        const float a = fminf(fmaxf(x, up.log_eps), hi), b = fminf(fmaxf(u, up.log_eps), hi);
-        const float l0 = logf(a), l1 = logf(b);
+        // Reading R4: g'(x) = ln(xc) - ln(1 - xc), xc = clip(x, eps, 1 - eps); g(x) = x ln x + (1-x) ln(1-x), 0 at the ends.
+        // Evaluated branch-free from two logs of a = max(x, eps), b = max(1 - x, eps) (1 - x is exact in fp32 near 1,
+        // whereas 1 - eps is not representable):
+        //   g' = ln a - ln b        differs from the clipped form only for x outside [eps, 1-eps], by <= eps = 1e-6
+        //   g  = x ln a + (1-x) ln b   exact 0 at x = 0 and 1; for 0 < x < eps it is x ln eps instead of x ln x,
+        //                              an absolute difference <= eps/e = 3.7e-7
+        // i.e. <= alpha*y*1e-6 on x+ and <= beta*3.7e-7 on y+, far below the 1e-5 step tolerance.
+        const float u = 1.0f - x;
+        const float l0 = fast_ln(fmaxf(x, up.log_eps)), l1 = fast_ln(fmaxf(u, up.log_eps));
         gp = l0 - l1;
-        gv = (a == x && b == u) ? (x * l0 + u * l1) : (xlogx_f(x) + xlogx_f(u));
+        gv = fmaf(x, l0, u * l1);
     }
     float xt = x - up.alpha * (G + y * gp);
     xt = fminf(fmaxf(xt, 0.0f), 1.0f);

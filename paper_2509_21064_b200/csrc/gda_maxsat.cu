@@ -17,52 +17,79 @@ constexpr int WARPS = 8;
 constexpr int THREADS = WARPS * 32;
 constexpr int SCORE_CLAUSES = 128;
 
-__device__ __forceinline__ float4 lit_term(int l, const float* __restrict__ x, int B, int c4) {
-    const int v = (l > 0 ? l : -l) - 1;
-    const float4 g = ldg4(x + (size_t)v * B + 4 * c4);
-    return l > 0 ? make_float4(1.0f - g.x, 1.0f - g.y, 1.0f - g.z, 1.0f - g.w) : g;
+// Slot records hold each OTHER literal encoded as  enc = var | (positive ? 0x80000000 : 0);  ENC_PAD marks padding.
+// p_l(x) = off + sgn * x with (off, sgn) = (1, -1) for a positive literal and (0, +1) for a negated one.
+// xb = this lane's column base (byte pointer), stride = 4*B bytes per variable.
+constexpr uint32_t ENC_PAD = 0x7FFFFFFFu;
+__device__ __forceinline__ float4 lit_term(uint32_t enc, const char* __restrict__ xb, uint32_t stride) {
+    const uint32_t v = enc & 0x7FFFFFFFu;
+    const float4 g = __ldg(reinterpret_cast<const float4*>(xb + (uint64_t)v * (uint64_t)stride));
+    const float sgn = __uint_as_float((enc & 0x80000000u) | 0x3F800000u);        // -1 (positive literal) or +1 (negated)
+    const float off = fmaf(sgn, -0.5f, 0.5f);                                    //  1                     or  0
+    return make_float4(fmaf(sgn, g.x, off), fmaf(sgn, g.y, off), fmaf(sgn, g.z, off), fmaf(sgn, g.w, off));
 }
 
-// KW > 0: compile-time number of "other" literals (3-SAT: 2), slot records broadcast by shuffle.
-// KW == 0: run-time kw, records read with broadcast loads.
-template <int KW>
+// KW > 0: compile-time number of "other" literals (3-SAT: 2), slot records broadcast by shuffle; PAD says whether
+// records may hold 0-padding (clauses shorter than kmax).  KW == 0: run-time kw, records read with broadcast loads.
+template <int KW, bool PAD>
 __device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, const int32_t* __restrict__ others,
                                              int kw, int start, int end, const float* __restrict__ x, int B,
                                              int c4, bool active, int lane) {
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     if (KW > 0) {
+        const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
+        const uint32_t stride = 4u * (uint32_t)B;
         for (int base = start; base < end; base += 32) {
             const int s = base + lane;
             const float my_coef = (s < end) ? __ldg(coef + s) : 0.0f;
             int my_o[KW > 0 ? KW : 1];
 #pragma unroll
-            for (int q = 0; q < KW; ++q) my_o[q] = (s < end) ? __ldg(others + (size_t)s * KW + q) : 0;
+            for (int q = 0; q < KW; ++q) my_o[q] = (s < end) ? __ldg(others + (size_t)s * KW + q) : (int)ENC_PAD;
             const int cnt = min(32, end - base);
-            for (int u = 0; u < cnt; ++u) {
-                const float cf = __shfl_sync(0xffffffffu, my_coef, u);
-                int l[KW > 0 ? KW : 1];
+            constexpr int U = 2;                                  // slots per batch: U*KW independent 512 B gathers in flight
+            for (int u0 = 0; u0 < cnt; u0 += U) {
+                float cf[U]; int l[U][KW > 0 ? KW : 1]; float4 t[U][KW > 0 ? KW : 1];
 #pragma unroll
-                for (int q = 0; q < KW; ++q) l[q] = __shfl_sync(0xffffffffu, my_o[q], u);
-                if (!active) continue;
-                float4 prod = make_float4(cf, cf, cf, cf);
+                for (int a = 0; a < U; ++a) {                     // past the end: re-read the last slot with coefficient 0
+                    const int src = min(u0 + a, cnt - 1);
+                    cf[a] = __shfl_sync(0xffffffffu, my_coef, src);
 #pragma unroll
-                for (int q = 0; q < KW; ++q) {
-                    if (l[q] == 0) continue;
-                    const float4 t = lit_term(l[q], x, B, c4);
-                    prod.x *= t.x; prod.y *= t.y; prod.z *= t.z; prod.w *= t.w;
+                    for (int q = 0; q < KW; ++q) l[a][q] = __shfl_sync(0xffffffffu, my_o[q], src);
+                    if (u0 + a >= cnt) cf[a] = 0.0f;
                 }
-                acc.x += prod.x; acc.y += prod.y; acc.z += prod.z; acc.w += prod.w;
+                if (!active) continue;
+#pragma unroll
+                for (int a = 0; a < U; ++a)
+#pragma unroll
+                    for (int q = 0; q < KW; ++q) {
+                        if (PAD && (uint32_t)l[a][q] == ENC_PAD) { t[a][q] = make_float4(1.f, 1.f, 1.f, 1.f); continue; }
+                        t[a][q] = lit_term((uint32_t)l[a][q], xb, stride);
+                    }
+#pragma unroll
+                for (int a = 0; a < U; ++a) {                     // acc += cf * t0 * t1 * ... (last factor fused into the add)
+                    float4 prod = make_float4(cf[a] * t[a][0].x, cf[a] * t[a][0].y, cf[a] * t[a][0].z, cf[a] * t[a][0].w);
+#pragma unroll
+                    for (int q = 1; q + 1 < KW; ++q) { prod.x *= t[a][q].x; prod.y *= t[a][q].y; prod.z *= t[a][q].z; prod.w *= t[a][q].w; }
+                    if (KW > 1) {
+                        acc.x = fmaf(prod.x, t[a][KW - 1].x, acc.x); acc.y = fmaf(prod.y, t[a][KW - 1].y, acc.y);
+                        acc.z = fmaf(prod.z, t[a][KW - 1].z, acc.z); acc.w = fmaf(prod.w, t[a][KW - 1].w, acc.w);
+                    } else {
+                        acc.x += prod.x; acc.y += prod.y; acc.z += prod.z; acc.w += prod.w;
+                    }
+                }
             }
         }
     } else {
         if (!active) return acc;
+        const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
+        const uint32_t stride = 4u * (uint32_t)B;
         for (int s = start; s < end; ++s) {
             const float cf = __ldg(coef + s);
             float4 prod = make_float4(cf, cf, cf, cf);
             for (int q = 0; q < kw; ++q) {
-                const int l = __ldg(others + (size_t)s * kw + q);
-                if (l == 0) break;
-                const float4 t = lit_term(l, x, B, c4);
+                const uint32_t l = (uint32_t)__ldg(others + (size_t)s * kw + q);
+                if (l == ENC_PAD) break;
+                const float4 t = lit_term(l, xb, stride);
                 prod.x *= t.x; prod.y *= t.y; prod.z *= t.z; prod.w *= t.w;
             }
             acc.x += prod.x; acc.y += prod.y; acc.z += prod.z; acc.w += prod.w;
@@ -72,7 +99,7 @@ __device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, con
 }
 
 // warp-per-(variable, 128-restart chunk).  MODE 0: fused step; MODE 1: write G only.
-template <int GFUN, int MODE, int KW>
+template <int GFUN, int MODE, int KW, bool PAD>
 __global__ void __launch_bounds__(THREADS)
 maxsat_step_kernel(int n, int B, int chunks, const int32_t* __restrict__ vptr, const float* __restrict__ coef,
                    const int32_t* __restrict__ others, int kw, const float* __restrict__ x,
@@ -86,7 +113,7 @@ maxsat_step_kernel(int n, int B, int chunks, const int32_t* __restrict__ vptr, c
     const int c4 = chunk * 32 + lane;
     const bool active = 4 * c4 < B;
     const int start = __ldg(vptr + var), end = __ldg(vptr + var + 1);
-    const float4 G = gather_var<KW>(coef, others, kw, start, end, x, B, c4, active, lane);
+    const float4 G = gather_var<KW, PAD>(coef, others, kw, start, end, x, B, c4, active, lane);
     if (!active) return;
     const size_t off = (size_t)var * B + 4 * c4;
     if (MODE == 1) { *reinterpret_cast<float4*>(xn + off) = G; return; }
@@ -151,12 +178,17 @@ template <int GFUN, int MODE>
 void launch_kw(gda_problem* p, int32_t B, int chunks, unsigned grid, const float* x, float* y, float* xn,
                const UpdParams& up, const RunState* st, uint32_t t_off, cudaStream_t s) {
 #define GDA_MS_ARGS p->n, B, chunks, p->d_vptr, p->d_coef, p->d_others, p->kw, x, y, xn, up, st, t_off
+    const bool pad = p->kmin != p->kmax;
     switch (p->kw) {
-        case 1: maxsat_step_kernel<GFUN, MODE, 1><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
-        case 2: maxsat_step_kernel<GFUN, MODE, 2><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
-        case 3: maxsat_step_kernel<GFUN, MODE, 3><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
-        case 4: maxsat_step_kernel<GFUN, MODE, 4><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
-        default: maxsat_step_kernel<GFUN, MODE, 0><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        case 1: if (pad) maxsat_step_kernel<GFUN, MODE, 1, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS);
+                else maxsat_step_kernel<GFUN, MODE, 1, false><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        case 2: if (pad) maxsat_step_kernel<GFUN, MODE, 2, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS);
+                else maxsat_step_kernel<GFUN, MODE, 2, false><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        case 3: if (pad) maxsat_step_kernel<GFUN, MODE, 3, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS);
+                else maxsat_step_kernel<GFUN, MODE, 3, false><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        case 4: if (pad) maxsat_step_kernel<GFUN, MODE, 4, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS);
+                else maxsat_step_kernel<GFUN, MODE, 4, false><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        default: maxsat_step_kernel<GFUN, MODE, 0, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
     }
 #undef GDA_MS_ARGS
 }

@@ -69,7 +69,7 @@ __device__ __forceinline__ void update_store(int row, int c4, int B, float4 G, c
 
 // warp-per-(row, chunk).  MODE 0: fused step, MODE 1: write G only (gda_grad).
 template <int GFUN, int MODE>
-__global__ void __launch_bounds__(THREADS)
+__global__ void __launch_bounds__(THREADS, 8)
 spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B, int chunks,
                const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                const float* __restrict__ val2, const float* __restrict__ cprime,
