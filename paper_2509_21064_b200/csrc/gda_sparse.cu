@@ -69,23 +69,23 @@ __device__ __forceinline__ void update_store(int row, int c4, int B, float4 G, c
 
 // warp-per-(row, chunk).  MODE 0: fused step, MODE 1: write G only (gda_grad).
 template <int GFUN, int MODE>
-__global__ void __launch_bounds__(THREADS, 8)
+__global__ void __launch_bounds__(THREADS)
 spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B, int chunks,
                const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                const float* __restrict__ val2, const float* __restrict__ cprime,
                const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
                UpdParams up, const RunState* __restrict__ st, uint32_t t_off) {
     const int lane = threadIdx.x & 31;
-    const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
-    if (item >= (long long)n_rows * chunks) return;
-    const int ridx = (int)(item / chunks);
-    const int chunk = (int)(item - (long long)ridx * chunks);
-    const int row = row_list ? __ldg(row_list + ridx) : ridx;
+    const uint32_t item = blockIdx.x * WARPS + (threadIdx.x >> 5);           // n * chunks < 2^30 (checked by gda_run)
+    const bool in_range = item < (uint32_t)n_rows * (uint32_t)chunks;
+    const uint32_t ridx = in_range ? item / (uint32_t)chunks : 0u;
+    const int chunk = (int)(item - ridx * (uint32_t)chunks);
+    const int row = row_list ? __ldg(row_list + ridx) : (int)ridx;
     const int c4 = chunk * 32 + lane;
-    const bool active = 4 * c4 < B;
-    const int start = __ldg(rowptr + row), end = __ldg(rowptr + row + 1);
-    float4 G = gather_row(col, val2, start, end, x, B, c4, active, lane);
+    const bool active = in_range && 4 * c4 < B;
+    const int start = __ldg(rowptr + row), end = in_range ? __ldg(rowptr + row + 1) : start;
     const float cp = __ldg(cprime + row);
+    float4 G = gather_row(col, val2, start, end, x, B, c4, active, lane);
     G.x += cp; G.y += cp; G.z += cp; G.w += cp;
     if (!active) return;
     if (MODE == 1) { *reinterpret_cast<float4*>(xn + (size_t)row * B + 4 * c4) = G; return; }
