@@ -147,6 +147,25 @@ extern "C" gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, cons
         st = upload(&p->d_heavy_rows, heavy);
         if (st == GDA_OK) st = upload(&p->d_light_rows, light);
     }
+    if (st == GDA_OK && (int64_t)h_col.size() <= 8 * (int64_t)n) {
+        // packed records for rows of degree <= 8 (one 64-byte load replaces rowptr -> col/val): 8 columns then 8
+        // values, zeros dropped, padding = (own row, 0); word 0 = -1 sends the row to the CSR path.
+        std::vector<int32_t> ell((size_t)n * 16);
+        for (int i = 0; i < n; ++i) {
+            int32_t* rec = ell.data() + (size_t)i * 16;
+            const int32_t deg = h_rowptr[i + 1] - h_rowptr[i];
+            for (int q = 0; q < 8; ++q) { rec[q] = i; rec[8 + q] = 0; }
+            if (deg > 8) { rec[0] = -1; continue; }
+            int cnt = 0;
+            for (int k = h_rowptr[i]; k < h_rowptr[i + 1]; ++k) {
+                if (h_val2[k] == 0.0f) continue;
+                rec[cnt] = h_col[k];
+                std::memcpy(&rec[8 + cnt], &h_val2[k], 4);
+                ++cnt;
+            }
+        }
+        st = upload(&p->d_ell, ell);
+    }
     if (st != GDA_OK) { gda_destroy(p); return st; }
     *out = p;
     return GDA_OK;
@@ -282,7 +301,7 @@ extern "C" void gda_destroy(gda_problem* p) {
     cudaDeviceSynchronize();
     free_workspace(p);
     cudaFree(p->d_rowptr); cudaFree(p->d_col); cudaFree(p->d_val2); cudaFree(p->d_cprime);
-    cudaFree(p->d_heavy_rows); cudaFree(p->d_light_rows);
+    cudaFree(p->d_heavy_rows); cudaFree(p->d_light_rows); cudaFree(p->d_ell);
     cudaFree(p->d_vptr); cudaFree(p->d_coef); cudaFree(p->d_others); cudaFree(p->d_cptr); cudaFree(p->d_lit); cudaFree(p->d_w);
     dense_release(p);
     if (p->own_stream) cudaStreamDestroy(p->own_stream);

@@ -100,6 +100,7 @@ struct gda_problem {
     int32_t* d_heavy_rows = nullptr; int32_t n_heavy = 0;   // rows handled by the row-split kernel
     int32_t* d_light_rows = nullptr; int32_t n_light = 0;   // nullptr = all rows, in order
     int32_t max_deg = 0;
+    int32_t* d_ell = nullptr;            // [n][16] packed low-degree rows: 8 cols + 8 val2 (see gda_sparse.cu); nullptr = not built
     // dense QUBO: Q_off in bf16 [n][n] (zero diagonal), r0 = Q_off 1 (row sums) for the centred operand
     __nv_bfloat16* d_Qbf = nullptr; float* d_rowsum = nullptr;
     void* tmap_Q = nullptr;              // CUtensorMap (128 B), host copy
@@ -182,9 +183,10 @@ __device__ __forceinline__ float side_from_hash(uint32_t seed_mix, uint32_t t, u
 __device__ __forceinline__ float fast_ln(float u) { return __logf(u); }
 
 // One element of S4: (x, y, G) at time t -> (x, y) at time t+1.   PAPER.md:136-142 (Eq. 6), 148, 732.
+// Split in two so that vector callers can test the (rare) perturbation condition once for several elements:
+// gda_update_nopert is Eq. 6 alone; gda_perturb applies reading R3/R3a to the tentative point.
 template <int GFUN>
-__device__ __forceinline__ void gda_update(float x, float y, float G, const UpdParams& up, uint32_t t,
-                                           uint32_t i, uint32_t b, float& xn, float& yn) {
+__device__ __forceinline__ void gda_update_nopert(float x, float y, float G, const UpdParams& up, float& xt, float& yn) {
     float gp, gv;
     if (GFUN == GDA_G_QUADRATIC) {
         gp = 2.0f * x - 1.0f;
@@ -202,19 +204,51 @@ __device__ __forceinline__ void gda_update(float x, float y, float G, const UpdP
         gp = l0 - l1;
         gv = fmaf(x, l0, u * l1);
     }
-    float xt = x - up.alpha * (G + y * gp);
+    xt = x - up.alpha * (G + y * gp);
     xt = fminf(fmaxf(xt, 0.0f), 1.0f);
     yn = y + up.beta * gv;
-    if (up.delta > 0.0f && fabsf(x - 0.5f) < up.delta && fabsf(xt - 0.5f) < up.delta) {
-        float s;
-        if (xt > 0.5f) s = 1.0f; else if (xt < 0.5f) s = -1.0f;
-        else if (x > 0.5f) s = 1.0f; else if (x < 0.5f) s = -1.0f;
-        else s = side_from_hash(up.seed_mix, t, i, b);
-        xt = 0.5f + up.delta * s;
-        if (fabsf(xt - 0.5f) < up.delta)                       // rounding fell inside: one ulp away from 1/2
-            xt = __int_as_float(__float_as_int(xt) + (s > 0.0f ? 1 : -1));
-        }
+}
+
+__device__ __forceinline__ bool gda_in_band(float x, float xt, float delta) {
+    return fabsf(x - 0.5f) < delta && fabsf(xt - 0.5f) < delta;           // false for delta == 0
+}
+
+__device__ __forceinline__ float gda_perturb(float x, float xt, float delta, uint32_t seed_mix, uint32_t t, uint32_t i, uint32_t b) {
+    float s;
+    if (xt > 0.5f) s = 1.0f; else if (xt < 0.5f) s = -1.0f;
+    else if (x > 0.5f) s = 1.0f; else if (x < 0.5f) s = -1.0f;
+    else s = side_from_hash(seed_mix, t, i, b);
+    xt = 0.5f + delta * s;
+    if (fabsf(xt - 0.5f) < delta)                              // rounding fell inside: one ulp away from 1/2
+        xt = __int_as_float(__float_as_int(xt) + (s > 0.0f ? 1 : -1));
+    return xt;
+}
+
+template <int GFUN>
+__device__ __forceinline__ void gda_update(float x, float y, float G, const UpdParams& up, uint32_t t,
+                                           uint32_t i, uint32_t b, float& xn, float& yn) {
+    float xt;
+    gda_update_nopert<GFUN>(x, y, G, up, xt, yn);
+    if (gda_in_band(x, xt, up.delta)) xt = gda_perturb(x, xt, up.delta, up.seed_mix, t, i, b);
     xn = xt;
+}
+
+// Four consecutive restarts b0..b0+3 of variable i: one test for the rare perturbation branch.
+template <int GFUN>
+__device__ __forceinline__ void gda_update4(const float4& x, const float4& y, const float4& G, const UpdParams& up,
+                                            uint32_t t, uint32_t i, uint32_t b0, float4& xn, float4& yn) {
+    gda_update_nopert<GFUN>(x.x, y.x, G.x, up, xn.x, yn.x);
+    gda_update_nopert<GFUN>(x.y, y.y, G.y, up, xn.y, yn.y);
+    gda_update_nopert<GFUN>(x.z, y.z, G.z, up, xn.z, yn.z);
+    gda_update_nopert<GFUN>(x.w, y.w, G.w, up, xn.w, yn.w);
+    const bool b_x = gda_in_band(x.x, xn.x, up.delta), b_y = gda_in_band(x.y, xn.y, up.delta);
+    const bool b_z = gda_in_band(x.z, xn.z, up.delta), b_w = gda_in_band(x.w, xn.w, up.delta);
+    if (b_x | b_y | b_z | b_w) {
+        if (b_x) xn.x = gda_perturb(x.x, xn.x, up.delta, up.seed_mix, t, i, b0 + 0);
+        if (b_y) xn.y = gda_perturb(x.y, xn.y, up.delta, up.seed_mix, t, i, b0 + 1);
+        if (b_z) xn.z = gda_perturb(x.z, xn.z, up.delta, up.seed_mix, t, i, b0 + 2);
+        if (b_w) xn.w = gda_perturb(x.w, xn.w, up.delta, up.seed_mix, t, i, b0 + 3);
+    }
 }
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }

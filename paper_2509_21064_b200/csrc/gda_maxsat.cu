@@ -121,11 +121,7 @@ maxsat_step_kernel(int n, int B, int chunks, const int32_t* __restrict__ vptr, c
     const float4 xv = ldg4(x + off);
     const float4 yv = *reinterpret_cast<const float4*>(y + off);
     float4 xo, yo;
-    const uint32_t b0 = 4u * (uint32_t)c4;
-    gda_update<GFUN>(xv.x, yv.x, G.x, up, t, (uint32_t)var, b0 + 0, xo.x, yo.x);
-    gda_update<GFUN>(xv.y, yv.y, G.y, up, t, (uint32_t)var, b0 + 1, xo.y, yo.y);
-    gda_update<GFUN>(xv.z, yv.z, G.z, up, t, (uint32_t)var, b0 + 2, xo.z, yo.z);
-    gda_update<GFUN>(xv.w, yv.w, G.w, up, t, (uint32_t)var, b0 + 3, xo.w, yo.w);
+    gda_update4<GFUN>(xv, yv, G, up, t, (uint32_t)var, 4u * (uint32_t)c4, xo, yo);
     *reinterpret_cast<float4*>(xn + off) = xo;
     *reinterpret_cast<float4*>(y + off) = yo;
 }

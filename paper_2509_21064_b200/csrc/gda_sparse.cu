@@ -21,76 +21,99 @@ __device__ __forceinline__ void fma4(float4& a, float v, const float4& g) {
     a.x = fmaf(v, g.x, a.x); a.y = fmaf(v, g.y, a.y); a.z = fmaf(v, g.z, a.z); a.w = fmaf(v, g.w, a.w);
 }
 
-// sum_k val2[k] * X[col[k]][c4]  for k in [start, end): (col,val) fetched 32 at a time, one per lane
+// One 512-byte gather: row c of X for this lane's four restarts.  xb = X + this lane's column offset (bytes),
+// stride = 4 B bytes per row; c * stride is one IMAD.WIDE.U32 (no 64-bit shifts and carries per gather).
+__device__ __forceinline__ float4 gather4(const char* __restrict__ xb, uint32_t stride, int c) {
+    return __ldg(reinterpret_cast<const float4*>(xb + (uint64_t)(uint32_t)c * (uint64_t)stride));
+}
+
+// acc += sum_{u < cnt} v_u * X[c_u][this lane's columns], where entry u's column is held by lane c_lane0 + u (in
+// word_c) and its value by lane v_lane0 + u (in word_v): broadcast by shuffle, 4 independent 512 B gathers in flight.
+// Every lane takes part with a VALID column offset (lanes past a ragged B are clamped by the caller and only their
+// stores are suppressed), so nothing here is predicated on "active".
+__device__ __forceinline__ void accumulate_lanes(float4& acc, int word_c, int c_lane0, int word_v, int v_lane0, int cnt,
+                                                 const char* __restrict__ xb, uint32_t stride) {
+    for (int u = 0; u < cnt; u += 4) {
+        int c[4]; float v[4]; float4 g[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {                        // past the end: the last entry again (same line) with value 0
+            const int e = min(u + q, cnt - 1);
+            c[q] = __shfl_sync(0xffffffffu, word_c, c_lane0 + e);
+            v[q] = __int_as_float(__shfl_sync(0xffffffffu, word_v, v_lane0 + e));
+            if (u + q >= cnt) v[q] = 0.0f;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) g[q] = gather4(xb, stride, c[q]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) fma4(acc, v[q], g[q]);
+    }
+}
+
+// sum_k val2[k] * X[col[k]][this lane's columns]  for k in [start, end): (col,val) fetched 32 at a time, one per lane
 __device__ __forceinline__ float4 gather_row(const int32_t* __restrict__ col, const float* __restrict__ val2,
-                                             int start, int end, const float* __restrict__ x, int B,
-                                             int c4, bool active, int lane) {
+                                             int start, int end, const char* __restrict__ xb, uint32_t stride, int lane) {
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int base = start; base < end; base += 32) {
         const int k = base + lane;
         const int my_c = (k < end) ? __ldg(col + k) : 0;
-        const float my_v = (k < end) ? __ldg(val2 + k) : 0.0f;
-        const int cnt = min(32, end - base);
-        int u = 0;
-        for (; u + 4 <= cnt; u += 4) {                       // 4 independent 512 B gathers in flight
-            int c[4]; float v[4]; float4 g[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) { c[q] = __shfl_sync(0xffffffffu, my_c, u + q); v[q] = __shfl_sync(0xffffffffu, my_v, u + q); }
-#pragma unroll
-            for (int q = 0; q < 4; ++q) g[q] = active ? ldg4(x + (size_t)c[q] * B + 4 * c4) : make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-            for (int q = 0; q < 4; ++q) fma4(acc, v[q], g[q]);
-        }
-        for (; u < cnt; ++u) {
-            const int c = __shfl_sync(0xffffffffu, my_c, u);
-            const float v = __shfl_sync(0xffffffffu, my_v, u);
-            if (active) fma4(acc, v, ldg4(x + (size_t)c * B + 4 * c4));
-        }
+        const int my_v = (k < end) ? __ldg(reinterpret_cast<const int*>(val2) + k) : 0;
+        accumulate_lanes(acc, my_c, 0, my_v, 0, min(32, end - base), xb, stride);
     }
     return acc;
 }
 
 template <int GFUN>
-__device__ __forceinline__ void update_store(int row, int c4, int B, float4 G, const float* __restrict__ x,
+__device__ __forceinline__ void update_store(int row, int c4, int B, bool active, float4 G, const float* __restrict__ x,
                                              float* __restrict__ y, float* __restrict__ xn,
                                              const UpdParams& up, uint32_t t) {
     const size_t off = (size_t)row * B + 4 * c4;
     const float4 xv = ldg4(x + off);
     const float4 yv = *reinterpret_cast<const float4*>(y + off);
     float4 xo, yo;
-    const uint32_t b0 = 4u * (uint32_t)c4;
-    gda_update<GFUN>(xv.x, yv.x, G.x, up, t, (uint32_t)row, b0 + 0, xo.x, yo.x);
-    gda_update<GFUN>(xv.y, yv.y, G.y, up, t, (uint32_t)row, b0 + 1, xo.y, yo.y);
-    gda_update<GFUN>(xv.z, yv.z, G.z, up, t, (uint32_t)row, b0 + 2, xo.z, yo.z);
-    gda_update<GFUN>(xv.w, yv.w, G.w, up, t, (uint32_t)row, b0 + 3, xo.w, yo.w);
+    gda_update4<GFUN>(xv, yv, G, up, t, (uint32_t)row, 4u * (uint32_t)c4, xo, yo);
+    if (!active) return;
     *reinterpret_cast<float4*>(xn + off) = xo;
     *reinterpret_cast<float4*>(y + off) = yo;
 }
 
-// warp-per-(row, chunk).  MODE 0: fused step, MODE 1: write G only (gda_grad).
-template <int GFUN, int MODE>
-__global__ void __launch_bounds__(THREADS)
-spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B, int chunks,
+// warp-per-(row, 128-restart chunk): blockIdx.y = chunk, the block's 8 warps take 8 consecutive rows.
+// MODE 0: fused step, MODE 1: write G only (gda_grad).
+// ELL: rows of degree <= 8 come as one packed 64-byte record (8 columns, 8 values; gda_api.cu) fetched with a single
+// coalesced load, which removes the rowptr -> (col, val) hop from the dependent chain of a row; a record whose word 0
+// is -1 sends the row through its CSR entries.  40 registers (6 blocks per SM).  Measured on config 3 (profiles/):
+// 17.3 us per step before, 16.3 us with the lean gather loop, 14.8 us with the records and 6 blocks per SM;
+// prefetching the row's own x, y lines into L1 up front was slower (15.1 us) and is not done.
+template <int GFUN, int MODE, bool ELL>
+__global__ void __launch_bounds__(THREADS, 6)
+spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
                const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
-               const float* __restrict__ val2, const float* __restrict__ cprime,
+               const float* __restrict__ val2, const int32_t* __restrict__ ell, const float* __restrict__ cprime,
                const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
                UpdParams up, const RunState* __restrict__ st, uint32_t t_off) {
     const int lane = threadIdx.x & 31;
-    const uint32_t item = blockIdx.x * WARPS + (threadIdx.x >> 5);           // n * chunks < 2^30 (checked by gda_run)
-    const bool in_range = item < (uint32_t)n_rows * (uint32_t)chunks;
-    const uint32_t ridx = in_range ? item / (uint32_t)chunks : 0u;
-    const int chunk = (int)(item - ridx * (uint32_t)chunks);
-    const int row = row_list ? __ldg(row_list + ridx) : (int)ridx;
-    const int c4 = chunk * 32 + lane;
-    const bool active = in_range && 4 * c4 < B;
-    const int start = __ldg(rowptr + row), end = in_range ? __ldg(rowptr + row + 1) : start;
+    const int ridx = blockIdx.x * WARPS + (threadIdx.x >> 5);
+    if (ridx >= n_rows) return;                              // warp-uniform
+    const int row = row_list ? __ldg(row_list + ridx) : ridx;
+    const bool active = 4 * (blockIdx.y * 32 + lane) < B;
+    const int c4 = active ? blockIdx.y * 32 + lane : B / 4 - 1;      // ragged B: idle lanes recompute the last float4
+    const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
+    const uint32_t stride = 4u * (uint32_t)B;
+    float4 G = make_float4(0.f, 0.f, 0.f, 0.f);
+    bool csr = true;
+    if (ELL) {
+        const int w = __ldg(ell + (size_t)row * 16 + (lane & 15));
+        csr = __shfl_sync(0xffffffffu, w, 0) < 0;
+        if (!csr) {
+            const int cnt = __popc(__ballot_sync(0xffffffffu, w != 0 && (lane & 24) == 8));   // values sit in lanes 8..15
+            accumulate_lanes(G, w, 0, w, 8, cnt, xb, stride);
+        }
+    }
+    if (csr) G = gather_row(col, val2, __ldg(rowptr + row), __ldg(rowptr + row + 1), xb, stride, lane);
     const float cp = __ldg(cprime + row);
-    float4 G = gather_row(col, val2, start, end, x, B, c4, active, lane);
     G.x += cp; G.y += cp; G.z += cp; G.w += cp;
-    if (!active) return;
-    if (MODE == 1) { *reinterpret_cast<float4*>(xn + (size_t)row * B + 4 * c4) = G; return; }
+    if (MODE == 1) { if (active) *reinterpret_cast<float4*>(xn + (size_t)row * B + 4 * c4) = G; return; }
     const uint32_t t = (st ? st->t : 0u) + t_off;
-    update_store<GFUN>(row, c4, B, G, x, y, xn, up, t);
+    update_store<GFUN>(row, c4, B, active, G, x, y, xn, up, t);
 }
 
 // row-split: one block per (heavy row, chunk); the 8 warps take interleaved 32-entry slices of the row
@@ -105,25 +128,26 @@ spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chu
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ridx = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
     const int row = __ldg(row_list + ridx);
-    const int c4 = chunk * 32 + lane;
-    const bool active = 4 * c4 < B;
+    const bool active = 4 * (chunk * 32 + lane) < B;
+    const int c4 = active ? chunk * 32 + lane : B / 4 - 1;
+    const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
     const int start = __ldg(rowptr + row), end = __ldg(rowptr + row + 1);
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int base = start + 32 * warp; base < end; base += 32 * WARPS) {
-        const float4 part = gather_row(col, val2, base, min(base + 32, end), x, B, c4, active, lane);
+        const float4 part = gather_row(col, val2, base, min(base + 32, end), xb, 4u * (uint32_t)B, lane);
         acc.x += part.x; acc.y += part.y; acc.z += part.z; acc.w += part.w;
     }
     red[warp][lane] = acc;
     __syncthreads();
-    if (warp != 0 || !active) return;
+    if (warp != 0) return;
     float4 G = red[0][lane];
 #pragma unroll
     for (int w = 1; w < WARPS; ++w) { const float4 r = red[w][lane]; G.x += r.x; G.y += r.y; G.z += r.z; G.w += r.w; }
     const float cp = __ldg(cprime + row);
     G.x += cp; G.y += cp; G.z += cp; G.w += cp;
-    if (MODE == 1) { *reinterpret_cast<float4*>(xn + (size_t)row * B + 4 * c4) = G; return; }
+    if (MODE == 1) { if (active) *reinterpret_cast<float4*>(xn + (size_t)row * B + 4 * c4) = G; return; }
     const uint32_t t = (st ? st->t : 0u) + t_off;
-    update_store<GFUN>(row, c4, B, G, x, y, xn, up, t);
+    update_store<GFUN>(row, c4, B, active, G, x, y, xn, up, t);
 }
 
 // S5 for sparse QUBO: partial[rb][b] = sum over the rows of block rb of x_hat_i ((Q_off x_hat)_i + c'_i)
@@ -196,14 +220,14 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     const int chunks = (B / 4 + 31) / 32;
     const int n_light = p->d_light_rows ? p->n_light : p->n;
     if (n_light > 0) {
-        const long long items = (long long)n_light * chunks;
-        const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
-        if (up.gfun == GDA_G_QUADRATIC)
-            spmm_step_warp<GDA_G_QUADRATIC, MODE><<<grid, THREADS, 0, s>>>(n_light, p->d_light_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off);
-        else
-            spmm_step_warp<GDA_G_ENTROPY, MODE><<<grid, THREADS, 0, s>>>(n_light, p->d_light_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off);
+        const dim3 grid((unsigned)((n_light + WARPS - 1) / WARPS), (unsigned)chunks);
+#define GDA_SP_ARGS n_light, p->d_light_rows, B, p->d_rowptr, p->d_col, p->d_val2, p->d_ell, p->d_cprime, x, y, xn, up, st, t_off
+#define GDA_SP_CASE(E) \
+        if (up.gfun == GDA_G_QUADRATIC) spmm_step_warp<GDA_G_QUADRATIC, MODE, E><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); \
+        else spmm_step_warp<GDA_G_ENTROPY, MODE, E><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS)
+        if (p->d_ell) { GDA_SP_CASE(true); } else { GDA_SP_CASE(false); }
+#undef GDA_SP_CASE
+#undef GDA_SP_ARGS
         if (launches) ++*launches;
     }
     if (p->n_heavy > 0) {

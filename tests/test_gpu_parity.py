@@ -235,10 +235,37 @@ def general_qubo_csr(n, seed, integral):
     return wl.QuboCSR(n, np.array(rowptr, np.int32), np.array(col, np.int32), np.array(val, np.float32), c)
 
 
-@pytest.mark.parametrize("case", ["star_isolated", "general_int", "general_float", "n1"])
+def degree_ladder_qubo(n_groups, seed):
+    """Rows of every degree 0..12 (the packed-record path takes degree <= 8, its CSR fallback the rest), explicit
+    zero entries, a linear term; average degree below 8 so that the records are built."""
+    rng = np.random.default_rng(seed)
+    n = 40 * n_groups
+    Q = np.zeros((n, n), dtype=np.float32)
+    stored = np.zeros((n, n), dtype=bool)
+    for g in range(n_groups):
+        hubs = np.arange(13) + 40 * g                    # hub d gets d neighbours among the 27 leaves of its group
+        leaves = np.arange(13, 40) + 40 * g
+        for d, hcol in enumerate(hubs):
+            for j in rng.choice(leaves, size=d, replace=False):
+                v = float(rng.integers(-2, 3))           # 0 now and then: stored explicitly
+                Q[hcol, j] = Q[j, hcol] = v
+                stored[hcol, j] = stored[j, hcol] = True
+    rowptr, col, val = [0], [], []
+    for i in range(n):
+        nz = np.nonzero(stored[i])[0]
+        col += list(nz)
+        val += list(Q[i, nz])
+        rowptr.append(len(col))
+    c = rng.integers(-2, 3, size=n).astype(np.float32)
+    return wl.QuboCSR(n, np.array(rowptr, np.int32), np.array(col, np.int32), np.array(val, np.float32), c)
+
+
+@pytest.mark.parametrize("case", ["star_isolated", "general_int", "general_float", "n1", "packed_rows"])
 def test_sparse_edge_cases(api, oracle, case):
     if case == "star_isolated":
         Pw, B = star_plus_isolated(700, 5), 8
+    elif case == "packed_rows":
+        Pw, B = degree_ladder_qubo(3, 5), 132
     elif case == "general_int":
         Pw, B = general_qubo_csr(37, 1, True), 4
     elif case == "general_float":
