@@ -15,7 +15,21 @@
 // rows per warp, and each thread writes 64 contiguous bytes of the next bf16 operand.
 //
 // Warp roles (384 threads, one persistent CTA per SM): warp 0 TMA producer, warp 1 MMA issuer (one
-// elected thread), warp 2 TMEM allocator, warps 4-11 epilogue (two warpgroups, 128 columns each).
+// elected thread), warp 2 TMEM allocator, warps 4-11 epilogue (two warpgroups, half of the tile's columns each).
+//
+// Operand feed.  A single CTA must take in 48 KB per 512-cycle k-block (A 16 KB + B 32 KB) and can hold only 4 such
+// stages; measured, that feed (not the tensor pipe) bounded the kernel (profiles/r1_dense_cfg4.md).  So CTAs run as
+// PAIRS (cluster of 2, tcgen05 cta_group::2): the pair computes 256 restarts x 256 variables per MMA (M = 256), each
+// CTA stages its own 128 rows of A and HALF of the Q tile (the tensor cores of both SMs read both halves), i.e.
+// 32 KB per CTA and k-block and 6 stages in flight.  The leader CTA (rank 0) issues the MMAs; both CTAs' TMA loads
+// signal the leader's full barrier; tcgen05.commit multicasts "slot free" and "accumulator ready" to both CTAs;
+// the peer's epilogue warps release the accumulator on the leader's barrier through the cluster address space.
+// Each CTA keeps its 128 rows of the accumulator in its own TMEM, so the epilogue is the same in both modes.
+// B = 128 (one block of restarts) or an odd number of 128-blocks runs the single-CTA variant (CG = 1).
+//
+// Tile schedule.  Work units are (CG x 128 restarts) x (256 variables), dealt round-robin to the clusters; when
+// the last round would be less than half full, its units are split into two 128-variable halves so that the tail
+// costs half a round (config 4: 256 units on 74 pairs = 3 rounds + 34 left -> 68 half units).
 #include "gda_internal.cuh"
 
 #include <cuda.h>
@@ -24,11 +38,16 @@
 
 namespace {
 
-constexpr int BM = 128, BN = 256, BK = 64, STAGES = 4, UMMA_K = 16;
-constexpr int A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int BM = 128, BN = 256, BK = 64, UMMA_K = 16, BBOX = 64;   // BBOX: rows of Q per TMA box
+constexpr int A_BYTES = BM * BK * 2;
 constexpr int NUM_THREADS = 384, EPI_WARP0 = 4, EPI_WARPS = 8;
 constexpr int TMEM_COLS = 512;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024;     // tiles + barriers + alignment slack
+// per CTA and pipeline stage: its 128 rows of A and its 256 / CG rows of Q; 4 stages of 48 KB or 6 stages of 32 KB
+template <int CG> struct Pipe {
+    static constexpr int STAGE_BYTES = A_BYTES + (BN / CG) * BK * 2;
+    static constexpr int STAGES = CG == 1 ? 4 : 6;
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024;     // tiles + barriers + alignment slack
+};
 
 enum { MODE_STEP = 0, MODE_GRAD = 1, MODE_SCORE = 2 };
 
@@ -63,6 +82,37 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
         ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1) : "memory");
 }
+// pair mode: the load lands in THIS CTA's shared memory and signals `bar` given as a shared::cluster address
+// (the leader's full barrier), which cta_group::2 allows
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, uint32_t bar_cluster, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar_cluster), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {                     // arrives on `bar` of both CTAs of the pair
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(bar), "h"((uint16_t)3) : "memory");
+}
+__device__ __forceinline__ void tc_mma_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t rank) {  // shared::cta -> shared::cluster of `rank`
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster) {
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
@@ -114,16 +164,40 @@ struct DenseArgs {
     const float* hvec;           // [n]  Q_off 1 + c'  (constant part of the gradient with the centred operand)
     const float* cprime;         // [n]  c + diag(Q)
     float* gout;                 // MODE_GRAD: [n][B] gradient
-    double* partial;             // MODE_SCORE: [n/128][B] partial objective sums
+    double* partial;             // MODE_SCORE: [n/64][B] partial objective sums
     UpdParams up;
     const RunState* st;
     uint32_t t_off;
 };
 
-template <int MODE, int GFUN>
+// Work unit u of the schedule described at the top: restarts [m0, m0 + 128) of THIS CTA, variables [n0, n0 + ncols).
+struct Unit { int m0, n0, ncols; };
+struct Schedule {
+    int num_msup, full_units, num_units;
+    __device__ __forceinline__ Schedule(int n, int B, int cl, int num_clusters) {
+        num_msup = B / (BM * cl);
+        const int S = num_msup * (n / BN);
+        const int left = S % num_clusters;
+        const bool split = left > 0 && 2 * left <= num_clusters;
+        full_units = split ? S - left : S;
+        num_units = split ? S + left : S;
+    }
+    __device__ __forceinline__ Unit get(int u, int cl, int rank) const {
+        int s = u, h = 0, ncols = BN;
+        if (u >= full_units) { s = full_units + ((u - full_units) >> 1); h = (u - full_units) & 1; ncols = BN / 2; }
+        Unit t;
+        t.m0 = ((s % num_msup) * cl + rank) * BM;
+        t.n0 = (s / num_msup) * BN + h * (BN / 2);
+        t.ncols = ncols;
+        return t;
+    }
+};
+
+template <int MODE, int GFUN, int CG>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                   const DenseArgs args) {
+    constexpr int STAGES = Pipe<CG>::STAGES, STAGE_BYTES = Pipe<CG>::STAGE_BYTES;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;            // SWIZZLE_128B needs 1024 B alignment
     const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
@@ -136,7 +210,10 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
         reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int num_m = args.B / BM, num_n = args.n / BN, num_tiles = num_m * num_n, num_kb = args.n / BK;
+    const int rank = CG > 1 ? (int)cluster_ctarank() : 0;                        // 0 = leader of the pair
+    const int cluster_id = blockIdx.x / CG, num_clusters = gridDim.x / CG;
+    const Schedule sched(args.n, args.B, CG, num_clusters);
+    const int num_kb = args.n / BK;
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_a) : "memory");
@@ -144,128 +221,191 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), EPI_WARPS); }
+        for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), CG * EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 2) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (warp == 2) {                                       // pair mode: the same warp of both CTAs allocates together
+        if (CG == 1) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(TMEM_COLS) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+        }
     }
     tc_fence_before();
-    __syncthreads();
+    if (CG > 1) cluster_sync_all(); else __syncthreads();      // the peer's barriers exist before anything signals them
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== TMA producer (both CTAs of a pair: own rows of A, own half of the Q tile) =====
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-                const int m_blk = tile % num_m, n_blk = tile / num_m;
+            for (int u = cluster_id; u < sched.num_units; u += num_clusters) {
+                const Unit t = sched.get(u, CG, rank);
+                const int slice = t.ncols / CG;                                   // rows of Q this CTA stages
+                const uint32_t bytes = (uint32_t)(CG * (A_BYTES + slice * BK * 2)); // both CTAs' loads land on the leader's barrier
                 for (int kb = 0; kb < num_kb; ++kb) {
-                    mbar_wait(empty_bar(stage), phase ^ 1u);
-                    mbar_expect_tx(full_bar(stage), STAGE_BYTES);
+                    mbar_wait(empty_bar(stage), phase ^ 1u);                      // the MMAs that read this slot have retired
                     const uint32_t a_dst = smem_base + stage * STAGE_BYTES;
-                    tma_load_2d(a_dst, &tmap_a, full_bar(stage), kb * BK, m_blk * BM);
-                    tma_load_2d(a_dst + A_BYTES, &tmap_b, full_bar(stage), kb * BK, n_blk * BN);
+                    if (CG == 1) {
+                        mbar_expect_tx(full_bar(stage), bytes);
+                        tma_load_2d(a_dst, &tmap_a, full_bar(stage), kb * BK, t.m0);
+                        for (int r = 0; r < slice; r += BBOX)
+                            tma_load_2d(a_dst + A_BYTES + (uint32_t)r * 128u, &tmap_b, full_bar(stage), kb * BK, t.n0 + r);
+                    } else {
+                        if (rank == 0) mbar_expect_tx(full_bar(stage), bytes);
+                        const uint32_t lead_bar = map_to_cta(full_bar(stage), 0);
+                        tma_load_2d_pair(a_dst, &tmap_a, lead_bar, kb * BK, t.m0);
+                        for (int r = 0; r < slice; r += BBOX)
+                            tma_load_2d_pair(a_dst + A_BYTES + (uint32_t)r * 128u, &tmap_b, lead_bar, kb * BK, t.n0 + rank * slice + r);
+                    }
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
             }
+            if (CG > 1)                                                            // every release aimed at this CTA has landed
+                for (int i = 0; i < STAGES; ++i) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer (one thread) =====
-        if (lane == 0) {
-            constexpr uint32_t idesc = make_idesc(BM, BN);
+        // ===== MMA issuer (one thread; pair mode: the leader CTA only) =====
+        if (lane == 0 && rank == 0) {
             int stage = 0; uint32_t phase = 0; int it = 0;
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
+            for (int u = cluster_id; u < sched.num_units; u += num_clusters, ++it) {
+                const Unit t = sched.get(u, CG, rank);
+                const uint32_t idesc = make_idesc(BM * CG, t.ncols);
                 const int as = it & 1;
                 const uint32_t aphase = (uint32_t)(it >> 1) & 1u;
-                mbar_wait(tempty_bar(as), aphase ^ 1u);                           // epilogue has drained this accumulator
+                mbar_wait(tempty_bar(as), aphase ^ 1u);                           // every epilogue warp has drained this accumulator
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
                 for (int kb = 0; kb < num_kb; ++kb) {
-                    mbar_wait(full_bar(stage), phase);                            // TMA bytes have landed
+                    mbar_wait(full_bar(stage), phase);                            // TMA bytes have landed (in both CTAs)
                     tc_fence_after();
                     const uint32_t a_addr = smem_base + stage * STAGE_BYTES;
                     const uint64_t adesc = make_sdesc(a_addr), bdesc = make_sdesc(a_addr + A_BYTES);
 #pragma unroll
-                    for (int k = 0; k < BK / UMMA_K; ++k)                          // +32 B per K=16 slice inside the swizzle atom
-                        tc_mma(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)((kb | k) != 0));
-                    tc_commit(empty_bar(stage));                                   // frees the smem slot when the MMAs retire
+                    for (int k = 0; k < BK / UMMA_K; ++k) {                        // +32 B per K=16 slice inside the swizzle atom
+                        if (CG == 1) tc_mma(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)((kb | k) != 0));
+                        else tc_mma_pair(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)((kb | k) != 0));
+                    }
+                    if (CG == 1) tc_commit(empty_bar(stage)); else tc_commit_pair(empty_bar(stage));   // slot free (both CTAs)
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
-                tc_commit(tfull_bar(as));                                          // accumulator complete -> epilogue
+                if (CG == 1) tc_commit(tfull_bar(as)); else tc_commit_pair(tfull_bar(as));             // accumulator complete
             }
         }
     } else if (warp >= EPI_WARP0) {
         // ===== epilogue: TMEM -> registers -> fused GDA update -> global =====
         const int ew = warp - EPI_WARP0;
         const int lane_grp = warp & 3;                      // TMEM lanes 32*lane_grp .. +31 are accessible to this warp
-        const int half = ew >> 2;                           // which 128 of the tile's 256 columns
-        const uint32_t t = (args.st ? args.st->t : 0u) + args.t_off;
+        const int half = ew >> 2;                           // which half of the tile's columns
+        const uint32_t tstep = (args.st ? args.st->t : 0u) + args.t_off;
         int it = 0;
-        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
-            const int m_blk = tile % num_m, n_blk = tile / num_m;
+        for (int u = cluster_id; u < sched.num_units; u += num_clusters, ++it) {
+            const Unit t = sched.get(u, CG, rank);
             const int as = it & 1;
             const uint32_t aphase = (uint32_t)(it >> 1) & 1u;
-            const int b = m_blk * BM + lane_grp * 32 + lane;                      // restart owned by this thread
+            const int b = t.m0 + lane_grp * 32 + lane;                            // restart owned by this thread
+            const int hcols = t.ncols >> 1;                                       // 128 or 64 columns per warpgroup
             mbar_wait(tfull_bar(as), aphase);
             tc_fence_after();
             double score = 0.0;
-            for (int cb = 0; cb < 4; ++cb) {
-                const int col0 = half * 128 + cb * 32;
-                const int i0 = n_blk * BN + col0;
+            for (int cb = 0; cb < hcols / 32; ++cb) {
+                const int col0 = half * hcols + cb * 32;
+                const int i0 = t.n0 + col0;
                 uint32_t acc[32];
                 tc_ld32(tmem_base + ((uint32_t)(lane_grp * 32) << 16) + (uint32_t)(as * BN + col0), acc);
+                // the constant part of the gradient for these 32 columns: one coalesced load, lane j holds column j
+                // (a per-element load would sit between the stores below and serialise the loop: the compiler must
+                // assume that x, y and hvec alias)
+                const float hv = __ldg(args.hvec + i0 + lane);
                 if (MODE == MODE_STEP) {
-                    float xv[32], yv[32];
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        xv[j] = args.x[(size_t)(i0 + j) * args.B + b];
-                        yv[j] = args.y[(size_t)(i0 + j) * args.B + b];
-                    }
-                    tc_wait_ld();
-                    uint32_t packed[16];
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) {
-                        const float G = fmaf(2.0f, __uint_as_float(acc[j]), __ldg(args.hvec + i0 + j));
-                        float xn, yn;
-                        gda_update<GFUN>(xv[j], yv[j], G, args.up, t, (uint32_t)(i0 + j), (uint32_t)b, xn, yn);
-                        args.x[(size_t)(i0 + j) * args.B + b] = xn;
-                        args.y[(size_t)(i0 + j) * args.B + b] = yn;
-                        const uint32_t zb = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(xn - 0.5f));
-                        if (j & 1) packed[j >> 1] |= zb << 16; else packed[j >> 1] = zb;
-                    }
+                    float* __restrict__ xp = args.x + (size_t)i0 * args.B + b;
+                    float* __restrict__ yp = args.y + (size_t)i0 * args.B + b;
                     uint4* zdst = reinterpret_cast<uint4*>(args.zt_out + (size_t)b * args.n + i0);
+                    tc_wait_ld();
 #pragma unroll
-                    for (int q = 0; q < 4; ++q)
-                        zdst[q] = make_uint4(packed[4 * q], packed[4 * q + 1], packed[4 * q + 2], packed[4 * q + 3]);
+                    for (int h = 0; h < 2; ++h) {                                 // 16 columns at a time: loads, updates, stores
+                        float xv[16], yv[16];
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            xv[j] = xp[(size_t)(16 * h + j) * args.B];
+                            yv[j] = yp[(size_t)(16 * h + j) * args.B];
+                        }
+                        // Eq. 6 for the 16 elements as independent, branch-free chains; the (rare) perturbation of
+                        // reading R3 is applied afterwards behind ONE test -- a branch per element serialises the loop
+                        float xt[16];
+                        uint32_t band = 0u;
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const float G = fmaf(2.0f, __uint_as_float(acc[16 * h + j]), __shfl_sync(0xffffffffu, hv, 16 * h + j));
+                            gda_update_nopert<GFUN>(xv[j], yv[j], G, args.up, xt[j], yv[j]);
+                            band |= gda_in_band(xv[j], xt[j], args.up.delta) ? (1u << j) : 0u;
+                        }
+                        if (band) {
+#pragma unroll
+                            for (int j = 0; j < 16; ++j)
+                                if (band & (1u << j))
+                                    xt[j] = gda_perturb(xv[j], xt[j], args.up.delta, args.up.seed_mix, tstep, (uint32_t)(i0 + 16 * h + j), (uint32_t)b);
+                        }
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) xv[j] = xt[j];
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            xp[(size_t)(16 * h + j) * args.B] = xv[j];
+                            yp[(size_t)(16 * h + j) * args.B] = yv[j];
+                        }
+#pragma unroll
+                        for (int q = 0; q < 2; ++q) {
+                            uint32_t pk[4];
+#pragma unroll
+                            for (int e = 0; e < 4; ++e) {
+                                const __nv_bfloat162 z2 = __floats2bfloat162_rn(xv[8 * q + 2 * e] - 0.5f, xv[8 * q + 2 * e + 1] - 0.5f);
+                                pk[e] = *reinterpret_cast<const uint32_t*>(&z2);
+                            }
+                            zdst[2 * h + q] = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                        }
+                    }
                 } else if (MODE == MODE_GRAD) {
                     tc_wait_ld();
 #pragma unroll
                     for (int j = 0; j < 32; ++j)
-                        args.gout[(size_t)(i0 + j) * args.B + b] = fmaf(2.0f, __uint_as_float(acc[j]), __ldg(args.hvec + i0 + j));
+                        args.gout[(size_t)(i0 + j) * args.B + b] = fmaf(2.0f, __uint_as_float(acc[j]), __shfl_sync(0xffffffffu, hv, j));
                 } else {
                     float xv[32];
+                    const float cpv = __ldg(args.cprime + i0 + lane);
 #pragma unroll
                     for (int j = 0; j < 32; ++j) xv[j] = args.x[(size_t)(i0 + j) * args.B + b];
                     tc_wait_ld();
 #pragma unroll
-                    for (int j = 0; j < 32; ++j)                                  // x_hat_i ((Q_off x_hat)_i + c'_i), fp32 row sums
-                        if (xv[j] > 0.5f) score += (double)__uint_as_float(acc[j]) + (double)__ldg(args.cprime + i0 + j);
+                    for (int j = 0; j < 32; ++j) {                                // x_hat_i ((Q_off x_hat)_i + c'_i), fp32 row sums
+                        const float cpj = __shfl_sync(0xffffffffu, cpv, j);
+                        if (xv[j] > 0.5f) score += (double)__uint_as_float(acc[j]) + (double)cpj;
+                    }
                 }
             }
-            if (MODE == MODE_SCORE) args.partial[(size_t)(n_blk * 2 + half) * args.B + b] = score;
+            if (MODE == MODE_SCORE) {                       // one partial per 64 variables; a 128-column share fills two slots
+                const int slot = (t.n0 + half * hcols) / 64;
+                args.partial[(size_t)slot * args.B + b] = score;
+                if (hcols == 128) args.partial[(size_t)(slot + 1) * args.B + b] = 0.0;
+            }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(tempty_bar(as));                           // 8 warps -> accumulator stage free
+            if (lane == 0) {                                                      // CG * 8 warps -> accumulator stage free
+                if (CG == 1) mbar_arrive(tempty_bar(as)); else mbar_arrive_cluster(map_to_cta(tempty_bar(as), 0));
+            }
         }
     }
     tc_fence_before();
-    __syncthreads();
+    if (CG > 1) cluster_sync_all(); else __syncthreads();      // no CTA leaves while its peer may still signal or read it
     if (warp == 2) {
         tc_fence_after();
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+        if (CG == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+        else asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
     }
 }
 
@@ -331,16 +471,26 @@ struct DenseHost {
 template <int MODE, int GFUN>
 gda_status launch_gemm(gda_problem* p, const CUtensorMap& ta, const DenseArgs& a, cudaStream_t s) {
     DenseHost* h = static_cast<DenseHost*>(p->tmap_Q);
-    auto kern = dense_gemm_kernel<MODE, GFUN>;
     static bool configured = false;
     if (!configured) {
-        GDA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        GDA_CUDA_TRY(cudaFuncSetAttribute(dense_gemm_kernel<MODE, GFUN, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, Pipe<2>::SMEM_BYTES));
+        GDA_CUDA_TRY(cudaFuncSetAttribute(dense_gemm_kernel<MODE, GFUN, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, Pipe<1>::SMEM_BYTES));
         configured = true;
     }
-    const int tiles = (a.B / BM) * (a.n / BN);
-    const int grid = tiles < p->num_sms ? tiles : p->num_sms;
-    kern<<<grid, NUM_THREADS, SMEM_BYTES, s>>>(ta, h->tmap_q, a);
-    GDA_CUDA_TRY(cudaGetLastError());
+    const bool pair = a.B % (BM * 2) == 0;                   // an odd number of 128-restart blocks runs single CTAs
+    const int cg = pair ? 2 : 1;
+    const int units = (a.B / (BM * cg)) * (a.n / BN);
+    const int max_clusters = p->num_sms / cg;
+    const int clusters = units < max_clusters ? units : max_clusters;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(clusters * cg)); cfg.blockDim = dim3(NUM_THREADS);
+    cfg.dynamicSmemBytes = pair ? Pipe<2>::SMEM_BYTES : Pipe<1>::SMEM_BYTES; cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cg; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (pair) GDA_CUDA_TRY(cudaLaunchKernelEx(&cfg, dense_gemm_kernel<MODE, GFUN, 2>, ta, h->tmap_q, a));
+    else GDA_CUDA_TRY(cudaLaunchKernelEx(&cfg, dense_gemm_kernel<MODE, GFUN, 1>, ta, h->tmap_q, a));
     return GDA_OK;
 }
 
@@ -381,7 +531,7 @@ gda_status dense_prepare(gda_problem* p, const float* Q, const float* c) {
     GDA_CUDA_TRY(cudaMemcpy(p->d_cprime, cp.data(), n * sizeof(float), cudaMemcpyHostToDevice));
     DenseHost* h = new DenseHost();
     p->tmap_Q = h;
-    return make_tmap(&h->tmap_q, p->d_Qbf, (uint64_t)n, (uint64_t)n, BN);
+    return make_tmap(&h->tmap_q, p->d_Qbf, (uint64_t)n, (uint64_t)n, BBOX);
 }
 
 void dense_release(gda_problem* p) {
@@ -425,7 +575,7 @@ gda_status dense_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaS
     return launch_gemm<MODE_GRAD, GDA_G_QUADRATIC>(p, *ta, a, s);
 }
 
-int32_t dense_num_partials(const gda_problem* p, int32_t) { return p->n / 128; }
+int32_t dense_num_partials(const gda_problem* p, int32_t) { return p->n / 64; }
 
 // S5: x_hat operand (exact in bf16), GEMM, per-thread column sums.  Scratch: the zt buffer NOT holding the current operand.
 gda_status dense_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,

@@ -398,7 +398,10 @@ TOL_GRAD_BF16 = 1e-2
 
 
 def dense_workloads():
-    return [wl.config(4, B=128, n_scale=0.0625), wl.config(4, B=384, n_scale=0.125), wl.config(4, B=256, n_scale=0.25)]
+    # (n, B) = (256, 128) one tile; (512, 384) unclustered half tiles; (1024, 256) clustered half tiles;
+    # (2560, 1024) clustered full tiles (40 units on 74 clusters: no split)
+    return [wl.config(4, B=128, n_scale=0.0625), wl.config(4, B=384, n_scale=0.125), wl.config(4, B=256, n_scale=0.25),
+            wl.config(4, B=1024, n_scale=0.625)]
 
 
 DENSE = dense_workloads()
