@@ -17,19 +17,23 @@
 // Warp roles (384 threads, one persistent CTA per SM): warp 0 TMA producer, warp 1 MMA issuer (one
 // elected thread), warp 2 TMEM allocator, warps 4-11 epilogue (two warpgroups, half of the tile's columns each).
 //
-// Operand feed.  A single CTA must take in 48 KB per 512-cycle k-block (A 16 KB + B 32 KB) and can hold only 4 such
-// stages; measured, that feed (not the tensor pipe) bounded the kernel (profiles/r1_dense_cfg4.md).  So CTAs run as
-// PAIRS (cluster of 2, tcgen05 cta_group::2): the pair computes 256 restarts x 256 variables per MMA (M = 256), each
-// CTA stages its own 128 rows of A and HALF of the Q tile (the tensor cores of both SMs read both halves), i.e.
-// 32 KB per CTA and k-block and 6 stages in flight.  The leader CTA (rank 0) issues the MMAs; both CTAs' TMA loads
-// signal the leader's full barrier; tcgen05.commit multicasts "slot free" and "accumulator ready" to both CTAs;
-// the peer's epilogue warps release the accumulator on the leader's barrier through the cluster address space.
-// Each CTA keeps its 128 rows of the accumulator in its own TMEM, so the epilogue is the same in both modes.
-// B = 128 (one block of restarts) or an odd number of 128-blocks runs the single-CTA variant (CG = 1).
+// Operand feed (measured, profiles/): with one CTA per 128 x 256 tile the kernel was bound by operand delivery, not
+// by the tensor pipe -- 48 KB per CTA and 512-cycle k-block out of L2, about 1.6 GB per step, which is what the L2
+// can deliver in the time the step took.  Hence, when the shape allows:
+//  * CTA PAIRS (tcgen05 cta_group::2, M = 256): each CTA stages its own 128 rows of A and HALF of the Q tile, the
+//    tensor cores of both SMs read both halves; 32 KB per CTA and k-block, 6 stages in flight.  The leader (even rank)
+//    issues the MMAs; both CTAs' TMA loads signal the leader's full barrier; tcgen05.commit multicasts "slot free" and
+//    "accumulator ready"; the peer's epilogue warps release the accumulator on the leader's barrier through the
+//    cluster address space.  Each CTA keeps its 128 rows of the accumulator in its own TMEM: same epilogue.
+//  * TWO PAIRS PER CLUSTER (NP = 2, cluster of 4) that work on the same 256 restarts and adjacent blocks of 256
+//    variables: each CTA loads half of its A rows and TMA-multicasts them to its counterpart in the other pair
+//    (24 KB per CTA and k-block).  A slot is reused when BOTH pairs have retired it (empty barrier count 2, every
+//    leader's commit goes to all four CTAs).
+// B an odd multiple of 128 runs single CTAs (CG = 1); n not a multiple of 512 runs pairs without the multicast.
 //
-// Tile schedule.  Work units are (CG x 128 restarts) x (256 variables), dealt round-robin to the clusters; when
-// the last round would be less than half full, its units are split into two 128-variable halves so that the tail
-// costs half a round (config 4: 256 units on 74 pairs = 3 rounds + 34 left -> 68 half units).
+// Tile schedule: work units of (CG x 128 restarts) x (NP x 256 variables) are dealt round-robin to the clusters.
+// A 128-variable "half" unit does NOT help the tail: measured, an N = 128 MMA takes as long as an N = 256 one (the
+// A-operand path of M = 128 rows per SM sets the instruction time), so units always span 256 variables per pair.
 #include "gda_internal.cuh"
 
 #include <cuda.h>
@@ -38,7 +42,7 @@
 
 namespace {
 
-constexpr int BM = 128, BN = 256, BK = 64, UMMA_K = 16, BBOX = 64;   // BBOX: rows of Q per TMA box
+constexpr int BM = 128, BN = 256, BK = 64, UMMA_K = 16, BBOX = 64;   // BBOX: rows per TMA box (both operands)
 constexpr int A_BYTES = BM * BK * 2;
 constexpr int NUM_THREADS = 384, EPI_WARP0 = 4, EPI_WARPS = 8;
 constexpr int TMEM_COLS = 512;
@@ -89,9 +93,16 @@ __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap
         "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
         ::"r"(dst), "l"(map), "r"(bar_cluster), "r"(c0), "r"(c1) : "memory");
 }
-__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {                     // arrives on `bar` of both CTAs of the pair
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar, uint16_t mask) {      // arrives on `bar` of every CTA in mask
     asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-                 ::"r"(bar), "h"((uint16_t)3) : "memory");
+                 ::"r"(bar), "h"(mask) : "memory");
+}
+// pair mode + multicast: the box lands at the same offset in every CTA of mask and signals, in each of them, the
+// barrier at bar's offset in that CTA's pair leader
+__device__ __forceinline__ void tma_load_2d_pair_mc(uint32_t dst, const CUtensorMap* map, uint32_t bar_cluster, int c0, int c1, uint16_t mask) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%3, %4}], [%2], %5;"
+        ::"r"(dst), "l"(map), "r"(bar_cluster), "r"(c0), "r"(c1), "h"(mask) : "memory");
 }
 __device__ __forceinline__ void tc_mma_pair(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
@@ -138,6 +149,14 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32]) {
           "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
         : "r"(taddr) : "memory");
 }
+__device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr) : "memory");
+}
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // K-major, 128-byte-swizzled shared-memory operand descriptor (rows of 64 bf16 = 128 B, 8-row groups 1024 B apart)
@@ -164,36 +183,25 @@ struct DenseArgs {
     const float* hvec;           // [n]  Q_off 1 + c'  (constant part of the gradient with the centred operand)
     const float* cprime;         // [n]  c + diag(Q)
     float* gout;                 // MODE_GRAD: [n][B] gradient
-    double* partial;             // MODE_SCORE: [n/64][B] partial objective sums
+    double* partial;             // MODE_SCORE: [n/128][B] partial objective sums
     UpdParams up;
     const RunState* st;
     uint32_t t_off;
 };
 
-// Work unit u of the schedule described at the top: restarts [m0, m0 + 128) of THIS CTA, variables [n0, n0 + ncols).
-struct Unit { int m0, n0, ncols; };
-struct Schedule {
-    int num_msup, full_units, num_units;
-    __device__ __forceinline__ Schedule(int n, int B, int cl, int num_clusters) {
-        num_msup = B / (BM * cl);
-        const int S = num_msup * (n / BN);
-        const int left = S % num_clusters;
-        const bool split = left > 0 && 2 * left <= num_clusters;
-        full_units = split ? S - left : S;
-        num_units = split ? S + left : S;
-    }
-    __device__ __forceinline__ Unit get(int u, int cl, int rank) const {
-        int s = u, h = 0, ncols = BN;
-        if (u >= full_units) { s = full_units + ((u - full_units) >> 1); h = (u - full_units) & 1; ncols = BN / 2; }
-        Unit t;
-        t.m0 = ((s % num_msup) * cl + rank) * BM;
-        t.n0 = (s / num_msup) * BN + h * (BN / 2);
-        t.ncols = ncols;
-        return t;
-    }
-};
+// Work unit u of the schedule described at the top: restarts [m0, m0 + 128) of THIS CTA, variables [n0, n0 + 256)
+// of its pair.  rank = rank in the cluster; pair = rank / CG, r = rank % CG.
+struct Unit { int m0, n0; };
+__device__ __forceinline__ Unit get_unit(int u, int B, int cg, int np, int rank) {
+    const int num_msup = B / (BM * cg);
+    Unit t;
+    t.m0 = ((u % num_msup) * cg + rank % cg) * BM;
+    t.n0 = ((u / num_msup) * np + rank / cg) * BN;
+    return t;
+}
+__device__ __forceinline__ int num_units(int n, int B, int cg, int np) { return (B / (BM * cg)) * (n / (BN * np)); }
 
-template <int MODE, int GFUN, int CG>
+template <int MODE, int GFUN, int CG, int NP>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                   const DenseArgs args) {
@@ -210,9 +218,12 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
         reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int rank = CG > 1 ? (int)cluster_ctarank() : 0;                        // 0 = leader of the pair
-    const int cluster_id = blockIdx.x / CG, num_clusters = gridDim.x / CG;
-    const Schedule sched(args.n, args.B, CG, num_clusters);
+    constexpr int CSIZE = CG * NP;                                               // CTAs per cluster
+    const int rank = CSIZE > 1 ? (int)cluster_ctarank() : 0;
+    const int lead = rank & ~(CG - 1);                                           // rank of this CTA's pair leader
+    const bool leader = rank == lead;
+    const int cluster_id = blockIdx.x / CSIZE, num_clusters = gridDim.x / CSIZE;
+    const int units = num_units(args.n, args.B, CG, NP);
     const int num_kb = args.n / BK;
 
     if (warp == 0 && lane == 0) {
@@ -220,7 +231,7 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_b) : "memory");
     }
     if (warp == 1 && lane == 0) {
-        for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), NP); }
         for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), CG * EPI_WARPS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -234,7 +245,7 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
         }
     }
     tc_fence_before();
-    if (CG > 1) cluster_sync_all(); else __syncthreads();      // the peer's barriers exist before anything signals them
+    if (CSIZE > 1) cluster_sync_all(); else __syncthreads();      // the peers' barriers exist before anything signals them
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
 
@@ -242,24 +253,34 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
         // ===== TMA producer (both CTAs of a pair: own rows of A, own half of the Q tile) =====
         if (lane == 0) {
             int stage = 0; uint32_t phase = 0;
-            for (int u = cluster_id; u < sched.num_units; u += num_clusters) {
-                const Unit t = sched.get(u, CG, rank);
-                const int slice = t.ncols / CG;                                   // rows of Q this CTA stages
-                const uint32_t bytes = (uint32_t)(CG * (A_BYTES + slice * BK * 2)); // both CTAs' loads land on the leader's barrier
+            constexpr int SLICE = BN / CG;                                        // rows of Q this CTA stages
+            constexpr uint32_t BYTES = (uint32_t)(CG * (A_BYTES + SLICE * BK * 2)); // a pair's loads land on its leader's barrier
+            for (int u = cluster_id; u < units; u += num_clusters) {
+                const Unit t = get_unit(u, args.B, CG, NP, rank);
                 for (int kb = 0; kb < num_kb; ++kb) {
-                    mbar_wait(empty_bar(stage), phase ^ 1u);                      // the MMAs that read this slot have retired
+                    mbar_wait(empty_bar(stage), phase ^ 1u);                      // every MMA that read this slot has retired
                     const uint32_t a_dst = smem_base + stage * STAGE_BYTES;
                     if (CG == 1) {
-                        mbar_expect_tx(full_bar(stage), bytes);
-                        tma_load_2d(a_dst, &tmap_a, full_bar(stage), kb * BK, t.m0);
-                        for (int r = 0; r < slice; r += BBOX)
+                        mbar_expect_tx(full_bar(stage), BYTES);
+                        for (int r = 0; r < BM; r += BBOX)
+                            tma_load_2d(a_dst + (uint32_t)r * 128u, &tmap_a, full_bar(stage), kb * BK, t.m0 + r);
+                        for (int r = 0; r < SLICE; r += BBOX)
                             tma_load_2d(a_dst + A_BYTES + (uint32_t)r * 128u, &tmap_b, full_bar(stage), kb * BK, t.n0 + r);
                     } else {
-                        if (rank == 0) mbar_expect_tx(full_bar(stage), bytes);
-                        const uint32_t lead_bar = map_to_cta(full_bar(stage), 0);
-                        tma_load_2d_pair(a_dst, &tmap_a, lead_bar, kb * BK, t.m0);
-                        for (int r = 0; r < slice; r += BBOX)
-                            tma_load_2d_pair(a_dst + A_BYTES + (uint32_t)r * 128u, &tmap_b, lead_bar, kb * BK, t.n0 + rank * slice + r);
+                        if (leader) mbar_expect_tx(full_bar(stage), BYTES);
+                        const uint32_t lead_bar = map_to_cta(full_bar(stage), (uint32_t)lead);
+                        if (NP == 1) {
+                            for (int r = 0; r < BM; r += BBOX)
+                                tma_load_2d_pair(a_dst + (uint32_t)r * 128u, &tmap_a, lead_bar, kb * BK, t.m0 + r);
+                        } else {                                                  // my half of the A rows, to both pairs
+                            static_assert(BM / 2 == BBOX, "one box per half of the A rows");
+                            const int half_rows = (rank / CG) * (BM / 2);
+                            const uint16_t mask = (uint16_t)((1u << (rank % CG)) | (1u << (rank % CG + CG)));
+                            tma_load_2d_pair_mc(a_dst + (uint32_t)half_rows * 128u, &tmap_a, lead_bar, kb * BK, t.m0 + half_rows, mask);
+                        }
+                        for (int r = 0; r < SLICE; r += BBOX)
+                            tma_load_2d_pair(a_dst + A_BYTES + (uint32_t)r * 128u, &tmap_b, lead_bar, kb * BK,
+                                             t.n0 + (rank % CG) * SLICE + r);
                     }
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
@@ -272,11 +293,12 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
         }
     } else if (warp == 1) {
         // ===== MMA issuer (one thread; pair mode: the leader CTA only) =====
-        if (lane == 0 && rank == 0) {
+        if (lane == 0 && leader) {
             int stage = 0; uint32_t phase = 0; int it = 0;
-            for (int u = cluster_id; u < sched.num_units; u += num_clusters, ++it) {
-                const Unit t = sched.get(u, CG, rank);
-                const uint32_t idesc = make_idesc(BM * CG, t.ncols);
+            constexpr uint32_t idesc = make_idesc(BM * CG, BN);
+            constexpr uint16_t ALL = (uint16_t)((1u << CSIZE) - 1u);
+            const uint16_t mine = (uint16_t)(((1u << CG) - 1u) << lead);
+            for (int u = cluster_id; u < units; u += num_clusters, ++it) {
                 const int as = it & 1;
                 const uint32_t aphase = (uint32_t)(it >> 1) & 1u;
                 mbar_wait(tempty_bar(as), aphase ^ 1u);                           // every epilogue warp has drained this accumulator
@@ -292,10 +314,10 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
                         if (CG == 1) tc_mma(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)((kb | k) != 0));
                         else tc_mma_pair(d_tmem, adesc + (uint64_t)(2 * k), bdesc + (uint64_t)(2 * k), idesc, (uint32_t)((kb | k) != 0));
                     }
-                    if (CG == 1) tc_commit(empty_bar(stage)); else tc_commit_pair(empty_bar(stage));   // slot free (both CTAs)
+                    if (CG == 1) tc_commit(empty_bar(stage)); else tc_commit_pair(empty_bar(stage), ALL);   // slot free, to every CTA of the cluster
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
-                if (CG == 1) tc_commit(tfull_bar(as)); else tc_commit_pair(tfull_bar(as));             // accumulator complete
+                if (CG == 1) tc_commit(tfull_bar(as)); else tc_commit_pair(tfull_bar(as), mine);       // accumulator complete (own pair)
             }
         }
     } else if (warp >= EPI_WARP0) {
@@ -305,16 +327,80 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
         const int half = ew >> 2;                           // which half of the tile's columns
         const uint32_t tstep = (args.st ? args.st->t : 0u) + args.t_off;
         int it = 0;
-        for (int u = cluster_id; u < sched.num_units; u += num_clusters, ++it) {
-            const Unit t = sched.get(u, CG, rank);
+        for (int u = cluster_id; u < units; u += num_clusters, ++it) {
+            const Unit t = get_unit(u, args.B, CG, NP, rank);
             const int as = it & 1;
             const uint32_t aphase = (uint32_t)(it >> 1) & 1u;
             const int b = t.m0 + lane_grp * 32 + lane;                            // restart owned by this thread
-            const int hcols = t.ncols >> 1;                                       // 128 or 64 columns per warpgroup
+            constexpr int hcols = BN / 2;                                         // 128 columns per warpgroup
             mbar_wait(tfull_bar(as), aphase);
             tc_fence_after();
             double score = 0.0;
-            for (int cb = 0; cb < hcols / 32; ++cb) {
+            if (MODE == MODE_STEP) {
+                // Rounds of 16 variables: 32 loads, 16 updates in registers, 32 + 2 stores.  (Keeping the loads of round
+                // r+1 in flight during round r -- two register buffers -- measured no faster: the epilogue is bound by
+                // the L2 bandwidth it shares with the operand feed, not by load latency.)
+                const int c_first = half * hcols;                                 // this warpgroup's first column in the tile
+                float* __restrict__ xp = args.x + (size_t)(t.n0 + c_first) * args.B + b;
+                float* __restrict__ yp = args.y + (size_t)(t.n0 + c_first) * args.B + b;
+                uint4* zdst = reinterpret_cast<uint4*>(args.zt_out + (size_t)b * args.n + t.n0 + c_first);
+                const uint32_t trow = tmem_base + ((uint32_t)(lane_grp * 32) << 16) + (uint32_t)(as * BN + c_first);
+                const int rounds = hcols / 16;
+                float xa[16], ya[16];
+                auto load16 = [&](float (&xv)[16], float (&yv)[16], int r) {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        xv[j] = xp[(size_t)(16 * r + j) * args.B];
+                        yv[j] = yp[(size_t)(16 * r + j) * args.B];
+                    }
+                };
+                auto round16 = [&](float (&xv)[16], float (&yv)[16], int r) {
+                    uint32_t acc[16];
+                    tc_ld16(trow + (uint32_t)(16 * r), acc);
+                    // constant part of the gradient: lane j (mod 16) fetches column j of the round, broadcast by shuffle
+                    // (a per-element load would sit between the stores and serialise: x, y and hvec may alias)
+                    const float hv = __ldg(args.hvec + t.n0 + c_first + 16 * r + (lane & 15));
+                    tc_wait_ld();
+                    // Eq. 6 for 16 elements as independent, branch-free chains; the (rare) perturbation of reading R3 is
+                    // applied afterwards behind ONE test -- a branch per element serialises the loop
+                    float xt[16];
+                    uint32_t band = 0u;
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        const float G = fmaf(2.0f, __uint_as_float(acc[j]), __shfl_sync(0xffffffffu, hv, j));
+                        gda_update_nopert<GFUN>(xv[j], yv[j], G, args.up, xt[j], yv[j]);
+                        band |= gda_in_band(xv[j], xt[j], args.up.delta) ? (1u << j) : 0u;
+                    }
+                    if (band) {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)
+                            if (band & (1u << j))
+                                xt[j] = gda_perturb(xv[j], xt[j], args.up.delta, args.up.seed_mix, tstep,
+                                                    (uint32_t)(t.n0 + c_first + 16 * r + j), (uint32_t)b);
+                    }
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        xp[(size_t)(16 * r + j) * args.B] = xt[j];
+                        yp[(size_t)(16 * r + j) * args.B] = yv[j];
+                    }
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) {
+                        uint32_t pk[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const __nv_bfloat162 z2 = __floats2bfloat162_rn(xt[8 * q + 2 * e] - 0.5f, xt[8 * q + 2 * e + 1] - 0.5f);
+                            pk[e] = *reinterpret_cast<const uint32_t*>(&z2);
+                        }
+                        zdst[2 * r + q] = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                    }
+                };
+#pragma unroll 1
+                for (int r = 0; r < rounds; ++r) {
+                    load16(xa, ya, r);
+                    round16(xa, ya, r);
+                }
+            }
+            for (int cb = 0; MODE != MODE_STEP && cb < hcols / 32; ++cb) {
                 const int col0 = half * hcols + cb * 32;
                 const int i0 = t.n0 + col0;
                 uint32_t acc[32];
@@ -323,54 +409,7 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
                 // (a per-element load would sit between the stores below and serialise the loop: the compiler must
                 // assume that x, y and hvec alias)
                 const float hv = __ldg(args.hvec + i0 + lane);
-                if (MODE == MODE_STEP) {
-                    float* __restrict__ xp = args.x + (size_t)i0 * args.B + b;
-                    float* __restrict__ yp = args.y + (size_t)i0 * args.B + b;
-                    uint4* zdst = reinterpret_cast<uint4*>(args.zt_out + (size_t)b * args.n + i0);
-                    tc_wait_ld();
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {                                 // 16 columns at a time: loads, updates, stores
-                        float xv[16], yv[16];
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) {
-                            xv[j] = xp[(size_t)(16 * h + j) * args.B];
-                            yv[j] = yp[(size_t)(16 * h + j) * args.B];
-                        }
-                        // Eq. 6 for the 16 elements as independent, branch-free chains; the (rare) perturbation of
-                        // reading R3 is applied afterwards behind ONE test -- a branch per element serialises the loop
-                        float xt[16];
-                        uint32_t band = 0u;
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) {
-                            const float G = fmaf(2.0f, __uint_as_float(acc[16 * h + j]), __shfl_sync(0xffffffffu, hv, 16 * h + j));
-                            gda_update_nopert<GFUN>(xv[j], yv[j], G, args.up, xt[j], yv[j]);
-                            band |= gda_in_band(xv[j], xt[j], args.up.delta) ? (1u << j) : 0u;
-                        }
-                        if (band) {
-#pragma unroll
-                            for (int j = 0; j < 16; ++j)
-                                if (band & (1u << j))
-                                    xt[j] = gda_perturb(xv[j], xt[j], args.up.delta, args.up.seed_mix, tstep, (uint32_t)(i0 + 16 * h + j), (uint32_t)b);
-                        }
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) xv[j] = xt[j];
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) {
-                            xp[(size_t)(16 * h + j) * args.B] = xv[j];
-                            yp[(size_t)(16 * h + j) * args.B] = yv[j];
-                        }
-#pragma unroll
-                        for (int q = 0; q < 2; ++q) {
-                            uint32_t pk[4];
-#pragma unroll
-                            for (int e = 0; e < 4; ++e) {
-                                const __nv_bfloat162 z2 = __floats2bfloat162_rn(xv[8 * q + 2 * e] - 0.5f, xv[8 * q + 2 * e + 1] - 0.5f);
-                                pk[e] = *reinterpret_cast<const uint32_t*>(&z2);
-                            }
-                            zdst[2 * h + q] = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-                        }
-                    }
-                } else if (MODE == MODE_GRAD) {
+                if (MODE == MODE_GRAD) {
                     tc_wait_ld();
 #pragma unroll
                     for (int j = 0; j < 32; ++j)
@@ -388,20 +427,19 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
                     }
                 }
             }
-            if (MODE == MODE_SCORE) {                       // one partial per 64 variables; a 128-column share fills two slots
-                const int slot = (t.n0 + half * hcols) / 64;
+            if (MODE == MODE_SCORE) {                       // one partial per 128 variables
+                const int slot = (t.n0 + half * hcols) / 128;
                 args.partial[(size_t)slot * args.B + b] = score;
-                if (hcols == 128) args.partial[(size_t)(slot + 1) * args.B + b] = 0.0;
             }
             tc_fence_before();
             __syncwarp();
             if (lane == 0) {                                                      // CG * 8 warps -> accumulator stage free
-                if (CG == 1) mbar_arrive(tempty_bar(as)); else mbar_arrive_cluster(map_to_cta(tempty_bar(as), 0));
+                if (CG == 1) mbar_arrive(tempty_bar(as)); else mbar_arrive_cluster(map_to_cta(tempty_bar(as), (uint32_t)lead));
             }
         }
     }
     tc_fence_before();
-    if (CG > 1) cluster_sync_all(); else __syncthreads();      // no CTA leaves while its peer may still signal or read it
+    if (CSIZE > 1) cluster_sync_all(); else __syncthreads();      // no CTA leaves while its peer may still signal or read it
     if (warp == 2) {
         tc_fence_after();
         if (CG == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
@@ -468,30 +506,41 @@ struct DenseHost {
     bool attr_set = false;
 };
 
+template <int MODE, int GFUN, int CG, int NP>
+gda_status launch_variant(gda_problem* p, const CUtensorMap& ta, const CUtensorMap& tq, const DenseArgs& a, cudaStream_t s) {
+    auto kern = dense_gemm_kernel<MODE, GFUN, CG, NP>;
+    constexpr int CSIZE = CG * NP;
+    static int max_clusters = 0;                              // co-resident clusters of this kernel (1 CTA per SM)
+    cudaLaunchConfig_t cfg = {};
+    cfg.blockDim = dim3(NUM_THREADS); cfg.dynamicSmemBytes = Pipe<CG>::SMEM_BYTES; cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CSIZE; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (max_clusters == 0) {
+        GDA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Pipe<CG>::SMEM_BYTES));
+        max_clusters = p->num_sms / CSIZE;
+        if (CSIZE > 2) {                                      // clusters of 4 do not pack all 148 SMs
+            cfg.gridDim = dim3((unsigned)(max_clusters * CSIZE));
+            int q = 0;
+            GDA_CUDA_TRY(cudaOccupancyMaxActiveClusters(&q, kern, &cfg));
+            if (q > 0 && q < max_clusters) max_clusters = q;
+        }
+    }
+    const int units = (a.B / (BM * CG)) * (a.n / (BN * NP));
+    const int rounds = (units + max_clusters - 1) / max_clusters;
+    const int clusters = (units + rounds - 1) / rounds;       // fewest clusters that still finish in `rounds` rounds
+    cfg.gridDim = dim3((unsigned)(clusters * CSIZE));
+    GDA_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tq, a));
+    return GDA_OK;
+}
+
 template <int MODE, int GFUN>
 gda_status launch_gemm(gda_problem* p, const CUtensorMap& ta, const DenseArgs& a, cudaStream_t s) {
     DenseHost* h = static_cast<DenseHost*>(p->tmap_Q);
-    static bool configured = false;
-    if (!configured) {
-        GDA_CUDA_TRY(cudaFuncSetAttribute(dense_gemm_kernel<MODE, GFUN, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, Pipe<2>::SMEM_BYTES));
-        GDA_CUDA_TRY(cudaFuncSetAttribute(dense_gemm_kernel<MODE, GFUN, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, Pipe<1>::SMEM_BYTES));
-        configured = true;
-    }
-    const bool pair = a.B % (BM * 2) == 0;                   // an odd number of 128-restart blocks runs single CTAs
-    const int cg = pair ? 2 : 1;
-    const int units = (a.B / (BM * cg)) * (a.n / BN);
-    const int max_clusters = p->num_sms / cg;
-    const int clusters = units < max_clusters ? units : max_clusters;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)(clusters * cg)); cfg.blockDim = dim3(NUM_THREADS);
-    cfg.dynamicSmemBytes = pair ? Pipe<2>::SMEM_BYTES : Pipe<1>::SMEM_BYTES; cfg.stream = s;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = (unsigned)cg; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
-    if (pair) GDA_CUDA_TRY(cudaLaunchKernelEx(&cfg, dense_gemm_kernel<MODE, GFUN, 2>, ta, h->tmap_q, a));
-    else GDA_CUDA_TRY(cudaLaunchKernelEx(&cfg, dense_gemm_kernel<MODE, GFUN, 1>, ta, h->tmap_q, a));
-    return GDA_OK;
+    if (a.B % (BM * 2) != 0) return launch_variant<MODE, GFUN, 1, 1>(p, ta, h->tmap_q, a, s);   // odd number of 128-restart blocks
+    if (a.n % (BN * 2) != 0) return launch_variant<MODE, GFUN, 2, 1>(p, ta, h->tmap_q, a, s);
+    return launch_variant<MODE, GFUN, 2, 2>(p, ta, h->tmap_q, a, s);
 }
 
 gda_status z_maps(gda_problem* p, int32_t B, const __nv_bfloat16* zt, const CUtensorMap** out) {
@@ -500,7 +549,7 @@ gda_status z_maps(gda_problem* p, int32_t B, const __nv_bfloat16* zt, const CUte
         if (h->z_ptr[k] == zt && h->z_B == B) { *out = &h->tmap_z[k]; return GDA_OK; }
     if (h->z_B != B) { h->z_ptr[0] = h->z_ptr[1] = nullptr; h->z_B = B; }
     const int k = h->z_ptr[0] == nullptr ? 0 : 1;
-    GDA_TRY(make_tmap(&h->tmap_z[k], zt, (uint64_t)B, (uint64_t)p->n, BM));
+    GDA_TRY(make_tmap(&h->tmap_z[k], zt, (uint64_t)B, (uint64_t)p->n, BBOX));
     h->z_ptr[k] = zt;
     *out = &h->tmap_z[k];
     return GDA_OK;
@@ -575,7 +624,7 @@ gda_status dense_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaS
     return launch_gemm<MODE_GRAD, GDA_G_QUADRATIC>(p, *ta, a, s);
 }
 
-int32_t dense_num_partials(const gda_problem* p, int32_t) { return p->n / 64; }
+int32_t dense_num_partials(const gda_problem* p, int32_t) { return p->n / 128; }
 
 // S5: x_hat operand (exact in bf16), GEMM, per-thread column sums.  Scratch: the zt buffer NOT holding the current operand.
 gda_status dense_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,

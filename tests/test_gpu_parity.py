@@ -398,10 +398,10 @@ TOL_GRAD_BF16 = 1e-2
 
 
 def dense_workloads():
-    # (n, B) = (256, 128) one tile; (512, 384) unclustered half tiles; (1024, 256) clustered half tiles;
-    # (2560, 1024) clustered full tiles (40 units on 74 clusters: no split)
+    # (n, B): (256, 128) one single-CTA tile; (512, 384) single CTAs; (1024, 256) and (2560, 1024) clusters of two CTA
+    # pairs with the A multicast (1 and 4 units per cluster); (768, 256) CTA pairs without the multicast
     return [wl.config(4, B=128, n_scale=0.0625), wl.config(4, B=384, n_scale=0.125), wl.config(4, B=256, n_scale=0.25),
-            wl.config(4, B=1024, n_scale=0.625)]
+            wl.config(4, B=1024, n_scale=0.625), wl.config(4, B=256, n_scale=0.1875)]
 
 
 DENSE = dense_workloads()
