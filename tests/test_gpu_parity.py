@@ -260,12 +260,33 @@ def degree_ladder_qubo(n_groups, seed):
     return wl.QuboCSR(n, np.array(rowptr, np.int32), np.array(col, np.int32), np.array(val, np.float32), c)
 
 
-@pytest.mark.parametrize("case", ["star_isolated", "general_int", "general_float", "n1", "packed_rows"])
+def dense_rows_qubo(n, seed):
+    """Small n, high degree: row degrees from 0 to about 120, so that rows are served by one, two and more than two
+    32-entry batches of the CSR path."""
+    rng = np.random.default_rng(seed)
+    prob = np.minimum(1.0, np.linspace(0.0, 1.6, n)[:, None] * np.linspace(1.0, 0.3, n)[None, :])
+    A = np.triu((rng.random((n, n)) < prob) * rng.integers(1, 4, size=(n, n)), 1).astype(np.float32)
+    A[0, :] = 0                                          # an empty row
+    Q = A + A.T
+    rowptr, col, val = [0], [], []
+    for i in range(n):
+        nz = np.nonzero(Q[i])[0]
+        col += list(nz)
+        val += list(Q[i, nz])
+        rowptr.append(len(col))
+    c = rng.integers(-3, 4, size=n).astype(np.float32)
+    return wl.QuboCSR(n, np.array(rowptr, np.int32), np.array(col, np.int32), np.array(val, np.float32), c)
+
+
+@pytest.mark.parametrize("case", ["star_isolated", "general_int", "general_float", "n1", "packed_rows", "long_rows"])
 def test_sparse_edge_cases(api, oracle, case):
     if case == "star_isolated":
         Pw, B = star_plus_isolated(700, 5), 8
     elif case == "packed_rows":
         Pw, B = degree_ladder_qubo(3, 5), 132
+    elif case == "long_rows":
+        Pw, B = dense_rows_qubo(301, 8), 76
+        assert Pw.rowptr[-1] >= 8 * Pw.n and (Pw.rowptr[1:] - Pw.rowptr[:-1]).max() > 64
     elif case == "general_int":
         Pw, B = general_qubo_csr(37, 1, True), 4
     elif case == "general_float":
@@ -280,7 +301,8 @@ def test_sparse_edge_cases(api, oracle, case):
     rng = np.random.default_rng(9)
     X = rng.random((n, B), dtype=np.float32)
     assert grad_rel_err(P.grad(dev(X)).cpu().numpy(), oracle.grad(OP, X.astype(np.float64))) <= TOL_STEP
-    h = wl.Hyper(3.0, 0.004 if case == "star_isolated" else 0.02, 0.05, 1e-4, 0, 1e-6, 333, 7, 77)   # odd eval_every
+    alpha = {"star_isolated": 0.004, "long_rows": 0.002}.get(case, 0.02)
+    h = wl.Hyper(3.0, alpha, 0.05, 1e-4, 0, 1e-6, 333, 7, 77)   # odd eval_every
     r = P.run(dev(X), 3.0, api.params_from_hyper(h), want_final=True)
     ref = oracle.run(OP, X, 3.0, **okw(h, iters=1, eval_every=1))
     r1 = P.run(dev(X), 3.0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
