@@ -26,6 +26,7 @@ _SRC = _HERE / "pdbo_oracle.c"
 
 KIND_QUBO_CSR, KIND_QUBO_DENSE, KIND_MAXSAT = 0, 1, 2
 G_QUADRATIC, G_ENTROPY = 0, 1
+DUAL_PER_VARIABLE, DUAL_SCALAR = 0, 1
 
 
 class _Problem(C.Structure):
@@ -38,7 +39,7 @@ class _Problem(C.Structure):
 class _Params(C.Structure):
     _fields_ = [("alpha", C.c_double), ("beta", C.c_double), ("delta", C.c_double),
                 ("log_eps", C.c_double), ("gfun", C.c_int32), ("iters", C.c_int32),
-                ("eval_every", C.c_int32), ("t0", C.c_int32), ("seed", C.c_uint64)]
+                ("eval_every", C.c_int32), ("t0", C.c_int32), ("seed", C.c_uint64), ("dual", C.c_int32)]
 
 
 def build(force: bool = False) -> None:
@@ -150,16 +151,20 @@ def F_binary(P: Problem, Xh: np.ndarray) -> np.ndarray:
 
 def run(P: Problem, X0: np.ndarray, Y0, *, alpha: float, beta: float, delta: float = 1e-4,
         gfun: int = G_QUADRATIC, log_eps: float = 1e-6, iters: int, eval_every: int, seed: int = 0,
-        t0: int = 0, col_ids: Optional[np.ndarray] = None, precision: str = "f64", nthreads: int = 1):
+        t0: int = 0, col_ids: Optional[np.ndarray] = None, precision: str = "f64", nthreads: int = 1,
+        dual: int = DUAL_PER_VARIABLE):
     """Algorithm 1 for every column of X0.  Y0 is an [n][B] array or a scalar (y-bar).
-    Returns dict(x_bin, obj, best_restart, x, y)."""
+    dual = DUAL_SCALAR runs PDBO-s (reading R14): one multiplier per restart, Y0 a scalar or a
+    [B] array, and the returned y is [B].  Returns dict(x_bin, obj, best_restart, x, y)."""
     rt = _real(precision)
     X0 = np.ascontiguousarray(X0, dtype=rt)
     n, B = X0.shape
     assert n == P.n
+    if dual == DUAL_SCALAR and not np.isscalar(Y0):
+        Y0 = np.broadcast_to(np.asarray(Y0, dtype=rt).reshape(1, B), (n, B))
     Y0a = np.full((n, B), Y0, dtype=rt) if np.isscalar(Y0) else np.ascontiguousarray(Y0, dtype=rt)
     assert Y0a.shape == (n, B)
-    hp = _Params(alpha, beta, delta, log_eps, gfun, iters, eval_every, t0, seed)
+    hp = _Params(alpha, beta, delta, log_eps, gfun, iters, eval_every, t0, seed, dual)
     x_bin = np.zeros((n, B), dtype=np.uint8)
     obj = np.empty(B, dtype=np.float64)
     best = C.c_int32(-1)
@@ -171,6 +176,9 @@ def run(P: Problem, X0: np.ndarray, Y0, *, alpha: float, beta: float, delta: flo
         C.c_void_p(x_bin.ctypes.data), C.c_void_p(obj.ctypes.data), C.byref(best),
         C.c_void_p(Xf.ctypes.data), C.c_void_p(Yf.ctypes.data), C.c_int32(nthreads))
     assert rc == 0
+    if dual == DUAL_SCALAR:
+        assert (Yf == Yf[0:1]).all()                     # the multiplier stays one number per restart
+        Yf = Yf[0].copy()
     return dict(x_bin=x_bin, obj=obj, best_restart=int(best.value), x=Xf, y=Yf)
 
 

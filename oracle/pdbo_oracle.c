@@ -1,7 +1,7 @@
 /* oracle/pdbo_oracle.c -- CPU ORACLE for PDBO (arxiv 2509.21064).  TEST INFRASTRUCTURE ONLY.
  *
  * A plain, slow, obviously-correct implementation of what the hot path computes, written from
- * /root/reference/PAPER.md and the readings R0-R13 listed in DESIGN.md.  It shares no code with the
+ * /root/reference/PAPER.md and the readings R0-R14 listed in DESIGN.md.  It shares no code with the
  * CUDA library; only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
  * legs may build, load or call it.  No blocking, fusion or reordering beyond what the paper states.
  *
@@ -10,7 +10,8 @@
  *
  * Parity pins (tests/test_oracle_pins.py): F by brute force and edge list; f by Def. 2.2 enumeration;
  * grad f by multilinearity; the Max-Cut fixed point at 1/2; Hessian 2(W+diag y)
- * (PAPER.md:606); step invariants; convex special case; 2^20 brute force.
+ * (PAPER.md:606); step invariants; convex special case; 2^20 brute force;
+ * PDBO-s: finite differences of L_s in x and mu, n = 1 equals PDBO, the multiplier stays one number per restart.
  * Unpinned: optimality of the objective reached on configs 2-5 (no optimum known) -- see DESIGN.md.
  *
  * Layout: iterates are [n][B] row-major (restart index contiguous), as at the library's C ABI.
@@ -34,6 +35,8 @@ typedef REAL real;
 #define KIND_MAXSAT 2
 #define G_QUADRATIC 0
 #define G_ENTROPY 1
+#define DUAL_PER_VARIABLE 0
+#define DUAL_SCALAR 1
 
 /* Problem data, all host pointers owned by the caller.
  * QUBO: F(x) = x^T Q x + c^T x for ANY square Q (diagonal and asymmetry allowed here; reading R1).
@@ -203,23 +206,30 @@ typedef struct {
     int32_t eval_every;   /* round + score every this many steps and at the end (R5) */
     int32_t t0;           /* iteration index of x0 (enters the tie-break hash only) */
     uint64_t seed;
+    int32_t dual;         /* DUAL_PER_VARIABLE (PDBO, Eq. 6) | DUAL_SCALAR (PDBO-s; reading R14) */
 } pdbo_params;
 
 /* ---- one simultaneous projected GDA step, Eq. (6) + perturbation (148, 732) --- */
 /* x, y: time-t values (contiguous, one restart).  xn, yn: time-(t+1) values.  G: scratch [n].        */
+/* PDBO-s (the single constraint sum_i g(x_i) = 0 with one multiplier mu; reading R14):     */
+/*   L_s(x, mu) = f(x) + mu sum_i g(x_i);  x+ = clip(x - alpha (grad f + mu g'(x)));  mu+ = mu + beta sum_i g(x_i) */
+/* mu is kept replicated in y[0..n): every entry receives the same increment.                               */
 static void gda_step(const pdbo_problem* P, const pdbo_params* hp, uint32_t t, uint32_t b,
                      const real* x, const real* y, real* xn, real* yn, real* G) {
     const int n = P->n;
     const real alpha = (real)hp->alpha, beta = (real)hp->beta, delta = (real)hp->delta;
     const real half = (real)0.5;
     grad_f(P, x, G);
+    real gsum = (real)0;                                       /* PDBO-s: grad_mu L_s = sum_i g(x_i^t), index order */
+    if (hp->dual == DUAL_SCALAR)
+        for (int i = 0; i < n; ++i) gsum += g_fun(hp->gfun, x[i]);
     for (int i = 0; i < n; ++i) {
         const real gp = g_prime(hp->gfun, x[i], (real)hp->log_eps);
         const real gv = g_fun(hp->gfun, x[i]);
         real xt = x[i] - alpha * (G[i] + y[i] * gp);           /* x - alpha * grad_x L          */
         if (xt < (real)0) xt = (real)0;                        /* projection onto [0,1]         */
         if (xt > (real)1) xt = (real)1;
-        yn[i] = y[i] + beta * gv;                              /* y + beta * grad_y L, uses x^t */
+        yn[i] = y[i] + beta * (hp->dual == DUAL_SCALAR ? gsum : gv);   /* y + beta * grad_y L, uses x^t */
         if (delta > (real)0 && fabs((double)(x[i] - half)) < (double)delta
                             && fabs((double)(xt - half)) < (double)delta) {
             int s;                                             /* R3: two successive in-band iterates */

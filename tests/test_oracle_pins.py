@@ -372,3 +372,68 @@ def test_scaled_configs_beat_random_assignment(oracle, idx, scale):
     rnd = oracle.F_binary(OP, (np.random.default_rng(0).random((w.problem.n, 64)) < 0.5).astype(np.uint8))
     assert np.array_equal(r["obj"], oracle.F_binary(OP, r["x_bin"]))
     assert r["obj"].max() < rnd.min()           # every restart beats the best of 64 random assignments
+
+
+# ---------------------------------------------------------------------------------------------
+# PDBO-s (reading R14): one multiplier mu per restart for the single constraint
+# sum_i g(x_i) = 0.  Pinned by finite differences of L_s(x, mu) = f(x) + mu sum_i g(x_i), with f from the
+# oracle's f_ext (itself pinned against Def. 2.2 above) and g typed out here.
+# ---------------------------------------------------------------------------------------------
+def _g_closed_form(gfun, x):
+    if gfun == 0:
+        return x * x - x
+    return x * np.log(x) + (1.0 - x) * np.log(1.0 - x)
+
+
+@pytest.mark.parametrize("gfun", [0, 1])
+@pytest.mark.parametrize("kind", ["qubo_csr", "maxsat"])
+def test_pdbo_s_step_is_gda_on_the_single_constraint_lagrangian(oracle, kind, gfun):
+    n = 6
+    rng = np.random.default_rng(17)
+    if kind == "maxsat":
+        P = oracle_problem(wl.random_ksat(n, 10, 3, 5))
+    else:
+        Q, c, rowptr, col, val = random_general_qubo(n, 4)
+        P = oracle.Problem.qubo_csr(n, rowptr, col, val, c)
+    x = 0.2 + 0.6 * rng.random(n)                               # interior: no clipping with a small step
+    mu, alpha, beta = 1.7, 1e-4, 0.3
+    Ls = lambda z, m: oracle.f_ext(P, z.reshape(n, 1))[0] + m * _g_closed_form(gfun, z).sum()
+    r = oracle.run(P, x.reshape(n, 1), mu, alpha=alpha, beta=beta, delta=0.0, gfun=gfun, iters=1, eval_every=1,
+                   dual=oracle.DUAL_SCALAR)
+    assert r["y"].shape == (1,)
+    grad_x = (x - r["x"][:, 0]) / alpha                          # x+ = x - alpha grad_x L_s
+    h = 1e-6
+    for i in range(n):
+        e = np.zeros(n); e[i] = h
+        assert grad_x[i] == pytest.approx((Ls(x + e, mu) - Ls(x - e, mu)) / (2 * h), rel=1e-6, abs=1e-6)
+    # mu+ = mu + beta dL_s/dmu = mu + beta sum_i g(x_i), from the time-t point
+    assert (r["y"][0] - mu) / beta == pytest.approx(_g_closed_form(gfun, x).sum(), rel=1e-12)
+    assert (r["y"][0] - mu) / beta == pytest.approx((Ls(x, mu + h) - Ls(x, mu - h)) / (2 * h), rel=1e-6)
+
+
+def test_pdbo_s_with_one_variable_is_pdbo(oracle):
+    P = oracle.Problem.qubo_csr(1, np.array([0, 1], np.int32), np.array([0], np.int32), np.array([-2.0]), np.array([1.5]))
+    X0 = np.array([[0.3, 0.5, 0.77, 0.5001]])
+    kw = dict(alpha=0.02, beta=0.05, delta=1e-4, gfun=0, iters=40, eval_every=7, seed=3)
+    a = oracle.run(P, X0, 2.0, **kw)
+    b = oracle.run(P, X0, 2.0, dual=oracle.DUAL_SCALAR, **kw)
+    assert np.array_equal(a["x"], b["x"]) and np.array_equal(a["y"][0], b["y"]) and np.array_equal(a["obj"], b["obj"])
+
+
+def test_pdbo_s_multiplier_is_shared_and_non_increasing(oracle):
+    w = wl.config(3, B=4, n_scale=0.02)
+    n = w.problem.n
+    OP = oracle_problem(w.problem)
+    X0 = wl.x0_uniform(n, 4, 9)
+    kw = hyper_kwargs(w.hyper, beta=w.hyper.beta / n)
+    mus, prev = [np.full(4, 6.0)], None
+    X, mu = X0.astype(np.float64), np.full(4, 6.0)
+    for t in range(30):
+        r = oracle.run(OP, X, mu, dual=oracle.DUAL_SCALAR, **dict(kw, iters=1, eval_every=1, t0=t))
+        gsum = (X * X - X).sum(axis=0)                           # quadratic g, typed out
+        assert np.allclose(r["y"] - mu, kw["beta"] * gsum, rtol=1e-12, atol=1e-15)
+        assert np.all(r["y"] <= mu) and np.all(r["y"] - mu >= -kw["beta"] * n / 4 - 1e-15)   # g in [-1/4, 0]
+        X, mu = r["x"], r["y"]
+    # one call of 30 steps is the same trajectory
+    full = oracle.run(OP, X0, 6.0, dual=oracle.DUAL_SCALAR, **dict(kw, iters=30, eval_every=10))
+    assert np.array_equal(full["x"], X) and np.array_equal(full["y"], mu)
