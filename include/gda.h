@@ -78,6 +78,14 @@ gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cptr, const in
 void gda_destroy(gda_problem* p); /* NULL-safe; synchronises the device before freeing */
 
 /* ---- the run ----------------------------------------------------------------------------------------- */
+/* Dual variables.  GDA_DUAL_PER_VARIABLE is the paper's method, one multiplier y_i per constraint g(x_i) = 0
+ * (Eq. 6).  GDA_DUAL_SCALAR is the ablation "PDBO-s": the single
+ * constraint sum_i g(x_i) = 0 with one multiplier mu per restart,
+ *     x+ = clip(x - alpha (grad f(x) + mu g'(x))),   mu+ = mu + beta sum_i g(x_i)      (reading R14)
+ * the sum accumulated in fp32 in a fixed order (deterministic).  In this mode lambda0 and lambda_final are
+ * DEVICE fp32 [B] (HOST [B] for gda_run_host).  Sparse QUBO and MaxSAT problems only (dense: UNSUPPORTED). */
+typedef enum { GDA_DUAL_PER_VARIABLE = 0, GDA_DUAL_SCALAR = 1 } gda_dual;
+
 typedef struct {
     float alpha;        /* primal step size > 0                                          */
     float beta;         /* dual step size > 0                                          */
@@ -88,12 +96,14 @@ typedef struct {
     int32_t gfun;       /* gda_gfun                                                                     */
     int32_t t0;         /* iteration index of x0 (only enters the exact-1/2 tie-break hash, R3)         */
     uint64_t seed;      /* seed of that hash                                                            */
+    int32_t dual;       /* gda_dual: per-variable multipliers (PDBO) or one per restart (PDBO-s)        */
+    int32_t reserved;   /* must be 0                                                                    */
 } gda_params;
 
 /* Optional extra outputs of gda_run; every pointer is DEVICE memory and may be NULL. */
 typedef struct {
     float* x_final;       /* [n][B] iterate x^T                                                         */
-    float* lambda_final;  /* [n][B] dual iterate y^T                                                    */
+    float* lambda_final;  /* [n][B] dual iterate y^T  ([B] with GDA_DUAL_SCALAR)                        */
     double* best_obj;     /* [1]    obj[best_restart]                                                   */
     double* trace_best;   /* [trace_cap] min over restarts of the best objective after evaluation k     */
     uint64_t* trace_ns;   /* [trace_cap] GPU globaltimer (ns) when evaluation k finished                */
@@ -104,13 +114,14 @@ typedef struct {
  *   x0          DEVICE fp32 [n][B], values in [0,1]           (x0 ~ U[0,1]^n); or NULL to RESUME:
  *               continue from the iterates, duals, iteration counter and best-so-far that the previous
  *               gda_run on this handle (same B) left in it -- lambda0 and params->t0 are then ignored
- *   lambda0     DEVICE fp32 [n][B] or NULL -> every entry = lambda0_scalar (y-bar)
+ *   lambda0     DEVICE fp32 [n][B] ([B] with GDA_DUAL_SCALAR) or NULL -> every entry = lambda0_scalar (y-bar)
  *   x_bin       DEVICE uint8 [n][B]: per restart, the rounded point x_hat = [x > 1/2] with the best
  *               objective seen at any evaluation (R5)
  *   obj         DEVICE double [B]: F(x_bin[:,b]) -- exact integers when all coefficients are integers
  *   best_restart DEVICE int32 [1]: argmin_b obj[b], ties -> lowest b (R6)
  * INVALID_ARG: null required pointer, B <= 0 or B % 4 != 0, alpha/beta <= 0 or non-finite, delta outside
- * [0, 1/2), eval_every <= 0, iters < 0, unknown gfun, log_eps outside (0, 1/2) with the entropy g.       */
+ * [0, 1/2), eval_every <= 0, iters < 0, unknown gfun or dual, log_eps outside (0, 1/2) with the entropy g;
+ * a resumed run (x0 == NULL) whose `dual` differs from the run it continues.                              */
 gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const float* lambda0, float lambda0_scalar,
                    const gda_params* params, uint8_t* x_bin, double* obj, int32_t* best_restart,
                    const gda_extra* extra, void* stream);

@@ -17,6 +17,7 @@ _lib = None
 
 STATUS = {0: "GDA_OK", 1: "GDA_ERR_INVALID_ARG", 2: "GDA_ERR_ALLOC", 3: "GDA_ERR_CUDA", 4: "GDA_ERR_UNSUPPORTED"}
 G_QUADRATIC, G_ENTROPY = 0, 1
+DUAL_PER_VARIABLE, DUAL_SCALAR = 0, 1
 DENSE_BF16 = 1
 
 
@@ -29,7 +30,7 @@ class GdaError(RuntimeError):
 class Params(C.Structure):
     _fields_ = [("alpha", C.c_float), ("beta", C.c_float), ("delta", C.c_float), ("log_eps", C.c_float),
                 ("iters", C.c_int32), ("eval_every", C.c_int32), ("gfun", C.c_int32), ("t0", C.c_int32),
-                ("seed", C.c_uint64)]
+                ("seed", C.c_uint64), ("dual", C.c_int32), ("reserved", C.c_int32)]
 
 
 class Extra(C.Structure):
@@ -88,8 +89,9 @@ def _hp(a):
     return None if a is None else a.ctypes.data
 
 
-def make_params(alpha, beta, delta=1e-4, log_eps=1e-6, iters=0, eval_every=100, gfun=G_QUADRATIC, t0=0, seed=0) -> Params:
-    return Params(alpha, beta, delta, log_eps, iters, eval_every, gfun, t0, seed)
+def make_params(alpha, beta, delta=1e-4, log_eps=1e-6, iters=0, eval_every=100, gfun=G_QUADRATIC, t0=0, seed=0,
+                dual=DUAL_PER_VARIABLE) -> Params:
+    return Params(alpha, beta, delta, log_eps, iters, eval_every, gfun, t0, seed, dual, 0)
 
 
 class Problem:
@@ -134,7 +136,7 @@ class Problem:
 
     # ---- gda_run --------------------------------------------------------------------------------
     def run(self, x0, lambda0, params: Params, *, want_final=False, trace_cap=0, stream=None):
-        """x0: CUDA float32 tensor [n][B]; lambda0: tensor [n][B] or a float (y-bar).
+        """x0: CUDA float32 tensor [n][B]; lambda0: tensor [n][B] ([B] with params.dual = DUAL_SCALAR) or a float (y-bar).
         Returns dict of CUDA tensors: x_bin, obj, best_restart (+ x, lam, best_obj, trace_best, trace_ns).
         Asynchronous on `stream` (default: torch's current stream)."""
         import torch
@@ -144,7 +146,8 @@ class Problem:
         self._last = (n, B, dev)
         l_ptr, l_scalar = None, 0.0
         if isinstance(lambda0, torch.Tensor):
-            assert lambda0.is_cuda and lambda0.dtype == torch.float32 and lambda0.is_contiguous() and lambda0.shape == x0.shape
+            assert lambda0.is_cuda and lambda0.dtype == torch.float32 and lambda0.is_contiguous()
+            assert lambda0.shape == ((B,) if params.dual == DUAL_SCALAR else x0.shape)
             l_ptr = lambda0.data_ptr()
         else:
             l_scalar = float(lambda0)
@@ -154,7 +157,7 @@ class Problem:
         ex = Extra()
         if want_final:
             out["x"] = torch.empty_like(x0)
-            out["lam"] = torch.empty_like(x0)
+            out["lam"] = torch.empty(B, dtype=torch.float32, device=dev) if params.dual == DUAL_SCALAR else torch.empty_like(x0)
             out["best_obj"] = torch.empty(1, dtype=torch.float64, device=dev)
             ex.x_final, ex.lambda_final, ex.best_obj = out["x"].data_ptr(), out["lam"].data_ptr(), out["best_obj"].data_ptr()
         if trace_cap > 0:
@@ -235,6 +238,6 @@ def create_from_workload(P) -> Problem:
 
 def params_from_hyper(h, **over) -> Params:
     d = dict(alpha=h.alpha, beta=h.beta, delta=h.delta, log_eps=h.log_eps, iters=h.iters,
-             eval_every=h.eval_every, gfun=h.gfun, t0=0, seed=h.seed)
+             eval_every=h.eval_every, gfun=h.gfun, t0=0, seed=h.seed, dual=getattr(h, "dual", DUAL_PER_VARIABLE))
     d.update(over)
     return make_params(**d)

@@ -291,6 +291,7 @@ static void free_workspace(gda_problem* p) {
     cudaFree(ws.obj_now); cudaFree(ws.improved); cudaFree(ws.partial); cudaFree(ws.state);
     cudaFree(ws.best_restart); cudaFree(ws.best_val); cudaFree(ws.trace_best); cudaFree(ws.trace_ns);
     cudaFree(ws.zt[0]); cudaFree(ws.zt[1]); cudaFree(ws.gtmp);
+    cudaFree(ws.mu[0]); cudaFree(ws.mu[1]); cudaFree(ws.ginc); cudaFree(ws.gpart);
     if (ws.h_x0) cudaFreeHost(ws.h_x0);
     if (ws.h_l0) cudaFreeHost(ws.h_l0);
     ws = Workspace();
@@ -353,6 +354,13 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     if (st == GDA_OK) st = dmalloc(&ws.improved, (size_t)B);
     ws.n_part = num_partials(p, B);
     if (st == GDA_OK) st = dmalloc((double**)&ws.partial, (size_t)ws.n_part * B);
+    if (p->kind != GDA_KIND_DENSE) {                          // PDBO-s state (a few rows of B floats)
+        ws.n_gpart = p->kind == GDA_KIND_SPARSE ? sparse_num_gparts(p) : maxsat_num_gparts(p);
+        if (st == GDA_OK) st = dmalloc(&ws.mu[0], (size_t)B);
+        if (st == GDA_OK) st = dmalloc(&ws.mu[1], (size_t)B);
+        if (st == GDA_OK) st = dmalloc(&ws.ginc, (size_t)GINC_GROUPS * B);
+        if (st == GDA_OK) st = dmalloc(&ws.gpart, (size_t)ws.n_gpart * B);
+    }
     if (st == GDA_OK) st = dmalloc(&ws.state, 1);
     if (st == GDA_OK) st = dmalloc(&ws.best_restart, 1);
     if (st == GDA_OK) st = dmalloc(&ws.best_val, 1);
@@ -402,14 +410,18 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     Workspace& ws = p->ws;
     const UpdParams up = make_upd(prm);
     int cur = parity;
+    const bool scalar = prm.dual == GDA_DUAL_SCALAR;
     for (int k = 0; k < len; ++k) {
         int64_t before = *launches;
+        ScalarDual sd;                                        // PDBO-s: mu follows the parity of x
+        if (scalar) { sd.mu_prev = ws.mu[cur]; sd.ginc = ws.ginc; sd.mu_cur = ws.mu[cur ^ 1]; sd.gpart = ws.gpart; }
         if (p->kind == GDA_KIND_SPARSE)
-            GDA_TRY(sparse_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, ws.state, (uint32_t)k, s, launches));
+            GDA_TRY(sparse_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         else if (p->kind == GDA_KIND_MAXSAT)
-            GDA_TRY(maxsat_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, ws.state, (uint32_t)k, s, launches));
+            GDA_TRY(maxsat_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         else
             GDA_TRY(dense_step(p, B, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, ws.state, (uint32_t)k, s, launches));
+        if (scalar) GDA_TRY(gsum_reduce(B, ws.gpart, ws.n_gpart, prm.beta, ws.ginc, s, launches));
         *step_launches += *launches - before;
         cur ^= 1;
     }
@@ -427,7 +439,7 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
 bool GraphKey::operator==(const GraphKey& o) const {
     return B == o.B && len == o.len && parity == o.parity && with_eval == o.with_eval &&
            prm.alpha == o.prm.alpha && prm.beta == o.prm.beta && prm.delta == o.prm.delta &&
-           prm.log_eps == o.prm.log_eps && prm.gfun == o.prm.gfun && prm.seed == o.prm.seed;
+           prm.log_eps == o.prm.log_eps && prm.gfun == o.prm.gfun && prm.seed == o.prm.seed && prm.dual == o.prm.dual;
 }
 
 static bool graphs_disabled() {
@@ -488,6 +500,13 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
     GDA_REQUIRE(prm->gfun == GDA_G_QUADRATIC || prm->gfun == GDA_G_ENTROPY, "gda_run: unknown gfun %d", prm->gfun);
     if (prm->gfun == GDA_G_ENTROPY)
         GDA_REQUIRE(prm->log_eps > 0.0f && prm->log_eps < 0.5f, "gda_run: log_eps must be in (0, 1/2) for the entropy g");
+    GDA_REQUIRE(prm->dual == GDA_DUAL_PER_VARIABLE || prm->dual == GDA_DUAL_SCALAR, "gda_run: unknown dual mode %d", prm->dual);
+    GDA_REQUIRE(prm->reserved == 0, "gda_run: params->reserved must be 0");
+    GDA_REQUIRE(x0 != nullptr || p->ws.dual == prm->dual, "gda_run: a resumed run must keep the dual mode of the run it continues");
+    if (prm->dual == GDA_DUAL_SCALAR && p->kind == GDA_KIND_DENSE) {
+        gda_set_error("gda_run: GDA_DUAL_SCALAR (PDBO-s) is implemented for sparse QUBO and MaxSAT problems only");
+        return GDA_ERR_UNSUPPORTED;
+    }
     if (p->kind == GDA_KIND_DENSE && B % 128 != 0) {
         gda_set_error("gda_run: the dense path needs B to be a multiple of 128 (got %d)", B);
         return GDA_ERR_UNSUPPORTED;
@@ -514,6 +533,7 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
     int parity = 0;
     if (x0) {
         ws.has_state = false;
+        ws.dual = prm->dual;
         GDA_TRY(run_init(p, B, x0, lambda0, lambda0_scalar, (uint32_t)prm->t0, s, &p->last_launches));
         if (p->kind == GDA_KIND_DENSE)
             GDA_TRY(dense_make_operand(p, B, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
@@ -537,7 +557,10 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
     GDA_CUDA_TRY(cudaMemcpyAsync(best_restart, ws.best_restart, sizeof(int32_t), cudaMemcpyDeviceToDevice, s));
     if (extra) {
         if (extra->x_final) GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, xfin, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
-        if (extra->lambda_final) GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.y, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        if (extra->lambda_final && prm->dual == GDA_DUAL_SCALAR)          // mu^T = mu + pending increment, [B]
+            GDA_TRY(mu_finalize(B, ws.mu[parity], ws.ginc, extra->lambda_final, s, &p->last_launches));
+        else if (extra->lambda_final)
+            GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.y, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
         if (extra->best_obj) GDA_CUDA_TRY(cudaMemcpyAsync(extra->best_obj, ws.best_val, sizeof(double), cudaMemcpyDeviceToDevice, s));
         const int32_t n_eval = std::max(1, full + (rem > 0 ? 1 : 0));
         const int32_t cnt = std::min(std::min(n_eval, extra->trace_cap), ws.trace_cap);
@@ -564,14 +587,15 @@ extern "C" gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, c
     // device staging: x0 -> x[1] would be clobbered by the run, so stage in dedicated buffers
     float* d_x0 = nullptr; float* d_l0 = nullptr; uint8_t* d_xb = nullptr; double* d_obj = nullptr; int32_t* d_best = nullptr;
     gda_status st = dmalloc(&d_x0, elems);
-    if (st == GDA_OK && lambda0) st = dmalloc(&d_l0, elems);
+    const size_t l0_elems = (prm && prm->dual == GDA_DUAL_SCALAR) ? (size_t)B : elems;
+    if (st == GDA_OK && lambda0) st = dmalloc(&d_l0, l0_elems);
     if (st == GDA_OK) st = dmalloc(&d_xb, elems);
     if (st == GDA_OK) st = dmalloc(&d_obj, (size_t)B);
     if (st == GDA_OK) st = dmalloc(&d_best, 1);
     cudaError_t e = cudaSuccess;
     if (st == GDA_OK) {
         e = cudaMemcpyAsync(d_x0, x0, elems * sizeof(float), cudaMemcpyHostToDevice, s);
-        if (e == cudaSuccess && lambda0) e = cudaMemcpyAsync(d_l0, lambda0, elems * sizeof(float), cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess && lambda0) e = cudaMemcpyAsync(d_l0, lambda0, l0_elems * sizeof(float), cudaMemcpyHostToDevice, s);
         if (e == cudaSuccess) st = gda_run(p, B, d_x0, d_l0, lambda0_scalar, prm, d_xb, d_obj, d_best, nullptr, s);
         if (st == GDA_OK && e == cudaSuccess) e = cudaMemcpyAsync(x_bin, d_xb, elems, cudaMemcpyDeviceToHost, s);
         if (st == GDA_OK && e == cudaSuccess) e = cudaMemcpyAsync(obj, d_obj, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, s);

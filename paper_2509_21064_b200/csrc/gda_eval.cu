@@ -120,14 +120,73 @@ init_state_kernel(int B, double* __restrict__ best_obj, int32_t* __restrict__ im
     if (b == 0) { st->t = t0; st->n_eval = 0; }
 }
 
+// PDBO-s: ginc[k][b] = beta * sum of the gpart rows of group k (rows dealt to 32 slices, every slice and then the
+// slices summed in a fixed order: deterministic).  grid (ceil(B/32), GINC_GROUPS), block (32, 32).
+__global__ void __launch_bounds__(1024)
+gsum_reduce_kernel(int B, const float* __restrict__ gpart, int n_gpart, float beta, float* __restrict__ ginc) {
+    __shared__ float red[32][33];
+    const int b = blockIdx.x * 32 + threadIdx.x, slice = threadIdx.y, group = blockIdx.y;
+    const int per = (n_gpart + GINC_GROUPS - 1) / GINC_GROUPS;
+    const int r0 = group * per, r1 = min(n_gpart, r0 + per);
+    float acc = 0.0f;
+    if (b < B)
+        for (int r = r0 + slice; r < r1; r += 32) acc += gpart[(size_t)r * B + b];
+    red[slice][threadIdx.x] = acc;
+    __syncthreads();
+    if (slice == 0 && b < B) {
+        float t = 0.0f;
+        for (int k = 0; k < 32; ++k) t += red[k][threadIdx.x];
+        ginc[(size_t)group * B + b] = beta * t;
+    }
+}
+
+__global__ void mu_finalize_kernel(int B, const float* __restrict__ mu, const float* __restrict__ ginc, float* __restrict__ out) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    float inc = 0.0f;
+    for (int k = 0; k < GINC_GROUPS; ++k) inc += ginc[(size_t)k * B + b];
+    out[b] = mu[b] + inc;
+}
+
+__global__ void mu_init_kernel(int B, const float* __restrict__ l0, float l0_scalar, float* __restrict__ mu, float* __restrict__ ginc) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    mu[b] = l0 ? l0[b] : l0_scalar;
+    for (int k = 0; k < GINC_GROUPS; ++k) ginc[(size_t)k * B + b] = 0.0f;
+}
+
 }  // namespace
+
+gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float beta, float* ginc, cudaStream_t s,
+                       int64_t* launches) {
+    gsum_reduce_kernel<<<dim3((unsigned)((B + 31) / 32), GINC_GROUPS), dim3(32, 32), 0, s>>>(B, gpart, n_gpart, beta, ginc);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status mu_finalize(int32_t B, const float* mu, const float* ginc, float* mu_out, cudaStream_t s, int64_t* launches) {
+    mu_finalize_kernel<<<(B + 255) / 256, 256, 0, s>>>(B, mu, ginc, mu_out);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, float* ginc, cudaStream_t s, int64_t* launches) {
+    mu_init_kernel<<<(B + 255) / 256, 256, 0, s>>>(B, l0, l0_scalar, mu, ginc);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
 
 gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0, float l0_scalar,
                     uint32_t t0, cudaStream_t s, int64_t* launches) {
     Workspace& ws = p->ws;
     const size_t elems = (size_t)p->n * B;
     GDA_CUDA_TRY(cudaMemcpyAsync(ws.x[0], x0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
-    if (l0) {
+    if (ws.dual == GDA_DUAL_SCALAR) {
+        GDA_TRY(mu_init(B, l0, l0_scalar, ws.mu[0], ws.ginc, s, launches));
+    } else if (l0) {
         GDA_CUDA_TRY(cudaMemcpyAsync(ws.y, l0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
     } else {
         const size_t n_vec = elems / 4;

@@ -39,6 +39,18 @@ struct UpdParams {
     int32_t gfun;
 };
 
+// PDBO-s (GDA_DUAL_SCALAR) state handed to the step kernels; mu_prev == nullptr means per-variable duals.
+// mu^t = mu_prev + sum_k ginc[k]: ginc holds the increment beta * sum_i g(x_i^{t-1}) as GINC_GROUPS partial sums
+// (zeros at the start of a run).  The step kernel writes mu^t to mu_cur (first block of every column chunk) and its
+// blocks' sums of g(x_i^t) to gpart; gsum_reduce turns gpart into the next ginc.
+constexpr int GINC_GROUPS = 8;
+struct ScalarDual {
+    const float* mu_prev = nullptr;   // [B]
+    const float* ginc = nullptr;      // [GINC_GROUPS][B]
+    float* mu_cur = nullptr;          // [B]
+    float* gpart = nullptr;           // [n_gpart][B]
+};
+
 // device-side run state (lives in the workspace)
 struct RunState {
     uint32_t t;          // iteration index of the iterate currently in x[cur]
@@ -54,6 +66,11 @@ struct Workspace {
     bool has_state = false;             // a previous gda_run left (x, y, best-so-far) here: x0 == NULL may resume
     float* x[2] = {nullptr, nullptr};   // [n][B] double buffer (Jacobi: every row reads all of x^t)
     float* y = nullptr;                 // [n][B], updated in place
+    float* mu[2] = {nullptr, nullptr};  // PDBO-s: [B] multipliers, double-buffered with the parity of x
+    float* ginc = nullptr;              // PDBO-s: [GINC_GROUPS][B] pending increment of mu
+    float* gpart = nullptr;             // PDBO-s: [n_gpart][B] per-block sums of g
+    int32_t n_gpart = 0;
+    int32_t dual = 0;                   // dual mode of the state held here
     uint8_t* x_bin = nullptr;           // [n][B] best-so-far rounded point
     double* best_obj = nullptr;         // [B]
     double* obj_now = nullptr;          // [B]
@@ -120,7 +137,8 @@ struct gda_problem {
 // ---------------------------------------------------------------------------------------------------
 // sparse QUBO (gda_sparse.cu)
 gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
-                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
+                       const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
+int32_t sparse_num_gparts(const gda_problem* p);
 gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);
 gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
                                  cudaStream_t s, int64_t* launches);
@@ -128,7 +146,8 @@ int32_t sparse_num_partials(const gda_problem* p, int32_t B);
 
 // MaxSAT (gda_maxsat.cu)
 gda_status maxsat_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
-                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
+                       const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
+int32_t maxsat_num_gparts(const gda_problem* p);
 gda_status maxsat_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);
 gda_status maxsat_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
                                  cudaStream_t s, int64_t* launches);
@@ -160,6 +179,11 @@ gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0,
                     uint32_t t0, cudaStream_t s, int64_t* launches);
 gda_status score_reduce(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj,
                         cudaStream_t s);
+// PDBO-s: ginc[k][b] = beta * (sum of gpart rows of group k), fixed order; mu_out = mu + sum_k ginc[k] (finalize)
+gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float beta, float* ginc, cudaStream_t s,
+                       int64_t* launches);
+gda_status mu_finalize(int32_t B, const float* mu, const float* ginc, float* mu_out, cudaStream_t s, int64_t* launches);
+gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, float* ginc, cudaStream_t s, int64_t* launches);
 
 // ---------------------------------------------------------------------------------------------------
 // device helpers: g, g', the fused update S4 (Eq. 6 + perturbation), the tie-break hash
@@ -209,6 +233,14 @@ __device__ __forceinline__ void gda_update_nopert(float x, float y, float G, con
     yn = y + up.beta * gv;
 }
 
+// g(x) alone (PDBO-s sums it over the variables of a restart); same expressions as in gda_update_nopert
+template <int GFUN>
+__device__ __forceinline__ float gda_g(float x, const UpdParams& up) {
+    if (GFUN == GDA_G_QUADRATIC) return x * x - x;
+    const float u = 1.0f - x;
+    return fmaf(x, fast_ln(fmaxf(x, up.log_eps)), u * fast_ln(fmaxf(u, up.log_eps)));
+}
+
 __device__ __forceinline__ bool gda_in_band(float x, float xt, float delta) {
     return fabsf(x - 0.5f) < delta && fabsf(xt - 0.5f) < delta;           // false for delta == 0
 }
@@ -251,7 +283,36 @@ __device__ __forceinline__ void gda_update4(const float4& x, const float4& y, co
     }
 }
 
+
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+
+// ---- PDBO-s helpers shared by the warp-per-(row, chunk) step kernels -------------------------------------------
+// mu^t for restarts 4 c4 .. 4 c4 + 3: the pending increment summed over its groups in index order, then added
+// (the same order as mu_finalize_kernel, so that the mu reported at the end of a run is the one the next step uses)
+__device__ __forceinline__ float4 scalar_dual_mu(const ScalarDual& sd, int B, int c4) {
+    float4 inc = ldg4(sd.ginc + 4 * c4);
+#pragma unroll
+    for (int k = 1; k < GINC_GROUPS; ++k) {
+        const float4 v = ldg4(sd.ginc + (size_t)k * B + 4 * c4);
+        inc.x += v.x; inc.y += v.y; inc.z += v.z; inc.w += v.w;
+    }
+    const float4 mu = ldg4(sd.mu_prev + 4 * c4);
+    return make_float4(mu.x + inc.x, mu.y + inc.y, mu.z + inc.z, mu.w + inc.w);
+}
+
+// One gpart row per block: the NW warps' sums of g (0 for warps without a row), added in warp order by warp 0.
+// Called by every thread of the block.
+template <int NW>
+__device__ __forceinline__ void scalar_dual_block_sum(float4 gs, float4 (*red)[32], int warp, int lane, bool active,
+                                                      float* __restrict__ gpart_row_c4) {
+    red[warp][lane] = gs;
+    __syncthreads();
+    if (warp != 0 || !active) return;
+    float4 t = red[0][lane];
+#pragma unroll
+    for (int w = 1; w < NW; ++w) { const float4 r = red[w][lane]; t.x += r.x; t.y += r.y; t.z += r.z; t.w += r.w; }
+    *reinterpret_cast<float4*>(gpart_row_c4) = t;
+}
 
 // Programmatic dependent launch (PDL): a step kernel lets its successor start launching right away and the successor
 // blocks at pdl_wait() -- placed after its index loads, before its first access to X / Y -- until this grid has

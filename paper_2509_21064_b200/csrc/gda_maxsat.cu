@@ -98,32 +98,45 @@ __device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, con
     return acc;
 }
 
-// warp-per-(variable, 128-restart chunk).  MODE 0: fused step; MODE 1: write G only.
-template <int GFUN, int MODE, int KW, bool PAD>
+// warp-per-(variable, 128-restart chunk): blockIdx.y = chunk, the block's 8 warps take 8 consecutive variables.
+// MODE 0: fused step; MODE 1: write G only.  DUAL (PDBO-s, MODE 0): one multiplier per restart (mu^t = sd.mu_prev +
+// sd.ginc), y untouched, the block's sum of g(x_i^t) goes to sd.gpart[blockIdx.x], block 0 records mu^t.
+template <int GFUN, int MODE, int KW, bool PAD, bool DUAL>
 __global__ void __launch_bounds__(THREADS)
-maxsat_step_kernel(int n, int B, int chunks, const int32_t* __restrict__ vptr, const float* __restrict__ coef,
+maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* __restrict__ coef,
                    const int32_t* __restrict__ others, int kw, const float* __restrict__ x,
-                   float* __restrict__ y, float* __restrict__ xn, UpdParams up,
+                   float* __restrict__ y, float* __restrict__ xn, UpdParams up, ScalarDual sd,
                    const RunState* __restrict__ st, uint32_t t_off) {
-    const int lane = threadIdx.x & 31;
-    const long long item = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
-    if (item >= (long long)n * chunks) return;
-    const int var = (int)(item / chunks);
-    const int chunk = (int)(item - (long long)var * chunks);
-    const int c4 = chunk * 32 + lane;
+    __shared__ float4 gred[DUAL ? WARPS : 1][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int var = blockIdx.x * WARPS + warp;
+    const int c4 = blockIdx.y * 32 + lane;
     const bool active = 4 * c4 < B;
-    const int start = __ldg(vptr + var), end = __ldg(vptr + var + 1);
-    const float4 G = gather_var<KW, PAD>(coef, others, kw, start, end, x, B, c4, active, lane);
-    if (!active) return;
-    const size_t off = (size_t)var * B + 4 * c4;
-    if (MODE == 1) { *reinterpret_cast<float4*>(xn + off) = G; return; }
-    const uint32_t t = (st ? st->t : 0u) + t_off;
-    const float4 xv = ldg4(x + off);
-    const float4 yv = *reinterpret_cast<const float4*>(y + off);
-    float4 xo, yo;
-    gda_update4<GFUN>(xv, yv, G, up, t, (uint32_t)var, 4u * (uint32_t)c4, xo, yo);
-    *reinterpret_cast<float4*>(xn + off) = xo;
-    *reinterpret_cast<float4*>(y + off) = yo;
+    float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = gs;
+    if (DUAL) mu = scalar_dual_mu(sd, B, active ? c4 : B / 4 - 1);
+    if (var < n) {                                           // warp-uniform
+        const int start = __ldg(vptr + var), end = __ldg(vptr + var + 1);
+        const float4 G = gather_var<KW, PAD>(coef, others, kw, start, end, x, B, c4, active, lane);
+        if (active) {
+            const size_t off = (size_t)var * B + 4 * c4;
+            if (MODE == 1) {
+                *reinterpret_cast<float4*>(xn + off) = G;
+            } else {
+                const uint32_t t = (st ? st->t : 0u) + t_off;
+                const float4 xv = ldg4(x + off);
+                const float4 yv = DUAL ? mu : *reinterpret_cast<const float4*>(y + off);
+                float4 xo, yo;
+                gda_update4<GFUN>(xv, yv, G, up, t, (uint32_t)var, 4u * (uint32_t)c4, xo, yo);
+                *reinterpret_cast<float4*>(xn + off) = xo;
+                if (DUAL) gs = make_float4(gda_g<GFUN>(xv.x, up), gda_g<GFUN>(xv.y, up), gda_g<GFUN>(xv.z, up), gda_g<GFUN>(xv.w, up));
+                else *reinterpret_cast<float4*>(y + off) = yo;
+            }
+        }
+    }
+    if (DUAL) {
+        if (blockIdx.x == 0 && warp == 0 && active) *reinterpret_cast<float4*>(sd.mu_cur + 4 * c4) = mu;
+        scalar_dual_block_sum<WARPS>(gs, gred, warp, lane, active, sd.gpart + (size_t)blockIdx.x * B + 4 * c4);
+    }
 }
 
 // S5: partial[cb][b] = sum over the clauses of block cb of w_j [every literal of C_j false under x_hat]
@@ -170,33 +183,28 @@ maxsat_score(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __re
     }
 }
 
-template <int GFUN, int MODE>
-void launch_kw(gda_problem* p, int32_t B, int chunks, unsigned grid, const float* x, float* y, float* xn,
-               const UpdParams& up, const RunState* st, uint32_t t_off, cudaStream_t s) {
-#define GDA_MS_ARGS p->n, B, chunks, p->d_vptr, p->d_coef, p->d_others, p->kw, x, y, xn, up, st, t_off
+template <int GFUN, int MODE, bool DUAL>
+void launch_kw(gda_problem* p, int32_t B, dim3 grid, const float* x, float* y, float* xn,
+               const UpdParams& up, const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s) {
+#define GDA_MS_ARGS p->n, B, p->d_vptr, p->d_coef, p->d_others, p->kw, x, y, xn, up, sd, st, t_off
+#define GDA_MS_CASE(K) \
+        case K: if (pad) maxsat_step_kernel<GFUN, MODE, K, true, DUAL><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); \
+                else maxsat_step_kernel<GFUN, MODE, K, false, DUAL><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
     const bool pad = p->kmin != p->kmax;
     switch (p->kw) {
-        case 1: if (pad) maxsat_step_kernel<GFUN, MODE, 1, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS);
-                else maxsat_step_kernel<GFUN, MODE, 1, false><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
-        case 2: if (pad) maxsat_step_kernel<GFUN, MODE, 2, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS);
-                else maxsat_step_kernel<GFUN, MODE, 2, false><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
-        case 3: if (pad) maxsat_step_kernel<GFUN, MODE, 3, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS);
-                else maxsat_step_kernel<GFUN, MODE, 3, false><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
-        case 4: if (pad) maxsat_step_kernel<GFUN, MODE, 4, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS);
-                else maxsat_step_kernel<GFUN, MODE, 4, false><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
-        default: maxsat_step_kernel<GFUN, MODE, 0, true><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        GDA_MS_CASE(1) GDA_MS_CASE(2) GDA_MS_CASE(3) GDA_MS_CASE(4)
+        default: maxsat_step_kernel<GFUN, MODE, 0, true, DUAL><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
     }
+#undef GDA_MS_CASE
 #undef GDA_MS_ARGS
 }
 
-template <int MODE>
+template <int MODE, bool DUAL>
 gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
-                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
-    const int chunks = (B / 4 + 31) / 32;
-    const long long items = (long long)p->n * chunks;
-    const unsigned grid = (unsigned)((items + WARPS - 1) / WARPS);
-    if (up.gfun == GDA_G_QUADRATIC) launch_kw<GDA_G_QUADRATIC, MODE>(p, B, chunks, grid, x, y, xn, up, st, t_off, s);
-    else launch_kw<GDA_G_ENTROPY, MODE>(p, B, chunks, grid, x, y, xn, up, st, t_off, s);
+                       const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+    const dim3 grid((unsigned)((p->n + WARPS - 1) / WARPS), (unsigned)((B / 4 + 31) / 32));
+    if (up.gfun == GDA_G_QUADRATIC) launch_kw<GDA_G_QUADRATIC, MODE, DUAL>(p, B, grid, x, y, xn, up, sd, st, t_off, s);
+    else launch_kw<GDA_G_ENTROPY, MODE, DUAL>(p, B, grid, x, y, xn, up, sd, st, t_off, s);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
@@ -205,14 +213,17 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
 }  // namespace
 
 gda_status maxsat_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
-                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
-    return launch_step<0>(p, B, x, y, xn, up, st, t_off, s, launches);
+                       const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+    if (sd.mu_prev) return launch_step<0, true>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
+    return launch_step<0, false>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
 }
+
+int32_t maxsat_num_gparts(const gda_problem* p) { return (p->n + WARPS - 1) / WARPS; }
 
 gda_status maxsat_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s) {
     UpdParams up{};
     up.gfun = GDA_G_QUADRATIC;
-    return launch_step<1>(p, B, x, nullptr, G, up, nullptr, 0, s, nullptr);
+    return launch_step<1, false>(p, B, x, nullptr, G, up, ScalarDual{}, nullptr, 0, s, nullptr);
 }
 
 int32_t maxsat_num_partials(const gda_problem* p, int32_t) { return (p->m + SCORE_CLAUSES - 1) / SCORE_CLAUSES; }

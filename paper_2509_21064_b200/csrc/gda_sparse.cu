@@ -62,18 +62,21 @@ __device__ __forceinline__ float4 gather_row(const int32_t* __restrict__ col, co
     return acc;
 }
 
-template <int GFUN>
+// S4 for one (row, float4 of restarts).  DUAL (PDBO-s): `mu` is this step's multiplier for the four restarts, y is
+// not touched, and the values of g(x^t) are returned in gs (0 for lanes past a ragged B).
+template <int GFUN, bool DUAL>
 __device__ __forceinline__ void update_store(int row, int c4, int B, bool active, float4 G, const float* __restrict__ x,
                                              float* __restrict__ y, float* __restrict__ xn,
-                                             const UpdParams& up, uint32_t t) {
+                                             const UpdParams& up, uint32_t t, float4 mu, float4& gs) {
     const size_t off = (size_t)row * B + 4 * c4;
     const float4 xv = ldg4(x + off);
-    const float4 yv = *reinterpret_cast<const float4*>(y + off);
+    const float4 yv = DUAL ? mu : *reinterpret_cast<const float4*>(y + off);
     float4 xo, yo;
     gda_update4<GFUN>(xv, yv, G, up, t, (uint32_t)row, 4u * (uint32_t)c4, xo, yo);
     if (!active) return;
     *reinterpret_cast<float4*>(xn + off) = xo;
-    *reinterpret_cast<float4*>(y + off) = yo;
+    if (DUAL) gs = make_float4(gda_g<GFUN>(xv.x, up), gda_g<GFUN>(xv.y, up), gda_g<GFUN>(xv.z, up), gda_g<GFUN>(xv.w, up));
+    else *reinterpret_cast<float4*>(y + off) = yo;
 }
 
 // warp-per-(row, 128-restart chunk): blockIdx.y = chunk, the block's 8 warps take 8 consecutive rows.
@@ -83,19 +86,45 @@ __device__ __forceinline__ void update_store(int row, int c4, int B, bool active
 // is -1 sends the row through its CSR entries.  40 registers (6 blocks per SM).  Measured on config 3 (profiles/):
 // 17.3 us per step before, 16.3 us with the lean gather loop, 14.8 us with the records and 6 blocks per SM;
 // prefetching the row's own x, y lines into L1 up front was slower (15.1 us) and is not done.
-template <int GFUN, int MODE, bool ELL>
+// DUAL (PDBO-s, MODE 0 only): the multiplier is one number per restart (mu^t = sd.mu_prev + sd.ginc), y is not
+// read or written, and the block leaves the sum of g(x_i^t) over its rows in sd.gpart[blockIdx.x]; the first block
+// of every column chunk also records mu^t in sd.mu_cur.
+template <int GFUN, int MODE, bool ELL, bool DUAL>
 __global__ void __launch_bounds__(THREADS, 6)
 spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
                const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                const float* __restrict__ val2, const int32_t* __restrict__ ell, const float* __restrict__ cprime,
                const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
-               UpdParams up, const RunState* __restrict__ st, uint32_t t_off) {
-    const int lane = threadIdx.x & 31;
-    const int ridx = blockIdx.x * WARPS + (threadIdx.x >> 5);
-    if (ridx >= n_rows) return;                              // warp-uniform
-    const int row = row_list ? __ldg(row_list + ridx) : ridx;
+               UpdParams up, ScalarDual sd, const RunState* __restrict__ st, uint32_t t_off) {
+    __shared__ float4 gred[DUAL ? WARPS : 1][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int ridx = blockIdx.x * WARPS + warp;
     const bool active = 4 * (blockIdx.y * 32 + lane) < B;
     const int c4 = active ? blockIdx.y * 32 + lane : B / 4 - 1;      // ragged B: idle lanes recompute the last float4
+    if (DUAL) {
+        float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = scalar_dual_mu(sd, B, c4);
+        if (ridx < n_rows) {                                 // warp-uniform
+            const int row = row_list ? __ldg(row_list + ridx) : ridx;
+            const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
+            const uint32_t stride = 4u * (uint32_t)B;
+            float4 G = make_float4(0.f, 0.f, 0.f, 0.f);
+            bool csr = true;
+            if (ELL) {
+                const int w = __ldg(ell + (size_t)row * 16 + (lane & 15));
+                csr = __shfl_sync(0xffffffffu, w, 0) < 0;
+                if (!csr) accumulate_lanes(G, w, 0, w, 8, __popc(__ballot_sync(0xffffffffu, w != 0 && (lane & 24) == 8)), xb, stride);
+            }
+            if (csr) G = gather_row(col, val2, __ldg(rowptr + row), __ldg(rowptr + row + 1), xb, stride, lane);
+            const float cp = __ldg(cprime + row);
+            G.x += cp; G.y += cp; G.z += cp; G.w += cp;
+            update_store<GFUN, true>(row, c4, B, active, G, x, y, xn, up, (st ? st->t : 0u) + t_off, mu, gs);
+        }
+        if (blockIdx.x == 0 && warp == 0 && active) *reinterpret_cast<float4*>(sd.mu_cur + 4 * c4) = mu;
+        scalar_dual_block_sum<WARPS>(gs, gred, warp, lane, active, sd.gpart + (size_t)blockIdx.x * B + 4 * c4);
+        return;
+    }
+    if (ridx >= n_rows) return;                              // warp-uniform
+    const int row = row_list ? __ldg(row_list + ridx) : ridx;
     const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
     const uint32_t stride = 4u * (uint32_t)B;
     float4 G = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -113,17 +142,20 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
     G.x += cp; G.y += cp; G.z += cp; G.w += cp;
     if (MODE == 1) { if (active) *reinterpret_cast<float4*>(xn + (size_t)row * B + 4 * c4) = G; return; }
     const uint32_t t = (st ? st->t : 0u) + t_off;
-    update_store<GFUN>(row, c4, B, active, G, x, y, xn, up, t);
+    float4 unused;
+    update_store<GFUN, false>(row, c4, B, active, G, x, y, xn, up, t, make_float4(0.f, 0.f, 0.f, 0.f), unused);
 }
 
 // row-split: one block per (heavy row, chunk); the 8 warps take interleaved 32-entry slices of the row
-template <int GFUN, int MODE>
+// DUAL: as above; the row's g values go to sd.gpart[gpart_row0 + ridx], and block 0 records mu^t when write_mu is set
+// (there is no warp-per-row launch to do it).
+template <int GFUN, int MODE, bool DUAL>
 __global__ void __launch_bounds__(THREADS)
 spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chunks,
                 const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                 const float* __restrict__ val2, const float* __restrict__ cprime,
                 const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
-                UpdParams up, const RunState* __restrict__ st, uint32_t t_off) {
+                UpdParams up, ScalarDual sd, int gpart_row0, int write_mu, const RunState* __restrict__ st, uint32_t t_off) {
     __shared__ float4 red[WARPS][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ridx = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
@@ -147,7 +179,13 @@ spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chu
     G.x += cp; G.y += cp; G.z += cp; G.w += cp;
     if (MODE == 1) { if (active) *reinterpret_cast<float4*>(xn + (size_t)row * B + 4 * c4) = G; return; }
     const uint32_t t = (st ? st->t : 0u) + t_off;
-    update_store<GFUN>(row, c4, B, active, G, x, y, xn, up, t);
+    float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = gs;
+    if (DUAL) {
+        mu = scalar_dual_mu(sd, B, c4);
+        if (write_mu && ridx == 0 && active) *reinterpret_cast<float4*>(sd.mu_cur + 4 * c4) = mu;
+    }
+    update_store<GFUN, DUAL>(row, c4, B, active, G, x, y, xn, up, t, mu, gs);
+    if (DUAL && active) *reinterpret_cast<float4*>(sd.gpart + (size_t)(gpart_row0 + ridx) * B + 4 * c4) = gs;
 }
 
 // S5 for sparse QUBO: partial[rb][b] = sum over the rows of block rb of x_hat_i ((Q_off x_hat)_i + c'_i)
@@ -214,17 +252,18 @@ spmm_score(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __re
     }
 }
 
-template <int MODE>
+template <int MODE, bool DUAL>
 gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
-                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+                       const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
     const int chunks = (B / 4 + 31) / 32;
     const int n_light = p->d_light_rows ? p->n_light : p->n;
+    const int light_blocks = (n_light + WARPS - 1) / WARPS;
     if (n_light > 0) {
-        const dim3 grid((unsigned)((n_light + WARPS - 1) / WARPS), (unsigned)chunks);
-#define GDA_SP_ARGS n_light, p->d_light_rows, B, p->d_rowptr, p->d_col, p->d_val2, p->d_ell, p->d_cprime, x, y, xn, up, st, t_off
+        const dim3 grid((unsigned)light_blocks, (unsigned)chunks);
+#define GDA_SP_ARGS n_light, p->d_light_rows, B, p->d_rowptr, p->d_col, p->d_val2, p->d_ell, p->d_cprime, x, y, xn, up, sd, st, t_off
 #define GDA_SP_CASE(E) \
-        if (up.gfun == GDA_G_QUADRATIC) spmm_step_warp<GDA_G_QUADRATIC, MODE, E><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); \
-        else spmm_step_warp<GDA_G_ENTROPY, MODE, E><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS)
+        if (up.gfun == GDA_G_QUADRATIC) spmm_step_warp<GDA_G_QUADRATIC, MODE, E, DUAL><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); \
+        else spmm_step_warp<GDA_G_ENTROPY, MODE, E, DUAL><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS)
         if (p->d_ell) { GDA_SP_CASE(true); } else { GDA_SP_CASE(false); }
 #undef GDA_SP_CASE
 #undef GDA_SP_ARGS
@@ -232,12 +271,13 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     }
     if (p->n_heavy > 0) {
         const unsigned grid = (unsigned)(p->n_heavy * chunks);
+        const int write_mu = n_light > 0 ? 0 : 1;
         if (up.gfun == GDA_G_QUADRATIC)
-            spmm_step_split<GDA_G_QUADRATIC, MODE><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off);
+            spmm_step_split<GDA_G_QUADRATIC, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, light_blocks, write_mu, st, t_off);
         else
-            spmm_step_split<GDA_G_ENTROPY, MODE><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off);
+            spmm_step_split<GDA_G_ENTROPY, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, light_blocks, write_mu, st, t_off);
         if (launches) ++*launches;
     }
     GDA_CUDA_TRY(cudaGetLastError());
@@ -249,14 +289,21 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
 int sparse_heavy_threshold() { return HEAVY_DEG; }
 
 gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
-                       const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
-    return launch_step<0>(p, B, x, y, xn, up, st, t_off, s, launches);
+                       const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+    if (sd.mu_prev) return launch_step<0, true>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
+    return launch_step<0, false>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
+}
+
+// PDBO-s: rows of sd.gpart written per step (one per block of the warp-per-row launch, one per heavy row)
+int32_t sparse_num_gparts(const gda_problem* p) {
+    const int n_light = p->d_light_rows ? p->n_light : p->n;
+    return (n_light + WARPS - 1) / WARPS + p->n_heavy;
 }
 
 gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s) {
     UpdParams up{};
     up.gfun = GDA_G_QUADRATIC;
-    return launch_step<1>(p, B, x, nullptr, G, up, nullptr, 0, s, nullptr);
+    return launch_step<1, false>(p, B, x, nullptr, G, up, ScalarDual{}, nullptr, 0, s, nullptr);
 }
 
 int32_t sparse_num_partials(const gda_problem* p, int32_t) { return (p->n + SCORE_ROWS - 1) / SCORE_ROWS; }

@@ -66,6 +66,7 @@ class Hyper:
     iters: int = 1000
     eval_every: int = 100
     seed: int = 0
+    dual: int = 0          # 0 per-variable multipliers (PDBO), 1 one multiplier per restart (PDBO-s)
 
 
 @dataclass
@@ -224,3 +225,16 @@ def config(idx: int, B: Optional[int] = None, n_scale: float = 1.0) -> Workload:
                         Hyper(2.0, 0.01, 0.005, 1e-4, 1, 1e-6, 5000, 100, 105), 1105,
                         "weighted Max-3-SAT ratio 4.26, w in 1..10, entropy g")
     raise ValueError("config index must be 1..5")
+
+
+def pdbo_s_variant(w: Workload) -> Workload:
+    """The same instance run as PDBO-s (reading R14): one multiplier per restart,
+    mu+ = mu + beta_s sum_i g(x_i).  The paper gives no step size for it; beta_s = beta / n keeps the multiplier's
+    rate of decrease equal to the average of the per-variable rates of PDBO."""
+    import copy
+    v = copy.deepcopy(w)
+    v.name = w.name + "_pdbo_s"
+    v.hyper.dual = 1
+    v.hyper.beta = w.hyper.beta / w.problem.n
+    v.note = w.note + "; PDBO-s (scalar dual, beta_s = beta/n)"
+    return v

@@ -18,5 +18,7 @@ def oracle_problem(P):
 def hyper_kwargs(h, **over):
     d = dict(alpha=h.alpha, beta=h.beta, delta=h.delta, gfun=h.gfun, log_eps=h.log_eps,
              iters=h.iters, eval_every=h.eval_every, seed=h.seed)
+    if getattr(h, "dual", 0):
+        d["dual"] = h.dual
     d.update(over)
     return d

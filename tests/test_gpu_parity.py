@@ -501,3 +501,97 @@ def test_dense_full_run(api, oracle, w):
     rnd = oracle.F_binary(OP, (np.random.default_rng(0).random((n, 64)) < 0.5).astype(np.uint8))
     assert obj.max() < rnd.min()
     P.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# PDBO-s (GDA_DUAL_SCALAR, reading R14): one multiplier per restart
+# ------------------------------------------------------------------------------------------------
+def pdbo_s_workloads():
+    return [wl.pdbo_s_variant(wl.config(3, B=260, n_scale=0.05)), wl.pdbo_s_variant(wl.config(2, B=132, n_scale=0.25)),
+            wl.pdbo_s_variant(wl.config(5, B=136, n_scale=0.05))]
+
+
+PDBO_S = pdbo_s_workloads()
+
+
+def mu_tolerance(h, n, mu):
+    """|mu+ - mu+_ref|: the multiplier itself to 1e-5 relative, plus the fp32 sum of n values of g (|g| <= ln 2)
+    accumulated blockwise: 1e-6 relative to its largest possible magnitude."""
+    return TOL_STEP * np.maximum(1.0, np.abs(mu)) + 1e-6 * f32(h.beta) * n
+
+
+@pytest.mark.parametrize("w", PDBO_S, ids=lambda w: w.name)
+def test_pdbo_s_teacher_forced_steps_and_resume(api, oracle, w):
+    OP = oracle_problem(w.problem)
+    P = api.create_from_workload(w.problem)
+    n, B, h = w.problem.n, w.B, w.hyper
+    x = dev(wl.x0_uniform(n, B, w.x0_seed))
+    mu = dev(np.linspace(0.5 * h.lambda0, h.lambda0, B).astype(np.float32))      # a different multiplier per restart
+    t = 0
+    for hop in (0, 1, 37, 200):
+        if hop:
+            r = P.run(x, mu, api.params_from_hyper(h, iters=hop, eval_every=50, t0=t), want_final=True)
+            x, mu, t = r["x"], r["lam"], t + hop
+        r1 = P.run(x, mu, api.params_from_hyper(h, iters=1, eval_every=1, t0=t), want_final=True)
+        assert r1["lam"].shape == (B,)
+        xg, mg = r1["x"].cpu().numpy().astype(np.float64), r1["lam"].cpu().numpy().astype(np.float64)
+        ref = assert_x_step_close(xg, x.cpu().numpy(), OP, oracle, okw(h, iters=1, eval_every=1, t0=t), mu.cpu().numpy())
+        assert (np.abs(mg - ref["y"]) <= mu_tolerance(h, n, ref["y"])).all(), (w.name, t)
+    # a run in two calls (3 steps + 2 resumed) is bit-identical to one call of 5 steps: the multiplier, its pending
+    # increment and the buffer parity survive in the handle, and the sums are deterministic
+    x0 = dev(wl.x0_uniform(n, B, w.x0_seed + 1))
+    a = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=5, eval_every=5), want_final=True)
+    xa, ma = a["x"].clone(), a["lam"].clone()
+    b = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=3, eval_every=3), want_final=True)
+    ex = api.Extra()
+    ex.x_final, ex.lambda_final = b["x"].data_ptr(), b["lam"].data_ptr()
+    prm = api.params_from_hyper(h, iters=2, eval_every=2)
+    api._check(api.lib().gda_run(P._h, B, None, None, 0.0, api.C.byref(prm), b["x_bin"].data_ptr(), b["obj"].data_ptr(),
+                                 b["best_restart"].data_ptr(), api.C.byref(ex), torch.cuda.current_stream().cuda_stream))
+    torch.cuda.synchronize()
+    assert torch.equal(b["x"], xa) and torch.equal(b["lam"], ma)
+    P.destroy()
+
+
+@pytest.mark.parametrize("w", PDBO_S, ids=lambda w: w.name)
+def test_pdbo_s_free_running_and_full_run(api, oracle, w):
+    OP = oracle_problem(w.problem)
+    P = api.create_from_workload(w.problem)
+    n, B, h = w.problem.n, w.B, w.hyper
+    X0 = wl.x0_uniform(n, B, w.x0_seed)
+    if h.gfun == 0:                                            # (c) 50 free steps, quadratic g (see test_free_running_50_steps)
+        r = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=50, eval_every=50), want_final=True)
+        ref = oracle.run(OP, X0, f32(h.lambda0), **okw(h, iters=50, eval_every=50))
+        assert np.abs(r["x"].cpu().numpy() - ref["x"]).max() <= TOL_TRAJ
+        assert (np.abs(r["lam"].cpu().numpy() - ref["y"]) <= 10 * mu_tolerance(h, n, ref["y"])).all()
+    iters = 1500
+    r = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=iters, eval_every=100))
+    obj, x_bin = r["obj"].cpu().numpy(), r["x_bin"].cpu().numpy()
+    assert np.array_equal(obj, oracle.F_binary(OP, x_bin))                     # (a) exact objective of the returned points
+    sub = slice(0, 32)
+    ref = oracle.run(OP, X0[:, sub], f32(h.lambda0), nthreads=4, **okw(h, iters=iters, eval_every=100))
+    assert_statistics_close(obj[sub], ref["obj"])                              # (d)
+    P.destroy()
+
+
+def test_pdbo_s_heavy_rows_and_argument_checks(api, oracle):
+    Pw = star_plus_isolated(700, 5)                             # row-split kernel + empty rows
+    OP = oracle_problem(Pw)
+    P = api.create_from_workload(Pw)
+    n, B = Pw.n, 8
+    X = np.random.default_rng(4).random((n, B), dtype=np.float32)
+    h = wl.Hyper(3.0, 0.004, 0.05 / n, 1e-4, 0, 1e-6, 1, 1, 77, 1)
+    r = P.run(dev(X), 3.0, api.params_from_hyper(h), want_final=True)
+    ref = oracle.run(OP, X, 3.0, **okw(h))
+    assert np.abs(r["x"].cpu().numpy() - ref["x"]).max() <= TOL_STEP
+    assert (np.abs(r["lam"].cpu().numpy() - ref["y"]) <= mu_tolerance(h, n, ref["y"])).all()
+    with pytest.raises(api.GdaError) as e:                      # a resumed run may not switch the dual mode
+        P.resume(api.params_from_hyper(h, dual=api.DUAL_PER_VARIABLE), r)
+    assert e.value.status == 1
+    P.destroy()
+    wd = wl.config(4, B=128, n_scale=0.0625)
+    Pd = api.create_from_workload(wd.problem)
+    with pytest.raises(api.GdaError) as e:
+        Pd.run(dev(wl.x0_uniform(wd.problem.n, 128, 1)), 1.0, api.params_from_hyper(wd.hyper, iters=1, dual=api.DUAL_SCALAR))
+    assert e.value.status == 4
+    Pd.destroy()
