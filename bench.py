@@ -53,7 +53,7 @@ def algorithmic_work(w: wl.Workload):
     """Per GDA step (one launch of the step kernel): algorithmic bytes / flops."""
     P, B = w.problem, w.B
     n = P.n
-    state = 16 * n * B                       # read x, y; write x, y (fp32)
+    state = (8 if getattr(w.hyper, "dual", 0) else 16) * n * B   # read x, y; write x, y (fp32); PDBO-s has no y array
     if w.kind == "qubo_csr":
         nnz = int(P.rowptr[-1])
         return dict(bound="hbm", bytes=state + 8 * nnz + 4 * (n + 1) + 4 * n, flops=2 * nnz * B)
@@ -125,7 +125,7 @@ def oracle_problem(P):
 def oracle_kwargs(h, iters):
     f = lambda v: float(np.float32(v))
     return dict(alpha=f(h.alpha), beta=f(h.beta), delta=f(h.delta), gfun=h.gfun, log_eps=f(h.log_eps),
-                iters=iters, eval_every=h.eval_every, seed=h.seed)
+                iters=iters, eval_every=h.eval_every, seed=h.seed, dual=getattr(h, "dual", 0))
 
 
 def oracle_sample_columns(w: wl.Workload, cores: int) -> int:
@@ -173,6 +173,8 @@ def run_reference(args, w: wl.Workload):
     per_step = h.eval_every if w.kind != "qubo_dense" else max(1, h.eval_every // 50)
     X = wl.x0_uniform(w.problem.n, w.B, w.x0_seed)[:, :Bo].copy().astype(np.float64)
     Y = np.full_like(X, float(np.float32(h.lambda0)))
+    if getattr(h, "dual", 0):
+        Y = Y[0].copy()                      # PDBO-s: one multiplier per restart
     kw = oracle_kwargs(h, per_step)
     kw["eval_every"] = per_step
     t = 0
@@ -333,7 +335,8 @@ def run_ours(args, w: wl.Workload):
             "dtype": "f32" if w.kind != "qubo_dense" else "bf16 x bf16 -> f32 (state f32)", "data": "synthetic",
             "config": {"workload": w.name, "baseline_config_index": args.config, "kind": w.kind, "n": n, "B_per_gpu": B,
                        "step": f"{iters_per_step} GDA iterations + 1 evaluation (one CUDA graph launch)",
-                       "hyper": {"lambda0": h.lambda0, "alpha": h.alpha, "beta": h.beta, "delta": h.delta, "gfun": h.gfun},
+                       "hyper": {"lambda0": h.lambda0, "alpha": h.alpha, "beta": h.beta, "delta": h.delta, "gfun": h.gfun,
+                                 "dual": "scalar (PDBO-s)" if getattr(h, "dual", 0) else "per-variable (PDBO)"},
                        "l2": "flushed between timed steps (256 MiB write, untimed)", "note": w.note},
             "whole_run": {"value": units / t_whole, "unit": "restart-iters/s", "ms_total": 1e3 * t_whole,
                           "iters": iters_per_step * K, "l2": "not flushed (one gda_run call)", "best_objective": best,
@@ -368,8 +371,11 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--B", type=int, default=None)
+    ap.add_argument("--pdbo-s", action="store_true", help="run the PDBO-s ablation (one multiplier per restart, PAPER.md:630-648)")
     args = ap.parse_args()
     w = wl.config(args.config, B=args.B)
+    if args.pdbo_s:
+        w = wl.pdbo_s_variant(w)
     if args.impl == "reference":
         run_reference(args, w)
     else:

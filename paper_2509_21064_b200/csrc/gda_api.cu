@@ -291,7 +291,7 @@ static void free_workspace(gda_problem* p) {
     cudaFree(ws.obj_now); cudaFree(ws.improved); cudaFree(ws.partial); cudaFree(ws.state);
     cudaFree(ws.best_restart); cudaFree(ws.best_val); cudaFree(ws.trace_best); cudaFree(ws.trace_ns);
     cudaFree(ws.zt[0]); cudaFree(ws.zt[1]); cudaFree(ws.gtmp);
-    cudaFree(ws.mu[0]); cudaFree(ws.mu[1]); cudaFree(ws.ginc); cudaFree(ws.gpart);
+    cudaFree(ws.mu[0]); cudaFree(ws.mu[1]); cudaFree(ws.gpart);
     if (ws.h_x0) cudaFreeHost(ws.h_x0);
     if (ws.h_l0) cudaFreeHost(ws.h_l0);
     ws = Workspace();
@@ -358,7 +358,6 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
         ws.n_gpart = p->kind == GDA_KIND_SPARSE ? sparse_num_gparts(p) : maxsat_num_gparts(p);
         if (st == GDA_OK) st = dmalloc(&ws.mu[0], (size_t)B);
         if (st == GDA_OK) st = dmalloc(&ws.mu[1], (size_t)B);
-        if (st == GDA_OK) st = dmalloc(&ws.ginc, (size_t)GINC_GROUPS * B);
         if (st == GDA_OK) st = dmalloc(&ws.gpart, (size_t)ws.n_gpart * B);
     }
     if (st == GDA_OK) st = dmalloc(&ws.state, 1);
@@ -414,14 +413,14 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     for (int k = 0; k < len; ++k) {
         int64_t before = *launches;
         ScalarDual sd;                                        // PDBO-s: mu follows the parity of x
-        if (scalar) { sd.mu_prev = ws.mu[cur]; sd.ginc = ws.ginc; sd.mu_cur = ws.mu[cur ^ 1]; sd.gpart = ws.gpart; }
+        if (scalar) { sd.mu = ws.mu[cur]; sd.gpart = ws.gpart; }
         if (p->kind == GDA_KIND_SPARSE)
             GDA_TRY(sparse_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         else if (p->kind == GDA_KIND_MAXSAT)
             GDA_TRY(maxsat_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         else
             GDA_TRY(dense_step(p, B, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, ws.state, (uint32_t)k, s, launches));
-        if (scalar) GDA_TRY(gsum_reduce(B, ws.gpart, ws.n_gpart, prm.beta, ws.ginc, s, launches));
+        if (scalar) GDA_TRY(gsum_reduce(B, ws.gpart, ws.n_gpart, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
         *step_launches += *launches - before;
         cur ^= 1;
     }
@@ -557,8 +556,8 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
     GDA_CUDA_TRY(cudaMemcpyAsync(best_restart, ws.best_restart, sizeof(int32_t), cudaMemcpyDeviceToDevice, s));
     if (extra) {
         if (extra->x_final) GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, xfin, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
-        if (extra->lambda_final && prm->dual == GDA_DUAL_SCALAR)          // mu^T = mu + pending increment, [B]
-            GDA_TRY(mu_finalize(B, ws.mu[parity], ws.ginc, extra->lambda_final, s, &p->last_launches));
+        if (extra->lambda_final && prm->dual == GDA_DUAL_SCALAR)          // mu^T, [B]
+            GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.mu[parity], (size_t)B * sizeof(float), cudaMemcpyDeviceToDevice, s));
         else if (extra->lambda_final)
             GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.y, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
         if (extra->best_obj) GDA_CUDA_TRY(cudaMemcpyAsync(extra->best_obj, ws.best_val, sizeof(double), cudaMemcpyDeviceToDevice, s));

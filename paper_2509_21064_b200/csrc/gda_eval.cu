@@ -120,60 +120,55 @@ init_state_kernel(int B, double* __restrict__ best_obj, int32_t* __restrict__ im
     if (b == 0) { st->t = t0; st->n_eval = 0; }
 }
 
-// PDBO-s: ginc[k][b] = beta * sum of the gpart rows of group k (rows dealt to 32 slices, every slice and then the
-// slices summed in a fixed order: deterministic).  grid (ceil(B/32), GINC_GROUPS), block (32, 32).
+// PDBO-s: mu_out[b] = mu_in[b] + beta * sum_r gpart[r][b].  grid ceil(B/32), block (32 restarts, 32 slices): rows are
+// dealt to the slices (8 independent loads in flight per thread), every slice and then the slices are added in index
+// order, so the sum is deterministic.  (A version with 64 row groups per column block and a last-block-done second
+// stage -- threadfence + counter -- was slower: 13 us against 5 us under ncu.)
 __global__ void __launch_bounds__(1024)
-gsum_reduce_kernel(int B, const float* __restrict__ gpart, int n_gpart, float beta, float* __restrict__ ginc) {
+gsum_reduce_kernel(int B, const float* __restrict__ gpart, int n_gpart, float beta, const float* __restrict__ mu_in,
+                   float* __restrict__ mu_out) {
     __shared__ float red[32][33];
-    const int b = blockIdx.x * 32 + threadIdx.x, slice = threadIdx.y, group = blockIdx.y;
-    const int per = (n_gpart + GINC_GROUPS - 1) / GINC_GROUPS;
-    const int r0 = group * per, r1 = min(n_gpart, r0 + per);
+    const int tx = threadIdx.x, slice = threadIdx.y;
+    const int b = blockIdx.x * 32 + tx;
     float acc = 0.0f;
-    if (b < B)
-        for (int r = r0 + slice; r < r1; r += 32) acc += gpart[(size_t)r * B + b];
-    red[slice][threadIdx.x] = acc;
+    if (b < B) {
+        int r = slice;
+        for (; r + 7 * 32 < n_gpart; r += 8 * 32) {
+            float v[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) v[q] = __ldg(gpart + (size_t)(r + 32 * q) * B + b);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) acc += v[q];
+        }
+        for (; r < n_gpart; r += 32) acc += __ldg(gpart + (size_t)r * B + b);
+    }
+    red[slice][tx] = acc;
     __syncthreads();
     if (slice == 0 && b < B) {
         float t = 0.0f;
-        for (int k = 0; k < 32; ++k) t += red[k][threadIdx.x];
-        ginc[(size_t)group * B + b] = beta * t;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) t += red[k][tx];
+        mu_out[b] = mu_in[b] + beta * t;
     }
 }
 
-__global__ void mu_finalize_kernel(int B, const float* __restrict__ mu, const float* __restrict__ ginc, float* __restrict__ out) {
+__global__ void mu_init_kernel(int B, const float* __restrict__ l0, float l0_scalar, float* __restrict__ mu) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B) return;
-    float inc = 0.0f;
-    for (int k = 0; k < GINC_GROUPS; ++k) inc += ginc[(size_t)k * B + b];
-    out[b] = mu[b] + inc;
-}
-
-__global__ void mu_init_kernel(int B, const float* __restrict__ l0, float l0_scalar, float* __restrict__ mu, float* __restrict__ ginc) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B) return;
-    mu[b] = l0 ? l0[b] : l0_scalar;
-    for (int k = 0; k < GINC_GROUPS; ++k) ginc[(size_t)k * B + b] = 0.0f;
+    if (b < B) mu[b] = l0 ? l0[b] : l0_scalar;
 }
 
 }  // namespace
 
-gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float beta, float* ginc, cudaStream_t s,
-                       int64_t* launches) {
-    gsum_reduce_kernel<<<dim3((unsigned)((B + 31) / 32), GINC_GROUPS), dim3(32, 32), 0, s>>>(B, gpart, n_gpart, beta, ginc);
+gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float beta, const float* mu_in, float* mu_out,
+                       cudaStream_t s, int64_t* launches) {
+    gsum_reduce_kernel<<<(unsigned)((B + 31) / 32), dim3(32, 32), 0, s>>>(B, gpart, n_gpart, beta, mu_in, mu_out);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
 }
 
-gda_status mu_finalize(int32_t B, const float* mu, const float* ginc, float* mu_out, cudaStream_t s, int64_t* launches) {
-    mu_finalize_kernel<<<(B + 255) / 256, 256, 0, s>>>(B, mu, ginc, mu_out);
-    if (launches) ++*launches;
-    GDA_CUDA_TRY(cudaGetLastError());
-    return GDA_OK;
-}
-
-gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, float* ginc, cudaStream_t s, int64_t* launches) {
-    mu_init_kernel<<<(B + 255) / 256, 256, 0, s>>>(B, l0, l0_scalar, mu, ginc);
+gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, cudaStream_t s, int64_t* launches) {
+    mu_init_kernel<<<(B + 255) / 256, 256, 0, s>>>(B, l0, l0_scalar, mu);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
@@ -185,7 +180,7 @@ gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0,
     const size_t elems = (size_t)p->n * B;
     GDA_CUDA_TRY(cudaMemcpyAsync(ws.x[0], x0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
     if (ws.dual == GDA_DUAL_SCALAR) {
-        GDA_TRY(mu_init(B, l0, l0_scalar, ws.mu[0], ws.ginc, s, launches));
+        GDA_TRY(mu_init(B, l0, l0_scalar, ws.mu[0], s, launches));
     } else if (l0) {
         GDA_CUDA_TRY(cudaMemcpyAsync(ws.y, l0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
     } else {

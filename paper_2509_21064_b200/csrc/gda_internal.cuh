@@ -39,15 +39,11 @@ struct UpdParams {
     int32_t gfun;
 };
 
-// PDBO-s (GDA_DUAL_SCALAR) state handed to the step kernels; mu_prev == nullptr means per-variable duals.
-// mu^t = mu_prev + sum_k ginc[k]: ginc holds the increment beta * sum_i g(x_i^{t-1}) as GINC_GROUPS partial sums
-// (zeros at the start of a run).  The step kernel writes mu^t to mu_cur (first block of every column chunk) and its
-// blocks' sums of g(x_i^t) to gpart; gsum_reduce turns gpart into the next ginc.
-constexpr int GINC_GROUPS = 8;
+// PDBO-s (GDA_DUAL_SCALAR) state handed to the step kernels; mu == nullptr means per-variable duals.
+// The step kernel reads this step's multipliers mu^t and leaves its blocks' sums of g(x_i^t) in gpart; gsum_reduce
+// then writes mu^{t+1} = mu^t + beta * sum(gpart) into the other mu buffer (the buffers follow the parity of x).
 struct ScalarDual {
-    const float* mu_prev = nullptr;   // [B]
-    const float* ginc = nullptr;      // [GINC_GROUPS][B]
-    float* mu_cur = nullptr;          // [B]
+    const float* mu = nullptr;        // [B]
     float* gpart = nullptr;           // [n_gpart][B]
 };
 
@@ -67,7 +63,6 @@ struct Workspace {
     float* x[2] = {nullptr, nullptr};   // [n][B] double buffer (Jacobi: every row reads all of x^t)
     float* y = nullptr;                 // [n][B], updated in place
     float* mu[2] = {nullptr, nullptr};  // PDBO-s: [B] multipliers, double-buffered with the parity of x
-    float* ginc = nullptr;              // PDBO-s: [GINC_GROUPS][B] pending increment of mu
     float* gpart = nullptr;             // PDBO-s: [n_gpart][B] per-block sums of g
     int32_t n_gpart = 0;
     int32_t dual = 0;                   // dual mode of the state held here
@@ -179,11 +174,10 @@ gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0,
                     uint32_t t0, cudaStream_t s, int64_t* launches);
 gda_status score_reduce(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj,
                         cudaStream_t s);
-// PDBO-s: ginc[k][b] = beta * (sum of gpart rows of group k), fixed order; mu_out = mu + sum_k ginc[k] (finalize)
-gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float beta, float* ginc, cudaStream_t s,
-                       int64_t* launches);
-gda_status mu_finalize(int32_t B, const float* mu, const float* ginc, float* mu_out, cudaStream_t s, int64_t* launches);
-gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, float* ginc, cudaStream_t s, int64_t* launches);
+// PDBO-s: mu_out[b] = mu_in[b] + beta * sum_r gpart[r][b], summed in a fixed order (deterministic)
+gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float beta, const float* mu_in, float* mu_out,
+                       cudaStream_t s, int64_t* launches);
+gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, cudaStream_t s, int64_t* launches);
 
 // ---------------------------------------------------------------------------------------------------
 // device helpers: g, g', the fused update S4 (Eq. 6 + perturbation), the tie-break hash
@@ -287,19 +281,6 @@ __device__ __forceinline__ void gda_update4(const float4& x, const float4& y, co
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
 // ---- PDBO-s helpers shared by the warp-per-(row, chunk) step kernels -------------------------------------------
-// mu^t for restarts 4 c4 .. 4 c4 + 3: the pending increment summed over its groups in index order, then added
-// (the same order as mu_finalize_kernel, so that the mu reported at the end of a run is the one the next step uses)
-__device__ __forceinline__ float4 scalar_dual_mu(const ScalarDual& sd, int B, int c4) {
-    float4 inc = ldg4(sd.ginc + 4 * c4);
-#pragma unroll
-    for (int k = 1; k < GINC_GROUPS; ++k) {
-        const float4 v = ldg4(sd.ginc + (size_t)k * B + 4 * c4);
-        inc.x += v.x; inc.y += v.y; inc.z += v.z; inc.w += v.w;
-    }
-    const float4 mu = ldg4(sd.mu_prev + 4 * c4);
-    return make_float4(mu.x + inc.x, mu.y + inc.y, mu.z + inc.z, mu.w + inc.w);
-}
-
 // One gpart row per block: the NW warps' sums of g (0 for warps without a row), added in warp order by warp 0.
 // Called by every thread of the block.
 template <int NW>

@@ -99,8 +99,8 @@ __device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, con
 }
 
 // warp-per-(variable, 128-restart chunk): blockIdx.y = chunk, the block's 8 warps take 8 consecutive variables.
-// MODE 0: fused step; MODE 1: write G only.  DUAL (PDBO-s, MODE 0): one multiplier per restart (mu^t = sd.mu_prev +
-// sd.ginc), y untouched, the block's sum of g(x_i^t) goes to sd.gpart[blockIdx.x], block 0 records mu^t.
+// MODE 0: fused step; MODE 1: write G only.  DUAL (PDBO-s, MODE 0): one multiplier per restart (sd.mu),
+// y untouched, the block's sum of g(x_i^t) goes to sd.gpart[blockIdx.x].
 template <int GFUN, int MODE, int KW, bool PAD, bool DUAL>
 __global__ void __launch_bounds__(THREADS)
 maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* __restrict__ coef,
@@ -113,7 +113,7 @@ maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* 
     const int c4 = blockIdx.y * 32 + lane;
     const bool active = 4 * c4 < B;
     float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = gs;
-    if (DUAL) mu = scalar_dual_mu(sd, B, active ? c4 : B / 4 - 1);
+    if (DUAL) mu = ldg4(sd.mu + 4 * (active ? c4 : B / 4 - 1));
     if (var < n) {                                           // warp-uniform
         const int start = __ldg(vptr + var), end = __ldg(vptr + var + 1);
         const float4 G = gather_var<KW, PAD>(coef, others, kw, start, end, x, B, c4, active, lane);
@@ -134,7 +134,6 @@ maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* 
         }
     }
     if (DUAL) {
-        if (blockIdx.x == 0 && warp == 0 && active) *reinterpret_cast<float4*>(sd.mu_cur + 4 * c4) = mu;
         scalar_dual_block_sum<WARPS>(gs, gred, warp, lane, active, sd.gpart + (size_t)blockIdx.x * B + 4 * c4);
     }
 }
@@ -214,7 +213,7 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
 
 gda_status maxsat_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
-    if (sd.mu_prev) return launch_step<0, true>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
+    if (sd.mu) return launch_step<0, true>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
     return launch_step<0, false>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
 }
 

@@ -86,9 +86,8 @@ __device__ __forceinline__ void update_store(int row, int c4, int B, bool active
 // is -1 sends the row through its CSR entries.  40 registers (6 blocks per SM).  Measured on config 3 (profiles/):
 // 17.3 us per step before, 16.3 us with the lean gather loop, 14.8 us with the records and 6 blocks per SM;
 // prefetching the row's own x, y lines into L1 up front was slower (15.1 us) and is not done.
-// DUAL (PDBO-s, MODE 0 only): the multiplier is one number per restart (mu^t = sd.mu_prev + sd.ginc), y is not
-// read or written, and the block leaves the sum of g(x_i^t) over its rows in sd.gpart[blockIdx.x]; the first block
-// of every column chunk also records mu^t in sd.mu_cur.
+// DUAL (PDBO-s, MODE 0 only): the multiplier is one number per restart (sd.mu), y is not read or written, and the
+// block leaves the sum of g(x_i^t) over its rows in sd.gpart[blockIdx.x].
 template <int GFUN, int MODE, bool ELL, bool DUAL>
 __global__ void __launch_bounds__(THREADS, 6)
 spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
@@ -102,7 +101,7 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
     const bool active = 4 * (blockIdx.y * 32 + lane) < B;
     const int c4 = active ? blockIdx.y * 32 + lane : B / 4 - 1;      // ragged B: idle lanes recompute the last float4
     if (DUAL) {
-        float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = scalar_dual_mu(sd, B, c4);
+        float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = ldg4(sd.mu + 4 * c4);
         if (ridx < n_rows) {                                 // warp-uniform
             const int row = row_list ? __ldg(row_list + ridx) : ridx;
             const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
@@ -119,7 +118,6 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
             G.x += cp; G.y += cp; G.z += cp; G.w += cp;
             update_store<GFUN, true>(row, c4, B, active, G, x, y, xn, up, (st ? st->t : 0u) + t_off, mu, gs);
         }
-        if (blockIdx.x == 0 && warp == 0 && active) *reinterpret_cast<float4*>(sd.mu_cur + 4 * c4) = mu;
         scalar_dual_block_sum<WARPS>(gs, gred, warp, lane, active, sd.gpart + (size_t)blockIdx.x * B + 4 * c4);
         return;
     }
@@ -147,15 +145,14 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
 }
 
 // row-split: one block per (heavy row, chunk); the 8 warps take interleaved 32-entry slices of the row
-// DUAL: as above; the row's g values go to sd.gpart[gpart_row0 + ridx], and block 0 records mu^t when write_mu is set
-// (there is no warp-per-row launch to do it).
+// DUAL: as above; the row's g values go to sd.gpart[gpart_row0 + ridx].
 template <int GFUN, int MODE, bool DUAL>
 __global__ void __launch_bounds__(THREADS)
 spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chunks,
                 const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                 const float* __restrict__ val2, const float* __restrict__ cprime,
                 const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
-                UpdParams up, ScalarDual sd, int gpart_row0, int write_mu, const RunState* __restrict__ st, uint32_t t_off) {
+                UpdParams up, ScalarDual sd, int gpart_row0, const RunState* __restrict__ st, uint32_t t_off) {
     __shared__ float4 red[WARPS][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ridx = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
@@ -181,8 +178,7 @@ spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chu
     const uint32_t t = (st ? st->t : 0u) + t_off;
     float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = gs;
     if (DUAL) {
-        mu = scalar_dual_mu(sd, B, c4);
-        if (write_mu && ridx == 0 && active) *reinterpret_cast<float4*>(sd.mu_cur + 4 * c4) = mu;
+        mu = ldg4(sd.mu + 4 * c4);
     }
     update_store<GFUN, DUAL>(row, c4, B, active, G, x, y, xn, up, t, mu, gs);
     if (DUAL && active) *reinterpret_cast<float4*>(sd.gpart + (size_t)(gpart_row0 + ridx) * B + 4 * c4) = gs;
@@ -271,13 +267,12 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     }
     if (p->n_heavy > 0) {
         const unsigned grid = (unsigned)(p->n_heavy * chunks);
-        const int write_mu = n_light > 0 ? 0 : 1;
         if (up.gfun == GDA_G_QUADRATIC)
             spmm_step_split<GDA_G_QUADRATIC, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, light_blocks, write_mu, st, t_off);
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, light_blocks, st, t_off);
         else
             spmm_step_split<GDA_G_ENTROPY, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, light_blocks, write_mu, st, t_off);
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, light_blocks, st, t_off);
         if (launches) ++*launches;
     }
     GDA_CUDA_TRY(cudaGetLastError());
@@ -290,7 +285,7 @@ int sparse_heavy_threshold() { return HEAVY_DEG; }
 
 gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
-    if (sd.mu_prev) return launch_step<0, true>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
+    if (sd.mu) return launch_step<0, true>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
     return launch_step<0, false>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
 }
 
