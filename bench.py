@@ -372,8 +372,13 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--B", type=int, default=None)
     ap.add_argument("--pdbo-s", action="store_true", help="run the PDBO-s ablation (one multiplier per restart, PAPER.md:630-648)")
+    ap.add_argument("--mis", default=None, metavar="N,D", help="instead of --config: MIS as a QUBO on a D-regular graph with N vertices (PAPER.md:1030-1036)")
     args = ap.parse_args()
-    w = wl.config(args.config, B=args.B)
+    if args.mis:
+        n_mis, d_mis = (int(v) for v in args.mis.split(","))
+        w = wl.mis(n_mis, d_mis, B=args.B or 12)
+    else:
+        w = wl.config(args.config, B=args.B)
     if args.pdbo_s:
         w = wl.pdbo_s_variant(w)
     if args.impl == "reference":

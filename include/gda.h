@@ -108,6 +108,9 @@ typedef struct {
     double* trace_best;   /* [trace_cap] min over restarts of the best objective after evaluation k     */
     uint64_t* trace_ns;   /* [trace_cap] GPU globaltimer (ns) when evaluation k finished                */
     int32_t trace_cap;    /* entries available in the two trace arrays (evaluations beyond it are dropped) */
+    int32_t* ones;        /* [B]    number of ones in x_bin[:, b].  With obj it decides feasibility where the     *
+                           *        objective is a penalised count, e.g. MIS as a QUBO:      *
+                           *        F = -|S| + lam * (edges inside S), so S is independent iff obj[b] == -ones[b] */
 } gda_extra;
 
 /* Algorithm 1 (reconstructed in DESIGN.md reading R0) for B restarts.

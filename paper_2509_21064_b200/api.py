@@ -35,7 +35,7 @@ class Params(C.Structure):
 
 class Extra(C.Structure):
     _fields_ = [("x_final", C.c_void_p), ("lambda_final", C.c_void_p), ("best_obj", C.c_void_p),
-                ("trace_best", C.c_void_p), ("trace_ns", C.c_void_p), ("trace_cap", C.c_int32)]
+                ("trace_best", C.c_void_p), ("trace_ns", C.c_void_p), ("trace_cap", C.c_int32), ("ones", C.c_void_p)]
 
 
 class Info(C.Structure):
@@ -135,9 +135,9 @@ class Problem:
             pass
 
     # ---- gda_run --------------------------------------------------------------------------------
-    def run(self, x0, lambda0, params: Params, *, want_final=False, trace_cap=0, stream=None):
+    def run(self, x0, lambda0, params: Params, *, want_final=False, trace_cap=0, want_ones=False, stream=None):
         """x0: CUDA float32 tensor [n][B]; lambda0: tensor [n][B] ([B] with params.dual = DUAL_SCALAR) or a float (y-bar).
-        Returns dict of CUDA tensors: x_bin, obj, best_restart (+ x, lam, best_obj, trace_best, trace_ns).
+        Returns dict of CUDA tensors: x_bin, obj, best_restart (+ x, lam, best_obj, ones, trace_best, trace_ns).
         Asynchronous on `stream` (default: torch's current stream)."""
         import torch
         assert x0.is_cuda and x0.dtype == torch.float32 and x0.is_contiguous() and x0.shape[0] == self.n
@@ -160,6 +160,9 @@ class Problem:
             out["lam"] = torch.empty(B, dtype=torch.float32, device=dev) if params.dual == DUAL_SCALAR else torch.empty_like(x0)
             out["best_obj"] = torch.empty(1, dtype=torch.float64, device=dev)
             ex.x_final, ex.lambda_final, ex.best_obj = out["x"].data_ptr(), out["lam"].data_ptr(), out["best_obj"].data_ptr()
+        if want_ones:
+            out["ones"] = torch.empty(B, dtype=torch.int32, device=dev)
+            ex.ones = out["ones"].data_ptr()
         if trace_cap > 0:
             out["trace_best"] = torch.full((trace_cap,), float("nan"), dtype=torch.float64, device=dev)
             out["trace_ns"] = torch.zeros(trace_cap, dtype=torch.int64, device=dev)

@@ -560,6 +560,7 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
             GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.mu[parity], (size_t)B * sizeof(float), cudaMemcpyDeviceToDevice, s));
         else if (extra->lambda_final)
             GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.y, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        if (extra->ones) GDA_TRY(eval_count_ones(p, B, ws.x_bin, extra->ones, s, &p->last_launches));
         if (extra->best_obj) GDA_CUDA_TRY(cudaMemcpyAsync(extra->best_obj, ws.best_val, sizeof(double), cudaMemcpyDeviceToDevice, s));
         const int32_t n_eval = std::max(1, full + (rem > 0 ? 1 : 0));
         const int32_t cnt = std::min(std::min(n_eval, extra->trace_cap), ws.trace_cap);

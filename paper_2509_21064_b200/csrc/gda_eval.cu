@@ -152,6 +152,30 @@ gsum_reduce_kernel(int B, const float* __restrict__ gpart, int n_gpart, float be
     }
 }
 
+// ones[b] = sum_i x_bin[i][b]: block = 128 restarts (uchar4 per lane) x 32 row slices, integer sums
+__global__ void __launch_bounds__(1024)
+count_ones_kernel(int n, int B, const uint8_t* __restrict__ x_bin, int32_t* __restrict__ ones) {
+    __shared__ int red[32][32][4];
+    const int lane = threadIdx.x, slice = threadIdx.y;
+    const int c = blockIdx.x * 128 + 4 * lane;
+    int acc[4] = {0, 0, 0, 0};
+    if (c < B)
+        for (int i = slice; i < n; i += 32) {
+            const uchar4 v = *reinterpret_cast<const uchar4*>(x_bin + (size_t)i * B + c);
+            acc[0] += v.x; acc[1] += v.y; acc[2] += v.z; acc[3] += v.w;
+        }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) red[slice][lane][q] = acc[q];
+    __syncthreads();
+    if (slice == 0 && c < B)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            int t = 0;
+            for (int k = 0; k < 32; ++k) t += red[k][lane][q];
+            ones[c + q] = t;
+        }
+}
+
 __global__ void mu_init_kernel(int B, const float* __restrict__ l0, float l0_scalar, float* __restrict__ mu) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b < B) mu[b] = l0 ? l0[b] : l0_scalar;
@@ -219,6 +243,13 @@ gda_status eval_commit(gda_problem* p, int32_t B, const float* x, const int32_t*
                        cudaStream_t s, int64_t* launches) {
     const size_t n_vec = (size_t)p->n * B / 4;
     commit_kernel<<<(unsigned)((n_vec + 255) / 256), 256, 0, s>>>(n_vec, B / 4, x, improved, x_bin);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status eval_count_ones(gda_problem* p, int32_t B, const uint8_t* x_bin, int32_t* ones, cudaStream_t s, int64_t* launches) {
+    count_ones_kernel<<<(unsigned)((B + 127) / 128), dim3(32, 32), 0, s>>>(p->n, B, x_bin, ones);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;

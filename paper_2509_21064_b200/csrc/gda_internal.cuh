@@ -170,6 +170,7 @@ gda_status eval_commit(gda_problem* p, int32_t B, const float* x, const int32_t*
                        cudaStream_t s, int64_t* launches);
 gda_status eval_argbest(int32_t B, const double* obj, int32_t* best_restart, double* best_val,
                         cudaStream_t s, int64_t* launches);
+gda_status eval_count_ones(gda_problem* p, int32_t B, const uint8_t* x_bin, int32_t* ones, cudaStream_t s, int64_t* launches);
 gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0, float l0_scalar,
                     uint32_t t0, cudaStream_t s, int64_t* launches);
 gda_status score_reduce(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj,

@@ -137,6 +137,61 @@ def maxcut_as_qubo(n: int, edges: np.ndarray, w: np.ndarray) -> QuboCSR:
                    c=(-wdeg).astype(np.float32), edges=edges, edge_w=w.astype(np.float32))
 
 
+def edges_regular(n: int, d: int, seed: int) -> np.ndarray:
+    """A simple d-regular graph on n vertices (n * d even) as the union of d perfect matchings (n even) drawn one
+    after the other; pairs that repeat an earlier edge are re-drawn among themselves and a few fresh pairs until
+    none is left.  Shape of the d-RRGs of the paper's MIS experiment, not a uniform sample."""
+    if n % 2 or d >= n:
+        raise ValueError("edges_regular needs an even n and d < n")
+    rng = np.random.Generator(np.random.PCG64(seed))
+    seen = set()
+    out = []
+    for _ in range(d):
+        perm = rng.permutation(n)
+        a, b = perm[0::2].copy(), perm[1::2].copy()
+        for _try in range(10000):
+            lo, hi = np.minimum(a, b), np.maximum(a, b)
+            code = lo.astype(np.int64) * n + hi
+            bad = np.array([c in seen for c in code.tolist()], dtype=bool)
+            if not bad.any():
+                break
+            pick = bad.copy()
+            pick[rng.integers(0, a.shape[0], size=max(4, int(bad.sum())))] = True      # some freedom to re-pair
+            verts = rng.permutation(np.concatenate([a[pick], b[pick]]))
+            a[pick], b[pick] = verts[0::2], verts[1::2]
+        else:
+            raise RuntimeError("edges_regular: could not complete a matching")
+        seen.update(code.tolist())
+        out.append(np.stack([lo, hi], axis=1))
+    return np.concatenate(out).astype(np.int64)
+
+
+def mis_as_qubo(n: int, edges: np.ndarray, lam: float = 4.0) -> QuboCSR:
+    """Maximum independent set as the QUBO  min -sum_i x_i + lam sum_{(i,j) in E} x_i x_j  (PAPER.md:1026-1028,
+    lam = 4): Q = (lam/2) A with A the symmetric adjacency matrix, c = -1.  For binary x,
+    F(x) = -|S| + lam * (number of edges inside S): S is independent iff F(x) = -|S|."""
+    i = np.concatenate([edges[:, 0], edges[:, 1]])
+    j = np.concatenate([edges[:, 1], edges[:, 0]])
+    order = np.lexsort((j, i))
+    i, j = i[order], j[order]
+    rowptr = np.zeros(n + 1, dtype=np.int64)
+    np.add.at(rowptr, i + 1, 1)
+    return QuboCSR(n=n, rowptr=np.cumsum(rowptr).astype(np.int32), col=j.astype(np.int32),
+                   val=np.full(i.shape[0], 0.5 * lam, dtype=np.float32), c=np.full(n, -1.0, dtype=np.float32),
+                   edges=edges, edge_w=np.full(edges.shape[0], lam, dtype=np.float32))
+
+
+def mis(n: int, d: int, B: int = 12, seed: int = 106, iters: int = 5000) -> Workload:
+    """MIS on a d-regular graph (d in {3, 100}, n in {1e4, 5e4}); Table 6: ybar = 5,
+    alpha = beta = 0.02, B = 10 (12 here: restarts come in multiples of 4).  With lam = 4 and degree d the no-flip
+    rule of reading R7 asks for alpha (lam d + ybar) < 1, which Table 6's alpha meets for d = 3 only; for larger d
+    alpha is scaled to 0.4 / (lam d / 2 + ybar)."""
+    P = mis_as_qubo(n, edges_regular(n, d, seed), 4.0)
+    alpha = 0.02 if d <= 8 else 0.4 / (2.0 * d + 5.0)
+    return Workload(f"mis_n{n}_d{d}", "qubo_csr", P, B, Hyper(5.0, alpha, 0.02, 1e-4, 0, 1e-6, iters, 100, seed),
+                    1000 + seed, f"MIS as QUBO (lam=4) on a {d}-regular graph")
+
+
 def round_to_bf16(a: np.ndarray) -> np.ndarray:
     """Round float32 values to the nearest bf16-representable value (ties to even), kept as float32."""
     u = np.ascontiguousarray(a, dtype=np.float32).view(np.uint32).astype(np.uint64)

@@ -33,7 +33,7 @@ def test_every_declared_symbol_is_exported(L):
 
 def test_struct_layouts_match_header():
     assert C.sizeof(api.Params) == 48 and api.Params.seed.offset == 32 and api.Params.dual.offset == 40
-    assert C.sizeof(api.Extra) == 48
+    assert C.sizeof(api.Extra) == 56 and api.Extra.ones.offset == 48
     assert C.sizeof(api.Info) == 40
 
 

@@ -595,3 +595,30 @@ def test_pdbo_s_heavy_rows_and_argument_checks(api, oracle):
         Pd.run(dev(wl.x0_uniform(wd.problem.n, 128, 1)), 1.0, api.params_from_hyper(wd.hyper, iters=1, dual=api.DUAL_SCALAR))
     assert e.value.status == 4
     Pd.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# MIS as a QUBO: linear term c = -1, Q = (lam/2) A; feasibility from (obj, ones)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,d,B", [(600, 3, 12), (400, 40, 8)])
+def test_mis_objective_cardinality_and_feasibility(api, oracle, n, d, B):
+    w = wl.mis(n, d, B=B, iters=2500)
+    OP = oracle_problem(w.problem)
+    P = api.create_from_workload(w.problem)
+    h, E = w.hyper, w.problem.edges
+    X0 = wl.x0_uniform(n, B, w.x0_seed)
+    assert grad_rel_err(P.grad(dev(X0)).cpu().numpy(), oracle.grad(OP, X0.astype(np.float64))) <= TOL_STEP
+    r1 = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+    ref1 = oracle.run(OP, X0, f32(h.lambda0), **okw(h, iters=1, eval_every=1))
+    assert np.abs(r1["x"].cpu().numpy() - ref1["x"]).max() <= TOL_STEP
+    r = P.run(dev(X0), h.lambda0, api.params_from_hyper(h), want_ones=True)
+    obj, xb, ones = r["obj"].cpu().numpy(), r["x_bin"].cpu().numpy(), r["ones"].cpu().numpy()
+    assert np.array_equal(obj, oracle.F_binary(OP, xb))                        # (a) exact objective
+    assert np.array_equal(ones, xb.sum(axis=0))                                # cardinality of the returned sets
+    inside = (xb[E[:, 0]] & xb[E[:, 1]]).sum(axis=0)                           # edges inside each set, by the edge list
+    assert np.array_equal(obj, -ones + 4.0 * inside)
+    assert np.array_equal(obj == -ones, inside == 0)                           # the feasibility rule of include/gda.h
+    ref = oracle.run(OP, X0, f32(h.lambda0), nthreads=4, **okw(h))
+    assert_statistics_close(obj, ref["obj"])                                   # (d)
+    assert (inside == 0).mean() >= 0.75 and -obj.min() > 0.3 * n / (1 + np.log(d))   # independent sets of sensible size
+    P.destroy()

@@ -62,3 +62,23 @@ def test_dense_qubo_is_bf16_representable_and_symmetric():
     assert np.all((P.Q.view(np.uint32) & 0xFFFF) == 0)          # low 16 mantissa bits are zero: exact in bf16
     r = wl.round_to_bf16(np.array([1.0, 1.00390625, 1.01171875, 3.14159], dtype=np.float32))
     assert r[0] == 1.0 and r[1] == 1.0 and r[2] == 1.015625     # ties to even
+
+
+def test_regular_graph_and_mis_qubo():
+    for n, d in ((60, 3), (40, 12)):
+        e = wl.edges_regular(n, d, 5)
+        assert e.shape == (n * d // 2, 2) and (e[:, 0] < e[:, 1]).all()
+        assert len({(int(a), int(b)) for a, b in e}) == e.shape[0]              # simple graph
+        assert (np.bincount(e.ravel(), minlength=n) == d).all()                 # d-regular
+        assert np.array_equal(e, wl.edges_regular(n, d, 5))                     # seeded
+        P = wl.mis_as_qubo(n, e, 4.0)
+        # F(x) = -|S| + lam * (edges inside S), checked by the edge list on random sets
+        rng = np.random.default_rng(0)
+        Q = np.zeros((n, n))
+        for i in range(n):
+            Q[i, P.col[P.rowptr[i]:P.rowptr[i + 1]]] = P.val[P.rowptr[i]:P.rowptr[i + 1]]
+        assert np.array_equal(Q, Q.T)
+        for _ in range(20):
+            x = (rng.random(n) < 0.3).astype(np.float64)
+            inside = int((x[e[:, 0]] * x[e[:, 1]]).sum())
+            assert x @ Q @ x + P.c @ x == -x.sum() + 4.0 * inside
