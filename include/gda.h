@@ -88,7 +88,7 @@ typedef enum { GDA_DUAL_PER_VARIABLE = 0, GDA_DUAL_SCALAR = 1 } gda_dual;
 
 typedef struct {
     float alpha;        /* primal step size > 0                                          */
-    float beta;         /* dual step size > 0                                          */
+    float beta;         /* dual step size >= 0; 0 keeps the multipliers fixed   */
     float delta;        /* perturbation band half-width in [0, 1/2); 0 disables (R3) */
     float log_eps;      /* clamp for g' of the entropy g, in (0, 1/2) (R4); ignored for the quadratic g */
     int32_t iters;      /* T_max >= 0: exactly this many GDA steps (R0)                                 */
@@ -122,7 +122,7 @@ typedef struct {
  *               objective seen at any evaluation (R5)
  *   obj         DEVICE double [B]: F(x_bin[:,b]) -- exact integers when all coefficients are integers
  *   best_restart DEVICE int32 [1]: argmin_b obj[b], ties -> lowest b (R6)
- * INVALID_ARG: null required pointer, B <= 0 or B % 4 != 0, alpha/beta <= 0 or non-finite, delta outside
+ * INVALID_ARG: null required pointer, B <= 0 or B % 4 != 0, alpha <= 0, beta < 0 or non-finite, delta outside
  * [0, 1/2), eval_every <= 0, iters < 0, unknown gfun or dual, log_eps outside (0, 1/2) with the entropy g;
  * a resumed run (x0 == NULL) whose `dual` differs from the run it continues.                              */
 gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const float* lambda0, float lambda0_scalar,
@@ -140,6 +140,16 @@ gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, const float*
  * gda_score: obj[b] = F(x_hat), x_hat = [X[:,b] > 1/2]; DEVICE fp32 X [n][B], DEVICE double obj[B] (S5). */
 gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float* G, void* stream);
 gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, void* stream);
+
+/* gda_lagrangian: out[b] = L(X[:,b], Y[:,b]) = f(x) + sum_i y_i g(x_i) at a CONTINUOUS point:
+ * f is the multilinear extension, products in fp32, sums in fp64.  DEVICE fp32 X [n][B] in [0,1];
+ * lambda DEVICE fp32 [n][B] or NULL -> every y_i = lambda_scalar; gfun / log_eps as in gda_params; DEVICE double out[B].
+ * This is the value behind the dual certificate of PAPER.md:1105-1114: for y with f_y = L(., y) convex (Max-Cut:
+ * y_i >= -lambda_min(W)), run gda_run with beta = 0 (the multipliers stay at lambda0) until x has converged; then
+ * out[b] <= min F, i.e. -out[b] is an upper bound on the maximum cut.  Sparse QUBO and MaxSAT problems (dense:
+ * UNSUPPORTED). */
+gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, const float* lambda, float lambda_scalar,
+                          int32_t gfun, float log_eps, double* out, void* stream);
 
 /* ---- queries ------------------------------------------------------------------------------------------ */
 typedef struct {

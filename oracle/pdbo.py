@@ -138,6 +138,19 @@ def f_ext(P: Problem, X: np.ndarray, precision: str = "f64") -> np.ndarray:
     return out
 
 
+def lagrangian(P: Problem, X: np.ndarray, Y, gfun: int = G_QUADRATIC, precision: str = "f64") -> np.ndarray:
+    """out[b] = L(X[:,b], Y[:,b]) = f(x) + sum_i y_i g(x_i).  Y an [n][B] array or a scalar."""
+    rt = _real(precision)
+    X = np.ascontiguousarray(X, dtype=rt)
+    Ya = np.full(X.shape, Y, dtype=rt) if np.isscalar(Y) else np.ascontiguousarray(Y, dtype=rt)
+    assert Ya.shape == X.shape
+    out = np.empty(X.shape[1], dtype=np.float64)
+    rc = _lib(precision).pdbo_lagrangian(C.byref(P.struct), C.c_int32(X.shape[1]), C.c_void_p(X.ctypes.data),
+                                         C.c_void_p(Ya.ctypes.data), C.c_int32(gfun), C.c_void_p(out.ctypes.data))
+    assert rc == 0
+    return out
+
+
 def F_binary(P: Problem, Xh: np.ndarray) -> np.ndarray:
     """out[b] = F(Xh[:,b]) for binary columns (uint8 [n][B])."""
     Xh = np.ascontiguousarray(Xh, dtype=np.uint8)

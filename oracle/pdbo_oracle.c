@@ -274,6 +274,24 @@ int pdbo_f(const pdbo_problem* P, int32_t B, const real* X, double* out) {
     return 0;
 }
 
+/* out[b] = L(X[:,b], Y[:,b]) = f(x) + sum_i y_i g(x_i); the value whose minimum over x, for y
+ * with L(., y) convex, is the dual certificate of PAPER.md:1105-1114. */
+int pdbo_lagrangian(const pdbo_problem* P, int32_t B, const real* X, const real* Y, int32_t gfun, double* out) {
+    const int n = P->n;
+    real* x = (real*)malloc(sizeof(real) * n);
+    if (!x) return 1;
+    for (int b = 0; b < B; ++b) {
+        double constraint = 0.0;
+        for (int i = 0; i < n; ++i) {
+            x[i] = X[(size_t)i * B + b];
+            constraint += (double)Y[(size_t)i * B + b] * (double)g_fun(gfun, x[i]);
+        }
+        out[b] = f_ext(P, x) + constraint;
+    }
+    free(x);
+    return 0;
+}
+
 /* out[b] = F(Xh[:,b]) on binary columns. */
 int pdbo_F(const pdbo_problem* P, int32_t B, const uint8_t* Xh, double* out) {
     const int n = P->n;

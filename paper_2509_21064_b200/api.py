@@ -45,7 +45,7 @@ class Info(C.Structure):
 
 
 EXPORTS = ["gda_create_qubo_csr", "gda_create_qubo_dense", "gda_create_maxsat", "gda_destroy", "gda_run",
-           "gda_run_host", "gda_grad", "gda_score", "gda_get_info", "gda_last_error", "gda_version"]
+           "gda_run_host", "gda_grad", "gda_score", "gda_lagrangian", "gda_get_info", "gda_last_error", "gda_version"]
 
 
 def lib():
@@ -66,6 +66,7 @@ def lib():
         L.gda_run_host.argtypes = [vp, i32, vp, vp, f32, C.POINTER(Params), vp, vp, vp, vp]
         L.gda_grad.argtypes = [vp, i32, vp, vp, vp]
         L.gda_score.argtypes = [vp, i32, vp, vp, vp]
+        L.gda_lagrangian.argtypes = [vp, i32, vp, vp, f32, i32, f32, vp, vp]
         L.gda_get_info.argtypes = [vp, C.POINTER(Info)]
         L.gda_last_error.restype = C.c_char_p
         L.gda_version.restype = C.c_char_p
@@ -220,6 +221,21 @@ class Problem:
         s = torch.cuda.current_stream(x.device).cuda_stream if stream is None else stream
         _check(lib().gda_score(self._h, x.shape[1], x.data_ptr(), obj.data_ptr(), s))
         return obj
+
+    def lagrangian(self, x, lam, gfun=G_QUADRATIC, log_eps=1e-6, stream=None):
+        """gda_lagrangian: L(x, y) = f(x) + sum_i y_i g(x_i) per restart; lam a CUDA tensor [n][B] or a float."""
+        import torch
+        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.shape[0] == self.n
+        out = torch.empty(x.shape[1], dtype=torch.float64, device=x.device)
+        l_ptr, l_scalar = None, 0.0
+        if isinstance(lam, torch.Tensor):
+            assert lam.is_cuda and lam.dtype == torch.float32 and lam.is_contiguous() and lam.shape == x.shape
+            l_ptr = lam.data_ptr()
+        else:
+            l_scalar = float(lam)
+        s = torch.cuda.current_stream(x.device).cuda_stream if stream is None else stream
+        _check(lib().gda_lagrangian(self._h, x.shape[1], x.data_ptr(), l_ptr, l_scalar, gfun, log_eps, out.data_ptr(), s))
+        return out
 
     def info(self) -> Info:
         inf = Info()

@@ -353,7 +353,8 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     if (st == GDA_OK) st = dmalloc(&ws.obj_now, (size_t)B);
     if (st == GDA_OK) st = dmalloc(&ws.improved, (size_t)B);
     ws.n_part = num_partials(p, B);
-    if (st == GDA_OK) st = dmalloc((double**)&ws.partial, (size_t)ws.n_part * B);
+    // + room for the y g(x) partial rows of gda_lagrangian
+    if (st == GDA_OK) st = dmalloc((double**)&ws.partial, ((size_t)ws.n_part + (size_t)(p->n + 63) / 64) * B);
     if (p->kind != GDA_KIND_DENSE) {                          // PDBO-s state (a few rows of B floats)
         ws.n_gpart = p->kind == GDA_KIND_SPARSE ? sparse_num_gparts(p) : maxsat_num_gparts(p);
         if (st == GDA_OK) st = dmalloc(&ws.mu[0], (size_t)B);
@@ -492,7 +493,7 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
                 "gda_run: x0 is NULL but the handle holds no state of a previous run with B = %d to resume", B);
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_run: B must be a positive multiple of 4 (got %d)", B);
     GDA_REQUIRE(std::isfinite(prm->alpha) && prm->alpha > 0.0f, "gda_run: alpha must be > 0");
-    GDA_REQUIRE(std::isfinite(prm->beta) && prm->beta > 0.0f, "gda_run: beta must be > 0");
+    GDA_REQUIRE(std::isfinite(prm->beta) && prm->beta >= 0.0f, "gda_run: beta must be >= 0");
     GDA_REQUIRE(prm->delta >= 0.0f && prm->delta < 0.5f, "gda_run: delta must be in [0, 1/2)");
     GDA_REQUIRE(prm->eval_every > 0, "gda_run: eval_every must be > 0");
     GDA_REQUIRE(prm->iters >= 0, "gda_run: iters must be >= 0");
@@ -648,4 +649,24 @@ extern "C" gda_status gda_get_info(const gda_problem* p, gda_info* info) {
     info->last_run_kernel_launches = p->last_launches;
     info->last_run_step_launches = p->last_step_launches;
     return GDA_OK;
+}
+
+extern "C" gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, const float* lambda, float lambda_scalar,
+                                     int32_t gfun, float log_eps, double* out, void* stream) {
+    GDA_REQUIRE(p != nullptr && x != nullptr && out != nullptr, "gda_lagrangian: null argument");
+    GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_lagrangian: B must be a positive multiple of 4 (got %d)", B);
+    GDA_REQUIRE(gfun == GDA_G_QUADRATIC || gfun == GDA_G_ENTROPY, "gda_lagrangian: unknown gfun %d", gfun);
+    if (gfun == GDA_G_ENTROPY) GDA_REQUIRE(log_eps > 0.0f && log_eps < 0.5f, "gda_lagrangian: log_eps must be in (0, 1/2)");
+    if (p->kind == GDA_KIND_DENSE) { gda_set_error("gda_lagrangian: sparse QUBO and MaxSAT problems only"); return GDA_ERR_UNSUPPORTED; }
+    GDA_CUDA_TRY(cudaSetDevice(p->device));
+    GDA_TRY(ensure_workspace(p, B));
+    cudaStream_t user, s;
+    GDA_TRY(pick_stream(p, stream, &user, &s));
+    double* part = static_cast<double*>(p->ws.partial);
+    int32_t n_f = 0, n_g = 0;
+    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_value_partials(p, B, x, part, &n_f, s));
+    else GDA_TRY(maxsat_value_partials(p, B, x, part, &n_f, s));
+    GDA_TRY(eval_yg_partials(p, B, x, lambda, lambda_scalar, gfun, log_eps, part + (size_t)n_f * B, &n_g, s));
+    GDA_TRY(eval_sum_partials(B, part, n_f + n_g, out, s));
+    return join_stream(p, user, s);
 }

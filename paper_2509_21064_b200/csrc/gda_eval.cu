@@ -152,6 +152,38 @@ gsum_reduce_kernel(int B, const float* __restrict__ gpart, int n_gpart, float be
     }
 }
 
+// partial[rb][b] = sum over the 64 rows of block rb of y_i g(x_i)   (the constraint part of L)
+template <int GFUN>
+__global__ void __launch_bounds__(256)
+yg_partials_kernel(int n, int B, const float* __restrict__ x, const float* __restrict__ y, float y_scalar,
+                   UpdParams up, double* __restrict__ partial) {
+    __shared__ double red[8][32][4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c4 = blockIdx.y * 32 + lane;
+    const bool active = 4 * c4 < B;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    if (active)
+        for (int r = warp; r < 64; r += 8) {
+            const int row = blockIdx.x * 64 + r;
+            if (row >= n) break;
+            const size_t off = (size_t)row * B + 4 * c4;
+            const float4 xv = ldg4(x + off);
+            const float4 yv = y ? ldg4(y + off) : make_float4(y_scalar, y_scalar, y_scalar, y_scalar);
+            acc[0] += (double)(yv.x * gda_g<GFUN>(xv.x, up)); acc[1] += (double)(yv.y * gda_g<GFUN>(xv.y, up));
+            acc[2] += (double)(yv.z * gda_g<GFUN>(xv.z, up)); acc[3] += (double)(yv.w * gda_g<GFUN>(xv.w, up));
+        }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) red[warp][lane][q] = acc[q];
+    __syncthreads();
+    if (warp == 0 && active)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            double t = red[0][lane][q];
+            for (int w = 1; w < 8; ++w) t += red[w][lane][q];
+            partial[(size_t)blockIdx.x * B + 4 * c4 + q] = t;
+        }
+}
+
 // ones[b] = sum_i x_bin[i][b]: block = 128 restarts (uchar4 per lane) x 32 row slices, integer sums
 __global__ void __launch_bounds__(1024)
 count_ones_kernel(int n, int B, const uint8_t* __restrict__ x_bin, int32_t* __restrict__ ones) {
@@ -244,6 +276,24 @@ gda_status eval_commit(gda_problem* p, int32_t B, const float* x, const int32_t*
     const size_t n_vec = (size_t)p->n * B / 4;
     commit_kernel<<<(unsigned)((n_vec + 255) / 256), 256, 0, s>>>(n_vec, B / 4, x, improved, x_bin);
     if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status eval_yg_partials(gda_problem* p, int32_t B, const float* x, const float* y, float y_scalar, int32_t gfun,
+                            float log_eps, double* partial, int32_t* n_part, cudaStream_t s) {
+    UpdParams up{};
+    up.log_eps = log_eps; up.gfun = gfun;
+    const dim3 grid((unsigned)((p->n + 63) / 64), (unsigned)((B / 4 + 31) / 32));
+    if (gfun == GDA_G_QUADRATIC) yg_partials_kernel<GDA_G_QUADRATIC><<<grid, 256, 0, s>>>(p->n, B, x, y, y_scalar, up, partial);
+    else yg_partials_kernel<GDA_G_ENTROPY><<<grid, 256, 0, s>>>(p->n, B, x, y, y_scalar, up, partial);
+    *n_part = (int32_t)grid.x;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status eval_sum_partials(int32_t B, const double* partial, int32_t n_part, double* out, cudaStream_t s) {
+    finalize_kernel<false><<<1, FIN_THREADS, 0, s>>>(B, partial, n_part, out, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0);
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
 }

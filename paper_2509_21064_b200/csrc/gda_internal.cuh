@@ -138,6 +138,8 @@ gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cuda
 gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
                                  cudaStream_t s, int64_t* launches);
 int32_t sparse_num_partials(const gda_problem* p, int32_t B);
+// f(x) (continuous x) as per-block partial sums, one row per block of 64 rows; returns the rows written
+gda_status sparse_value_partials(gda_problem* p, int32_t B, const float* x, double* partial, int32_t* n_part, cudaStream_t s);
 
 // MaxSAT (gda_maxsat.cu)
 gda_status maxsat_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
@@ -147,6 +149,7 @@ gda_status maxsat_grad(gda_problem* p, int32_t B, const float* x, float* G, cuda
 gda_status maxsat_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
                                  cudaStream_t s, int64_t* launches);
 int32_t maxsat_num_partials(const gda_problem* p, int32_t B);
+gda_status maxsat_value_partials(gda_problem* p, int32_t B, const float* x, double* partial, int32_t* n_part, cudaStream_t s);
 
 // dense QUBO (gda_dense.cu)
 gda_status dense_prepare(gda_problem* p, const float* Q_host, const float* c_host);   // at create
@@ -170,6 +173,10 @@ gda_status eval_commit(gda_problem* p, int32_t B, const float* x, const int32_t*
                        cudaStream_t s, int64_t* launches);
 gda_status eval_argbest(int32_t B, const double* obj, int32_t* best_restart, double* best_val,
                         cudaStream_t s, int64_t* launches);
+// sum_i y_i g(x_i) as partial sums over blocks of 64 rows (y == nullptr: y_scalar); double reduction of partial rows
+gda_status eval_yg_partials(gda_problem* p, int32_t B, const float* x, const float* y, float y_scalar, int32_t gfun,
+                            float log_eps, double* partial, int32_t* n_part, cudaStream_t s);
+gda_status eval_sum_partials(int32_t B, const double* partial, int32_t n_part, double* out, cudaStream_t s);
 gda_status eval_count_ones(gda_problem* p, int32_t B, const uint8_t* x_bin, int32_t* ones, cudaStream_t s, int64_t* launches);
 gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0, float l0_scalar,
                     uint32_t t0, cudaStream_t s, int64_t* launches);

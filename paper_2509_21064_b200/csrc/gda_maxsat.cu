@@ -182,6 +182,42 @@ maxsat_score(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __re
     }
 }
 
+// f(x) at a continuous point: partial[cb][b] = sum over the clauses of block cb of w_j prod_{l in C_j} p_l(x)
+// (PAPER.md:196); products in fp32, sums in fp64
+__global__ void __launch_bounds__(THREADS)
+maxsat_value(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __restrict__ lit,
+             const float* __restrict__ w, const float* __restrict__ x, double* __restrict__ partial) {
+    __shared__ double red[WARPS][32][4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c4 = blockIdx.y * 32 + lane;
+    const bool active = 4 * c4 < B;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    if (active)
+        for (int r = warp; r < SCORE_CLAUSES; r += WARPS) {
+            const int j = blockIdx.x * SCORE_CLAUSES + r;
+            if (j >= m) break;
+            const float wj = __ldg(w + j);
+            float4 prod = make_float4(wj, wj, wj, wj);
+            for (int a = __ldg(cptr + j); a < __ldg(cptr + j + 1); ++a) {
+                const int l = __ldg(lit + a);
+                const float4 g = ldg4(x + (size_t)((l > 0 ? l : -l) - 1) * B + 4 * c4);
+                if (l > 0) { prod.x *= 1.0f - g.x; prod.y *= 1.0f - g.y; prod.z *= 1.0f - g.z; prod.w *= 1.0f - g.w; }
+                else { prod.x *= g.x; prod.y *= g.y; prod.z *= g.z; prod.w *= g.w; }
+            }
+            acc[0] += (double)prod.x; acc[1] += (double)prod.y; acc[2] += (double)prod.z; acc[3] += (double)prod.w;
+        }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) red[warp][lane][q] = acc[q];
+    __syncthreads();
+    if (warp == 0 && active)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            double t = red[0][lane][q];
+            for (int k = 1; k < WARPS; ++k) t += red[k][lane][q];
+            partial[(size_t)blockIdx.x * B + 4 * c4 + q] = t;
+        }
+}
+
 template <int GFUN, int MODE, bool DUAL>
 void launch_kw(gda_problem* p, int32_t B, dim3 grid, const float* x, float* y, float* xn,
                const UpdParams& up, const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s) {
@@ -236,6 +272,14 @@ gda_status maxsat_score_partials(gda_problem* p, int32_t B, const float* x, void
     else
         maxsat_score<false><<<grid, THREADS, 0, s>>>(p->m, B, p->d_cptr, p->d_lit, p->d_w, x, partial);
     if (launches) ++*launches;
+    *n_part = (int32_t)grid.x;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status maxsat_value_partials(gda_problem* p, int32_t B, const float* x, double* partial, int32_t* n_part, cudaStream_t s) {
+    const dim3 grid((unsigned)maxsat_num_partials(p, B), (unsigned)((B / 4 + 31) / 32));
+    maxsat_value<<<grid, THREADS, 0, s>>>(p->m, B, p->d_cptr, p->d_lit, p->d_w, x, partial);
     *n_part = (int32_t)grid.x;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;

@@ -248,6 +248,39 @@ spmm_score(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __re
     }
 }
 
+// f(x) at a continuous point (multilinear extension of the QUBO, reading R1):
+// partial[rb][b] = sum over the rows of block rb of x_i ((Q_off x)_i + c'_i); products in fp32, sums in fp64
+__global__ void __launch_bounds__(THREADS)
+spmm_value(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+           const float* __restrict__ val2, const float* __restrict__ cprime, const float* __restrict__ x,
+           double* __restrict__ partial) {
+    __shared__ double red[WARPS][32][4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool active = 4 * (blockIdx.y * 32 + lane) < B;
+    const int c4 = active ? blockIdx.y * 32 + lane : B / 4 - 1;
+    const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int r = warp; r < SCORE_ROWS; r += WARPS) {
+        const int row = blockIdx.x * SCORE_ROWS + r;
+        if (row >= n) break;                                 // warp-uniform
+        const float4 G = gather_row(col, val2, __ldg(rowptr + row), __ldg(rowptr + row + 1), xb, 4u * (uint32_t)B, lane);
+        const float4 xi = ldg4(x + (size_t)row * B + 4 * c4);
+        const float cp = __ldg(cprime + row);
+        acc[0] += (double)(xi.x * fmaf(0.5f, G.x, cp)); acc[1] += (double)(xi.y * fmaf(0.5f, G.y, cp));   // val2 = 2 Q_ij
+        acc[2] += (double)(xi.z * fmaf(0.5f, G.z, cp)); acc[3] += (double)(xi.w * fmaf(0.5f, G.w, cp));
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) red[warp][lane][q] = acc[q];
+    __syncthreads();
+    if (warp == 0 && active)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            double t = red[0][lane][q];
+            for (int w = 1; w < WARPS; ++w) t += red[w][lane][q];
+            partial[(size_t)blockIdx.x * B + 4 * c4 + q] = t;
+        }
+}
+
 template <int MODE, bool DUAL>
 gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
@@ -312,6 +345,14 @@ gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void
     else
         spmm_score<false><<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
     if (launches) ++*launches;
+    *n_part = (int32_t)grid.x;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status sparse_value_partials(gda_problem* p, int32_t B, const float* x, double* partial, int32_t* n_part, cudaStream_t s) {
+    const dim3 grid((unsigned)sparse_num_partials(p, B), (unsigned)((B / 4 + 31) / 32));
+    spmm_value<<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
     *n_part = (int32_t)grid.x;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;

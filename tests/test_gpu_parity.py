@@ -622,3 +622,45 @@ def test_mis_objective_cardinality_and_feasibility(api, oracle, n, d, B):
     assert_statistics_close(obj, ref["obj"])                                   # (d)
     assert (inside == 0).mean() >= 0.75 and -obj.min() > 0.3 * n / (1 + np.log(d))   # independent sets of sensible size
     P.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# gda_lagrangian and the dual certificate; beta = 0 keeps the multipliers fixed
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("w", [SMALL[1], SMALL[2], SMALL[3], SMALL[4]], ids=lambda w: w.name)
+def test_lagrangian_value_matches_oracle(api, oracle, w):
+    OP = oracle_problem(w.problem)
+    P = api.create_from_workload(w.problem)
+    n, B, h = w.problem.n, w.B, w.hyper
+    rng = np.random.default_rng(12)
+    X = rng.random((n, B), dtype=np.float32)
+    X[:, 0] = X[:, 0] > 0.5                                     # a binary column: L = F there
+    Y = rng.normal(size=(n, B)).astype(np.float32)
+    for lam, lam_ref in ((dev(Y), Y.astype(np.float64)), (1.5, 1.5)):
+        got = P.lagrangian(dev(X), lam, gfun=h.gfun, log_eps=h.log_eps).cpu().numpy()
+        ref = oracle.lagrangian(OP, X.astype(np.float64), lam_ref, h.gfun)
+        scale = np.abs(oracle.f_ext(OP, X.astype(np.float64))) + np.abs(ref) + n        # fp32 products, fp64 sums
+        assert (np.abs(got - ref) <= 1e-5 * scale).all()
+    assert abs(P.lagrangian(dev(X), dev(Y), gfun=h.gfun, log_eps=h.log_eps)[0].item()
+               - oracle.F_binary(OP, X[:, :1].astype(np.uint8))[0]) <= 1e-5 * n
+    P.destroy()
+
+
+def test_maxcut_dual_certificate(api, oracle):
+    w = wl.config(2, B=8, n_scale=0.25)                          # n = 200 Max-Cut, unit weights
+    Pw, n = w.problem, w.problem.n
+    P = api.create_from_workload(Pw)
+    Wm = np.zeros((n, n))
+    Wm[Pw.edges[:, 0], Pw.edges[:, 1]] = Wm[Pw.edges[:, 1], Pw.edges[:, 0]] = 1.0
+    ybar = float(-np.linalg.eigvalsh(Wm)[0] + 0.25)              # f_y convex
+    m = Pw.edges.shape[0]
+    x0 = dev(wl.x0_uniform(n, 8, 3))
+    prm = api.make_params(alpha=0.5 / (np.abs(Wm).sum(axis=1).max() + ybar), beta=0.0, delta=0.0, iters=3000, eval_every=3000)
+    r = P.run(x0, ybar, prm, want_final=True)
+    assert torch.all(r["lam"] == np.float32(ybar))              # beta = 0: multipliers untouched
+    assert (r["x"] - 0.5).abs().max().item() < 1e-5              # the minimiser of the convex f_y
+    bound = P.lagrangian(r["x"], ybar).cpu().numpy()
+    assert np.allclose(bound, -m / 2 - np.float32(ybar) * n / 4, rtol=1e-5)         # closed form of min f_y
+    cut = -P.run(x0, 6.0, api.params_from_hyper(w.hyper, iters=1500))["obj"].cpu().numpy()
+    assert (cut <= -bound + 1e-6).all()                         # every cut found respects the certificate
+    P.destroy()

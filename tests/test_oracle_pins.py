@@ -437,3 +437,32 @@ def test_pdbo_s_multiplier_is_shared_and_non_increasing(oracle):
     # one call of 30 steps is the same trajectory
     full = oracle.run(OP, X0, 6.0, dual=oracle.DUAL_SCALAR, **dict(kw, iters=30, eval_every=10))
     assert np.array_equal(full["x"], X) and np.array_equal(full["y"], mu)
+
+
+# ---------------------------------------------------------------------------------------------
+# The Lagrangian value and the dual certificate
+# ---------------------------------------------------------------------------------------------
+def test_lagrangian_value_and_maxcut_dual_certificate(oracle):
+    w = wl.config(1)                                             # n = 20, 101 unit edges, optimum 67 by brute force
+    P, n = w.problem, w.problem.n
+    OP = oracle_problem(P)
+    rng = np.random.default_rng(5)
+    X, Y = rng.random((n, 3)), rng.normal(size=(n, 3))
+    for gfun in (0, 1):                                          # L = f + sum y g, f by Def. 2.2-pinned f_ext, g typed out
+        want = oracle.f_ext(OP, X) + (Y * _g_closed_form(gfun, X)).sum(axis=0)
+        assert np.allclose(oracle.lagrangian(OP, X, Y, gfun), want, rtol=1e-13, atol=1e-12)
+    # binary points: g = 0, so L = F whatever y is
+    Xb = (rng.random((n, 4)) < 0.5).astype(np.float64)
+    assert np.array_equal(oracle.lagrangian(OP, Xb, Y[:, :1].repeat(4, axis=1), 0), oracle.F_binary(OP, Xb.astype(np.uint8)))
+    # dual certificate: with y = ybar 1 and ybar > -lambda_min(W), f_y is strictly convex (Hessian 2(W + ybar I),
+    # PAPER.md:606), its minimiser is 1/2 1 and min f_y = -m/2 - ybar n/4 in closed form
+    W = np.zeros((n, n))
+    W[P.edges[:, 0], P.edges[:, 1]] = W[P.edges[:, 1], P.edges[:, 0]] = 1.0
+    ybar = float(-np.linalg.eigvalsh(W)[0] + 0.25)
+    m = P.edges.shape[0]
+    r = oracle.run(OP, rng.random((n, 2)), ybar, alpha=0.02, beta=0.0, delta=0.0, gfun=0, iters=4000, eval_every=4000)
+    assert np.all(r["y"] == ybar)                                # beta = 0: the multipliers do not move
+    assert np.abs(r["x"] - 0.5).max() < 1e-9                     # gradient descent on the convex f_y reaches 1/2 1
+    bound = oracle.lagrangian(OP, r["x"], ybar, 0)
+    assert np.allclose(bound, -m / 2 - ybar * n / 4, rtol=1e-12)
+    assert np.all(-bound >= 67) and np.all(bound <= oracle.F_binary(OP, all_bits(n)).min())   # a valid bound on the max cut
