@@ -23,6 +23,7 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 _BUILD = _HERE / "_build"
 _SRC = _HERE / "pdbo_oracle.c"
+_SRC_KCUT = _HERE / "kcut_oracle.c"
 
 KIND_QUBO_CSR, KIND_QUBO_DENSE, KIND_MAXSAT = 0, 1, 2
 G_QUADRATIC, G_ENTROPY = 0, 1
@@ -47,11 +48,11 @@ def build(force: bool = False) -> None:
     _BUILD.mkdir(exist_ok=True)
     for tag, real in (("f64", "double"), ("f32", "float")):
         out = _BUILD / f"liboracle_{tag}.so"
-        if out.exists() and not force and out.stat().st_mtime >= _SRC.stat().st_mtime:
+        if out.exists() and not force and out.stat().st_mtime >= max(_SRC.stat().st_mtime, _SRC_KCUT.stat().st_mtime):
             continue
         tmp = out.with_suffix(f".tmp{os.getpid()}.so")
         cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", f"-DREAL={real}",
-               "-o", str(tmp), str(_SRC), "-lm"]
+               "-o", str(tmp), str(_SRC), str(_SRC_KCUT), "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, out)
 
