@@ -75,6 +75,20 @@ gda_status gda_create_qubo_dense(int32_t n, const float* Q, const float* c, int3
 gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cptr, const int32_t* lit, const float* w,
                              gda_problem** out);
 
+/* Max-k-Cut (Appendix B): minimise Tr(X W X^T) over X in R^{k x n} with one-hot columns, i.e.
+ * maximise the weight of the edges between different parts, cut = (sum_ij W_ij - obj) / 2.  HOST CSR of the
+ * SYMMETRIC weight matrix W (both directions stored), 2 <= k <= 8.  The method runs on logits Z with
+ * X_{:,i} = SoftMax(Z_{:,i}) (readings K1-K5), so for such a problem gda_run takes
+ *   x0           DEVICE fp32 [k][n][B]: the initial logits Z^0
+ *   lambda0      DEVICE fp32 [n][B] or NULL (lambda0_scalar)
+ *   x_bin        DEVICE uint8 [n][B]: per restart the LABELS (argmax_j Z_ji, lowest j on ties) of the best evaluation
+ *   obj          DEVICE double [B]: Tr(Xh W Xh^T) of those labels (exact integers for integer weights)
+ *   extra->x_final [k][n][B] logits Z^T; params->delta is ignored (no perturbation is described for this variant);
+ *   params->dual must be GDA_DUAL_PER_VARIABLE.  gda_grad / gda_score / gda_lagrangian: UNSUPPORTED.
+ * INVALID_ARG: as gda_create_qubo_csr, plus a non-zero diagonal entry and k outside [2, 8]. */
+gda_status gda_create_maxkcut(int32_t n, int32_t k, const int32_t* rowptr, const int32_t* col, const float* val,
+                              gda_problem** out);
+
 void gda_destroy(gda_problem* p); /* NULL-safe; synchronises the device before freeing */
 
 /* ---- the run ----------------------------------------------------------------------------------------- */
@@ -153,7 +167,7 @@ gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, const float
 
 /* ---- queries ------------------------------------------------------------------------------------------ */
 typedef struct {
-    int32_t kind;        /* 0 sparse QUBO, 1 dense QUBO, 2 MaxSAT                                       */
+    int32_t kind;        /* 0 sparse QUBO, 1 dense QUBO, 2 MaxSAT, 3 Max-k-Cut                          */
     int32_t n;
     int64_t nnz;         /* off-diagonal non-zeros (sparse), n*n (dense), literals (MaxSAT)             */
     int32_t m;           /* clauses (MaxSAT), else 0                                                    */

@@ -44,7 +44,7 @@ class Info(C.Structure):
                 ("last_run_step_launches", C.c_int64)]
 
 
-EXPORTS = ["gda_create_qubo_csr", "gda_create_qubo_dense", "gda_create_maxsat", "gda_destroy", "gda_run",
+EXPORTS = ["gda_create_qubo_csr", "gda_create_qubo_dense", "gda_create_maxsat", "gda_create_maxkcut", "gda_destroy", "gda_run",
            "gda_run_host", "gda_grad", "gda_score", "gda_lagrangian", "gda_get_info", "gda_last_error", "gda_version"]
 
 
@@ -60,6 +60,7 @@ def lib():
         L.gda_create_qubo_csr.argtypes = [i32, vp, vp, vp, vp, C.POINTER(vp)]
         L.gda_create_qubo_dense.argtypes = [i32, vp, vp, i32, C.POINTER(vp)]
         L.gda_create_maxsat.argtypes = [i32, i32, vp, vp, vp, C.POINTER(vp)]
+        L.gda_create_maxkcut.argtypes = [i32, i32, vp, vp, vp, C.POINTER(vp)]
         L.gda_destroy.argtypes = [vp]
         L.gda_destroy.restype = None
         L.gda_run.argtypes = [vp, i32, vp, vp, f32, C.POINTER(Params), vp, vp, vp, C.POINTER(Extra), vp]
@@ -98,9 +99,10 @@ def make_params(alpha, beta, delta=1e-4, log_eps=1e-6, iters=0, eval_every=100, 
 class Problem:
     """Owns a gda_problem* handle."""
 
-    def __init__(self, handle: int, n: int):
+    def __init__(self, handle: int, n: int, k: int = 0):
         self._h = C.c_void_p(handle)
         self.n = n
+        self.k = k          # Max-k-Cut: number of parts (x0 / x are then [k][n][B] logits); 0 otherwise
 
     # ---- constructors (gda_create_*) ----------------------------------------------------------
     @staticmethod
@@ -124,6 +126,13 @@ class Problem:
         _check(lib().gda_create_maxsat(n, m, _hp(cptr), _hp(lit), _hp(w), C.byref(h)))
         return Problem(h.value, n)
 
+    @staticmethod
+    def create_maxkcut(n, k, rowptr, col, val) -> "Problem":
+        rowptr, col, val = _host(rowptr, np.int32), _host(col, np.int32), _host(val, np.float32)
+        h = C.c_void_p()
+        _check(lib().gda_create_maxkcut(n, k, _hp(rowptr), _hp(col), _hp(val), C.byref(h)))
+        return Problem(h.value, n, k)
+
     def destroy(self):
         if self._h:
             lib().gda_destroy(self._h)
@@ -141,14 +150,15 @@ class Problem:
         Returns dict of CUDA tensors: x_bin, obj, best_restart (+ x, lam, best_obj, ones, trace_best, trace_ns).
         Asynchronous on `stream` (default: torch's current stream)."""
         import torch
-        assert x0.is_cuda and x0.dtype == torch.float32 and x0.is_contiguous() and x0.shape[0] == self.n
-        n, B = x0.shape
+        assert x0.is_cuda and x0.dtype == torch.float32 and x0.is_contiguous()
+        assert tuple(x0.shape[:-1]) == ((self.k, self.n) if self.k else (self.n,))
+        n, B = self.n, x0.shape[-1]
         dev = x0.device
         self._last = (n, B, dev)
         l_ptr, l_scalar = None, 0.0
         if isinstance(lambda0, torch.Tensor):
             assert lambda0.is_cuda and lambda0.dtype == torch.float32 and lambda0.is_contiguous()
-            assert lambda0.shape == ((B,) if params.dual == DUAL_SCALAR else x0.shape)
+            assert lambda0.shape == ((B,) if params.dual == DUAL_SCALAR else (n, B))
             l_ptr = lambda0.data_ptr()
         else:
             l_scalar = float(lambda0)
@@ -157,8 +167,8 @@ class Problem:
                    best_restart=torch.empty(1, dtype=torch.int32, device=dev))
         ex = Extra()
         if want_final:
-            out["x"] = torch.empty_like(x0)
-            out["lam"] = torch.empty(B, dtype=torch.float32, device=dev) if params.dual == DUAL_SCALAR else torch.empty_like(x0)
+            out["x"] = torch.empty_like(x0)                      # Max-k-Cut: the logits [k][n][B]
+            out["lam"] = torch.empty((B,) if params.dual == DUAL_SCALAR else (n, B), dtype=torch.float32, device=dev)
             out["best_obj"] = torch.empty(1, dtype=torch.float64, device=dev)
             ex.x_final, ex.lambda_final, ex.best_obj = out["x"].data_ptr(), out["lam"].data_ptr(), out["best_obj"].data_ptr()
         if want_ones:
@@ -252,6 +262,8 @@ def create_from_workload(P) -> Problem:
         return Problem.create_qubo_dense(P.n, P.Q, P.c)
     if isinstance(P, wl.MaxSat):
         return Problem.create_maxsat(P.n, P.m, P.cptr, P.lit, P.w)
+    if isinstance(P, wl.MaxKCut):
+        return Problem.create_maxkcut(P.n, P.k, P.rowptr, P.col, P.val)
     raise TypeError(type(P))
 
 

@@ -172,6 +172,26 @@ extern "C" gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, cons
 }
 
 // ---------------------------------------------------------------------------------------------------
+// create: Max-k-Cut -- the same symmetric CSR (validated, sorted, doubled) as the sparse QUBO with c = 0
+// ---------------------------------------------------------------------------------------------------
+extern "C" gda_status gda_create_maxkcut(int32_t n, int32_t k, const int32_t* rowptr, const int32_t* col, const float* val,
+                                         gda_problem** out) {
+    if (out) *out = nullptr;
+    GDA_REQUIRE(out != nullptr, "gda_create_maxkcut: out is NULL");
+    GDA_REQUIRE(k >= 2 && k <= 8, "gda_create_maxkcut: k must be in [2, 8] (got %d)", k);
+    GDA_REQUIRE(n > 0 && rowptr != nullptr, "gda_create_maxkcut: n must be > 0 and rowptr non-NULL");
+    for (int i = 0; i < n; ++i)
+        for (int a = rowptr[i]; a < rowptr[i + 1]; ++a)
+            GDA_REQUIRE(col == nullptr || col[a] != i || val[a] == 0.0f, "gda_create_maxkcut: non-zero diagonal entry at node %d", i);
+    gda_problem* p = nullptr;
+    GDA_TRY(gda_create_qubo_csr(n, rowptr, col, val, nullptr, &p));
+    p->kind = GDA_KIND_KCUT;
+    p->kparts = k;
+    *out = p;
+    return GDA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // create: dense QUBO (the heavy lifting is in gda_dense.cu)
 // ---------------------------------------------------------------------------------------------------
 extern "C" gda_status gda_create_qubo_dense(int32_t n, const float* Q, const float* c, int32_t flags,
@@ -290,7 +310,7 @@ static void free_workspace(gda_problem* p) {
     cudaFree(ws.x[0]); cudaFree(ws.x[1]); cudaFree(ws.y); cudaFree(ws.x_bin); cudaFree(ws.best_obj);
     cudaFree(ws.obj_now); cudaFree(ws.improved); cudaFree(ws.partial); cudaFree(ws.state);
     cudaFree(ws.best_restart); cudaFree(ws.best_val); cudaFree(ws.trace_best); cudaFree(ws.trace_ns);
-    cudaFree(ws.zt[0]); cudaFree(ws.zt[1]); cudaFree(ws.gtmp);
+    cudaFree(ws.zt[0]); cudaFree(ws.zt[1]); cudaFree(ws.gtmp); cudaFree(ws.z); cudaFree(ws.lab);
     cudaFree(ws.mu[0]); cudaFree(ws.mu[1]); cudaFree(ws.gpart);
     if (ws.h_x0) cudaFreeHost(ws.h_x0);
     if (ws.h_l0) cudaFreeHost(ws.h_l0);
@@ -316,6 +336,7 @@ static int32_t num_partials(const gda_problem* p, int32_t B) {
     switch (p->kind) {
         case GDA_KIND_SPARSE: return sparse_num_partials(p, B);
         case GDA_KIND_MAXSAT: return maxsat_num_partials(p, B);
+        case GDA_KIND_KCUT: return kcut_num_partials(p, B);
         default: return dense_num_partials(p, B);
     }
 }
@@ -339,14 +360,19 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     GDA_CUDA_TRY(cudaDeviceSynchronize());
     free_workspace(p);
     const size_t elems = (size_t)p->n * B;
+    const size_t xelems = p->kind == GDA_KIND_KCUT ? elems * p->kparts : elems;   // Max-k-Cut: k planes
     gda_status st = GDA_OK;
     if (p->kind != GDA_KIND_DENSE) {
-        if (st == GDA_OK) st = dmalloc(&ws.x[1], elems);
+        if (st == GDA_OK) st = dmalloc(&ws.x[1], xelems);
     } else {
         if (st == GDA_OK) st = dmalloc(&ws.zt[0], elems);
         if (st == GDA_OK) st = dmalloc(&ws.zt[1], elems);
     }
-    if (st == GDA_OK) st = dmalloc(&ws.x[0], elems);
+    if (p->kind == GDA_KIND_KCUT) {
+        if (st == GDA_OK) st = dmalloc(&ws.z, xelems);
+        if (st == GDA_OK) st = dmalloc(&ws.lab, elems);
+    }
+    if (st == GDA_OK) st = dmalloc(&ws.x[0], xelems);
     if (st == GDA_OK) st = dmalloc(&ws.y, elems);
     if (st == GDA_OK) st = dmalloc(&ws.x_bin, elems);
     if (st == GDA_OK) st = dmalloc(&ws.best_obj, (size_t)B);
@@ -355,7 +381,7 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     ws.n_part = num_partials(p, B);
     // + room for the y g(x) partial rows of gda_lagrangian
     if (st == GDA_OK) st = dmalloc((double**)&ws.partial, ((size_t)ws.n_part + (size_t)(p->n + 63) / 64) * B);
-    if (p->kind != GDA_KIND_DENSE) {                          // PDBO-s state (a few rows of B floats)
+    if (p->kind == GDA_KIND_SPARSE || p->kind == GDA_KIND_MAXSAT) {   // PDBO-s state (a few rows of B floats)
         ws.n_gpart = p->kind == GDA_KIND_SPARSE ? sparse_num_gparts(p) : maxsat_num_gparts(p);
         if (st == GDA_OK) st = dmalloc(&ws.mu[0], (size_t)B);
         if (st == GDA_OK) st = dmalloc(&ws.mu[1], (size_t)B);
@@ -419,6 +445,8 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
             GDA_TRY(sparse_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         else if (p->kind == GDA_KIND_MAXSAT)
             GDA_TRY(maxsat_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
+        else if (p->kind == GDA_KIND_KCUT)
+            GDA_TRY(kcut_step(p, B, ws.x[cur], ws.z, ws.y, ws.x[cur ^ 1], up, s, launches));
         else
             GDA_TRY(dense_step(p, B, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, ws.state, (uint32_t)k, s, launches));
         if (scalar) GDA_TRY(gsum_reduce(B, ws.gpart, ws.n_gpart, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
@@ -429,10 +457,12 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     int32_t n_part = 0;
     if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
     else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
+    else if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_score_partials(p, B, ws.z, ws.lab, ws.partial, &n_part, s, launches));
     else { ws.score_scratch = cur ^ 1; GDA_TRY(dense_score_partials(p, B, xcur, ws.partial, &n_part, s, launches)); }
     GDA_TRY(eval_finalize(p, B, ws.partial, n_part, ws.obj_now, ws.best_obj, ws.improved, ws.state, ws.trace_best,
                           ws.trace_ns, ws.trace_cap, (uint32_t)len, s, launches));
-    GDA_TRY(eval_commit(p, B, xcur, ws.improved, ws.x_bin, s, launches));
+    if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_commit(p, B, ws.lab, ws.improved, ws.x_bin, s, launches));
+    else GDA_TRY(eval_commit(p, B, xcur, ws.improved, ws.x_bin, s, launches));
     return GDA_OK;
 }
 
@@ -503,6 +533,10 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
     GDA_REQUIRE(prm->dual == GDA_DUAL_PER_VARIABLE || prm->dual == GDA_DUAL_SCALAR, "gda_run: unknown dual mode %d", prm->dual);
     GDA_REQUIRE(prm->reserved == 0, "gda_run: params->reserved must be 0");
     GDA_REQUIRE(x0 != nullptr || p->ws.dual == prm->dual, "gda_run: a resumed run must keep the dual mode of the run it continues");
+    if (prm->dual == GDA_DUAL_SCALAR && p->kind == GDA_KIND_KCUT) {
+        gda_set_error("gda_run: Max-k-Cut problems need GDA_DUAL_PER_VARIABLE");
+        return GDA_ERR_UNSUPPORTED;
+    }
     if (prm->dual == GDA_DUAL_SCALAR && p->kind == GDA_KIND_DENSE) {
         gda_set_error("gda_run: GDA_DUAL_SCALAR (PDBO-s) is implemented for sparse QUBO and MaxSAT problems only");
         return GDA_ERR_UNSUPPORTED;
@@ -511,7 +545,7 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
         gda_set_error("gda_run: the dense path needs B to be a multiple of 128 (got %d)", B);
         return GDA_ERR_UNSUPPORTED;
     }
-    if ((int64_t)p->n * (int64_t)B >= ((int64_t)1 << 30)) {
+    if ((int64_t)p->n * (int64_t)B * (p->kind == GDA_KIND_KCUT ? p->kparts : 1) >= ((int64_t)1 << 30)) {
         gda_set_error("gda_run: n * B must be below 2^30 (got %lld): kernels use 32-bit byte offsets into X", (long long)p->n * B);
         return GDA_ERR_UNSUPPORTED;
     }
@@ -537,6 +571,8 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
         GDA_TRY(run_init(p, B, x0, lambda0, lambda0_scalar, (uint32_t)prm->t0, s, &p->last_launches));
         if (p->kind == GDA_KIND_DENSE)
             GDA_TRY(dense_make_operand(p, B, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
+        if (p->kind == GDA_KIND_KCUT)                       // run_init put the logits in z; x[0] = SoftMax(z)
+            GDA_TRY(kcut_softmax(p, B, ws.z, ws.x[0], s, &p->last_launches));
     } else {
         parity = ws.parity;      // resume: iterates, duals, best-so-far and the iteration counter stay as they are
     }
@@ -556,7 +592,9 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
     GDA_CUDA_TRY(cudaMemcpyAsync(obj, ws.best_obj, (size_t)B * sizeof(double), cudaMemcpyDeviceToDevice, s));
     GDA_CUDA_TRY(cudaMemcpyAsync(best_restart, ws.best_restart, sizeof(int32_t), cudaMemcpyDeviceToDevice, s));
     if (extra) {
-        if (extra->x_final) GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, xfin, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        if (extra->x_final && p->kind == GDA_KIND_KCUT)      // the logits Z^T, [k][n][B]
+            GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, ws.z, elems * p->kparts * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        else if (extra->x_final) GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, xfin, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
         if (extra->lambda_final && prm->dual == GDA_DUAL_SCALAR)          // mu^T, [B]
             GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.mu[parity], (size_t)B * sizeof(float), cudaMemcpyDeviceToDevice, s));
         else if (extra->lambda_final)
@@ -587,7 +625,8 @@ extern "C" gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, c
     const size_t elems = (size_t)p->n * B;
     // device staging: x0 -> x[1] would be clobbered by the run, so stage in dedicated buffers
     float* d_x0 = nullptr; float* d_l0 = nullptr; uint8_t* d_xb = nullptr; double* d_obj = nullptr; int32_t* d_best = nullptr;
-    gda_status st = dmalloc(&d_x0, elems);
+    const size_t x0_elems = p->kind == GDA_KIND_KCUT ? elems * p->kparts : elems;
+    gda_status st = dmalloc(&d_x0, x0_elems);
     const size_t l0_elems = (prm && prm->dual == GDA_DUAL_SCALAR) ? (size_t)B : elems;
     if (st == GDA_OK && lambda0) st = dmalloc(&d_l0, l0_elems);
     if (st == GDA_OK) st = dmalloc(&d_xb, elems);
@@ -595,7 +634,7 @@ extern "C" gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, c
     if (st == GDA_OK) st = dmalloc(&d_best, 1);
     cudaError_t e = cudaSuccess;
     if (st == GDA_OK) {
-        e = cudaMemcpyAsync(d_x0, x0, elems * sizeof(float), cudaMemcpyHostToDevice, s);
+        e = cudaMemcpyAsync(d_x0, x0, x0_elems * sizeof(float), cudaMemcpyHostToDevice, s);
         if (e == cudaSuccess && lambda0) e = cudaMemcpyAsync(d_l0, lambda0, l0_elems * sizeof(float), cudaMemcpyHostToDevice, s);
         if (e == cudaSuccess) st = gda_run(p, B, d_x0, d_l0, lambda0_scalar, prm, d_xb, d_obj, d_best, nullptr, s);
         if (st == GDA_OK && e == cudaSuccess) e = cudaMemcpyAsync(x_bin, d_xb, elems, cudaMemcpyDeviceToHost, s);
@@ -616,6 +655,7 @@ extern "C" gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, c
 extern "C" gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float* G, void* stream) {
     GDA_REQUIRE(p != nullptr && x != nullptr && G != nullptr, "gda_grad: null argument");
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_grad: B must be a positive multiple of 4 (got %d)", B);
+    if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_grad: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
     if (p->kind == GDA_KIND_DENSE && B % 128 != 0) { gda_set_error("gda_grad: the dense path needs B %% 128 == 0"); return GDA_ERR_UNSUPPORTED; }
     GDA_CUDA_TRY(cudaSetDevice(p->device));
     cudaStream_t user, s;
@@ -630,6 +670,7 @@ extern "C" gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float*
 extern "C" gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, void* stream) {
     GDA_REQUIRE(p != nullptr && x != nullptr && obj != nullptr, "gda_score: null argument");
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_score: B must be a positive multiple of 4 (got %d)", B);
+    if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_score: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
     if (p->kind == GDA_KIND_DENSE && B % 128 != 0) { gda_set_error("gda_score: the dense path needs B %% 128 == 0"); return GDA_ERR_UNSUPPORTED; }
     GDA_CUDA_TRY(cudaSetDevice(p->device));
     GDA_TRY(ensure_workspace(p, B));
@@ -657,7 +698,7 @@ extern "C" gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, 
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_lagrangian: B must be a positive multiple of 4 (got %d)", B);
     GDA_REQUIRE(gfun == GDA_G_QUADRATIC || gfun == GDA_G_ENTROPY, "gda_lagrangian: unknown gfun %d", gfun);
     if (gfun == GDA_G_ENTROPY) GDA_REQUIRE(log_eps > 0.0f && log_eps < 0.5f, "gda_lagrangian: log_eps must be in (0, 1/2)");
-    if (p->kind == GDA_KIND_DENSE) { gda_set_error("gda_lagrangian: sparse QUBO and MaxSAT problems only"); return GDA_ERR_UNSUPPORTED; }
+    if (p->kind == GDA_KIND_DENSE || p->kind == GDA_KIND_KCUT) { gda_set_error("gda_lagrangian: sparse QUBO and MaxSAT problems only"); return GDA_ERR_UNSUPPORTED; }
     GDA_CUDA_TRY(cudaSetDevice(p->device));
     GDA_TRY(ensure_workspace(p, B));
     cudaStream_t user, s;

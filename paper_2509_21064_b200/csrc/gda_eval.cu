@@ -234,7 +234,10 @@ gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0,
                     uint32_t t0, cudaStream_t s, int64_t* launches) {
     Workspace& ws = p->ws;
     const size_t elems = (size_t)p->n * B;
-    GDA_CUDA_TRY(cudaMemcpyAsync(ws.x[0], x0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+    if (p->kind == GDA_KIND_KCUT)
+        GDA_CUDA_TRY(cudaMemcpyAsync(ws.z, x0, elems * p->kparts * sizeof(float), cudaMemcpyDeviceToDevice, s));
+    else
+        GDA_CUDA_TRY(cudaMemcpyAsync(ws.x[0], x0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
     if (ws.dual == GDA_DUAL_SCALAR) {
         GDA_TRY(mu_init(B, l0, l0_scalar, ws.mu[0], s, launches));
     } else if (l0) {

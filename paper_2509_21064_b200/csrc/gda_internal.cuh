@@ -28,7 +28,7 @@ void gda_set_error(const char* fmt, ...);
         if (s__ != GDA_OK) return s__;       \
     } while (0)
 
-enum { GDA_KIND_SPARSE = 0, GDA_KIND_DENSE = 1, GDA_KIND_MAXSAT = 2 };
+enum { GDA_KIND_SPARSE = 0, GDA_KIND_DENSE = 1, GDA_KIND_MAXSAT = 2, GDA_KIND_KCUT = 3 };
 
 // ---------------------------------------------------------------------------------------------------
 // update parameters handed to the kernels by value
@@ -62,6 +62,8 @@ struct Workspace {
     bool has_state = false;             // a previous gda_run left (x, y, best-so-far) here: x0 == NULL may resume
     float* x[2] = {nullptr, nullptr};   // [n][B] double buffer (Jacobi: every row reads all of x^t)
     float* y = nullptr;                 // [n][B], updated in place
+    float* z = nullptr;                 // Max-k-Cut: logits [k][n][B], updated in place (x[] then holds SoftMax(z), [k][n][B])
+    uint8_t* lab = nullptr;             // Max-k-Cut: labels of the current iterate at an evaluation, [n][B]
     float* mu[2] = {nullptr, nullptr};  // PDBO-s: [B] multipliers, double-buffered with the parity of x
     float* gpart = nullptr;             // PDBO-s: [n_gpart][B] per-block sums of g
     int32_t n_gpart = 0;
@@ -103,6 +105,7 @@ struct gda_problem {
     int32_t n = 0;
     int64_t nnz = 0;
     int32_t m = 0;
+    int32_t kparts = 0;                  // Max-k-Cut: number of parts k (0 otherwise)
     int32_t integral = 0;
     int device = 0;
     int num_sms = 148;
@@ -150,6 +153,16 @@ gda_status maxsat_score_partials(gda_problem* p, int32_t B, const float* x, void
                                  cudaStream_t s, int64_t* launches);
 int32_t maxsat_num_partials(const gda_problem* p, int32_t B);
 gda_status maxsat_value_partials(gda_problem* p, int32_t B, const float* x, double* partial, int32_t* n_part, cudaStream_t s);
+
+// Max-k-Cut (gda_kcut.cu): x = SoftMax(z) planes [k][n][B]
+gda_status kcut_step(gda_problem* p, int32_t B, const float* x, float* z, float* y, float* xn, const UpdParams& up,
+                     cudaStream_t s, int64_t* launches);
+gda_status kcut_softmax(gda_problem* p, int32_t B, const float* z, float* x, cudaStream_t s, int64_t* launches);
+gda_status kcut_score_partials(gda_problem* p, int32_t B, const float* z, uint8_t* lab, void* partial, int32_t* n_part,
+                               cudaStream_t s, int64_t* launches);
+gda_status kcut_commit(gda_problem* p, int32_t B, const uint8_t* lab, const int32_t* improved, uint8_t* x_bin,
+                       cudaStream_t s, int64_t* launches);
+int32_t kcut_num_partials(const gda_problem* p, int32_t B);
 
 // dense QUBO (gda_dense.cu)
 gda_status dense_prepare(gda_problem* p, const float* Q_host, const float* c_host);   // at create

@@ -55,6 +55,18 @@ class MaxSat:
 
 
 @dataclass
+class MaxKCut:
+    """Max-k-Cut: symmetric weight matrix W as CSR (both directions), k parts."""
+    n: int
+    k: int
+    rowptr: np.ndarray
+    col: np.ndarray
+    val: np.ndarray
+    edges: np.ndarray = None
+    edge_w: np.ndarray = None
+
+
+@dataclass
 class Hyper:
     """(y-bar, alpha, beta, delta, g) and run lengths for one config (Table 6; R7)."""
     lambda0: float
@@ -280,6 +292,23 @@ def config(idx: int, B: Optional[int] = None, n_scale: float = 1.0) -> Workload:
                         Hyper(2.0, 0.01, 0.005, 1e-4, 1, 1e-6, 5000, 100, 105), 1105,
                         "weighted Max-3-SAT ratio 4.26, w in 1..10, entropy g")
     raise ValueError("config index must be 1..5")
+
+
+def maxkcut(n: int, m: int, k: int = 3, B: int = 128, seed: int = 107, weights: str = "unit", iters: int = 5000) -> Workload:
+    """Max-k-Cut on G(n, m).  Table 6: B = 100, ybar = 6, alpha = beta = 0.01; the initial logits are
+    Z^0 ~ U[0,1)^(k x n x B) (reading K2; `z0_uniform`)."""
+    e = edges_gnm(n, m, seed)
+    w = edge_weights(m, seed, weights)
+    q = maxcut_as_qubo(n, e, w)                          # same symmetric CSR of W
+    P = MaxKCut(n=n, k=k, rowptr=q.rowptr, col=q.col, val=q.val, edges=e, edge_w=w)
+    return Workload(f"max{k}cut_n{n}", "maxkcut", P, B, Hyper(6.0, 0.01, 0.01, 0.0, 0, 1e-6, iters, 100, seed), 1000 + seed,
+                    f"Max-{k}-Cut G({n},{m}), {weights} weights")
+
+
+def z0_uniform(k: int, n: int, B: int, seed: int) -> np.ndarray:
+    """Initial logits Z^0 ~ U[0,1)^(k x n x B), float32, layout [k][n][B] (reading K2)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    return rng.random((k, n, B), dtype=np.float32)
 
 
 def pdbo_s_variant(w: Workload) -> Workload:
