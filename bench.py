@@ -57,6 +57,9 @@ def algorithmic_work(w: wl.Workload):
     if w.kind == "qubo_csr":
         nnz = int(P.rowptr[-1])
         return dict(bound="hbm", bytes=state + 8 * nnz + 4 * (n + 1) + 4 * n, flops=2 * nnz * B)
+    if w.kind == "maxkcut":                  # read X, Z (k planes each) and y; write the same
+        nnz = int(P.rowptr[-1])
+        return dict(bound="hbm", bytes=(4 * P.k + 2) * 4 * n * B + 8 * nnz + 4 * (n + 1), flops=2 * nnz * B * P.k)
     if w.kind == "maxsat":
         L = int(P.lit.shape[0])
         k = L // P.m
@@ -115,11 +118,37 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 def oracle_problem(P):
     from oracle import pdbo
+    if isinstance(P, wl.MaxKCut):
+        from oracle import kcut
+        return kcut.Problem(P.n, P.k, P.rowptr, P.col, P.val.astype(np.float64))
     if isinstance(P, wl.QuboCSR):
         return pdbo.Problem.qubo_csr(P.n, P.rowptr, P.col, P.val, P.c)
     if isinstance(P, wl.QuboDense):
         return pdbo.Problem.qubo_dense(P.n, P.Q, P.c)
     return pdbo.Problem.maxsat(P.n, P.m, P.cptr, P.lit, P.w)
+
+
+def start_point(w: wl.Workload, seed: int) -> np.ndarray:
+    """x0 ~ U[0,1) [n][B], or the logits Z0 [k][n][B] of a Max-k-Cut workload."""
+    if w.kind == "maxkcut":
+        return wl.z0_uniform(w.problem.k, w.problem.n, w.B, seed)
+    return wl.x0_uniform(w.problem.n, w.B, seed)
+
+
+def oracle_run(w: wl.Workload, OP, X, Y, iters, eval_every, nthreads, t0=0):
+    """One oracle call on the columns X[..., :]; returns (x, y) of the last iterate."""
+    h = w.hyper
+    f = lambda v: float(np.float32(v))
+    if w.kind == "maxkcut":
+        from oracle import kcut
+        r = kcut.run(OP, X, Y, alpha=f(h.alpha), beta=f(h.beta), gfun=h.gfun, log_eps=f(h.log_eps), iters=iters,
+                     eval_every=eval_every, nthreads=nthreads)
+        return r["z"], r["y"]
+    from oracle import pdbo
+    kw = oracle_kwargs(h, iters)
+    kw["eval_every"] = eval_every
+    r = pdbo.run(OP, X, Y, nthreads=nthreads, t0=t0, **kw)
+    return r["x"], r["y"]
 
 
 def oracle_kwargs(h, iters):
@@ -140,20 +169,23 @@ def time_oracle(w: wl.Workload, budget_s: float):
     cores = max(1, min(pdbo.max_threads(), os.cpu_count() or 1))
     OP = oracle_problem(w.problem)
     Bo = oracle_sample_columns(w, cores)
-    X0 = wl.x0_uniform(w.problem.n, w.B, w.x0_seed)[:, :Bo].copy()
+    X0 = start_point(w, w.x0_seed)[..., :Bo].copy()
     h = w.hyper
+    lam = float(np.float32(h.lambda0)) if not getattr(h, "dual", 0) else np.full(Bo, np.float32(h.lambda0), dtype=np.float64)
     it = 2 if w.kind == "qubo_dense" else 10
-    pdbo.run(OP, X0, float(np.float32(h.lambda0)), nthreads=cores, **oracle_kwargs(h, it))     # thread-pool warm-up
+    oracle_run(w, OP, X0, lam, it, h.eval_every, cores)                                       # thread-pool warm-up
     t0 = time.perf_counter()
-    pdbo.run(OP, X0, float(np.float32(h.lambda0)), nthreads=cores, **oracle_kwargs(h, it))
+    oracle_run(w, OP, X0, lam, it, h.eval_every, cores)
     per_iter = (time.perf_counter() - t0) / it
     iters = int(max(it, min(h.iters, budget_s / max(per_iter, 1e-9))))
     mult = int(min(w.B // Bo, max(1.0, budget_s / max(iters * per_iter, 1e-9))))   # more columns if the budget allows
     if mult > 1:
         Bo *= mult
-        X0 = wl.x0_uniform(w.problem.n, w.B, w.x0_seed)[:, :Bo].copy()
+        X0 = start_point(w, w.x0_seed)[..., :Bo].copy()
+        if getattr(h, "dual", 0):
+            lam = np.full(Bo, np.float32(h.lambda0), dtype=np.float64)
     t0 = time.perf_counter()
-    pdbo.run(OP, X0, float(np.float32(h.lambda0)), nthreads=cores, **oracle_kwargs(h, iters))
+    oracle_run(w, OP, X0, lam, iters, h.eval_every, cores)
     dt = time.perf_counter() - t0
     return dict(value=Bo * iters / dt, unit="restart-iters/s", cores=cores, kind="oracle",
                 sample=f"{Bo} of {w.B} restarts x {iters} GDA iterations of {w.name}, fp64, gcc -O2 -fopenmp, {dt:.1f} s")
@@ -171,20 +203,18 @@ def run_reference(args, w: wl.Workload):
     Bo = oracle_sample_columns(w, cores)
     h = w.hyper
     per_step = h.eval_every if w.kind != "qubo_dense" else max(1, h.eval_every // 50)
-    X = wl.x0_uniform(w.problem.n, w.B, w.x0_seed)[:, :Bo].copy().astype(np.float64)
-    Y = np.full_like(X, float(np.float32(h.lambda0)))
+    X = start_point(w, w.x0_seed)[..., :Bo].copy().astype(np.float64)
+    Y = np.full((w.problem.n, Bo), float(np.float32(h.lambda0)))
     if getattr(h, "dual", 0):
         Y = Y[0].copy()                      # PDBO-s: one multiplier per restart
-    kw = oracle_kwargs(h, per_step)
-    kw["eval_every"] = per_step
     t = 0
     for _ in range(args.warmup):
-        r = pdbo.run(OP, X, Y, nthreads=cores, t0=t, **kw)
-        X, Y, t = r["x"], r["y"], t + per_step
+        X, Y = oracle_run(w, OP, X, Y, per_step, per_step, cores, t0=t)
+        t += per_step
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        r = pdbo.run(OP, X, Y, nthreads=cores, t0=t, **kw)
-        X, Y, t = r["x"], r["y"], t + per_step
+        X, Y = oracle_run(w, OP, X, Y, per_step, per_step, cores, t0=t)
+        t += per_step
     dt = time.perf_counter() - t0
     value = Bo * per_step * args.steps / dt
     sample = f"{Bo} of {w.B} restarts, {per_step} GDA iterations + 1 evaluation per step, fp64 oracle"
@@ -225,7 +255,7 @@ def run_ours(args, w: wl.Workload):
     h, B, n = w.hyper, w.B, w.problem.n
     K, W = args.steps, max(args.warmup, 3)
     P = api.create_from_workload(w.problem)
-    x0_host = torch.from_numpy(wl.x0_uniform(n, B, multirank.rank_x0_seed(w.x0_seed, rank))).pin_memory()   # each rank: its own restarts
+    x0_host = torch.from_numpy(start_point(w, multirank.rank_x0_seed(w.x0_seed, rank))).pin_memory()   # each rank: its own restarts
     x0 = x0_host.to(dev, non_blocking=True)
     stream = torch.cuda.Stream(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -341,7 +371,7 @@ def run_ours(args, w: wl.Workload):
             "whole_run": {"value": units / t_whole, "unit": "restart-iters/s", "ms_total": 1e3 * t_whole,
                           "iters": iters_per_step * K, "l2": "not flushed (one gda_run call)", "best_objective": best,
                           "best_vs_time": trace},
-            "e2e": {"value": units / t_e2e, "unit": "restart-iters/s", "h2d_bytes_per_step": 4 * n * B / K,
+            "e2e": {"value": units / t_e2e, "unit": "restart-iters/s", "h2d_bytes_per_step": x0_host.numel() * 4 / K,
                     "d2h_bytes_per_step": (n * B + 8 * B + 4) / K, "ms_total": 1e3 * t_e2e,
                     "note": "gda_run_host: one call of K steps; x0 H2D and x_bin/obj/best D2H once per call, amortised per step"},
             "gpu_launches": int(launches),
@@ -372,11 +402,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--B", type=int, default=None)
     ap.add_argument("--pdbo-s", action="store_true", help="run the PDBO-s ablation (one multiplier per restart, PAPER.md:630-648)")
+    ap.add_argument("--maxkcut", default=None, metavar="N,M,K", help="instead of --config: Max-K-Cut on G(N, M) (PAPER.md:784-828)")
     ap.add_argument("--mis", default=None, metavar="N,D", help="instead of --config: MIS as a QUBO on a D-regular graph with N vertices (PAPER.md:1030-1036)")
     args = ap.parse_args()
     if args.mis:
         n_mis, d_mis = (int(v) for v in args.mis.split(","))
         w = wl.mis(n_mis, d_mis, B=args.B or 12)
+    elif args.maxkcut:
+        n_k, m_k, k_k = (int(v) for v in args.maxkcut.split(","))
+        w = wl.maxkcut(n_k, m_k, k_k, B=args.B or 128)
     else:
         w = wl.config(args.config, B=args.B)
     if args.pdbo_s:
