@@ -1,0 +1,78 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (one gda_run of `eval_every` steps
+= one CUDA-graph launch), on sampled restart columns the oracle can compute one by one, plus properties that hold at
+any size."""
+import numpy as np
+import pytest
+
+from paper_2509_21064_b200 import workloads as wl
+from tests.helpers import oracle_problem, hyper_kwargs
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def api():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2509_21064_b200 import api as _api
+    _api.lib()
+    return _api
+
+
+def f32(v):
+    return float(np.float32(v))
+
+
+def okw(h, **over):
+    d = hyper_kwargs(h, **over)
+    for k in ("alpha", "beta", "delta", "log_eps"):
+        d[k] = f32(d[k])
+    return d
+
+
+@pytest.mark.parametrize("idx", [2, 3, 5, 4])
+def test_full_size_config_on_sampled_restarts(api, oracle, idx):
+    w = wl.config(idx)
+    Pw, h, B = w.problem, w.hyper, w.B
+    n = Pw.n
+    dense = idx == 4
+    OP = oracle_problem(Pw)
+    P = api.create_from_workload(Pw)
+    X0 = wl.x0_uniform(n, B, w.x0_seed)
+    x0 = torch.from_numpy(X0).cuda()
+    cols = np.array([0, 1, B // 3, B // 2 + 1, B - 2, B - 1] if not dense else [0, B // 2 + 1, B - 1], dtype=np.int32)
+    # (b) one step from x0: sampled columns against the oracle (the hash sees the true column ids)
+    r1 = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+    ref = oracle.run(OP, X0[:, cols], f32(h.lambda0), col_ids=cols, nthreads=4, **okw(h, iters=1, eval_every=1))
+    xg = r1["x"][:, torch.from_numpy(cols).long().cuda()].cpu().numpy()
+    yg = r1["lam"][:, torch.from_numpy(cols).long().cuda()].cpu().numpy()
+    if dense:
+        Gref = oracle.grad(OP, X0[:, cols].astype(np.float64))
+        tol = f32(h.alpha) * 1e-2 * np.abs(Gref).max(axis=0, keepdims=True) + 1e-5        # bf16 operand: gradient 1e-2 (north star)
+        assert (np.abs(xg - ref["x"]) <= tol).all()
+    else:
+        assert np.abs(xg - ref["x"]).max() <= 1e-5
+    assert (np.abs(yg - ref["y"]) <= 1e-5 * np.maximum(1.0, np.abs(ref["y"]))).all()
+    # the timed launch configuration: eval_every steps + one evaluation in one graph launch, then a resumed one
+    steps = h.eval_every
+    r = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=steps), want_final=True)
+    P.resume(api.params_from_hyper(h, iters=steps), r)
+    torch.cuda.synchronize()
+    x, lam = r["x"], r["lam"]                                    # iterates after the FIRST call (resume leaves them)
+    assert bool(((x >= 0) & (x <= 1)).all())                     # projection (Eq. 6)
+    gmin = 0.25 if h.gfun == 0 else float(np.log(2.0))
+    dec = h.lambda0 - lam
+    assert bool((dec >= -1e-6).all()) and bool((dec <= steps * f32(h.beta) * gmin * (1 + 1e-5) + 1e-6).all())
+    obj = r["obj"].cpu().numpy()
+    xb = r["x_bin"][:, torch.from_numpy(cols).long().cuda()].cpu().numpy()
+    Fref = oracle.F_binary(OP, xb)                               # (a) objective of the returned points, sampled columns
+    if dense:
+        tolF = 1e-5 * (xb.astype(np.float64).T @ np.abs(Pw.Q.astype(np.float64)) @ xb.astype(np.float64)).diagonal() + 1e-3
+        assert (np.abs(obj[cols] - Fref) <= tolF).all()
+    else:
+        assert np.array_equal(obj[cols], Fref)
+    assert int(r["best_restart"].item()) == int(np.argmin(obj))  # S6, ties -> lowest index
+    if idx in (2, 3):                                            # far better than a random cut already (m/2 in expectation)
+        assert -obj.max() > 0.55 * np.abs(Pw.edge_w).sum() if idx == 2 else -obj.max() > 0
+    P.destroy()
