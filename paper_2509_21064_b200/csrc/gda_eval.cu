@@ -8,7 +8,7 @@
 
 namespace {
 
-constexpr int FIN_THREADS = 256;
+constexpr int FIN_COLS = 256, FIN_SLICES = 4, FIN_THREADS = FIN_COLS * FIN_SLICES;
 
 __device__ __forceinline__ uint64_t globaltimer_ns() {
     uint64_t t;
@@ -16,8 +16,10 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
     return t;
 }
 
-// obj_now[b] = sum_p partial[p][b] in the fixed order p = 0..n_part-1 (deterministic); best-so-far update.
-// One block; thread 0 afterwards records the trace entry and advances the run state.
+// obj_now[b] = sum_p partial[p][b]; best-so-far update.  One block of 256 columns x 4 row slices: slice s adds the rows
+// p = s, s + 4, ... (8 independent loads in flight), the four slice sums are added in slice order -- a fixed order, so
+// the result is deterministic (and exact for integral instances).  Thread 0 afterwards records the trace entry and
+// advances the run state.
 template <bool INTEGRAL>
 __global__ void __launch_bounds__(FIN_THREADS)
 finalize_kernel(int B, const void* __restrict__ partial, int n_part, double* __restrict__ obj_now,
@@ -25,20 +27,41 @@ finalize_kernel(int B, const void* __restrict__ partial, int n_part, double* __r
                 double* __restrict__ trace_best, uint64_t* __restrict__ trace_ns, int trace_cap,
                 uint32_t advance_t) {
     using acc_t = typename std::conditional<INTEGRAL, long long, double>::type;
+    __shared__ acc_t red[FIN_SLICES][FIN_COLS];
     __shared__ double smin[FIN_THREADS / 32];
     const acc_t* part = reinterpret_cast<const acc_t*>(partial);
+    const int col = threadIdx.x % FIN_COLS, slice = threadIdx.x / FIN_COLS;
     double local_min = CUDART_INF;
-    for (int b = threadIdx.x; b < B; b += FIN_THREADS) {
+    for (int b0 = 0; b0 < B; b0 += FIN_COLS) {
+        const int b = b0 + col;
         acc_t s = 0;
-        for (int q = 0; q < n_part; ++q) s += part[(size_t)q * B + b];
-        const double v = (double)s;
-        if (obj_now) obj_now[b] = v;
-        if (best_obj) {
-            double best = best_obj[b];
-            const int imp = v < best;
-            if (imp) { best = v; best_obj[b] = v; }
-            improved[b] = imp;
-            local_min = fmin(local_min, best);
+        if (b < B) {
+            int q = slice;
+            for (; q + 7 * FIN_SLICES < n_part; q += 8 * FIN_SLICES) {
+                acc_t v[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) v[u] = part[(size_t)(q + u * FIN_SLICES) * B + b];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) s += v[u];
+            }
+            for (; q < n_part; q += FIN_SLICES) s += part[(size_t)q * B + b];
+        }
+        __syncthreads();                                     // red[] of the previous pass has been consumed
+        red[slice][col] = s;
+        __syncthreads();
+        if (slice == 0 && b < B) {
+            acc_t t = red[0][col];
+#pragma unroll
+            for (int k = 1; k < FIN_SLICES; ++k) t += red[k][col];
+            const double v = (double)t;
+            if (obj_now) obj_now[b] = v;
+            if (best_obj) {
+                double best = best_obj[b];
+                const int imp = v < best;
+                if (imp) { best = v; best_obj[b] = v; }
+                improved[b] = imp;
+                local_min = fmin(local_min, best);
+            }
         }
     }
     if (!st) return;
