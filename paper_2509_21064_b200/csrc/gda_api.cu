@@ -310,10 +310,8 @@ static void free_workspace(gda_problem* p) {
     cudaFree(ws.x[0]); cudaFree(ws.x[1]); cudaFree(ws.y); cudaFree(ws.x_bin); cudaFree(ws.best_obj);
     cudaFree(ws.obj_now); cudaFree(ws.improved); cudaFree(ws.partial); cudaFree(ws.state);
     cudaFree(ws.best_restart); cudaFree(ws.best_val); cudaFree(ws.trace_best); cudaFree(ws.trace_ns);
-    cudaFree(ws.zt[0]); cudaFree(ws.zt[1]); cudaFree(ws.gtmp); cudaFree(ws.z); cudaFree(ws.lab);
+    cudaFree(ws.zt[0]); cudaFree(ws.zt[1]); cudaFree(ws.z); cudaFree(ws.lab);
     cudaFree(ws.mu[0]); cudaFree(ws.mu[1]); cudaFree(ws.gpart);
-    if (ws.h_x0) cudaFreeHost(ws.h_x0);
-    if (ws.h_l0) cudaFreeHost(ws.h_l0);
     ws = Workspace();
 }
 

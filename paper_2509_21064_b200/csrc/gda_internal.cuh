@@ -83,9 +83,6 @@ struct Workspace {
     // dense path
     __nv_bfloat16* zt[2] = {nullptr, nullptr};  // [B][n] bf16 GEMM operand (centred x - 1/2, or x_hat)
     int32_t score_scratch = 1;                  // which zt buffer dense scoring may clobber (the one not holding z^t)
-    float* gtmp = nullptr;                      // [n][B] gradient scratch for gda_grad on the dense path
-    // host staging for gda_run_host
-    float* h_x0 = nullptr; float* h_l0 = nullptr;
 };
 
 struct GraphKey {
@@ -316,20 +313,4 @@ __device__ __forceinline__ void scalar_dual_block_sum(float4 gs, float4 (*red)[3
     *reinterpret_cast<float4*>(gpart_row_c4) = t;
 }
 
-// Programmatic dependent launch (PDL): a step kernel lets its successor start launching right away and the successor
-// blocks at pdl_wait() -- placed after its index loads, before its first access to X / Y -- until this grid has
-// completed and its writes are visible.  Hides the ~2.5 us kernel-to-kernel latency inside a captured chunk.
-__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-
-template <typename... KArgs, typename... Args>
-inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args... args) {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
-}
 #endif
