@@ -206,20 +206,28 @@ spmm_score(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __re
         for (int base = start; base < end; base += 32) {
             const int k = base + lane;
             const int my_c = (k < end) ? __ldg(col + k) : 0;
-            const float my_v = (k < end) ? __ldg(val2 + k) : 0.0f;
+            const float my_v = (k < end) ? __ldg(val2 + k) : 0.0f;          // lanes past the end: (row 0, value 0)
             const int cnt = min(32, end - base);
-            for (int u = 0; u < cnt; ++u) {
-                const int c = __shfl_sync(0xffffffffu, my_c, u);
-                const float v = __shfl_sync(0xffffffffu, my_v, u);
+            for (int u = 0; u < cnt; u += 4) {                               // 4 independent gathers in flight
+                int c[4]; float v[4]; float4 g[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {                                // u + q <= 31
+                    c[q] = __shfl_sync(0xffffffffu, my_c, u + q);
+                    v[q] = __shfl_sync(0xffffffffu, my_v, u + q);
+                }
                 if (!active) continue;
-                const float4 g = ldg4(x + (size_t)c * B + 4 * c4);
-                if (INTEGRAL) {
-                    const int vi = __float2int_rn(v);
-                    si[0] += g.x > 0.5f ? vi : 0; si[1] += g.y > 0.5f ? vi : 0;
-                    si[2] += g.z > 0.5f ? vi : 0; si[3] += g.w > 0.5f ? vi : 0;
-                } else {
-                    s[0] += g.x > 0.5f ? v : 0.f; s[1] += g.y > 0.5f ? v : 0.f;
-                    s[2] += g.z > 0.5f ? v : 0.f; s[3] += g.w > 0.5f ? v : 0.f;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) g[q] = ldg4(x + (size_t)c[q] * B + 4 * c4);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if (INTEGRAL) {
+                        const int vi = __float2int_rn(v[q]);
+                        si[0] += g[q].x > 0.5f ? vi : 0; si[1] += g[q].y > 0.5f ? vi : 0;
+                        si[2] += g[q].z > 0.5f ? vi : 0; si[3] += g[q].w > 0.5f ? vi : 0;
+                    } else {
+                        s[0] += g[q].x > 0.5f ? v[q] : 0.f; s[1] += g[q].y > 0.5f ? v[q] : 0.f;
+                        s[2] += g[q].z > 0.5f ? v[q] : 0.f; s[3] += g[q].w > 0.5f ? v[q] : 0.f;
+                    }
                 }
             }
         }
