@@ -15,7 +15,7 @@ namespace {
 constexpr int WARPS = 8;
 constexpr int THREADS = WARPS * 32;
 constexpr int HEAVY_DEG = 256;     // rows above this use the row-split kernel
-constexpr int SCORE_ROWS = 64;     // rows per block in the scoring kernel
+constexpr int SCORE_ROWS = 64;     // most rows per block in the scoring kernels (fewer when that leaves SMs idle)
 
 __device__ __forceinline__ void fma4(float4& a, float v, const float4& g) {
     a.x = fmaf(v, g.x, a.x); a.y = fmaf(v, g.y, a.y); a.z = fmaf(v, g.z, a.z); a.w = fmaf(v, g.w, a.w);
@@ -187,7 +187,7 @@ spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chu
 // S5 for sparse QUBO: partial[rb][b] = sum over the rows of block rb of x_hat_i ((Q_off x_hat)_i + c'_i)
 template <bool INTEGRAL>
 __global__ void __launch_bounds__(THREADS)
-spmm_score(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+spmm_score(int n, int B, int rows_per_block, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
            const float* __restrict__ val2, const float* __restrict__ cprime, const float* __restrict__ x,
            void* __restrict__ partial) {
     using acc_t = typename std::conditional<INTEGRAL, long long, double>::type;
@@ -195,9 +195,9 @@ spmm_score(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __re
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int c4 = blockIdx.y * 32 + lane;
     const bool active = 4 * c4 < B;
-    const int row0 = blockIdx.x * SCORE_ROWS;
+    const int row0 = blockIdx.x * rows_per_block;
     acc_t acc[4] = {0, 0, 0, 0};
-    for (int r = warp; r < SCORE_ROWS; r += WARPS) {
+    for (int r = warp; r < rows_per_block; r += WARPS) {
         const int row = row0 + r;
         if (row >= n) break;
         const int start = __ldg(rowptr + row), end = __ldg(rowptr + row + 1);
@@ -259,7 +259,7 @@ spmm_score(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __re
 // f(x) at a continuous point (multilinear extension of the QUBO, reading R1):
 // partial[rb][b] = sum over the rows of block rb of x_i ((Q_off x)_i + c'_i); products in fp32, sums in fp64
 __global__ void __launch_bounds__(THREADS)
-spmm_value(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+spmm_value(int n, int B, int rows_per_block, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
            const float* __restrict__ val2, const float* __restrict__ cprime, const float* __restrict__ x,
            double* __restrict__ partial) {
     __shared__ double red[WARPS][32][4];
@@ -268,8 +268,8 @@ spmm_value(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __re
     const int c4 = active ? blockIdx.y * 32 + lane : B / 4 - 1;
     const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
-    for (int r = warp; r < SCORE_ROWS; r += WARPS) {
-        const int row = blockIdx.x * SCORE_ROWS + r;
+    for (int r = warp; r < rows_per_block; r += WARPS) {
+        const int row = blockIdx.x * rows_per_block + r;
         if (row >= n) break;                                 // warp-uniform
         const float4 G = gather_row(col, val2, __ldg(rowptr + row), __ldg(rowptr + row + 1), xb, 4u * (uint32_t)B, lane);
         const float4 xi = ldg4(x + (size_t)row * B + 4 * c4);
@@ -342,16 +342,25 @@ gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cuda
     return launch_step<1, false>(p, B, x, nullptr, G, up, ScalarDual{}, nullptr, 0, s, nullptr);
 }
 
-int32_t sparse_num_partials(const gda_problem* p, int32_t) { return (p->n + SCORE_ROWS - 1) / SCORE_ROWS; }
+// rows per block of the scoring kernels: 64, halved down to 8 (one per warp) while the grid would leave SMs without
+// two blocks (config 2: n = 800, 8 chunks -> 16 rows per block, 400 blocks)
+static int score_rows(const gda_problem* p, int32_t B) {
+    const long long chunks = (B / 4 + 31) / 32;
+    int rows = SCORE_ROWS;
+    while (rows > WARPS && ((p->n + rows - 1) / rows) * chunks < 2LL * p->num_sms) rows >>= 1;
+    return rows;
+}
+
+int32_t sparse_num_partials(const gda_problem* p, int32_t B) { const int r = score_rows(p, B); return (p->n + r - 1) / r; }
 
 gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
                                  cudaStream_t s, int64_t* launches) {
     const int chunks = (B / 4 + 31) / 32;
     dim3 grid((unsigned)sparse_num_partials(p, B), (unsigned)chunks);
     if (p->integral)
-        spmm_score<true><<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
+        spmm_score<true><<<grid, THREADS, 0, s>>>(p->n, B, score_rows(p, B), p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
     else
-        spmm_score<false><<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
+        spmm_score<false><<<grid, THREADS, 0, s>>>(p->n, B, score_rows(p, B), p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
     if (launches) ++*launches;
     *n_part = (int32_t)grid.x;
     GDA_CUDA_TRY(cudaGetLastError());
@@ -360,7 +369,7 @@ gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void
 
 gda_status sparse_value_partials(gda_problem* p, int32_t B, const float* x, double* partial, int32_t* n_part, cudaStream_t s) {
     const dim3 grid((unsigned)sparse_num_partials(p, B), (unsigned)((B / 4 + 31) / 32));
-    spmm_value<<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
+    spmm_value<<<grid, THREADS, 0, s>>>(p->n, B, score_rows(p, B), p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
     *n_part = (int32_t)grid.x;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
