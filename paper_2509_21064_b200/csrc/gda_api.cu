@@ -435,7 +435,13 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     const UpdParams up = make_upd(prm);
     int cur = parity;
     const bool scalar = prm.dual == GDA_DUAL_SCALAR;
-    for (int k = 0; k < len; ++k) {
+    int resident = 0;                                         // tiny sparse problems: the whole chunk in one launch
+    if (p->kind == GDA_KIND_SPARSE && !scalar) {
+        const int64_t before = *launches;
+        GDA_TRY(sparse_steps_resident(p, B, len, ws.x[cur], ws.y, ws.x[cur ^ (len & 1)], up, ws.state, s, launches, &resident));
+        if (resident) { *step_launches += *launches - before; cur ^= (len & 1); }
+    }
+    for (int k = 0; k < len && !resident; ++k) {
         int64_t before = *launches;
         ScalarDual sd;                                        // PDBO-s: mu follows the parity of x
         if (scalar) { sd.mu = ws.mu[cur]; sd.gpart = ws.gpart; }

@@ -134,6 +134,8 @@ struct gda_problem {
 gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
 int32_t sparse_num_gparts(const gda_problem* p);
+gda_status sparse_steps_resident(gda_problem* p, int32_t B, int32_t len, const float* x_in, float* y, float* x_out,
+                                 const UpdParams& up, const RunState* st, cudaStream_t s, int64_t* launches, int* done);
 gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);
 gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
                                  cudaStream_t s, int64_t* launches);

@@ -184,6 +184,53 @@ spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chu
     if (DUAL && active) *reinterpret_cast<float4*>(sd.gpart + (size_t)(gpart_row0 + ridx) * B + 4 * c4) = gs;
 }
 
+// ---- resident variant for tiny problems (config 1: n = 20, B = 64) -----------------------------------------------
+// When the whole state and the CSR fit one block's shared memory (n B <= RESIDENT_MAX elements: x double-buffered and
+// y, 12 bytes per element), a chunk of `len` GDA steps is ONE launch of one block: the iterates stay in shared memory, steps are
+// separated by __syncthreads(), and only the last iterate goes back to global memory.  Config 1: 1.4 us per step
+// (one SM's issue rate: about 3000 warp instructions per step) instead of 2.2 us per kernel launch.  The arithmetic per element is that of spmm_step_warp (same
+// order of the row's entries, same fused update).
+constexpr int RESIDENT_MAX = 12288;
+constexpr int RESIDENT_THREADS = 1024;
+constexpr int RESIDENT_SMEM = 200 * 1024;         // state + the whole CSR
+
+template <int GFUN>
+__global__ void __launch_bounds__(RESIDENT_THREADS)
+spmm_steps_resident(int n, int B, int nnz, int len, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                    const float* __restrict__ val2, const float* __restrict__ cprime, const float* __restrict__ x_in,
+                    float* __restrict__ y, float* __restrict__ x_out, UpdParams up, const RunState* __restrict__ st) {
+    extern __shared__ float sm[];
+    const int total = n * B;
+    float* xa = sm;                                          // x^t and x^{t+1} alternate between xa and xb
+    float* xb = sm + total;
+    float* ys = sm + 2 * total;
+    float* cps = ys + total;                                 // c'[n]
+    float* vs = cps + n;                                     // val2[nnz]
+    int* cs = reinterpret_cast<int*>(vs + nnz);              // col[nnz]
+    int* rp = cs + nnz;                                      // rowptr[n + 1]
+    for (int e = threadIdx.x; e < total; e += RESIDENT_THREADS) { xa[e] = x_in[e]; ys[e] = y[e]; }
+    for (int e = threadIdx.x; e < nnz; e += RESIDENT_THREADS) { vs[e] = val2[e]; cs[e] = col[e] * B; }
+    for (int e = threadIdx.x; e <= n; e += RESIDENT_THREADS) { rp[e] = rowptr[e]; if (e < n) cps[e] = cprime[e]; }
+    __syncthreads();
+    const uint32_t t0 = st ? st->t : 0u;
+    for (int k = 0; k < len; ++k) {
+        for (int e = threadIdx.x; e < total; e += RESIDENT_THREADS) {
+            const int i = e / B, b = e - i * B;
+            float acc = 0.0f;
+            const int a1 = rp[i + 1];
+#pragma unroll 4
+            for (int a = rp[i]; a < a1; ++a) acc = fmaf(vs[a], xa[cs[a] + b], acc);     // loads of later entries issue early
+            float xn, yn;
+            gda_update<GFUN>(xa[e], ys[e], acc + cps[i], up, t0 + (uint32_t)k, (uint32_t)i, (uint32_t)b, xn, yn);
+            xb[e] = xn;
+            ys[e] = yn;
+        }
+        __syncthreads();
+        float* tmp = xa; xa = xb; xb = tmp;
+    }
+    for (int e = threadIdx.x; e < total; e += RESIDENT_THREADS) { x_out[e] = xa[e]; y[e] = ys[e]; }
+}
+
 // S5 for sparse QUBO: partial[rb][b] = sum over the rows of block rb of x_hat_i ((Q_off x_hat)_i + c'_i)
 template <bool INTEGRAL>
 __global__ void __launch_bounds__(THREADS)
@@ -372,5 +419,28 @@ gda_status sparse_value_partials(gda_problem* p, int32_t B, const float* x, doub
     spmm_value<<<grid, THREADS, 0, s>>>(p->n, B, score_rows(p, B), p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, partial);
     *n_part = (int32_t)grid.x;
     GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+// `len` steps in one launch when the state fits one block's shared memory; *done = 0 when it does not
+gda_status sparse_steps_resident(gda_problem* p, int32_t B, int32_t len, const float* x_in, float* y, float* x_out,
+                                 const UpdParams& up, const RunState* st, cudaStream_t s, int64_t* launches, int* done) {
+    *done = 0;
+    const long long total = (long long)p->n * B;
+    const size_t smem = ((size_t)total * 3 + (size_t)p->n * 2 + 1 + (size_t)p->nnz * 2) * sizeof(float);   // x, x, y, c', rowptr, col, val
+    if (total > RESIDENT_MAX || len <= 0 || smem > (size_t)RESIDENT_SMEM) return GDA_OK;
+    static bool configured = false;
+    if (!configured) {
+        GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_QUADRATIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));
+        GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_ENTROPY>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));
+        configured = true;
+    }
+    if (up.gfun == GDA_G_QUADRATIC)
+        spmm_steps_resident<GDA_G_QUADRATIC><<<1, RESIDENT_THREADS, smem, s>>>(p->n, B, (int)p->nnz, len, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x_in, y, x_out, up, st);
+    else
+        spmm_steps_resident<GDA_G_ENTROPY><<<1, RESIDENT_THREADS, smem, s>>>(p->n, B, (int)p->nnz, len, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x_in, y, x_out, up, st);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    *done = 1;
     return GDA_OK;
 }

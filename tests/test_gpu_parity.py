@@ -384,7 +384,7 @@ def test_zero_iterations_and_lambda_tensor_and_default_stream(api, oracle):
     s.synchronize()
     ref = oracle.run(OP, X0, lam, **okw(h, iters=3, eval_every=2))
     assert np.abs(r["x"].cpu().numpy() - ref["x"]).max() <= 3 * TOL_STEP
-    assert P.info().last_run_step_launches == 3
+    assert P.info().last_run_step_launches == 2     # n B = 1600 elements: the resident kernel, one launch per chunk (2 + 1 steps)
     P.destroy()
 
 
