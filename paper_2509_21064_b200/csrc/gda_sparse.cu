@@ -144,6 +144,50 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
     update_store<GFUN, false>(row, c4, B, active, G, x, y, xn, up, t, make_float4(0.f, 0.f, 0.f, 0.f), unused);
 }
 
+// ---- narrow variant for few restarts (B <= 64; the paper's own runs use B = 10, Table 6) ---------------------------
+// With one warp per (row, 128-restart chunk) only B / 4 of the 32 lanes have work when B is small (3 lanes at B = 12).
+// Here G = the smallest power of two >= B / 4 lanes serve one row and a warp takes 32 / G rows at once: lane = (row in
+// the warp, float4 of restarts).  Every lane walks its OWN row's entries (the loads of (col, val) are broadcasts inside
+// its lane group), four gathers in flight, up to the longest row of the warp with the shorter rows predicated off.
+template <int GFUN, int G>
+__global__ void __launch_bounds__(THREADS)
+spmm_step_narrow(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                 const float* __restrict__ val2, const float* __restrict__ cprime, const float* __restrict__ x,
+                 float* __restrict__ y, float* __restrict__ xn, UpdParams up, const RunState* __restrict__ st, uint32_t t_off) {
+    constexpr int R = 32 / G;                                // rows per warp
+    const int lane = threadIdx.x & 31;
+    const int row_raw = (blockIdx.x * WARPS + (threadIdx.x >> 5)) * R + lane / G;
+    const int cl = lane % G;
+    const bool active = row_raw < n && 4 * cl < B;
+    const int row = min(row_raw, n - 1);                     // idle lanes recompute a valid element, only stores are suppressed
+    const int c4 = 4 * cl < B ? cl : 0;
+    const int start = __ldg(rowptr + row);
+    const int deg = row_raw < n ? __ldg(rowptr + row + 1) - start : 0;
+    int maxdeg = deg;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) maxdeg = max(maxdeg, __shfl_xor_sync(0xffffffffu, maxdeg, o));
+    const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
+    const uint32_t stride = 4u * (uint32_t)B;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int a = 0; a < maxdeg; a += 4) {
+        int c[4]; float v[4]; float4 g[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {                        // past the row's end: (own row, 0)
+            const bool ok = a + q < deg;
+            c[q] = ok ? __ldg(col + start + a + q) : row;
+            v[q] = ok ? __ldg(val2 + start + a + q) : 0.0f;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) g[q] = gather4(xb, stride, c[q]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) fma4(acc, v[q], g[q]);
+    }
+    const float cp = __ldg(cprime + row);
+    acc.x += cp; acc.y += cp; acc.z += cp; acc.w += cp;
+    float4 unused;
+    update_store<GFUN, false>(row, c4, B, active, acc, x, y, xn, up, (st ? st->t : 0u) + t_off, make_float4(0.f, 0.f, 0.f, 0.f), unused);
+}
+
 // row-split: one block per (heavy row, chunk); the 8 warps take interleaved 32-entry slices of the row
 // DUAL: as above; the row's g values go to sd.gpart[gpart_row0 + ridx].
 template <int GFUN, int MODE, bool DUAL>
@@ -340,6 +384,19 @@ template <int MODE, bool DUAL>
 gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
     const int chunks = (B / 4 + 31) / 32;
+    if (MODE == 0 && !DUAL && B <= 64) {                      // few restarts: several rows per warp
+        int G = 1;
+        while (4 * G < B) G <<= 1;
+        const unsigned grid = (unsigned)((p->n + WARPS * (32 / G) - 1) / (WARPS * (32 / G)));
+#define GDA_NW_CASE(GG) case GG: \
+        if (up.gfun == GDA_G_QUADRATIC) spmm_step_narrow<GDA_G_QUADRATIC, GG><<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off); \
+        else spmm_step_narrow<GDA_G_ENTROPY, GG><<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off); break;
+        switch (G) { GDA_NW_CASE(1) GDA_NW_CASE(2) GDA_NW_CASE(4) GDA_NW_CASE(8) GDA_NW_CASE(16) default: break; }
+#undef GDA_NW_CASE
+        if (launches) ++*launches;
+        GDA_CUDA_TRY(cudaGetLastError());
+        return GDA_OK;
+    }
     const int n_light = p->d_light_rows ? p->n_light : p->n;
     const int light_blocks = (n_light + WARPS - 1) / WARPS;
     if (n_light > 0) {

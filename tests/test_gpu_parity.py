@@ -664,3 +664,27 @@ def test_maxcut_dual_certificate(api, oracle):
     cut = -P.run(x0, 6.0, api.params_from_hyper(w.hyper, iters=1500))["obj"].cpu().numpy()
     assert (cut <= -bound + 1e-6).all()                         # every cut found respects the certificate
     P.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# few restarts (B <= 64, the paper's B = 10): the narrow sparse kernel, several rows per warp
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("B,scale", [(4, 0.25), (12, 0.1), (20, 0.1), (40, 0.05), (64, 0.05)])
+def test_few_restarts_narrow_kernel(api, oracle, B, scale):
+    w = wl.config(3, B=B, n_scale=scale)                        # n B > 12288: not the resident kernel
+    assert w.problem.n * B > 12288
+    OP = oracle_problem(w.problem)
+    P = api.create_from_workload(w.problem)
+    n, h = w.problem.n, w.hyper
+    X0 = wl.x0_uniform(n, B, w.x0_seed)
+    X0[5, 0], X0[6, B - 1] = 0.5, 0.5                            # exact 1/2: the tie-break hash sees (row, restart)
+    lam = np.random.default_rng(2).random((n, B), dtype=np.float32) * 6
+    r1 = P.run(dev(X0), dev(lam), api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+    ref = assert_x_step_close(r1["x"].cpu().numpy().astype(np.float64), X0, OP, oracle, okw(h, iters=1, eval_every=1), lam)
+    assert (np.abs(r1["lam"].cpu().numpy() - ref["y"]) <= TOL_STEP * np.maximum(1.0, np.abs(ref["y"]))).all()
+    r = P.run(dev(X0), 6.0, api.params_from_hyper(h, iters=1200, eval_every=100))
+    obj = r["obj"].cpu().numpy()
+    assert np.array_equal(obj, oracle.F_binary(OP, r["x_bin"].cpu().numpy()))
+    refr = oracle.run(OP, X0, 6.0, nthreads=4, **okw(h, iters=1200, eval_every=100))
+    assert_statistics_close(obj, refr["obj"])
+    P.destroy()
