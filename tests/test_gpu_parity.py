@@ -688,3 +688,29 @@ def test_few_restarts_narrow_kernel(api, oracle, B, scale):
     refr = oracle.run(OP, X0, 6.0, nthreads=4, **okw(h, iters=1200, eval_every=100))
     assert_statistics_close(obj, refr["obj"])
     P.destroy()
+
+
+@pytest.mark.parametrize("B,gfun", [(12, 1), (40, 0)])
+def test_few_restarts_maxsat(api, oracle, B, gfun):
+    w = wl.config(5, B=B, n_scale=0.1)                          # n = 1000, the paper's Max-k-SAT runs use B = 10 (3 of 32 lanes)
+    w.hyper.gfun = gfun
+    OP = oracle_problem(w.problem)
+    P = api.create_from_workload(w.problem)
+    n, h = w.problem.n, w.hyper
+    X0 = wl.x0_uniform(n, B, w.x0_seed)
+    assert grad_rel_err(P.grad(dev(X0)).cpu().numpy(), oracle.grad(OP, X0.astype(np.float64))) <= TOL_STEP
+    x, lam, t = dev(X0), torch.full((n, B), h.lambda0, dtype=torch.float32, device="cuda"), 0
+    for hop in (0, 30, 300):
+        if hop:
+            r = P.run(x, lam, api.params_from_hyper(h, iters=hop, eval_every=50, t0=t), want_final=True)
+            x, lam, t = r["x"], r["lam"], t + hop
+        r1 = P.run(x, lam, api.params_from_hyper(h, iters=1, eval_every=1, t0=t), want_final=True)
+        ref = assert_x_step_close(r1["x"].cpu().numpy().astype(np.float64), x.cpu().numpy(), OP, oracle,
+                                  okw(h, iters=1, eval_every=1, t0=t), lam.cpu().numpy())
+        assert (np.abs(r1["lam"].cpu().numpy() - ref["y"]) <= TOL_STEP * np.maximum(1.0, np.abs(ref["y"]))).all()
+    r = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=1500, eval_every=100))
+    obj = r["obj"].cpu().numpy()
+    assert np.array_equal(obj, oracle.F_binary(OP, r["x_bin"].cpu().numpy()))
+    refr = oracle.run(OP, X0, f32(h.lambda0), nthreads=4, **okw(h, iters=1500, eval_every=100))
+    assert_statistics_close(obj, refr["obj"])
+    P.destroy()
