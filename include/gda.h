@@ -97,7 +97,7 @@ void gda_destroy(gda_problem* p); /* NULL-safe; synchronises the device before f
  * constraint sum_i g(x_i) = 0 with one multiplier mu per restart,
  *     x+ = clip(x - alpha (grad f(x) + mu g'(x))),   mu+ = mu + beta sum_i g(x_i)      (reading R14)
  * the sum accumulated in fp32 in a fixed order (deterministic).  In this mode lambda0 and lambda_final are
- * DEVICE fp32 [B] (HOST [B] for gda_run_host).  Sparse QUBO and MaxSAT problems only (dense: UNSUPPORTED). */
+ * DEVICE fp32 [B] (HOST [B] for gda_run_host).  Not for Max-k-Cut problems (UNSUPPORTED). */
 typedef enum { GDA_DUAL_PER_VARIABLE = 0, GDA_DUAL_SCALAR = 1 } gda_dual;
 
 typedef struct {

@@ -379,8 +379,8 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     ws.n_part = num_partials(p, B);
     // + room for the y g(x) partial rows of gda_lagrangian
     if (st == GDA_OK) st = dmalloc((double**)&ws.partial, ((size_t)ws.n_part + (size_t)(p->n + 63) / 64) * B);
-    if (p->kind == GDA_KIND_SPARSE || p->kind == GDA_KIND_MAXSAT) {   // PDBO-s state (a few rows of B floats)
-        ws.n_gpart = p->kind == GDA_KIND_SPARSE ? sparse_num_gparts(p) : maxsat_num_gparts(p);
+    if (p->kind != GDA_KIND_KCUT) {                           // PDBO-s state (a few rows of B floats)
+        ws.n_gpart = p->kind == GDA_KIND_SPARSE ? sparse_num_gparts(p) : p->kind == GDA_KIND_MAXSAT ? maxsat_num_gparts(p) : p->n / 128;
         if (st == GDA_OK) st = dmalloc(&ws.mu[0], (size_t)B);
         if (st == GDA_OK) st = dmalloc(&ws.mu[1], (size_t)B);
         if (st == GDA_OK) st = dmalloc(&ws.gpart, (size_t)ws.n_gpart * B);
@@ -452,7 +452,7 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
         else if (p->kind == GDA_KIND_KCUT)
             GDA_TRY(kcut_step(p, B, ws.x[cur], ws.z, ws.y, ws.x[cur ^ 1], up, s, launches));
         else
-            GDA_TRY(dense_step(p, B, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, ws.state, (uint32_t)k, s, launches));
+            GDA_TRY(dense_step(p, B, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         if (scalar) GDA_TRY(gsum_reduce(B, ws.gpart, ws.n_gpart, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
         *step_launches += *launches - before;
         cur ^= 1;
@@ -539,10 +539,6 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
     GDA_REQUIRE(x0 != nullptr || p->ws.dual == prm->dual, "gda_run: a resumed run must keep the dual mode of the run it continues");
     if (prm->dual == GDA_DUAL_SCALAR && p->kind == GDA_KIND_KCUT) {
         gda_set_error("gda_run: Max-k-Cut problems need GDA_DUAL_PER_VARIABLE");
-        return GDA_ERR_UNSUPPORTED;
-    }
-    if (prm->dual == GDA_DUAL_SCALAR && p->kind == GDA_KIND_DENSE) {
-        gda_set_error("gda_run: GDA_DUAL_SCALAR (PDBO-s) is implemented for sparse QUBO and MaxSAT problems only");
         return GDA_ERR_UNSUPPORTED;
     }
     if (p->kind == GDA_KIND_DENSE && B % 128 != 0) {

@@ -53,7 +53,7 @@ template <int CG> struct Pipe {
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024;     // tiles + barriers + alignment slack
 };
 
-enum { MODE_STEP = 0, MODE_GRAD = 1, MODE_SCORE = 2 };
+enum { MODE_STEP = 0, MODE_GRAD = 1, MODE_SCORE = 2, MODE_STEP_S = 3 };   // MODE_STEP_S: PDBO-s step (one multiplier per restart)
 
 // ---- PTX wrappers -------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -184,6 +184,8 @@ struct DenseArgs {
     const float* cprime;         // [n]  c + diag(Q)
     float* gout;                 // MODE_GRAD: [n][B] gradient
     double* partial;             // MODE_SCORE: [n/128][B] partial objective sums
+    const float* mu;             // MODE_STEP_S: [B] this step's multipliers
+    float* gpart;                // MODE_STEP_S: [n/128][B] sums of g(x_i^t) over each 128-variable share
     UpdParams up;
     const RunState* st;
     uint32_t t_off;
@@ -206,6 +208,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1)
 dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                   const DenseArgs args) {
     constexpr int STAGES = Pipe<CG>::STAGES, STAGE_BYTES = Pipe<CG>::STAGE_BYTES;
+    constexpr bool STEP = MODE == MODE_STEP || MODE == MODE_STEP_S, SDUAL = MODE == MODE_STEP_S;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;            // SWIZZLE_128B needs 1024 B alignment
     const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
@@ -336,22 +339,25 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
             mbar_wait(tfull_bar(as), aphase);
             tc_fence_after();
             double score = 0.0;
-            if (MODE == MODE_STEP) {
-                // Rounds of 16 variables: 32 loads, 16 updates in registers, 32 + 2 stores.  (Keeping the loads of round
-                // r+1 in flight during round r -- two register buffers -- measured no faster: the epilogue is bound by
-                // the L2 bandwidth it shares with the operand feed, not by load latency.)
+            if (STEP) {
+                // Rounds of 16 variables: 32 loads, 16 updates in registers, 32 + 2 stores (double buffering, more warps and
+                // bulk-async staging were all measured: no faster).  PDBO-s (SDUAL): the multiplier is
+                // one number per restart, y is neither read nor written, and the thread's sum of g(x_i^t) over its 128
+                // variables goes to gpart.
                 const int c_first = half * hcols;                                 // this warpgroup's first column in the tile
                 float* __restrict__ xp = args.x + (size_t)(t.n0 + c_first) * args.B + b;
                 float* __restrict__ yp = args.y + (size_t)(t.n0 + c_first) * args.B + b;
                 uint4* zdst = reinterpret_cast<uint4*>(args.zt_out + (size_t)b * args.n + t.n0 + c_first);
                 const uint32_t trow = tmem_base + ((uint32_t)(lane_grp * 32) << 16) + (uint32_t)(as * BN + c_first);
                 const int rounds = hcols / 16;
+                const float mu_b = SDUAL ? __ldg(args.mu + b) : 0.0f;
+                float gsum = 0.0f;
                 float xa[16], ya[16];
                 auto load16 = [&](float (&xv)[16], float (&yv)[16], int r) {
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
                         xv[j] = xp[(size_t)(16 * r + j) * args.B];
-                        yv[j] = yp[(size_t)(16 * r + j) * args.B];
+                        yv[j] = SDUAL ? mu_b : yp[(size_t)(16 * r + j) * args.B];
                     }
                 };
                 auto round16 = [&](float (&xv)[16], float (&yv)[16], int r) {
@@ -368,6 +374,7 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
                         const float G = fmaf(2.0f, __uint_as_float(acc[j]), __shfl_sync(0xffffffffu, hv, j));
+                        if (SDUAL) gsum += gda_g<GFUN>(xv[j], args.up);
                         gda_update_nopert<GFUN>(xv[j], yv[j], G, args.up, xt[j], yv[j]);
                         band |= gda_in_band(xv[j], xt[j], args.up.delta) ? (1u << j) : 0u;
                     }
@@ -381,7 +388,7 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
                         xp[(size_t)(16 * r + j) * args.B] = xt[j];
-                        yp[(size_t)(16 * r + j) * args.B] = yv[j];
+                        if (!SDUAL) yp[(size_t)(16 * r + j) * args.B] = yv[j];
                     }
 #pragma unroll
                     for (int q = 0; q < 2; ++q) {
@@ -399,8 +406,9 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
                     load16(xa, ya, r);
                     round16(xa, ya, r);
                 }
+                if (SDUAL) args.gpart[(size_t)((t.n0 + c_first) / 128) * args.B + b] = gsum;
             }
-            for (int cb = 0; MODE != MODE_STEP && cb < hcols / 32; ++cb) {
+            for (int cb = 0; !STEP && cb < hcols / 32; ++cb) {
                 const int col0 = half * hcols + cb * 32;
                 const int i0 = t.n0 + col0;
                 uint32_t acc[32];
@@ -601,13 +609,18 @@ gda_status dense_make_operand(gda_problem* p, int32_t B, const float* x, __nv_bf
 }
 
 gda_status dense_step(gda_problem* p, int32_t B, float* x, float* y, const __nv_bfloat16* zt_in, __nv_bfloat16* zt_out,
-                      const UpdParams& up, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
+                      const UpdParams& up, const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s,
+                      int64_t* launches) {
     const CUtensorMap* ta;
     GDA_TRY(z_maps(p, B, zt_in, &ta));
     DenseArgs a{};
     a.n = p->n; a.B = B; a.x = x; a.y = y; a.zt_out = zt_out; a.hvec = p->d_rowsum; a.cprime = p->d_cprime;
-    a.up = up; a.st = st; a.t_off = t_off;
+    a.up = up; a.st = st; a.t_off = t_off; a.mu = sd.mu; a.gpart = sd.gpart;
     if (launches) ++*launches;
+    if (sd.mu) {                                               // PDBO-s
+        if (up.gfun == GDA_G_QUADRATIC) return launch_gemm<MODE_STEP_S, GDA_G_QUADRATIC>(p, *ta, a, s);
+        return launch_gemm<MODE_STEP_S, GDA_G_ENTROPY>(p, *ta, a, s);
+    }
     if (up.gfun == GDA_G_QUADRATIC) return launch_gemm<MODE_STEP, GDA_G_QUADRATIC>(p, *ta, a, s);
     return launch_gemm<MODE_STEP, GDA_G_ENTROPY>(p, *ta, a, s);
 }

@@ -168,7 +168,7 @@ gda_status dense_prepare(gda_problem* p, const float* Q_host, const float* c_hos
 gda_status dense_make_operand(gda_problem* p, int32_t B, const float* x, __nv_bfloat16* zt, int hat,
                               cudaStream_t s, int64_t* launches);
 gda_status dense_step(gda_problem* p, int32_t B, float* x, float* y, const __nv_bfloat16* zt_in,
-                      __nv_bfloat16* zt_out, const UpdParams& up, const RunState* st, uint32_t t_off,
+                      __nv_bfloat16* zt_out, const UpdParams& up, const ScalarDual& sd, const RunState* st, uint32_t t_off,
                       cudaStream_t s, int64_t* launches);
 gda_status dense_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);
 gda_status dense_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,

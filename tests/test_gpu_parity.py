@@ -589,12 +589,6 @@ def test_pdbo_s_heavy_rows_and_argument_checks(api, oracle):
         P.resume(api.params_from_hyper(h, dual=api.DUAL_PER_VARIABLE), r)
     assert e.value.status == 1
     P.destroy()
-    wd = wl.config(4, B=128, n_scale=0.0625)
-    Pd = api.create_from_workload(wd.problem)
-    with pytest.raises(api.GdaError) as e:
-        Pd.run(dev(wl.x0_uniform(wd.problem.n, 128, 1)), 1.0, api.params_from_hyper(wd.hyper, iters=1, dual=api.DUAL_SCALAR))
-    assert e.value.status == 4
-    Pd.destroy()
 
 
 # ------------------------------------------------------------------------------------------------
@@ -713,4 +707,33 @@ def test_few_restarts_maxsat(api, oracle, B, gfun):
     assert np.array_equal(obj, oracle.F_binary(OP, r["x_bin"].cpu().numpy()))
     refr = oracle.run(OP, X0, f32(h.lambda0), nthreads=4, **okw(h, iters=1500, eval_every=100))
     assert_statistics_close(obj, refr["obj"])
+    P.destroy()
+
+
+@pytest.mark.parametrize("w", [DENSE[0], DENSE[2], DENSE[4]], ids=lambda w: f"{w.name}_n{w.problem.n}_B{w.B}")
+def test_pdbo_s_dense(api, oracle, w):
+    """PDBO-s on the tcgen05 path: the multiplier comes from a [B] array, y is not touched, the epilogue threads' sums
+    of g go through gsum_reduce."""
+    ws = wl.pdbo_s_variant(w)
+    OP = oracle_problem(ws.problem)
+    P = api.create_from_workload(ws.problem)
+    n, B, h = ws.problem.n, ws.B, ws.hyper
+    x = dev(wl.x0_uniform(n, B, ws.x0_seed))
+    mu = dev(np.linspace(0.5 * h.lambda0, h.lambda0, B).astype(np.float32))
+    for hop in (0, 3, 40):
+        if hop:
+            r = P.run(x, mu, api.params_from_hyper(h, iters=hop, eval_every=20), want_final=True)
+            x, mu = r["x"], r["lam"]
+        r1 = P.run(x, mu, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+        xp = x.cpu().numpy()
+        ref = oracle.run(OP, xp, mu.cpu().numpy(), **okw(h, iters=1, eval_every=1, delta=0.0))
+        Gref = oracle.grad(OP, xp.astype(np.float64))
+        tol = f32(h.alpha) * TOL_GRAD_BF16 * np.abs(Gref).max(axis=0, keepdims=True) + TOL_STEP      # bf16 operand (north star)
+        xg = r1["x"].cpu().numpy().astype(np.float64)
+        far = np.abs(xg - ref["x"]) > tol
+        assert far.mean() < 5e-3 and (np.abs(xg[far] - 0.5) <= 1.01e-4 + 1e-6).all()               # only perturbed entries differ
+        assert (np.abs(r1["lam"].cpu().numpy() - ref["y"]) <= mu_tolerance(h, n, ref["y"])).all()
+    r = P.run(dev(wl.x0_uniform(n, B, 5)), h.lambda0, api.params_from_hyper(h, iters=600, eval_every=100))
+    obj, xb = r["obj"].cpu().numpy(), r["x_bin"].cpu().numpy()
+    assert (np.abs(obj - oracle.F_binary(OP, xb)) <= dense_F_tolerance(ws.problem, xb)).all()
     P.destroy()
