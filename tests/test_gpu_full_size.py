@@ -76,3 +76,32 @@ def test_full_size_config_on_sampled_restarts(api, oracle, idx):
     if idx in (2, 3):                                            # far better than a random cut already (m/2 in expectation)
         assert -obj.max() > 0.55 * np.abs(Pw.edge_w).sum() if idx == 2 else -obj.max() > 0
     P.destroy()
+
+
+def statistics_close(obj, obj_ref):
+    """(d): mean and best objective within 0.5 % of the oracle's, with the sampling-noise floor of
+    tests/test_gpu_parity.py::assert_statistics_close (the two runs are independent samples)."""
+    nb = obj.shape[0]
+    sd = float(np.sqrt(0.5 * (obj.var() + obj_ref.var())))
+    ok_mean = abs(obj.mean() - obj_ref.mean()) <= max(0.005 * abs(obj_ref.mean()), 3.0 * sd * np.sqrt(2.0 / nb))
+    ok_best = abs(obj.min() - obj_ref.min()) <= max(0.005 * abs(obj_ref.min()), sd)
+    return ok_mean and ok_best
+
+
+@pytest.mark.parametrize("idx", [2, 3, 5])
+def test_full_length_run_statistics_match_the_oracle(api, oracle, idx):
+    """(d) at full size AND full length: all B restarts on the GPU, the first 32 of them through the oracle
+    (fp64, OpenMP over restarts) for the whole `iters` of the config."""
+    w = wl.config(idx)
+    Pw, h, B = w.problem, w.hyper, w.B
+    OP = oracle_problem(Pw)
+    P = api.create_from_workload(Pw)
+    X0 = wl.x0_uniform(Pw.n, B, w.x0_seed)
+    r = P.run(torch.from_numpy(X0).cuda(), h.lambda0, api.params_from_hyper(h))
+    obj = r["obj"].cpu().numpy()
+    sub = np.arange(32, dtype=np.int32)
+    ref = oracle.run(OP, X0[:, sub], f32(h.lambda0), col_ids=sub, nthreads=16, **okw(h))
+    assert np.array_equal(obj[sub], oracle.F_binary(OP, r["x_bin"][:, :32].cpu().numpy()))
+    assert statistics_close(obj[sub], ref["obj"]), (obj[sub].mean(), ref["obj"].mean(), obj[sub].min(), ref["obj"].min())
+    assert abs(obj.mean() - ref["obj"].mean()) <= 0.01 * abs(ref["obj"].mean()) + 3.0 * ref["obj"].std()   # the other restarts too
+    P.destroy()
