@@ -68,6 +68,20 @@ static gda_status device_setup(gda_problem* p) {
     return GDA_OK;
 }
 
+// Entry points run on the problem's device and leave the caller's current device as they found it.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; cudaGetLastError(); }
+        if (prev != dev) err = cudaSetDevice(dev); else prev = -1;            // nothing to restore
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+#define GDA_ON_DEVICE(p) DeviceGuard dev_guard__((p)->device); GDA_CUDA_TRY(dev_guard__.err)
+
 static bool is_integer_valued(float v, float limit) { return std::isfinite(v) && v == std::nearbyint(v) && std::fabs(v) <= limit; }
 
 // ---------------------------------------------------------------------------------------------------
@@ -180,9 +194,14 @@ extern "C" gda_status gda_create_maxkcut(int32_t n, int32_t k, const int32_t* ro
     GDA_REQUIRE(out != nullptr, "gda_create_maxkcut: out is NULL");
     GDA_REQUIRE(k >= 2 && k <= 8, "gda_create_maxkcut: k must be in [2, 8] (got %d)", k);
     GDA_REQUIRE(n > 0 && rowptr != nullptr, "gda_create_maxkcut: n must be > 0 and rowptr non-NULL");
+    // the CSR is validated in full by gda_create_qubo_csr below; what the diagonal scan itself reads is checked first
+    GDA_REQUIRE(rowptr[0] == 0, "gda_create_maxkcut: rowptr[0] must be 0");
+    for (int i = 0; i < n; ++i)
+        GDA_REQUIRE(rowptr[i + 1] >= rowptr[i], "gda_create_maxkcut: rowptr decreases at row %d", i);
+    GDA_REQUIRE(rowptr[n] == 0 || (col != nullptr && val != nullptr), "gda_create_maxkcut: col/val is NULL");
     for (int i = 0; i < n; ++i)
         for (int a = rowptr[i]; a < rowptr[i + 1]; ++a)
-            GDA_REQUIRE(col == nullptr || col[a] != i || val[a] == 0.0f, "gda_create_maxkcut: non-zero diagonal entry at node %d", i);
+            GDA_REQUIRE(col[a] != i || val[a] == 0.0f, "gda_create_maxkcut: non-zero diagonal entry at node %d", i);
     gda_problem* p = nullptr;
     GDA_TRY(gda_create_qubo_csr(n, rowptr, col, val, nullptr, &p));
     p->kind = GDA_KIND_KCUT;
@@ -317,6 +336,7 @@ static void free_workspace(gda_problem* p) {
 
 extern "C" void gda_destroy(gda_problem* p) {
     if (!p) return;
+    DeviceGuard guard(p->device);
     cudaDeviceSynchronize();
     free_workspace(p);
     cudaFree(p->d_rowptr); cudaFree(p->d_col); cudaFree(p->d_val2); cudaFree(p->d_cprime);
@@ -470,10 +490,21 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     return GDA_OK;
 }
 
+// Keys are compared bitwise on canonicalised parameters (canonical_params): fields the kernels ignore are zeroed, so an
+// uninitialised or NaN log_eps with the quadratic g cannot force a re-capture on every chunk.
 bool GraphKey::operator==(const GraphKey& o) const {
     return B == o.B && len == o.len && parity == o.parity && with_eval == o.with_eval &&
-           prm.alpha == o.prm.alpha && prm.beta == o.prm.beta && prm.delta == o.prm.delta &&
-           prm.log_eps == o.prm.log_eps && prm.gfun == o.prm.gfun && prm.seed == o.prm.seed && prm.dual == o.prm.dual;
+           std::memcmp(&prm.alpha, &o.prm.alpha, sizeof(float)) == 0 && std::memcmp(&prm.beta, &o.prm.beta, sizeof(float)) == 0 &&
+           std::memcmp(&prm.delta, &o.prm.delta, sizeof(float)) == 0 && std::memcmp(&prm.log_eps, &o.prm.log_eps, sizeof(float)) == 0 &&
+           prm.gfun == o.prm.gfun && prm.seed == o.prm.seed && prm.dual == o.prm.dual;
+}
+
+static gda_params canonical_params(const gda_problem* p, const gda_params& in) {
+    gda_params c = in;
+    if (c.gfun == GDA_G_QUADRATIC) c.log_eps = 0.0f;          // ignored by the quadratic g
+    if (p->kind == GDA_KIND_KCUT) c.delta = 0.0f;             // no perturbation for Max-k-Cut (reading K3)
+    c.iters = 0; c.eval_every = 0; c.t0 = 0; c.reserved = 0;  // not part of a chunk's identity
+    return c;
 }
 
 static bool graphs_disabled() {
@@ -487,7 +518,7 @@ static gda_status launch_chunk(gda_problem* p, int32_t B, int32_t len, int32_t p
         return enqueue_chunk(p, B, len, parity, prm, s, &p->last_launches, &p->last_step_launches);
     }
     GraphKey key;
-    key.B = B; key.len = len; key.parity = parity; key.with_eval = 1; key.prm = prm;
+    key.B = B; key.len = len; key.parity = parity; key.with_eval = 1; key.prm = canonical_params(p, prm);
     CachedGraph* hit = nullptr;
     for (auto& g : p->graphs) if (g.key == key) { hit = &g; break; }
     if (!hit) {
@@ -552,11 +583,13 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
     return GDA_OK;
 }
 
-extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const float* lambda0, float lambda0_scalar,
-                              const gda_params* prm, uint8_t* x_bin, double* obj, int32_t* best_restart,
-                              const gda_extra* extra, void* stream) {
+// The run itself.  `host` says where x0, lambda0, x_bin, obj and best_restart live: the copies in and out are
+// cudaMemcpyDefault (unified addressing tells host from device), everything between them is the same.
+static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const float* lambda0, float lambda0_scalar,
+                           const gda_params* prm, uint8_t* x_bin, double* obj, int32_t* best_restart,
+                           const gda_extra* extra, void* stream, bool host) {
     GDA_TRY(check_run_args(p, B, x0, prm, x_bin, obj, best_restart));
-    GDA_CUDA_TRY(cudaSetDevice(p->device));
+    GDA_ON_DEVICE(p);
     GDA_TRY(ensure_workspace(p, B));
     cudaStream_t user, s;
     GDA_TRY(pick_stream(p, stream, &user, &s));
@@ -568,6 +601,7 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
     if (x0) {
         ws.has_state = false;
         ws.dual = prm->dual;
+        ws.n_eval_host = 0;
         GDA_TRY(run_init(p, B, x0, lambda0, lambda0_scalar, (uint32_t)prm->t0, s, &p->last_launches));
         if (p->kind == GDA_KIND_DENSE)
             GDA_TRY(dense_make_operand(p, B, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
@@ -577,6 +611,7 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
         parity = ws.parity;      // resume: iterates, duals, best-so-far and the iteration counter stay as they are
     }
     const int32_t full = prm->iters / prm->eval_every, rem = prm->iters % prm->eval_every;
+    const int32_t n_eval = std::max(1, full + (rem > 0 ? 1 : 0)), trace_off = ws.n_eval_host;
     for (int32_t c = 0; c < full; ++c) {
         GDA_TRY(launch_chunk(p, B, prm->eval_every, parity, *prm, s));
         parity ^= (prm->eval_every & 1);
@@ -588,9 +623,9 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
     ws.parity = parity;
     ws.has_state = true;
     const float* xfin = (p->kind == GDA_KIND_DENSE) ? ws.x[0] : ws.x[parity];
-    GDA_CUDA_TRY(cudaMemcpyAsync(x_bin, ws.x_bin, elems, cudaMemcpyDeviceToDevice, s));
-    GDA_CUDA_TRY(cudaMemcpyAsync(obj, ws.best_obj, (size_t)B * sizeof(double), cudaMemcpyDeviceToDevice, s));
-    GDA_CUDA_TRY(cudaMemcpyAsync(best_restart, ws.best_restart, sizeof(int32_t), cudaMemcpyDeviceToDevice, s));
+    GDA_CUDA_TRY(cudaMemcpyAsync(x_bin, ws.x_bin, elems, cudaMemcpyDefault, s));
+    GDA_CUDA_TRY(cudaMemcpyAsync(obj, ws.best_obj, (size_t)B * sizeof(double), cudaMemcpyDefault, s));
+    GDA_CUDA_TRY(cudaMemcpyAsync(best_restart, ws.best_restart, sizeof(int32_t), cudaMemcpyDefault, s));
     if (extra) {
         if (extra->x_final && p->kind == GDA_KIND_KCUT)      // the logits Z^T, [k][n][B]
             GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, ws.z, elems * p->kparts * sizeof(float), cudaMemcpyDeviceToDevice, s));
@@ -601,52 +636,32 @@ extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const 
             GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.y, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
         if (extra->ones) GDA_TRY(eval_count_ones(p, B, ws.x_bin, extra->ones, s, &p->last_launches));
         if (extra->best_obj) GDA_CUDA_TRY(cudaMemcpyAsync(extra->best_obj, ws.best_val, sizeof(double), cudaMemcpyDeviceToDevice, s));
-        const int32_t n_eval = std::max(1, full + (rem > 0 ? 1 : 0));
-        const int32_t cnt = std::min(std::min(n_eval, extra->trace_cap), ws.trace_cap);
-        if (extra->trace_best && cnt > 0) GDA_CUDA_TRY(cudaMemcpyAsync(extra->trace_best, ws.trace_best, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToDevice, s));
-        if (extra->trace_ns && cnt > 0) GDA_CUDA_TRY(cudaMemcpyAsync(extra->trace_ns, ws.trace_ns, (size_t)cnt * sizeof(uint64_t), cudaMemcpyDeviceToDevice, s));
+        // THIS call's evaluations: a resumed run appends to the trace of the run it continues (n_eval is not reset)
+        const int32_t cnt = std::min(std::min(n_eval, extra->trace_cap), ws.trace_cap - trace_off);
+        if (extra->trace_best && cnt > 0) GDA_CUDA_TRY(cudaMemcpyAsync(extra->trace_best, ws.trace_best + trace_off, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToDevice, s));
+        if (extra->trace_ns && cnt > 0) GDA_CUDA_TRY(cudaMemcpyAsync(extra->trace_ns, ws.trace_ns + trace_off, (size_t)cnt * sizeof(uint64_t), cudaMemcpyDeviceToDevice, s));
     }
-    return join_stream(p, user, s);
+    ws.n_eval_host = std::min(ws.trace_cap, trace_off + n_eval);
+    GDA_TRY(join_stream(p, user, s));
+    if (host) GDA_CUDA_TRY(cudaStreamSynchronize(user));     // the HOST results are valid when the call returns
+    return GDA_OK;
+}
+
+extern "C" gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const float* lambda0, float lambda0_scalar,
+                              const gda_params* prm, uint8_t* x_bin, double* obj, int32_t* best_restart,
+                              const gda_extra* extra, void* stream) {
+    return run_impl(p, B, x0, lambda0, lambda0_scalar, prm, x_bin, obj, best_restart, extra, stream, false);
 }
 
 // ---------------------------------------------------------------------------------------------------
-// gda_run_host: same run, HOST buffers in and out (copies are part of the call)
+// gda_run_host: same run, HOST buffers in and out (the copies are part of the call).  No staging buffers and no
+// allocation per call: x0 / lambda0 are copied straight into the workspace and the results straight out of it.
 // ---------------------------------------------------------------------------------------------------
 extern "C" gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, const float* lambda0,
                                    float lambda0_scalar, const gda_params* prm, uint8_t* x_bin, double* obj,
                                    int32_t* best_restart, void* stream) {
     GDA_REQUIRE(x0 != nullptr, "gda_run_host: x0 is required");
-    GDA_TRY(check_run_args(p, B, x0, prm, x_bin, obj, best_restart));
-    GDA_CUDA_TRY(cudaSetDevice(p->device));
-    GDA_TRY(ensure_workspace(p, B));
-    cudaStream_t user, s;
-    GDA_TRY(pick_stream(p, stream, &user, &s));
-    Workspace& ws = p->ws;
-    const size_t elems = (size_t)p->n * B;
-    // device staging: x0 -> x[1] would be clobbered by the run, so stage in dedicated buffers
-    float* d_x0 = nullptr; float* d_l0 = nullptr; uint8_t* d_xb = nullptr; double* d_obj = nullptr; int32_t* d_best = nullptr;
-    const size_t x0_elems = p->kind == GDA_KIND_KCUT ? elems * p->kparts : elems;
-    gda_status st = dmalloc(&d_x0, x0_elems);
-    const size_t l0_elems = (prm && prm->dual == GDA_DUAL_SCALAR) ? (size_t)B : elems;
-    if (st == GDA_OK && lambda0) st = dmalloc(&d_l0, l0_elems);
-    if (st == GDA_OK) st = dmalloc(&d_xb, elems);
-    if (st == GDA_OK) st = dmalloc(&d_obj, (size_t)B);
-    if (st == GDA_OK) st = dmalloc(&d_best, 1);
-    cudaError_t e = cudaSuccess;
-    if (st == GDA_OK) {
-        e = cudaMemcpyAsync(d_x0, x0, x0_elems * sizeof(float), cudaMemcpyHostToDevice, s);
-        if (e == cudaSuccess && lambda0) e = cudaMemcpyAsync(d_l0, lambda0, l0_elems * sizeof(float), cudaMemcpyHostToDevice, s);
-        if (e == cudaSuccess) st = gda_run(p, B, d_x0, d_l0, lambda0_scalar, prm, d_xb, d_obj, d_best, nullptr, s);
-        if (st == GDA_OK && e == cudaSuccess) e = cudaMemcpyAsync(x_bin, d_xb, elems, cudaMemcpyDeviceToHost, s);
-        if (st == GDA_OK && e == cudaSuccess) e = cudaMemcpyAsync(obj, d_obj, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, s);
-        if (st == GDA_OK && e == cudaSuccess) e = cudaMemcpyAsync(best_restart, d_best, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    }
-    cudaFree(d_x0); cudaFree(d_l0); cudaFree(d_xb); cudaFree(d_obj); cudaFree(d_best);
-    (void)ws;
-    if (st != GDA_OK) return st;
-    if (e != cudaSuccess) { gda_set_error("gda_run_host: %s", cudaGetErrorString(e)); return GDA_ERR_CUDA; }
-    return join_stream(p, user, s);
+    return run_impl(p, B, x0, lambda0, lambda0_scalar, prm, x_bin, obj, best_restart, nullptr, stream, true);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -657,7 +672,7 @@ extern "C" gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float*
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_grad: B must be a positive multiple of 4 (got %d)", B);
     if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_grad: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
     if (p->kind == GDA_KIND_DENSE && B % 128 != 0) { gda_set_error("gda_grad: the dense path needs B %% 128 == 0"); return GDA_ERR_UNSUPPORTED; }
-    GDA_CUDA_TRY(cudaSetDevice(p->device));
+    GDA_ON_DEVICE(p);
     cudaStream_t user, s;
     if (p->kind == GDA_KIND_DENSE) GDA_TRY(ensure_workspace(p, B));
     GDA_TRY(pick_stream(p, stream, &user, &s));
@@ -672,7 +687,7 @@ extern "C" gda_status gda_score(gda_problem* p, int32_t B, const float* x, doubl
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_score: B must be a positive multiple of 4 (got %d)", B);
     if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_score: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
     if (p->kind == GDA_KIND_DENSE && B % 128 != 0) { gda_set_error("gda_score: the dense path needs B %% 128 == 0"); return GDA_ERR_UNSUPPORTED; }
-    GDA_CUDA_TRY(cudaSetDevice(p->device));
+    GDA_ON_DEVICE(p);
     GDA_TRY(ensure_workspace(p, B));
     cudaStream_t user, s;
     GDA_TRY(pick_stream(p, stream, &user, &s));
@@ -699,7 +714,7 @@ extern "C" gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, 
     GDA_REQUIRE(gfun == GDA_G_QUADRATIC || gfun == GDA_G_ENTROPY, "gda_lagrangian: unknown gfun %d", gfun);
     if (gfun == GDA_G_ENTROPY) GDA_REQUIRE(log_eps > 0.0f && log_eps < 0.5f, "gda_lagrangian: log_eps must be in (0, 1/2)");
     if (p->kind == GDA_KIND_DENSE || p->kind == GDA_KIND_KCUT) { gda_set_error("gda_lagrangian: sparse QUBO and MaxSAT problems only"); return GDA_ERR_UNSUPPORTED; }
-    GDA_CUDA_TRY(cudaSetDevice(p->device));
+    GDA_ON_DEVICE(p);
     GDA_TRY(ensure_workspace(p, B));
     cudaStream_t user, s;
     GDA_TRY(pick_stream(p, stream, &user, &s));

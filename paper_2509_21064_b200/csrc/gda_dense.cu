@@ -511,14 +511,16 @@ struct DenseHost {
     CUtensorMap tmap_z[2];
     const void* z_ptr[2] = {nullptr, nullptr};
     int32_t z_B = 0;
-    bool attr_set = false;
+    // co-resident clusters per kernel variant (1 CTA per SM), found -- together with the shared-memory opt-in -- on this
+    // handle's first launch of the variant: per handle, hence per device, and no process-wide state
+    int max_clusters[4 * 2 * 3] = {};
 };
 
 template <int MODE, int GFUN, int CG, int NP>
 gda_status launch_variant(gda_problem* p, const CUtensorMap& ta, const CUtensorMap& tq, const DenseArgs& a, cudaStream_t s) {
     auto kern = dense_gemm_kernel<MODE, GFUN, CG, NP>;
     constexpr int CSIZE = CG * NP;
-    static int max_clusters = 0;                              // co-resident clusters of this kernel (1 CTA per SM)
+    int& max_clusters = static_cast<DenseHost*>(p->tmap_Q)->max_clusters[(MODE * 2 + GFUN) * 3 + (CG - 1) + (NP - 1)];
     cudaLaunchConfig_t cfg = {};
     cfg.blockDim = dim3(NUM_THREADS); cfg.dynamicSmemBytes = Pipe<CG>::SMEM_BYTES; cfg.stream = s;
     cudaLaunchAttribute attr[1];

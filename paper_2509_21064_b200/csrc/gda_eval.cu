@@ -257,14 +257,16 @@ gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0,
                     uint32_t t0, cudaStream_t s, int64_t* launches) {
     Workspace& ws = p->ws;
     const size_t elems = (size_t)p->n * B;
+    // x0 / l0 may be HOST pointers (gda_run_host): cudaMemcpyDefault tells by unified addressing
     if (p->kind == GDA_KIND_KCUT)
-        GDA_CUDA_TRY(cudaMemcpyAsync(ws.z, x0, elems * p->kparts * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        GDA_CUDA_TRY(cudaMemcpyAsync(ws.z, x0, elems * p->kparts * sizeof(float), cudaMemcpyDefault, s));
     else
-        GDA_CUDA_TRY(cudaMemcpyAsync(ws.x[0], x0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        GDA_CUDA_TRY(cudaMemcpyAsync(ws.x[0], x0, elems * sizeof(float), cudaMemcpyDefault, s));
     if (ws.dual == GDA_DUAL_SCALAR) {
-        GDA_TRY(mu_init(B, l0, l0_scalar, ws.mu[0], s, launches));
+        if (l0) GDA_CUDA_TRY(cudaMemcpyAsync(ws.mu[0], l0, (size_t)B * sizeof(float), cudaMemcpyDefault, s));
+        else GDA_TRY(mu_init(B, nullptr, l0_scalar, ws.mu[0], s, launches));
     } else if (l0) {
-        GDA_CUDA_TRY(cudaMemcpyAsync(ws.y, l0, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        GDA_CUDA_TRY(cudaMemcpyAsync(ws.y, l0, elems * sizeof(float), cudaMemcpyDefault, s));
     } else {
         const size_t n_vec = elems / 4;
         fill_kernel<<<(unsigned)((n_vec + 255) / 256), 256, 0, s>>>(n_vec, reinterpret_cast<float4*>(ws.y), l0_scalar);

@@ -80,6 +80,7 @@ struct Workspace {
     double* trace_best = nullptr;       // internal trace buffers (copied out on request)
     uint64_t* trace_ns = nullptr;
     int32_t trace_cap = 0;
+    int32_t n_eval_host = 0;            // evaluations recorded in the trace so far (run + resumed runs)
     // dense path
     __nv_bfloat16* zt[2] = {nullptr, nullptr};  // [B][n] bf16 GEMM operand (centred x - 1/2, or x_hat)
     int32_t score_scratch = 1;                  // which zt buffer dense scoring may clobber (the one not holding z^t)
@@ -112,6 +113,7 @@ struct gda_problem {
     int32_t* d_heavy_rows = nullptr; int32_t n_heavy = 0;   // rows handled by the row-split kernel
     int32_t* d_light_rows = nullptr; int32_t n_light = 0;   // nullptr = all rows, in order
     int32_t max_deg = 0;
+    bool resident_configured = false;    // shared-memory opt-in of the resident kernels done on this handle's device
     int32_t* d_ell = nullptr;            // [n][16] packed low-degree rows: 8 cols + 8 val2 (see gda_sparse.cu); nullptr = not built
     // dense QUBO: Q_off in bf16 [n][n] (zero diagonal), r0 = Q_off 1 (row sums) for the centred operand
     __nv_bfloat16* d_Qbf = nullptr; float* d_rowsum = nullptr;

@@ -225,7 +225,8 @@ void launch_kw(gda_problem* p, int32_t B, dim3 grid, const float* x, float* y, f
 #define GDA_MS_CASE(K) \
         case K: if (pad) maxsat_step_kernel<GFUN, MODE, K, true, DUAL><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); \
                 else maxsat_step_kernel<GFUN, MODE, K, false, DUAL><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
-    const bool pad = p->kmin != p->kmax;
+    // records hold ENC_PAD when clauses are shorter than kmax -- and ALWAYS when kmax == 1 (kw is then 1 with no other literal)
+    const bool pad = p->kmin != p->kmax || p->kmax == 1;
     switch (p->kw) {
         GDA_MS_CASE(1) GDA_MS_CASE(2) GDA_MS_CASE(3) GDA_MS_CASE(4)
         default: maxsat_step_kernel<GFUN, MODE, 0, true, DUAL><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;

@@ -486,7 +486,7 @@ gda_status sparse_steps_resident(gda_problem* p, int32_t B, int32_t len, const f
     const long long total = (long long)p->n * B;
     const size_t smem = ((size_t)total * 3 + (size_t)p->n * 2 + 1 + (size_t)p->nnz * 2) * sizeof(float);   // x, x, y, c', rowptr, col, val
     if (total > RESIDENT_MAX || len <= 0 || smem > (size_t)RESIDENT_SMEM) return GDA_OK;
-    static bool configured = false;
+    bool& configured = p->resident_configured;               // per handle (hence per device), not per process
     if (!configured) {
         GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_QUADRATIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));
         GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_ENTROPY>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));

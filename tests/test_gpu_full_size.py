@@ -107,6 +107,30 @@ def test_full_length_run_statistics_match_the_oracle(api, oracle, idx):
     P.destroy()
 
 
+def test_config4_full_length_run_statistics_match_the_oracle(api, oracle):
+    """(d) for the dense config at full size AND full length: all 4096 restarts for 2000 iterations on the GPU (the
+    cluster-of-pairs variant bench.py times), 16 of them through the fp64 oracle (n^2 work per restart-step: about
+    a minute and a half on 16 cores)."""
+    w = wl.config(4)
+    Pw, h, B = w.problem, w.hyper, w.B
+    OP = oracle_problem(Pw)
+    P = api.create_from_workload(Pw)
+    X0 = wl.x0_uniform(Pw.n, B, w.x0_seed)
+    r = P.run(torch.from_numpy(X0).cuda(), h.lambda0, api.params_from_hyper(h))
+    obj = r["obj"].cpu().numpy()
+    sub = np.arange(0, B, B // 16, dtype=np.int32)[:16]           # one column out of every 256: every cluster position
+    ref = oracle.run(OP, X0[:, sub], f32(h.lambda0), col_ids=sub, nthreads=16, **okw(h))
+    xb = r["x_bin"][:, torch.from_numpy(sub).long().cuda()].cpu().numpy()
+    Fref = oracle.F_binary(OP, xb)                               # (a) fp64 with the dense path's relative tolerance
+    tolF = 1e-5 * (xb.astype(np.float64).T @ np.abs(Pw.Q.astype(np.float64)) @ xb.astype(np.float64)).diagonal() + 1e-3
+    assert (np.abs(obj[sub] - Fref) <= tolF).all()
+    print(f"cfg4 full run: GPU mean {obj[sub].mean():.1f} best {obj[sub].min():.1f} (all restarts: mean {obj.mean():.1f} "
+          f"best {obj.min():.1f}); oracle mean {ref['obj'].mean():.1f} best {ref['obj'].min():.1f}")
+    assert statistics_close(obj[sub], ref["obj"]), (obj[sub].mean(), ref["obj"].mean(), obj[sub].min(), ref["obj"].min())
+    assert abs(obj.mean() - ref["obj"].mean()) <= 0.005 * abs(ref["obj"].mean()) + 3.0 * ref["obj"].std() / 4.0
+    P.destroy()
+
+
 def test_mis_on_a_3_regular_graph_against_the_papers_table_13(api):
     """MIS on a random 3-regular graph with 10^4 vertices, the paper's own setting (Table 6
     hyper-parameters).  The instances are the paper's only in distribution, so this is context, not parity: the best

@@ -316,12 +316,14 @@ def test_sparse_edge_cases(api, oracle, case):
     P.destroy()
 
 
-@pytest.mark.parametrize("case", ["mixed_k", "long_clauses", "unweighted", "float_weights"])
+@pytest.mark.parametrize("case", ["mixed_k", "long_clauses", "unweighted", "float_weights", "unit_only", "unit_and_pairs"])
 def test_maxsat_edge_cases(api, oracle, case):
     rng = np.random.default_rng(21)
     n = 60
-    if case in ("mixed_k", "long_clauses"):
-        ks = rng.integers(1, 6, size=150) if case == "mixed_k" else rng.integers(5, 9, size=40)
+    if case in ("mixed_k", "long_clauses", "unit_only", "unit_and_pairs"):
+        ks = {"mixed_k": rng.integers(1, 6, size=150), "long_clauses": rng.integers(5, 9, size=40),
+              "unit_only": np.ones(45, dtype=np.int64),         # kmax = 1: every "other literal" slot is padding
+              "unit_and_pairs": rng.integers(1, 3, size=120)}[case]
         lits, cptr = [], [0]
         for k in ks:
             v = rng.choice(n, size=k, replace=False)
@@ -386,6 +388,66 @@ def test_zero_iterations_and_lambda_tensor_and_default_stream(api, oracle):
     assert np.abs(r["x"].cpu().numpy() - ref["x"]).max() <= 3 * TOL_STEP
     assert P.info().last_run_step_launches == 2     # n B = 1600 elements: the resident kernel, one launch per chunk (2 + 1 steps)
     P.destroy()
+
+
+def test_resumed_run_returns_its_own_slice_of_the_trace(api):
+    """A resumed gda_run (x0 == NULL) appends to the evaluation trace of the run it continues; the caller's trace
+    buffers receive THIS call's evaluations (gda_extra.trace_best / trace_ns), not the earliest entries."""
+    w = wl.config(3, B=64, n_scale=0.05)
+    P = api.create_from_workload(w.problem)
+    n, B, h = w.problem.n, w.B, w.hyper
+    x0 = dev(wl.x0_uniform(n, B, 7))
+    whole = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=600, eval_every=100), trace_cap=8)
+    tb_whole = whole["trace_best"].cpu().numpy()[:6]
+    first = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=400, eval_every=100), trace_cap=8)
+    tb = torch.full((8,), float("nan"), dtype=torch.float64, device="cuda")
+    tn = torch.zeros(8, dtype=torch.int64, device="cuda")
+    ex = api.Extra()
+    ex.trace_best, ex.trace_ns, ex.trace_cap = tb.data_ptr(), tn.data_ptr(), 8
+    prm = api.params_from_hyper(h, iters=200, eval_every=100)
+    api._check(api.lib().gda_run(P._h, B, None, None, 0.0, api.C.byref(prm), first["x_bin"].data_ptr(), first["obj"].data_ptr(),
+                                 first["best_restart"].data_ptr(), api.C.byref(ex), torch.cuda.current_stream().cuda_stream))
+    torch.cuda.synchronize()
+    assert np.array_equal(first["trace_best"].cpu().numpy()[:4], tb_whole[:4])
+    assert np.array_equal(tb.cpu().numpy()[:2], tb_whole[4:6]) and np.isnan(tb.cpu().numpy()[2:]).all()
+    assert (tn.cpu().numpy()[:2] > first["trace_ns"].cpu().numpy()[3]).all()
+    P.destroy()
+
+
+def test_two_handles_from_two_threads(api, oracle):
+    """include/gda.h only forbids sharing ONE handle: two handles driven from two host threads at the same time
+    (first-call kernel configuration included) give the results of the serial runs."""
+    import threading
+    ws = [wl.config(1), wl.config(4, B=128, n_scale=0.0625), wl.config(1), wl.config(4, B=256, n_scale=0.125)]
+    prms = [api.params_from_hyper(w.hyper, iters=120, eval_every=40) for w in ws]
+    x0s = [dev(wl.x0_uniform(w.problem.n, w.B, w.x0_seed)) for w in ws]
+    serial = []
+    for w, prm, x0 in zip(ws, prms, x0s):
+        P = api.create_from_workload(w.problem)
+        serial.append(P.run(x0, w.hyper.lambda0, prm)["obj"].cpu().numpy())
+        P.destroy()
+    results, errors = [None] * len(ws), []
+
+    def work(k):
+        try:
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                P = api.create_from_workload(ws[k].problem)
+                for _ in range(3):
+                    r = P.run(x0s[k], ws[k].hyper.lambda0, prms[k])
+                s.synchronize()
+                results[k] = r["obj"].cpu().numpy()
+                P.destroy()
+        except Exception as e:      # noqa: BLE001
+            errors.append(e)
+
+    torch.cuda.synchronize()
+    th = [threading.Thread(target=work, args=(k,)) for k in range(len(ws))]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    assert not errors, errors
+    for a, b in zip(results, serial):
+        assert np.array_equal(a, b)
 
 
 def test_run_host_matches_device_run(api):
