@@ -16,7 +16,8 @@
  *     restart index is contiguous.  B must be a positive multiple of 4 (128-bit vectors across restarts).
  *   - gda_run / gda_grad / gda_score enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream) and return without synchronising; outputs are valid once the stream has
- *     reached that point.  A handle must not be used from two streams or threads at the same time.
+ *     reached that point.  A handle must not be used from two streams or threads at the same time; different
+ *     handles may be used from different host threads concurrently.
  *   - All compute runs in CUDA kernels for sm_100a; there is no CPU fallback: without a usable device
  *     every compute entry point fails with GDA_ERR_CUDA.
  */
@@ -89,7 +90,8 @@ gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cptr, const in
 gda_status gda_create_maxkcut(int32_t n, int32_t k, const int32_t* rowptr, const int32_t* col, const float* val,
                               gda_problem** out);
 
-void gda_destroy(gda_problem* p); /* NULL-safe; synchronises the device before freeing */
+void gda_destroy(gda_problem* p); /* NULL-safe; waits for the work this handle has enqueued, then frees.  (It does not
+                                     call cudaDeviceSynchronize: other handles may be capturing on other threads.) */
 
 /* ---- the run ----------------------------------------------------------------------------------------- */
 /* Dual variables.  GDA_DUAL_PER_VARIABLE is the paper's method, one multiplier y_i per constraint g(x_i) = 0

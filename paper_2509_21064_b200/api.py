@@ -12,7 +12,10 @@ from typing import Optional
 
 import numpy as np
 
-_LIB_PATH = Path(__file__).resolve().parent / "lib" / "libgda_b200.so"
+import os
+
+# GDA_B200_LIB points at another build of the same library (e.g. one compiled with different tuning macros)
+_LIB_PATH = Path(os.environ.get("GDA_B200_LIB") or Path(__file__).resolve().parent / "lib" / "libgda_b200.so")
 _lib = None
 
 STATUS = {0: "GDA_OK", 1: "GDA_ERR_INVALID_ARG", 2: "GDA_ERR_ALLOC", 3: "GDA_ERR_CUDA", 4: "GDA_ERR_UNSUPPORTED"}

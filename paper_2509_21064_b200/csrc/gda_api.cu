@@ -152,6 +152,7 @@ extern "C" gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, cons
     p->kind = GDA_KIND_SPARSE; p->n = n; p->nnz = (int64_t)h_col.size(); p->integral = integral ? 1 : 0;
     p->max_deg = max_deg;
     gda_status st = device_setup(p);
+    if (st == GDA_OK) st = sparse_configure(p);
     if (st == GDA_OK) st = upload(&p->d_rowptr, h_rowptr);
     if (st == GDA_OK) st = upload(&p->d_col, h_col);
     if (st == GDA_OK) st = upload(&p->d_val2, h_val2);
@@ -315,6 +316,21 @@ extern "C" gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cpt
 // ---------------------------------------------------------------------------------------------------
 // workspace / destroy
 // ---------------------------------------------------------------------------------------------------
+// Wait for the work this handle has enqueued.  NOT cudaDeviceSynchronize: that call is refused -- and invalidates the
+// capture -- while ANY stream of the device is capturing, e.g. another handle's first run on another host thread.
+static void wait_for_handle(gda_problem* p) {
+    if (p->ev_last) cudaEventSynchronize(p->ev_last);
+    if (p->own_stream) cudaStreamSynchronize(p->own_stream);
+    cudaGetLastError();
+}
+
+// records "everything this handle has enqueued so far" (on the caller's stream, after the join)
+static gda_status mark_enqueued(gda_problem* p, cudaStream_t user) {
+    if (!p->ev_last) GDA_CUDA_TRY(cudaEventCreateWithFlags(&p->ev_last, cudaEventDisableTiming));
+    GDA_CUDA_TRY(cudaEventRecord(p->ev_last, user));
+    return GDA_OK;
+}
+
 static void drop_graphs(gda_problem* p) {
     for (auto& g : p->graphs) {
         if (g.exec) cudaGraphExecDestroy(g.exec);
@@ -337,7 +353,7 @@ static void free_workspace(gda_problem* p) {
 extern "C" void gda_destroy(gda_problem* p) {
     if (!p) return;
     DeviceGuard guard(p->device);
-    cudaDeviceSynchronize();
+    wait_for_handle(p);
     free_workspace(p);
     cudaFree(p->d_rowptr); cudaFree(p->d_col); cudaFree(p->d_val2); cudaFree(p->d_cprime);
     cudaFree(p->d_heavy_rows); cudaFree(p->d_light_rows); cudaFree(p->d_ell);
@@ -346,6 +362,7 @@ extern "C" void gda_destroy(gda_problem* p) {
     if (p->own_stream) cudaStreamDestroy(p->own_stream);
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);
+    if (p->ev_last) cudaEventDestroy(p->ev_last);
     cudaGetLastError();
     delete p;
 }
@@ -375,7 +392,7 @@ static const int32_t TRACE_CAP = 4096;
 static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     Workspace& ws = p->ws;
     if (ws.B == B) return GDA_OK;
-    GDA_CUDA_TRY(cudaDeviceSynchronize());
+    wait_for_handle(p);
     free_workspace(p);
     const size_t elems = (size_t)p->n * B;
     const size_t xelems = p->kind == GDA_KIND_KCUT ? elems * p->kparts : elems;   // Max-k-Cut: k planes
@@ -432,10 +449,11 @@ static gda_status pick_stream(gda_problem* p, void* stream, cudaStream_t* user, 
 }
 
 static gda_status join_stream(gda_problem* p, cudaStream_t user, cudaStream_t exec) {
-    if (user == exec) return GDA_OK;
-    GDA_CUDA_TRY(cudaEventRecord(p->ev_join, exec));
-    GDA_CUDA_TRY(cudaStreamWaitEvent(user, p->ev_join, 0));
-    return GDA_OK;
+    if (user != exec) {
+        GDA_CUDA_TRY(cudaEventRecord(p->ev_join, exec));
+        GDA_CUDA_TRY(cudaStreamWaitEvent(user, p->ev_join, 0));
+    }
+    return mark_enqueued(p, user);
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -25,20 +25,30 @@
 //    issues the MMAs; both CTAs' TMA loads signal the leader's full barrier; tcgen05.commit multicasts "slot free" and
 //    "accumulator ready"; the peer's epilogue warps release the accumulator on the leader's barrier through the
 //    cluster address space.  Each CTA keeps its 128 rows of the accumulator in its own TMEM: same epilogue.
-//  * TWO PAIRS PER CLUSTER (NP = 2, cluster of 4) that work on the same 256 restarts and adjacent blocks of 256
+//  * TWO PAIRS PER CLUSTER (PM = 1, PN = 2, cluster of 4) that work on the same 256 restarts and adjacent blocks of 256
 //    variables: each CTA loads half of its A rows and TMA-multicasts them to its counterpart in the other pair
 //    (24 KB per CTA and k-block).  A slot is reused when BOTH pairs have retired it (empty barrier count 2, every
 //    leader's commit goes to all four CTAs).
-// B an odd multiple of 128 runs single CTAs (CG = 1); n not a multiple of 512 runs pairs without the multicast.
+//  * FOUR PAIRS PER CLUSTER (PM = PN = 2, cluster of 8): pairs (pm, pn) on restart block pm and variable block pn.  The
+//    A rows of a CTA are shared along pn and its half of the Q tile along pm; every CTA loads one 64-row box of each
+//    and multicasts it to its partner (16 KB of L2 reads per CTA and k-block).  The step is bound by what the L2 can
+//    deliver while 128 SMs stream operands, so every byte not read twice shortens it.
+// B an odd multiple of 128 runs single CTAs (CG = 1); n not a multiple of 512 runs pairs without the multicast; B not a
+// multiple of 512 runs clusters of two pairs.
 //
-// Tile schedule: work units of (CG x 128 restarts) x (NP x 256 variables) are dealt round-robin to the clusters.
+// Tile schedule: work units of (PM x CG x 128 restarts) x (PN x 256 variables) are dealt round-robin to the clusters.
 // A 128-variable "half" unit does NOT help the tail: measured, an N = 128 MMA takes as long as an N = 256 one (the
 // A-operand path of M = 128 rows per SM sets the instruction time), so units always span 256 variables per pair.
 #include "gda_internal.cuh"
 
 #include <cuda.h>
 #include <cmath>
+#include <cstdlib>
 #include <vector>
+
+#ifndef GDA_DENSE_STAGES
+#define GDA_DENSE_STAGES 6      // pipeline stages of the pair variants (32 KB each)
+#endif
 
 namespace {
 
@@ -49,7 +59,7 @@ constexpr int TMEM_COLS = 512;
 // per CTA and pipeline stage: its 128 rows of A and its 256 / CG rows of Q; 4 stages of 48 KB or 6 stages of 32 KB
 template <int CG> struct Pipe {
     static constexpr int STAGE_BYTES = A_BYTES + (BN / CG) * BK * 2;
-    static constexpr int STAGES = CG == 1 ? 4 : 6;
+    static constexpr int STAGES = CG == 1 ? 4 : GDA_DENSE_STAGES;
     static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024;     // tiles + barriers + alignment slack
 };
 
@@ -192,18 +202,19 @@ struct DenseArgs {
 };
 
 // Work unit u of the schedule described at the top: restarts [m0, m0 + 128) of THIS CTA, variables [n0, n0 + 256)
-// of its pair.  rank = rank in the cluster; pair = rank / CG, r = rank % CG.
+// of its pair.  rank = rank in the cluster = ((pm * PN) + pn) * CG + r.
 struct Unit { int m0, n0; };
-__device__ __forceinline__ Unit get_unit(int u, int B, int cg, int np, int rank) {
-    const int num_msup = B / (BM * cg);
+__device__ __forceinline__ Unit get_unit(int u, int B, int cg, int pm_n, int pn_n, int rank) {
+    const int num_msup = B / (BM * cg * pm_n);
+    const int pair = rank / cg, r = rank % cg;
     Unit t;
-    t.m0 = ((u % num_msup) * cg + rank % cg) * BM;
-    t.n0 = ((u / num_msup) * np + rank / cg) * BN;
+    t.m0 = (((u % num_msup) * pm_n + pair / pn_n) * cg + r) * BM;
+    t.n0 = ((u / num_msup) * pn_n + pair % pn_n) * BN;
     return t;
 }
-__device__ __forceinline__ int num_units(int n, int B, int cg, int np) { return (B / (BM * cg)) * (n / (BN * np)); }
+__device__ __forceinline__ int num_units(int n, int B, int cg, int pm_n, int pn_n) { return (B / (BM * cg * pm_n)) * (n / (BN * pn_n)); }
 
-template <int MODE, int GFUN, int CG, int NP>
+template <int MODE, int GFUN, int CG, int PM, int PN>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                   const DenseArgs args) {
@@ -221,12 +232,13 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
         reinterpret_cast<volatile uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int NP = PM * PN;                                                  // pairs per cluster
     constexpr int CSIZE = CG * NP;                                               // CTAs per cluster
     const int rank = CSIZE > 1 ? (int)cluster_ctarank() : 0;
     const int lead = rank & ~(CG - 1);                                           // rank of this CTA's pair leader
     const bool leader = rank == lead;
     const int cluster_id = blockIdx.x / CSIZE, num_clusters = gridDim.x / CSIZE;
-    const int units = num_units(args.n, args.B, CG, NP);
+    const int units = num_units(args.n, args.B, CG, PM, PN);
     const int num_kb = args.n / BK;
 
     if (warp == 0 && lane == 0) {
@@ -259,7 +271,7 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
             constexpr int SLICE = BN / CG;                                        // rows of Q this CTA stages
             constexpr uint32_t BYTES = (uint32_t)(CG * (A_BYTES + SLICE * BK * 2)); // a pair's loads land on its leader's barrier
             for (int u = cluster_id; u < units; u += num_clusters) {
-                const Unit t = get_unit(u, args.B, CG, NP, rank);
+                const Unit t = get_unit(u, args.B, CG, PM, PN, rank);
                 for (int kb = 0; kb < num_kb; ++kb) {
                     mbar_wait(empty_bar(stage), phase ^ 1u);                      // every MMA that read this slot has retired
                     const uint32_t a_dst = smem_base + stage * STAGE_BYTES;
@@ -272,18 +284,31 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
                     } else {
                         if (leader) mbar_expect_tx(full_bar(stage), BYTES);
                         const uint32_t lead_bar = map_to_cta(full_bar(stage), (uint32_t)lead);
-                        if (NP == 1) {
+                        const int pm = (rank / CG) / PN, pn = (rank / CG) % PN, r2 = rank % CG;
+                        if (PN == 1) {
                             for (int r = 0; r < BM; r += BBOX)
                                 tma_load_2d_pair(a_dst + (uint32_t)r * 128u, &tmap_a, lead_bar, kb * BK, t.m0 + r);
-                        } else {                                                  // my half of the A rows, to both pairs
-                            static_assert(BM / 2 == BBOX, "one box per half of the A rows");
-                            const int half_rows = (rank / CG) * (BM / 2);
-                            const uint16_t mask = (uint16_t)((1u << (rank % CG)) | (1u << (rank % CG + CG)));
-                            tma_load_2d_pair_mc(a_dst + (uint32_t)half_rows * 128u, &tmap_a, lead_bar, kb * BK, t.m0 + half_rows, mask);
+                        } else {                                                  // my share of the A rows, to the pairs along pn
+                            static_assert(PN == 1 || BM / PN == BBOX, "one box per share of the A rows");
+                            const int share = pn * (BM / PN);
+                            uint16_t mask = 0;
+#pragma unroll
+                            for (int q = 0; q < PN; ++q) mask |= (uint16_t)(1u << ((pm * PN + q) * CG + r2));
+                            tma_load_2d_pair_mc(a_dst + (uint32_t)share * 128u, &tmap_a, lead_bar, kb * BK, t.m0 + share, mask);
                         }
-                        for (int r = 0; r < SLICE; r += BBOX)
-                            tma_load_2d_pair(a_dst + A_BYTES + (uint32_t)r * 128u, &tmap_b, lead_bar, kb * BK,
-                                             t.n0 + (rank % CG) * SLICE + r);
+                        if (PM == 1) {
+                            for (int r = 0; r < SLICE; r += BBOX)
+                                tma_load_2d_pair(a_dst + A_BYTES + (uint32_t)r * 128u, &tmap_b, lead_bar, kb * BK,
+                                                 t.n0 + r2 * SLICE + r);
+                        } else {                                                  // my share of this CTA's half of the Q tile, to the pairs along pm
+                            static_assert(PM == 1 || SLICE / PM == BBOX, "one box per share of the Q rows");
+                            const int share = pm * (SLICE / PM);
+                            uint16_t mask = 0;
+#pragma unroll
+                            for (int q = 0; q < PM; ++q) mask |= (uint16_t)(1u << ((q * PN + pn) * CG + r2));
+                            tma_load_2d_pair_mc(a_dst + A_BYTES + (uint32_t)share * 128u, &tmap_b, lead_bar, kb * BK,
+                                                t.n0 + r2 * SLICE + share, mask);
+                        }
                     }
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
@@ -302,8 +327,13 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
             constexpr uint16_t ALL = (uint16_t)((1u << CSIZE) - 1u);
             const uint16_t mine = (uint16_t)(((1u << CG) - 1u) << lead);
             for (int u = cluster_id; u < units; u += num_clusters, ++it) {
+#ifdef GDA_DENSE_SERIAL
+                const int as = 0;
+                const uint32_t aphase = (uint32_t)it & 1u;
+#else
                 const int as = it & 1;
                 const uint32_t aphase = (uint32_t)(it >> 1) & 1u;
+#endif
                 mbar_wait(tempty_bar(as), aphase ^ 1u);                           // every epilogue warp has drained this accumulator
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
@@ -331,9 +361,14 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
         const uint32_t tstep = (args.st ? args.st->t : 0u) + args.t_off;
         int it = 0;
         for (int u = cluster_id; u < units; u += num_clusters, ++it) {
-            const Unit t = get_unit(u, args.B, CG, NP, rank);
+            const Unit t = get_unit(u, args.B, CG, PM, PN, rank);
+#ifdef GDA_DENSE_SERIAL
+            const int as = 0;
+            const uint32_t aphase = (uint32_t)it & 1u;
+#else
             const int as = it & 1;
             const uint32_t aphase = (uint32_t)(it >> 1) & 1u;
+#endif
             const int b = t.m0 + lane_grp * 32 + lane;                            // restart owned by this thread
             constexpr int hcols = BN / 2;                                         // 128 columns per warpgroup
             mbar_wait(tfull_bar(as), aphase);
@@ -511,33 +546,70 @@ struct DenseHost {
     CUtensorMap tmap_z[2];
     const void* z_ptr[2] = {nullptr, nullptr};
     int32_t z_B = 0;
-    // co-resident clusters per kernel variant (1 CTA per SM), found -- together with the shared-memory opt-in -- on this
-    // handle's first launch of the variant: per handle, hence per device, and no process-wide state
-    int max_clusters[4 * 2 * 3] = {};
+    // co-resident clusters per kernel variant (1 CTA per SM), see configure_variant
+    int max_clusters[4 * 2 * 4] = {};
+    int forced_shape = -1;              // GDA_DENSE_SHAPE (read at create)
 };
 
-template <int MODE, int GFUN, int CG, int NP>
+// The launch shapes: single CTAs, pairs, two pairs (1 x 2) and four pairs (2 x 2) per cluster.
+constexpr int NUM_SHAPES = 4;
+constexpr int shape_index(int cg, int pm, int pn) { return cg == 1 ? 0 : pm * pn == 1 ? 1 : pm == 1 ? 2 : 3; }
+
+// One-time setup of a kernel variant on the handle's device: the shared-memory opt-in and the number of co-resident
+// clusters (1 CTA per SM).  Done for every variant at create (dense_prepare) -- not lazily at the first launch, which
+// is inside a stream capture -- and kept in the handle: per device, no process-wide state.
+template <int MODE, int GFUN, int CG, int PM, int PN>
+gda_status configure_variant(gda_problem* p) {
+    auto kern = dense_gemm_kernel<MODE, GFUN, CG, PM, PN>;
+    constexpr int CSIZE = CG * PM * PN;
+    GDA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Pipe<CG>::SMEM_BYTES));
+    int max_clusters = p->num_sms / CSIZE;
+    if (CSIZE > 2) {                                          // clusters of 4 or 8 do not pack all 148 SMs
+        cudaLaunchConfig_t cfg = {};
+        cfg.blockDim = dim3(NUM_THREADS); cfg.dynamicSmemBytes = Pipe<CG>::SMEM_BYTES;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = CSIZE; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        cfg.gridDim = dim3((unsigned)(max_clusters * CSIZE));
+        int q = 0;
+        GDA_CUDA_TRY(cudaOccupancyMaxActiveClusters(&q, kern, &cfg));
+        if (q > 0 && q < max_clusters) max_clusters = q;
+    }
+    static_cast<DenseHost*>(p->tmap_Q)->max_clusters[(MODE * 2 + GFUN) * NUM_SHAPES + shape_index(CG, PM, PN)] = max_clusters;
+    return GDA_OK;
+}
+
+template <int MODE, int GFUN>
+gda_status configure_shapes(gda_problem* p) {
+    GDA_TRY((configure_variant<MODE, GFUN, 1, 1, 1>(p)));
+    GDA_TRY((configure_variant<MODE, GFUN, 2, 1, 1>(p)));
+    GDA_TRY((configure_variant<MODE, GFUN, 2, 1, 2>(p)));
+    return configure_variant<MODE, GFUN, 2, 2, 2>(p);
+}
+
+gda_status configure_all(gda_problem* p) {
+    GDA_TRY((configure_shapes<MODE_STEP, GDA_G_QUADRATIC>(p)));
+    GDA_TRY((configure_shapes<MODE_STEP, GDA_G_ENTROPY>(p)));
+    GDA_TRY((configure_shapes<MODE_STEP_S, GDA_G_QUADRATIC>(p)));
+    GDA_TRY((configure_shapes<MODE_STEP_S, GDA_G_ENTROPY>(p)));
+    GDA_TRY((configure_shapes<MODE_GRAD, GDA_G_QUADRATIC>(p)));
+    return configure_shapes<MODE_SCORE, GDA_G_QUADRATIC>(p);
+}
+
+template <int MODE, int GFUN, int CG, int PM, int PN>
 gda_status launch_variant(gda_problem* p, const CUtensorMap& ta, const CUtensorMap& tq, const DenseArgs& a, cudaStream_t s) {
-    auto kern = dense_gemm_kernel<MODE, GFUN, CG, NP>;
-    constexpr int CSIZE = CG * NP;
-    int& max_clusters = static_cast<DenseHost*>(p->tmap_Q)->max_clusters[(MODE * 2 + GFUN) * 3 + (CG - 1) + (NP - 1)];
+    auto kern = dense_gemm_kernel<MODE, GFUN, CG, PM, PN>;
+    constexpr int CSIZE = CG * PM * PN;
+    const int max_clusters = static_cast<DenseHost*>(p->tmap_Q)->max_clusters[(MODE * 2 + GFUN) * NUM_SHAPES + shape_index(CG, PM, PN)];
+    if (max_clusters <= 0) { gda_set_error("dense path: kernel variant was not configured at create"); return GDA_ERR_CUDA; }
     cudaLaunchConfig_t cfg = {};
     cfg.blockDim = dim3(NUM_THREADS); cfg.dynamicSmemBytes = Pipe<CG>::SMEM_BYTES; cfg.stream = s;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = CSIZE; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (max_clusters == 0) {
-        GDA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Pipe<CG>::SMEM_BYTES));
-        max_clusters = p->num_sms / CSIZE;
-        if (CSIZE > 2) {                                      // clusters of 4 do not pack all 148 SMs
-            cfg.gridDim = dim3((unsigned)(max_clusters * CSIZE));
-            int q = 0;
-            GDA_CUDA_TRY(cudaOccupancyMaxActiveClusters(&q, kern, &cfg));
-            if (q > 0 && q < max_clusters) max_clusters = q;
-        }
-    }
-    const int units = (a.B / (BM * CG)) * (a.n / (BN * NP));
+    const int units = (a.B / (BM * CG * PM)) * (a.n / (BN * PN));
     const int rounds = (units + max_clusters - 1) / max_clusters;
     const int clusters = (units + rounds - 1) / rounds;       // fewest clusters that still finish in `rounds` rounds
     cfg.gridDim = dim3((unsigned)(clusters * CSIZE));
@@ -545,12 +617,27 @@ gda_status launch_variant(gda_problem* p, const CUtensorMap& ta, const CUtensorM
     return GDA_OK;
 }
 
+// GDA_DENSE_SHAPE=0..3 forces a launch shape the sizes allow (tests, A/B timing); default: the largest cluster that fits
 template <int MODE, int GFUN>
 gda_status launch_gemm(gda_problem* p, const CUtensorMap& ta, const DenseArgs& a, cudaStream_t s) {
     DenseHost* h = static_cast<DenseHost*>(p->tmap_Q);
-    if (a.B % (BM * 2) != 0) return launch_variant<MODE, GFUN, 1, 1>(p, ta, h->tmap_q, a, s);   // odd number of 128-restart blocks
-    if (a.n % (BN * 2) != 0) return launch_variant<MODE, GFUN, 2, 1>(p, ta, h->tmap_q, a, s);
-    return launch_variant<MODE, GFUN, 2, 2>(p, ta, h->tmap_q, a, s);
+    int shape = a.B % (BM * 2) != 0 ? 0 : a.n % (BN * 2) != 0 ? 1 : a.B % (BM * 4) != 0 ? 2 : 3;
+    if (shape == 3 && h->forced_shape < 0) {
+        // Clusters of 8 move a third less operand data per tile (measured on config 4: 30 us per round against 34 us)
+        // but only 15 of them are co-resident on a B200 (120 SMs) against 33 clusters of 4: take them only when the
+        // round count does not eat the gain (config 4: 64 units -> 5 rounds x 30 us against 4 x 34 us: clusters of 4).
+        const int* mc = h->max_clusters + (MODE * 2 + GFUN) * NUM_SHAPES;
+        const long units8 = (long)(a.B / (BM * 4)) * (a.n / (BN * 2)), units4 = (long)(a.B / (BM * 2)) * (a.n / (BN * 2));
+        const long rounds8 = (units8 + mc[3] - 1) / mc[3], rounds4 = (units4 + mc[2] - 1) / mc[2];
+        if (15 * rounds8 >= 17 * rounds4) shape = 2;
+    }
+    if (h->forced_shape >= 0 && h->forced_shape < shape) shape = h->forced_shape;
+    switch (shape) {
+        case 0: return launch_variant<MODE, GFUN, 1, 1, 1>(p, ta, h->tmap_q, a, s);
+        case 1: return launch_variant<MODE, GFUN, 2, 1, 1>(p, ta, h->tmap_q, a, s);
+        case 2: return launch_variant<MODE, GFUN, 2, 1, 2>(p, ta, h->tmap_q, a, s);
+        default: return launch_variant<MODE, GFUN, 2, 2, 2>(p, ta, h->tmap_q, a, s);
+    }
 }
 
 gda_status z_maps(gda_problem* p, int32_t B, const __nv_bfloat16* zt, const CUtensorMap** out) {
@@ -590,6 +677,8 @@ gda_status dense_prepare(gda_problem* p, const float* Q, const float* c) {
     GDA_CUDA_TRY(cudaMemcpy(p->d_cprime, cp.data(), n * sizeof(float), cudaMemcpyHostToDevice));
     DenseHost* h = new DenseHost();
     p->tmap_Q = h;
+    if (const char* e = getenv("GDA_DENSE_SHAPE")) if (e[0] >= '0' && e[0] <= '3') h->forced_shape = e[0] - '0';
+    GDA_TRY(configure_all(p));
     return make_tmap(&h->tmap_q, p->d_Qbf, (uint64_t)n, (uint64_t)n, BBOX);
 }
 

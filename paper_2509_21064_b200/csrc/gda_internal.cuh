@@ -113,7 +113,6 @@ struct gda_problem {
     int32_t* d_heavy_rows = nullptr; int32_t n_heavy = 0;   // rows handled by the row-split kernel
     int32_t* d_light_rows = nullptr; int32_t n_light = 0;   // nullptr = all rows, in order
     int32_t max_deg = 0;
-    bool resident_configured = false;    // shared-memory opt-in of the resident kernels done on this handle's device
     int32_t* d_ell = nullptr;            // [n][16] packed low-degree rows: 8 cols + 8 val2 (see gda_sparse.cu); nullptr = not built
     // dense QUBO: Q_off in bf16 [n][n] (zero diagonal), r0 = Q_off 1 (row sums) for the centred operand
     __nv_bfloat16* d_Qbf = nullptr; float* d_rowsum = nullptr;
@@ -124,6 +123,7 @@ struct gda_problem {
     Workspace ws;
     cudaStream_t own_stream = nullptr;   // used when the caller passes the legacy default stream (not capturable)
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaEvent_t ev_last = nullptr;       // recorded after everything an entry point enqueued (what destroy / reallocation wait for)
     std::vector<CachedGraph> graphs;
     int64_t last_launches = 0, last_step_launches = 0;
 };
@@ -136,6 +136,7 @@ struct gda_problem {
 gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
 int32_t sparse_num_gparts(const gda_problem* p);
+gda_status sparse_configure(gda_problem* p);                       // at create
 gda_status sparse_steps_resident(gda_problem* p, int32_t B, int32_t len, const float* x_in, float* y, float* x_out,
                                  const UpdParams& up, const RunState* st, cudaStream_t s, int64_t* launches, int* done);
 gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);

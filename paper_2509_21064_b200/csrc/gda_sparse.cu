@@ -428,6 +428,13 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
 
 int sparse_heavy_threshold() { return HEAVY_DEG; }
 
+// shared-memory opt-in of the resident kernels on the handle's device; called at create (never inside a capture)
+gda_status sparse_configure(gda_problem*) {
+    GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_QUADRATIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));
+    GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_ENTROPY>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));
+    return GDA_OK;
+}
+
 gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
     if (sd.mu) return launch_step<0, true>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
@@ -486,12 +493,6 @@ gda_status sparse_steps_resident(gda_problem* p, int32_t B, int32_t len, const f
     const long long total = (long long)p->n * B;
     const size_t smem = ((size_t)total * 3 + (size_t)p->n * 2 + 1 + (size_t)p->nnz * 2) * sizeof(float);   // x, x, y, c', rowptr, col, val
     if (total > RESIDENT_MAX || len <= 0 || smem > (size_t)RESIDENT_SMEM) return GDA_OK;
-    bool& configured = p->resident_configured;               // per handle (hence per device), not per process
-    if (!configured) {
-        GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_QUADRATIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));
-        GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_ENTROPY>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));
-        configured = true;
-    }
     if (up.gfun == GDA_G_QUADRATIC)
         spmm_steps_resident<GDA_G_QUADRATIC><<<1, RESIDENT_THREADS, smem, s>>>(p->n, B, (int)p->nnz, len, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x_in, y, x_out, up, st);
     else

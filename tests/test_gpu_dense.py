@@ -1,6 +1,6 @@
 """GPU parity of the DENSE path (tcgen05 GEMM gradient + fused update, config 4) against the CPU oracle, on every
-launch variant the library has: single CTAs (CG=1), CTA pairs (CG=2, NP=1) and clusters of two pairs with the A
-multicast (CG=2, NP=2) -- the variant config 4 runs.
+launch variant the library has: single CTAs (CG=1), CTA pairs (CG=2), clusters of two pairs with the A multicast and
+clusters of four pairs (2 x 2) with the A and Q multicast -- the variant config 4 runs.
 
 north_star requirements, as for every config: (b) teacher-forced single steps (gradient within 1e-2 on the bf16
 path), here with the DEFAULT delta so that the perturbation branch of the epilogue is compared too; (c) free-running
@@ -52,12 +52,26 @@ def variants():
     return [("single_cta", wl.config(4, B=128, n_scale=0.0625)),          # n=256,  B=128 : CG=1
             ("single_cta_3x", wl.config(4, B=384, n_scale=0.125)),        # n=512,  B=384 : CG=1, three restart blocks
             ("pair", wl.config(4, B=256, n_scale=0.1875)),                # n=768,  B=256 : CG=2, NP=1
-            ("cluster", wl.config(4, B=256, n_scale=0.25)),               # n=1024, B=256 : CG=2, NP=2
-            ("cluster_4units", wl.config(4, B=1024, n_scale=0.625))]      # n=2560, B=1024: CG=2, NP=2, several units per cluster
+            ("cluster", wl.config(4, B=256, n_scale=0.25)),               # n=1024, B=256 : CG=2, 1 x 2 pairs (cluster of 4), A multicast
+            ("cluster8", wl.config(4, B=512, n_scale=0.25)),              # n=1024, B=512 : CG=2, 2 x 2 pairs (cluster of 8), A and Q multicast
+            ("cluster8_10", wl.config(4, B=1024, n_scale=0.625)),         # n=2560, B=1024: ten clusters of 8
+            ("cluster8_units", wl.config(4, B=2048, n_scale=0.5))]        # n=2048, B=2048: clusters of 8 with two units each (forced:
+                                                                          # the library would pick clusters of 4 for this size)
 
 
 VARIANTS = variants()
 IDS = [v[0] for v in VARIANTS]
+
+
+def create(api, name, problem):
+    """gda_create_qubo_dense; GDA_DENSE_SHAPE (read at create) forces the cluster-of-8 launch shape where asked."""
+    import os
+    if name == "cluster8_units":
+        os.environ["GDA_DENSE_SHAPE"] = "3"
+    try:
+        return api.create_from_workload(problem)
+    finally:
+        os.environ.pop("GDA_DENSE_SHAPE", None)
 
 
 def sample_columns(B, k=24):
@@ -106,7 +120,7 @@ def test_dense_teacher_forced_steps_default_delta(api, oracle, name, w):
     """(b) on every variant, with the perturbation ON.  Gradient: within the north star's 1e-2 AND within 8 standard
     deviations of the bf16 rounding model; x+: alpha times that; y+: 1e-5 (no GEMM in the dual step)."""
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create(api, name, w.problem)
     n, B, h = w.problem.n, w.B, w.hyper
     cols = sample_columns(B)
     ci = torch.from_numpy(cols).long().cuda()
@@ -125,15 +139,18 @@ def test_dense_teacher_forced_steps_default_delta(api, oracle, name, w):
         sig = grad_sigma(w.problem, xp)
         assert (np.abs(G - Gref) <= TOL_GRAD_BF16 * gmax).all()                                  # north star (b), bf16 path
         assert (np.abs(G - Gref) <= 8.0 * sig + TOL_STEP * gmax).all(), float((np.abs(G - Gref) / (8.0 * sig + TOL_STEP * gmax)).max())
-        r1 = P.run(x, lam, api.params_from_hyper(h, iters=1, eval_every=1, t0=t), want_final=True)
-        xg, yg = r1["x"][:, ci].cpu().numpy().astype(np.float64), r1["lam"][:, ci].cpu().numpy().astype(np.float64)
         tol_x = f32(h.alpha) * (8.0 * sig + TOL_STEP * gmax) + TOL_STEP
-        ref, amb = assert_dense_step_close(xg, xp, lp, cols, OP, oracle, okw(h, iters=1, eval_every=1, t0=t), tol_x)
-        assert (np.abs(yg - ref["y"]) / np.maximum(1.0, np.abs(ref["y"]))).max() <= TOL_STEP, (name, t)
-        in_band = np.abs(xp.astype(np.float64) - 0.5) < f32(h.delta)
-        perturbed_seen += int((in_band & (np.abs(np.abs(ref["x"] - 0.5) - f32(h.delta)) < 1e-6)).sum())
-        assert amb < 0.25, (name, t, amb)
-    assert perturbed_seen > 0, "no perturbed entry was compared: the states do not reach the band"
+        # the default delta = 1e-4, and a wide band (2e-2) that catches about a tenth of the entries once the iterates
+        # have settled (the fixed point of the convex start sits near, not at, 1/2 when the linear term is non-zero)
+        for delta in (h.delta, 2e-2):
+            r1 = P.run(x, lam, api.params_from_hyper(h, iters=1, eval_every=1, t0=t, delta=delta), want_final=True)
+            xg, yg = r1["x"][:, ci].cpu().numpy().astype(np.float64), r1["lam"][:, ci].cpu().numpy().astype(np.float64)
+            ref, amb = assert_dense_step_close(xg, xp, lp, cols, OP, oracle, okw(h, iters=1, eval_every=1, t0=t, delta=delta), tol_x)
+            assert (np.abs(yg - ref["y"]) / np.maximum(1.0, np.abs(ref["y"]))).max() <= TOL_STEP, (name, t)
+            in_band = np.abs(xp.astype(np.float64) - 0.5) < f32(delta)
+            perturbed_seen += int((in_band & (np.abs(np.abs(ref["x"] - 0.5) - f32(delta)) < 1e-6)).sum())
+            assert amb < 0.05, (name, t, amb)
+    assert perturbed_seen > 100, "too few perturbed entries were compared: the states do not reach the band"
     P.destroy()
 
 
@@ -142,7 +159,7 @@ def test_dense_teacher_forced_steps_default_delta(api, oracle, name, w):
 def test_dense_free_running_50_steps(api, oracle, name, w, delta):
     """(c): 50 free-running steps from x0, max |x - x_ref| <= 1e-3 against the fp64 oracle on sampled columns."""
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create(api, name, w.problem)
     n, B, h = w.problem.n, w.B, w.hyper
     cols = sample_columns(B)
     ci = torch.from_numpy(cols).long().cuda()
@@ -152,7 +169,9 @@ def test_dense_free_running_50_steps(api, oracle, name, w, delta):
     ex = np.abs(r["x"][:, ci].cpu().numpy() - ref["x"])
     ey = np.abs(r["lam"][:, ci].cpu().numpy() - ref["y"])
     print(f"dense free-running 50 steps [{name}, delta={delta}]: max|dx| = {ex.max():.3e}, max|dy| = {ey.max():.3e}")
-    assert ex.max() <= TOL_TRAJ and ey.max() <= TOL_TRAJ * max(1.0, h.lambda0 / 10)
+    assert ex.max() <= TOL_TRAJ
+    # y+ = y + beta g(x), |g'| <= 1: the dual inherits at most beta * |dx| per step, plus half an ulp of y (fp32) per addition
+    assert ey.max() <= 50 * (f32(h.beta) * TOL_TRAJ + 2.0 ** -24 * h.lambda0)
     # (a) on the way: the objective of the returned points, sampled columns, fp64 with the dense path's relative tolerance
     xb = r["x_bin"][:, ci].cpu().numpy()
     Fref = oracle.F_binary(OP, xb)
@@ -173,7 +192,7 @@ def integer_dense_qubo_with_zero_gradient_at_half(n, seed):
     return wl.QuboDense(n=n, Q=Q, c=c.astype(np.float32))
 
 
-@pytest.mark.parametrize("n,B", [(256, 128), (768, 256), (1024, 256), (1536, 512)], ids=["single_cta", "pair", "cluster", "cluster_2units"])
+@pytest.mark.parametrize("n,B", [(256, 128), (768, 256), (1024, 256), (1536, 512)], ids=["single_cta", "pair", "cluster", "cluster8_units"])
 def test_dense_tie_break_at_exact_half_matches_oracle(api, oracle, n, B):
     """x = 1/2 everywhere and a zero gradient: x~ = x = 1/2 exactly, so the side of the perturbation is the hash bit of
     (seed, t, i, b) for EVERY element (reading R3).  Bit-for-bit against the oracle's fp32 build."""
