@@ -162,13 +162,8 @@ def oracle_sample_columns(w: wl.Workload, cores: int) -> int:
     return max(1, min(w.B, cores if w.kind != "qubo_dense" else min(cores, 8)))
 
 
-def time_oracle(w: wl.Workload, budget_s: float):
-    """cpu_baseline: the oracle as it stands (fp64, OpenMP over restarts) on a bounded sample."""
-    from oracle import pdbo
-    pdbo.build()
-    cores = max(1, min(pdbo.max_threads(), os.cpu_count() or 1))
+def _time_oracle_once(w: wl.Workload, budget_s: float, cores: int, Bo: int):
     OP = oracle_problem(w.problem)
-    Bo = oracle_sample_columns(w, cores)
     X0 = start_point(w, w.x0_seed)[..., :Bo].copy()
     h = w.hyper
     lam = float(np.float32(h.lambda0)) if not getattr(h, "dual", 0) else np.full(Bo, np.float32(h.lambda0), dtype=np.float64)
@@ -187,8 +182,41 @@ def time_oracle(w: wl.Workload, budget_s: float):
     t0 = time.perf_counter()
     oracle_run(w, OP, X0, lam, iters, h.eval_every, cores)
     dt = time.perf_counter() - t0
-    return dict(value=Bo * iters / dt, unit="restart-iters/s", cores=cores, kind="oracle",
-                sample=f"{Bo} of {w.B} restarts x {iters} GDA iterations of {w.name}, fp64, gcc -O2 -fopenmp, {dt:.1f} s")
+    return Bo, iters, dt
+
+
+def time_oracle(w: wl.Workload, budget_s: float):
+    """cpu_baseline: the oracle as it stands (fp64, gcc -O2, OpenMP over restarts) on a bounded sample -- on all host
+    cores, and (`one_core`) single-threaded with the process pinned to one core."""
+    from oracle import pdbo
+    pdbo.build()
+    cores = max(1, min(pdbo.max_threads(), os.cpu_count() or 1))
+    Bo, iters, dt = _time_oracle_once(w, budget_s, cores, oracle_sample_columns(w, cores))
+    out = dict(value=Bo * iters / dt, unit="restart-iters/s", cores=cores, kind="oracle",
+               sample=f"{Bo} of {w.B} restarts x {iters} GDA iterations of {w.name}, fp64, gcc -O2 -fopenmp, {dt:.1f} s")
+    try:
+        allowed = os.sched_getaffinity(0)
+        os.sched_setaffinity(0, {min(allowed)})
+        try:
+            B1, it1, dt1 = _time_oracle_once(w, max(2.0, budget_s / 4), 1, 1)
+        finally:
+            os.sched_setaffinity(0, allowed)
+        out["one_core"] = dict(value=B1 * it1 / dt1, unit="restart-iters/s", cores=1, pinned_to_core=min(allowed),
+                               sample=f"{B1} restart(s) x {it1} GDA iterations, single thread, {dt1:.1f} s")
+    except (AttributeError, OSError) as e:            # no affinity control on this host
+        out["one_core"] = dict(unavailable=str(e))
+    return out
+
+
+def config_dict(args, w: wl.Workload):
+    """The `config` both arms print (identical keys and values: the driver compares them)."""
+    h = w.hyper
+    return {"workload": w.name, "baseline_config_index": args.config if not (args.mis or args.maxkcut) else None,
+            "kind": w.kind, "n": w.problem.n, "B_per_gpu": w.B,
+            "step": f"{h.eval_every} GDA iterations + 1 evaluation (one CUDA graph launch on the GPU arm)",
+            "hyper": {"lambda0": h.lambda0, "alpha": h.alpha, "beta": h.beta, "delta": h.delta, "gfun": h.gfun,
+                      "dual": "scalar (PDBO-s)" if getattr(h, "dual", 0) else "per-variable (PDBO)"},
+            "l2": "flushed between timed steps (256 MiB write, untimed)", "note": w.note}
 
 
 def run_reference(args, w: wl.Workload):
@@ -222,7 +250,7 @@ def run_reference(args, w: wl.Workload):
         "impl": "reference", "metric": "restart-iterations/s", "value": value, "unit": "restart-iters/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "n": w.problem.n, "B": w.B, "note": w.note},
+        "config": config_dict(args, w),
         "cpu_baseline": {"value": value, "unit": "restart-iters/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "restart-iters/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -231,6 +259,164 @@ def run_reference(args, w: wl.Workload):
 # ------------------------------------------------------------------------------------------------
 # our arm
 # ------------------------------------------------------------------------------------------------
+L2_BYTES = 126 * 1024 * 1024
+
+
+def state_bytes(w: wl.Workload) -> int:
+    """x double buffer + y (sparse / MaxSAT), x + y + two bf16 operands (dense), k planes for Max-k-Cut."""
+    n, B = w.problem.n, w.B
+    if w.kind == "qubo_dense":
+        return 12 * n * B
+    if w.kind == "maxkcut":
+        return (3 * w.problem.k + 1) * 4 * n * B
+    return 12 * n * B
+
+
+def ncu_record(w: wl.Workload) -> dict:
+    tf = ROOT / "profiles" / "ncu_traffic.json"
+    if not tf.exists():
+        return {}
+    d = json.loads(tf.read_text())
+    return d.get(f"{w.name}_B{w.B}", d.get(w.name, {}))
+
+
+def roofline_block(w: wl.Workload, peaks, t_step_mean, t_step_median, t_eval):
+    """roofline of the step kernel: algorithmic work per launch / its average duration, the duration being
+    (one captured chunk - one evaluation) / eval_every from CUDA events (it includes the graph's launch gaps)."""
+    work = algorithmic_work(w)
+    ipe = w.hyper.eval_every
+    t_kernel = max(t_step_mean - t_eval, 1e-9) / ipe
+    t_kernel_med = max(t_step_median - t_eval, 1e-9) / ipe
+    if work["bound"] == "hbm":
+        achieved, peak, unit = work["bytes"] / t_kernel / 1e9, peaks["hbm_gbs"], "GB/s"
+    else:
+        achieved, peak, unit = work["flops"] / t_kernel / 1e12, peaks["bf16_tflops_sustained"], "TFLOP/s"
+    rec = ncu_record(w)
+    resident = state_bytes(w) < L2_BYTES
+    if work["bound"] == "tensor":
+        basis = "algorithmic flops / step-kernel time, against the measured SUSTAINED cuBLAS bf16 peak (the kernel is timed inside a long step)"
+    elif resident:
+        basis = (f"ALGORITHMIC bytes (16 B per variable-restart + structure, each once) / step-kernel time against the measured HBM copy peak; "
+                 f"the state ({state_bytes(w) / 1e6:.1f} MB) is L2-RESIDENT on a B200 (126 MB L2), so this is not achieved HBM bandwidth: "
+                 f"warm DRAM traffic is ~0 and what bounds the kernel is L2 -> SM delivery (l2_to_sm_bytes)")
+    else:
+        basis = (f"algorithmic bytes / step-kernel time against the measured HBM copy peak; the state ({state_bytes(w) / 1e6:.1f} MB) exceeds "
+                 f"the 126 MB L2, so the step streams from HBM")
+    return {"bound": work["bound"], "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
+            "traffic": rec.get("bytes"), "l2_to_sm_bytes": rec.get("l2_to_sm_bytes"), "traffic_source": rec.get("source"),
+            "peak_source": peaks["source"], "kernel": rec.get("kernel", "step kernel (gradient + fused update)"),
+            "us_per_launch": t_kernel * 1e6, "us_per_launch_median": t_kernel_med * 1e6,
+            "frac_median": achieved / peak * t_kernel / t_kernel_med,
+            "algorithmic_bytes_per_launch": work["bytes"], "algorithmic_flops_per_launch": work["flops"],
+            "eval_us": t_eval * 1e6, "state_l2_resident": resident, "basis": basis}
+
+
+class Session:
+    """One device, one stream, the flush buffer; measures workloads one after the other."""
+
+    def __init__(self, local_rank, rank, world):
+        import torch
+        self.torch, self.rank, self.world, self.local_rank = torch, rank, world, local_rank
+        self.dev = torch.device("cuda", local_rank)
+        self.stream = torch.cuda.Stream(self.dev)
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=self.dev)
+
+    def sync_all(self):
+        import torch.distributed as dist
+        self.torch.cuda.synchronize(self.dev)
+        if self.world > 1:
+            dist.barrier()
+            self.torch.cuda.synchronize(self.dev)
+
+    def measure(self, w: wl.Workload, K: int, W: int, peaks, full: bool):
+        """K timed steps (flushed L2), the evaluation alone, clocks; with full=True also the whole run, the trace and
+        the end-to-end numbers through gda_run_host."""
+        torch = self.torch
+        from paper_2509_21064_b200 import api, multirank
+        h, B, n = w.hyper, w.B, w.problem.n
+        P = api.create_from_workload(w.problem)
+        x0_host = torch.from_numpy(start_point(w, multirank.rank_x0_seed(w.x0_seed, self.rank))).pin_memory()
+        x0 = x0_host.to(self.dev, non_blocking=True)
+        stream, flush = self.stream, self.flush
+        prm_step = api.params_from_hyper(h, iters=h.eval_every)
+        prm0 = api.params_from_hyper(h, iters=0)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        res = {}
+        with torch.cuda.stream(stream):
+            out = P.run(x0, h.lambda0, prm_step)                          # warm-up: captures the graph, warms clocks
+            for _ in range(W - 1):
+                P.resume(prm_step, out)
+            self.sync_all()
+            sampler = ClockSampler(self.local_rank)
+            sampler.start()
+            out = P.run(x0, h.lambda0, prm0)
+            launches = P.info().last_run_kernel_launches
+            self.sync_all()
+            for k in range(K):                                            # timed: K steps, L2 flushed (untimed) between them
+                flush.fill_(k & 0xFF)
+                ev[k][0].record(stream)
+                P.resume(prm_step, out)
+                ev[k][1].record(stream)
+                launches += P.info().last_run_kernel_launches
+            self.sync_all()
+            step_ms = [a.elapsed_time(b) for a, b in ev]
+            res["best_flushed"] = float(out["obj"].min().item())
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            P.resume(prm0, out)                                           # evaluation alone (one evaluation-only call)
+            self.sync_all()
+            e0.record(stream)
+            for _ in range(10):
+                P.resume(prm0, out)
+            e1.record(stream)
+            self.sync_all()
+            t_eval = e0.elapsed_time(e1) / 1e3 / 10
+            if not full:
+                res["clocks"] = sampler.stop()
+            else:
+                prm_all = api.params_from_hyper(h, iters=h.eval_every * K)
+                self.sync_all()
+                e0.record(stream)                                         # whole_run: one gda_run of K steps, no flush
+                out = P.run(x0, h.lambda0, prm_all, trace_cap=min(K, 4096))
+                e1.record(stream)
+                self.sync_all()
+                res["t_whole"] = e0.elapsed_time(e1) / 1e3
+                res["clocks"] = sampler.stop()
+                res["trace"] = (out["trace_best"].cpu().numpy(), out["trace_ns"].cpu().numpy())
+                # ---- e2e through gda_run_host, HOST buffers (pinned), copies inside the timed region ----
+                xb_host = torch.empty((n, B), dtype=torch.uint8).pin_memory()
+                obj_host = torch.empty(B, dtype=torch.float64).pin_memory()
+                best_host = torch.empty(1, dtype=torch.int32).pin_memory()
+                hp = (x0_host.data_ptr(), h.lambda0)
+                op = (xb_host.data_ptr(), obj_host.data_ptr(), best_host.data_ptr(), stream.cuda_stream)
+                P.run_host_ptrs(B, *hp, prm_step, *op)
+                self.sync_all()
+                w0 = time.perf_counter()                                  # (1) per step: H2D of the step's input, D2H of its result
+                for _ in range(K):
+                    P.run_host_ptrs(B, *hp, prm_step, *op)
+                self.sync_all()
+                res["t_e2e_steps"] = time.perf_counter() - w0
+                w0 = time.perf_counter()                                  # (2) the way a user runs it: one call of K steps
+                P.run_host_ptrs(B, *hp, prm_all, *op)
+                self.sync_all()
+                res["t_e2e_one_call"] = time.perf_counter() - w0
+                res["h2d"] = x0_host.numel() * 4
+                res["d2h"] = n * B + 8 * B + 4
+                res["out"] = out
+        res.update(step_ms=step_ms, t_eval=t_eval, launches=int(launches))
+        res["roofline"] = roofline_block(w, peaks, sum(step_ms) / 1e3 / K, statistics.median(step_ms) / 1e3, t_eval)
+        res["P"] = P
+        return res
+
+
+def secondary_line(w: wl.Workload, r, K):
+    """One entry of `secondary`: the same measurement (K flushed steps, CUDA events) on another workload."""
+    t = sum(r["step_ms"]) / 1e3
+    return {"workload": w.name, "kind": w.kind, "n": w.problem.n, "B": w.B, "steps": K,
+            "value": w.B * w.hyper.eval_every * K / t, "unit": "restart-iters/s", "ms_per_step": 1e3 * t / K,
+            "ms_per_step_median": statistics.median(r["step_ms"]), "roofline": r["roofline"], "clocks": r["clocks"],
+            "best_objective": r["best_flushed"], "gpu_launches": r["launches"]}
+
+
 def run_ours(args, w: wl.Workload):
     import torch
     import torch.distributed as dist
@@ -254,139 +440,66 @@ def run_ours(args, w: wl.Workload):
     peaks = load_peaks()
     h, B, n = w.hyper, w.B, w.problem.n
     K, W = args.steps, max(args.warmup, 3)
-    P = api.create_from_workload(w.problem)
-    x0_host = torch.from_numpy(start_point(w, multirank.rank_x0_seed(w.x0_seed, rank))).pin_memory()   # each rank: its own restarts
-    x0 = x0_host.to(dev, non_blocking=True)
-    stream = torch.cuda.Stream(dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    prm_step = api.params_from_hyper(h, iters=h.eval_every)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-
-    def sync_all():
-        torch.cuda.synchronize(dev)
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize(dev)
-
-    with torch.cuda.stream(stream):
-        # ---- warm-up: W steps (captures the CUDA graph, warms caches and clocks) ----
-        out = P.run(x0, h.lambda0, prm_step)
-        for _ in range(W - 1):
-            P.resume(prm_step, out)
-        sync_all()
-        sampler = ClockSampler(local_rank)
-        sampler.start()
-        # ---- timed: K steps, L2 flushed (untimed) between them ----
-        out = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=0))
-        launches = P.info().last_run_kernel_launches
-        sync_all()
-        wall0 = time.perf_counter()
-        for k in range(K):
-            flush.fill_(k & 0xFF)
-            ev[k][0].record(stream)
-            P.resume(prm_step, out)
-            ev[k][1].record(stream)
-            launches += P.info().last_run_kernel_launches
-        sync_all()
-        wall = time.perf_counter() - wall0
-        step_ms = [a.elapsed_time(b) for a, b in ev]
-        t_steps = sum(step_ms) / 1e3
-        best_flushed = float(out["obj"].min().item())
-
-        # ---- whole_run: one gda_run of K steps, no flush ----
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        prm_all = api.params_from_hyper(h, iters=h.eval_every * K)
-        sync_all()
-        e0.record(stream)
-        out = P.run(x0, h.lambda0, prm_all, trace_cap=min(K, 4096))
-        e1.record(stream)
-        sync_all()
-        t_whole = e0.elapsed_time(e1) / 1e3
-        whole_launches = P.info().last_run_kernel_launches
-        step_launches = P.info().last_run_step_launches
-
-        # ---- evaluation alone (one evaluation-only call), to isolate the step kernel's share ----
-        prm0 = api.params_from_hyper(h, iters=0)
-        P.resume(prm0, out)
-        sync_all()
-        e0.record(stream)
-        for _ in range(10):
-            P.resume(prm0, out)
-        e1.record(stream)
-        sync_all()
-        t_eval = e0.elapsed_time(e1) / 1e3 / 10
-        clocks = sampler.stop()
-
-        # ---- e2e: HOST buffers through gda_run_host (copies inside the timed region) ----
-        xb_host = torch.empty((n, B), dtype=torch.uint8).pin_memory()
-        obj_host = torch.empty(B, dtype=torch.float64).pin_memory()
-        best_host = torch.empty(1, dtype=torch.int32).pin_memory()
-        P.run_host_ptrs(B, x0_host.data_ptr(), h.lambda0, api.params_from_hyper(h, iters=h.eval_every),
-                        xb_host.data_ptr(), obj_host.data_ptr(), best_host.data_ptr(), stream.cuda_stream)
-        sync_all()
-        w0 = time.perf_counter()
-        e0.record(stream)
-        P.run_host_ptrs(B, x0_host.data_ptr(), h.lambda0, prm_all, xb_host.data_ptr(), obj_host.data_ptr(),
-                        best_host.data_ptr(), stream.cuda_stream)
-        e1.record(stream)
-        sync_all()
-        t_e2e = max(e0.elapsed_time(e1) / 1e3, 0.0)
-        t_e2e_wall = time.perf_counter() - w0
-
-    t_steps, t_whole, t_e2e, t_eval = (multirank.max_over_ranks(v, world, dev)
-                                       for v in (t_steps, t_whole, max(t_e2e, t_e2e_wall), t_eval))
+    S = Session(local_rank, rank, world)
+    r = S.measure(w, K, W, peaks, full=True)
+    out, P = r["out"], r["P"]
+    t_steps = multirank.max_over_ranks(sum(r["step_ms"]) / 1e3, world, dev)
+    t_whole, t_e2e, t_e2e1 = (multirank.max_over_ranks(r[k], world, dev) for k in ("t_whole", "t_e2e_steps", "t_e2e_one_call"))
     best, best_rank, best_restart = multirank.combine_best(float(out["obj"].min().item()),
                                                             int(out["best_restart"].item()), rank, world, dev)
+    launches = r["launches"]
+    P.destroy()
+
+    # ---- secondary workloads, same process, same method (default headline run on one GPU only) ----
+    secondary = []
+    if world == 1 and not args.no_secondary and args.config == HEADLINE_CONFIG and not (args.mis or args.maxkcut or args.pdbo_s or args.B):
+        Ks = max(5, min(K, args.secondary_steps))
+        for sw in (wl.config(3, B=1024), wl.config(4), wl.config(5), wl.config(2), wl.config(1), wl.pdbo_s_variant(wl.config(3))):
+            rs = S.measure(sw, Ks, 3, peaks, full=False)
+            rs["P"].destroy()
+            secondary.append(secondary_line(sw, rs, Ks))
 
     iters_per_step = h.eval_every
     units = world * B * iters_per_step * K
-    work = algorithmic_work(w)
-    t_kernel = max((t_steps / K - t_eval), 1e-9) / iters_per_step        # avg duration of one step-kernel launch
-    if work["bound"] == "hbm":
-        achieved, peak, unit = work["bytes"] / t_kernel / 1e9, peaks["hbm_gbs"], "GB/s"
-    else:
-        achieved, peak, unit = work["flops"] / t_kernel / 1e12, peaks["bf16_tflops_sustained"], "TFLOP/s"
-    traffic = None
-    tf = ROOT / "profiles" / "ncu_traffic.json"
-    if tf.exists():
-        traffic = json.loads(tf.read_text()).get(w.name, {}).get("bytes")
-    trace = None
-    if "trace_best" in out:
-        tb_, tn_ = out["trace_best"].cpu().numpy(), out["trace_ns"].cpu().numpy()
-        sel = sorted(set([0, len(tb_) // 4, len(tb_) // 2, len(tb_) - 1]))
-        trace = [{"ms": float((tn_[i] - tn_[0]) / 1e6 + t_whole * 1e3 / K), "best": float(tb_[i])} for i in sel]
+    tb_, tn_ = r["trace"]
+    sel = sorted(set([0, len(tb_) // 4, len(tb_) // 2, len(tb_) - 1]))
+    # device timestamps (globaltimer) of the evaluations; the run's start is the last evaluation minus the event-timed run
+    t_end_ns = float(tn_[-1])
+    ms_at = lambda i: max(0.0, t_whole * 1e3 - (t_end_ns - float(tn_[i])) / 1e6)
+    trace = [{"ms": ms_at(i), "best": float(tb_[i])} for i in sel]
+    first_best = int(np.argmax(tb_ == tb_[-1]))                # earliest evaluation that holds the final best
 
     if rank == 0:
         cpu = time_oracle(w, args.cpu_budget) if world == 1 and not args.no_cpu_baseline else None
         line = {
             "metric": "restart-iterations/s", "value": units / t_steps, "unit": "restart-iters/s",
             "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": 1e3 * t_steps / K,
+            "ms_per_step_median": statistics.median(r["step_ms"]),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if w.kind != "qubo_dense" else "bf16 x bf16 -> f32 (state f32)", "data": "synthetic",
-            "config": {"workload": w.name, "baseline_config_index": args.config, "kind": w.kind, "n": n, "B_per_gpu": B,
-                       "step": f"{iters_per_step} GDA iterations + 1 evaluation (one CUDA graph launch)",
-                       "hyper": {"lambda0": h.lambda0, "alpha": h.alpha, "beta": h.beta, "delta": h.delta, "gfun": h.gfun,
-                                 "dual": "scalar (PDBO-s)" if getattr(h, "dual", 0) else "per-variable (PDBO)"},
-                       "l2": "flushed between timed steps (256 MiB write, untimed)", "note": w.note},
+            "config": config_dict(args, w),
             "whole_run": {"value": units / t_whole, "unit": "restart-iters/s", "ms_total": 1e3 * t_whole,
                           "iters": iters_per_step * K, "l2": "not flushed (one gda_run call)", "best_objective": best,
-                          "best_vs_time": trace},
-            "e2e": {"value": units / t_e2e, "unit": "restart-iters/s", "h2d_bytes_per_step": x0_host.numel() * 4 / K,
-                    "d2h_bytes_per_step": (n * B + 8 * B + 4) / K, "ms_total": 1e3 * t_e2e,
-                    "note": "gda_run_host: one call of K steps; x0 H2D and x_bin/obj/best D2H once per call, amortised per step"},
+                          "best_vs_time": trace, "time_to_best_ms": ms_at(first_best),
+                          "time_to_best_note": "earliest evaluation at which the best objective of the run was held (PAPER.md:214), "
+                                               "from the device-side globaltimer trace"},
+            "e2e": {"value": units / t_e2e, "unit": "restart-iters/s", "h2d_bytes_per_step": r["h2d"],
+                    "d2h_bytes_per_step": r["d2h"], "ms_total": 1e3 * t_e2e,
+                    "note": "K calls of gda_run_host, one step each: every step copies its start point x0 from pinned host memory "
+                            "(H2D) and reads x_bin / obj / best_restart back (D2H) inside the timed region (host wall clock)",
+                    "one_call": {"value": units / t_e2e1, "ms_total": 1e3 * t_e2e1, "h2d_bytes": r["h2d"], "d2h_bytes": r["d2h"],
+                                 "note": "the way a solver is used: ONE gda_run_host call of K steps, copies once"}},
             "gpu_launches": int(launches),
-            "roofline": {"bound": work["bound"], "achieved": achieved, "peak": peak, "unit": unit,
-                         "frac": achieved / peak, "traffic": traffic, "peak_source": peaks["source"],
-                         "kernel": "step kernel (gradient + fused update)", "us_per_launch": t_kernel * 1e6,
-                         "algorithmic_bytes_per_launch": work["bytes"], "algorithmic_flops_per_launch": work["flops"],
-                         "eval_us": t_eval * 1e6},
-            "clocks": clocks,
-            "best_objective": best, "best_rank": best_rank, "best_restart": best_restart, "best_objective_flushed_run": best_flushed,
+            "roofline": r["roofline"],
+            "clocks": r["clocks"],
+            "best_objective": best, "best_rank": best_rank, "best_restart": best_restart,
+            "best_objective_flushed_run": r["best_flushed"],
         }
+        if secondary:
+            line["secondary"] = secondary
         if cpu:
             line["cpu_baseline"] = cpu
         print(json.dumps(line))
-    P.destroy()
     if world > 1:
         dist.destroy_process_group()
 
@@ -400,6 +513,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the secondary workloads of the default run")
+    ap.add_argument("--secondary-steps", type=int, default=20, help="timed steps per secondary workload")
     ap.add_argument("--B", type=int, default=None)
     ap.add_argument("--pdbo-s", action="store_true", help="run the PDBO-s ablation (one multiplier per restart, PAPER.md:630-648)")
     ap.add_argument("--maxkcut", default=None, metavar="N,M,K", help="instead of --config: Max-K-Cut on G(N, M) (PAPER.md:784-828)")

@@ -162,6 +162,7 @@ extern "C" gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, cons
         st = upload(&p->d_heavy_rows, heavy);
         if (st == GDA_OK) st = upload(&p->d_light_rows, light);
     }
+    if (st == GDA_OK) st = sparse_build_slab(p, h_rowptr, h_col, h_val2);
     if (st == GDA_OK && (int64_t)h_col.size() <= 8 * (int64_t)n) {
         // packed records for rows of degree <= 8 (one 64-byte load replaces rowptr -> col/val): 8 columns then 8
         // values, zeros dropped, padding = (own row, 0); word 0 = -1 sends the row to the CSR path.
@@ -346,7 +347,7 @@ static void free_workspace(gda_problem* p) {
     cudaFree(ws.obj_now); cudaFree(ws.improved); cudaFree(ws.partial); cudaFree(ws.state);
     cudaFree(ws.best_restart); cudaFree(ws.best_val); cudaFree(ws.trace_best); cudaFree(ws.trace_ns);
     cudaFree(ws.zt[0]); cudaFree(ws.zt[1]); cudaFree(ws.z); cudaFree(ws.lab);
-    cudaFree(ws.mu[0]); cudaFree(ws.mu[1]); cudaFree(ws.gpart);
+    cudaFree(ws.mu[0]); cudaFree(ws.mu[1]); cudaFree(ws.gpart); cudaFree(ws.block_min);
     ws = Workspace();
 }
 
@@ -357,6 +358,7 @@ extern "C" void gda_destroy(gda_problem* p) {
     free_workspace(p);
     cudaFree(p->d_rowptr); cudaFree(p->d_col); cudaFree(p->d_val2); cudaFree(p->d_cprime);
     cudaFree(p->d_heavy_rows); cudaFree(p->d_light_rows); cudaFree(p->d_ell);
+    cudaFree(p->d_slab_ent); cudaFree(p->d_slab_goff); cudaFree(p->d_slab_grow); cudaFree(p->d_slab_ent16);
     cudaFree(p->d_vptr); cudaFree(p->d_coef); cudaFree(p->d_others); cudaFree(p->d_cptr); cudaFree(p->d_lit); cudaFree(p->d_w);
     dense_release(p);
     if (p->own_stream) cudaStreamDestroy(p->own_stream);
@@ -423,6 +425,7 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
         if (st == GDA_OK) st = dmalloc(&ws.gpart, (size_t)ws.n_gpart * B);
     }
     if (st == GDA_OK) st = dmalloc(&ws.state, 1);
+    if (st == GDA_OK) st = dmalloc(&ws.block_min, (size_t)(B + 31) / 32);
     if (st == GDA_OK) st = dmalloc(&ws.best_restart, 1);
     if (st == GDA_OK) st = dmalloc(&ws.best_val, 1);
     ws.trace_cap = TRACE_CAP;
@@ -473,13 +476,13 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     const UpdParams up = make_upd(prm);
     int cur = parity;
     const bool scalar = prm.dual == GDA_DUAL_SCALAR;
-    int resident = 0;                                         // tiny sparse problems: the whole chunk in one launch
-    if (p->kind == GDA_KIND_SPARSE && !scalar) {
+    if (p->kind == GDA_KIND_SPARSE && !scalar) {              // small n: steps AND evaluation in one launch, state on chip
+        int slab = 0;
         const int64_t before = *launches;
-        GDA_TRY(sparse_steps_resident(p, B, len, ws.x[cur], ws.y, ws.x[cur ^ (len & 1)], up, ws.state, s, launches, &resident));
-        if (resident) { *step_launches += *launches - before; cur ^= (len & 1); }
+        GDA_TRY(sparse_chunk_slab(p, B, len, ws.x[cur], ws.x[cur ^ (len & 1)], ws.y, up, s, launches, &slab));   // buffer parity as the per-step kernels leave it
+        if (slab) { *step_launches += *launches - before; return GDA_OK; }
     }
-    for (int k = 0; k < len && !resident; ++k) {
+    for (int k = 0; k < len; ++k) {
         int64_t before = *launches;
         ScalarDual sd;                                        // PDBO-s: mu follows the parity of x
         if (scalar) { sd.mu = ws.mu[cur]; sd.gpart = ws.gpart; }

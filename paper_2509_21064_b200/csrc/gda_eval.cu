@@ -5,10 +5,11 @@
 #include "gda_internal.cuh"
 
 #include <math_constants.h>
+#include <algorithm>
 
 namespace {
 
-constexpr int FIN_COLS = 256, FIN_SLICES = 4, FIN_THREADS = FIN_COLS * FIN_SLICES;
+constexpr int FIN_COLS = 32, FIN_SLICES = 32;                // block = 32 restarts x 32 row slices
 
 __device__ __forceinline__ uint64_t globaltimer_ns() {
     uint64_t t;
@@ -16,84 +17,97 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
     return t;
 }
 
-// obj_now[b] = sum_p partial[p][b]; best-so-far update.  One block of 256 columns x 4 row slices: slice s adds the rows
-// p = s, s + 4, ... (8 independent loads in flight), the four slice sums are added in slice order -- a fixed order, so
-// the result is deterministic (and exact for integral instances).  Thread 0 afterwards records the trace entry and
-// advances the run state.
+// obj_now[b] = sum_p partial[p][b]; best-so-far update.  grid = ceil(B / 32) blocks of (32 restarts, 32 row slices):
+// slice s adds the rows p = s, s + 32, ... (8 independent loads in flight), the 32 slice sums are then added in slice
+// order -- a fixed order, so the result is deterministic (and exact for integral instances).  The last block to finish
+// (a ticket in the run state) takes the minimum of the blocks' best values -- order-independent -- records the trace
+// entry, advances the run state and publishes whether ANY restart improved, which lets the commit kernel return at once.
+// ld = row stride of `partial` (>= B).
 template <bool INTEGRAL>
-__global__ void __launch_bounds__(FIN_THREADS)
-finalize_kernel(int B, const void* __restrict__ partial, int n_part, double* __restrict__ obj_now,
-                double* __restrict__ best_obj, int32_t* __restrict__ improved, RunState* st,
-                double* __restrict__ trace_best, uint64_t* __restrict__ trace_ns, int trace_cap,
-                uint32_t advance_t) {
+__global__ void __launch_bounds__(FIN_COLS * FIN_SLICES)
+finalize_kernel(int B, int ld, const void* __restrict__ partial, int n_part, double* __restrict__ obj_now,
+                double* __restrict__ best_obj, int32_t* __restrict__ improved, RunState* st, double* block_min,
+                double* __restrict__ trace_best, uint64_t* __restrict__ trace_ns, int trace_cap, uint32_t advance_t) {
     using acc_t = typename std::conditional<INTEGRAL, long long, double>::type;
-    __shared__ acc_t red[FIN_SLICES][FIN_COLS];
-    __shared__ double smin[FIN_THREADS / 32];
+    __shared__ acc_t red[FIN_SLICES][FIN_COLS + 1];
     const acc_t* part = reinterpret_cast<const acc_t*>(partial);
-    const int col = threadIdx.x % FIN_COLS, slice = threadIdx.x / FIN_COLS;
-    double local_min = CUDART_INF;
-    for (int b0 = 0; b0 < B; b0 += FIN_COLS) {
-        const int b = b0 + col;
-        acc_t s = 0;
-        if (b < B) {
-            int q = slice;
-            for (; q + 7 * FIN_SLICES < n_part; q += 8 * FIN_SLICES) {
-                acc_t v[8];
+    const int col = threadIdx.x, slice = threadIdx.y;
+    const int b = blockIdx.x * FIN_COLS + col;
+    acc_t s = 0;
+    if (b < B) {
+        int q = slice;
+        for (; q + 7 * FIN_SLICES < n_part; q += 8 * FIN_SLICES) {
+            acc_t v[8];
 #pragma unroll
-                for (int u = 0; u < 8; ++u) v[u] = part[(size_t)(q + u * FIN_SLICES) * B + b];
+            for (int u = 0; u < 8; ++u) v[u] = part[(size_t)(q + u * FIN_SLICES) * ld + b];
 #pragma unroll
-                for (int u = 0; u < 8; ++u) s += v[u];
-            }
-            for (; q < n_part; q += FIN_SLICES) s += part[(size_t)q * B + b];
+            for (int u = 0; u < 8; ++u) s += v[u];
         }
-        __syncthreads();                                     // red[] of the previous pass has been consumed
-        red[slice][col] = s;
-        __syncthreads();
-        if (slice == 0 && b < B) {
-            acc_t t = red[0][col];
+        for (; q < n_part; q += FIN_SLICES) s += part[(size_t)q * ld + b];
+    }
+    red[slice][col] = s;
+    __syncthreads();
+    if (slice != 0) return;                                  // warp 0 = the 32 restarts of this block
+    double local_min = CUDART_INF;
+    int imp = 0;
+    if (b < B) {
+        acc_t t = red[0][col];
 #pragma unroll
-            for (int k = 1; k < FIN_SLICES; ++k) t += red[k][col];
-            const double v = (double)t;
-            if (obj_now) obj_now[b] = v;
-            if (best_obj) {
-                double best = best_obj[b];
-                const int imp = v < best;
-                if (imp) { best = v; best_obj[b] = v; }
-                improved[b] = imp;
-                local_min = fmin(local_min, best);
-            }
+        for (int k = 1; k < FIN_SLICES; ++k) t += red[k][col];
+        const double v = (double)t;
+        if (obj_now) obj_now[b] = v;
+        if (best_obj) {
+            double best = best_obj[b];
+            imp = v < best;
+            if (imp) { best = v; best_obj[b] = v; }
+            improved[b] = imp;
+            local_min = best;
         }
     }
     if (!st) return;
     for (int o = 16; o > 0; o >>= 1) local_min = fmin(local_min, __shfl_xor_sync(0xffffffffu, local_min, o));
-    if ((threadIdx.x & 31) == 0) smin[threadIdx.x >> 5] = local_min;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double m = smin[0];
-        for (int w = 1; w < FIN_THREADS / 32; ++w) m = fmin(m, smin[w]);
+    imp = __any_sync(0xffffffffu, imp);
+    unsigned ticket = 0;
+    if (col == 0) {
+        block_min[blockIdx.x] = local_min;
+        if (imp) atomicOr(&st->imp_accum, 1u);
+        __threadfence();
+        ticket = atomicAdd(&st->ticket, 1u);
+    }
+    ticket = __shfl_sync(0xffffffffu, ticket, 0);
+    if (ticket != gridDim.x - 1) return;
+    __threadfence();                                         // last block: every block's minimum is visible
+    double m = CUDART_INF;
+    for (int k = col; k < (int)gridDim.x; k += 32) m = fmin(m, __ldcg(block_min + k));
+    for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (col == 0) {
         const uint32_t k = st->n_eval;
         if (trace_best && (int)k < trace_cap) { trace_best[k] = m; trace_ns[k] = globaltimer_ns(); }
         st->n_eval = k + 1;
         st->t += advance_t;
+        st->any_improved = atomicExch(&st->imp_accum, 0u);
+        st->ticket = 0;
     }
 }
 
-// x_bin[:, b] = [x[:, b] > 1/2] for every restart b whose objective improved at this evaluation
+// x_bin[:, b] = [x[:, b] > 1/2] for every restart b whose objective improved at this evaluation; returns at once when
+// none did (the usual case late in a run).  Grid-stride over float4 vectors.
 __global__ void __launch_bounds__(256)
 commit_kernel(size_t n_vec, int B4, const float* __restrict__ x, const int32_t* __restrict__ improved,
-              uint8_t* __restrict__ x_bin) {
-    const size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (v >= n_vec) return;
-    const int c4 = (int)(v % (size_t)B4);
-    const int4 imp = __ldg(reinterpret_cast<const int4*>(improved) + c4);
-    if (!(imp.x | imp.y | imp.z | imp.w)) return;
-    const float4 xv = ldg4(x + 4 * v);
-    uchar4 o = reinterpret_cast<uchar4*>(x_bin)[v];
-    if (imp.x) o.x = xv.x > 0.5f;
-    if (imp.y) o.y = xv.y > 0.5f;
-    if (imp.z) o.z = xv.z > 0.5f;
-    if (imp.w) o.w = xv.w > 0.5f;
-    reinterpret_cast<uchar4*>(x_bin)[v] = o;
+              const RunState* __restrict__ st, uint8_t* __restrict__ x_bin) {
+    if (st && st->any_improved == 0u) return;
+    for (size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x; v < n_vec; v += (size_t)gridDim.x * blockDim.x) {
+        const int c4 = (int)(v % (size_t)B4);
+        const int4 imp = __ldg(reinterpret_cast<const int4*>(improved) + c4);
+        if (!(imp.x | imp.y | imp.z | imp.w)) continue;
+        const float4 xv = ldg4(x + 4 * v);
+        uchar4 o = reinterpret_cast<uchar4*>(x_bin)[v];
+        if (imp.x) o.x = xv.x > 0.5f;
+        if (imp.y) o.y = xv.y > 0.5f;
+        if (imp.z) o.z = xv.z > 0.5f;
+        if (imp.w) o.w = xv.w > 0.5f;
+        reinterpret_cast<uchar4*>(x_bin)[v] = o;
+    }
 }
 
 // S6: argmin over restarts, ties -> lowest index; warp shuffles, then one warp over the per-warp winners
@@ -140,7 +154,7 @@ __global__ void __launch_bounds__(256)
 init_state_kernel(int B, double* __restrict__ best_obj, int32_t* __restrict__ improved, RunState* st, uint32_t t0) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b < B) { best_obj[b] = CUDART_INF; improved[b] = 0; }
-    if (b == 0) { st->t = t0; st->n_eval = 0; }
+    if (b == 0) { st->t = t0; st->n_eval = 0; st->ticket = 0; st->imp_accum = 0; st->any_improved = 1; }
 }
 
 // PDBO-s: mu_out[b] = mu_in[b] + beta * sum_r gpart[r][b].  grid ceil(B/32), block (32 restarts, 32 slices): rows are
@@ -283,12 +297,14 @@ gda_status eval_finalize(gda_problem* p, int32_t B, const void* partial, int32_t
                          double* best_obj, int32_t* improved, RunState* st, double* trace_best,
                          uint64_t* trace_ns, int32_t trace_cap, uint32_t advance_t, cudaStream_t s,
                          int64_t* launches) {
+    const unsigned grid = (unsigned)((B + FIN_COLS - 1) / FIN_COLS);
+    const dim3 block(FIN_COLS, FIN_SLICES);
     if (p->integral)
-        finalize_kernel<true><<<1, FIN_THREADS, 0, s>>>(B, partial, n_part, obj_now, best_obj, improved, st,
-                                                        trace_best, trace_ns, trace_cap, advance_t);
+        finalize_kernel<true><<<grid, block, 0, s>>>(B, B, partial, n_part, obj_now, best_obj, improved, st, p->ws.block_min,
+                                                     trace_best, trace_ns, trace_cap, advance_t);
     else
-        finalize_kernel<false><<<1, FIN_THREADS, 0, s>>>(B, partial, n_part, obj_now, best_obj, improved, st,
-                                                         trace_best, trace_ns, trace_cap, advance_t);
+        finalize_kernel<false><<<grid, block, 0, s>>>(B, B, partial, n_part, obj_now, best_obj, improved, st, p->ws.block_min,
+                                                      trace_best, trace_ns, trace_cap, advance_t);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
@@ -302,7 +318,8 @@ gda_status score_reduce(gda_problem* p, int32_t B, const void* partial, int32_t 
 gda_status eval_commit(gda_problem* p, int32_t B, const float* x, const int32_t* improved, uint8_t* x_bin,
                        cudaStream_t s, int64_t* launches) {
     const size_t n_vec = (size_t)p->n * B / 4;
-    commit_kernel<<<(unsigned)((n_vec + 255) / 256), 256, 0, s>>>(n_vec, B / 4, x, improved, x_bin);
+    const unsigned grid = (unsigned)std::min<size_t>((n_vec + 255) / 256, (size_t)p->num_sms * 8);
+    commit_kernel<<<grid, 256, 0, s>>>(n_vec, B / 4, x, improved, p->ws.state, x_bin);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
@@ -321,7 +338,8 @@ gda_status eval_yg_partials(gda_problem* p, int32_t B, const float* x, const flo
 }
 
 gda_status eval_sum_partials(int32_t B, const double* partial, int32_t n_part, double* out, cudaStream_t s) {
-    finalize_kernel<false><<<1, FIN_THREADS, 0, s>>>(B, partial, n_part, out, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0);
+    finalize_kernel<false><<<(unsigned)((B + FIN_COLS - 1) / FIN_COLS), dim3(FIN_COLS, FIN_SLICES), 0, s>>>(
+        B, B, partial, n_part, out, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0);
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
 }

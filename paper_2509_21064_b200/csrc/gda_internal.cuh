@@ -49,8 +49,11 @@ struct ScalarDual {
 
 // device-side run state (lives in the workspace)
 struct RunState {
-    uint32_t t;          // iteration index of the iterate currently in x[cur]
-    uint32_t n_eval;     // evaluations done so far in this run
+    uint32_t t;             // iteration index of the iterate currently in x[cur]
+    uint32_t n_eval;        // evaluations done so far in this run
+    uint32_t ticket;        // blocks of the current finalize launch that are done (reset by the last one)
+    uint32_t imp_accum;     // OR of "a restart of my block improved" over the blocks of the current finalize launch
+    uint32_t any_improved;  // ... of the last completed evaluation: 0 lets commit_kernel return at once
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -75,6 +78,7 @@ struct Workspace {
     void* partial = nullptr;            // [n_part][B] int64 or double partial objective sums
     int32_t n_part = 0;
     RunState* state = nullptr;
+    double* block_min = nullptr;        // [ceil(B / 32)] per-block minima of the best objectives (finalize)
     int32_t* best_restart = nullptr;    // [1]
     double* best_val = nullptr;         // [1]
     double* trace_best = nullptr;       // internal trace buffers (copied out on request)
@@ -113,6 +117,11 @@ struct gda_problem {
     int32_t* d_heavy_rows = nullptr; int32_t n_heavy = 0;   // rows handled by the row-split kernel
     int32_t* d_light_rows = nullptr; int32_t n_light = 0;   // nullptr = all rows, in order
     int32_t max_deg = 0;
+    // slab path (small n, gda_sparse.cu): sliced ELL of (column byte offset, val2) pairs, 16 rows per group
+    int2* d_slab_ent = nullptr; int32_t* d_slab_goff = nullptr; int32_t* d_slab_grow = nullptr;
+    int32_t slab_groups = 0, slab_slots = 0; int64_t slab_real = 0;
+    uint16_t* d_slab_ent16 = nullptr; uint32_t slab_cbits = 0; int32_t slab_passes = 0;   // compact form (one |val2|), else null
+    int32_t slab_mode = 0;               // GDA_SPARSE_PATH at create: 1 "slab" always, -1 "stream" never, 0 by the cost model
     int32_t* d_ell = nullptr;            // [n][16] packed low-degree rows: 8 cols + 8 val2 (see gda_sparse.cu); nullptr = not built
     // dense QUBO: Q_off in bf16 [n][n] (zero diagonal), r0 = Q_off 1 (row sums) for the centred operand
     __nv_bfloat16* d_Qbf = nullptr; float* d_rowsum = nullptr;
@@ -137,8 +146,11 @@ gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, floa
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
 int32_t sparse_num_gparts(const gda_problem* p);
 gda_status sparse_configure(gda_problem* p);                       // at create
-gda_status sparse_steps_resident(gda_problem* p, int32_t B, int32_t len, const float* x_in, float* y, float* x_out,
-                                 const UpdParams& up, const RunState* st, cudaStream_t s, int64_t* launches, int* done);
+// small n: sliced-ELL structure built at create, and one launch per chunk (steps + evaluation) when it applies
+gda_status sparse_build_slab(gda_problem* p, const std::vector<int32_t>& rowptr, const std::vector<int32_t>& col,
+                             const std::vector<float>& val2);
+gda_status sparse_chunk_slab(gda_problem* p, int32_t B, int32_t len, const float* x_in, float* x_out, float* y,
+                             const UpdParams& up, cudaStream_t s, int64_t* launches, int* done);
 gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);
 gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
                                  cudaStream_t s, int64_t* launches);

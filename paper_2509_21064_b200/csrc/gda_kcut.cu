@@ -207,7 +207,8 @@ kcut_score_kernel(int n, int B, const int32_t* __restrict__ rowptr, const int32_
 // best-so-far labels: x_bin[:, b] = lab[:, b] for every restart whose objective improved at this evaluation
 __global__ void __launch_bounds__(256)
 kcut_commit_kernel(size_t n_vec, int B4, const uint8_t* __restrict__ lab, const int32_t* __restrict__ improved,
-                   uint8_t* __restrict__ x_bin) {
+                   const RunState* __restrict__ st, uint8_t* __restrict__ x_bin) {
+    if (st->any_improved == 0u) return;                      // no restart improved at this evaluation (finalize_kernel)
     const size_t v = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= n_vec) return;
     const int b0 = 4 * (int)(v % (size_t)B4);
@@ -266,7 +267,7 @@ gda_status kcut_score_partials(gda_problem* p, int32_t B, const float* z, uint8_
 gda_status kcut_commit(gda_problem* p, int32_t B, const uint8_t* lab, const int32_t* improved, uint8_t* x_bin,
                        cudaStream_t s, int64_t* launches) {
     const size_t n_vec = (size_t)p->n * B / 4;
-    kcut_commit_kernel<<<(unsigned)((n_vec + 255) / 256), 256, 0, s>>>(n_vec, B / 4, lab, improved, x_bin);
+    kcut_commit_kernel<<<(unsigned)((n_vec + 255) / 256), 256, 0, s>>>(n_vec, B / 4, lab, improved, p->ws.state, x_bin);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;

@@ -10,6 +10,13 @@
 // Rows with more than HEAVY_DEG non-zeros are split across the 8 warps of a block (row-split variant).
 #include "gda_internal.cuh"
 
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <math_constants.h>
+#define CUDART_INF_SLAB CUDART_INF
+
 namespace {
 
 constexpr int WARPS = 8;
@@ -228,51 +235,279 @@ spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chu
     if (DUAL && active) *reinterpret_cast<float4*>(sd.gpart + (size_t)(gpart_row0 + ridx) * B + 4 * c4) = gs;
 }
 
-// ---- resident variant for tiny problems (config 1: n = 20, B = 64) -----------------------------------------------
-// When the whole state and the CSR fit one block's shared memory (n B <= RESIDENT_MAX elements: x double-buffered and
-// y, 12 bytes per element), a chunk of `len` GDA steps is ONE launch of one block: the iterates stay in shared memory, steps are
-// separated by __syncthreads(), and only the last iterate goes back to global memory.  Config 1: 1.4 us per step
-// (one SM's issue rate: about 3000 warp instructions per step) instead of 2.2 us per kernel launch.  The arithmetic per element is that of spmm_step_warp (same
-// order of the row's entries, same fused update).
-constexpr int RESIDENT_MAX = 12288;
-constexpr int RESIDENT_THREADS = 1024;
-constexpr int RESIDENT_SMEM = 200 * 1024;         // state + the whole CSR
+// ---- slab variant for small n: a whole chunk of steps AND its evaluation in one launch ---------------------------------
+// Restarts are independent, so a CTA that owns a slab of SLAB_S = 8 restarts for ALL n rows needs nobody
+// else: x (double-buffered: the update is simultaneous, Eq. 6), y and c' live in shared memory for the whole chunk
+// (12 B x n x 8 per CTA: n <= 2300), the steps are separated by __syncthreads(), and global memory sees the state only at
+// the chunk's two ends.  The gathers -- what bounds config 2 (n = 800, degree 48: 157 MB per step out of L2 at 12 us) --
+// become shared-memory reads: floor = nnz x B x 4 B / (SMs x 128 B/clk), 5 us per step for config 2.
+//
+// Work split: lane = (row r of a group of 16 rows, quad q of the slab's 8 restarts); every lane walks ITS OWN row, so
+// there is no reduction across lanes.  The structure is a sliced ELL built at create (gda_api.cu): rows sorted by degree
+// and dealt to groups of 16; slot k of a group holds one (column byte offset, 2 Q_ij) pair per row, 128 contiguous
+// bytes, so the warp's fetch of slot k is ONE coalesced line (two lanes per address).  A gather is an LDS.128: the
+// hardware serves 8 lanes = 4 rows x 32 B per pass, conflict-free iff the 4 columns differ mod 4 -- the entries of
+// every 4 rows that share a pass are therefore ordered at create such that they do (zero-valued padding where the
+// greedy matching cannot; a few per cent).
+//
+// The evaluation (S5, S6's per-restart part) is fused: the CTA scores its 8 restarts exactly (integers for integral
+// instances, fixed summation order otherwise), updates best_obj / improved, commits x_hat of improved restarts to x_bin
+// and takes part in the same last-block ticket as finalize_kernel for the trace and the run state.
+constexpr int SLAB_S = 8, SLAB_ROWS = 16, SLAB_MAX_THREADS = 1024;
+constexpr int SLAB_SMEM_LIMIT = 226 * 1024;                  // dynamic shared memory of a CTA (the kernel also has a few static bytes)
 
-template <int GFUN>
-__global__ void __launch_bounds__(RESIDENT_THREADS)
-spmm_steps_resident(int n, int B, int nnz, int len, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
-                    const float* __restrict__ val2, const float* __restrict__ cprime, const float* __restrict__ x_in,
-                    float* __restrict__ y, float* __restrict__ x_out, UpdParams up, const RunState* __restrict__ st) {
-    extern __shared__ float sm[];
-    const int total = n * B;
-    float* xa = sm;                                          // x^t and x^{t+1} alternate between xa and xb
-    float* xb = sm + total;
-    float* ys = sm + 2 * total;
-    float* cps = ys + total;                                 // c'[n]
-    float* vs = cps + n;                                     // val2[nnz]
-    int* cs = reinterpret_cast<int*>(vs + nnz);              // col[nnz]
-    int* rp = cs + nnz;                                      // rowptr[n + 1]
-    for (int e = threadIdx.x; e < total; e += RESIDENT_THREADS) { xa[e] = x_in[e]; ys[e] = y[e]; }
-    for (int e = threadIdx.x; e < nnz; e += RESIDENT_THREADS) { vs[e] = val2[e]; cs[e] = col[e] * B; }
-    for (int e = threadIdx.x; e <= n; e += RESIDENT_THREADS) { rp[e] = rowptr[e]; if (e < n) cps[e] = cprime[e]; }
+struct SlabArgs {
+    int n, B, len, n_groups, groups_per_warp, n_pass;
+    const int2* ent;                 // general: [slot][16 rows] (col * 32 bytes, bits of val2)
+    const uint2* ent16;              // compact: [pass][16 rows] four 16-bit entries: bit 15 = sign of val2, bits 0..11 = column
+    uint32_t cbits;                  // compact: bits of |val2|, the one magnitude all entries share
+    const int32_t* goff;             // [n_groups + 1] first slot of a group (lengths are multiples of 4)
+    const int32_t* grow;             // [n_groups * 16] row index, -1 = no row
+    const float* cprime;
+    const float* x_in; float* x_out; // [n][B]: x^t is read from x_in at the start, x^{t+len} written to x_out at the end
+    float* y;                        // [n][B], in place (a CTA touches nothing outside its slab, so x_in may equal x_out)
+    UpdParams up;
+    RunState* st;
+    double* best_obj; int32_t* improved; uint8_t* x_bin; double* block_min;
+    double* trace_best; uint64_t* trace_ns; int trace_cap;
+};
+
+__device__ __forceinline__ uint64_t slab_globaltimer_ns() {
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+// One pass = 4 slots of this lane's row: byte offsets of the 4 gathered rows of x and their values.
+struct SlabPass { int off[4]; float val[4]; };
+
+// COMPACT (every non-zero |2 Q_ij| is the same number: unit, +-1 or constant weights -- Max-Cut on the paper's graphs,
+// MIS): 2 bytes per entry, the whole structure copied into shared memory once per chunk, so a step reads nothing but
+// shared memory.  Otherwise: 8 bytes per entry from global memory (L2), fetched one pass ahead.
+template <bool COMPACT>
+__device__ __forceinline__ SlabPass slab_fetch(const SlabArgs& a, const uint2* __restrict__ cst, int pass, int r) {
+    SlabPass p;
+    if (COMPACT) {
+        const uint2 w = cst[pass * SLAB_ROWS + r];
+        const uint32_t e[4] = {w.x & 0xFFFFu, w.x >> 16, w.y & 0xFFFFu, w.y >> 16};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            p.off[u] = (int)((e[u] & 0xFFFu) << 5);
+            p.val[u] = __uint_as_float(a.cbits ^ ((e[u] & 0x8000u) << 16));
+        }
+    } else {
+        const int2* ep = a.ent + (size_t)pass * 4 * SLAB_ROWS + r;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int2 e = __ldg(ep + u * SLAB_ROWS);
+            p.off[u] = e.x;
+            p.val[u] = __int_as_float(e.y);
+        }
+    }
+    return p;
+}
+
+// groups are sorted by falling length; warp w takes groups w, 2W-1-w, 2W+w, ... (serpentine), so that every warp gets
+// long and short ones and the per-step barrier does not wait for the warp with the longest rows
+__device__ __forceinline__ int slab_group(int i, int warp, int warps) { return (i & 1) ? i * warps + (warps - 1 - warp) : i * warps + warp; }
+
+template <int GFUN, bool INTEGRAL, bool COMPACT>
+__global__ void __launch_bounds__(SLAB_MAX_THREADS, 1)
+spmm_chunk_slab(const SlabArgs a) {
+    using acc_t = typename std::conditional<INTEGRAL, long long, double>::type;
+    extern __shared__ float4 slab_smem[];
+    const int nrow = a.n + (COMPACT ? 4 : 0);                 // compact: four rows of zeros, what padding entries gather
+    float* xa = reinterpret_cast<float*>(slab_smem);          // x^t  [nrow][8]
+    float* xb = xa + (size_t)nrow * SLAB_S;                   // x^{t+1}
+    float* ys = xb + (size_t)nrow * SLAB_S;                   // y [n][8]
+    float* cps = ys + (size_t)a.n * SLAB_S;                   // c' [n]
+    acc_t* red = reinterpret_cast<acc_t*>(cps + ((a.n + 3) & ~3));   // [warps][8] per-warp objective sums
+    uint2* cst = reinterpret_cast<uint2*>(red + (blockDim.x >> 5) * SLAB_S);   // compact structure [n_pass][16]
+    __shared__ int s_imp[SLAB_S];
+    __shared__ unsigned s_last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    const int r = lane >> 1, q = lane & 1;
+    const int b0 = blockIdx.x * SLAB_S;                       // first restart of the slab
+
+    // ---- load the slab (32 bytes per row and array; a ragged B, a multiple of 4, may lack the slab's second quad) ----
+    for (int e = threadIdx.x; e < a.n * 2; e += blockDim.x) {
+        const int row = e >> 1, qq = e & 1;
+        float4 xv = make_float4(0.f, 0.f, 0.f, 0.f), yv = xv;
+        if (b0 + 4 * qq < a.B) {
+            const size_t off = (size_t)row * a.B + b0 + 4 * qq;
+            xv = ldg4(a.x_in + off);
+            yv = ldg4(a.y + off);
+        }
+        reinterpret_cast<float4*>(xa)[e] = xv;
+        reinterpret_cast<float4*>(ys)[e] = yv;
+    }
+    for (int e = threadIdx.x; e < a.n; e += blockDim.x) cps[e] = __ldg(a.cprime + e);
+    if (COMPACT) {
+        for (int e = threadIdx.x; e < a.n_pass * SLAB_ROWS; e += blockDim.x) cst[e] = __ldg(a.ent16 + e);
+        if (threadIdx.x < 8) {                                // the zero rows, in both buffers
+            reinterpret_cast<float4*>(xa)[a.n * 2 + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
+            reinterpret_cast<float4*>(xb)[a.n * 2 + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+    }
     __syncthreads();
-    const uint32_t t0 = st ? st->t : 0u;
-    for (int k = 0; k < len; ++k) {
-        for (int e = threadIdx.x; e < total; e += RESIDENT_THREADS) {
-            const int i = e / B, b = e - i * B;
-            float acc = 0.0f;
-            const int a1 = rp[i + 1];
-#pragma unroll 4
-            for (int a = rp[i]; a < a1; ++a) acc = fmaf(vs[a], xa[cs[a] + b], acc);     // loads of later entries issue early
-            float xn, yn;
-            gda_update<GFUN>(xa[e], ys[e], acc + cps[i], up, t0 + (uint32_t)k, (uint32_t)i, (uint32_t)b, xn, yn);
-            xb[e] = xn;
-            ys[e] = yn;
+
+    const uint32_t t0 = a.st->t;
+    const char* xq = reinterpret_cast<const char*>(xa) + 16 * q;        // + column byte offset = this lane's float4 of row col
+
+    // ---- len GDA steps, state on chip ----
+    for (int k = 0; k < a.len; ++k) {
+        for (int i = 0; i < a.groups_per_warp; ++i) {
+            const int g = slab_group(i, warp, warps);
+            if (g >= a.n_groups) break;
+            const int p0 = __ldg(a.goff + g) >> 2, p1 = __ldg(a.goff + g + 1) >> 2;
+            const int row = __ldg(a.grow + g * SLAB_ROWS + r);
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+            // the structure of the NEXT pass is fetched before this pass's gathers, so that its latency hides behind them
+            SlabPass cur = slab_fetch<COMPACT>(a, cst, min(p0, a.n_pass - 1), r), nxt;
+#pragma unroll 1
+            for (int ps = p0; ps < p1; ++ps) {
+                nxt = slab_fetch<COMPACT>(a, cst, min(ps + 1, a.n_pass - 1), r);
+                float4 gv[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) gv[u] = *reinterpret_cast<const float4*>(xq + cur.off[u]);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) fma4(acc, cur.val[u], gv[u]);
+                cur = nxt;
+            }
+            if (row >= 0) {
+                const float cp = cps[row];
+                acc.x += cp; acc.y += cp; acc.z += cp; acc.w += cp;
+                const int idx = row * 2 + q;
+                const float4 xv = reinterpret_cast<const float4*>(xa)[idx];
+                const float4 yv = reinterpret_cast<const float4*>(ys)[idx];
+                float4 xo, yo;
+                gda_update4<GFUN>(xv, yv, acc, a.up, t0 + (uint32_t)k, (uint32_t)row, (uint32_t)(b0 + 4 * q), xo, yo);
+                reinterpret_cast<float4*>(xb)[idx] = xo;
+                reinterpret_cast<float4*>(ys)[idx] = yo;
+            }
         }
         __syncthreads();
         float* tmp = xa; xa = xb; xb = tmp;
+        xq = reinterpret_cast<const char*>(xa) + 16 * q;
     }
-    for (int e = threadIdx.x; e < total; e += RESIDENT_THREADS) { x_out[e] = xa[e]; y[e] = ys[e]; }
+
+    // ---- write the state back ----
+    for (int e = threadIdx.x; e < a.n * 2; e += blockDim.x) {
+        const int row = e >> 1, qq = e & 1;
+        if (b0 + 4 * qq < a.B) {
+            const size_t off = (size_t)row * a.B + b0 + 4 * qq;
+            *reinterpret_cast<float4*>(a.x_out + off) = reinterpret_cast<const float4*>(xa)[e];
+            *reinterpret_cast<float4*>(a.y + off) = reinterpret_cast<const float4*>(ys)[e];
+        }
+    }
+
+    // ---- S5: exact objective of x_hat = [x > 1/2] for the slab's restarts: sum_i x_hat_i ((Q_off x_hat)_i + c'_i) ----
+    acc_t obj4[4] = {0, 0, 0, 0};
+    for (int i = 0; i < a.groups_per_warp; ++i) {
+        const int g = slab_group(i, warp, warps);
+        if (g >= a.n_groups) break;
+        const int p0 = __ldg(a.goff + g) >> 2, p1 = __ldg(a.goff + g + 1) >> 2;
+        const int row = __ldg(a.grow + g * SLAB_ROWS + r);
+        float sf[4] = {0.f, 0.f, 0.f, 0.f};                  // fp32 row sums of val2 * x_hat_j (as spmm_score)
+        int si[4] = {0, 0, 0, 0};
+        for (int ps = p0; ps < p1; ++ps) {
+            const SlabPass e = slab_fetch<COMPACT>(a, cst, ps, r);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const float4 gv = *reinterpret_cast<const float4*>(xq + e.off[u]);
+                if (INTEGRAL) {
+                    const int vi = __float2int_rn(e.val[u]);
+                    si[0] += gv.x > 0.5f ? vi : 0; si[1] += gv.y > 0.5f ? vi : 0;
+                    si[2] += gv.z > 0.5f ? vi : 0; si[3] += gv.w > 0.5f ? vi : 0;
+                } else {
+                    const float v = e.val[u];
+                    sf[0] += gv.x > 0.5f ? v : 0.f; sf[1] += gv.y > 0.5f ? v : 0.f;
+                    sf[2] += gv.z > 0.5f ? v : 0.f; sf[3] += gv.w > 0.5f ? v : 0.f;
+                }
+            }
+        }
+        if (row >= 0) {
+            const float4 xi = reinterpret_cast<const float4*>(xa)[row * 2 + q];
+            const float cp = cps[row];
+            const bool on[4] = {xi.x > 0.5f, xi.y > 0.5f, xi.z > 0.5f, xi.w > 0.5f};
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (!on[u]) continue;
+                if (INTEGRAL) obj4[u] += (long long)(si[u] / 2) + (long long)__float2int_rn(cp);   // val2 = 2 Q_ij: even
+                else obj4[u] += 0.5 * (double)sf[u] + (double)cp;
+            }
+        }
+    }
+    // rows of the warp: lanes with the same quad, in a fixed butterfly order; then the warps in index order
+#pragma unroll
+    for (int o = 2; o < 32; o <<= 1)
+#pragma unroll
+        for (int u = 0; u < 4; ++u) obj4[u] += __shfl_xor_sync(0xffffffffu, obj4[u], o);
+    if (lane < 2)
+#pragma unroll
+        for (int u = 0; u < 4; ++u) red[warp * SLAB_S + 4 * lane + u] = obj4[u];
+    __syncthreads();
+    double my_best = CUDART_INF_SLAB;
+    if (threadIdx.x < SLAB_S) {
+        const int b = b0 + threadIdx.x;
+        int imp = 0;
+        if (b < a.B) {
+            acc_t t = red[threadIdx.x];
+            for (int w = 1; w < warps; ++w) t += red[w * SLAB_S + threadIdx.x];
+            const double v = (double)t;
+            double best = a.best_obj[b];
+            imp = v < best;
+            if (imp) { best = v; a.best_obj[b] = v; }
+            a.improved[b] = imp;
+            my_best = best;
+        }
+        s_imp[threadIdx.x] = imp;
+    }
+    if (warp == 0) {                                         // ticket of the evaluation (see finalize_kernel)
+        for (int o = 4; o > 0; o >>= 1) my_best = fmin(my_best, __shfl_xor_sync(0xffffffffu, my_best, o));
+        const int any = __any_sync(0xffffffffu, threadIdx.x < SLAB_S && s_imp[threadIdx.x & 7]);
+        if (lane == 0) {
+            a.block_min[blockIdx.x] = my_best;
+            if (any) atomicOr(&a.st->imp_accum, 1u);
+            __threadfence();
+            s_last = atomicAdd(&a.st->ticket, 1u) == gridDim.x - 1 ? 1u : 0u;
+        }
+    }
+    __syncthreads();
+    // ---- commit x_hat of the improved restarts (8 bytes per row, masked) ----
+    uint64_t mask = 0;
+#pragma unroll
+    for (int u = 0; u < SLAB_S; ++u) mask |= s_imp[u] ? (0xFFull << (8 * u)) : 0ull;
+    if (mask) {
+        for (int row = threadIdx.x; row < a.n; row += blockDim.x) {
+            const float4 v0 = reinterpret_cast<const float4*>(xa)[row * 2], v1 = reinterpret_cast<const float4*>(xa)[row * 2 + 1];
+            const uint64_t bits = (uint64_t)(v0.x > 0.5f) | ((uint64_t)(v0.y > 0.5f) << 8) | ((uint64_t)(v0.z > 0.5f) << 16) |
+                                  ((uint64_t)(v0.w > 0.5f) << 24) | ((uint64_t)(v1.x > 0.5f) << 32) | ((uint64_t)(v1.y > 0.5f) << 40) |
+                                  ((uint64_t)(v1.z > 0.5f) << 48) | ((uint64_t)(v1.w > 0.5f) << 56);
+            uint8_t* dst = a.x_bin + (size_t)row * a.B + b0;
+            if (b0 + SLAB_S <= a.B && (a.B & 7) == 0) {       // aligned 8-byte read-modify-write
+                uint64_t* d8 = reinterpret_cast<uint64_t*>(dst);
+                *d8 = (*d8 & ~mask) | (bits & mask);
+            } else {
+                for (int u = 0; u < SLAB_S; ++u)
+                    if (b0 + u < a.B && s_imp[u]) dst[u] = (uint8_t)((bits >> (8 * u)) & 1u);
+            }
+        }
+    }
+    if (s_last && warp == 0) {                               // every other block has finished (and read st->t long ago)
+        __threadfence();
+        double m = CUDART_INF_SLAB;
+        for (int kk = lane; kk < (int)gridDim.x; kk += 32) m = fmin(m, __ldcg(a.block_min + kk));
+        for (int o = 16; o > 0; o >>= 1) m = fmin(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (lane == 0) {
+            const uint32_t kk = a.st->n_eval;
+            if (a.trace_best && (int)kk < a.trace_cap) { a.trace_best[kk] = m; a.trace_ns[kk] = slab_globaltimer_ns(); }
+            a.st->n_eval = kk + 1;
+            a.st->t = t0 + (uint32_t)a.len;
+            a.st->any_improved = atomicExch(&a.st->imp_accum, 0u);
+            a.st->ticket = 0;
+        }
+    }
 }
 
 // S5 for sparse QUBO: partial[rb][b] = sum over the rows of block rb of x_hat_i ((Q_off x_hat)_i + c'_i)
@@ -428,10 +663,17 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
 
 int sparse_heavy_threshold() { return HEAVY_DEG; }
 
-// shared-memory opt-in of the resident kernels on the handle's device; called at create (never inside a capture)
+// shared-memory opt-in of the slab kernels on the handle's device; called at create (never inside a capture)
+template <int GFUN, bool INTEGRAL, bool COMPACT>
+static gda_status slab_opt_in() {
+    GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_chunk_slab<GFUN, INTEGRAL, COMPACT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SLAB_SMEM_LIMIT));
+    return GDA_OK;
+}
 gda_status sparse_configure(gda_problem*) {
-    GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_QUADRATIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));
-    GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_steps_resident<GDA_G_ENTROPY>, cudaFuncAttributeMaxDynamicSharedMemorySize, RESIDENT_SMEM));
+    GDA_TRY((slab_opt_in<GDA_G_QUADRATIC, true, true>()));   GDA_TRY((slab_opt_in<GDA_G_QUADRATIC, true, false>()));
+    GDA_TRY((slab_opt_in<GDA_G_QUADRATIC, false, true>()));  GDA_TRY((slab_opt_in<GDA_G_QUADRATIC, false, false>()));
+    GDA_TRY((slab_opt_in<GDA_G_ENTROPY, true, true>()));     GDA_TRY((slab_opt_in<GDA_G_ENTROPY, true, false>()));
+    GDA_TRY((slab_opt_in<GDA_G_ENTROPY, false, true>()));    GDA_TRY((slab_opt_in<GDA_G_ENTROPY, false, false>()));
     return GDA_OK;
 }
 
@@ -486,17 +728,167 @@ gda_status sparse_value_partials(gda_problem* p, int32_t B, const float* x, doub
     return GDA_OK;
 }
 
-// `len` steps in one launch when the state fits one block's shared memory; *done = 0 when it does not
-gda_status sparse_steps_resident(gda_problem* p, int32_t B, int32_t len, const float* x_in, float* y, float* x_out,
-                                 const UpdParams& up, const RunState* st, cudaStream_t s, int64_t* launches, int* done) {
+// ---- slab path, host side ------------------------------------------------------------------------------------------
+// Largest n whose slab state (x, x, y: 96 B per row; c': 4 B) and reduction scratch fit the 227 KB a CTA may use
+static size_t slab_smem_bytes(int n, int warps, int compact_passes) {       // compact_passes < 0: general structure (global memory)
+    const size_t nrow = (size_t)n + (compact_passes >= 0 ? 4 : 0);
+    return (2 * nrow * SLAB_S + (size_t)n * SLAB_S + ((n + 3) & ~3)) * sizeof(float) + (size_t)warps * SLAB_S * sizeof(double) +
+           (compact_passes >= 0 ? (size_t)compact_passes * SLAB_ROWS * sizeof(uint2) : 0);
+}
+
+// Build the sliced-ELL structure described above spmm_chunk_slab.  Called at create with the off-diagonal CSR
+// (val2 = 2 Q_ij).  Leaves p->slab_* null when n is too large for the slab kernel.
+gda_status sparse_build_slab(gda_problem* p, const std::vector<int32_t>& rowptr, const std::vector<int32_t>& col,
+                             const std::vector<float>& val2) {
+    const int n = p->n;
+    if (slab_smem_bytes(n, 32, -1) > (size_t)SLAB_SMEM_LIMIT) return GDA_OK;
+    // rows sorted by degree (descending, stable): the 16 rows of a group have similar lengths, so little padding
+    std::vector<int32_t> order(n);
+    for (int i = 0; i < n; ++i) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rowptr[a + 1] - rowptr[a] > rowptr[b + 1] - rowptr[b]; });
+    const int n_groups = (n + SLAB_ROWS - 1) / SLAB_ROWS;
+    std::vector<int32_t> goff(n_groups + 1, 0), grow((size_t)n_groups * SLAB_ROWS, -1);
+    std::vector<int2> ent;
+    std::vector<std::vector<int2>> sched(SLAB_ROWS);           // per row of the group: its slots in order
+    int64_t real_entries = 0;
+    for (int g = 0; g < n_groups; ++g) {
+        for (int r = 0; r < SLAB_ROWS; ++r) {
+            sched[r].clear();
+            if (g * SLAB_ROWS + r < n) grow[(size_t)g * SLAB_ROWS + r] = order[g * SLAB_ROWS + r];
+        }
+        // the four rows 4h .. 4h+3 share every LDS.128 pass: order their entries such that the four columns of a pass
+        // differ mod 4 (one 32-byte row of x per bank group).  Greedy: per pass, the assignment of distinct classes to
+        // the rows that uses up the most entries, ties to the largest remaining queues; zero-valued padding elsewhere.
+        for (int h = 0; h < SLAB_ROWS / 4; ++h) {
+            std::vector<int2> queue[4][4];                      // [row in the subgroup][column class]
+            int remaining = 0;
+            for (int j = 0; j < 4; ++j) {
+                const int row = grow[(size_t)g * SLAB_ROWS + 4 * h + j];
+                if (row < 0) continue;
+                for (int k = rowptr[row]; k < rowptr[row + 1]; ++k) {
+                    if (val2[k] == 0.0f) continue;              // explicit zeros contribute nothing
+                    int2 e;
+                    e.x = col[k] * (SLAB_S * 4);
+                    std::memcpy(&e.y, &val2[k], 4);
+                    queue[j][col[k] & 3].push_back(e);
+                    ++remaining;
+                }
+            }
+            real_entries += remaining;
+            static const int perms[24][4] = {{0,1,2,3},{0,1,3,2},{0,2,1,3},{0,2,3,1},{0,3,1,2},{0,3,2,1},{1,0,2,3},{1,0,3,2},
+                {1,2,0,3},{1,2,3,0},{1,3,0,2},{1,3,2,0},{2,0,1,3},{2,0,3,1},{2,1,0,3},{2,1,3,0},{2,3,0,1},{2,3,1,0},
+                {3,0,1,2},{3,0,2,1},{3,1,0,2},{3,1,2,0},{3,2,0,1},{3,2,1,0}};
+            while (remaining > 0) {
+                int best = 0; long best_score = -1;
+                for (int pi = 0; pi < 24; ++pi) {
+                    long used = 0, left = 0;
+                    for (int j = 0; j < 4; ++j) { const size_t sz = queue[j][perms[pi][j]].size(); used += sz > 0; left += (long)sz; }
+                    const long score = used * 1000000L + left;
+                    if (score > best_score) { best_score = score; best = pi; }
+                }
+                for (int j = 0; j < 4; ++j) {
+                    const int c = perms[best][j];
+                    int2 e;
+                    if (!queue[j][c].empty()) { e = queue[j][c].back(); queue[j][c].pop_back(); --remaining; }
+                    else { e.x = -1 - c; e.y = 0; }                                // padding of class c, value 0 (resolved below)
+                    sched[4 * h + j].push_back(e);
+                }
+            }
+        }
+        size_t len = 0;
+        for (int r = 0; r < SLAB_ROWS; ++r) len = std::max(len, sched[r].size());
+        len = (len + 3) & ~(size_t)3;                           // the kernel walks 4 slots at a time
+        for (size_t k = 0; k < len; ++k)
+            for (int r = 0; r < SLAB_ROWS; ++r) {
+                int2 e;
+                if (k < sched[r].size()) e = sched[r][k];
+                else { e.x = -1 - (int)((k + r) & 3); e.y = 0; }
+                ent.push_back(e);
+            }
+        goff[g + 1] = goff[g] + (int32_t)len;
+    }
+    // one more pass of padding that belongs to no group: what the "next pass" prefetch of the last pass reads
+    for (int k = 0; k < 4 * SLAB_ROWS; ++k) { int2 e; e.x = -1 - (k & 3); e.y = 0; ent.push_back(e); }
+    p->slab_groups = n_groups;
+    p->slab_slots = goff[n_groups] + 4;
+    p->slab_real = real_entries;
+    // compact form: every non-zero |val2| is the same number, columns (and the four zero rows n .. n+3 that padding
+    // entries gather) fit 12 bits, and the structure fits shared memory next to the state
+    uint32_t cbits = 0;
+    bool compact = n + 4 <= 4096;
+    for (size_t k = 0; k < ent.size() && compact; ++k) {
+        if (ent[k].x < 0) continue;
+        const uint32_t mag = (uint32_t)ent[k].y & 0x7FFFFFFFu;
+        if (cbits == 0) cbits = mag;
+        compact = mag == cbits;
+    }
+    const int n_pass = p->slab_slots / 4;
+    compact = compact && cbits != 0 && slab_smem_bytes(n, 32, n_pass) <= (size_t)SLAB_SMEM_LIMIT;
+    if (compact) {
+        std::vector<uint16_t> e16((size_t)n_pass * SLAB_ROWS * 4);
+        for (int ps = 0; ps < n_pass; ++ps)
+            for (int r = 0; r < SLAB_ROWS; ++r)
+                for (int u = 0; u < 4; ++u) {
+                    const int2 e = ent[((size_t)ps * 4 + u) * SLAB_ROWS + r];
+                    // padding of class c gathers the zero row n + j with (n + j) mod 4 == c
+                    const uint32_t colv = e.x < 0 ? (uint32_t)(n + ((((-1 - e.x) - n) % 4) + 4) % 4) : (uint32_t)(e.x / (SLAB_S * 4));
+                    e16[((size_t)ps * SLAB_ROWS + r) * 4 + u] = (uint16_t)(colv | (((uint32_t)e.y >> 31) << 15));
+                }
+        GDA_CUDA_TRY(cudaMalloc((void**)&p->d_slab_ent16, e16.size() * sizeof(uint16_t)));
+        GDA_CUDA_TRY(cudaMemcpy(p->d_slab_ent16, e16.data(), e16.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        p->slab_cbits = cbits;
+        p->slab_passes = n_pass;
+    }
+    // general form: padding gathers a real row of the wanted class (value 0)
+    for (auto& e : ent) if (e.x < 0) e.x = std::min(-1 - e.x, n - 1) * (SLAB_S * 4);
+    const size_t bytes = std::max<size_t>(ent.size(), 1) * sizeof(int2);
+    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_slab_ent, bytes));
+    if (!ent.empty()) GDA_CUDA_TRY(cudaMemcpy(p->d_slab_ent, ent.data(), ent.size() * sizeof(int2), cudaMemcpyHostToDevice));
+    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_slab_goff, goff.size() * sizeof(int32_t)));
+    GDA_CUDA_TRY(cudaMemcpy(p->d_slab_goff, goff.data(), goff.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_slab_grow, grow.size() * sizeof(int32_t)));
+    GDA_CUDA_TRY(cudaMemcpy(p->d_slab_grow, grow.data(), grow.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    if (const char* e = getenv("GDA_SPARSE_PATH")) p->slab_mode = !strcmp(e, "slab") ? 1 : !strcmp(e, "stream") ? -1 : 0;
+    return GDA_OK;
+}
+
+// Is the slab kernel the faster way to run a chunk at this B?  Its step costs the shared-memory gathers of one CTA
+// (slots x 16 rows x 32 B at 128 B per clock) times the number of waves of B / 8 CTAs; the streaming kernel one launch
+// (about 2.5 us) or its L2 gathers (nnz x B x 4 B at about 13 TB/s, measured on config 2), whichever is larger.
+static bool slab_wanted(const gda_problem* p, int32_t B) {
+    if (!p->d_slab_ent || p->slab_mode < 0) return false;
+    if (p->slab_mode > 0) return true;
+    const double ctas = (B + SLAB_S - 1) / SLAB_S, waves = std::ceil(ctas / p->num_sms);
+    const double t_slab = waves * ((double)p->slab_slots * SLAB_ROWS * 32.0 / 128.0 / 1.9e3 + 0.3);   // us
+    const double t_stream = std::max(2.5, (double)p->nnz * B * 4.0 / 13e6);                             // us
+    return t_slab < t_stream;
+}
+
+// One launch = `len` steps + the evaluation, when the slab kernel applies; *done = 0 when it does not.
+gda_status sparse_chunk_slab(gda_problem* p, int32_t B, int32_t len, const float* x_in, float* x_out, float* y,
+                             const UpdParams& up, cudaStream_t s, int64_t* launches, int* done) {
     *done = 0;
-    const long long total = (long long)p->n * B;
-    const size_t smem = ((size_t)total * 3 + (size_t)p->n * 2 + 1 + (size_t)p->nnz * 2) * sizeof(float);   // x, x, y, c', rowptr, col, val
-    if (total > RESIDENT_MAX || len <= 0 || smem > (size_t)RESIDENT_SMEM) return GDA_OK;
-    if (up.gfun == GDA_G_QUADRATIC)
-        spmm_steps_resident<GDA_G_QUADRATIC><<<1, RESIDENT_THREADS, smem, s>>>(p->n, B, (int)p->nnz, len, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x_in, y, x_out, up, st);
-    else
-        spmm_steps_resident<GDA_G_ENTROPY><<<1, RESIDENT_THREADS, smem, s>>>(p->n, B, (int)p->nnz, len, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x_in, y, x_out, up, st);
+    if (!slab_wanted(p, B)) return GDA_OK;
+    Workspace& ws = p->ws;
+    const int per_warp = (p->slab_groups + 31) / 32;
+    const int warps = std::max(1, (p->slab_groups + per_warp - 1) / per_warp);
+    const bool compact = p->d_slab_ent16 != nullptr;
+    SlabArgs a{};
+    a.n = p->n; a.B = B; a.len = len; a.n_groups = p->slab_groups; a.groups_per_warp = per_warp; a.n_pass = p->slab_slots / 4;
+    a.ent = p->d_slab_ent; a.ent16 = reinterpret_cast<const uint2*>(p->d_slab_ent16); a.cbits = p->slab_cbits;
+    a.goff = p->d_slab_goff; a.grow = p->d_slab_grow; a.cprime = p->d_cprime;
+    a.x_in = x_in; a.x_out = x_out; a.y = y; a.up = up; a.st = ws.state;
+    a.best_obj = ws.best_obj; a.improved = ws.improved; a.x_bin = ws.x_bin; a.block_min = ws.block_min;
+    a.trace_best = ws.trace_best; a.trace_ns = ws.trace_ns; a.trace_cap = ws.trace_cap;
+    const unsigned grid = (unsigned)((B + SLAB_S - 1) / SLAB_S);
+    const size_t smem = slab_smem_bytes(p->n, warps, compact ? a.n_pass : -1);
+    const bool quad = up.gfun == GDA_G_QUADRATIC;
+#define GDA_SLAB_LAUNCH(G, I, C) spmm_chunk_slab<G, I, C><<<grid, warps * 32, smem, s>>>(a)
+#define GDA_SLAB_IC(G) do { if (p->integral) { if (compact) GDA_SLAB_LAUNCH(G, true, true); else GDA_SLAB_LAUNCH(G, true, false); } \
+                            else { if (compact) GDA_SLAB_LAUNCH(G, false, true); else GDA_SLAB_LAUNCH(G, false, false); } } while (0)
+    if (quad) GDA_SLAB_IC(GDA_G_QUADRATIC); else GDA_SLAB_IC(GDA_G_ENTROPY);
+#undef GDA_SLAB_IC
+#undef GDA_SLAB_LAUNCH
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     *done = 1;

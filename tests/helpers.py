@@ -22,3 +22,18 @@ def hyper_kwargs(h, **over):
         d["dual"] = h.dual
     d.update(over)
     return d
+
+
+def create_problem(api, w_or_problem, sparse_path=None):
+    """gda_create_* for a workload (or a bare problem container).  `sparse_path` = "slab" | "stream" (or
+    workload.extra["sparse_path"]) forces the sparse launch path through GDA_SPARSE_PATH, which the library reads at
+    create; None leaves the choice to its cost model."""
+    import os
+    problem = getattr(w_or_problem, "problem", w_or_problem)
+    path = sparse_path or getattr(w_or_problem, "extra", {}).get("sparse_path")
+    if path:
+        os.environ["GDA_SPARSE_PATH"] = path
+    try:
+        return api.create_from_workload(problem)
+    finally:
+        os.environ.pop("GDA_SPARSE_PATH", None)

@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 
 from paper_2509_21064_b200 import workloads as wl
-from tests.helpers import oracle_problem, hyper_kwargs
+from tests.helpers import oracle_problem, hyper_kwargs, create_problem
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -51,6 +51,13 @@ def small_workloads():
     q.hyper.gfun = 0
     q.name += "_quadratic"
     out.append(q)
+    # small n takes the slab kernel (one launch per chunk, state on chip); the same instances through the streaming
+    # kernels (one launch per step: spmm_step_warp with and without the packed records, spmm_step_narrow)
+    for idx, kw in ((1, {}), (2, dict(B=132, n_scale=0.25)), (3, dict(B=260, n_scale=0.05))):
+        v = wl.config(idx, **kw)
+        v.name += "_stream"
+        v.extra["sparse_path"] = "stream"
+        out.append(v)
     return out
 
 
@@ -100,7 +107,7 @@ def grad_rel_err(G, Gref):
 @pytest.mark.parametrize("w", SMALL, ids=lambda w: w.name)
 def test_gradient_and_score_match_oracle(api, oracle, w):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B = w.problem.n, w.B
     rng = np.random.default_rng(5)
     X = rng.random((n, B), dtype=np.float32)
@@ -117,7 +124,7 @@ def test_gradient_and_score_match_oracle(api, oracle, w):
 @pytest.mark.parametrize("w", SMALL, ids=lambda w: w.name)
 def test_teacher_forced_steps(api, oracle, w):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, w.B, w.hyper
     x = dev(wl.x0_uniform(n, B, w.x0_seed))
     lam = torch.full((n, B), h.lambda0, dtype=torch.float32, device="cuda")
@@ -137,7 +144,7 @@ def test_teacher_forced_steps(api, oracle, w):
 @pytest.mark.parametrize("w", SMALL, ids=lambda w: w.name)
 def test_free_running_50_steps(api, oracle, w, delta):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, w.B, w.hyper
     X0 = wl.x0_uniform(n, B, w.x0_seed)
     r = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=50, eval_every=25, delta=delta), want_final=True)
@@ -166,7 +173,7 @@ def test_free_running_50_steps(api, oracle, w, delta):
 @pytest.mark.parametrize("w", SMALL, ids=lambda w: w.name)
 def test_full_run_objectives(api, oracle, w):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, w.B, w.hyper
     iters = min(h.iters, 3000)
     X0 = wl.x0_uniform(n, B, w.x0_seed)
@@ -278,8 +285,9 @@ def dense_rows_qubo(n, seed):
     return wl.QuboCSR(n, np.array(rowptr, np.int32), np.array(col, np.int32), np.array(val, np.float32), c)
 
 
+@pytest.mark.parametrize("path", ["slab", "stream"])
 @pytest.mark.parametrize("case", ["star_isolated", "general_int", "general_float", "n1", "packed_rows", "long_rows"])
-def test_sparse_edge_cases(api, oracle, case):
+def test_sparse_edge_cases(api, oracle, case, path):
     if case == "star_isolated":
         Pw, B = star_plus_isolated(700, 5), 8
     elif case == "packed_rows":
@@ -295,7 +303,7 @@ def test_sparse_edge_cases(api, oracle, case):
         Pw, B = wl.QuboCSR(1, np.array([0, 1], np.int32), np.array([0], np.int32), np.array([-2.0], np.float32),
                            np.array([1.0], np.float32)), 4
     OP = oracle_problem(Pw)
-    P = api.create_from_workload(Pw)
+    P = create_problem(api, Pw, sparse_path=path)
     assert P.info().integral == (0 if case == "general_float" else 1)
     n = Pw.n
     rng = np.random.default_rng(9)
@@ -355,11 +363,12 @@ def test_maxsat_edge_cases(api, oracle, case):
     P.destroy()
 
 
-def test_tie_break_at_exact_half_matches_oracle(api, oracle):
+@pytest.mark.parametrize("path", ["slab", "stream"])
+def test_tie_break_at_exact_half_matches_oracle(api, oracle, path):
     # Max-Cut at x = 1/2: zero gradient, so the side of the perturbation is the hash bit (R3)
     w = wl.config(1)
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w, sparse_path=path)
     n, B = w.problem.n, 8
     X = np.full((n, B), 0.5, dtype=np.float32)
     seed = (5 << 32) | 99
@@ -374,7 +383,7 @@ def test_tie_break_at_exact_half_matches_oracle(api, oracle):
 def test_zero_iterations_and_lambda_tensor_and_default_stream(api, oracle):
     w = wl.config(3, B=8, n_scale=0.01)
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, 8, w.hyper
     X0 = wl.x0_uniform(n, B, 3)
     r = P.run(dev(X0), 6.0, api.params_from_hyper(h, iters=0))                 # evaluates the start point
@@ -386,7 +395,7 @@ def test_zero_iterations_and_lambda_tensor_and_default_stream(api, oracle):
     s.synchronize()
     ref = oracle.run(OP, X0, lam, **okw(h, iters=3, eval_every=2))
     assert np.abs(r["x"].cpu().numpy() - ref["x"]).max() <= 3 * TOL_STEP
-    assert P.info().last_run_step_launches == 2     # n B = 1600 elements: the resident kernel, one launch per chunk (2 + 1 steps)
+    assert P.info().last_run_step_launches == 2     # small n: the slab kernel, one launch per chunk (2 + 1 steps)
     P.destroy()
 
 
@@ -394,7 +403,7 @@ def test_resumed_run_returns_its_own_slice_of_the_trace(api):
     """A resumed gda_run (x0 == NULL) appends to the evaluation trace of the run it continues; the caller's trace
     buffers receive THIS call's evaluations (gda_extra.trace_best / trace_ns), not the earliest entries."""
     w = wl.config(3, B=64, n_scale=0.05)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, w.B, w.hyper
     x0 = dev(wl.x0_uniform(n, B, 7))
     whole = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=600, eval_every=100), trace_cap=8)
@@ -423,7 +432,7 @@ def test_two_handles_from_two_threads(api, oracle):
     x0s = [dev(wl.x0_uniform(w.problem.n, w.B, w.x0_seed)) for w in ws]
     serial = []
     for w, prm, x0 in zip(ws, prms, x0s):
-        P = api.create_from_workload(w.problem)
+        P = create_problem(api, w)
         serial.append(P.run(x0, w.hyper.lambda0, prm)["obj"].cpu().numpy())
         P.destroy()
     results, errors = [None] * len(ws), []
@@ -452,7 +461,7 @@ def test_two_handles_from_two_threads(api, oracle):
 
 def test_run_host_matches_device_run(api):
     w = wl.config(3, B=16, n_scale=0.02)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     X0 = wl.x0_uniform(w.problem.n, 16, 4)
     prm = api.params_from_hyper(w.hyper, iters=300)
     a = P.run(dev(X0), 6.0, prm)
@@ -464,7 +473,7 @@ def test_run_host_matches_device_run(api):
 
 def test_run_arguments_are_validated(api):
     w = wl.config(1)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     x = dev(wl.x0_uniform(w.problem.n, 8, 1))
     for bad in (dict(alpha=0.0), dict(beta=-1.0), dict(delta=0.5), dict(eval_every=0), dict(iters=-1), dict(gfun=7)):
         with pytest.raises(api.GdaError) as e:
@@ -500,7 +509,7 @@ def dense_F_tolerance(Pw, x_bin):
 @pytest.mark.parametrize("w", DENSE, ids=lambda w: f"{w.name}_n{w.problem.n}_B{w.B}")
 def test_dense_gradient_and_score(api, oracle, w):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B = w.problem.n, w.B
     rng = np.random.default_rng(6)
     X = rng.random((n, B), dtype=np.float32)
@@ -522,7 +531,7 @@ def test_dense_gradient_and_score(api, oracle, w):
 @pytest.mark.parametrize("w", DENSE[:2], ids=lambda w: f"{w.name}_n{w.problem.n}_B{w.B}")
 def test_dense_teacher_forced_steps(api, oracle, w):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, w.B, w.hyper
     x = dev(wl.x0_uniform(n, B, w.x0_seed))
     lam = torch.full((n, B), h.lambda0, dtype=torch.float32, device="cuda")
@@ -546,7 +555,7 @@ def test_dense_teacher_forced_steps(api, oracle, w):
 @pytest.mark.parametrize("w", DENSE[:2], ids=lambda w: f"{w.name}_n{w.problem.n}_B{w.B}")
 def test_dense_full_run(api, oracle, w):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, w.B, w.hyper
     X0 = wl.x0_uniform(n, B, w.x0_seed)
     iters = 1500
@@ -585,7 +594,7 @@ def mu_tolerance(h, n, mu):
 @pytest.mark.parametrize("w", PDBO_S, ids=lambda w: w.name)
 def test_pdbo_s_teacher_forced_steps_and_resume(api, oracle, w):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, w.B, w.hyper
     x = dev(wl.x0_uniform(n, B, w.x0_seed))
     mu = dev(np.linspace(0.5 * h.lambda0, h.lambda0, B).astype(np.float32))      # a different multiplier per restart
@@ -618,7 +627,7 @@ def test_pdbo_s_teacher_forced_steps_and_resume(api, oracle, w):
 @pytest.mark.parametrize("w", PDBO_S, ids=lambda w: w.name)
 def test_pdbo_s_free_running_and_full_run(api, oracle, w):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, w.B, w.hyper
     X0 = wl.x0_uniform(n, B, w.x0_seed)
     if h.gfun == 0:                                            # (c) 50 free steps, quadratic g (see test_free_running_50_steps)
@@ -660,7 +669,7 @@ def test_pdbo_s_heavy_rows_and_argument_checks(api, oracle):
 def test_mis_objective_cardinality_and_feasibility(api, oracle, n, d, B):
     w = wl.mis(n, d, B=B, iters=2500)
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     h, E = w.hyper, w.problem.edges
     X0 = wl.x0_uniform(n, B, w.x0_seed)
     assert grad_rel_err(P.grad(dev(X0)).cpu().numpy(), oracle.grad(OP, X0.astype(np.float64))) <= TOL_STEP
@@ -686,7 +695,7 @@ def test_mis_objective_cardinality_and_feasibility(api, oracle, n, d, B):
 @pytest.mark.parametrize("w", [SMALL[1], SMALL[2], SMALL[3], SMALL[4]], ids=lambda w: w.name)
 def test_lagrangian_value_matches_oracle(api, oracle, w):
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, B, h = w.problem.n, w.B, w.hyper
     rng = np.random.default_rng(12)
     X = rng.random((n, B), dtype=np.float32)
@@ -727,10 +736,9 @@ def test_maxcut_dual_certificate(api, oracle):
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("B,scale", [(4, 0.25), (12, 0.1), (20, 0.1), (40, 0.05), (64, 0.05)])
 def test_few_restarts_narrow_kernel(api, oracle, B, scale):
-    w = wl.config(3, B=B, n_scale=scale)                        # n B > 12288: not the resident kernel
-    assert w.problem.n * B > 12288
+    w = wl.config(3, B=B, n_scale=scale)                        # forced to the streaming path (n is small enough for the slab kernel)
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w, sparse_path="stream")
     n, h = w.problem.n, w.hyper
     X0 = wl.x0_uniform(n, B, w.x0_seed)
     X0[5, 0], X0[6, B - 1] = 0.5, 0.5                            # exact 1/2: the tie-break hash sees (row, restart)
@@ -751,7 +759,7 @@ def test_few_restarts_maxsat(api, oracle, B, gfun):
     w = wl.config(5, B=B, n_scale=0.1)                          # n = 1000, the paper's Max-k-SAT runs use B = 10 (3 of 32 lanes)
     w.hyper.gfun = gfun
     OP = oracle_problem(w.problem)
-    P = api.create_from_workload(w.problem)
+    P = create_problem(api, w)
     n, h = w.problem.n, w.hyper
     X0 = wl.x0_uniform(n, B, w.x0_seed)
     assert grad_rel_err(P.grad(dev(X0)).cpu().numpy(), oracle.grad(OP, X0.astype(np.float64))) <= TOL_STEP
