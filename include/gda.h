@@ -37,7 +37,7 @@ typedef enum {
     GDA_ERR_INVALID_ARG = 1, /* null pointer, bad size, asymmetric Q, index out of range, bad parameter ... */
     GDA_ERR_ALLOC = 2,       /* host or device allocation failed */
     GDA_ERR_CUDA = 3,        /* a CUDA call or kernel launch failed (message has the CUDA error string) */
-    GDA_ERR_UNSUPPORTED = 4  /* valid request this build cannot serve (e.g. dense n not a multiple of 256) */
+    GDA_ERR_UNSUPPORTED = 4  /* valid request this build cannot serve (e.g. a dense problem without GDA_DENSE_BF16) */
 } gda_status;
 
 /* binarity function g (default quadratic; entropy for Max-k-SAT, 580/592) */
@@ -64,8 +64,9 @@ gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, const int32_t* 
 
 /* gda_create_qubo_dense: HOST Q row-major [n][n] (symmetric), HOST c[n] or NULL.  flags must contain
  *   GDA_DENSE_BF16: Q is rounded to bf16 (lossless when Q is bf16-representable, reading R13)
- *   and the gradient is a tcgen05 GEMM with fp32 accumulation.  UNSUPPORTED: n not a multiple of 256 or
- *   flags without GDA_DENSE_BF16.  gda_run on a dense problem needs B to be a multiple of 128. */
+ *   and the gradient is a tcgen05 GEMM with fp32 accumulation.  UNSUPPORTED: flags without GDA_DENSE_BF16.
+ *   Any n > 0 and any B (a multiple of 4) are served: internally n is zero-padded to a multiple of 256 and B to a
+ *   multiple of 128 (the GEMM tile), which costs the padded work but changes no result. */
 gda_status gda_create_qubo_dense(int32_t n, const float* Q, const float* c, int32_t flags, gda_problem** out);
 
 /* Weighted MaxSAT: F(x) = sum_j w_j [clause j unsatisfied] = sum_j w_j prod_{l in C_j} p_l(x)
@@ -85,7 +86,7 @@ gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cptr, const in
  *   x_bin        DEVICE uint8 [n][B]: per restart the LABELS (argmax_j Z_ji, lowest j on ties) of the best evaluation
  *   obj          DEVICE double [B]: Tr(Xh W Xh^T) of those labels (exact integers for integer weights)
  *   extra->x_final [k][n][B] logits Z^T; params->delta is ignored (no perturbation is described for this variant);
- *   params->dual must be GDA_DUAL_PER_VARIABLE.  gda_grad / gda_score / gda_lagrangian: UNSUPPORTED.
+ *   params->dual must be GDA_DUAL_PER_VARIABLE.  gda_grad / gda_lagrangian: UNSUPPORTED.
  * INVALID_ARG: as gda_create_qubo_csr, plus a non-zero diagonal entry and k outside [2, 8]. */
 gda_status gda_create_maxkcut(int32_t n, int32_t k, const int32_t* rowptr, const int32_t* col, const float* val,
                               gda_problem** out);
@@ -153,7 +154,10 @@ gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, const float*
 
 /* ---- single steps of the path, exposed for parity tests and profiling ---------------------------------
  * gda_grad:  G = grad f(X), DEVICE fp32 [n][B] in and out (S1 sparse / S2 dense / S3 MaxSAT of DESIGN.md).
- * gda_score: obj[b] = F(x_hat), x_hat = [X[:,b] > 1/2]; DEVICE fp32 X [n][B], DEVICE double obj[B] (S5). */
+ *            Max-k-Cut: UNSUPPORTED.
+ * gda_score: obj[b] = F(x_hat), x_hat = [X[:,b] > 1/2]; DEVICE fp32 X [n][B], DEVICE double obj[B] (S5).
+ *            Max-k-Cut: X is the logits [k][n][B], scored by their labels argmax_j Z_ji (lowest j on ties).
+ * On a DENSE problem both (and gda_lagrangian) use the handle's run state as scratch: a later gda_run must pass x0. */
 gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float* G, void* stream);
 gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, void* stream);
 
@@ -162,8 +166,8 @@ gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, voi
  * lambda DEVICE fp32 [n][B] or NULL -> every y_i = lambda_scalar; gfun / log_eps as in gda_params; DEVICE double out[B].
  * This is the value behind the dual certificate of PAPER.md:1105-1114: for y with f_y = L(., y) convex (Max-Cut:
  * y_i >= -lambda_min(W)), run gda_run with beta = 0 (the multipliers stay at lambda0) until x has converged; then
- * out[b] <= min F, i.e. -out[b] is an upper bound on the maximum cut.  Sparse QUBO and MaxSAT problems (dense:
- * UNSUPPORTED). */
+ * out[b] <= min F, i.e. -out[b] is an upper bound on the maximum cut.  Dense problems: f comes from the tcgen05
+ * gradient, f = sum_i x_i (G_i + c'_i) / 2, i.e. with the bf16 operand's error (reading R13).  Max-k-Cut: UNSUPPORTED. */
 gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, const float* lambda, float lambda_scalar,
                           int32_t gfun, float log_eps, double* out, void* stream);
 

@@ -228,11 +228,13 @@ class Problem:
         return G
 
     def score(self, x, stream=None):
+        """gda_score: x [n][B] (Max-k-Cut: the logits [k][n][B], scored by their argmax labels)."""
         import torch
-        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.shape[0] == self.n
-        obj = torch.empty(x.shape[1], dtype=torch.float64, device=x.device)
+        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()
+        assert tuple(x.shape[:-1]) == ((self.k, self.n) if self.k else (self.n,))
+        obj = torch.empty(x.shape[-1], dtype=torch.float64, device=x.device)
         s = torch.cuda.current_stream(x.device).cuda_stream if stream is None else stream
-        _check(lib().gda_score(self._h, x.shape[1], x.data_ptr(), obj.data_ptr(), s))
+        _check(lib().gda_score(self._h, x.shape[-1], x.data_ptr(), obj.data_ptr(), s))
         return obj
 
     def lagrangian(self, x, lam, gfun=G_QUADRATIC, log_eps=1e-6, stream=None):

@@ -149,7 +149,7 @@ extern "C" gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, cons
 
     gda_problem* p = new (std::nothrow) gda_problem();
     if (!p) { gda_set_error("host allocation failed"); return GDA_ERR_ALLOC; }
-    p->kind = GDA_KIND_SPARSE; p->n = n; p->nnz = (int64_t)h_col.size(); p->integral = integral ? 1 : 0;
+    p->kind = GDA_KIND_SPARSE; p->n = n; p->n_pad = n; p->nnz = (int64_t)h_col.size(); p->integral = integral ? 1 : 0;
     p->max_deg = max_deg;
     gda_status st = device_setup(p);
     if (st == GDA_OK) st = sparse_configure(p);
@@ -222,7 +222,6 @@ extern "C" gda_status gda_create_qubo_dense(int32_t n, const float* Q, const flo
     GDA_REQUIRE(n > 0, "gda_create_qubo_dense: n must be > 0 (got %d)", n);
     GDA_REQUIRE(Q != nullptr, "gda_create_qubo_dense: Q is NULL");
     if (!(flags & GDA_DENSE_BF16)) { gda_set_error("gda_create_qubo_dense: only GDA_DENSE_BF16 is implemented"); return GDA_ERR_UNSUPPORTED; }
-    if (n % 256 != 0) { gda_set_error("gda_create_qubo_dense: n must be a multiple of 256 (got %d)", n); return GDA_ERR_UNSUPPORTED; }
     for (int i = 0; i < n; ++i) {
         GDA_REQUIRE(!c || std::isfinite(c[i]), "gda_create_qubo_dense: non-finite c[%d]", i);
         for (int j = i; j < n; ++j) {
@@ -233,7 +232,7 @@ extern "C" gda_status gda_create_qubo_dense(int32_t n, const float* Q, const flo
     }
     gda_problem* p = new (std::nothrow) gda_problem();
     if (!p) { gda_set_error("host allocation failed"); return GDA_ERR_ALLOC; }
-    p->kind = GDA_KIND_DENSE; p->n = n; p->nnz = (int64_t)n * n; p->integral = 0;
+    p->kind = GDA_KIND_DENSE; p->n = n; p->n_pad = (n + 255) / 256 * 256; p->nnz = (int64_t)n * n; p->integral = 0;
     gda_status st = device_setup(p);
     if (st == GDA_OK) st = dense_prepare(p, Q, c);
     if (st != GDA_OK) { gda_destroy(p); return st; }
@@ -300,7 +299,7 @@ extern "C" gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cpt
     }
     gda_problem* p = new (std::nothrow) gda_problem();
     if (!p) { gda_set_error("host allocation failed"); return GDA_ERR_ALLOC; }
-    p->kind = GDA_KIND_MAXSAT; p->n = n; p->m = m; p->nnz = L; p->integral = integral ? 1 : 0;
+    p->kind = GDA_KIND_MAXSAT; p->n = n; p->n_pad = n; p->m = m; p->nnz = L; p->integral = integral ? 1 : 0;
     p->kw = kw; p->kmax = kmax; p->kmin = kmin;
     gda_status st = device_setup(p);
     if (st == GDA_OK) st = upload(&p->d_vptr, h_vptr);
@@ -347,7 +346,7 @@ static void free_workspace(gda_problem* p) {
     cudaFree(ws.obj_now); cudaFree(ws.improved); cudaFree(ws.partial); cudaFree(ws.state);
     cudaFree(ws.best_restart); cudaFree(ws.best_val); cudaFree(ws.trace_best); cudaFree(ws.trace_ns);
     cudaFree(ws.zt[0]); cudaFree(ws.zt[1]); cudaFree(ws.z); cudaFree(ws.lab);
-    cudaFree(ws.mu[0]); cudaFree(ws.mu[1]); cudaFree(ws.gpart); cudaFree(ws.block_min);
+    cudaFree(ws.mu[0]); cudaFree(ws.mu[1]); cudaFree(ws.gpart); cudaFree(ws.block_min); cudaFree(ws.gacc);
     ws = Workspace();
 }
 
@@ -391,12 +390,15 @@ static gda_status dmalloc(T** ptr, size_t count) {
 
 static const int32_t TRACE_CAP = 4096;
 
+static int32_t lead_dim(const gda_problem* p, int32_t B) { return p->kind == GDA_KIND_DENSE ? (B + 127) / 128 * 128 : B; }
+
 static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     Workspace& ws = p->ws;
     if (ws.B == B) return GDA_OK;
     wait_for_handle(p);
     free_workspace(p);
-    const size_t elems = (size_t)p->n * B;
+    const int32_t ld = lead_dim(p, B);                                            // dense: full 128-restart tiles
+    const size_t elems = (size_t)p->n_pad * ld;
     const size_t xelems = p->kind == GDA_KIND_KCUT ? elems * p->kparts : elems;   // Max-k-Cut: k planes
     gda_status st = GDA_OK;
     if (p->kind != GDA_KIND_DENSE) {
@@ -412,17 +414,19 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     if (st == GDA_OK) st = dmalloc(&ws.x[0], xelems);
     if (st == GDA_OK) st = dmalloc(&ws.y, elems);
     if (st == GDA_OK) st = dmalloc(&ws.x_bin, elems);
-    if (st == GDA_OK) st = dmalloc(&ws.best_obj, (size_t)B);
-    if (st == GDA_OK) st = dmalloc(&ws.obj_now, (size_t)B);
-    if (st == GDA_OK) st = dmalloc(&ws.improved, (size_t)B);
-    ws.n_part = num_partials(p, B);
+    if (st == GDA_OK) st = dmalloc(&ws.best_obj, (size_t)ld);
+    if (st == GDA_OK) st = dmalloc(&ws.obj_now, (size_t)ld);
+    if (st == GDA_OK) st = dmalloc(&ws.improved, (size_t)ld);
+    ws.B = B; ws.ld = ld;                                      // the partial counts below depend on them
+    ws.n_part = num_partials(p, ld);
     // + room for the y g(x) partial rows of gda_lagrangian
-    if (st == GDA_OK) st = dmalloc((double**)&ws.partial, ((size_t)ws.n_part + (size_t)(p->n + 63) / 64) * B);
+    if (st == GDA_OK) st = dmalloc((double**)&ws.partial, ((size_t)ws.n_part + (size_t)(p->n_pad + 63) / 64 * 2) * ld);
     if (p->kind != GDA_KIND_KCUT) {                           // PDBO-s state (a few rows of B floats)
-        ws.n_gpart = p->kind == GDA_KIND_SPARSE ? sparse_num_gparts(p) : p->kind == GDA_KIND_MAXSAT ? maxsat_num_gparts(p) : p->n / 128;
-        if (st == GDA_OK) st = dmalloc(&ws.mu[0], (size_t)B);
-        if (st == GDA_OK) st = dmalloc(&ws.mu[1], (size_t)B);
-        if (st == GDA_OK) st = dmalloc(&ws.gpart, (size_t)ws.n_gpart * B);
+        ws.n_gpart = p->kind == GDA_KIND_DENSE ? p->n_pad / 128 : p->kind == GDA_KIND_MAXSAT ? maxsat_num_gparts(p) : 0;
+        if (st == GDA_OK) st = dmalloc(&ws.mu[0], (size_t)ld);
+        if (st == GDA_OK) st = dmalloc(&ws.mu[1], (size_t)ld);
+        if (st == GDA_OK) st = dmalloc(&ws.gpart, (size_t)ws.n_gpart * ld);
+        if (st == GDA_OK && p->kind == GDA_KIND_SPARSE) st = dmalloc(&ws.gacc, (size_t)GDA_GACC_WAYS * B);
     }
     if (st == GDA_OK) st = dmalloc(&ws.state, 1);
     if (st == GDA_OK) st = dmalloc(&ws.block_min, (size_t)(B + 31) / 32);
@@ -432,7 +436,18 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     if (st == GDA_OK) st = dmalloc(&ws.trace_best, (size_t)TRACE_CAP);
     if (st == GDA_OK) st = dmalloc(&ws.trace_ns, (size_t)TRACE_CAP);
     if (st != GDA_OK) { free_workspace(p); return st; }
-    ws.B = B;
+    return GDA_OK;
+}
+
+// [rows][ld] in the workspace -> [rows][B] at the caller (host or device)
+static gda_status copy_out(void* dst, size_t B, const void* src, size_t ld, size_t rows, size_t esz, cudaStream_t s) {
+    if (ld == B) GDA_CUDA_TRY(cudaMemcpyAsync(dst, src, rows * B * esz, cudaMemcpyDefault, s));
+    else GDA_CUDA_TRY(cudaMemcpy2DAsync(dst, B * esz, src, ld * esz, B * esz, rows, cudaMemcpyDefault, s));
+    return GDA_OK;
+}
+static gda_status copy_in(void* dst, size_t ld, const void* src, size_t B, size_t rows, size_t esz, cudaStream_t s) {
+    if (ld == B) GDA_CUDA_TRY(cudaMemcpyAsync(dst, src, rows * B * esz, cudaMemcpyDefault, s));
+    else GDA_CUDA_TRY(cudaMemcpy2DAsync(dst, ld * esz, src, B * esz, B * esz, rows, cudaMemcpyDefault, s));
     return GDA_OK;
 }
 
@@ -485,7 +500,7 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     for (int k = 0; k < len; ++k) {
         int64_t before = *launches;
         ScalarDual sd;                                        // PDBO-s: mu follows the parity of x
-        if (scalar) { sd.mu = ws.mu[cur]; sd.gpart = ws.gpart; }
+        if (scalar) { sd.mu = ws.mu[cur]; sd.gpart = ws.gpart; sd.gacc = ws.gacc; sd.B = B; }
         if (p->kind == GDA_KIND_SPARSE)
             GDA_TRY(sparse_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         else if (p->kind == GDA_KIND_MAXSAT)
@@ -493,8 +508,11 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
         else if (p->kind == GDA_KIND_KCUT)
             GDA_TRY(kcut_step(p, B, ws.x[cur], ws.z, ws.y, ws.x[cur ^ 1], up, s, launches));
         else
-            GDA_TRY(dense_step(p, B, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
-        if (scalar) GDA_TRY(gsum_reduce(B, ws.gpart, ws.n_gpart, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
+            GDA_TRY(dense_step(p, ws.ld, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
+        if (scalar && p->kind != GDA_KIND_SPARSE)
+            GDA_TRY(gsum_reduce(ws.ld, ws.gpart, ws.n_gpart, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
+        else if (scalar)
+            GDA_TRY(mu_finalize(B, ws.gacc, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
         *step_launches += *launches - before;
         cur ^= 1;
     }
@@ -503,11 +521,11 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
     else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
     else if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_score_partials(p, B, ws.z, ws.lab, ws.partial, &n_part, s, launches));
-    else { ws.score_scratch = cur ^ 1; GDA_TRY(dense_score_partials(p, B, xcur, ws.partial, &n_part, s, launches)); }
-    GDA_TRY(eval_finalize(p, B, ws.partial, n_part, ws.obj_now, ws.best_obj, ws.improved, ws.state, ws.trace_best,
+    else { ws.score_scratch = cur ^ 1; GDA_TRY(dense_score_partials(p, ws.ld, xcur, ws.partial, &n_part, s, launches)); }
+    GDA_TRY(eval_finalize(p, B, ws.ld, ws.partial, n_part, ws.obj_now, ws.best_obj, ws.improved, ws.state, ws.trace_best,
                           ws.trace_ns, ws.trace_cap, (uint32_t)len, s, launches));
     if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_commit(p, B, ws.lab, ws.improved, ws.x_bin, s, launches));
-    else GDA_TRY(eval_commit(p, B, xcur, ws.improved, ws.x_bin, s, launches));
+    else GDA_TRY(eval_commit(p, ws.ld, xcur, ws.improved, ws.x_bin, s, launches));
     return GDA_OK;
 }
 
@@ -593,11 +611,7 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
         gda_set_error("gda_run: Max-k-Cut problems need GDA_DUAL_PER_VARIABLE");
         return GDA_ERR_UNSUPPORTED;
     }
-    if (p->kind == GDA_KIND_DENSE && B % 128 != 0) {
-        gda_set_error("gda_run: the dense path needs B to be a multiple of 128 (got %d)", B);
-        return GDA_ERR_UNSUPPORTED;
-    }
-    if ((int64_t)p->n * (int64_t)B * (p->kind == GDA_KIND_KCUT ? p->kparts : 1) >= ((int64_t)1 << 30)) {
+    if ((int64_t)p->n_pad * (int64_t)lead_dim(p, B) * (p->kind == GDA_KIND_KCUT ? p->kparts : 1) >= ((int64_t)1 << 30)) {
         gda_set_error("gda_run: n * B must be below 2^30 (got %lld): kernels use 32-bit byte offsets into X", (long long)p->n * B);
         return GDA_ERR_UNSUPPORTED;
     }
@@ -625,7 +639,7 @@ static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const flo
         ws.n_eval_host = 0;
         GDA_TRY(run_init(p, B, x0, lambda0, lambda0_scalar, (uint32_t)prm->t0, s, &p->last_launches));
         if (p->kind == GDA_KIND_DENSE)
-            GDA_TRY(dense_make_operand(p, B, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
+            GDA_TRY(dense_make_operand(p, ws.ld, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
         if (p->kind == GDA_KIND_KCUT)                       // run_init put the logits in z; x[0] = SoftMax(z)
             GDA_TRY(kcut_softmax(p, B, ws.z, ws.x[0], s, &p->last_launches));
     } else {
@@ -644,17 +658,18 @@ static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const flo
     ws.parity = parity;
     ws.has_state = true;
     const float* xfin = (p->kind == GDA_KIND_DENSE) ? ws.x[0] : ws.x[parity];
-    GDA_CUDA_TRY(cudaMemcpyAsync(x_bin, ws.x_bin, elems, cudaMemcpyDefault, s));
+    const size_t ld = (size_t)ws.ld, n = (size_t)p->n;
+    GDA_TRY(copy_out(x_bin, (size_t)B, ws.x_bin, ld, n, 1, s));
     GDA_CUDA_TRY(cudaMemcpyAsync(obj, ws.best_obj, (size_t)B * sizeof(double), cudaMemcpyDefault, s));
     GDA_CUDA_TRY(cudaMemcpyAsync(best_restart, ws.best_restart, sizeof(int32_t), cudaMemcpyDefault, s));
     if (extra) {
         if (extra->x_final && p->kind == GDA_KIND_KCUT)      // the logits Z^T, [k][n][B]
             GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, ws.z, elems * p->kparts * sizeof(float), cudaMemcpyDeviceToDevice, s));
-        else if (extra->x_final) GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, xfin, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+        else if (extra->x_final) GDA_TRY(copy_out(extra->x_final, (size_t)B, xfin, ld, n, sizeof(float), s));
         if (extra->lambda_final && prm->dual == GDA_DUAL_SCALAR)          // mu^T, [B]
             GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.mu[parity], (size_t)B * sizeof(float), cudaMemcpyDeviceToDevice, s));
         else if (extra->lambda_final)
-            GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.y, elems * sizeof(float), cudaMemcpyDeviceToDevice, s));
+            GDA_TRY(copy_out(extra->lambda_final, (size_t)B, ws.y, ld, n, sizeof(float), s));
         if (extra->ones) GDA_TRY(eval_count_ones(p, B, ws.x_bin, extra->ones, s, &p->last_launches));
         if (extra->best_obj) GDA_CUDA_TRY(cudaMemcpyAsync(extra->best_obj, ws.best_val, sizeof(double), cudaMemcpyDeviceToDevice, s));
         // THIS call's evaluations: a resumed run appends to the trace of the run it continues (n_eval is not reset)
@@ -692,31 +707,49 @@ extern "C" gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float*
     GDA_REQUIRE(p != nullptr && x != nullptr && G != nullptr, "gda_grad: null argument");
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_grad: B must be a positive multiple of 4 (got %d)", B);
     if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_grad: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
-    if (p->kind == GDA_KIND_DENSE && B % 128 != 0) { gda_set_error("gda_grad: the dense path needs B %% 128 == 0"); return GDA_ERR_UNSUPPORTED; }
     GDA_ON_DEVICE(p);
     cudaStream_t user, s;
     if (p->kind == GDA_KIND_DENSE) GDA_TRY(ensure_workspace(p, B));
     GDA_TRY(pick_stream(p, stream, &user, &s));
     if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_grad(p, B, x, G, s));
     else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_grad(p, B, x, G, s));
-    else GDA_TRY(dense_grad(p, B, x, G, s));
+    else {
+        Workspace& ws = p->ws;                               // the handle's run state is scratch here (has_state = false)
+        if (ws.ld == B && p->n_pad == p->n) {
+            GDA_TRY(dense_grad(p, B, x, G, s));
+        } else {                                             // ragged sizes: through the zero-padded workspace arrays
+            GDA_CUDA_TRY(cudaMemsetAsync(ws.x[0], 0, (size_t)p->n_pad * ws.ld * sizeof(float), s));
+            GDA_TRY(copy_in(ws.x[0], (size_t)ws.ld, x, (size_t)B, (size_t)p->n, sizeof(float), s));
+            GDA_TRY(dense_grad(p, ws.ld, ws.x[0], ws.y, s));
+            GDA_TRY(copy_out(G, (size_t)B, ws.y, (size_t)ws.ld, (size_t)p->n, sizeof(float), s));
+        }
+    }
     return join_stream(p, user, s);
 }
 
 extern "C" gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, void* stream) {
     GDA_REQUIRE(p != nullptr && x != nullptr && obj != nullptr, "gda_score: null argument");
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_score: B must be a positive multiple of 4 (got %d)", B);
-    if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_score: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
-    if (p->kind == GDA_KIND_DENSE && B % 128 != 0) { gda_set_error("gda_score: the dense path needs B %% 128 == 0"); return GDA_ERR_UNSUPPORTED; }
     GDA_ON_DEVICE(p);
     GDA_TRY(ensure_workspace(p, B));
     cudaStream_t user, s;
     GDA_TRY(pick_stream(p, stream, &user, &s));
+    Workspace& ws = p->ws;
     int32_t n_part = 0;
-    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr));
-    else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr));
-    else { p->ws.has_state = false; p->ws.score_scratch = 1; GDA_TRY(dense_score_partials(p, B, x, p->ws.partial, &n_part, s, nullptr)); }
-    GDA_TRY(score_reduce(p, B, p->ws.partial, n_part, obj, s));
+    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, x, ws.partial, &n_part, s, nullptr));
+    else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, x, ws.partial, &n_part, s, nullptr));
+    else if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_score_partials(p, B, x, ws.lab, ws.partial, &n_part, s, nullptr));   // x = logits [k][n][B]
+    else {
+        ws.has_state = false; ws.score_scratch = 1;
+        const float* xs = x;
+        if (ws.ld != B || p->n_pad != p->n) {                // ragged sizes: zero-padded copy (x_hat = 0 adds nothing)
+            GDA_CUDA_TRY(cudaMemsetAsync(ws.x[0], 0, (size_t)p->n_pad * ws.ld * sizeof(float), s));
+            GDA_TRY(copy_in(ws.x[0], (size_t)ws.ld, x, (size_t)B, (size_t)p->n, sizeof(float), s));
+            xs = ws.x[0];
+        }
+        GDA_TRY(dense_score_partials(p, ws.ld, xs, ws.partial, &n_part, s, nullptr));
+    }
+    GDA_TRY(score_reduce(p, B, ws.ld, ws.partial, n_part, obj, s));
     return join_stream(p, user, s);
 }
 
@@ -734,16 +767,35 @@ extern "C" gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, 
     GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_lagrangian: B must be a positive multiple of 4 (got %d)", B);
     GDA_REQUIRE(gfun == GDA_G_QUADRATIC || gfun == GDA_G_ENTROPY, "gda_lagrangian: unknown gfun %d", gfun);
     if (gfun == GDA_G_ENTROPY) GDA_REQUIRE(log_eps > 0.0f && log_eps < 0.5f, "gda_lagrangian: log_eps must be in (0, 1/2)");
-    if (p->kind == GDA_KIND_DENSE || p->kind == GDA_KIND_KCUT) { gda_set_error("gda_lagrangian: sparse QUBO and MaxSAT problems only"); return GDA_ERR_UNSUPPORTED; }
+    if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_lagrangian: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
     GDA_ON_DEVICE(p);
     GDA_TRY(ensure_workspace(p, B));
     cudaStream_t user, s;
     GDA_TRY(pick_stream(p, stream, &user, &s));
-    double* part = static_cast<double*>(p->ws.partial);
+    Workspace& ws = p->ws;
+    double* part = static_cast<double*>(ws.partial);
     int32_t n_f = 0, n_g = 0;
+    if (p->kind == GDA_KIND_DENSE) {
+        // f(x) = sum_i x_i (G_i + c'_i) / 2 with G = grad f(x) from the tcgen05 GEMM (bf16 operand: reading R13); the
+        // run state of the handle is scratch here, as for gda_grad
+        ws.has_state = false;
+        const size_t ld = (size_t)ws.ld;
+        GDA_CUDA_TRY(cudaMemsetAsync(ws.x[0], 0, (size_t)p->n_pad * ld * sizeof(float), s));
+        GDA_TRY(copy_in(ws.x[0], ld, x, (size_t)B, (size_t)p->n, sizeof(float), s));
+        GDA_TRY(dense_grad(p, ws.ld, ws.x[0], ws.y, s));
+        GDA_TRY(eval_xg_partials(p, ws.ld, ws.x[0], ws.y, part, &n_f, s));
+        const float* lam = lambda;
+        if (lambda && ld != (size_t)B) {                     // y at the padded stride: G's buffer is free once eval_xg_partials has run
+            GDA_TRY(copy_in(ws.y, ld, lambda, (size_t)B, (size_t)p->n, sizeof(float), s));
+            lam = ws.y;
+        }
+        GDA_TRY(eval_yg_partials(p, p->n, ws.ld, ws.x[0], lam, lambda_scalar, gfun, log_eps, part + (size_t)n_f * ld, &n_g, s));
+        GDA_TRY(eval_sum_partials(B, ws.ld, part, n_f + n_g, out, s));
+        return join_stream(p, user, s);
+    }
     if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_value_partials(p, B, x, part, &n_f, s));
     else GDA_TRY(maxsat_value_partials(p, B, x, part, &n_f, s));
-    GDA_TRY(eval_yg_partials(p, B, x, lambda, lambda_scalar, gfun, log_eps, part + (size_t)n_f * B, &n_g, s));
-    GDA_TRY(eval_sum_partials(B, part, n_f + n_g, out, s));
+    GDA_TRY(eval_yg_partials(p, p->n, B, x, lambda, lambda_scalar, gfun, log_eps, part + (size_t)n_f * B, &n_g, s));
+    GDA_TRY(eval_sum_partials(B, B, part, n_f + n_g, out, s));
     return join_stream(p, user, s);
 }

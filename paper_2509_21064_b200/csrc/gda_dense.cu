@@ -646,7 +646,7 @@ gda_status z_maps(gda_problem* p, int32_t B, const __nv_bfloat16* zt, const CUte
         if (h->z_ptr[k] == zt && h->z_B == B) { *out = &h->tmap_z[k]; return GDA_OK; }
     if (h->z_B != B) { h->z_ptr[0] = h->z_ptr[1] = nullptr; h->z_B = B; }
     const int k = h->z_ptr[0] == nullptr ? 0 : 1;
-    GDA_TRY(make_tmap(&h->tmap_z[k], zt, (uint64_t)B, (uint64_t)p->n, BBOX));
+    GDA_TRY(make_tmap(&h->tmap_z[k], zt, (uint64_t)B, (uint64_t)p->n_pad, BBOX));
     h->z_ptr[k] = zt;
     *out = &h->tmap_z[k];
     return GDA_OK;
@@ -654,16 +654,20 @@ gda_status z_maps(gda_problem* p, int32_t B, const __nv_bfloat16* zt, const CUte
 
 }  // namespace
 
+// Ragged sizes are served by ZERO PADDING: n is rounded up to a multiple of 256 and (in the workspace) B to a multiple
+// of 128, so the kernels only ever see full tiles.  A padding variable has a zero row and column in Q_off, the start
+// value x = 0 and a huge constant gradient (h = c' = 1e30): Eq. 6 keeps it at x = 0 (clip), where g(0) = 0, g'(0) is
+// finite, the perturbation band is far away and x_hat = 0 adds nothing to F; its operand entry z = -1/2 multiplies
+// zeros.  Padding restarts run like any other and are never read.
 gda_status dense_prepare(gda_problem* p, const float* Q, const float* c) {
-    const int n = p->n;
-    if (n % BN != 0) { gda_set_error("dense path: n must be a multiple of %d (got %d)", BN, n); return GDA_ERR_UNSUPPORTED; }
-    std::vector<__nv_bfloat16> qb((size_t)n * n);
-    std::vector<float> hvec(n), cp(n);
+    const int n = p->n, np = p->n_pad;
+    std::vector<__nv_bfloat16> qb((size_t)np * np, __float2bfloat16_rn(0.0f));
+    std::vector<float> hvec(np, 1e30f), cp(np, 1e30f);
     for (int i = 0; i < n; ++i) {
         double rs = 0.0;
         for (int j = 0; j < n; ++j) {
             const __nv_bfloat16 v = __float2bfloat16_rn(j == i ? 0.0f : Q[(size_t)i * n + j]);
-            qb[(size_t)i * n + j] = v;
+            qb[(size_t)i * np + j] = v;
             rs += (double)__bfloat162float(v);
         }
         cp[i] = (c ? c[i] : 0.0f) + Q[(size_t)i * n + i];                // fold the diagonal (reading R1)
@@ -671,15 +675,15 @@ gda_status dense_prepare(gda_problem* p, const float* Q, const float* c) {
     }
     GDA_CUDA_TRY(cudaMalloc((void**)&p->d_Qbf, qb.size() * sizeof(__nv_bfloat16)));
     GDA_CUDA_TRY(cudaMemcpy(p->d_Qbf, qb.data(), qb.size() * sizeof(__nv_bfloat16), cudaMemcpyHostToDevice));
-    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_rowsum, n * sizeof(float)));
-    GDA_CUDA_TRY(cudaMemcpy(p->d_rowsum, hvec.data(), n * sizeof(float), cudaMemcpyHostToDevice));
-    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_cprime, n * sizeof(float)));
-    GDA_CUDA_TRY(cudaMemcpy(p->d_cprime, cp.data(), n * sizeof(float), cudaMemcpyHostToDevice));
+    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_rowsum, np * sizeof(float)));
+    GDA_CUDA_TRY(cudaMemcpy(p->d_rowsum, hvec.data(), np * sizeof(float), cudaMemcpyHostToDevice));
+    GDA_CUDA_TRY(cudaMalloc((void**)&p->d_cprime, np * sizeof(float)));
+    GDA_CUDA_TRY(cudaMemcpy(p->d_cprime, cp.data(), np * sizeof(float), cudaMemcpyHostToDevice));
     DenseHost* h = new DenseHost();
     p->tmap_Q = h;
     if (const char* e = getenv("GDA_DENSE_SHAPE")) if (e[0] >= '0' && e[0] <= '3') h->forced_shape = e[0] - '0';
     GDA_TRY(configure_all(p));
-    return make_tmap(&h->tmap_q, p->d_Qbf, (uint64_t)n, (uint64_t)n, BBOX);
+    return make_tmap(&h->tmap_q, p->d_Qbf, (uint64_t)np, (uint64_t)np, BBOX);
 }
 
 void dense_release(gda_problem* p) {
@@ -691,9 +695,9 @@ void dense_release(gda_problem* p) {
 
 gda_status dense_make_operand(gda_problem* p, int32_t B, const float* x, __nv_bfloat16* zt, int hat, cudaStream_t s,
                               int64_t* launches) {
-    dim3 grid((unsigned)(p->n / 32), (unsigned)(B / 32));
-    if (hat) make_operand_kernel<1><<<grid, 256, 0, s>>>(p->n, B, x, zt);
-    else make_operand_kernel<0><<<grid, 256, 0, s>>>(p->n, B, x, zt);
+    dim3 grid((unsigned)(p->n_pad / 32), (unsigned)(B / 32));
+    if (hat) make_operand_kernel<1><<<grid, 256, 0, s>>>(p->n_pad, B, x, zt);
+    else make_operand_kernel<0><<<grid, 256, 0, s>>>(p->n_pad, B, x, zt);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
@@ -705,7 +709,7 @@ gda_status dense_step(gda_problem* p, int32_t B, float* x, float* y, const __nv_
     const CUtensorMap* ta;
     GDA_TRY(z_maps(p, B, zt_in, &ta));
     DenseArgs a{};
-    a.n = p->n; a.B = B; a.x = x; a.y = y; a.zt_out = zt_out; a.hvec = p->d_rowsum; a.cprime = p->d_cprime;
+    a.n = p->n_pad; a.B = B; a.x = x; a.y = y; a.zt_out = zt_out; a.hvec = p->d_rowsum; a.cprime = p->d_cprime;
     a.up = up; a.st = st; a.t_off = t_off; a.mu = sd.mu; a.gpart = sd.gpart;
     if (launches) ++*launches;
     if (sd.mu) {                                               // PDBO-s
@@ -724,11 +728,11 @@ gda_status dense_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaS
     const CUtensorMap* ta;
     GDA_TRY(z_maps(p, B, ws.zt[0], &ta));
     DenseArgs a{};
-    a.n = p->n; a.B = B; a.hvec = p->d_rowsum; a.cprime = p->d_cprime; a.gout = G;
+    a.n = p->n_pad; a.B = B; a.hvec = p->d_rowsum; a.cprime = p->d_cprime; a.gout = G;
     return launch_gemm<MODE_GRAD, GDA_G_QUADRATIC>(p, *ta, a, s);
 }
 
-int32_t dense_num_partials(const gda_problem* p, int32_t) { return p->n / 128; }
+int32_t dense_num_partials(const gda_problem* p, int32_t) { return p->n_pad / 128; }
 
 // S5: x_hat operand (exact in bf16), GEMM, per-thread column sums.  Scratch: the zt buffer NOT holding the current operand.
 gda_status dense_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
@@ -739,7 +743,7 @@ gda_status dense_score_partials(gda_problem* p, int32_t B, const float* x, void*
     const CUtensorMap* ta;
     GDA_TRY(z_maps(p, B, scratch, &ta));
     DenseArgs a{};
-    a.n = p->n; a.B = B; a.x = const_cast<float*>(x); a.hvec = p->d_rowsum; a.cprime = p->d_cprime;
+    a.n = p->n_pad; a.B = B; a.x = const_cast<float*>(x); a.hvec = p->d_rowsum; a.cprime = p->d_cprime;
     a.partial = static_cast<double*>(partial);
     *n_part = dense_num_partials(p, B);
     if (launches) ++*launches;

@@ -221,16 +221,48 @@ yg_partials_kernel(int n, int B, const float* __restrict__ x, const float* __res
         }
 }
 
+// dense f(x) at a continuous point from its gradient: f = sum_i x_i ((Q_off x)_i + c'_i) and G = 2 Q_off x + c', so
+// f = sum_i x_i (G_i + c'_i) / 2.  partial[rb][b] over blocks of 64 rows; products in fp32, sums in fp64.
+__global__ void __launch_bounds__(256)
+xg_partials_kernel(int n, int B, const float* __restrict__ x, const float* __restrict__ G, const float* __restrict__ cprime,
+                   double* __restrict__ partial) {
+    __shared__ double red[8][32][4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c4 = blockIdx.y * 32 + lane;
+    const bool active = 4 * c4 < B;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    if (active)
+        for (int r = warp; r < 64; r += 8) {
+            const int row = blockIdx.x * 64 + r;
+            if (row >= n) break;
+            const size_t off = (size_t)row * B + 4 * c4;
+            const float4 xv = ldg4(x + off), gv = ldg4(G + off);
+            const float cp = __ldg(cprime + row);
+            acc[0] += (double)(0.5f * xv.x * (gv.x + cp)); acc[1] += (double)(0.5f * xv.y * (gv.y + cp));
+            acc[2] += (double)(0.5f * xv.z * (gv.z + cp)); acc[3] += (double)(0.5f * xv.w * (gv.w + cp));
+        }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) red[warp][lane][q] = acc[q];
+    __syncthreads();
+    if (warp == 0 && active)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            double t = red[0][lane][q];
+            for (int w = 1; w < 8; ++w) t += red[w][lane][q];
+            partial[(size_t)blockIdx.x * B + 4 * c4 + q] = t;
+        }
+}
+
 // ones[b] = sum_i x_bin[i][b]: block = 128 restarts (uchar4 per lane) x 32 row slices, integer sums
 __global__ void __launch_bounds__(1024)
-count_ones_kernel(int n, int B, const uint8_t* __restrict__ x_bin, int32_t* __restrict__ ones) {
+count_ones_kernel(int n, int B, int ld, const uint8_t* __restrict__ x_bin, int32_t* __restrict__ ones) {
     __shared__ int red[32][32][4];
     const int lane = threadIdx.x, slice = threadIdx.y;
     const int c = blockIdx.x * 128 + 4 * lane;
     int acc[4] = {0, 0, 0, 0};
     if (c < B)
         for (int i = slice; i < n; i += 32) {
-            const uchar4 v = *reinterpret_cast<const uchar4*>(x_bin + (size_t)i * B + c);
+            const uchar4 v = *reinterpret_cast<const uchar4*>(x_bin + (size_t)i * ld + c);
             acc[0] += v.x; acc[1] += v.y; acc[2] += v.z; acc[3] += v.w;
         }
 #pragma unroll
@@ -243,6 +275,17 @@ count_ones_kernel(int n, int B, const uint8_t* __restrict__ x_bin, int32_t* __re
             for (int k = 0; k < 32; ++k) t += red[k][lane][q];
             ones[c + q] = t;
         }
+}
+
+// PDBO-s, sparse / MaxSAT paths: close the step -- mu_out = mu_in + beta * (exact integer sum of the ways) / 2^32
+__global__ void __launch_bounds__(128)
+mu_finalize_kernel(int B, unsigned long long* __restrict__ gacc, float beta, const float* __restrict__ mu_in, float* __restrict__ mu_out) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    long long t = 0;
+#pragma unroll
+    for (int k = 0; k < GDA_GACC_WAYS; ++k) { t += (long long)gacc[(size_t)k * B + b]; gacc[(size_t)k * B + b] = 0ull; }
+    mu_out[b] = mu_in[b] + beta * (float)((double)t / GDA_GACC_SCALE);
 }
 
 __global__ void mu_init_kernel(int B, const float* __restrict__ l0, float l0_scalar, float* __restrict__ mu) {
@@ -260,6 +303,14 @@ gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float bet
     return GDA_OK;
 }
 
+gda_status mu_finalize(int32_t B, unsigned long long* gacc, float beta, const float* mu_in, float* mu_out, cudaStream_t s,
+                       int64_t* launches) {
+    mu_finalize_kernel<<<(unsigned)((B + 127) / 128), 128, 0, s>>>(B, gacc, beta, mu_in, mu_out);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
 gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, cudaStream_t s, int64_t* launches) {
     mu_init_kernel<<<(B + 255) / 256, 256, 0, s>>>(B, l0, l0_scalar, mu);
     if (launches) ++*launches;
@@ -267,85 +318,107 @@ gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, cudaS
     return GDA_OK;
 }
 
+// [rows][B] at the caller (host or device: cudaMemcpyDefault tells by unified addressing) -> [..][ld] in the workspace
+static gda_status copy_in(void* dst, size_t ld, const void* src, size_t B, size_t rows, size_t esz, cudaStream_t s) {
+    if (ld == B) GDA_CUDA_TRY(cudaMemcpyAsync(dst, src, rows * B * esz, cudaMemcpyDefault, s));
+    else GDA_CUDA_TRY(cudaMemcpy2DAsync(dst, ld * esz, src, B * esz, B * esz, rows, cudaMemcpyDefault, s));
+    return GDA_OK;
+}
+
 gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0, float l0_scalar,
                     uint32_t t0, cudaStream_t s, int64_t* launches) {
     Workspace& ws = p->ws;
-    const size_t elems = (size_t)p->n * B;
-    // x0 / l0 may be HOST pointers (gda_run_host): cudaMemcpyDefault tells by unified addressing
-    if (p->kind == GDA_KIND_KCUT)
-        GDA_CUDA_TRY(cudaMemcpyAsync(ws.z, x0, elems * p->kparts * sizeof(float), cudaMemcpyDefault, s));
-    else
-        GDA_CUDA_TRY(cudaMemcpyAsync(ws.x[0], x0, elems * sizeof(float), cudaMemcpyDefault, s));
+    const size_t ld = (size_t)ws.ld, elems = (size_t)p->n_pad * ld;          // padded only on the dense path
+    const bool padded = ld != (size_t)B || p->n_pad != p->n;
+    if (p->kind == GDA_KIND_KCUT) {
+        GDA_CUDA_TRY(cudaMemcpyAsync(ws.z, x0, (size_t)p->n * B * p->kparts * sizeof(float), cudaMemcpyDefault, s));
+    } else {
+        if (padded) GDA_CUDA_TRY(cudaMemsetAsync(ws.x[0], 0, elems * sizeof(float), s));   // padding variables and restarts start at 0
+        GDA_TRY(copy_in(ws.x[0], ld, x0, (size_t)B, (size_t)p->n, sizeof(float), s));
+    }
     if (ws.dual == GDA_DUAL_SCALAR) {
+        if (ws.gacc)                                         // nothing pending from an earlier (possibly failed) run
+            GDA_CUDA_TRY(cudaMemsetAsync(ws.gacc, 0, (size_t)GDA_GACC_WAYS * B * sizeof(unsigned long long), s));
+        GDA_TRY(mu_init((int32_t)ld, nullptr, l0 ? 0.0f : l0_scalar, ws.mu[0], s, launches));
         if (l0) GDA_CUDA_TRY(cudaMemcpyAsync(ws.mu[0], l0, (size_t)B * sizeof(float), cudaMemcpyDefault, s));
-        else GDA_TRY(mu_init(B, nullptr, l0_scalar, ws.mu[0], s, launches));
     } else if (l0) {
-        GDA_CUDA_TRY(cudaMemcpyAsync(ws.y, l0, elems * sizeof(float), cudaMemcpyDefault, s));
+        if (padded) GDA_CUDA_TRY(cudaMemsetAsync(ws.y, 0, elems * sizeof(float), s));
+        GDA_TRY(copy_in(ws.y, ld, l0, (size_t)B, (size_t)p->n, sizeof(float), s));
     } else {
         const size_t n_vec = elems / 4;
         fill_kernel<<<(unsigned)((n_vec + 255) / 256), 256, 0, s>>>(n_vec, reinterpret_cast<float4*>(ws.y), l0_scalar);
         if (launches) ++*launches;
     }
     GDA_CUDA_TRY(cudaMemsetAsync(ws.x_bin, 0, elems, s));
-    init_state_kernel<<<(B + 255) / 256, 256, 0, s>>>(B, ws.best_obj, ws.improved, ws.state, t0);
+    init_state_kernel<<<(unsigned)((ld + 255) / 256), 256, 0, s>>>((int)ld, ws.best_obj, ws.improved, ws.state, t0);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
 }
 
-gda_status eval_finalize(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj_now,
+gda_status eval_finalize(gda_problem* p, int32_t B, int32_t ld, const void* partial, int32_t n_part, double* obj_now,
                          double* best_obj, int32_t* improved, RunState* st, double* trace_best,
                          uint64_t* trace_ns, int32_t trace_cap, uint32_t advance_t, cudaStream_t s,
                          int64_t* launches) {
     const unsigned grid = (unsigned)((B + FIN_COLS - 1) / FIN_COLS);
     const dim3 block(FIN_COLS, FIN_SLICES);
     if (p->integral)
-        finalize_kernel<true><<<grid, block, 0, s>>>(B, B, partial, n_part, obj_now, best_obj, improved, st, p->ws.block_min,
+        finalize_kernel<true><<<grid, block, 0, s>>>(B, ld, partial, n_part, obj_now, best_obj, improved, st, p->ws.block_min,
                                                      trace_best, trace_ns, trace_cap, advance_t);
     else
-        finalize_kernel<false><<<grid, block, 0, s>>>(B, B, partial, n_part, obj_now, best_obj, improved, st, p->ws.block_min,
+        finalize_kernel<false><<<grid, block, 0, s>>>(B, ld, partial, n_part, obj_now, best_obj, improved, st, p->ws.block_min,
                                                       trace_best, trace_ns, trace_cap, advance_t);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
 }
 
-gda_status score_reduce(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj,
+gda_status score_reduce(gda_problem* p, int32_t B, int32_t ld, const void* partial, int32_t n_part, double* obj,
                         cudaStream_t s) {
-    return eval_finalize(p, B, partial, n_part, obj, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, s, nullptr);
+    return eval_finalize(p, B, ld, partial, n_part, obj, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, s, nullptr);
 }
 
-gda_status eval_commit(gda_problem* p, int32_t B, const float* x, const int32_t* improved, uint8_t* x_bin,
+// every row of the (padded) state, every column of the (padded) stride: improved[] is 0 for padding restarts
+gda_status eval_commit(gda_problem* p, int32_t ld, const float* x, const int32_t* improved, uint8_t* x_bin,
                        cudaStream_t s, int64_t* launches) {
-    const size_t n_vec = (size_t)p->n * B / 4;
+    const size_t n_vec = (size_t)p->n_pad * ld / 4;
     const unsigned grid = (unsigned)std::min<size_t>((n_vec + 255) / 256, (size_t)p->num_sms * 8);
-    commit_kernel<<<grid, 256, 0, s>>>(n_vec, B / 4, x, improved, p->ws.state, x_bin);
+    commit_kernel<<<grid, 256, 0, s>>>(n_vec, ld / 4, x, improved, p->ws.state, x_bin);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
 }
 
-gda_status eval_yg_partials(gda_problem* p, int32_t B, const float* x, const float* y, float y_scalar, int32_t gfun,
+gda_status eval_yg_partials(gda_problem* p, int32_t n_rows, int32_t B, const float* x, const float* y, float y_scalar, int32_t gfun,
                             float log_eps, double* partial, int32_t* n_part, cudaStream_t s) {
+    (void)p;
     UpdParams up{};
     up.log_eps = log_eps; up.gfun = gfun;
-    const dim3 grid((unsigned)((p->n + 63) / 64), (unsigned)((B / 4 + 31) / 32));
-    if (gfun == GDA_G_QUADRATIC) yg_partials_kernel<GDA_G_QUADRATIC><<<grid, 256, 0, s>>>(p->n, B, x, y, y_scalar, up, partial);
-    else yg_partials_kernel<GDA_G_ENTROPY><<<grid, 256, 0, s>>>(p->n, B, x, y, y_scalar, up, partial);
+    const dim3 grid((unsigned)((n_rows + 63) / 64), (unsigned)((B / 4 + 31) / 32));
+    if (gfun == GDA_G_QUADRATIC) yg_partials_kernel<GDA_G_QUADRATIC><<<grid, 256, 0, s>>>(n_rows, B, x, y, y_scalar, up, partial);
+    else yg_partials_kernel<GDA_G_ENTROPY><<<grid, 256, 0, s>>>(n_rows, B, x, y, y_scalar, up, partial);
     *n_part = (int32_t)grid.x;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
 }
 
-gda_status eval_sum_partials(int32_t B, const double* partial, int32_t n_part, double* out, cudaStream_t s) {
+gda_status eval_xg_partials(gda_problem* p, int32_t ld, const float* x, const float* G, double* partial, int32_t* n_part, cudaStream_t s) {
+    const dim3 grid((unsigned)((p->n + 63) / 64), (unsigned)((ld / 4 + 31) / 32));
+    xg_partials_kernel<<<grid, 256, 0, s>>>(p->n, ld, x, G, p->d_cprime, partial);
+    *n_part = (int32_t)grid.x;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status eval_sum_partials(int32_t B, int32_t ld, const double* partial, int32_t n_part, double* out, cudaStream_t s) {
     finalize_kernel<false><<<(unsigned)((B + FIN_COLS - 1) / FIN_COLS), dim3(FIN_COLS, FIN_SLICES), 0, s>>>(
-        B, B, partial, n_part, out, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0);
+        B, ld, partial, n_part, out, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0);
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
 }
 
 gda_status eval_count_ones(gda_problem* p, int32_t B, const uint8_t* x_bin, int32_t* ones, cudaStream_t s, int64_t* launches) {
-    count_ones_kernel<<<(unsigned)((B + 127) / 128), dim3(32, 32), 0, s>>>(p->n, B, x_bin, ones);
+    count_ones_kernel<<<(unsigned)((B + 127) / 128), dim3(32, 32), 0, s>>>(p->n, B, p->ws.ld, x_bin, ones);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;

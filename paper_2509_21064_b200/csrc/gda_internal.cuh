@@ -40,12 +40,24 @@ struct UpdParams {
 };
 
 // PDBO-s (GDA_DUAL_SCALAR) state handed to the step kernels; mu == nullptr means per-variable duals.
-// The step kernel reads this step's multipliers mu^t and leaves its blocks' sums of g(x_i^t) in gpart; gsum_reduce
-// then writes mu^{t+1} = mu^t + beta * sum(gpart) into the other mu buffer (the buffers follow the parity of x).
+// Sparse path: a step kernel reads this step's multipliers mu^t; every block adds its sum of g(x_i^t)
+// (fp32, fixed order inside the block) to one of GDA_GACC_WAYS accumulators per restart in 64-bit FIXED POINT (2^-32)
+// with integer reductions -- exact, hence independent of the order in which blocks arrive: deterministic -- and a
+// B-thread kernel (mu_finalize) adds the ways, writes mu^{t+1} = mu^t + beta * sum into the other mu buffer (the
+// buffers follow the parity of x) and clears them (config 3: 20.2 us per iteration against 22.1 us with partial rows).
+// MaxSAT and dense paths: the blocks / epilogue threads leave their sums as rows of gpart and gsum_reduce adds them in a
+// fixed order and writes mu^{t+1} (on the MaxSAT kernel the integer reductions measured slower: 52.7 against 46.1 us).
 struct ScalarDual {
-    const float* mu = nullptr;        // [B]
-    float* gpart = nullptr;           // [n_gpart][B]
+    const float* mu = nullptr;                 // [B] this step's multipliers
+    unsigned long long* gacc = nullptr;        // [GDA_GACC_WAYS][B] sums of g(x_i^t), fixed point (two's complement), zero between steps
+    int32_t B = 0;
+    float* gpart = nullptr;                    // MaxSAT: [ceil(n / 8)][B]; dense: [n / 128][B]
 };
+constexpr double GDA_GACC_SCALE = 4294967296.0;   // 2^32
+#ifndef GDA_GACC_WAYS_N
+#define GDA_GACC_WAYS_N 16
+#endif
+constexpr int GDA_GACC_WAYS = GDA_GACC_WAYS_N;                 // blocks spread over this many accumulators: few same-address atomics
 
 // device-side run state (lives in the workspace)
 struct RunState {
@@ -61,6 +73,7 @@ struct RunState {
 // ---------------------------------------------------------------------------------------------------
 struct Workspace {
     int32_t B = 0;
+    int32_t ld = 0;                     // row stride of the state arrays: B, except dense problems (B rounded up to a multiple of 128)
     int32_t parity = 0;                 // which x / zt buffer holds the current iterate
     bool has_state = false;             // a previous gda_run left (x, y, best-so-far) here: x0 == NULL may resume
     float* x[2] = {nullptr, nullptr};   // [n][B] double buffer (Jacobi: every row reads all of x^t)
@@ -68,8 +81,9 @@ struct Workspace {
     float* z = nullptr;                 // Max-k-Cut: logits [k][n][B], updated in place (x[] then holds SoftMax(z), [k][n][B])
     uint8_t* lab = nullptr;             // Max-k-Cut: labels of the current iterate at an evaluation, [n][B]
     float* mu[2] = {nullptr, nullptr};  // PDBO-s: [B] multipliers, double-buffered with the parity of x
-    float* gpart = nullptr;             // PDBO-s: [n_gpart][B] per-block sums of g
+    float* gpart = nullptr;             // PDBO-s, MaxSAT and dense paths: [n_gpart][B] partial sums of g
     int32_t n_gpart = 0;
+    unsigned long long* gacc = nullptr; // PDBO-s, sparse path: [GDA_GACC_WAYS][B] fixed-point sums of g (ScalarDual)
     int32_t dual = 0;                   // dual mode of the state held here
     uint8_t* x_bin = nullptr;           // [n][B] best-so-far rounded point
     double* best_obj = nullptr;         // [B]
@@ -105,6 +119,7 @@ struct CachedGraph {
 struct gda_problem {
     int32_t kind = 0;
     int32_t n = 0;
+    int32_t n_pad = 0;                   // rows of the state arrays: n, except dense problems (n rounded up to a multiple of 256)
     int64_t nnz = 0;
     int32_t m = 0;
     int32_t kparts = 0;                  // Max-k-Cut: number of parts k (0 otherwise)
@@ -144,7 +159,6 @@ struct gda_problem {
 // sparse QUBO (gda_sparse.cu)
 gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches);
-int32_t sparse_num_gparts(const gda_problem* p);
 gda_status sparse_configure(gda_problem* p);                       // at create
 // small n: sliced-ELL structure built at create, and one launch per chunk (steps + evaluation) when it applies
 gda_status sparse_build_slab(gda_problem* p, const std::vector<int32_t>& rowptr, const std::vector<int32_t>& col,
@@ -192,27 +206,32 @@ int32_t dense_num_partials(const gda_problem* p, int32_t B);
 void dense_release(gda_problem* p);
 
 // shared evaluation tail (gda_eval.cu)
-gda_status eval_finalize(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj_now,
+gda_status eval_finalize(gda_problem* p, int32_t B, int32_t ld, const void* partial, int32_t n_part, double* obj_now,
                          double* best_obj, int32_t* improved, RunState* st, double* trace_best,
                          uint64_t* trace_ns, int32_t trace_cap, uint32_t advance_t, cudaStream_t s,
                          int64_t* launches);
-gda_status eval_commit(gda_problem* p, int32_t B, const float* x, const int32_t* improved, uint8_t* x_bin,
+gda_status eval_commit(gda_problem* p, int32_t ld, const float* x, const int32_t* improved, uint8_t* x_bin,
                        cudaStream_t s, int64_t* launches);
 gda_status eval_argbest(int32_t B, const double* obj, int32_t* best_restart, double* best_val,
                         cudaStream_t s, int64_t* launches);
 // sum_i y_i g(x_i) as partial sums over blocks of 64 rows (y == nullptr: y_scalar); double reduction of partial rows
-gda_status eval_yg_partials(gda_problem* p, int32_t B, const float* x, const float* y, float y_scalar, int32_t gfun,
+gda_status eval_yg_partials(gda_problem* p, int32_t n_rows, int32_t B, const float* x, const float* y, float y_scalar, int32_t gfun,
                             float log_eps, double* partial, int32_t* n_part, cudaStream_t s);
-gda_status eval_sum_partials(int32_t B, const double* partial, int32_t n_part, double* out, cudaStream_t s);
+gda_status eval_sum_partials(int32_t B, int32_t ld, const double* partial, int32_t n_part, double* out, cudaStream_t s);
+// dense Lagrangian: partial[rb][b] = sum over the 64 rows of block rb of x_i (G_i + c'_i) / 2  (= f(x) with G = grad f)
+gda_status eval_xg_partials(gda_problem* p, int32_t ld, const float* x, const float* G, double* partial, int32_t* n_part, cudaStream_t s);
 gda_status eval_count_ones(gda_problem* p, int32_t B, const uint8_t* x_bin, int32_t* ones, cudaStream_t s, int64_t* launches);
 gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0, float l0_scalar,
                     uint32_t t0, cudaStream_t s, int64_t* launches);
-gda_status score_reduce(gda_problem* p, int32_t B, const void* partial, int32_t n_part, double* obj,
+gda_status score_reduce(gda_problem* p, int32_t B, int32_t ld, const void* partial, int32_t n_part, double* obj,
                         cudaStream_t s);
 // PDBO-s: mu_out[b] = mu_in[b] + beta * sum_r gpart[r][b], summed in a fixed order (deterministic)
 gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float beta, const float* mu_in, float* mu_out,
                        cudaStream_t s, int64_t* launches);
 gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, cudaStream_t s, int64_t* launches);
+// PDBO-s, sparse / MaxSAT: mu_out[b] = mu_in[b] + beta * (sum of the ways of gacc[.][b]) / 2^32; clears gacc
+gda_status mu_finalize(int32_t B, unsigned long long* gacc, float beta, const float* mu_in, float* mu_out, cudaStream_t s,
+                       int64_t* launches);
 
 // ---------------------------------------------------------------------------------------------------
 // device helpers: g, g', the fused update S4 (Eq. 6 + perturbation), the tie-break hash
@@ -316,8 +335,19 @@ __device__ __forceinline__ void gda_update4(const float4& x, const float4& y, co
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
 // ---- PDBO-s helpers shared by the warp-per-(row, chunk) step kernels -------------------------------------------
-// One gpart row per block: the NW warps' sums of g (0 for warps without a row), added in warp order by warp 0.
-// Called by every thread of the block.
+// scalar_dual_commit: ONE warp adds its block's sums t (lane = float4 of restarts c4) to accumulator `way`.
+__device__ __forceinline__ void scalar_dual_commit(float4 t, bool active, int c4, unsigned way, const ScalarDual& sd) {
+    if (!active) return;
+    unsigned long long* acc = sd.gacc + (size_t)(way % GDA_GACC_WAYS) * sd.B + 4 * c4;
+    atomicAdd(acc + 0, (unsigned long long)__double2ll_rn((double)t.x * GDA_GACC_SCALE));
+    atomicAdd(acc + 1, (unsigned long long)__double2ll_rn((double)t.y * GDA_GACC_SCALE));
+    atomicAdd(acc + 2, (unsigned long long)__double2ll_rn((double)t.z * GDA_GACC_SCALE));
+    atomicAdd(acc + 3, (unsigned long long)__double2ll_rn((double)t.w * GDA_GACC_SCALE));
+}
+
+// Called by every thread of a block whose NW warps hold their sums of g in gs (0 for warps / lanes without work): the
+// warps' sums are added in warp order by warp 0, which then commits them.
+// One gpart row per block (MaxSAT path): the NW warps' sums of g, added in warp order by warp 0; gsum_reduce adds the rows.
 template <int NW>
 __device__ __forceinline__ void scalar_dual_block_sum(float4 gs, float4 (*red)[32], int warp, int lane, bool active,
                                                       float* __restrict__ gpart_row_c4) {
@@ -328,6 +358,18 @@ __device__ __forceinline__ void scalar_dual_block_sum(float4 gs, float4 (*red)[3
 #pragma unroll
     for (int w = 1; w < NW; ++w) { const float4 r = red[w][lane]; t.x += r.x; t.y += r.y; t.z += r.z; t.w += r.w; }
     *reinterpret_cast<float4*>(gpart_row_c4) = t;
+}
+
+template <int NW>
+__device__ __forceinline__ void scalar_dual_finish(float4 gs, float4 (*red)[32], int warp, int lane, bool active, int c4,
+                                                   unsigned way, const ScalarDual& sd) {
+    red[warp][lane] = gs;
+    __syncthreads();
+    if (warp != 0) return;
+    float4 t = red[0][lane];
+#pragma unroll
+    for (int w = 1; w < NW; ++w) { const float4 r = red[w][lane]; t.x += r.x; t.y += r.y; t.z += r.z; t.w += r.w; }
+    scalar_dual_commit(t, active, c4, way, sd);
 }
 
 #endif

@@ -11,6 +11,8 @@
 // the slot records, which are fetched with one coalesced load per 32 slots.
 #include "gda_internal.cuh"
 
+#include <algorithm>
+
 namespace {
 
 constexpr int WARPS = 8;
@@ -109,11 +111,11 @@ maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* 
                    const RunState* __restrict__ st, uint32_t t_off) {
     __shared__ float4 gred[DUAL ? WARPS : 1][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int var = blockIdx.x * WARPS + warp;
     const int c4 = blockIdx.y * 32 + lane;
     const bool active = 4 * c4 < B;
     float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = gs;
     if (DUAL) mu = ldg4(sd.mu + 4 * (active ? c4 : B / 4 - 1));
+    const int var = blockIdx.x * WARPS + warp;
     if (var < n) {                                           // warp-uniform
         const int start = __ldg(vptr + var), end = __ldg(vptr + var + 1);
         const float4 G = gather_var<KW, PAD>(coef, others, kw, start, end, x, B, c4, active, lane);
@@ -133,9 +135,7 @@ maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* 
             }
         }
     }
-    if (DUAL) {
-        scalar_dual_block_sum<WARPS>(gs, gred, warp, lane, active, sd.gpart + (size_t)blockIdx.x * B + 4 * c4);
-    }
+    if (DUAL) scalar_dual_block_sum<WARPS>(gs, gred, warp, lane, active, sd.gpart + (size_t)blockIdx.x * B + 4 * c4);
 }
 
 // S5: partial[cb][b] = sum over the clauses of block cb of w_j [every literal of C_j false under x_hat]
@@ -238,7 +238,8 @@ void launch_kw(gda_problem* p, int32_t B, dim3 grid, const float* x, float* y, f
 template <int MODE, bool DUAL>
 gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
-    const dim3 grid((unsigned)((p->n + WARPS - 1) / WARPS), (unsigned)((B / 4 + 31) / 32));
+    const int groups = (p->n + WARPS - 1) / WARPS, chunks = (B / 4 + 31) / 32;
+    const dim3 grid((unsigned)groups, (unsigned)chunks);
     if (up.gfun == GDA_G_QUADRATIC) launch_kw<GDA_G_QUADRATIC, MODE, DUAL>(p, B, grid, x, y, xn, up, sd, st, t_off, s);
     else launch_kw<GDA_G_ENTROPY, MODE, DUAL>(p, B, grid, x, y, xn, up, sd, st, t_off, s);
     if (launches) ++*launches;

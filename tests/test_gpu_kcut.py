@@ -127,3 +127,18 @@ def test_arguments_and_unsupported_calls(api):
     torch.cuda.synchronize()
     assert torch.equal(b["x"], za)
     P.destroy()
+
+
+def test_score_of_given_logits_matches_the_oracle(api):
+    """gda_score on a Max-k-Cut problem: labels = argmax_j Z_ji (lowest j on ties, reading K4), objective Tr(Xh W Xh^T)."""
+    from oracle import kcut
+    w = CASES[0]
+    Pw = w.problem
+    P = api.create_from_workload(Pw)
+    OK = kcut.Problem(Pw.n, Pw.k, Pw.rowptr, Pw.col, Pw.val.astype(np.float64))
+    Z = wl.z0_uniform(Pw.k, Pw.n, w.B, 9)
+    Z[:, :5, 0] = 0.25                                            # ties: label 0
+    obj = P.score(dev(Z)).cpu().numpy()
+    lab = Z.argmax(axis=0).astype(np.uint8)                       # numpy's argmax also takes the first maximum
+    assert np.array_equal(obj, kcut.objective(OK, lab))
+    P.destroy()
