@@ -311,6 +311,19 @@ def roofline_block(w: wl.Workload, peaks, t_step_mean, t_step_median, t_eval):
             "eval_us": t_eval * 1e6, "state_l2_resident": resident, "basis": basis}
 
 
+def smem_roofline(w: wl.Workload, t_kernel_s: float, sm_count: int, sm_max_mhz: float):
+    """The slab kernel (small n: state in shared memory, one launch per chunk) is bound by shared-memory gathers, not by
+    HBM: nnz x B x 4 bytes of neighbour values per step against 128 B per clock and SM."""
+    nnz = int(w.problem.rowptr[-1])
+    gathered = nnz * w.B * 4
+    peak = sm_count * 128 * sm_max_mhz * 1e6 / 1e9
+    ach = gathered / t_kernel_s / 1e9
+    return {"bound": "smem", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+            "gathered_bytes_per_step": gathered, "ctas": (w.B + 7) // 8,
+            "basis": f"shared-memory bytes gathered per GDA step / step time against {sm_count} SMs x 128 B/clk x {sm_max_mhz:.0f} MHz "
+                     f"(the launch has {(w.B + 7) // 8} CTAs of 8 restarts: at most that many SMs work)"}
+
+
 class Session:
     """One device, one stream, the flush buffer; measures workloads one after the other."""
 
@@ -361,6 +374,7 @@ class Session:
             self.sync_all()
             step_ms = [a.elapsed_time(b) for a, b in ev]
             res["best_flushed"] = float(out["obj"].min().item())
+            res["chunk_fused"] = h.eval_every > 1 and P.info().last_run_step_launches == 1   # the slab kernel ran the chunk
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             P.resume(prm0, out)                                           # evaluation alone (one evaluation-only call)
             self.sync_all()
@@ -404,6 +418,11 @@ class Session:
                 res["out"] = out
         res.update(step_ms=step_ms, t_eval=t_eval, launches=int(launches))
         res["roofline"] = roofline_block(w, peaks, sum(step_ms) / 1e3 / K, statistics.median(step_ms) / 1e3, t_eval)
+        if w.kind == "qubo_csr" and res.get("chunk_fused"):
+            props = torch.cuda.get_device_properties(self.dev)
+            res["roofline"]["kernel"] = "spmm_chunk_slab (one launch = eval_every steps + the evaluation, state in shared memory)"
+            res["roofline"]["on_chip"] = smem_roofline(w, res["roofline"]["us_per_launch"] * 1e-6, props.multi_processor_count,
+                                                       (res["clocks"] or {}).get("sm_max_mhz") or 1965.0)
         res["P"] = P
         return res
 
