@@ -737,66 +737,78 @@ gda_status sparse_build_slab(gda_problem* p, const std::vector<int32_t>& rowptr,
                              const std::vector<float>& val2) {
     const int n = p->n;
     if (slab_smem_bytes(n, 32, -1) > (size_t)SLAB_SMEM_LIMIT) return GDA_OK;
-    // rows sorted by degree (descending, stable): the 16 rows of a group have similar lengths, so little padding
+    // rows sorted by degree (descending, stable): the rows that share passes have similar lengths, so little padding
     std::vector<int32_t> order(n);
     for (int i = 0; i < n; ++i) order[i] = i;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rowptr[a + 1] - rowptr[a] > rowptr[b + 1] - rowptr[b]; });
-    const int n_groups = (n + SLAB_ROWS - 1) / SLAB_ROWS;
+    // 1. quads of four rows of similar degree.  The four rows of a quad share every LDS.128 pass: order their entries
+    //    such that the four columns of a pass differ mod 4 (one 32-byte row of x per bank group).  Greedy: per pass, the
+    //    assignment of distinct classes to the rows that uses up the most entries, ties to the largest remaining
+    //    queues; zero-valued padding elsewhere.
+    struct Quad { int32_t row[4]; std::vector<int2> sched[4]; size_t len = 0; };
+    const int n_quads = (n + 3) / 4;
+    std::vector<Quad> quads(n_quads);
+    int64_t real_entries = 0;
+    static const int perms[24][4] = {{0,1,2,3},{0,1,3,2},{0,2,1,3},{0,2,3,1},{0,3,1,2},{0,3,2,1},{1,0,2,3},{1,0,3,2},
+        {1,2,0,3},{1,2,3,0},{1,3,0,2},{1,3,2,0},{2,0,1,3},{2,0,3,1},{2,1,0,3},{2,1,3,0},{2,3,0,1},{2,3,1,0},
+        {3,0,1,2},{3,0,2,1},{3,1,0,2},{3,1,2,0},{3,2,0,1},{3,2,1,0}};
+    for (int qd = 0; qd < n_quads; ++qd) {
+        Quad& Q4 = quads[qd];
+        std::vector<int2> queue[4][4];                          // [row of the quad][column class]
+        int remaining = 0;
+        for (int j = 0; j < 4; ++j) {
+            const int row = 4 * qd + j < n ? order[4 * qd + j] : -1;
+            Q4.row[j] = row;
+            if (row < 0) continue;
+            for (int k = rowptr[row]; k < rowptr[row + 1]; ++k) {
+                if (val2[k] == 0.0f) continue;                  // explicit zeros contribute nothing
+                int2 e;
+                e.x = col[k] * (SLAB_S * 4);
+                std::memcpy(&e.y, &val2[k], 4);
+                queue[j][col[k] & 3].push_back(e);
+                ++remaining;
+            }
+        }
+        real_entries += remaining;
+        while (remaining > 0) {
+            int best = 0; long best_score = -1;
+            for (int pi = 0; pi < 24; ++pi) {
+                long used = 0, left = 0;
+                for (int j = 0; j < 4; ++j) { const size_t sz = queue[j][perms[pi][j]].size(); used += sz > 0; left += (long)sz; }
+                const long score = used * 1000000L + left;
+                if (score > best_score) { best_score = score; best = pi; }
+            }
+            for (int j = 0; j < 4; ++j) {
+                const int c = perms[best][j];
+                int2 e;
+                if (!queue[j][c].empty()) { e = queue[j][c].back(); queue[j][c].pop_back(); --remaining; }
+                else { e.x = -1 - c; e.y = 0; }                                    // padding of class c, value 0 (resolved below)
+                Q4.sched[j].push_back(e);
+            }
+            ++Q4.len;
+        }
+    }
+    // 2. quads sorted by the length of their schedule, four of them per 16-row group (a warp walks them in lockstep,
+    //    so a group costs its longest quad)
+    std::vector<int32_t> qorder(n_quads);
+    for (int i = 0; i < n_quads; ++i) qorder[i] = i;
+    std::stable_sort(qorder.begin(), qorder.end(), [&](int a, int b) { return quads[a].len > quads[b].len; });
+    const int n_groups = (n_quads + 3) / 4;
     std::vector<int32_t> goff(n_groups + 1, 0), grow((size_t)n_groups * SLAB_ROWS, -1);
     std::vector<int2> ent;
-    std::vector<std::vector<int2>> sched(SLAB_ROWS);           // per row of the group: its slots in order
-    int64_t real_entries = 0;
     for (int g = 0; g < n_groups; ++g) {
-        for (int r = 0; r < SLAB_ROWS; ++r) {
-            sched[r].clear();
-            if (g * SLAB_ROWS + r < n) grow[(size_t)g * SLAB_ROWS + r] = order[g * SLAB_ROWS + r];
-        }
-        // the four rows 4h .. 4h+3 share every LDS.128 pass: order their entries such that the four columns of a pass
-        // differ mod 4 (one 32-byte row of x per bank group).  Greedy: per pass, the assignment of distinct classes to
-        // the rows that uses up the most entries, ties to the largest remaining queues; zero-valued padding elsewhere.
-        for (int h = 0; h < SLAB_ROWS / 4; ++h) {
-            std::vector<int2> queue[4][4];                      // [row in the subgroup][column class]
-            int remaining = 0;
-            for (int j = 0; j < 4; ++j) {
-                const int row = grow[(size_t)g * SLAB_ROWS + 4 * h + j];
-                if (row < 0) continue;
-                for (int k = rowptr[row]; k < rowptr[row + 1]; ++k) {
-                    if (val2[k] == 0.0f) continue;              // explicit zeros contribute nothing
-                    int2 e;
-                    e.x = col[k] * (SLAB_S * 4);
-                    std::memcpy(&e.y, &val2[k], 4);
-                    queue[j][col[k] & 3].push_back(e);
-                    ++remaining;
-                }
-            }
-            real_entries += remaining;
-            static const int perms[24][4] = {{0,1,2,3},{0,1,3,2},{0,2,1,3},{0,2,3,1},{0,3,1,2},{0,3,2,1},{1,0,2,3},{1,0,3,2},
-                {1,2,0,3},{1,2,3,0},{1,3,0,2},{1,3,2,0},{2,0,1,3},{2,0,3,1},{2,1,0,3},{2,1,3,0},{2,3,0,1},{2,3,1,0},
-                {3,0,1,2},{3,0,2,1},{3,1,0,2},{3,1,2,0},{3,2,0,1},{3,2,1,0}};
-            while (remaining > 0) {
-                int best = 0; long best_score = -1;
-                for (int pi = 0; pi < 24; ++pi) {
-                    long used = 0, left = 0;
-                    for (int j = 0; j < 4; ++j) { const size_t sz = queue[j][perms[pi][j]].size(); used += sz > 0; left += (long)sz; }
-                    const long score = used * 1000000L + left;
-                    if (score > best_score) { best_score = score; best = pi; }
-                }
-                for (int j = 0; j < 4; ++j) {
-                    const int c = perms[best][j];
-                    int2 e;
-                    if (!queue[j][c].empty()) { e = queue[j][c].back(); queue[j][c].pop_back(); --remaining; }
-                    else { e.x = -1 - c; e.y = 0; }                                // padding of class c, value 0 (resolved below)
-                    sched[4 * h + j].push_back(e);
-                }
-            }
-        }
         size_t len = 0;
-        for (int r = 0; r < SLAB_ROWS; ++r) len = std::max(len, sched[r].size());
+        for (int h = 0; h < 4; ++h)
+            if (4 * g + h < n_quads) len = std::max(len, quads[qorder[4 * g + h]].len);
         len = (len + 3) & ~(size_t)3;                           // the kernel walks 4 slots at a time
+        for (int h = 0; h < 4; ++h)
+            for (int j = 0; j < 4; ++j)
+                if (4 * g + h < n_quads) grow[(size_t)g * SLAB_ROWS + 4 * h + j] = quads[qorder[4 * g + h]].row[j];
         for (size_t k = 0; k < len; ++k)
             for (int r = 0; r < SLAB_ROWS; ++r) {
                 int2 e;
-                if (k < sched[r].size()) e = sched[r][k];
+                const int h = r >> 2, j = r & 3;
+                if (4 * g + h < n_quads && k < quads[qorder[4 * g + h]].sched[j].size()) e = quads[qorder[4 * g + h]].sched[j][k];
                 else { e.x = -1 - (int)((k + r) & 3); e.y = 0; }
                 ent.push_back(e);
             }
