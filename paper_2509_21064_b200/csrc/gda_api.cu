@@ -65,6 +65,7 @@ static gda_status device_setup(gda_problem* p) {
         return GDA_ERR_UNSUPPORTED;
     }
     p->num_sms = prop.multiProcessorCount;
+    p->l2_bytes = prop.l2CacheSize > 0 ? (int64_t)prop.l2CacheSize : p->l2_bytes;
     return GDA_OK;
 }
 

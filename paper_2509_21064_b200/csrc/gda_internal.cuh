@@ -126,6 +126,7 @@ struct gda_problem {
     int32_t integral = 0;
     int device = 0;
     int num_sms = 148;
+    int64_t l2_bytes = 126 << 20;
     // sparse QUBO: off-diagonal CSR with val2 = Q_ij + Q_ji (= 2 Q_ij), cprime = c + diag(Q)
     int32_t* d_rowptr = nullptr; int32_t* d_col = nullptr; float* d_val2 = nullptr;
     float* d_cprime = nullptr;           // also used by the dense path

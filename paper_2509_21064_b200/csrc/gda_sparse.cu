@@ -95,7 +95,7 @@ __device__ __forceinline__ void update_store(int row, int c4, int B, bool active
 // prefetching the row's own x, y lines into L1 up front was slower (15.1 us) and is not done.
 // DUAL (PDBO-s, MODE 0 only): the multiplier is one number per restart (sd.mu), y is not read or written, and the
 // block's sum of g(x_i^t) goes through scalar_dual_finish (fixed-point integer reductions; mu_finalize closes the step).
-template <int GFUN, int MODE, bool ELL, bool DUAL>
+template <int GFUN, int MODE, bool ELL, bool DUAL, bool PF>
 __global__ void __launch_bounds__(THREADS, 6)
 spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
                const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
@@ -133,6 +133,13 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
     const int row = row_list ? __ldg(row_list + ridx) : ridx;
     const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
     const uint32_t stride = 4u * (uint32_t)B;
+    // HBM-streaming case (the state does not fit L2: PF): start the row's own x, y lines towards L2 now, so
+    // that the DRAM latency hides behind the gather chain (config 3's graph at B = 1024: 73.2 -> 67.6 us per step; with
+    // an L2-resident state the extra instructions cost 2.5 %, hence the switch)
+    if (MODE == 0 && PF && (lane & 7) == 0) {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(x + (size_t)row * B + 4 * c4));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(y + (size_t)row * B + 4 * c4));
+    }
     float4 G = make_float4(0.f, 0.f, 0.f, 0.f);
     bool csr = true;
     if (ELL) {
@@ -635,13 +642,16 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     }
     const int n_light = p->d_light_rows ? p->n_light : p->n;
     const int light_blocks = (n_light + WARPS - 1) / WARPS;
+    const bool pf = MODE == 0 && !DUAL && 12.0 * (double)p->n * (double)B > 0.8 * (double)p->l2_bytes;   // the streaming switch (see spmm_step_warp)
     if (n_light > 0) {
         const dim3 grid((unsigned)light_blocks, (unsigned)chunks);
 #define GDA_SP_ARGS n_light, p->d_light_rows, B, p->d_rowptr, p->d_col, p->d_val2, p->d_ell, p->d_cprime, x, y, xn, up, sd, st, t_off
+#define GDA_SP_PF(G, E) do { if (pf) spmm_step_warp<G, MODE, E, DUAL, (MODE == 0 && !DUAL)><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); \
+                             else spmm_step_warp<G, MODE, E, DUAL, false><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); } while (0)
 #define GDA_SP_CASE(E) \
-        if (up.gfun == GDA_G_QUADRATIC) spmm_step_warp<GDA_G_QUADRATIC, MODE, E, DUAL><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); \
-        else spmm_step_warp<GDA_G_ENTROPY, MODE, E, DUAL><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS)
+        if (up.gfun == GDA_G_QUADRATIC) GDA_SP_PF(GDA_G_QUADRATIC, E); else GDA_SP_PF(GDA_G_ENTROPY, E)
         if (p->d_ell) { GDA_SP_CASE(true); } else { GDA_SP_CASE(false); }
+#undef GDA_SP_PF
 #undef GDA_SP_CASE
 #undef GDA_SP_ARGS
         if (launches) ++*launches;
