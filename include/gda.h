@@ -139,6 +139,7 @@ typedef struct {
  *               objective seen at any evaluation (R5)
  *   obj         DEVICE double [B]: F(x_bin[:,b]) -- exact integers when all coefficients are integers
  *   best_restart DEVICE int32 [1]: argmin_b obj[b], ties -> lowest b (R6)
+ * UNSUPPORTED: n * B >= 2^30 elements (after the dense path's padding; times k for Max-k-Cut).
  * INVALID_ARG: null required pointer, B <= 0 or B % 4 != 0, alpha <= 0, beta < 0 or non-finite, delta outside
  * [0, 1/2), eval_every <= 0, iters < 0, unknown gfun or dual, log_eps outside (0, 1/2) with the entropy g;
  * a resumed run (x0 == NULL) whose `dual` differs from the run it continues.                              */

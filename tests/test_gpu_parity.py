@@ -459,6 +459,27 @@ def test_two_handles_from_two_threads(api, oracle):
         assert np.array_equal(a, b)
 
 
+@pytest.mark.parametrize("kind", ["sparse_stream", "sparse_slab", "maxsat", "dense"])
+def test_run_without_cuda_graphs_is_bit_identical(api, kind):
+    """GDA_NO_GRAPH=1 (read at every chunk) enqueues the same kernels directly instead of replaying a captured graph."""
+    import os
+    w = {"sparse_stream": wl.config(3, B=132, n_scale=0.05), "sparse_slab": wl.config(2, B=64, n_scale=0.25),
+         "maxsat": wl.config(5, B=64, n_scale=0.05), "dense": wl.config(4, B=128, n_scale=0.0625)}[kind]
+    P = create_problem(api, w, sparse_path="stream" if kind == "sparse_stream" else None)
+    x0 = dev(wl.x0_uniform(w.problem.n, w.B, w.x0_seed))
+    prm = api.params_from_hyper(w.hyper, iters=230, eval_every=50)
+    a = P.run(x0, w.hyper.lambda0, prm, want_final=True)
+    xa, oa, ba = a["x"].clone(), a["obj"].clone(), a["x_bin"].clone()
+    os.environ["GDA_NO_GRAPH"] = "1"
+    try:
+        b = P.run(x0, w.hyper.lambda0, prm, want_final=True)
+        torch.cuda.synchronize()
+    finally:
+        os.environ.pop("GDA_NO_GRAPH", None)
+    assert torch.equal(b["x"], xa) and torch.equal(b["obj"], oa) and torch.equal(b["x_bin"], ba)
+    P.destroy()
+
+
 def test_run_host_matches_device_run(api):
     w = wl.config(3, B=16, n_scale=0.02)
     P = create_problem(api, w)
