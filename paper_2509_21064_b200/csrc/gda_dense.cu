@@ -12,7 +12,8 @@
 //   D fp32 in TMEM: lane = restart b (128 per tile), column = variable i (256 per tile), two accumulator
 //   stages (2 x 256 = 512 columns) so the epilogue of tile t overlaps the MMAs of tile t+1.
 // With lanes = restarts the epilogue's accesses to the fp32 state X, Y ([n][B]) are coalesced 128-byte
-// rows per warp, and each thread writes 64 contiguous bytes of the next bf16 operand.
+// rows per warp; the next bf16 operand ([B][n], a restart's variables contiguous) leaves through a swizzled staging
+// tile per warp in shared memory and TMA stores of 32 x 64 boxes (whole 128-byte lines).
 //
 // Warp roles (384 threads, one persistent CTA per SM): warp 0 TMA producer, warp 1 MMA issuer (one
 // elected thread), warp 2 TMEM allocator, warps 4-11 epilogue (two warpgroups, half of the tile's columns each).
@@ -56,11 +57,14 @@ constexpr int BM = 128, BN = 256, BK = 64, UMMA_K = 16, BBOX = 64;   // BBOX: ro
 constexpr int A_BYTES = BM * BK * 2;
 constexpr int NUM_THREADS = 384, EPI_WARP0 = 4, EPI_WARPS = 8;
 constexpr int TMEM_COLS = 512;
+// epilogue staging of the NEXT bf16 operand: per epilogue warp 32 restarts x 64 variables (128-byte rows, 128-byte swizzle),
+// written back by TMA stores as whole 128-byte lines (16-byte stores straight from registers leave half-filled sectors)
+constexpr int ZST_COLS = 64, ZST_WARP_BYTES = 32 * ZST_COLS * 2, ZST_BYTES = 8 * ZST_WARP_BYTES;
 // per CTA and pipeline stage: its 128 rows of A and its 256 / CG rows of Q; 4 stages of 48 KB or 6 stages of 32 KB
 template <int CG> struct Pipe {
     static constexpr int STAGE_BYTES = A_BYTES + (BN / CG) * BK * 2;
     static constexpr int STAGES = CG == 1 ? 4 : GDA_DENSE_STAGES;
-    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 256 + 1024;     // tiles + barriers + alignment slack
+    static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + ZST_BYTES + 256 + 1024;   // tiles + operand staging + barriers + alignment slack
 };
 
 enum { MODE_STEP = 0, MODE_GRAD = 1, MODE_SCORE = 2, MODE_STEP_S = 3 };   // MODE_STEP_S: PDBO-s step (one multiplier per restart)
@@ -167,6 +171,18 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&v)[16]) {
           "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
         : "r"(taddr) : "memory");
 }
+// TMA store of one box from shared memory (bulk async-group completion)
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t src, int c0, int c1) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+                 ::"l"(map), "r"(src), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // K-major, 128-byte-swizzled shared-memory operand descriptor (rows of 64 bf16 = 128 B, 8-row groups 1024 B apart)
@@ -217,12 +233,13 @@ __device__ __forceinline__ int num_units(int n, int B, int cg, int pm_n, int pn_
 template <int MODE, int GFUN, int CG, int PM, int PN>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
-                  const DenseArgs args) {
+                  const __grid_constant__ CUtensorMap tmap_zo, const DenseArgs args) {
     constexpr int STAGES = Pipe<CG>::STAGES, STAGE_BYTES = Pipe<CG>::STAGE_BYTES;
     constexpr bool STEP = MODE == MODE_STEP || MODE == MODE_STEP_S, SDUAL = MODE == MODE_STEP_S;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;            // SWIZZLE_128B needs 1024 B alignment
-    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;
+    const uint32_t zst_base = smem_base + STAGES * STAGE_BYTES;                  // 1024-byte aligned (stages are multiples of 1 KB)
+    const uint32_t bar_base = zst_base + ZST_BYTES;
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
     auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + s); };
@@ -244,6 +261,7 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_a) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_b) : "memory");
+        if (STEP) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap_zo) : "memory");
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), NP); }
@@ -375,14 +393,16 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
             tc_fence_after();
             double score = 0.0;
             if (STEP) {
-                // Rounds of 16 variables: 32 loads, 16 updates in registers, 32 + 2 stores (double buffering, more warps and
-                // bulk-async staging were all measured: no faster).  PDBO-s (SDUAL): the multiplier is
+                // Rounds of 16 variables: 32 loads, 16 updates in registers, 32 stores + 32 bytes of the next operand into the
+                // staging tile (double buffering with and without setmaxnreg, more warps and bulk-async staging of x, y were
+                // all measured: no faster).  PDBO-s (SDUAL): the multiplier is
                 // one number per restart, y is neither read nor written, and the thread's sum of g(x_i^t) over its 128
                 // variables goes to gpart.
                 const int c_first = half * hcols;                                 // this warpgroup's first column in the tile
                 float* __restrict__ xp = args.x + (size_t)(t.n0 + c_first) * args.B + b;
                 float* __restrict__ yp = args.y + (size_t)(t.n0 + c_first) * args.B + b;
-                uint4* zdst = reinterpret_cast<uint4*>(args.zt_out + (size_t)b * args.n + t.n0 + c_first);
+                const uint32_t zst_warp = zst_base + (uint32_t)ew * ZST_WARP_BYTES;  // this warp's staging tile: row = lane
+                const uint32_t zst_row = zst_warp + (uint32_t)lane * 128u;
                 const uint32_t trow = tmem_base + ((uint32_t)(lane_grp * 32) << 16) + (uint32_t)(as * BN + c_first);
                 const int rounds = hcols / 16;
                 const float mu_b = SDUAL ? __ldg(args.mu + b) : 0.0f;
@@ -425,6 +445,13 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
                         xp[(size_t)(16 * r + j) * args.B] = xt[j];
                         if (!SDUAL) yp[(size_t)(16 * r + j) * args.B] = yv[j];
                     }
+                    // next operand: 16 bf16 of this restart's row into the warp's staging tile (16-byte chunk c of row l
+                    // sits at chunk c ^ (l & 7): the 128-byte swizzle of the store map, and conflict-free); every fourth
+                    // round one lane hands the 32 x 64 tile to the TMA unit
+                    if ((r & 3) == 0) {
+                        if (lane == 0) bulk_wait_read0();                         // the previous tile has left shared memory
+                        __syncwarp();
+                    }
 #pragma unroll
                     for (int q = 0; q < 2; ++q) {
                         uint32_t pk[4];
@@ -433,7 +460,16 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
                             const __nv_bfloat162 z2 = __floats2bfloat162_rn(xt[8 * q + 2 * e] - 0.5f, xt[8 * q + 2 * e + 1] - 0.5f);
                             pk[e] = *reinterpret_cast<const uint32_t*>(&z2);
                         }
-                        zdst[2 * r + q] = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                        const uint32_t chunk = (uint32_t)(2 * (r & 3) + q);
+                        st_shared_v4(zst_row + ((chunk ^ (uint32_t)(lane & 7)) << 4), pk[0], pk[1], pk[2], pk[3]);
+                    }
+                    if ((r & 3) == 3) {
+                        fence_async_smem();
+                        __syncwarp();
+                        if (lane == 0) {
+                            tma_store_2d(&tmap_zo, zst_warp, t.n0 + c_first + ZST_COLS * (r >> 2), t.m0 + lane_grp * 32);
+                            bulk_commit();
+                        }
                     }
                 };
 #pragma unroll 1
@@ -480,6 +516,7 @@ dense_gemm_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_const
                 if (CG == 1) mbar_arrive(tempty_bar(as)); else mbar_arrive_cluster(map_to_cta(tempty_bar(as), (uint32_t)lead));
             }
         }
+        if (STEP && lane == 0) bulk_wait0();                  // this lane's operand stores are complete before the CTA retires
     }
     tc_fence_before();
     if (CSIZE > 1) cluster_sync_all(); else __syncthreads();      // no CTA leaves while its peer may still signal or read it
@@ -543,7 +580,8 @@ gda_status make_tmap(CUtensorMap* map, const void* base, uint64_t rows, uint64_t
 
 struct DenseHost {
     CUtensorMap tmap_q;
-    CUtensorMap tmap_z[2];
+    CUtensorMap tmap_z[2];              // operand loads: boxes of 64 rows
+    CUtensorMap tmap_zs[2];             // operand stores from the epilogue: boxes of 32 rows (one epilogue warp's restarts)
     const void* z_ptr[2] = {nullptr, nullptr};
     int32_t z_B = 0;
     // co-resident clusters per kernel variant (1 CTA per SM), see configure_variant
@@ -598,7 +636,7 @@ gda_status configure_all(gda_problem* p) {
 }
 
 template <int MODE, int GFUN, int CG, int PM, int PN>
-gda_status launch_variant(gda_problem* p, const CUtensorMap& ta, const CUtensorMap& tq, const DenseArgs& a, cudaStream_t s) {
+gda_status launch_variant(gda_problem* p, const CUtensorMap& ta, const CUtensorMap& tq, const CUtensorMap& tzo, const DenseArgs& a, cudaStream_t s) {
     auto kern = dense_gemm_kernel<MODE, GFUN, CG, PM, PN>;
     constexpr int CSIZE = CG * PM * PN;
     const int max_clusters = static_cast<DenseHost*>(p->tmap_Q)->max_clusters[(MODE * 2 + GFUN) * NUM_SHAPES + shape_index(CG, PM, PN)];
@@ -613,13 +651,13 @@ gda_status launch_variant(gda_problem* p, const CUtensorMap& ta, const CUtensorM
     const int rounds = (units + max_clusters - 1) / max_clusters;
     const int clusters = (units + rounds - 1) / rounds;       // fewest clusters that still finish in `rounds` rounds
     cfg.gridDim = dim3((unsigned)(clusters * CSIZE));
-    GDA_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tq, a));
+    GDA_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ta, tq, tzo, a));
     return GDA_OK;
 }
 
 // GDA_DENSE_SHAPE=0..3 forces a launch shape the sizes allow (tests, A/B timing); default: the largest cluster that fits
 template <int MODE, int GFUN>
-gda_status launch_gemm(gda_problem* p, const CUtensorMap& ta, const DenseArgs& a, cudaStream_t s) {
+gda_status launch_gemm(gda_problem* p, const CUtensorMap& ta, const CUtensorMap& tzo, const DenseArgs& a, cudaStream_t s) {
     DenseHost* h = static_cast<DenseHost*>(p->tmap_Q);
     int shape = a.B % (BM * 2) != 0 ? 0 : a.n % (BN * 2) != 0 ? 1 : a.B % (BM * 4) != 0 ? 2 : 3;
     if (shape == 3 && h->forced_shape < 0) {
@@ -633,22 +671,28 @@ gda_status launch_gemm(gda_problem* p, const CUtensorMap& ta, const DenseArgs& a
     }
     if (h->forced_shape >= 0 && h->forced_shape < shape) shape = h->forced_shape;
     switch (shape) {
-        case 0: return launch_variant<MODE, GFUN, 1, 1, 1>(p, ta, h->tmap_q, a, s);
-        case 1: return launch_variant<MODE, GFUN, 2, 1, 1>(p, ta, h->tmap_q, a, s);
-        case 2: return launch_variant<MODE, GFUN, 2, 1, 2>(p, ta, h->tmap_q, a, s);
-        default: return launch_variant<MODE, GFUN, 2, 2, 2>(p, ta, h->tmap_q, a, s);
+        case 0: return launch_variant<MODE, GFUN, 1, 1, 1>(p, ta, h->tmap_q, tzo, a, s);
+        case 1: return launch_variant<MODE, GFUN, 2, 1, 1>(p, ta, h->tmap_q, tzo, a, s);
+        case 2: return launch_variant<MODE, GFUN, 2, 1, 2>(p, ta, h->tmap_q, tzo, a, s);
+        default: return launch_variant<MODE, GFUN, 2, 2, 2>(p, ta, h->tmap_q, tzo, a, s);
     }
 }
 
-gda_status z_maps(gda_problem* p, int32_t B, const __nv_bfloat16* zt, const CUtensorMap** out) {
+// the load map of an operand buffer and (store != NULL) its store map
+gda_status z_maps(gda_problem* p, int32_t B, const __nv_bfloat16* zt, const CUtensorMap** load, const CUtensorMap** store = nullptr) {
     DenseHost* h = static_cast<DenseHost*>(p->tmap_Q);
-    for (int k = 0; k < 2; ++k)
-        if (h->z_ptr[k] == zt && h->z_B == B) { *out = &h->tmap_z[k]; return GDA_OK; }
-    if (h->z_B != B) { h->z_ptr[0] = h->z_ptr[1] = nullptr; h->z_B = B; }
-    const int k = h->z_ptr[0] == nullptr ? 0 : 1;
-    GDA_TRY(make_tmap(&h->tmap_z[k], zt, (uint64_t)B, (uint64_t)p->n_pad, BBOX));
-    h->z_ptr[k] = zt;
-    *out = &h->tmap_z[k];
+    int k = -1;
+    for (int q = 0; q < 2; ++q)
+        if (h->z_ptr[q] == zt && h->z_B == B) k = q;
+    if (k < 0) {
+        if (h->z_B != B || (h->z_ptr[0] && h->z_ptr[1])) { h->z_ptr[0] = h->z_ptr[1] = nullptr; h->z_B = B; }   // stale entries
+        k = h->z_ptr[0] == nullptr ? 0 : 1;
+        GDA_TRY(make_tmap(&h->tmap_z[k], zt, (uint64_t)B, (uint64_t)p->n_pad, BBOX));
+        GDA_TRY(make_tmap(&h->tmap_zs[k], zt, (uint64_t)B, (uint64_t)p->n_pad, 32));
+        h->z_ptr[k] = zt;
+    }
+    if (load) *load = &h->tmap_z[k];
+    if (store) *store = &h->tmap_zs[k];
     return GDA_OK;
 }
 
@@ -706,18 +750,20 @@ gda_status dense_make_operand(gda_problem* p, int32_t B, const float* x, __nv_bf
 gda_status dense_step(gda_problem* p, int32_t B, float* x, float* y, const __nv_bfloat16* zt_in, __nv_bfloat16* zt_out,
                       const UpdParams& up, const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s,
                       int64_t* launches) {
-    const CUtensorMap* ta;
+    const CUtensorMap *ta, *tzo;
     GDA_TRY(z_maps(p, B, zt_in, &ta));
+    GDA_TRY(z_maps(p, B, zt_out, nullptr, &tzo));
+    GDA_TRY(z_maps(p, B, zt_in, &ta));                        // (a miss on zt_out may have dropped stale entries)
     DenseArgs a{};
     a.n = p->n_pad; a.B = B; a.x = x; a.y = y; a.zt_out = zt_out; a.hvec = p->d_rowsum; a.cprime = p->d_cprime;
     a.up = up; a.st = st; a.t_off = t_off; a.mu = sd.mu; a.gpart = sd.gpart;
     if (launches) ++*launches;
     if (sd.mu) {                                               // PDBO-s
-        if (up.gfun == GDA_G_QUADRATIC) return launch_gemm<MODE_STEP_S, GDA_G_QUADRATIC>(p, *ta, a, s);
-        return launch_gemm<MODE_STEP_S, GDA_G_ENTROPY>(p, *ta, a, s);
+        if (up.gfun == GDA_G_QUADRATIC) return launch_gemm<MODE_STEP_S, GDA_G_QUADRATIC>(p, *ta, *tzo, a, s);
+        return launch_gemm<MODE_STEP_S, GDA_G_ENTROPY>(p, *ta, *tzo, a, s);
     }
-    if (up.gfun == GDA_G_QUADRATIC) return launch_gemm<MODE_STEP, GDA_G_QUADRATIC>(p, *ta, a, s);
-    return launch_gemm<MODE_STEP, GDA_G_ENTROPY>(p, *ta, a, s);
+    if (up.gfun == GDA_G_QUADRATIC) return launch_gemm<MODE_STEP, GDA_G_QUADRATIC>(p, *ta, *tzo, a, s);
+    return launch_gemm<MODE_STEP, GDA_G_ENTROPY>(p, *ta, *tzo, a, s);
 }
 
 // gda_grad: operand from x (centred), GEMM, G written out.  Uses zt[0] of the workspace as scratch.
@@ -729,7 +775,7 @@ gda_status dense_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaS
     GDA_TRY(z_maps(p, B, ws.zt[0], &ta));
     DenseArgs a{};
     a.n = p->n_pad; a.B = B; a.hvec = p->d_rowsum; a.cprime = p->d_cprime; a.gout = G;
-    return launch_gemm<MODE_GRAD, GDA_G_QUADRATIC>(p, *ta, a, s);
+    return launch_gemm<MODE_GRAD, GDA_G_QUADRATIC>(p, *ta, *ta, a, s);
 }
 
 int32_t dense_num_partials(const gda_problem* p, int32_t) { return p->n_pad / 128; }
@@ -747,5 +793,5 @@ gda_status dense_score_partials(gda_problem* p, int32_t B, const float* x, void*
     a.partial = static_cast<double*>(partial);
     *n_part = dense_num_partials(p, B);
     if (launches) ++*launches;
-    return launch_gemm<MODE_SCORE, GDA_G_QUADRATIC>(p, *ta, a, s);
+    return launch_gemm<MODE_SCORE, GDA_G_QUADRATIC>(p, *ta, *ta, a, s);
 }
