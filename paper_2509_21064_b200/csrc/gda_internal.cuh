@@ -132,6 +132,7 @@ struct gda_problem {
     float* d_cprime = nullptr;           // also used by the dense path
     int32_t* d_heavy_rows = nullptr; int32_t n_heavy = 0;   // rows handled by the row-split kernel
     int32_t* d_light_rows = nullptr; int32_t n_light = 0;   // nullptr = all rows, in order
+    int32_t* d_local_rows = nullptr;                         // the light rows grouped by adjacency (locality_order), or nullptr
     int32_t max_deg = 0;
     // slab path (small n, gda_sparse.cu): sliced ELL of (column byte offset, val2) pairs, 16 rows per group
     int2* d_slab_ent = nullptr; int32_t* d_slab_goff = nullptr; int32_t* d_slab_grow = nullptr;

@@ -645,7 +645,8 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     const bool pf = MODE == 0 && !DUAL && 12.0 * (double)p->n * (double)B > 0.8 * (double)p->l2_bytes;   // the streaming switch (see spmm_step_warp)
     if (n_light > 0) {
         const dim3 grid((unsigned)light_blocks, (unsigned)chunks);
-#define GDA_SP_ARGS n_light, p->d_light_rows, B, p->d_rowptr, p->d_col, p->d_val2, p->d_ell, p->d_cprime, x, y, xn, up, sd, st, t_off
+        const int32_t* row_list = (DUAL && p->d_local_rows) ? p->d_local_rows : p->d_light_rows;   // PDBO-s: rows grouped by adjacency
+#define GDA_SP_ARGS n_light, row_list, B, p->d_rowptr, p->d_col, p->d_val2, p->d_ell, p->d_cprime, x, y, xn, up, sd, st, t_off
 #define GDA_SP_PF(G, E) do { if (pf) spmm_step_warp<G, MODE, E, DUAL, (MODE == 0 && !DUAL)><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); \
                              else spmm_step_warp<G, MODE, E, DUAL, false><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); } while (0)
 #define GDA_SP_CASE(E) \

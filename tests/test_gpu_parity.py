@@ -666,6 +666,30 @@ def test_pdbo_s_free_running_and_full_run(api, oracle, w):
     P.destroy()
 
 
+def test_pdbo_s_row_grouping_is_bit_identical(api):
+    """The PDBO-s step kernel walks the rows grouped by adjacency (locality_order in gda_api.cu; GDA_SPARSE_LOCALITY=0, read
+    at create, switches the list off).  Which rows share a block changes nothing that is computed: the sums of g are exact
+    integers (fixed point), so iterates, multipliers and objectives agree bit for bit."""
+    import os
+    w = wl.pdbo_s_variant(wl.config(3, B=260, n_scale=0.2))
+    h = w.hyper
+    x0 = dev(wl.x0_uniform(w.problem.n, w.B, w.x0_seed))
+    prm = api.params_from_hyper(h, iters=230, eval_every=50)
+    res = []
+    for sw in ("1", "0"):
+        os.environ["GDA_SPARSE_LOCALITY"] = sw
+        try:
+            P = create_problem(api, w)
+        finally:
+            os.environ.pop("GDA_SPARSE_LOCALITY", None)
+        r = P.run(x0, h.lambda0, prm, want_final=True)
+        torch.cuda.synchronize()
+        res.append((r["x"].clone(), r["lam"].clone(), r["obj"].clone(), r["x_bin"].clone()))
+        P.destroy()
+    for a, b in zip(*res):
+        assert torch.equal(a, b)
+
+
 def test_pdbo_s_heavy_rows_and_argument_checks(api, oracle):
     Pw = star_plus_isolated(700, 5)                             # row-split kernel + empty rows
     OP = oracle_problem(Pw)
