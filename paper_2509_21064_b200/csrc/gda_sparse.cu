@@ -75,15 +75,18 @@ template <int GFUN, bool DUAL>
 __device__ __forceinline__ void update_store(int row, int c4, int B, bool active, float4 G, const float* __restrict__ x,
                                              float* __restrict__ y, float* __restrict__ xn,
                                              const UpdParams& up, uint32_t t, float4 mu, float4& gs) {
-    const size_t off = (size_t)row * B + 4 * c4;
-    const float4 xv = ldg4(x + off);
-    const float4 yv = DUAL ? mu : *reinterpret_cast<const float4*>(y + off);
+    // byte offset of (row, c4) as ONE 32 x 32 -> 64-bit multiply-add per array (n * B < 2^30 elements is checked by
+    // gda_run): the generic 64-bit index arithmetic costs a dozen instructions and a register pair more
+    const uint64_t off = (uint64_t)(uint32_t)row * (uint64_t)(4u * (uint32_t)B) + (uint64_t)(16u * (uint32_t)c4);
+    const float4 xv = __ldg(reinterpret_cast<const float4*>(reinterpret_cast<const char*>(x) + off));
+    float4* yp = reinterpret_cast<float4*>(reinterpret_cast<char*>(y) + off);
+    const float4 yv = DUAL ? mu : *yp;
     float4 xo, yo;
     gda_update4<GFUN>(xv, yv, G, up, t, (uint32_t)row, 4u * (uint32_t)c4, xo, yo);
     if (!active) return;
-    *reinterpret_cast<float4*>(xn + off) = xo;
+    *reinterpret_cast<float4*>(reinterpret_cast<char*>(xn) + off) = xo;
     if (DUAL) gs = make_float4(gda_g<GFUN>(xv.x, up), gda_g<GFUN>(xv.y, up), gda_g<GFUN>(xv.z, up), gda_g<GFUN>(xv.w, up));
-    else *reinterpret_cast<float4*>(y + off) = yo;
+    else *yp = yo;
 }
 
 // warp-per-(row, 128-restart chunk): blockIdx.y = chunk, the block's 8 warps take 8 consecutive rows.
