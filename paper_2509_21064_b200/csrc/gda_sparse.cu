@@ -21,6 +21,10 @@ namespace {
 
 constexpr int WARPS = 8;
 constexpr int THREADS = WARPS * 32;
+// warps per block of spmm_step_warp: 4 (12 blocks per SM) -- a block's slot is free only when its slowest warp is done, and
+// with 4 warps less of the SM waits (config 3: 14.9 -> 14.4 us per step, B = 1024: 66.6 -> 63.9 us); PDBO-s keeps 8: every
+// block ends in a reduction and a set of atomics, and twice the blocks cost more than they gain (19.1 -> 21.7 us)
+__host__ __device__ constexpr int warp_kernel_warps(bool dual) { return dual ? 8 : 4; }
 constexpr int HEAVY_DEG = 256;     // rows above this use the row-split kernel
 constexpr int SCORE_ROWS = 64;     // most rows per block in the scoring kernels (fewer when that leaves SMs idle)
 
@@ -99,15 +103,16 @@ __device__ __forceinline__ void update_store(int row, int c4, int B, bool active
 // DUAL (PDBO-s, MODE 0 only): the multiplier is one number per restart (sd.mu), y is not read or written, and the
 // block's sum of g(x_i^t) goes through scalar_dual_finish (fixed-point integer reductions; mu_finalize closes the step).
 template <int GFUN, int MODE, bool ELL, bool DUAL, bool PF>
-__global__ void __launch_bounds__(THREADS, 6)
+__global__ void __launch_bounds__(32 * warp_kernel_warps(DUAL), 6 * 8 / warp_kernel_warps(DUAL))
 spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
                const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                const float* __restrict__ val2, const int32_t* __restrict__ ell, const float* __restrict__ cprime,
                const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
                UpdParams up, ScalarDual sd, const RunState* __restrict__ st, uint32_t t_off) {
-    __shared__ float4 gred[DUAL ? WARPS : 1][32];
+    constexpr int WW = warp_kernel_warps(DUAL);
+    __shared__ float4 gred[DUAL ? WW : 1][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int ridx = blockIdx.x * WARPS + warp;
+    const int ridx = blockIdx.x * WW + warp;
     const bool active = 4 * (blockIdx.y * 32 + lane) < B;
     const int c4 = active ? blockIdx.y * 32 + lane : B / 4 - 1;      // ragged B: idle lanes recompute the last float4
     if (DUAL) {
@@ -129,7 +134,7 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
             G.x += cp; G.y += cp; G.z += cp; G.w += cp;
             update_store<GFUN, true>(row, c4, B, active, G, x, y, xn, up, (st ? st->t : 0u) + t_off, mu, gs);
         }
-        scalar_dual_finish<WARPS>(gs, gred, warp, lane, active, c4, blockIdx.x, sd);
+        scalar_dual_finish<WW>(gs, gred, warp, lane, active, c4, blockIdx.x, sd);
         return;
     }
     if (ridx >= n_rows) return;                              // warp-uniform
@@ -644,14 +649,15 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
         return GDA_OK;
     }
     const int n_light = p->d_light_rows ? p->n_light : p->n;
-    const int light_blocks = (n_light + WARPS - 1) / WARPS;
+    constexpr int WW = warp_kernel_warps(DUAL), WTHREADS = 32 * WW;
+    const int light_blocks = (n_light + WW - 1) / WW;
     const bool pf = MODE == 0 && !DUAL && 12.0 * (double)p->n * (double)B > 0.8 * (double)p->l2_bytes;   // the streaming switch (see spmm_step_warp)
     if (n_light > 0) {
         const dim3 grid((unsigned)light_blocks, (unsigned)chunks);
         const int32_t* row_list = (DUAL && p->d_local_rows) ? p->d_local_rows : p->d_light_rows;   // PDBO-s: rows grouped by adjacency
 #define GDA_SP_ARGS n_light, row_list, B, p->d_rowptr, p->d_col, p->d_val2, p->d_ell, p->d_cprime, x, y, xn, up, sd, st, t_off
-#define GDA_SP_PF(G, E) do { if (pf) spmm_step_warp<G, MODE, E, DUAL, (MODE == 0 && !DUAL)><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); \
-                             else spmm_step_warp<G, MODE, E, DUAL, false><<<grid, THREADS, 0, s>>>(GDA_SP_ARGS); } while (0)
+#define GDA_SP_PF(G, E) do { if (pf) spmm_step_warp<G, MODE, E, DUAL, (MODE == 0 && !DUAL)><<<grid, WTHREADS, 0, s>>>(GDA_SP_ARGS); \
+                             else spmm_step_warp<G, MODE, E, DUAL, false><<<grid, WTHREADS, 0, s>>>(GDA_SP_ARGS); } while (0)
 #define GDA_SP_CASE(E) \
         if (up.gfun == GDA_G_QUADRATIC) GDA_SP_PF(GDA_G_QUADRATIC, E); else GDA_SP_PF(GDA_G_ENTROPY, E)
         if (p->d_ell) { GDA_SP_CASE(true); } else { GDA_SP_CASE(false); }
