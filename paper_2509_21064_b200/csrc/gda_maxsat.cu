@@ -17,6 +17,9 @@ namespace {
 
 constexpr int WARPS = 8;
 constexpr int THREADS = WARPS * 32;
+// warps per block of the step kernel: 2 -- a block's slot frees only when its slowest warp is done (config 5: 41.05 us per
+// step with 8 warps, 39.75 with 4, 39.35 with 2); PDBO-s: 8, one gpart row per block of 8 variables
+__host__ __device__ constexpr int step_warps(bool dual) { return dual ? WARPS : 2; }
 constexpr int SCORE_CLAUSES = 128;
 
 // Slot records hold each OTHER literal encoded as  enc = var | (positive ? 0x80000000 : 0);  ENC_PAD marks padding.
@@ -104,18 +107,19 @@ __device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, con
 // MODE 0: fused step; MODE 1: write G only.  DUAL (PDBO-s, MODE 0): one multiplier per restart (sd.mu),
 // y untouched, the block's sum of g(x_i^t) goes to sd.gpart[blockIdx.x].
 template <int GFUN, int MODE, int KW, bool PAD, bool DUAL>
-__global__ void __launch_bounds__(THREADS)
+__global__ void __launch_bounds__(32 * step_warps(DUAL))
 maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* __restrict__ coef,
                    const int32_t* __restrict__ others, int kw, const float* __restrict__ x,
                    float* __restrict__ y, float* __restrict__ xn, UpdParams up, ScalarDual sd,
                    const RunState* __restrict__ st, uint32_t t_off) {
-    __shared__ float4 gred[DUAL ? WARPS : 1][32];
+    constexpr int SW = step_warps(DUAL);
+    __shared__ float4 gred[DUAL ? SW : 1][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int c4 = blockIdx.y * 32 + lane;
     const bool active = 4 * c4 < B;
     float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = gs;
     if (DUAL) mu = ldg4(sd.mu + 4 * (active ? c4 : B / 4 - 1));
-    const int var = blockIdx.x * WARPS + warp;
+    const int var = blockIdx.x * SW + warp;
     if (var < n) {                                           // warp-uniform
         const int start = __ldg(vptr + var), end = __ldg(vptr + var + 1);
         const float4 G = gather_var<KW, PAD>(coef, others, kw, start, end, x, B, c4, active, lane);
@@ -135,7 +139,7 @@ maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* 
             }
         }
     }
-    if (DUAL) scalar_dual_block_sum<WARPS>(gs, gred, warp, lane, active, sd.gpart + (size_t)blockIdx.x * B + 4 * c4);
+    if (DUAL) scalar_dual_block_sum<SW>(gs, gred, warp, lane, active, sd.gpart + (size_t)blockIdx.x * B + 4 * c4);
 }
 
 // S5: partial[cb][b] = sum over the clauses of block cb of w_j [every literal of C_j false under x_hat]
@@ -223,13 +227,13 @@ void launch_kw(gda_problem* p, int32_t B, dim3 grid, const float* x, float* y, f
                const UpdParams& up, const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s) {
 #define GDA_MS_ARGS p->n, B, p->d_vptr, p->d_coef, p->d_others, p->kw, x, y, xn, up, sd, st, t_off
 #define GDA_MS_CASE(K) \
-        case K: if (pad) maxsat_step_kernel<GFUN, MODE, K, true, DUAL><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); \
-                else maxsat_step_kernel<GFUN, MODE, K, false, DUAL><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        case K: if (pad) maxsat_step_kernel<GFUN, MODE, K, true, DUAL><<<grid, 32 * step_warps(DUAL), 0, s>>>(GDA_MS_ARGS); \
+                else maxsat_step_kernel<GFUN, MODE, K, false, DUAL><<<grid, 32 * step_warps(DUAL), 0, s>>>(GDA_MS_ARGS); break;
     // records hold ENC_PAD when clauses are shorter than kmax -- and ALWAYS when kmax == 1 (kw is then 1 with no other literal)
     const bool pad = p->kmin != p->kmax || p->kmax == 1;
     switch (p->kw) {
         GDA_MS_CASE(1) GDA_MS_CASE(2) GDA_MS_CASE(3) GDA_MS_CASE(4)
-        default: maxsat_step_kernel<GFUN, MODE, 0, true, DUAL><<<grid, THREADS, 0, s>>>(GDA_MS_ARGS); break;
+        default: maxsat_step_kernel<GFUN, MODE, 0, true, DUAL><<<grid, 32 * step_warps(DUAL), 0, s>>>(GDA_MS_ARGS); break;
     }
 #undef GDA_MS_CASE
 #undef GDA_MS_ARGS
@@ -238,7 +242,7 @@ void launch_kw(gda_problem* p, int32_t B, dim3 grid, const float* x, float* y, f
 template <int MODE, bool DUAL>
 gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
-    const int groups = (p->n + WARPS - 1) / WARPS, chunks = (B / 4 + 31) / 32;
+    const int groups = (p->n + step_warps(DUAL) - 1) / step_warps(DUAL), chunks = (B / 4 + 31) / 32;
     const dim3 grid((unsigned)groups, (unsigned)chunks);
     if (up.gfun == GDA_G_QUADRATIC) launch_kw<GDA_G_QUADRATIC, MODE, DUAL>(p, B, grid, x, y, xn, up, sd, st, t_off, s);
     else launch_kw<GDA_G_ENTROPY, MODE, DUAL>(p, B, grid, x, y, xn, up, sd, st, t_off, s);
