@@ -172,14 +172,15 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
 // Here G = the smallest power of two >= B / 4 lanes serve one row and a warp takes 32 / G rows at once: lane = (row in
 // the warp, float4 of restarts).  Every lane walks its OWN row's entries (the loads of (col, val) are broadcasts inside
 // its lane group), four gathers in flight, up to the longest row of the warp with the shorter rows predicated off.
+constexpr int NARROW_WARPS = 4;      // per block (MIS n = 5e4, d = 100, B = 12: 46.6 us per step with 8, 42.5 with 4 or 2, 46.1 with 1)
 template <int GFUN, int G>
-__global__ void __launch_bounds__(THREADS)
+__global__ void __launch_bounds__(32 * NARROW_WARPS)
 spmm_step_narrow(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                  const float* __restrict__ val2, const float* __restrict__ cprime, const float* __restrict__ x,
                  float* __restrict__ y, float* __restrict__ xn, UpdParams up, const RunState* __restrict__ st, uint32_t t_off) {
     constexpr int R = 32 / G;                                // rows per warp
     const int lane = threadIdx.x & 31;
-    const int row_raw = (blockIdx.x * WARPS + (threadIdx.x >> 5)) * R + lane / G;
+    const int row_raw = (blockIdx.x * NARROW_WARPS + (threadIdx.x >> 5)) * R + lane / G;
     const int cl = lane % G;
     const bool active = row_raw < n && 4 * cl < B;
     const int row = min(row_raw, n - 1);                     // idle lanes recompute a valid element, only stores are suppressed
@@ -638,10 +639,10 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     if (MODE == 0 && !DUAL && B <= 64) {                      // few restarts: several rows per warp
         int G = 1;
         while (4 * G < B) G <<= 1;
-        const unsigned grid = (unsigned)((p->n + WARPS * (32 / G) - 1) / (WARPS * (32 / G)));
+        const unsigned grid = (unsigned)((p->n + NARROW_WARPS * (32 / G) - 1) / (NARROW_WARPS * (32 / G)));
 #define GDA_NW_CASE(GG) case GG: \
-        if (up.gfun == GDA_G_QUADRATIC) spmm_step_narrow<GDA_G_QUADRATIC, GG><<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off); \
-        else spmm_step_narrow<GDA_G_ENTROPY, GG><<<grid, THREADS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off); break;
+        if (up.gfun == GDA_G_QUADRATIC) spmm_step_narrow<GDA_G_QUADRATIC, GG><<<grid, 32 * NARROW_WARPS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off); \
+        else spmm_step_narrow<GDA_G_ENTROPY, GG><<<grid, 32 * NARROW_WARPS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off); break;
         switch (G) { GDA_NW_CASE(1) GDA_NW_CASE(2) GDA_NW_CASE(4) GDA_NW_CASE(8) GDA_NW_CASE(16) default: break; }
 #undef GDA_NW_CASE
         if (launches) ++*launches;
