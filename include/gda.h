@@ -13,7 +13,11 @@
  *   - "HOST" / "DEVICE" says where a pointer must live.  The library never frees or keeps caller memory
  *     (problem data is copied at create).
  *   - Iterates are fp32, layout [n][B] row-major: element (variable i, restart b) at i*B + b, so the
- *     restart index is contiguous.  B must be a positive multiple of 4 (128-bit vectors across restarts).
+ *     restart index is contiguous.  Any B >= 1 is served (the paper runs B = 1, 10, 100, 1000: PAPER.md:836-843, 873-878):
+ *     the kernels work on 128-bit vectors of 4 restarts, so inside its workspace the library pads the restart axis with
+ *     zero-initialised restarts up to a multiple of 4 (dense problems: 128) that run along and are never read -- not by
+ *     the evaluation, the trace, the arg-best or the copies out.  With B % 4 != 0 gda_grad / gda_score / gda_lagrangian go
+ *     through zero-padded copies in the workspace (and, like dense problems always, invalidate a state to resume from).
  *   - gda_run / gda_grad / gda_score enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream) and return without synchronising; outputs are valid once the stream has
  *     reached that point.  A handle must not be used from two streams or threads at the same time; different
@@ -65,7 +69,7 @@ gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, const int32_t* 
 /* gda_create_qubo_dense: HOST Q row-major [n][n] (symmetric), HOST c[n] or NULL.  flags must contain
  *   GDA_DENSE_BF16: Q is rounded to bf16 (lossless when Q is bf16-representable, reading R13)
  *   and the gradient is a tcgen05 GEMM with fp32 accumulation.  UNSUPPORTED: flags without GDA_DENSE_BF16.
- *   Any n > 0 and any B (a multiple of 4) are served: internally n is zero-padded to a multiple of 256 and B to a
+ *   Any n > 0 and any B > 0 are served: internally n is zero-padded to a multiple of 256 and B to a
  *   multiple of 128 (the GEMM tile), which costs the padded work but changes no result. */
 gda_status gda_create_qubo_dense(int32_t n, const float* Q, const float* c, int32_t flags, gda_problem** out);
 
@@ -140,7 +144,7 @@ typedef struct {
  *   obj         DEVICE double [B]: F(x_bin[:,b]) -- exact integers when all coefficients are integers
  *   best_restart DEVICE int32 [1]: argmin_b obj[b], ties -> lowest b (R6)
  * UNSUPPORTED: n * B >= 2^30 elements (after the dense path's padding; times k for Max-k-Cut).
- * INVALID_ARG: null required pointer, B <= 0 or B % 4 != 0, alpha <= 0, beta < 0 or non-finite, delta outside
+ * INVALID_ARG: null required pointer, B <= 0, alpha <= 0, beta < 0 or non-finite, delta outside
  * [0, 1/2), eval_every <= 0, iters < 0, unknown gfun or dual, log_eps outside (0, 1/2) with the entropy g;
  * a resumed run (x0 == NULL) whose `dual` differs from the run it continues.                              */
 gda_status gda_run(gda_problem* p, int32_t B, const float* x0, const float* lambda0, float lambda0_scalar,

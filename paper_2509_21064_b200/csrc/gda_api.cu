@@ -451,7 +451,10 @@ static gda_status dmalloc(T** ptr, size_t count) {
 
 static const int32_t TRACE_CAP = 4096;
 
-static int32_t lead_dim(const gda_problem* p, int32_t B) { return p->kind == GDA_KIND_DENSE ? (B + 127) / 128 * 128 : B; }
+// Row stride of the state arrays: the kernels work on float4s of restarts (dense: on 128-restart tiles), so any B >= 1 is served
+// by zero-initialised PADDING RESTARTS up to the next multiple of 4 (128).  They run like any other restart and are never read:
+// the evaluation, the trace, the arg-best and the copies out see the first B columns.
+static int32_t lead_dim(const gda_problem* p, int32_t B) { return p->kind == GDA_KIND_DENSE ? (B + 127) / 128 * 128 : (B + 3) / 4 * 4; }
 
 static gda_status ensure_workspace(gda_problem* p, int32_t B) {
     Workspace& ws = p->ws;
@@ -487,10 +490,10 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
         if (st == GDA_OK) st = dmalloc(&ws.mu[0], (size_t)ld);
         if (st == GDA_OK) st = dmalloc(&ws.mu[1], (size_t)ld);
         if (st == GDA_OK) st = dmalloc(&ws.gpart, (size_t)ws.n_gpart * ld);
-        if (st == GDA_OK && p->kind == GDA_KIND_SPARSE) st = dmalloc(&ws.gacc, (size_t)GDA_GACC_WAYS * B);
+        if (st == GDA_OK && p->kind == GDA_KIND_SPARSE) st = dmalloc(&ws.gacc, (size_t)GDA_GACC_WAYS * ld);
     }
     if (st == GDA_OK) st = dmalloc(&ws.state, 1);
-    if (st == GDA_OK) st = dmalloc(&ws.block_min, (size_t)(B + 31) / 32);
+    if (st == GDA_OK) st = dmalloc(&ws.block_min, (size_t)(ld + 7) / 8);          // one per block of finalize_kernel (32 restarts) or of the slab kernel (8)
     if (st == GDA_OK) st = dmalloc(&ws.best_restart, 1);
     if (st == GDA_OK) st = dmalloc(&ws.best_val, 1);
     ws.trace_cap = TRACE_CAP;
@@ -555,37 +558,37 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     if (p->kind == GDA_KIND_SPARSE && !scalar) {              // small n: steps AND evaluation in one launch, state on chip
         int slab = 0;
         const int64_t before = *launches;
-        GDA_TRY(sparse_chunk_slab(p, B, len, ws.x[cur], ws.x[cur ^ (len & 1)], ws.y, up, s, launches, &slab));   // buffer parity as the per-step kernels leave it
+        GDA_TRY(sparse_chunk_slab(p, B, ws.ld, len, ws.x[cur], ws.x[cur ^ (len & 1)], ws.y, up, s, launches, &slab));   // buffer parity as the per-step kernels leave it
         if (slab) { *step_launches += *launches - before; return GDA_OK; }
     }
     for (int k = 0; k < len; ++k) {
         int64_t before = *launches;
         ScalarDual sd;                                        // PDBO-s: mu follows the parity of x
-        if (scalar) { sd.mu = ws.mu[cur]; sd.gpart = ws.gpart; sd.gacc = ws.gacc; sd.B = B; }
+        if (scalar) { sd.mu = ws.mu[cur]; sd.gpart = ws.gpart; sd.gacc = ws.gacc; sd.B = ws.ld; }
         if (p->kind == GDA_KIND_SPARSE)
-            GDA_TRY(sparse_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
+            GDA_TRY(sparse_step(p, ws.ld, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         else if (p->kind == GDA_KIND_MAXSAT)
-            GDA_TRY(maxsat_step(p, B, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
+            GDA_TRY(maxsat_step(p, ws.ld, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         else if (p->kind == GDA_KIND_KCUT)
-            GDA_TRY(kcut_step(p, B, ws.x[cur], ws.z, ws.y, ws.x[cur ^ 1], up, s, launches));
+            GDA_TRY(kcut_step(p, ws.ld, ws.x[cur], ws.z, ws.y, ws.x[cur ^ 1], up, s, launches));
         else
             GDA_TRY(dense_step(p, ws.ld, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         if (scalar && p->kind != GDA_KIND_SPARSE)
             GDA_TRY(gsum_reduce(ws.ld, ws.gpart, ws.n_gpart, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
         else if (scalar)
-            GDA_TRY(mu_finalize(B, ws.gacc, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
+            GDA_TRY(mu_finalize(ws.ld, ws.gacc, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
         *step_launches += *launches - before;
         cur ^= 1;
     }
     const float* xcur = (p->kind == GDA_KIND_DENSE) ? ws.x[0] : ws.x[cur];
     int32_t n_part = 0;
-    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
-    else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, xcur, ws.partial, &n_part, s, launches));
-    else if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_score_partials(p, B, ws.z, ws.lab, ws.partial, &n_part, s, launches));
+    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, ws.ld, xcur, ws.partial, &n_part, s, launches));
+    else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, ws.ld, xcur, ws.partial, &n_part, s, launches));
+    else if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_score_partials(p, ws.ld, ws.z, ws.lab, ws.partial, &n_part, s, launches));
     else { ws.score_scratch = cur ^ 1; GDA_TRY(dense_score_partials(p, ws.ld, xcur, ws.partial, &n_part, s, launches)); }
     GDA_TRY(eval_finalize(p, B, ws.ld, ws.partial, n_part, ws.obj_now, ws.best_obj, ws.improved, ws.state, ws.trace_best,
                           ws.trace_ns, ws.trace_cap, (uint32_t)len, s, launches));
-    if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_commit(p, B, ws.lab, ws.improved, ws.x_bin, s, launches));
+    if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_commit(p, ws.ld, ws.lab, ws.improved, ws.x_bin, s, launches));
     else GDA_TRY(eval_commit(p, ws.ld, xcur, ws.improved, ws.x_bin, s, launches));
     return GDA_OK;
 }
@@ -656,7 +659,7 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
                 "gda_run: x_bin, obj and best_restart are required");
     GDA_REQUIRE(x0 != nullptr || (p->ws.has_state && p->ws.B == B),
                 "gda_run: x0 is NULL but the handle holds no state of a previous run with B = %d to resume", B);
-    GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_run: B must be a positive multiple of 4 (got %d)", B);
+    GDA_REQUIRE(B > 0, "gda_run: B must be positive (got %d)", B);
     GDA_REQUIRE(std::isfinite(prm->alpha) && prm->alpha > 0.0f, "gda_run: alpha must be > 0");
     GDA_REQUIRE(std::isfinite(prm->beta) && prm->beta >= 0.0f, "gda_run: beta must be >= 0");
     GDA_REQUIRE(prm->delta >= 0.0f && prm->delta < 0.5f, "gda_run: delta must be in [0, 1/2)");
@@ -702,7 +705,7 @@ static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const flo
         if (p->kind == GDA_KIND_DENSE)
             GDA_TRY(dense_make_operand(p, ws.ld, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
         if (p->kind == GDA_KIND_KCUT)                       // run_init put the logits in z; x[0] = SoftMax(z)
-            GDA_TRY(kcut_softmax(p, B, ws.z, ws.x[0], s, &p->last_launches));
+            GDA_TRY(kcut_softmax(p, ws.ld, ws.z, ws.x[0], s, &p->last_launches));
     } else {
         parity = ws.parity;      // resume: iterates, duals, best-so-far and the iteration counter stay as they are
     }
@@ -725,7 +728,7 @@ static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const flo
     GDA_CUDA_TRY(cudaMemcpyAsync(best_restart, ws.best_restart, sizeof(int32_t), cudaMemcpyDefault, s));
     if (extra) {
         if (extra->x_final && p->kind == GDA_KIND_KCUT)      // the logits Z^T, [k][n][B]
-            GDA_CUDA_TRY(cudaMemcpyAsync(extra->x_final, ws.z, elems * p->kparts * sizeof(float), cudaMemcpyDeviceToDevice, s));
+            GDA_TRY(copy_out(extra->x_final, (size_t)B, ws.z, ld, n * (size_t)p->kparts, sizeof(float), s));
         else if (extra->x_final) GDA_TRY(copy_out(extra->x_final, (size_t)B, xfin, ld, n, sizeof(float), s));
         if (extra->lambda_final && prm->dual == GDA_DUAL_SCALAR)          // mu^T, [B]
             GDA_CUDA_TRY(cudaMemcpyAsync(extra->lambda_final, ws.mu[parity], (size_t)B * sizeof(float), cudaMemcpyDeviceToDevice, s));
@@ -766,13 +769,22 @@ extern "C" gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, c
 // ---------------------------------------------------------------------------------------------------
 extern "C" gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float* G, void* stream) {
     GDA_REQUIRE(p != nullptr && x != nullptr && G != nullptr, "gda_grad: null argument");
-    GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_grad: B must be a positive multiple of 4 (got %d)", B);
+    GDA_REQUIRE(B > 0, "gda_grad: B must be positive (got %d)", B);
     if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_grad: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
     GDA_ON_DEVICE(p);
     cudaStream_t user, s;
-    if (p->kind == GDA_KIND_DENSE) GDA_TRY(ensure_workspace(p, B));
+    const bool staged = p->kind != GDA_KIND_DENSE && lead_dim(p, B) != B;     // B % 4 != 0: through the padded workspace arrays
+    if (p->kind == GDA_KIND_DENSE || staged) GDA_TRY(ensure_workspace(p, B));
     GDA_TRY(pick_stream(p, stream, &user, &s));
-    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_grad(p, B, x, G, s));
+    if (staged) {
+        Workspace& ws = p->ws;                               // the handle's run state is scratch here (has_state = false)
+        ws.has_state = false;
+        GDA_CUDA_TRY(cudaMemsetAsync(ws.x[0], 0, (size_t)p->n * ws.ld * sizeof(float), s));
+        GDA_TRY(copy_in(ws.x[0], (size_t)ws.ld, x, (size_t)B, (size_t)p->n, sizeof(float), s));
+        if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_grad(p, ws.ld, ws.x[0], ws.x[1], s));
+        else GDA_TRY(maxsat_grad(p, ws.ld, ws.x[0], ws.x[1], s));
+        GDA_TRY(copy_out(G, (size_t)B, ws.x[1], (size_t)ws.ld, (size_t)p->n, sizeof(float), s));
+    } else if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_grad(p, B, x, G, s));
     else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_grad(p, B, x, G, s));
     else {
         Workspace& ws = p->ws;                               // the handle's run state is scratch here (has_state = false)
@@ -790,16 +802,24 @@ extern "C" gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float*
 
 extern "C" gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, void* stream) {
     GDA_REQUIRE(p != nullptr && x != nullptr && obj != nullptr, "gda_score: null argument");
-    GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_score: B must be a positive multiple of 4 (got %d)", B);
+    GDA_REQUIRE(B > 0, "gda_score: B must be positive (got %d)", B);
     GDA_ON_DEVICE(p);
     GDA_TRY(ensure_workspace(p, B));
     cudaStream_t user, s;
     GDA_TRY(pick_stream(p, stream, &user, &s));
     Workspace& ws = p->ws;
     int32_t n_part = 0;
-    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, B, x, ws.partial, &n_part, s, nullptr));
-    else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, B, x, ws.partial, &n_part, s, nullptr));
-    else if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_score_partials(p, B, x, ws.lab, ws.partial, &n_part, s, nullptr));   // x = logits [k][n][B]
+    if (p->kind != GDA_KIND_DENSE && ws.ld != B) {           // B % 4 != 0: a zero-padded copy at the workspace's row stride
+        ws.has_state = false;
+        float* dst = p->kind == GDA_KIND_KCUT ? ws.z : ws.x[0];
+        const size_t rows = (size_t)p->n * (p->kind == GDA_KIND_KCUT ? p->kparts : 1);
+        GDA_CUDA_TRY(cudaMemsetAsync(dst, 0, rows * ws.ld * sizeof(float), s));
+        GDA_TRY(copy_in(dst, (size_t)ws.ld, x, (size_t)B, rows, sizeof(float), s));
+        x = dst;
+    }
+    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_score_partials(p, ws.ld, x, ws.partial, &n_part, s, nullptr));
+    else if (p->kind == GDA_KIND_MAXSAT) GDA_TRY(maxsat_score_partials(p, ws.ld, x, ws.partial, &n_part, s, nullptr));
+    else if (p->kind == GDA_KIND_KCUT) GDA_TRY(kcut_score_partials(p, ws.ld, x, ws.lab, ws.partial, &n_part, s, nullptr));   // x = logits [k][n][B]
     else {
         ws.has_state = false; ws.score_scratch = 1;
         const float* xs = x;
@@ -825,7 +845,7 @@ extern "C" gda_status gda_get_info(const gda_problem* p, gda_info* info) {
 extern "C" gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, const float* lambda, float lambda_scalar,
                                      int32_t gfun, float log_eps, double* out, void* stream) {
     GDA_REQUIRE(p != nullptr && x != nullptr && out != nullptr, "gda_lagrangian: null argument");
-    GDA_REQUIRE(B > 0 && B % 4 == 0, "gda_lagrangian: B must be a positive multiple of 4 (got %d)", B);
+    GDA_REQUIRE(B > 0, "gda_lagrangian: B must be positive (got %d)", B);
     GDA_REQUIRE(gfun == GDA_G_QUADRATIC || gfun == GDA_G_ENTROPY, "gda_lagrangian: unknown gfun %d", gfun);
     if (gfun == GDA_G_ENTROPY) GDA_REQUIRE(log_eps > 0.0f && log_eps < 0.5f, "gda_lagrangian: log_eps must be in (0, 1/2)");
     if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_lagrangian: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
@@ -854,9 +874,21 @@ extern "C" gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, 
         GDA_TRY(eval_sum_partials(B, ws.ld, part, n_f + n_g, out, s));
         return join_stream(p, user, s);
     }
-    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_value_partials(p, B, x, part, &n_f, s));
-    else GDA_TRY(maxsat_value_partials(p, B, x, part, &n_f, s));
-    GDA_TRY(eval_yg_partials(p, p->n, B, x, lambda, lambda_scalar, gfun, log_eps, part + (size_t)n_f * B, &n_g, s));
-    GDA_TRY(eval_sum_partials(B, B, part, n_f + n_g, out, s));
+    const size_t ld = (size_t)ws.ld;
+    if (ld != (size_t)B) {                                   // B % 4 != 0: zero-padded copies at the workspace's row stride
+        ws.has_state = false;
+        GDA_CUDA_TRY(cudaMemsetAsync(ws.x[0], 0, (size_t)p->n * ld * sizeof(float), s));
+        GDA_TRY(copy_in(ws.x[0], ld, x, (size_t)B, (size_t)p->n, sizeof(float), s));
+        x = ws.x[0];
+        if (lambda) {
+            GDA_CUDA_TRY(cudaMemsetAsync(ws.y, 0, (size_t)p->n * ld * sizeof(float), s));
+            GDA_TRY(copy_in(ws.y, ld, lambda, (size_t)B, (size_t)p->n, sizeof(float), s));
+            lambda = ws.y;
+        }
+    }
+    if (p->kind == GDA_KIND_SPARSE) GDA_TRY(sparse_value_partials(p, ws.ld, x, part, &n_f, s));
+    else GDA_TRY(maxsat_value_partials(p, ws.ld, x, part, &n_f, s));
+    GDA_TRY(eval_yg_partials(p, p->n, ws.ld, x, lambda, lambda_scalar, gfun, log_eps, part + (size_t)n_f * ld, &n_g, s));
+    GDA_TRY(eval_sum_partials(B, ws.ld, part, n_f + n_g, out, s));
     return join_stream(p, user, s);
 }

@@ -328,17 +328,18 @@ static gda_status copy_in(void* dst, size_t ld, const void* src, size_t B, size_
 gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0, float l0_scalar,
                     uint32_t t0, cudaStream_t s, int64_t* launches) {
     Workspace& ws = p->ws;
-    const size_t ld = (size_t)ws.ld, elems = (size_t)p->n_pad * ld;          // padded only on the dense path
+    const size_t ld = (size_t)ws.ld, elems = (size_t)p->n_pad * ld;          // padding: restarts up to a multiple of 4 (dense: 128), dense variables up to 256
     const bool padded = ld != (size_t)B || p->n_pad != p->n;
     if (p->kind == GDA_KIND_KCUT) {
-        GDA_CUDA_TRY(cudaMemcpyAsync(ws.z, x0, (size_t)p->n * B * p->kparts * sizeof(float), cudaMemcpyDefault, s));
+        if (padded) GDA_CUDA_TRY(cudaMemsetAsync(ws.z, 0, elems * p->kparts * sizeof(float), s));   // padding restarts: logits 0
+        GDA_TRY(copy_in(ws.z, ld, x0, (size_t)B, (size_t)p->n * p->kparts, sizeof(float), s));
     } else {
         if (padded) GDA_CUDA_TRY(cudaMemsetAsync(ws.x[0], 0, elems * sizeof(float), s));   // padding variables and restarts start at 0
         GDA_TRY(copy_in(ws.x[0], ld, x0, (size_t)B, (size_t)p->n, sizeof(float), s));
     }
     if (ws.dual == GDA_DUAL_SCALAR) {
         if (ws.gacc)                                         // nothing pending from an earlier (possibly failed) run
-            GDA_CUDA_TRY(cudaMemsetAsync(ws.gacc, 0, (size_t)GDA_GACC_WAYS * B * sizeof(unsigned long long), s));
+            GDA_CUDA_TRY(cudaMemsetAsync(ws.gacc, 0, (size_t)GDA_GACC_WAYS * ld * sizeof(unsigned long long), s));
         GDA_TRY(mu_init((int32_t)ld, nullptr, l0 ? 0.0f : l0_scalar, ws.mu[0], s, launches));
         if (l0) GDA_CUDA_TRY(cudaMemcpyAsync(ws.mu[0], l0, (size_t)B * sizeof(float), cudaMemcpyDefault, s));
     } else if (l0) {

@@ -274,7 +274,8 @@ constexpr int SLAB_S = 8, SLAB_ROWS = 16, SLAB_MAX_THREADS = 1024;
 constexpr int SLAB_SMEM_LIMIT = 226 * 1024;                  // dynamic shared memory of a CTA (the kernel also has a few static bytes)
 
 struct SlabArgs {
-    int n, B, len, n_groups, groups_per_warp, n_pass;
+    int n, B, len, n_groups, groups_per_warp, n_pass;   // B: restarts (row stride) including padding restarts
+    int B_eval;                      // restarts that count: the evaluation skips the padding restarts b >= B_eval
     const int2* ent;                 // general: [slot][16 rows] (col * 32 bytes, bits of val2)
     const uint2* ent16;              // compact: [pass][16 rows] four 16-bit entries: bit 15 = sign of val2, bits 0..11 = column
     uint32_t cbits;                  // compact: bits of |val2|, the one magnitude all entries share
@@ -468,7 +469,7 @@ spmm_chunk_slab(const SlabArgs a) {
     if (threadIdx.x < SLAB_S) {
         const int b = b0 + threadIdx.x;
         int imp = 0;
-        if (b < a.B) {
+        if (b < a.B_eval) {
             acc_t t = red[threadIdx.x];
             for (int w = 1; w < warps; ++w) t += red[w * SLAB_S + threadIdx.x];
             const double v = (double)t;
@@ -893,7 +894,7 @@ static bool slab_wanted(const gda_problem* p, int32_t B) {
 }
 
 // One launch = `len` steps + the evaluation, when the slab kernel applies; *done = 0 when it does not.
-gda_status sparse_chunk_slab(gda_problem* p, int32_t B, int32_t len, const float* x_in, float* x_out, float* y,
+gda_status sparse_chunk_slab(gda_problem* p, int32_t B_eval, int32_t B, int32_t len, const float* x_in, float* x_out, float* y,
                              const UpdParams& up, cudaStream_t s, int64_t* launches, int* done) {
     *done = 0;
     if (!slab_wanted(p, B)) return GDA_OK;
@@ -902,7 +903,7 @@ gda_status sparse_chunk_slab(gda_problem* p, int32_t B, int32_t len, const float
     const int warps = std::max(1, (p->slab_groups + per_warp - 1) / per_warp);
     const bool compact = p->d_slab_ent16 != nullptr;
     SlabArgs a{};
-    a.n = p->n; a.B = B; a.len = len; a.n_groups = p->slab_groups; a.groups_per_warp = per_warp; a.n_pass = p->slab_slots / 4;
+    a.n = p->n; a.B = B; a.B_eval = B_eval; a.len = len; a.n_groups = p->slab_groups; a.groups_per_warp = per_warp; a.n_pass = p->slab_slots / 4;
     a.ent = p->d_slab_ent; a.ent16 = reinterpret_cast<const uint2*>(p->d_slab_ent16); a.cbits = p->slab_cbits;
     a.goff = p->d_slab_goff; a.grow = p->d_slab_grow; a.cprime = p->d_cprime;
     a.x_in = x_in; a.x_out = x_out; a.y = y; a.up = up; a.st = ws.state;

@@ -500,8 +500,6 @@ def test_run_arguments_are_validated(api):
         with pytest.raises(api.GdaError) as e:
             P.run(x, 6.0, api.params_from_hyper(w.hyper, **bad))
         assert e.value.status == 1
-    with pytest.raises(api.GdaError):
-        P.run(dev(wl.x0_uniform(w.problem.n, 6, 1)), 6.0, api.params_from_hyper(w.hyper))     # B % 4 != 0
     P.destroy()
 
 
