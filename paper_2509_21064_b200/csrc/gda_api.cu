@@ -555,10 +555,11 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     const UpdParams up = make_upd(prm);
     int cur = parity;
     const bool scalar = prm.dual == GDA_DUAL_SCALAR;
-    if (p->kind == GDA_KIND_SPARSE && !scalar) {              // small n: steps AND evaluation in one launch, state on chip
+    if (p->kind == GDA_KIND_SPARSE) {                         // small n: steps AND evaluation in one launch, state on chip
         int slab = 0;
         const int64_t before = *launches;
-        GDA_TRY(sparse_chunk_slab(p, B, ws.ld, len, ws.x[cur], ws.x[cur ^ (len & 1)], ws.y, up, s, launches, &slab));   // buffer parity as the per-step kernels leave it
+        GDA_TRY(sparse_chunk_slab(p, B, ws.ld, len, ws.x[cur], ws.x[cur ^ (len & 1)], ws.y, scalar ? ws.mu[cur] : nullptr,
+                                  scalar ? ws.mu[cur ^ (len & 1)] : nullptr, up, s, launches, &slab));   // buffer parity as the per-step kernels leave it
         if (slab) { *step_launches += *launches - before; return GDA_OK; }
     }
     for (int k = 0; k < len; ++k) {

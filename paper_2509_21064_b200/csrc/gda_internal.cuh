@@ -166,6 +166,7 @@ gda_status sparse_configure(gda_problem* p);                       // at create
 gda_status sparse_build_slab(gda_problem* p, const std::vector<int32_t>& rowptr, const std::vector<int32_t>& col,
                              const std::vector<float>& val2);
 gda_status sparse_chunk_slab(gda_problem* p, int32_t B_eval, int32_t B, int32_t len, const float* x_in, float* x_out, float* y,
+                             const float* mu_in, float* mu_out,     // PDBO-s: [B] multipliers before / after the chunk; NULL = PDBO
                              const UpdParams& up, cudaStream_t s, int64_t* launches, int* done);
 gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);
 gda_status sparse_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,

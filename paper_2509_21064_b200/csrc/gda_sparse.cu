@@ -284,6 +284,7 @@ struct SlabArgs {
     const float* cprime;
     const float* x_in; float* x_out; // [n][B]: x^t is read from x_in at the start, x^{t+len} written to x_out at the end
     float* y;                        // [n][B], in place (a CTA touches nothing outside its slab, so x_in may equal x_out)
+    const float* mu_in; float* mu_out;   // PDBO-s (DUAL): [B] multipliers at the chunk's start / end; y is not touched
     UpdParams up;
     RunState* st;
     double* best_obj; int32_t* improved; uint8_t* x_bin; double* block_min;
@@ -329,7 +330,10 @@ __device__ __forceinline__ SlabPass slab_fetch(const SlabArgs& a, const uint2* _
 // long and short ones and the per-step barrier does not wait for the warp with the longest rows
 __device__ __forceinline__ int slab_group(int i, int warp, int warps) { return (i & 1) ? i * warps + (warps - 1 - warp) : i * warps + warp; }
 
-template <int GFUN, bool INTEGRAL, bool COMPACT>
+// DUAL (PDBO-s, reading R14): one multiplier per restart instead of y.  The CTA holds ALL rows of its restarts, so the sum of
+// g(x_i^t) over the variables is a reduction inside the CTA -- lanes of a warp by a fixed butterfly, the warps in index order --
+// and the multiplier's update costs one more barrier per step: no atomics, no second kernel, deterministic.
+template <int GFUN, bool INTEGRAL, bool COMPACT, bool DUAL>
 __global__ void __launch_bounds__(SLAB_MAX_THREADS, 1)
 spmm_chunk_slab(const SlabArgs a) {
     using acc_t = typename std::conditional<INTEGRAL, long long, double>::type;
@@ -343,6 +347,8 @@ spmm_chunk_slab(const SlabArgs a) {
     uint2* cst = reinterpret_cast<uint2*>(red + (blockDim.x >> 5) * SLAB_S);   // compact structure [n_pass][16]
     __shared__ int s_imp[SLAB_S];
     __shared__ unsigned s_last;
+    __shared__ __align__(16) float s_mu[SLAB_S];                            // DUAL: this step's multipliers of the slab's restarts
+    float (*s_gred)[SLAB_S] = reinterpret_cast<float (*)[SLAB_S]>(red);   // DUAL: the warps' sums of g(x_i^t) (red is free until the evaluation)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
     const int r = lane >> 1, q = lane & 1;
     const int b0 = blockIdx.x * SLAB_S;                       // first restart of the slab
@@ -354,11 +360,12 @@ spmm_chunk_slab(const SlabArgs a) {
         if (b0 + 4 * qq < a.B) {
             const size_t off = (size_t)row * a.B + b0 + 4 * qq;
             xv = ldg4(a.x_in + off);
-            yv = ldg4(a.y + off);
+            if (!DUAL) yv = ldg4(a.y + off);
         }
         reinterpret_cast<float4*>(xa)[e] = xv;
-        reinterpret_cast<float4*>(ys)[e] = yv;
+        if (!DUAL) reinterpret_cast<float4*>(ys)[e] = yv;
     }
+    if (DUAL && threadIdx.x < SLAB_S) s_mu[threadIdx.x] = b0 + (int)threadIdx.x < a.B ? __ldg(a.mu_in + b0 + threadIdx.x) : 0.0f;
     for (int e = threadIdx.x; e < a.n; e += blockDim.x) cps[e] = __ldg(a.cprime + e);
     if (COMPACT) {
         for (int e = threadIdx.x; e < a.n_pass * SLAB_ROWS; e += blockDim.x) cst[e] = __ldg(a.ent16 + e);
@@ -374,6 +381,8 @@ spmm_chunk_slab(const SlabArgs a) {
 
     // ---- len GDA steps, state on chip ----
     for (int k = 0; k < a.len; ++k) {
+        float4 gs = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float4 mu4 = DUAL ? *reinterpret_cast<const float4*>(s_mu + 4 * q) : gs;
         for (int i = 0; i < a.groups_per_warp; ++i) {
             const int g = slab_group(i, warp, warps);
             if (g >= a.n_groups) break;
@@ -397,11 +406,30 @@ spmm_chunk_slab(const SlabArgs a) {
                 acc.x += cp; acc.y += cp; acc.z += cp; acc.w += cp;
                 const int idx = row * 2 + q;
                 const float4 xv = reinterpret_cast<const float4*>(xa)[idx];
-                const float4 yv = reinterpret_cast<const float4*>(ys)[idx];
+                const float4 yv = DUAL ? mu4 : reinterpret_cast<const float4*>(ys)[idx];
                 float4 xo, yo;
                 gda_update4<GFUN>(xv, yv, acc, a.up, t0 + (uint32_t)k, (uint32_t)row, (uint32_t)(b0 + 4 * q), xo, yo);
                 reinterpret_cast<float4*>(xb)[idx] = xo;
-                reinterpret_cast<float4*>(ys)[idx] = yo;
+                if (DUAL) {
+                    gs.x += gda_g<GFUN>(xv.x, a.up); gs.y += gda_g<GFUN>(xv.y, a.up);
+                    gs.z += gda_g<GFUN>(xv.z, a.up); gs.w += gda_g<GFUN>(xv.w, a.up);
+                } else {
+                    reinterpret_cast<float4*>(ys)[idx] = yo;
+                }
+            }
+        }
+        if (DUAL) {                                          // rows of the warp (lanes with the same quad), then the warps
+#pragma unroll
+            for (int o = 2; o < 32; o <<= 1) {
+                gs.x += __shfl_xor_sync(0xffffffffu, gs.x, o); gs.y += __shfl_xor_sync(0xffffffffu, gs.y, o);
+                gs.z += __shfl_xor_sync(0xffffffffu, gs.z, o); gs.w += __shfl_xor_sync(0xffffffffu, gs.w, o);
+            }
+            if (lane < 2) *reinterpret_cast<float4*>(&s_gred[warp][4 * lane]) = gs;
+            __syncthreads();
+            if (threadIdx.x < SLAB_S) {
+                float t = s_gred[0][threadIdx.x];
+                for (int w = 1; w < warps; ++w) t += s_gred[w][threadIdx.x];
+                s_mu[threadIdx.x] += a.up.beta * t;          // mu^{t+1} = mu^t + beta_s sum_i g(x_i^t)
             }
         }
         __syncthreads();
@@ -415,9 +443,10 @@ spmm_chunk_slab(const SlabArgs a) {
         if (b0 + 4 * qq < a.B) {
             const size_t off = (size_t)row * a.B + b0 + 4 * qq;
             *reinterpret_cast<float4*>(a.x_out + off) = reinterpret_cast<const float4*>(xa)[e];
-            *reinterpret_cast<float4*>(a.y + off) = reinterpret_cast<const float4*>(ys)[e];
+            if (!DUAL) *reinterpret_cast<float4*>(a.y + off) = reinterpret_cast<const float4*>(ys)[e];
         }
     }
+    if (DUAL && threadIdx.x < SLAB_S && b0 + (int)threadIdx.x < a.B) a.mu_out[b0 + threadIdx.x] = s_mu[threadIdx.x];
 
     // ---- S5: exact objective of x_hat = [x > 1/2] for the slab's restarts: sum_i x_hat_i ((Q_off x_hat)_i + c'_i) ----
     acc_t obj4[4] = {0, 0, 0, 0};
@@ -689,7 +718,8 @@ int sparse_heavy_threshold() { return HEAVY_DEG; }
 // shared-memory opt-in of the slab kernels on the handle's device; called at create (never inside a capture)
 template <int GFUN, bool INTEGRAL, bool COMPACT>
 static gda_status slab_opt_in() {
-    GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_chunk_slab<GFUN, INTEGRAL, COMPACT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SLAB_SMEM_LIMIT));
+    GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_chunk_slab<GFUN, INTEGRAL, COMPACT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SLAB_SMEM_LIMIT));
+    GDA_CUDA_TRY(cudaFuncSetAttribute(spmm_chunk_slab<GFUN, INTEGRAL, COMPACT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SLAB_SMEM_LIMIT));
     return GDA_OK;
 }
 gda_status sparse_configure(gda_problem*) {
@@ -895,7 +925,7 @@ static bool slab_wanted(const gda_problem* p, int32_t B) {
 
 // One launch = `len` steps + the evaluation, when the slab kernel applies; *done = 0 when it does not.
 gda_status sparse_chunk_slab(gda_problem* p, int32_t B_eval, int32_t B, int32_t len, const float* x_in, float* x_out, float* y,
-                             const UpdParams& up, cudaStream_t s, int64_t* launches, int* done) {
+                             const float* mu_in, float* mu_out, const UpdParams& up, cudaStream_t s, int64_t* launches, int* done) {
     *done = 0;
     if (!slab_wanted(p, B)) return GDA_OK;
     Workspace& ws = p->ws;
@@ -906,13 +936,14 @@ gda_status sparse_chunk_slab(gda_problem* p, int32_t B_eval, int32_t B, int32_t 
     a.n = p->n; a.B = B; a.B_eval = B_eval; a.len = len; a.n_groups = p->slab_groups; a.groups_per_warp = per_warp; a.n_pass = p->slab_slots / 4;
     a.ent = p->d_slab_ent; a.ent16 = reinterpret_cast<const uint2*>(p->d_slab_ent16); a.cbits = p->slab_cbits;
     a.goff = p->d_slab_goff; a.grow = p->d_slab_grow; a.cprime = p->d_cprime;
-    a.x_in = x_in; a.x_out = x_out; a.y = y; a.up = up; a.st = ws.state;
+    a.x_in = x_in; a.x_out = x_out; a.y = y; a.mu_in = mu_in; a.mu_out = mu_out; a.up = up; a.st = ws.state;
     a.best_obj = ws.best_obj; a.improved = ws.improved; a.x_bin = ws.x_bin; a.block_min = ws.block_min;
     a.trace_best = ws.trace_best; a.trace_ns = ws.trace_ns; a.trace_cap = ws.trace_cap;
     const unsigned grid = (unsigned)((B + SLAB_S - 1) / SLAB_S);
     const size_t smem = slab_smem_bytes(p->n, warps, compact ? a.n_pass : -1);
     const bool quad = up.gfun == GDA_G_QUADRATIC;
-#define GDA_SLAB_LAUNCH(G, I, C) spmm_chunk_slab<G, I, C><<<grid, warps * 32, smem, s>>>(a)
+#define GDA_SLAB_LAUNCH(G, I, C) do { if (mu_in) spmm_chunk_slab<G, I, C, true><<<grid, warps * 32, smem, s>>>(a); \
+                                      else spmm_chunk_slab<G, I, C, false><<<grid, warps * 32, smem, s>>>(a); } while (0)
 #define GDA_SLAB_IC(G) do { if (p->integral) { if (compact) GDA_SLAB_LAUNCH(G, true, true); else GDA_SLAB_LAUNCH(G, true, false); } \
                             else { if (compact) GDA_SLAB_LAUNCH(G, false, true); else GDA_SLAB_LAUNCH(G, false, false); } } while (0)
     if (quad) GDA_SLAB_IC(GDA_G_QUADRATIC); else GDA_SLAB_IC(GDA_G_ENTROPY);

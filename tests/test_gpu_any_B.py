@@ -62,7 +62,9 @@ def workload(kind, B):
         w.hyper.gfun = 0
         return w, None
     if kind == "pdbo_s":
-        return wl.pdbo_s_variant(wl.config(3, B=B, n_scale=0.05)), None
+        return wl.pdbo_s_variant(wl.config(3, B=B, n_scale=0.05)), "stream"
+    if kind == "pdbo_s_slab":
+        return wl.pdbo_s_variant(wl.config(2, B=B, n_scale=0.25)), "slab"
     if kind == "pdbo_s_maxsat":
         return wl.pdbo_s_variant(wl.config(5, B=B, n_scale=0.05)), None
     if kind == "dense":
@@ -71,7 +73,7 @@ def workload(kind, B):
 
 
 CASES = [("slab", 1), ("slab", 10), ("slab", 13), ("stream", 1), ("stream", 10), ("stream", 70), ("stream", 131),
-         ("maxsat", 3), ("maxsat", 10), ("maxsat", 130), ("maxsat_quadratic", 6), ("pdbo_s", 10), ("pdbo_s", 70),
+         ("maxsat", 3), ("maxsat", 10), ("maxsat", 130), ("maxsat_quadratic", 6), ("pdbo_s", 10), ("pdbo_s", 70), ("pdbo_s_slab", 10), ("pdbo_s_slab", 13),
          ("pdbo_s_maxsat", 10), ("dense", 10), ("dense", 1)]
 
 

@@ -597,8 +597,16 @@ def test_dense_full_run(api, oracle, w):
 # PDBO-s (GDA_DUAL_SCALAR, reading R14): one multiplier per restart
 # ------------------------------------------------------------------------------------------------
 def pdbo_s_workloads():
-    return [wl.pdbo_s_variant(wl.config(3, B=260, n_scale=0.05)), wl.pdbo_s_variant(wl.config(2, B=132, n_scale=0.25)),
-            wl.pdbo_s_variant(wl.config(5, B=136, n_scale=0.05))]
+    out = [wl.pdbo_s_variant(wl.config(3, B=260, n_scale=0.05)), wl.pdbo_s_variant(wl.config(2, B=132, n_scale=0.25)),
+           wl.pdbo_s_variant(wl.config(5, B=136, n_scale=0.05))]
+    # the sparse instances are small enough for the slab kernel (multiplier update inside the CTA); the same instances
+    # through the streaming kernels (fixed-point sums + mu_finalize_kernel)
+    for w in out[:2]:
+        v = wl.pdbo_s_variant(wl.config(3, B=260, n_scale=0.05)) if w is out[0] else wl.pdbo_s_variant(wl.config(2, B=132, n_scale=0.25))
+        v.name += "_stream"
+        v.extra["sparse_path"] = "stream"
+        out.append(v)
+    return out
 
 
 PDBO_S = pdbo_s_workloads()
@@ -677,7 +685,7 @@ def test_pdbo_s_row_grouping_is_bit_identical(api):
     for sw in ("1", "0"):
         os.environ["GDA_SPARSE_LOCALITY"] = sw
         try:
-            P = create_problem(api, w)
+            P = create_problem(api, w, sparse_path="stream")
         finally:
             os.environ.pop("GDA_SPARSE_LOCALITY", None)
         r = P.run(x0, h.lambda0, prm, want_final=True)
