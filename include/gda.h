@@ -76,8 +76,12 @@ gda_status gda_create_qubo_dense(int32_t n, const float* Q, const float* c, int3
 /* Weighted MaxSAT: F(x) = sum_j w_j [clause j unsatisfied] = sum_j w_j prod_{l in C_j} p_l(x)
  * (weights: DESIGN.md reading R9).  HOST cptr[m+1], lit[cptr[m]] with
  * lit = +(var+1) for a positive literal (p = 1 - x) and -(var+1) for a negated one (p = x), HOST w[m] or
- * NULL (= all 1).  INVALID_ARG: empty clause, variable out of range, a variable repeated inside one clause
- * (the product would not be the multilinear extension, reading R2), non-finite or negative weight. */
+ * NULL (= all 1).  Weights may have either sign: the same entry point then minimises ANY polynomial given as a sum of
+ * weighted literal products over distinct variables (Prop. 2.4, is stated for polynomials) -- a monomial
+ * a prod_{i in S} x_i is the clause of the negated literals of S with weight a, and the indicator of a joint assignment of
+ * a clique (the terms of MAP inference on a binary MRF) is the clause that assignment falsifies.
+ * INVALID_ARG: empty clause, variable out of range, a variable repeated inside one clause (the product would not be the
+ * multilinear extension, reading R2), non-finite weight.  UNSUPPORTED: a clause of more than 65 literals. */
 gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cptr, const int32_t* lit, const float* w,
                              gda_problem** out);
 

@@ -331,7 +331,7 @@ extern "C" gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cpt
         for (size_t a = 1; a < tmp.size(); ++a)
             GDA_REQUIRE(tmp[a] != tmp[a - 1], "gda_create_maxsat: variable %d repeated in clause %d", tmp[a], j);
         const float wj = w ? w[j] : 1.0f;
-        GDA_REQUIRE(std::isfinite(wj) && wj >= 0.0f, "gda_create_maxsat: weight of clause %d is negative or non-finite", j);
+        GDA_REQUIRE(std::isfinite(wj), "gda_create_maxsat: weight of clause %d is non-finite", j);   // any sign: a polynomial in literal-product form
         integral = integral && is_integer_valued(wj, 1048576.0f);
     }
     if (kmax > 65) { gda_set_error("gda_create_maxsat: clauses longer than 65 literals are not supported (got %d)", kmax); return GDA_ERR_UNSUPPORTED; }

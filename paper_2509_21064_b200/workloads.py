@@ -240,6 +240,59 @@ def random_ksat(n: int, m: int, k: int, seed: int, wmax: int = 10) -> MaxSat:
     return MaxSat(n=n, m=m, cptr=cptr, lit=lit, w=w)
 
 
+def random_pubo(n: int, m: int, kmax: int, seed: int, wmax: int = 6) -> MaxSat:
+    """A polynomial in literal-product form with SIGNED integer weights: m terms of 1..kmax distinct variables, uniform
+    literal signs, weights uniform in {-wmax..wmax} without 0 (Prop. 2.4: the extension of a polynomial)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    lits, cptr = [], [0]
+    for _ in range(m):
+        k = int(rng.integers(1, kmax + 1))
+        v = rng.choice(n, size=k, replace=False)
+        lits += list((2 * rng.integers(0, 2, size=k) - 1) * (v + 1))
+        cptr.append(len(lits))
+    w = rng.integers(1, wmax + 1, size=m) * (2 * rng.integers(0, 2, size=m) - 1)
+    return MaxSat(n=n, m=m, cptr=np.array(cptr, np.int32), lit=np.array(lits, np.int32), w=w.astype(np.float32))
+
+
+def qubo_as_literal_products(n: int, Q: np.ndarray, c: np.ndarray) -> MaxSat:
+    """x^T Q x + c^T x on binary x as weighted literal products: {not i, not j} with weight Q_ij + Q_ji for i < j and
+    {not i} with weight Q_ii + c_i (x_i^2 = x_i); zero terms are dropped."""
+    lits, cptr, w = [], [0], []
+    for i in range(n):
+        d = float(Q[i, i] + c[i])
+        if d != 0.0:
+            lits.append(-(i + 1)); cptr.append(len(lits)); w.append(d)
+        for j in range(i + 1, n):
+            q = float(Q[i, j] + Q[j, i])
+            if q != 0.0:
+                lits += [-(i + 1), -(j + 1)]; cptr.append(len(lits)); w.append(q)
+    return MaxSat(n=n, m=len(w), cptr=np.array(cptr, np.int32), lit=np.array(lits, np.int32), w=np.array(w, np.float32))
+
+
+def binary_mrf_grid(rows: int, cols: int, seed: int, scale: int = 4) -> MaxSat:
+    """MAP inference on a binary pairwise MRF as a polynomial in literal-product form: a rows x cols
+    grid, integer energies theta_i(a) and theta_ij(a, b) uniform in {-scale..scale}; every table entry is the weight of the
+    indicator of its assignment, i.e. of the clause that assignment falsifies (a positive literal is false at 0)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    n = rows * cols
+    lits, cptr, w = [], [0], []
+    lit_false_at = lambda v, a: (v + 1) if a == 0 else -(v + 1)      # the literal of variable v that is false when x_v = a
+    def add(term, weight):
+        if weight != 0:
+            lits.extend(term); cptr.append(len(lits)); w.append(float(weight))
+    for v in range(n):
+        for a in (0, 1):
+            add([lit_false_at(v, a)], int(rng.integers(-scale, scale + 1)))
+    for r in range(rows):
+        for q in range(cols):
+            v = r * cols + q
+            for u in ([v + 1] if q + 1 < cols else []) + ([v + cols] if r + 1 < rows else []):
+                for a in (0, 1):
+                    for b in (0, 1):
+                        add([lit_false_at(v, a), lit_false_at(u, b)], int(rng.integers(-scale, scale + 1)))
+    return MaxSat(n=n, m=len(w), cptr=np.array(cptr, np.int32), lit=np.array(lits, np.int32), w=np.array(w, np.float32))
+
+
 def x0_uniform(n: int, B: int, seed: int) -> np.ndarray:
     """x0 ~ U[0,1)^(n x B), float32, layout [n][B]."""
     rng = np.random.Generator(np.random.PCG64(seed))

@@ -324,11 +324,16 @@ def test_sparse_edge_cases(api, oracle, case, path):
     P.destroy()
 
 
-@pytest.mark.parametrize("case", ["mixed_k", "long_clauses", "unweighted", "float_weights", "unit_only", "unit_and_pairs"])
+@pytest.mark.parametrize("case", ["mixed_k", "long_clauses", "unweighted", "float_weights", "unit_only", "unit_and_pairs",
+                                  "signed_weights", "binary_mrf"])
 def test_maxsat_edge_cases(api, oracle, case):
     rng = np.random.default_rng(21)
     n = 60
-    if case in ("mixed_k", "long_clauses", "unit_only", "unit_and_pairs"):
+    if case == "signed_weights":                               # a general polynomial in literal-product form (Prop. 2.4)
+        S = wl.random_pubo(n, 300, 4, 41)
+    elif case == "binary_mrf":                                 # MAP on a binary pairwise MRF, 6 x 10 grid
+        S = wl.binary_mrf_grid(6, 10, 42)
+    elif case in ("mixed_k", "long_clauses", "unit_only", "unit_and_pairs"):
         ks = {"mixed_k": rng.integers(1, 6, size=150), "long_clauses": rng.integers(5, 9, size=40),
               "unit_only": np.ones(45, dtype=np.int64),         # kmax = 1: every "other literal" slot is padding
               "unit_and_pairs": rng.integers(1, 3, size=120)}[case]

@@ -69,16 +69,52 @@ def test_F_maxsat_matches_truth_table(oracle):
     assert np.array_equal(F1, ref1)
 
 
+def test_signed_literal_products_are_polynomials(oracle):
+    """Weights of either sign turn the clause form into a general polynomial (Prop. 2.4).  Pinned by the
+    literal truth table with signed weights, by a QUBO rewritten as literal products -- F, f and grad f must agree with the
+    QUBO evaluators, which have pins of their own -- and by a binary pairwise MRF against its energy tables."""
+    S = wl.random_pubo(8, 40, 4, 31)
+    assert (S.w < 0).any() and (S.w > 0).any()
+    X = all_bits(8)
+    ref = np.array([oracle.unsat_weight(S.cptr, S.lit, S.w, X[:, k]) for k in range(X.shape[1])])
+    assert np.array_equal(oracle.F_binary(oracle_problem(S), X), ref)
+    n = 7
+    Q, c, rowptr, col, val = random_general_qubo(n, 12)
+    PQ = oracle.Problem.qubo_dense(n, Q, c)
+    PL = oracle_problem(wl.qubo_as_literal_products(n, Q, c))
+    Xb = all_bits(n)
+    assert np.allclose(oracle.F_binary(PL, Xb), oracle.F_binary(PQ, Xb), rtol=0, atol=1e-9)
+    Xc = np.random.default_rng(5).random((n, 6))
+    assert np.allclose(oracle.f_ext(PL, Xc), oracle.f_ext(PQ, Xc), rtol=1e-12, atol=1e-12)
+    assert np.allclose(oracle.grad(PL, Xc), oracle.grad(PQ, Xc), rtol=1e-12, atol=1e-12)
+    # binary MRF on a 3 x 3 grid: energy of an assignment = sum of the table entries it selects; rebuilt here from the
+    # clause list by the rule "an entry counts iff every literal of its clause is false"
+    M = wl.binary_mrf_grid(3, 3, 7)
+    Xm = all_bits(9)
+    E = np.zeros(Xm.shape[1])
+    for j in range(M.m):
+        sel = np.ones(Xm.shape[1], dtype=bool)
+        for l in M.lit[M.cptr[j]:M.cptr[j + 1]]:
+            v = abs(int(l)) - 1
+            sel &= (Xm[v] == 0) if l > 0 else (Xm[v] == 1)
+        E += M.w[j] * sel
+    assert np.array_equal(oracle.F_binary(oracle_problem(M), Xm), E)
+    # every pairwise table contributes exactly one entry per assignment, every unary table one
+    assert M.m <= 2 * 9 + 4 * 12
+
+
 # ---------------------------------------------------------------------------------------------
 # f: closed form (Prop. 2.4) against Def. 2.2 by enumeration; extension property; Lemma 2.3
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("kind", ["qubo_csr", "qubo_dense", "maxsat"])
+@pytest.mark.parametrize("kind", ["qubo_csr", "qubo_dense", "maxsat", "pubo"])
 def test_f_closed_form_equals_definition_2_2(oracle, kind):
     n = 7
     rng = np.random.default_rng(3)
     if kind == "maxsat":
         W = wl.random_ksat(n, 12, 3, 21)
         P = oracle_problem(W)
+    elif kind == "pubo":                                      # signed weights, terms of 1..4 literals
+        P = oracle_problem(wl.random_pubo(n, 20, 4, 23))
     else:
         Q, c, rowptr, col, val = random_general_qubo(n, 2)   # non-zero diagonal: exercises x_i^2 -> x_i (R1)
         P = oracle.Problem.qubo_csr(n, rowptr, col, val, c) if kind == "qubo_csr" \
@@ -99,12 +135,14 @@ def test_f_closed_form_equals_definition_2_2(oracle, kind):
 # ---------------------------------------------------------------------------------------------
 # grad f: multilinearity gives d_i f(x) = f(x | x_i=1) - f(x | x_i=0) EXACTLY
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("kind", ["qubo_csr", "qubo_dense", "maxsat", "maxcut"])
+@pytest.mark.parametrize("kind", ["qubo_csr", "qubo_dense", "maxsat", "maxcut", "pubo"])
 def test_grad_equals_multilinear_difference(oracle, kind):
     n = 9
     rng = np.random.default_rng(4)
     if kind == "maxsat":
         P = oracle_problem(wl.random_ksat(n, 25, 3, 22))
+    elif kind == "pubo":
+        P = oracle_problem(wl.random_pubo(n, 30, 4, 24))
     elif kind == "maxcut":
         e = wl.edges_gnp(n, 0.5, 6)
         P = oracle_problem(wl.maxcut_as_qubo(n, e, wl.edge_weights(e.shape[0], 6, "pm1")))
