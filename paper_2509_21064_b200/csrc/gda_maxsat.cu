@@ -36,10 +36,13 @@ __device__ __forceinline__ float4 lit_term(uint32_t enc, const char* __restrict_
 
 // KW > 0: compile-time number of "other" literals (3-SAT: 2), slot records broadcast by shuffle; PAD says whether
 // records may hold 0-padding (clauses shorter than kmax).  KW == 0: run-time kw, records read with broadcast loads.
+// Few restarts (B <= 64): the warp's lanes form ngrp groups of 32 / ngrp lanes; a group covers all restarts and the groups
+// take DIFFERENT slots of the variable at the same time (group grp: slots grp, grp + ngrp, ...) -- with one group and 3 of
+// 32 lanes active at B = 12 the 13 slots of a variable are 13 dependent round trips.  The caller adds the groups' sums.
 template <int KW, bool PAD>
 __device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, const int32_t* __restrict__ others,
                                              int kw, int start, int end, const float* __restrict__ x, int B,
-                                             int c4, bool active, int lane) {
+                                             int c4, bool active, int lane, int grp = 0, int ngrp = 1) {
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     if (KW > 0) {
         const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
@@ -52,15 +55,16 @@ __device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, con
             for (int q = 0; q < KW; ++q) my_o[q] = (s < end) ? __ldg(others + (size_t)s * KW + q) : (int)ENC_PAD;
             const int cnt = min(32, end - base);
             constexpr int U = 2;                                  // slots per batch: U*KW independent 512 B gathers in flight
-            for (int u0 = 0; u0 < cnt; u0 += U) {
+            for (int u0 = 0; u0 < cnt; u0 += U * ngrp) {
                 float cf[U]; int l[U][KW > 0 ? KW : 1]; float4 t[U][KW > 0 ? KW : 1];
 #pragma unroll
                 for (int a = 0; a < U; ++a) {                     // past the end: re-read the last slot with coefficient 0
-                    const int src = min(u0 + a, cnt - 1);
+                    const int idx = u0 + a * ngrp + grp;
+                    const int src = min(idx, cnt - 1);
                     cf[a] = __shfl_sync(0xffffffffu, my_coef, src);
 #pragma unroll
                     for (int q = 0; q < KW; ++q) l[a][q] = __shfl_sync(0xffffffffu, my_o[q], src);
-                    if (u0 + a >= cnt) cf[a] = 0.0f;
+                    if (idx >= cnt) cf[a] = 0.0f;
                 }
                 if (!active) continue;
 #pragma unroll
@@ -106,24 +110,33 @@ __device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, con
 // warp-per-(variable, 128-restart chunk): blockIdx.y = chunk, the block's 8 warps take 8 consecutive variables.
 // MODE 0: fused step; MODE 1: write G only.  DUAL (PDBO-s, MODE 0): one multiplier per restart (sd.mu),
 // y untouched, the block's sum of g(x_i^t) goes to sd.gpart[blockIdx.x].
-template <int GFUN, int MODE, int KW, bool PAD, bool DUAL>
+// NARROW (B <= 64, step only, KW > 0): lanes_per_group = the power of two >= B / 4 lanes cover the restarts, the warp's
+// 32 / lanes_per_group groups share the slots of the variable (gather_var) and their sums are added by a butterfly.
+template <int GFUN, int MODE, int KW, bool PAD, bool DUAL, bool NARROW = false>
 __global__ void __launch_bounds__(32 * step_warps(DUAL))
 maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* __restrict__ coef,
                    const int32_t* __restrict__ others, int kw, const float* __restrict__ x,
                    float* __restrict__ y, float* __restrict__ xn, UpdParams up, ScalarDual sd,
-                   const RunState* __restrict__ st, uint32_t t_off) {
+                   const RunState* __restrict__ st, uint32_t t_off, int lanes_per_group = 32) {
     constexpr int SW = step_warps(DUAL);
     __shared__ float4 gred[DUAL ? SW : 1][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int c4 = blockIdx.y * 32 + lane;
+    const int grp = NARROW ? lane / lanes_per_group : 0, ngrp = NARROW ? 32 / lanes_per_group : 1;
+    const int c4 = NARROW ? lane % lanes_per_group : blockIdx.y * 32 + lane;
     const bool active = 4 * c4 < B;
     float4 gs = make_float4(0.f, 0.f, 0.f, 0.f), mu = gs;
     if (DUAL) mu = ldg4(sd.mu + 4 * (active ? c4 : B / 4 - 1));
     const int var = blockIdx.x * SW + warp;
     if (var < n) {                                           // warp-uniform
         const int start = __ldg(vptr + var), end = __ldg(vptr + var + 1);
-        const float4 G = gather_var<KW, PAD>(coef, others, kw, start, end, x, B, c4, active, lane);
-        if (active) {
+        float4 G = gather_var<KW, PAD>(coef, others, kw, start, end, x, B, c4, active, lane, grp, ngrp);
+        if (NARROW) {
+            for (int o = lanes_per_group; o < 32; o <<= 1) {  // the groups' sums, in a fixed order
+                G.x += __shfl_xor_sync(0xffffffffu, G.x, o); G.y += __shfl_xor_sync(0xffffffffu, G.y, o);
+                G.z += __shfl_xor_sync(0xffffffffu, G.z, o); G.w += __shfl_xor_sync(0xffffffffu, G.w, o);
+            }
+        }
+        if (active && grp == 0) {
             const size_t off = (size_t)var * B + 4 * c4;
             if (MODE == 1) {
                 *reinterpret_cast<float4*>(xn + off) = G;
@@ -222,15 +235,26 @@ maxsat_value(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __re
         }
 }
 
+static bool maxsat_narrow_disabled() {
+    const char* e = getenv("GDA_MAXSAT_NARROW");
+    return e && e[0] == '0';
+}
+
 template <int GFUN, int MODE, bool DUAL>
 void launch_kw(gda_problem* p, int32_t B, dim3 grid, const float* x, float* y, float* xn,
                const UpdParams& up, const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s) {
 #define GDA_MS_ARGS p->n, B, p->d_vptr, p->d_coef, p->d_others, p->kw, x, y, xn, up, sd, st, t_off
 #define GDA_MS_CASE(K) \
-        case K: if (pad) maxsat_step_kernel<GFUN, MODE, K, true, DUAL><<<grid, 32 * step_warps(DUAL), 0, s>>>(GDA_MS_ARGS); \
+        case K: if (narrow) { if (pad) maxsat_step_kernel<GFUN, 0, K, true, false, true><<<grid, 32 * step_warps(false), 0, s>>>(GDA_MS_ARGS, lanes); \
+                              else maxsat_step_kernel<GFUN, 0, K, false, false, true><<<grid, 32 * step_warps(false), 0, s>>>(GDA_MS_ARGS, lanes); } \
+                else if (pad) maxsat_step_kernel<GFUN, MODE, K, true, DUAL><<<grid, 32 * step_warps(DUAL), 0, s>>>(GDA_MS_ARGS); \
                 else maxsat_step_kernel<GFUN, MODE, K, false, DUAL><<<grid, 32 * step_warps(DUAL), 0, s>>>(GDA_MS_ARGS); break;
     // records hold ENC_PAD when clauses are shorter than kmax -- and ALWAYS when kmax == 1 (kw is then 1 with no other literal)
     const bool pad = p->kmin != p->kmax || p->kmax == 1;
+    // few restarts: slot groups (gather_var); B <= 64 is one 128-restart chunk, so grid.y == 1
+    const bool narrow = MODE == 0 && !DUAL && B <= 64 && p->kw <= 4 && !maxsat_narrow_disabled();
+    int lanes = 1;
+    while (4 * lanes < B) lanes <<= 1;
     switch (p->kw) {
         GDA_MS_CASE(1) GDA_MS_CASE(2) GDA_MS_CASE(3) GDA_MS_CASE(4)
         default: maxsat_step_kernel<GFUN, MODE, 0, true, DUAL><<<grid, 32 * step_warps(DUAL), 0, s>>>(GDA_MS_ARGS); break;
