@@ -277,7 +277,8 @@ def ncu_record(w: wl.Workload) -> dict:
     if not tf.exists():
         return {}
     d = json.loads(tf.read_text())
-    return d.get(f"{w.name}_B{w.B}", d.get(w.name, {}))
+    rec = d.get(f"{w.name}_B{w.B}", d.get(w.name, {}))
+    return rec if rec.get("B", w.B) == w.B else {}          # a capture at another batch size says nothing about this one
 
 
 def roofline_block(w: wl.Workload, peaks, t_step_mean, t_step_median, t_eval):
@@ -473,7 +474,10 @@ def run_ours(args, w: wl.Workload):
     secondary = []
     if world == 1 and not args.no_secondary and args.config == HEADLINE_CONFIG and not (args.mis or args.maxkcut or args.pdbo_s or args.B):
         Ks = max(5, min(K, args.secondary_steps))
-        for sw in (wl.config(3, B=1024), wl.config(4), wl.config(5), wl.config(2), wl.config(1), wl.pdbo_s_variant(wl.config(3))):
+        # the configs of BASELINE.json, config 3's graph at the paper's largest batch (HBM-streaming), PDBO-s, and two of the
+        # paper's own small-batch settings (Max-k-SAT and MIS run B = 10: Table 6, 1040-1048 Table 13)
+        for sw in (wl.config(3, B=1024), wl.config(4), wl.config(5), wl.config(2), wl.config(1), wl.pdbo_s_variant(wl.config(3)),
+                   wl.pdbo_s_variant(wl.config(2)), wl.config(5, B=10), wl.mis(10000, 100, B=10)):
             rs = S.measure(sw, Ks, 3, peaks, full=False)
             rs["P"].destroy()
             secondary.append(secondary_line(sw, rs, Ks))
