@@ -24,6 +24,10 @@ constexpr int THREADS = WARPS * 32;
 // warps per block of spmm_step_warp: 4 (12 blocks per SM) -- a block's slot is free only when its slowest warp is done, and
 // with 4 warps less of the SM waits (config 3: 14.9 -> 14.4 us per step, B = 1024: 66.6 -> 63.9 us); PDBO-s keeps 8: every
 // block ends in a reduction and a set of atomics, and twice the blocks cost more than they gain (19.1 -> 21.7 us)
+static bool narrow_split_disabled() {
+    const char* e = getenv("GDA_NARROW_SPLIT");
+    return e && e[0] == '0';
+}
 __host__ __device__ constexpr int warp_kernel_warps(bool dual) { return dual ? 8 : 4; }
 constexpr int HEAVY_DEG = 256;     // rows above this use the row-split kernel
 constexpr int SCORE_ROWS = 64;     // most rows per block in the scoring kernels (fewer when that leaves SMs idle)
@@ -173,16 +177,20 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
 // the warp, float4 of restarts).  Every lane walks its OWN row's entries (the loads of (col, val) are broadcasts inside
 // its lane group), four gathers in flight, up to the longest row of the warp with the shorter rows predicated off.
 constexpr int NARROW_WARPS = 4;      // per block (MIS n = 5e4, d = 100, B = 12: 46.6 us per step with 8, 42.5 with 4 or 2, 46.1 with 1)
+// Long rows with few restarts (MIS d = 100 at B = 10: 100 entries per row, 1 250 warps in all at n = 10^4) are split further:
+// S = 2^split_log2 lane groups per row take the row's batches of four entries in turn (group s: batches s, s + S, ...) and add
+// their sums by a butterfly; a warp then holds 32 / (G S) rows.
 template <int GFUN, int G>
 __global__ void __launch_bounds__(32 * NARROW_WARPS)
 spmm_step_narrow(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                  const float* __restrict__ val2, const float* __restrict__ cprime, const float* __restrict__ x,
-                 float* __restrict__ y, float* __restrict__ xn, UpdParams up, const RunState* __restrict__ st, uint32_t t_off) {
-    constexpr int R = 32 / G;                                // rows per warp
+                 float* __restrict__ y, float* __restrict__ xn, UpdParams up, const RunState* __restrict__ st, uint32_t t_off,
+                 int split_log2) {
+    const int S = 1 << split_log2, R = 32 / (G * S);         // lane groups per row, rows per warp
     const int lane = threadIdx.x & 31;
-    const int row_raw = (blockIdx.x * NARROW_WARPS + (threadIdx.x >> 5)) * R + lane / G;
-    const int cl = lane % G;
-    const bool active = row_raw < n && 4 * cl < B;
+    const int row_raw = (blockIdx.x * NARROW_WARPS + (threadIdx.x >> 5)) * R + lane / (G * S);
+    const int cl = lane % G, sg = (lane / G) & (S - 1);
+    const bool active = row_raw < n && 4 * cl < B && sg == 0;
     const int row = min(row_raw, n - 1);                     // idle lanes recompute a valid element, only stores are suppressed
     const int c4 = 4 * cl < B ? cl : 0;
     const int start = __ldg(rowptr + row);
@@ -193,7 +201,7 @@ spmm_step_narrow(int n, int B, const int32_t* __restrict__ rowptr, const int32_t
     const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
     const uint32_t stride = 4u * (uint32_t)B;
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int a = 0; a < maxdeg; a += 4) {
+    for (int a = 4 * sg; a < maxdeg; a += 4 * S) {
         int c[4]; float v[4]; float4 g[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {                        // past the row's end: (own row, 0)
@@ -205,6 +213,10 @@ spmm_step_narrow(int n, int B, const int32_t* __restrict__ rowptr, const int32_t
         for (int q = 0; q < 4; ++q) g[q] = gather4(xb, stride, c[q]);
 #pragma unroll
         for (int q = 0; q < 4; ++q) fma4(acc, v[q], g[q]);
+    }
+    for (int o = G; o < G * S; o <<= 1) {                    // the row's lane groups, in a fixed order
+        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o); acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+        acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o); acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
     }
     const float cp = __ldg(cprime + row);
     acc.x += cp; acc.y += cp; acc.z += cp; acc.w += cp;
@@ -669,10 +681,15 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     if (MODE == 0 && !DUAL && B <= 64) {                      // few restarts: several rows per warp
         int G = 1;
         while (4 * G < B) G <<= 1;
-        const unsigned grid = (unsigned)((p->n + NARROW_WARPS * (32 / G) - 1) / (NARROW_WARPS * (32 / G)));
+        // lane groups per row: as many as give every group about two batches of four entries of an average row
+        int split_log2 = 0;
+        if (!narrow_split_disabled())
+            while ((G << (split_log2 + 1)) <= 32 && (8 << (split_log2 + 1)) <= p->nnz / std::max(p->n, 1)) ++split_log2;
+        const int rows_per_block = NARROW_WARPS * (32 / (G << split_log2));
+        const unsigned grid = (unsigned)((p->n + rows_per_block - 1) / rows_per_block);
 #define GDA_NW_CASE(GG) case GG: \
-        if (up.gfun == GDA_G_QUADRATIC) spmm_step_narrow<GDA_G_QUADRATIC, GG><<<grid, 32 * NARROW_WARPS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off); \
-        else spmm_step_narrow<GDA_G_ENTROPY, GG><<<grid, 32 * NARROW_WARPS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off); break;
+        if (up.gfun == GDA_G_QUADRATIC) spmm_step_narrow<GDA_G_QUADRATIC, GG><<<grid, 32 * NARROW_WARPS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off, split_log2); \
+        else spmm_step_narrow<GDA_G_ENTROPY, GG><<<grid, 32 * NARROW_WARPS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off, split_log2); break;
         switch (G) { GDA_NW_CASE(1) GDA_NW_CASE(2) GDA_NW_CASE(4) GDA_NW_CASE(8) GDA_NW_CASE(16) default: break; }
 #undef GDA_NW_CASE
         if (launches) ++*launches;
