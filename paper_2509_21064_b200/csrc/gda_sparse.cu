@@ -24,9 +24,22 @@ constexpr int THREADS = WARPS * 32;
 // warps per block of spmm_step_warp: 4 (12 blocks per SM) -- a block's slot is free only when its slowest warp is done, and
 // with 4 warps less of the SM waits (config 3: 14.9 -> 14.4 us per step, B = 1024: 66.6 -> 63.9 us); PDBO-s keeps 8: every
 // block ends in a reduction and a set of atomics, and twice the blocks cost more than they gain (19.1 -> 21.7 us)
-static bool narrow_split_disabled() {
+// Config 2's graph (n = 800, degree 48) through the streaming kernels, us per step: B = 100 8.66 with a warp per row, 4.38 with
+// the rows split; B = 256 8.72 / 6.58; B = 512 9.10 / 11.21; B = 1024 12.08 / 20.37 (the slab kernel: 8.4 at any B).
+static bool split_all_rows(const gda_problem* p, int32_t B) {
+    const char* e = getenv("GDA_SPARSE_SPLIT_ALL");
+    if (e && e[0]) return e[0] == '1';
+    const int64_t chunks = (B / 4 + 31) / 32;
+    return B > 32 && (int64_t)p->n * chunks < (int64_t)p->num_sms * 12 && p->nnz >= 16 * (int64_t)p->n;   // B <= 32: the narrow kernel splits rows itself
+}
+// narrow kernel (B <= 64): lane groups per row, as many as give every group about two batches of four entries of an average row
+static int narrow_split_log2(const gda_problem* p, int32_t B) {
     const char* e = getenv("GDA_NARROW_SPLIT");
-    return e && e[0] == '0';
+    if (e && e[0] == '0') return 0;
+    int G = 1, split_log2 = 0;
+    while (4 * G < B) G <<= 1;
+    while ((G << (split_log2 + 1)) <= 32 && (8 << (split_log2 + 1)) <= p->nnz / std::max(p->n, 1)) ++split_log2;
+    return split_log2;
 }
 __host__ __device__ constexpr int warp_kernel_warps(bool dual) { return dual ? 8 : 4; }
 constexpr int HEAVY_DEG = 256;     // rows above this use the row-split kernel
@@ -224,26 +237,28 @@ spmm_step_narrow(int n, int B, const int32_t* __restrict__ rowptr, const int32_t
     update_store<GFUN, false>(row, c4, B, active, acc, x, y, xn, up, (st ? st->t : 0u) + t_off, make_float4(0.f, 0.f, 0.f, 0.f), unused);
 }
 
-// row-split: one block per (heavy row, chunk); the 8 warps take interleaved 32-entry slices of the row
-// DUAL: as above.
+// row-split: one block per (row, chunk); the 8 warps take interleaved slices of `slice` entries of the row (32 for the rows
+// above HEAVY_DEG).  row_list == NULL: every row -- used with slices of 8 when the whole launch would otherwise be a few warps
+// per SM that each walk a long row (n = 800, degree 48 at B = 100, the paper's batch size on the 800-node Gset graphs: 800
+// warps in all; 8.7 -> see launch_step).  DUAL: as above.
 template <int GFUN, int MODE, bool DUAL>
 __global__ void __launch_bounds__(THREADS)
 spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chunks,
                 const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                 const float* __restrict__ val2, const float* __restrict__ cprime,
                 const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
-                UpdParams up, ScalarDual sd, const RunState* __restrict__ st, uint32_t t_off) {
+                UpdParams up, ScalarDual sd, const RunState* __restrict__ st, uint32_t t_off, int slice) {
     __shared__ float4 red[WARPS][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ridx = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
-    const int row = __ldg(row_list + ridx);
+    const int row = row_list ? __ldg(row_list + ridx) : ridx;
     const bool active = 4 * (chunk * 32 + lane) < B;
     const int c4 = active ? chunk * 32 + lane : B / 4 - 1;
     const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
     const int start = __ldg(rowptr + row), end = __ldg(rowptr + row + 1);
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int base = start + 32 * warp; base < end; base += 32 * WARPS) {
-        const float4 part = gather_row(col, val2, base, min(base + 32, end), xb, 4u * (uint32_t)B, lane);
+    for (int base = start + slice * warp; base < end; base += slice * WARPS) {
+        const float4 part = gather_row(col, val2, base, min(base + slice, end), xb, 4u * (uint32_t)B, lane);
         acc.x += part.x; acc.y += part.y; acc.z += part.z; acc.w += part.w;
     }
     red[warp][lane] = acc;
@@ -678,13 +693,10 @@ template <int MODE, bool DUAL>
 gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
     const int chunks = (B / 4 + 31) / 32;
-    if (MODE == 0 && !DUAL && B <= 64) {                      // few restarts: several rows per warp
+    if (MODE == 0 && !DUAL && B <= 64 && !split_all_rows(p, B)) {   // few restarts: several rows per warp
         int G = 1;
         while (4 * G < B) G <<= 1;
-        // lane groups per row: as many as give every group about two batches of four entries of an average row
-        int split_log2 = 0;
-        if (!narrow_split_disabled())
-            while ((G << (split_log2 + 1)) <= 32 && (8 << (split_log2 + 1)) <= p->nnz / std::max(p->n, 1)) ++split_log2;
+        const int split_log2 = narrow_split_log2(p, B);
         const int rows_per_block = NARROW_WARPS * (32 / (G << split_log2));
         const unsigned grid = (unsigned)((p->n + rows_per_block - 1) / rows_per_block);
 #define GDA_NW_CASE(GG) case GG: \
@@ -692,6 +704,20 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
         else spmm_step_narrow<GDA_G_ENTROPY, GG><<<grid, 32 * NARROW_WARPS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, st, t_off, split_log2); break;
         switch (G) { GDA_NW_CASE(1) GDA_NW_CASE(2) GDA_NW_CASE(4) GDA_NW_CASE(8) GDA_NW_CASE(16) default: break; }
 #undef GDA_NW_CASE
+        if (launches) ++*launches;
+        GDA_CUDA_TRY(cudaGetLastError());
+        return GDA_OK;
+    }
+    // A launch of few warps that each walk a long row (small n, high degree, one or two chunks of restarts) is bound by the
+    // latency of the serial walk: every row then goes through the row-split kernel with slices of 8 entries instead.
+    if (split_all_rows(p, B)) {
+        const unsigned grid = (unsigned)(p->n * chunks);
+        if (up.gfun == GDA_G_QUADRATIC)
+            spmm_step_split<GDA_G_QUADRATIC, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n, nullptr, B, chunks, p->d_rowptr,
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off, 8);
+        else
+            spmm_step_split<GDA_G_ENTROPY, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n, nullptr, B, chunks, p->d_rowptr,
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off, 8);
         if (launches) ++*launches;
         GDA_CUDA_TRY(cudaGetLastError());
         return GDA_OK;
@@ -718,10 +744,10 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
         const unsigned grid = (unsigned)(p->n_heavy * chunks);
         if (up.gfun == GDA_G_QUADRATIC)
             spmm_step_split<GDA_G_QUADRATIC, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off);
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off, 32);
         else
             spmm_step_split<GDA_G_ENTROPY, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off);
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off, 32);
         if (launches) ++*launches;
     }
     GDA_CUDA_TRY(cudaGetLastError());
@@ -935,8 +961,12 @@ static bool slab_wanted(const gda_problem* p, int32_t B) {
     if (!p->d_slab_ent || p->slab_mode < 0) return false;
     if (p->slab_mode > 0) return true;
     const double ctas = (B + SLAB_S - 1) / SLAB_S, waves = std::ceil(ctas / p->num_sms);
-    const double t_slab = waves * ((double)p->slab_slots * SLAB_ROWS * 32.0 / 128.0 / 1.9e3 + 0.3);   // us
-    const double t_stream = std::max(2.5, (double)p->nnz * B * 4.0 / 13e6);                             // us
+    const double t_slab = waves * (1.3 * (double)p->slab_slots * SLAB_ROWS * 32.0 / 128.0 / 1.9e3 + 0.3);   // us (1.3: structure, own state, barriers; config 2: 8.4)
+    // streaming step, us: the gathers out of the L2 at 13 TB/s, a launch, and -- few warps that each walk a long row -- the
+    // latency of that walk (measured on config 2's graph, see split_all_rows)
+    const double gather_us = (double)p->nnz * B * 4.0 / 13e6;
+    const double deg = (double)p->nnz / std::max(p->n, 1) / (B <= 64 && !split_all_rows(p, B) ? (double)(1 << narrow_split_log2(p, B)) : 1.0);   // entries one lane group walks
+    const double t_stream = split_all_rows(p, B) ? 3.2 + 1.1 * gather_us : std::max(std::max(2.5, gather_us), 1.5 + 0.15 * deg);
     return t_slab < t_stream;
 }
 

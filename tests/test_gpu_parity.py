@@ -324,6 +324,47 @@ def test_sparse_edge_cases(api, oracle, case, path):
     P.destroy()
 
 
+@pytest.mark.parametrize("dual", [0, 1])
+@pytest.mark.parametrize("case,B", [("long_rows", 76), ("long_rows", 40), ("star_isolated", 132), ("general_float", 260), ("cfg2", 100)])
+def test_all_rows_through_the_row_split_kernel(api, oracle, case, B, dual):
+    """Few warps that each walk a long row are bound by the latency of that walk (config 2's graph at the paper's B = 100:
+    800 warps); the launcher then sends EVERY row through the row-split kernel with slices of 8 entries
+    (split_all_rows in gda_sparse.cu; forced here with GDA_SPARSE_SPLIT_ALL=1, which is read at every launch)."""
+    import os
+    if case == "cfg2":
+        w = wl.config(2, B=B, n_scale=0.5)
+        Pw, h = w.problem, w.hyper
+    else:
+        Pw = {"long_rows": lambda: dense_rows_qubo(301, 8), "star_isolated": lambda: star_plus_isolated(700, 5),
+              "general_float": lambda: general_qubo_csr(37, 2, False)}[case]()
+        h = wl.Hyper(3.0, 0.004, 0.01, 1e-4, 0, 1e-6, 300, 50, 7)
+    if dual:
+        h = wl.Hyper(h.lambda0, h.alpha, h.beta / Pw.n, h.delta, h.gfun, h.log_eps, h.iters, h.eval_every, h.seed, 1)
+    OP = oracle_problem(Pw)
+    n = Pw.n
+    X0 = wl.x0_uniform(n, B, 17)
+    os.environ["GDA_SPARSE_SPLIT_ALL"] = "1"
+    try:
+        P = create_problem(api, Pw, sparse_path="stream")
+        r1 = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+        ref = oracle.run(OP, X0, f32(h.lambda0), **okw(h, iters=1, eval_every=1))
+        assert np.abs(r1["x"].cpu().numpy() - ref["x"]).max() <= TOL_STEP
+        tol_y = mu_tolerance(h, n, ref["y"]) if dual else TOL_STEP * np.maximum(1.0, np.abs(ref["y"]))
+        assert (np.abs(r1["lam"].cpu().numpy() - ref["y"]) <= tol_y).all()
+        assert P.info().last_run_step_launches == (2 if dual else 1)            # one step kernel for all rows (+ mu_finalize)
+        r = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=230, eval_every=50), want_final=True)
+        obj, Fref = r["obj"].cpu().numpy(), oracle.F_binary(OP, r["x_bin"].cpu().numpy())
+        assert np.array_equal(obj, Fref) if case != "general_float" else np.allclose(obj, Fref, rtol=1e-6, atol=1e-5)
+        G = P.grad(dev(X0)).cpu().numpy()
+        assert grad_rel_err(G, oracle.grad(OP, X0.astype(np.float64))) <= TOL_STEP
+        os.environ["GDA_SPARSE_SPLIT_ALL"] = "0"                 # the same run with a warp per row: same objective values
+        r0 = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+        assert np.abs(r0["x"].cpu().numpy() - r1["x"].cpu().numpy()).max() <= 2 * TOL_STEP
+    finally:
+        os.environ.pop("GDA_SPARSE_SPLIT_ALL", None)
+    P.destroy()
+
+
 @pytest.mark.parametrize("case", ["mixed_k", "long_clauses", "unweighted", "float_weights", "unit_only", "unit_and_pairs",
                                   "signed_weights", "binary_mrf"])
 def test_maxsat_edge_cases(api, oracle, case):
