@@ -11,6 +11,8 @@
 // update and the new softmax happen in registers.
 #include "gda_internal.cuh"
 
+#include <cstdlib>
+
 namespace {
 
 constexpr int WARPS = 8;
@@ -20,14 +22,19 @@ constexpr int SCORE_ROWS = 64;
 
 __device__ __forceinline__ float4 ld4c(const char* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
-template <int GFUN, int K>
-__global__ void __launch_bounds__(32 * SW)
+// SPLIT: one block of SPLIT_WARPS warps per (node, chunk); the warps take interleaved slices of 8 neighbours and warp 0 adds
+// their sums in warp order and finishes the node.  Used when the launch would otherwise be a few warps per SM that each walk
+// a long row (Max-3-Cut on the 800-node, degree-48 graph at the paper's B = 100: 800 warps, 12.95 -> see kcut_step).
+constexpr int SPLIT_WARPS = 8, SPLIT_SLICE = 8;
+template <int GFUN, int K, bool SPLIT = false>
+__global__ void __launch_bounds__(32 * (SPLIT ? SPLIT_WARPS : SW))
 kcut_step_kernel(int n, int B, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
                  const float* __restrict__ val2, const float* __restrict__ x, float* __restrict__ z,
                  float* __restrict__ y, float* __restrict__ xn, UpdParams up) {
-    const int lane = threadIdx.x & 31;
-    const int row = blockIdx.x * SW + (threadIdx.x >> 5);
-    if (row >= n) return;                                    // warp-uniform
+    __shared__ float4 red[SPLIT ? SPLIT_WARPS : 1][SPLIT ? K : 1][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int row = SPLIT ? blockIdx.x : blockIdx.x * SW + warp;
+    if (row >= n) return;                                    // warp-uniform (SPLIT: block-uniform)
     const bool active = 4 * (blockIdx.y * 32 + lane) < B;
     const int c4 = active ? blockIdx.y * 32 + lane : B / 4 - 1;
     const uint32_t stride = 4u * (uint32_t)B;                // bytes per node row
@@ -38,11 +45,12 @@ kcut_step_kernel(int n, int B, const int32_t* __restrict__ rowptr, const int32_t
     float4 S[K];                                             // S_j = sum_l 2 W_il X_jl = dTr/dX_ji
 #pragma unroll
     for (int j = 0; j < K; ++j) S[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int base = start; base < end; base += 32) {
+    constexpr int SLICE = SPLIT ? SPLIT_SLICE : 32, STEP = SPLIT ? SPLIT_SLICE * SPLIT_WARPS : 32;
+    for (int base = start + (SPLIT ? SLICE * warp : 0); base < end; base += STEP) {
+        const int cnt = min(SLICE, end - base);
         const int e = base + lane;
-        const int my_c = e < end ? __ldg(col + e) : 0;
-        const float my_v = e < end ? __ldg(val2 + e) : 0.0f;
-        const int cnt = min(32, end - base);
+        const int my_c = lane < cnt ? __ldg(col + e) : 0;
+        const float my_v = lane < cnt ? __ldg(val2 + e) : 0.0f;
         for (int u = 0; u < cnt; u += 2) {                   // two neighbours x K planes in flight; past the end: value 0
             const int c0 = __shfl_sync(0xffffffffu, my_c, u), c1 = __shfl_sync(0xffffffffu, my_c, min(u + 1, 31));
             const float v0 = __shfl_sync(0xffffffffu, my_v, u);
@@ -63,12 +71,28 @@ kcut_step_kernel(int n, int B, const int32_t* __restrict__ rowptr, const int32_t
         }
     }
 
+    // the node's own X, Z, y (SPLIT: warp 0 has them in flight while it waits for the other warps' sums)
     const size_t off = (size_t)row * B + 4 * c4;
     const size_t pl = (size_t)n * B;
     float4 X[K], Z[K];
+    float4 yv = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (!SPLIT || warp == 0) {
 #pragma unroll
-    for (int j = 0; j < K; ++j) { X[j] = ldg4(x + j * pl + off); Z[j] = *reinterpret_cast<const float4*>(z + j * pl + off); }
-    const float4 yv = *reinterpret_cast<const float4*>(y + off);
+        for (int j = 0; j < K; ++j) { X[j] = ldg4(x + j * pl + off); Z[j] = *reinterpret_cast<const float4*>(z + j * pl + off); }
+        yv = *reinterpret_cast<const float4*>(y + off);
+    }
+    if (SPLIT) {
+#pragma unroll
+        for (int j = 0; j < K; ++j) red[warp][j][lane] = S[j];
+        __syncthreads();
+        if (warp != 0) return;
+#pragma unroll
+        for (int j = 0; j < K; ++j) {
+            float4 t = red[0][j][lane];
+            for (int w = 1; w < SPLIT_WARPS; ++w) { const float4 r = red[w][j][lane]; t.x += r.x; t.y += r.y; t.z += r.z; t.w += r.w; }
+            S[j] = t;
+        }
+    }
 
     // per component (restart): g, D, the softmax chain rule, the step, the new softmax
     float4 yo;
@@ -225,7 +249,12 @@ kcut_commit_kernel(size_t n_vec, int B4, const uint8_t* __restrict__ lab, const 
 template <int GFUN>
 void launch_k(gda_problem* p, int32_t B, dim3 grid, const float* x, float* z, float* y, float* xn, const UpdParams& up,
               cudaStream_t s) {
-#define KCUT_CASE(K) case K: kcut_step_kernel<GFUN, K><<<grid, 32 * SW, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, x, z, y, xn, up); break;
+    // few warps that each walk a long row: split the rows (the rule of the sparse QUBO path, gda_sparse.cu)
+    const char* e = getenv("GDA_SPARSE_SPLIT_ALL");
+    const bool split = e && e[0] ? e[0] == '1'
+                                 : (int64_t)p->n * grid.y < (int64_t)p->num_sms * 12 && p->nnz >= 16 * (int64_t)p->n;
+#define KCUT_CASE(K) case K: if (split) kcut_step_kernel<GFUN, K, true><<<dim3((unsigned)p->n, grid.y), 32 * SPLIT_WARPS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, x, z, y, xn, up); \
+                             else kcut_step_kernel<GFUN, K><<<grid, 32 * SW, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, x, z, y, xn, up); break;
     switch (p->kparts) { KCUT_CASE(2) KCUT_CASE(3) KCUT_CASE(4) KCUT_CASE(5) KCUT_CASE(6) KCUT_CASE(7) KCUT_CASE(8) default: break; }
 #undef KCUT_CASE
 }
