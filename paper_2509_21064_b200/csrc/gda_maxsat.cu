@@ -158,7 +158,7 @@ maxsat_step_kernel(int n, int B, const int32_t* __restrict__ vptr, const float* 
 // S5: partial[cb][b] = sum over the clauses of block cb of w_j [every literal of C_j false under x_hat]
 template <bool INTEGRAL>
 __global__ void __launch_bounds__(THREADS)
-maxsat_score(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __restrict__ lit,
+maxsat_score(int m, int B, int clauses_per_block, const int32_t* __restrict__ cptr, const int32_t* __restrict__ lit,
              const float* __restrict__ w, const float* __restrict__ x, void* __restrict__ partial) {
     using acc_t = typename std::conditional<INTEGRAL, long long, double>::type;
     __shared__ acc_t red[WARPS][32][4];
@@ -167,8 +167,8 @@ maxsat_score(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __re
     const bool active = 4 * c4 < B;
     acc_t acc[4] = {0, 0, 0, 0};
     if (active) {
-        for (int r = warp; r < SCORE_CLAUSES; r += WARPS) {
-            const int j = blockIdx.x * SCORE_CLAUSES + r;
+        for (int r = warp; r < clauses_per_block; r += WARPS) {
+            const int j = blockIdx.x * clauses_per_block + r;
             if (j >= m) break;
             bool unsat[4] = {true, true, true, true};
             for (int a = __ldg(cptr + j); a < __ldg(cptr + j + 1); ++a) {
@@ -202,7 +202,7 @@ maxsat_score(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __re
 // f(x) at a continuous point: partial[cb][b] = sum over the clauses of block cb of w_j prod_{l in C_j} p_l(x)
 // (PAPER.md:196); products in fp32, sums in fp64
 __global__ void __launch_bounds__(THREADS)
-maxsat_value(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __restrict__ lit,
+maxsat_value(int m, int B, int clauses_per_block, const int32_t* __restrict__ cptr, const int32_t* __restrict__ lit,
              const float* __restrict__ w, const float* __restrict__ x, double* __restrict__ partial) {
     __shared__ double red[WARPS][32][4];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -210,8 +210,8 @@ maxsat_value(int m, int B, const int32_t* __restrict__ cptr, const int32_t* __re
     const bool active = 4 * c4 < B;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
     if (active)
-        for (int r = warp; r < SCORE_CLAUSES; r += WARPS) {
-            const int j = blockIdx.x * SCORE_CLAUSES + r;
+        for (int r = warp; r < clauses_per_block; r += WARPS) {
+            const int j = blockIdx.x * clauses_per_block + r;
             if (j >= m) break;
             const float wj = __ldg(w + j);
             float4 prod = make_float4(wj, wj, wj, wj);
@@ -291,16 +291,23 @@ gda_status maxsat_grad(gda_problem* p, int32_t B, const float* x, float* G, cuda
     return launch_step<1, false>(p, B, x, nullptr, G, up, ScalarDual{}, nullptr, 0, s, nullptr);
 }
 
-int32_t maxsat_num_partials(const gda_problem* p, int32_t) { return (p->m + SCORE_CLAUSES - 1) / SCORE_CLAUSES; }
+// clauses per block of the scoring kernels: at most SCORE_CLAUSES, fewer when that grid would leave the machine idle -- a warp
+// walks its clauses one after the other (config 5 at B = 10: 333 blocks, 16 clauses per warp, 25 us per evaluation)
+static int score_clauses(const gda_problem* p, int32_t B) {
+    const int64_t chunks = (B / 4 + 31) / 32;
+    const int64_t want = ((int64_t)p->m * chunks / ((int64_t)p->num_sms * 8) + 7) / 8 * 8;
+    return (int)std::min<int64_t>(SCORE_CLAUSES, std::max<int64_t>(8, want));
+}
+int32_t maxsat_num_partials(const gda_problem* p, int32_t B) { const int c = score_clauses(p, B); return (p->m + c - 1) / c; }
 
 gda_status maxsat_score_partials(gda_problem* p, int32_t B, const float* x, void* partial, int32_t* n_part,
                                  cudaStream_t s, int64_t* launches) {
     const int chunks = (B / 4 + 31) / 32;
     dim3 grid((unsigned)maxsat_num_partials(p, B), (unsigned)chunks);
     if (p->integral)
-        maxsat_score<true><<<grid, THREADS, 0, s>>>(p->m, B, p->d_cptr, p->d_lit, p->d_w, x, partial);
+        maxsat_score<true><<<grid, THREADS, 0, s>>>(p->m, B, score_clauses(p, B), p->d_cptr, p->d_lit, p->d_w, x, partial);
     else
-        maxsat_score<false><<<grid, THREADS, 0, s>>>(p->m, B, p->d_cptr, p->d_lit, p->d_w, x, partial);
+        maxsat_score<false><<<grid, THREADS, 0, s>>>(p->m, B, score_clauses(p, B), p->d_cptr, p->d_lit, p->d_w, x, partial);
     if (launches) ++*launches;
     *n_part = (int32_t)grid.x;
     GDA_CUDA_TRY(cudaGetLastError());
@@ -309,7 +316,7 @@ gda_status maxsat_score_partials(gda_problem* p, int32_t B, const float* x, void
 
 gda_status maxsat_value_partials(gda_problem* p, int32_t B, const float* x, double* partial, int32_t* n_part, cudaStream_t s) {
     const dim3 grid((unsigned)maxsat_num_partials(p, B), (unsigned)((B / 4 + 31) / 32));
-    maxsat_value<<<grid, THREADS, 0, s>>>(p->m, B, p->d_cptr, p->d_lit, p->d_w, x, partial);
+    maxsat_value<<<grid, THREADS, 0, s>>>(p->m, B, score_clauses(p, B), p->d_cptr, p->d_lit, p->d_w, x, partial);
     *n_part = (int32_t)grid.x;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
