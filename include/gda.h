@@ -15,8 +15,9 @@
  *   - Iterates are fp32, layout [n][B] row-major: element (variable i, restart b) at i*B + b, so the
  *     restart index is contiguous.  Any B >= 1 is served (the paper runs B = 1, 10, 100, 1000: PAPER.md:836-843, 873-878):
  *     the kernels work on 128-bit vectors of 4 restarts, so inside its workspace the library pads the restart axis with
- *     zero-initialised restarts up to a multiple of 4 (dense problems: 128) that run along and are never read -- not by
- *     the evaluation, the trace, the arg-best or the copies out.  With B % 4 != 0 gda_grad / gda_score / gda_lagrangian go
+ *     zero-initialised restarts up to a multiple of 4 (dense problems: 128; sometimes 8 for B <= 64, so that a row is whole
+ *     32-byte sectors) that run along and are never read -- not by
+ *     the evaluation, the trace, the arg-best or the copies out.  When the row stride differs from B, gda_grad / gda_score / gda_lagrangian go
  *     through zero-padded copies in the workspace (and, like dense problems always, invalidate a state to resume from).
  *   - gda_run / gda_grad / gda_score enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream) and return without synchronising; outputs are valid once the stream has
