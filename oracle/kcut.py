@@ -42,6 +42,32 @@ def objective(P: Problem, labels: np.ndarray) -> np.ndarray:
     return out
 
 
+def lagrangian(P: Problem, Z: np.ndarray, Y, gfun: int = G_QUADRATIC, precision: str = "f64") -> np.ndarray:
+    """out[b] = L(SoftMax(Z[:,:,b]), Y[:,b]) = Tr(X W X^T) + sum_i y_i g(X_:,i).  Y [n][B] or a scalar."""
+    rt = pdbo._real(precision)
+    Z = np.ascontiguousarray(Z, dtype=rt)
+    k, n, B = Z.shape
+    assert k == P.k and n == P.n
+    Ya = np.full((n, B), Y, dtype=rt) if np.isscalar(Y) else np.ascontiguousarray(Y, dtype=rt)
+    out = np.empty(B, dtype=np.float64)
+    rc = pdbo._lib(precision).kcut_lagrangian_batch(C.byref(P.struct), C.c_int32(B), C.c_void_p(Z.ctypes.data),
+                                                    C.c_void_p(Ya.ctypes.data), C.c_int32(gfun), C.c_void_p(out.ctypes.data))
+    assert rc == 0
+    return out
+
+
+def grad(P: Problem, Z: np.ndarray, precision: str = "f64") -> np.ndarray:
+    """grad_Z of Tr(X W X^T) at X = SoftMax(Z), [k][n][B] (the softmax chain rule of PAPER.md:816-824)."""
+    rt = pdbo._real(precision)
+    Z = np.ascontiguousarray(Z, dtype=rt)
+    k, n, B = Z.shape
+    assert k == P.k and n == P.n
+    out = np.empty_like(Z)
+    rc = pdbo._lib(precision).kcut_grad_batch(C.byref(P.struct), C.c_int32(B), C.c_void_p(Z.ctypes.data), C.c_void_p(out.ctypes.data))
+    assert rc == 0
+    return out
+
+
 def run(P: Problem, Z0: np.ndarray, Y0, *, alpha: float, beta: float, gfun: int = G_QUADRATIC, log_eps: float = 1e-6,
         iters: int, eval_every: int, precision: str = "f64", nthreads: int = 1):
     """GDA on L(SoftMax(Z), y) for every restart.  Z0 [k][n][B] logits, Y0 an [n][B] array or a scalar.

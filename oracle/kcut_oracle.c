@@ -8,9 +8,11 @@
  *   g(v) = sum_j v_j^2 - 1 (quadratic)  |  sum_j v_j log v_j (entropy)
  *   GDA "as in Section 3.2":  Z+ = Z - alpha grad_Z L,  y+ = y + beta g(X_{:,i})   (K1)
  *
- * Parity pins (tests/test_oracle_pins.py): the objective against the edge list over all k^n labelings; k = 2 against
+ * Parity pins (tests/test_kcut_oracle_pins.py): the objective against the edge list over all k^n labelings; k = 2 against
  * the Max-Cut QUBO evaluator; grad_Z L against finite differences of L typed out in the test; conservation of
- * sum_j Z_ji (the softmax Jacobian annihilates constants); y non-increasing; a whole run against brute force.
+ * sum_j Z_ji (the softmax Jacobian annihilates constants); y non-increasing; a whole run against brute force;
+ * kcut_lagrangian_batch against the same typed-out L and against the objective at one-hot points; kcut_grad_batch
+ * against finite differences of that L with y = 0.
  *
  * Layout: Z, X are [k][n][B] row-major (restart index contiguous), y and the labels [n][B].
  */
@@ -96,6 +98,58 @@ static void kcut_step(const kcut_problem* P, const kcut_params* hp, const real* 
             zn[(size_t)j * n + i] = z[(size_t)j * n + i] - alpha * x[(size_t)j * n + i] * (D[j] - mean);
         yn[i] = y[i] + beta * g_col(hp->gfun, n, k, x, i);       /* uses X^t */
     }
+}
+
+/* L(SoftMax(Z), y) = Tr(X W X^T) + sum_i y_i g(X_{:,i}) per restart; Z [k][n][B], Y [n][B] */
+int kcut_lagrangian_batch(const kcut_problem* P, int32_t B, const real* Z, const real* Y, int32_t gfun, double* out) {
+    const int n = P->n, k = P->k;
+    const size_t kn = (size_t)k * n;
+    real* z = (real*)malloc(sizeof(real) * kn);
+    real* x = (real*)malloc(sizeof(real) * kn);
+    if (!z || !x) { free(z); free(x); return 1; }
+    for (int b = 0; b < B; ++b) {
+        for (size_t e = 0; e < kn; ++e) z[e] = Z[e * B + b];
+        softmax_cols(n, k, z, x);
+        double L = 0.0;
+        for (int i = 0; i < n; ++i) {
+            for (int j = 0; j < k; ++j) {                        /* Tr(X W X^T) = sum_j sum_{i,l} X_ji W_il X_jl */
+                double s = 0.0;
+                for (int a = P->rowptr[i]; a < P->rowptr[i + 1]; ++a) s += P->val[a] * (double)x[(size_t)j * n + P->col[a]];
+                L += (double)x[(size_t)j * n + i] * s;
+            }
+            L += (double)Y[(size_t)i * B + b] * (double)g_col(gfun, n, k, x, i);
+        }
+        out[b] = L;
+    }
+    free(z); free(x);
+    return 0;
+}
+
+/* grad_Z of f(SoftMax(Z)) = Tr(X W X^T): dTr/dX_ji = 2 (X W)_ji (W symmetric), then the softmax chain rule
+ * d/dZ_ji = X_ji (D_ji - sum_l X_li D_li)  (the y = 0 part of kcut_step).  Z, out [k][n][B] */
+int kcut_grad_batch(const kcut_problem* P, int32_t B, const real* Z, real* out) {
+    const int n = P->n, k = P->k;
+    const size_t kn = (size_t)k * n;
+    real* z = (real*)malloc(sizeof(real) * kn);
+    real* x = (real*)malloc(sizeof(real) * kn);
+    real* D = (real*)malloc(sizeof(real) * k);
+    if (!z || !x || !D) { free(z); free(x); free(D); return 1; }
+    for (int b = 0; b < B; ++b) {
+        for (size_t e = 0; e < kn; ++e) z[e] = Z[e * B + b];
+        softmax_cols(n, k, z, x);
+        for (int i = 0; i < n; ++i) {
+            real mean = (real)0;
+            for (int j = 0; j < k; ++j) {
+                real s = (real)0;
+                for (int a = P->rowptr[i]; a < P->rowptr[i + 1]; ++a) s += (real)2 * (real)P->val[a] * x[(size_t)j * n + P->col[a]];
+                D[j] = s;
+                mean += x[(size_t)j * n + i] * s;
+            }
+            for (int j = 0; j < k; ++j) out[((size_t)j * n + i) * B + b] = x[(size_t)j * n + i] * (D[j] - mean);
+        }
+    }
+    free(z); free(x); free(D);
+    return 0;
 }
 
 int kcut_objective_batch(const kcut_problem* P, int32_t B, const uint8_t* labels, double* out) {

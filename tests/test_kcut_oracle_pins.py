@@ -80,6 +80,33 @@ def test_one_step_is_gda_on_the_lagrangian(gfun):
     assert np.array_equal(lab, np.argmax(r["z"][:, :, 0], axis=0))                   # rounding = argmax (K4)
 
 
+@pytest.mark.parametrize("gfun", [0, 1])
+def test_lagrangian_and_gradient_functions(gfun):
+    """kcut.lagrangian against L(SoftMax(Z), y) typed out above and, at one-hot points, against the
+    objective; kcut.grad against central differences of that L with y = 0, and against the softmax Jacobian's null space."""
+    n, k, B = 7, 3, 5
+    e, w, W, csr = small_graph(n, 11, 8)
+    P = kcut.Problem(n, k, *csr)
+    rng = np.random.default_rng(6)
+    Z, Y = rng.normal(size=(k, n, B)), rng.uniform(0.0, 3.0, size=(n, B))
+    got = kcut.lagrangian(P, Z, Y, gfun)
+    for b in range(B):
+        assert got[b] == pytest.approx(lagrangian(W, Z[:, :, b], Y[:, b], gfun)[0], rel=1e-12, abs=1e-12)
+    assert np.allclose(kcut.lagrangian(P, Z, 2.0, gfun), kcut.lagrangian(P, Z, np.full((n, B), 2.0), gfun), rtol=0, atol=1e-12)
+    labs = rng.integers(0, k, size=(n, B)).astype(np.uint8)                          # one-hot columns: g = 0, L = the objective
+    Zh = 60.0 * np.eye(k)[labs.T].transpose(2, 1, 0)                                 # [k][n][B], margin 60 between logits
+    assert np.allclose(kcut.lagrangian(P, Zh, Y, gfun), kcut.objective(P, labs), rtol=0, atol=1e-9)
+    G = kcut.grad(P, Z)
+    h = 1e-6
+    for b in range(2):
+        for j in range(k):
+            for i in range(n):
+                E = np.zeros((k, n)); E[j, i] = h
+                fd = (lagrangian(W, Z[:, :, b] + E, np.zeros(n), 0)[0] - lagrangian(W, Z[:, :, b] - E, np.zeros(n), 0)[0]) / (2 * h)
+                assert G[j, i, b] == pytest.approx(fd, rel=2e-6, abs=2e-7)
+    assert np.abs(G.sum(axis=0)).max() <= 1e-12                                      # shifts of a column's logits change nothing
+
+
 def test_softmax_invariants_along_a_run():
     n, k = 30, 3
     e, w, W, csr = small_graph(n, 70, 7, weights="unit")
