@@ -95,7 +95,7 @@ gda_status gda_create_maxsat(int32_t n, int32_t m, const int32_t* cptr, const in
  *   x_bin        DEVICE uint8 [n][B]: per restart the LABELS (argmax_j Z_ji, lowest j on ties) of the best evaluation
  *   obj          DEVICE double [B]: Tr(Xh W Xh^T) of those labels (exact integers for integer weights)
  *   extra->x_final [k][n][B] logits Z^T; params->delta is ignored (no perturbation is described for this variant);
- *   params->dual must be GDA_DUAL_PER_VARIABLE.  gda_grad / gda_lagrangian: UNSUPPORTED.
+ *   params->dual must be GDA_DUAL_PER_VARIABLE.  gda_grad / gda_score / gda_lagrangian take the logits (see there).
  * INVALID_ARG: as gda_create_qubo_csr, plus a non-zero diagonal entry and k outside [2, 8]. */
 gda_status gda_create_maxkcut(int32_t n, int32_t k, const int32_t* rowptr, const int32_t* col, const float* val,
                               gda_problem** out);
@@ -164,10 +164,12 @@ gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, const float*
 
 /* ---- single steps of the path, exposed for parity tests and profiling ---------------------------------
  * gda_grad:  G = grad f(X), DEVICE fp32 [n][B] in and out (S1 sparse / S2 dense / S3 MaxSAT of DESIGN.md).
- *            Max-k-Cut: UNSUPPORTED.
+ *            Max-k-Cut: X is the logits Z [k][n][B] and G [k][n][B] = grad_Z Tr(X W X^T) at X = SoftMax(Z), i.e.
+ *            X_ji (D_ji - sum_l X_li D_li) with D = 2 X W (the y = 0 part of the step, reading K1).
  * gda_score: obj[b] = F(x_hat), x_hat = [X[:,b] > 1/2]; DEVICE fp32 X [n][B], DEVICE double obj[B] (S5).
  *            Max-k-Cut: X is the logits [k][n][B], scored by their labels argmax_j Z_ji (lowest j on ties).
- * On a DENSE problem both (and gda_lagrangian) use the handle's run state as scratch: a later gda_run must pass x0. */
+ * On a DENSE or Max-k-Cut problem (and whenever the row stride differs from B) they and gda_lagrangian use the handle's run
+ * state as scratch: a later gda_run must pass x0. */
 gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float* G, void* stream);
 gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, void* stream);
 
@@ -177,7 +179,8 @@ gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, voi
  * This is the value behind the dual certificate of PAPER.md:1105-1114: for y with f_y = L(., y) convex (Max-Cut:
  * y_i >= -lambda_min(W)), run gda_run with beta = 0 (the multipliers stay at lambda0) until x has converged; then
  * out[b] <= min F, i.e. -out[b] is an upper bound on the maximum cut.  Dense problems: f comes from the tcgen05
- * gradient, f = sum_i x_i (G_i + c'_i) / 2, i.e. with the bf16 operand's error (reading R13).  Max-k-Cut: UNSUPPORTED. */
+ * gradient, f = sum_i x_i (G_i + c'_i) / 2, i.e. with the bf16 operand's error (reading R13).  Max-k-Cut: X is the logits Z [k][n][B] and
+ * out[b] = L(SoftMax(Z), y) = Tr(X W X^T) + sum_i y_i g(X_:,i) with g of a column as in PAPER.md:802-806 (log_eps unused). */
 gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, const float* lambda, float lambda_scalar,
                           int32_t gfun, float log_eps, double* out, void* stream);
 

@@ -220,11 +220,13 @@ class Problem:
 
     # ---- gda_grad / gda_score ---------------------------------------------------------------------
     def grad(self, x, stream=None):
+        """gda_grad: grad f(x) for x [n][B] (Max-k-Cut: x = the logits [k][n][B], the gradient of Tr(X W X^T) w.r.t. them)."""
         import torch
-        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.shape[0] == self.n
+        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()
+        assert tuple(x.shape[:-1]) == ((self.k, self.n) if self.k else (self.n,))
         G = torch.empty_like(x)
         s = torch.cuda.current_stream(x.device).cuda_stream if stream is None else stream
-        _check(lib().gda_grad(self._h, x.shape[1], x.data_ptr(), G.data_ptr(), s))
+        _check(lib().gda_grad(self._h, x.shape[-1], x.data_ptr(), G.data_ptr(), s))
         return G
 
     def score(self, x, stream=None):
@@ -240,16 +242,18 @@ class Problem:
     def lagrangian(self, x, lam, gfun=G_QUADRATIC, log_eps=1e-6, stream=None):
         """gda_lagrangian: L(x, y) = f(x) + sum_i y_i g(x_i) per restart; lam a CUDA tensor [n][B] or a float."""
         import torch
-        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.shape[0] == self.n
-        out = torch.empty(x.shape[1], dtype=torch.float64, device=x.device)
+        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()
+        assert tuple(x.shape[:-1]) == ((self.k, self.n) if self.k else (self.n,))      # Max-k-Cut: the logits [k][n][B]
+        B = x.shape[-1]
+        out = torch.empty(B, dtype=torch.float64, device=x.device)
         l_ptr, l_scalar = None, 0.0
         if isinstance(lam, torch.Tensor):
-            assert lam.is_cuda and lam.dtype == torch.float32 and lam.is_contiguous() and lam.shape == x.shape
+            assert lam.is_cuda and lam.dtype == torch.float32 and lam.is_contiguous() and tuple(lam.shape) == (self.n, B)
             l_ptr = lam.data_ptr()
         else:
             l_scalar = float(lam)
         s = torch.cuda.current_stream(x.device).cuda_stream if stream is None else stream
-        _check(lib().gda_lagrangian(self._h, x.shape[1], x.data_ptr(), l_ptr, l_scalar, gfun, log_eps, out.data_ptr(), s))
+        _check(lib().gda_lagrangian(self._h, B, x.data_ptr(), l_ptr, l_scalar, gfun, log_eps, out.data_ptr(), s))
         return out
 
     def info(self) -> Info:

@@ -782,9 +782,23 @@ extern "C" gda_status gda_run_host(gda_problem* p, int32_t B, const float* x0, c
 extern "C" gda_status gda_grad(gda_problem* p, int32_t B, const float* x, float* G, void* stream) {
     GDA_REQUIRE(p != nullptr && x != nullptr && G != nullptr, "gda_grad: null argument");
     GDA_REQUIRE(B > 0, "gda_grad: B must be positive (got %d)", B);
-    if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_grad: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
     GDA_ON_DEVICE(p);
     cudaStream_t user, s;
+    if (p->kind == GDA_KIND_KCUT) {
+        // x = the logits Z [k][n][B]; G = grad_Z Tr(X W X^T) at X = SoftMax(Z).  Through the workspace
+        // (z, x[0] = SoftMax, x[1] = G): the handle's run state is scratch here
+        GDA_TRY(ensure_workspace(p, B));
+        GDA_TRY(pick_stream(p, stream, &user, &s));
+        Workspace& ws = p->ws;
+        ws.has_state = false;
+        const size_t rows = (size_t)p->n * p->kparts, ld = (size_t)ws.ld;
+        if (ld != (size_t)B) GDA_CUDA_TRY(cudaMemsetAsync(ws.z, 0, rows * ld * sizeof(float), s));
+        GDA_TRY(copy_in(ws.z, ld, x, (size_t)B, rows, sizeof(float), s));
+        GDA_TRY(kcut_softmax(p, ws.ld, ws.z, ws.x[0], s, nullptr));
+        GDA_TRY(kcut_grad(p, ws.ld, ws.x[0], ws.x[1], s));
+        GDA_TRY(copy_out(G, (size_t)B, ws.x[1], ld, rows, sizeof(float), s));
+        return join_stream(p, user, s);
+    }
     const bool staged = p->kind != GDA_KIND_DENSE && lead_dim(p, B) != B;     // B % 4 != 0: through the padded workspace arrays
     if (p->kind == GDA_KIND_DENSE || staged) GDA_TRY(ensure_workspace(p, B));
     GDA_TRY(pick_stream(p, stream, &user, &s));
@@ -860,7 +874,6 @@ extern "C" gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, 
     GDA_REQUIRE(B > 0, "gda_lagrangian: B must be positive (got %d)", B);
     GDA_REQUIRE(gfun == GDA_G_QUADRATIC || gfun == GDA_G_ENTROPY, "gda_lagrangian: unknown gfun %d", gfun);
     if (gfun == GDA_G_ENTROPY) GDA_REQUIRE(log_eps > 0.0f && log_eps < 0.5f, "gda_lagrangian: log_eps must be in (0, 1/2)");
-    if (p->kind == GDA_KIND_KCUT) { gda_set_error("gda_lagrangian: not available for Max-k-Cut problems"); return GDA_ERR_UNSUPPORTED; }
     GDA_ON_DEVICE(p);
     GDA_TRY(ensure_workspace(p, B));
     cudaStream_t user, s;
@@ -868,6 +881,23 @@ extern "C" gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, 
     Workspace& ws = p->ws;
     double* part = static_cast<double*>(ws.partial);
     int32_t n_f = 0, n_g = 0;
+    if (p->kind == GDA_KIND_KCUT) {
+        // x = the logits Z [k][n][B], lambda [n][B]: L(SoftMax(Z), y) = Tr(X W X^T) + sum_i y_i g(X_:,i)
+        ws.has_state = false;
+        const size_t rows = (size_t)p->n * p->kparts, ld = (size_t)ws.ld;
+        if (ld != (size_t)B) GDA_CUDA_TRY(cudaMemsetAsync(ws.z, 0, rows * ld * sizeof(float), s));
+        GDA_TRY(copy_in(ws.z, ld, x, (size_t)B, rows, sizeof(float), s));
+        GDA_TRY(kcut_softmax(p, ws.ld, ws.z, ws.x[0], s, nullptr));
+        const float* lam = lambda;
+        if (lambda && ld != (size_t)B) {
+            GDA_CUDA_TRY(cudaMemsetAsync(ws.y, 0, (size_t)p->n * ld * sizeof(float), s));
+            GDA_TRY(copy_in(ws.y, ld, lambda, (size_t)B, (size_t)p->n, sizeof(float), s));
+            lam = ws.y;
+        }
+        GDA_TRY(kcut_value_partials(p, ws.ld, ws.x[0], lam, lambda_scalar, gfun, part, &n_f, s));
+        GDA_TRY(eval_sum_partials(B, ws.ld, part, n_f, out, s));
+        return join_stream(p, user, s);
+    }
     if (p->kind == GDA_KIND_DENSE) {
         // f(x) = sum_i x_i (G_i + c'_i) / 2 with G = grad f(x) from the tcgen05 GEMM (bf16 operand: reading R13); the
         // run state of the handle is scratch here, as for gda_grad

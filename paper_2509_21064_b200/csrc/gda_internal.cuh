@@ -191,6 +191,9 @@ gda_status kcut_step(gda_problem* p, int32_t B, const float* x, float* z, float*
 gda_status kcut_softmax(gda_problem* p, int32_t B, const float* z, float* x, cudaStream_t s, int64_t* launches);
 gda_status kcut_score_partials(gda_problem* p, int32_t B, const float* z, uint8_t* lab, void* partial, int32_t* n_part,
                                cudaStream_t s, int64_t* launches);
+gda_status kcut_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s);                 // x = SoftMax(z), [k][n][B]
+gda_status kcut_value_partials(gda_problem* p, int32_t B, const float* x, const float* y, float y_scalar, int32_t gfun,
+                               double* partial, int32_t* n_part, cudaStream_t s);
 gda_status kcut_commit(gda_problem* p, int32_t B, const uint8_t* lab, const int32_t* improved, uint8_t* x_bin,
                        cudaStream_t s, int64_t* launches);
 int32_t kcut_num_partials(const gda_problem* p, int32_t B);

@@ -294,6 +294,89 @@ gda_status kcut_score_partials(gda_problem* p, int32_t B, const float* z, uint8_
     return GDA_OK;
 }
 
+// gda_grad / gda_lagrangian for Max-k-Cut (not on the hot path: plain warp-per-node loops, k at run time).
+//   MODE 0: G[j][i][b] = X_ji (D_ji - sum_l X_li D_li), D = 2 X W: grad_Z of Tr(X W X^T) at X = SoftMax(Z)
+//   MODE 1: partial[rb][b] = sum over the nodes i of block rb of  sum_j X_ji (X W)_ji + y_i g(X_:,i)
+static __device__ __forceinline__ void fma4(float4& a, float v, const float4& g) {
+    a.x = fmaf(v, g.x, a.x); a.y = fmaf(v, g.y, a.y); a.z = fmaf(v, g.z, a.z); a.w = fmaf(v, g.w, a.w);
+}
+template <int MODE>
+__global__ void __launch_bounds__(THREADS)
+kcut_aux_kernel(int n, int B, int k, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ col,
+                const float* __restrict__ val2, const float* __restrict__ x, const float* __restrict__ y, float y_scalar,
+                int gfun, float* __restrict__ G, double* __restrict__ partial) {
+    __shared__ double red[MODE == 1 ? WARPS : 1][32][4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c4 = blockIdx.y * 32 + lane;
+    const bool active = 4 * c4 < B;
+    const size_t pl = (size_t)n * B;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int r = warp; r < SCORE_ROWS && active; r += WARPS) {
+        const int row = blockIdx.x * SCORE_ROWS + r;
+        if (row >= n) break;
+        const size_t off = (size_t)row * B + 4 * c4;
+        float4 S[8], X[8];
+        for (int j = 0; j < k; ++j) { S[j] = make_float4(0.f, 0.f, 0.f, 0.f); X[j] = ldg4(x + j * pl + off); }
+        for (int a = __ldg(rowptr + row); a < __ldg(rowptr + row + 1); ++a) {
+            const int c = __ldg(col + a);
+            const float v = __ldg(val2 + a);
+            for (int j = 0; j < k; ++j) fma4(S[j], v, ldg4(x + j * pl + (size_t)c * B + 4 * c4));
+        }
+        if (MODE == 0) {
+            float4 mean = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int j = 0; j < k; ++j) { mean.x = fmaf(X[j].x, S[j].x, mean.x); mean.y = fmaf(X[j].y, S[j].y, mean.y); mean.z = fmaf(X[j].z, S[j].z, mean.z); mean.w = fmaf(X[j].w, S[j].w, mean.w); }
+            for (int j = 0; j < k; ++j)
+                *reinterpret_cast<float4*>(G + j * pl + off) = make_float4(X[j].x * (S[j].x - mean.x), X[j].y * (S[j].y - mean.y),
+                                                                          X[j].z * (S[j].z - mean.z), X[j].w * (S[j].w - mean.w));
+        } else {
+            const float4 yv = y ? *reinterpret_cast<const float4*>(y + off) : make_float4(y_scalar, y_scalar, y_scalar, y_scalar);
+            const float yq[4] = {yv.x, yv.y, yv.z, yv.w};
+            for (int q = 0; q < 4; ++q) {
+                double tr = 0.0, g = 0.0;
+                for (int j = 0; j < k; ++j) {
+                    const float v = q == 0 ? X[j].x : q == 1 ? X[j].y : q == 2 ? X[j].z : X[j].w;
+                    const float sv = q == 0 ? S[j].x : q == 1 ? S[j].y : q == 2 ? S[j].z : S[j].w;
+                    tr += 0.5 * (double)v * (double)sv;                      // val2 = 2 W_il
+                    if (gfun == GDA_G_QUADRATIC) g += (double)v * (double)v;
+                    else if (v > 0.0f) g += (double)v * (double)logf(v);
+                }
+                if (gfun == GDA_G_QUADRATIC) g -= 1.0;
+                acc[q] += tr + (double)yq[q] * g;
+            }
+        }
+    }
+    if (MODE == 1) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) red[warp][lane][q] = acc[q];
+        __syncthreads();
+        if (warp == 0 && active) {
+            double* out = partial + (size_t)blockIdx.x * B + 4 * c4;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                double t = red[0][lane][q];
+                for (int w = 1; w < WARPS; ++w) t += red[w][lane][q];
+                out[q] = t;
+            }
+        }
+    }
+}
+
+gda_status kcut_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s) {
+    const dim3 grid((unsigned)kcut_num_partials(p, B), (unsigned)((B / 4 + 31) / 32));
+    kcut_aux_kernel<0><<<grid, THREADS, 0, s>>>(p->n, B, p->kparts, p->d_rowptr, p->d_col, p->d_val2, x, nullptr, 0.0f, 0, G, nullptr);
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
+gda_status kcut_value_partials(gda_problem* p, int32_t B, const float* x, const float* y, float y_scalar, int32_t gfun,
+                               double* partial, int32_t* n_part, cudaStream_t s) {
+    const dim3 grid((unsigned)kcut_num_partials(p, B), (unsigned)((B / 4 + 31) / 32));
+    kcut_aux_kernel<1><<<grid, THREADS, 0, s>>>(p->n, B, p->kparts, p->d_rowptr, p->d_col, p->d_val2, x, y, y_scalar, gfun, nullptr, partial);
+    *n_part = (int32_t)grid.x;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
+}
+
 gda_status kcut_commit(gda_problem* p, int32_t B, const uint8_t* lab, const int32_t* improved, uint8_t* x_bin,
                        cudaStream_t s, int64_t* launches) {
     const size_t n_vec = (size_t)p->n * B / 4;

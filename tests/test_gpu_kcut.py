@@ -170,3 +170,26 @@ def test_score_of_given_logits_matches_the_oracle(api):
     lab = Z.argmax(axis=0).astype(np.uint8)                       # numpy's argmax also takes the first maximum
     assert np.array_equal(obj, kcut.objective(OK, lab))
     P.destroy()
+
+
+@pytest.mark.parametrize("w", CASES[:3] + [wl.maxkcut(90, 300, 3, B=10, seed=29)], ids=lambda w: f"{w.name}_B{w.B}")
+def test_gradient_and_lagrangian_of_the_softmax_form(api, w):
+    """gda_grad / gda_lagrangian on Max-k-Cut problems: grad_Z Tr(X W X^T) and L(SoftMax(Z), y)."""
+    Pw = w.problem
+    n, k, B = Pw.n, Pw.k, w.B
+    OP = kcut.Problem(n, k, Pw.rowptr, Pw.col, Pw.val.astype(np.float64))
+    P = api.create_from_workload(Pw)
+    rng = np.random.default_rng(3)
+    Z = (2.0 * rng.standard_normal((k, n, B))).astype(np.float32)
+    G = P.grad(dev(Z)).cpu().numpy()
+    Gref = kcut.grad(OP, Z.astype(np.float64))
+    assert G.shape == Z.shape
+    assert np.abs(G - Gref).max() <= TOL_STEP * max(1.0, np.abs(Gref).max())
+    Y = (3.0 * rng.random((n, B))).astype(np.float32)
+    for gfun in (0, 1):
+        L = P.lagrangian(dev(Z), dev(Y), gfun=gfun).cpu().numpy()
+        Lref = kcut.lagrangian(OP, Z.astype(np.float64), Y.astype(np.float64), gfun)
+        assert L.shape == (B,) and (np.abs(L - Lref) <= 1e-5 * np.maximum(1.0, np.abs(Lref))).all()
+        Ls = P.lagrangian(dev(Z), 1.5, gfun=gfun).cpu().numpy()
+        assert (np.abs(Ls - kcut.lagrangian(OP, Z.astype(np.float64), 1.5, gfun)) <= 1e-5 * np.maximum(1.0, np.abs(Lref))).all()
+    P.destroy()
