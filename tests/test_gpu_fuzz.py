@@ -130,3 +130,35 @@ def test_random_maxkcut(api, seed):
     r = P.run(dev(Z), h.lambda0, api.params_from_hyper(h, iters=120, eval_every=50))
     assert np.array_equal(r["obj"].cpu().numpy(), kcut.objective(OP, r["x_bin"].cpu().numpy()))
     P.destroy()
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_random_dense_qubo(api, oracle, seed):
+    """Dense path at random (mostly ragged) sizes: zero padding of variables and restarts, every cluster shape the sizes allow.
+    Tolerances: the north star's 1e-2 on the gradient (bf16 operand, reading R13) and what it implies for one step."""
+    rng = np.random.default_rng(6000 + seed)
+    n = int(rng.choice([1, 7, 100, 255, 256, 300, 513, 700]))
+    B = int(rng.choice([1, 10, 128, 130, 256, 300, 512]))
+    A = rng.standard_normal((n, n)).astype(np.float32)
+    Q = np.triu(A, 1) + np.triu(A, 1).T + np.diag(rng.standard_normal(n)).astype(np.float32)
+    Q = torch.from_numpy(Q).to(torch.bfloat16).to(torch.float32).numpy()          # bf16-representable (reading R13)
+    c = rng.standard_normal(n).astype(np.float32)
+    Pw = wl.QuboDense(n, Q, c)
+    s = 2.0 * np.sqrt(n)
+    h = wl.Hyper(1.75 * s, 1.0 / (4.0 * (s + 1.75 * s)), 4.0 * 1.75 * s / 1000.0, 1e-4, int(rng.integers(0, 2)), 1e-6, 120, 50, seed)
+    OP = oracle_problem(Pw)
+    P = api.create_from_workload(Pw)
+    X = rng.random((n, B), dtype=np.float32)
+    G = P.grad(dev(X)).cpu().numpy()
+    Gref = oracle.grad(OP, X.astype(np.float64))
+    gmax = np.maximum(np.abs(Gref).max(axis=0), 1.0)
+    assert (np.abs(G - Gref).max(axis=0) <= 1e-2 * gmax).all(), (n, B)
+    r1 = P.run(dev(X), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+    ref = oracle.run(OP, X, f32(h.lambda0), **okw(h, iters=1, eval_every=1))
+    assert (np.abs(r1["x"].cpu().numpy() - ref["x"]).max(axis=0) <= f32(h.alpha) * 1e-2 * gmax + 1e-5).all(), (n, B)
+    assert np.abs(r1["lam"].cpu().numpy() - ref["y"]).max() <= TOL_STEP * max(1.0, f32(h.lambda0))
+    r = P.run(dev(X), h.lambda0, api.params_from_hyper(h))
+    obj, Fref = r["obj"].cpu().numpy(), oracle.F_binary(OP, r["x_bin"].cpu().numpy())
+    assert np.allclose(obj, Fref, rtol=1e-5, atol=1e-5 * max(1.0, float(np.abs(Q).sum()) / max(n, 1)) * n)
+    assert int(r["best_restart"].item()) == int(np.argmin(obj))
+    P.destroy()
