@@ -501,7 +501,7 @@ static gda_status ensure_workspace(gda_problem* p, int32_t B) {
         if (st == GDA_OK) st = dmalloc(&ws.mu[0], (size_t)ld);
         if (st == GDA_OK) st = dmalloc(&ws.mu[1], (size_t)ld);
         if (st == GDA_OK) st = dmalloc(&ws.gpart, (size_t)ws.n_gpart * ld);
-        if (st == GDA_OK && p->kind == GDA_KIND_SPARSE) st = dmalloc(&ws.gacc, (size_t)GDA_GACC_WAYS * ld);
+        if (st == GDA_OK && p->kind == GDA_KIND_SPARSE) st = dmalloc(&ws.gacc, 2 * (size_t)GDA_GACC_WAYS * ld);   // S^t and S^{t+1}, by the parity of x
     }
     if (st == GDA_OK) st = dmalloc(&ws.state, 1);
     if (st == GDA_OK) st = dmalloc(&ws.block_min, (size_t)(ld + 7) / 8);          // one per block of finalize_kernel (32 restarts) or of the slab kernel (8)
@@ -576,7 +576,13 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
     for (int k = 0; k < len; ++k) {
         int64_t before = *launches;
         ScalarDual sd;                                        // PDBO-s: mu follows the parity of x
-        if (scalar) { sd.mu = ws.mu[cur]; sd.gpart = ws.gpart; sd.gacc = ws.gacc; sd.B = ws.ld; }
+        if (scalar) {
+            sd.mu = ws.mu[cur]; sd.mu_out = ws.mu[cur ^ 1]; sd.gpart = ws.gpart; sd.B = ws.ld; sd.beta = prm.beta; sd.advance = 1;
+            if (ws.gacc) {                                    // sparse path: S^t by the parity of x^t, S^{t+1} into the other half
+                const size_t half = (size_t)GDA_GACC_WAYS * ws.ld;
+                sd.gacc = ws.gacc + (size_t)cur * half; sd.gacc_next = ws.gacc + (size_t)(cur ^ 1) * half;
+            }
+        }
         if (p->kind == GDA_KIND_SPARSE)
             GDA_TRY(sparse_step(p, ws.ld, ws.x[cur], ws.y, ws.x[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         else if (p->kind == GDA_KIND_MAXSAT)
@@ -587,8 +593,6 @@ static gda_status enqueue_chunk(gda_problem* p, int32_t B, int32_t len, int32_t 
             GDA_TRY(dense_step(p, ws.ld, ws.x[0], ws.y, ws.zt[cur], ws.zt[cur ^ 1], up, sd, ws.state, (uint32_t)k, s, launches));
         if (scalar && p->kind != GDA_KIND_SPARSE)
             GDA_TRY(gsum_reduce(ws.ld, ws.gpart, ws.n_gpart, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
-        else if (scalar)
-            GDA_TRY(mu_finalize(ws.ld, ws.gacc, prm.beta, ws.mu[cur], ws.mu[cur ^ 1], s, launches));
         *step_launches += *launches - before;
         cur ^= 1;
     }
@@ -716,6 +720,8 @@ static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const flo
         GDA_TRY(run_init(p, B, x0, lambda0, lambda0_scalar, (uint32_t)prm->t0, s, &p->last_launches));
         if (p->kind == GDA_KIND_DENSE)
             GDA_TRY(dense_make_operand(p, ws.ld, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
+        if (p->kind == GDA_KIND_SPARSE && prm->dual == GDA_DUAL_SCALAR)      // S^0 for the pipelined multiplier update (parity 0)
+            GDA_TRY(sparse_dual_init(p, ws.ld, ws.x[0], prm->gfun, ws.gacc, s, &p->last_launches));
         if (p->kind == GDA_KIND_KCUT)                       // run_init put the logits in z; x[0] = SoftMax(z)
             GDA_TRY(kcut_softmax(p, ws.ld, ws.z, ws.x[0], s, &p->last_launches));
     } else {

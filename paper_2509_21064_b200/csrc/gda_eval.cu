@@ -277,17 +277,6 @@ count_ones_kernel(int n, int B, int ld, const uint8_t* __restrict__ x_bin, int32
         }
 }
 
-// PDBO-s, sparse / MaxSAT paths: close the step -- mu_out = mu_in + beta * (exact integer sum of the ways) / 2^32
-__global__ void __launch_bounds__(128)
-mu_finalize_kernel(int B, unsigned long long* __restrict__ gacc, float beta, const float* __restrict__ mu_in, float* __restrict__ mu_out) {
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B) return;
-    long long t = 0;
-#pragma unroll
-    for (int k = 0; k < GDA_GACC_WAYS; ++k) { t += (long long)gacc[(size_t)k * B + b]; gacc[(size_t)k * B + b] = 0ull; }
-    mu_out[b] = mu_in[b] + beta * (float)((double)t / GDA_GACC_SCALE);
-}
-
 __global__ void mu_init_kernel(int B, const float* __restrict__ l0, float l0_scalar, float* __restrict__ mu) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b < B) mu[b] = l0 ? l0[b] : l0_scalar;
@@ -298,14 +287,6 @@ __global__ void mu_init_kernel(int B, const float* __restrict__ l0, float l0_sca
 gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float beta, const float* mu_in, float* mu_out,
                        cudaStream_t s, int64_t* launches) {
     gsum_reduce_kernel<<<(unsigned)((B + 31) / 32), dim3(32, 32), 0, s>>>(B, gpart, n_gpart, beta, mu_in, mu_out);
-    if (launches) ++*launches;
-    GDA_CUDA_TRY(cudaGetLastError());
-    return GDA_OK;
-}
-
-gda_status mu_finalize(int32_t B, unsigned long long* gacc, float beta, const float* mu_in, float* mu_out, cudaStream_t s,
-                       int64_t* launches) {
-    mu_finalize_kernel<<<(unsigned)((B + 127) / 128), 128, 0, s>>>(B, gacc, beta, mu_in, mu_out);
     if (launches) ++*launches;
     GDA_CUDA_TRY(cudaGetLastError());
     return GDA_OK;
@@ -338,8 +319,8 @@ gda_status run_init(gda_problem* p, int32_t B, const float* x0, const float* l0,
         GDA_TRY(copy_in(ws.x[0], ld, x0, (size_t)B, (size_t)p->n, sizeof(float), s));
     }
     if (ws.dual == GDA_DUAL_SCALAR) {
-        if (ws.gacc)                                         // nothing pending from an earlier (possibly failed) run
-            GDA_CUDA_TRY(cudaMemsetAsync(ws.gacc, 0, (size_t)GDA_GACC_WAYS * ld * sizeof(unsigned long long), s));
+        if (ws.gacc)                                         // nothing pending from an earlier (possibly failed) run; both parities
+            GDA_CUDA_TRY(cudaMemsetAsync(ws.gacc, 0, 2 * (size_t)GDA_GACC_WAYS * ld * sizeof(unsigned long long), s));
         GDA_TRY(mu_init((int32_t)ld, nullptr, l0 ? 0.0f : l0_scalar, ws.mu[0], s, launches));
         if (l0) GDA_CUDA_TRY(cudaMemcpyAsync(ws.mu[0], l0, (size_t)B * sizeof(float), cudaMemcpyDefault, s));
     } else if (l0) {

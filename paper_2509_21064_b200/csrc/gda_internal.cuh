@@ -40,16 +40,23 @@ struct UpdParams {
 };
 
 // PDBO-s (GDA_DUAL_SCALAR) state handed to the step kernels; mu == nullptr means per-variable duals.
-// Sparse path: a step kernel reads this step's multipliers mu^t; every block adds its sum of g(x_i^t)
-// (fp32, fixed order inside the block) to one of GDA_GACC_WAYS accumulators per restart in 64-bit FIXED POINT (2^-32)
-// with integer reductions -- exact, hence independent of the order in which blocks arrive: deterministic -- and a
-// B-thread kernel (mu_finalize) adds the ways, writes mu^{t+1} = mu^t + beta * sum into the other mu buffer (the
-// buffers follow the parity of x) and clears them (config 3: 20.2 us per iteration against 22.1 us with partial rows).
+// Sparse path: the step kernel of iteration t reads the multipliers mu^t.  Every block adds the sum of g over the values
+// x^{t+1} IT WRITES (fp32, fixed order inside the block) to one of GDA_GACC_WAYS accumulators per restart in 64-bit FIXED
+// POINT (2^-32) with integer reductions -- exact, hence independent of the order in which blocks arrive: deterministic.  So
+// S^{t+1} = sum_i g(x_i^{t+1}) is complete when the kernel ends, one iteration BEFORE it is needed, and the multiplier update
+// mu^{t+1} = mu^t + beta S^t costs no launch of its own: block 0 of every 128-restart chunk of kernel t adds the ways of S^t
+// (left by kernel t - 1; by sparse_dual_init for t = 0), writes mu^{t+1} into the other mu buffer and clears them, while the
+// rest of the kernel runs (config 3: 22.1 us per iteration with partial rows and a reduce kernel, 19.8 with the fixed-point
+// sums and a B-thread finalize kernel, see DESIGN.md for this scheme).  mu and the accumulators follow the parity of x.
 // MaxSAT and dense paths: the blocks / epilogue threads leave their sums as rows of gpart and gsum_reduce adds them in a
 // fixed order and writes mu^{t+1} (on the MaxSAT kernel the integer reductions measured slower: 52.7 against 46.1 us).
 struct ScalarDual {
-    const float* mu = nullptr;                 // [B] this step's multipliers
-    unsigned long long* gacc = nullptr;        // [GDA_GACC_WAYS][B] sums of g(x_i^t), fixed point (two's complement), zero between steps
+    const float* mu = nullptr;                 // [B] this step's multipliers mu^t
+    unsigned long long* gacc = nullptr;        // [GDA_GACC_WAYS][B] S^t = sum_i g(x_i^t), fixed point (two's complement): complete; consumed and cleared
+    unsigned long long* gacc_next = nullptr;   // [GDA_GACC_WAYS][B] S^{t+1}: accumulated by this kernel (zero at its start)
+    float* mu_out = nullptr;                   // [B] mu^{t+1}, written by block 0 of every chunk of the launch with advance != 0
+    float beta = 0.0f;
+    int32_t advance = 0;
     int32_t B = 0;
     float* gpart = nullptr;                    // MaxSAT: [ceil(n / 8)][B]; dense: [n / 128][B]
 };
@@ -236,8 +243,8 @@ gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float bet
                        cudaStream_t s, int64_t* launches);
 gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, cudaStream_t s, int64_t* launches);
 // PDBO-s, sparse / MaxSAT: mu_out[b] = mu_in[b] + beta * (sum of the ways of gacc[.][b]) / 2^32; clears gacc
-gda_status mu_finalize(int32_t B, unsigned long long* gacc, float beta, const float* mu_in, float* mu_out, cudaStream_t s,
-                       int64_t* launches);
+gda_status sparse_dual_init(gda_problem* p, int32_t B, const float* x, int32_t gfun, unsigned long long* gacc, cudaStream_t s,
+                            int64_t* launches);      // S^0 = sum_i g(x_i^0) into the accumulators (start of a PDBO-s run)
 
 // ---------------------------------------------------------------------------------------------------
 // device helpers: g, g', the fused update S4 (Eq. 6 + perturbation), the tie-break hash
@@ -344,11 +351,40 @@ __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpre
 // scalar_dual_commit: ONE warp adds its block's sums t (lane = float4 of restarts c4) to accumulator `way`.
 __device__ __forceinline__ void scalar_dual_commit(float4 t, bool active, int c4, unsigned way, const ScalarDual& sd) {
     if (!active) return;
-    unsigned long long* acc = sd.gacc + (size_t)(way % GDA_GACC_WAYS) * sd.B + 4 * c4;
+    unsigned long long* acc = sd.gacc_next + (size_t)(way % GDA_GACC_WAYS) * sd.B + 4 * c4;
     atomicAdd(acc + 0, (unsigned long long)__double2ll_rn((double)t.x * GDA_GACC_SCALE));
     atomicAdd(acc + 1, (unsigned long long)__double2ll_rn((double)t.y * GDA_GACC_SCALE));
     atomicAdd(acc + 2, (unsigned long long)__double2ll_rn((double)t.z * GDA_GACC_SCALE));
     atomicAdd(acc + 3, (unsigned long long)__double2ll_rn((double)t.w * GDA_GACC_SCALE));
+}
+
+// A block of NW warps closes the multiplier update for the 128 restarts of its chunk (lane = float4 of restarts c4):
+// mu^{t+1} = mu^t + beta S^t, S^t the exact integer sum of the ways, and clears the ways.  Warp w takes the ways
+// w, w + NW, ... (four independent 16-byte loads per lane and way: one round trip), warp 0 adds the warps' sums.
+// Must be called by every thread of the block.
+template <int NW>
+__device__ __forceinline__ void scalar_dual_advance(long long (*adv)[32][4], int warp, int lane, bool active, int c4,
+                                                    const ScalarDual& sd) {
+    long long t[4] = {0, 0, 0, 0};
+    if (active) {
+        for (int k = warp; k < GDA_GACC_WAYS; k += NW) {
+            ulonglong2* p = reinterpret_cast<ulonglong2*>(sd.gacc + (size_t)k * sd.B + 4 * c4);
+            const ulonglong2 a = p[0], b = p[1];
+            t[0] += (long long)a.x; t[1] += (long long)a.y; t[2] += (long long)b.x; t[3] += (long long)b.y;
+            p[0] = make_ulonglong2(0ull, 0ull); p[1] = make_ulonglong2(0ull, 0ull);
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) adv[warp][lane][q] = t[q];
+    __syncthreads();
+    if (warp != 0 || !active) return;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        long long s = adv[0][lane][q];
+        for (int w = 1; w < NW; ++w) s += adv[w][lane][q];
+        const int b = 4 * c4 + q;
+        sd.mu_out[b] = sd.mu[b] + sd.beta * (float)((double)s / GDA_GACC_SCALE);
+    }
 }
 
 // Called by every thread of a block whose NW warps hold their sums of g in gs (0 for warps / lanes without work): the

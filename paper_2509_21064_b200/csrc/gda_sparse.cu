@@ -91,7 +91,8 @@ __device__ __forceinline__ float4 gather_row(const int32_t* __restrict__ col, co
 }
 
 // S4 for one (row, float4 of restarts).  DUAL (PDBO-s): `mu` is this step's multiplier for the four restarts, y is
-// not touched, and the values of g(x^t) are returned in gs (0 for lanes past a ragged B).
+// not touched, and g of the NEW iterate x^{t+1} is returned in gs (0 for lanes past a ragged B): the sum the multiplier
+// update of the NEXT iteration needs (ScalarDual in gda_internal.cuh).
 template <int GFUN, bool DUAL>
 __device__ __forceinline__ void update_store(int row, int c4, int B, bool active, float4 G, const float* __restrict__ x,
                                              float* __restrict__ y, float* __restrict__ xn,
@@ -106,7 +107,7 @@ __device__ __forceinline__ void update_store(int row, int c4, int B, bool active
     gda_update4<GFUN>(xv, yv, G, up, t, (uint32_t)row, 4u * (uint32_t)c4, xo, yo);
     if (!active) return;
     *reinterpret_cast<float4*>(reinterpret_cast<char*>(xn) + off) = xo;
-    if (DUAL) gs = make_float4(gda_g<GFUN>(xv.x, up), gda_g<GFUN>(xv.y, up), gda_g<GFUN>(xv.z, up), gda_g<GFUN>(xv.w, up));
+    if (DUAL) gs = make_float4(gda_g<GFUN>(xo.x, up), gda_g<GFUN>(xo.y, up), gda_g<GFUN>(xo.z, up), gda_g<GFUN>(xo.w, up));   // g of x^{t+1}: S^{t+1}
     else *yp = yo;
 }
 
@@ -118,7 +119,8 @@ __device__ __forceinline__ void update_store(int row, int c4, int B, bool active
 // 17.3 us per step before, 16.3 us with the lean gather loop, 14.8 us with the records and 6 blocks per SM;
 // prefetching the row's own x, y lines into L1 up front was slower (15.1 us) and is not done.
 // DUAL (PDBO-s, MODE 0 only): the multiplier is one number per restart (sd.mu), y is not read or written, and the
-// block's sum of g(x_i^t) goes through scalar_dual_finish (fixed-point integer reductions; mu_finalize closes the step).
+// block's sum of g over the values it writes goes through scalar_dual_finish (fixed-point integer reductions); block 0 of
+// every chunk also closes the multiplier update of this iteration from the sums the previous kernel left (scalar_dual_advance).
 template <int GFUN, int MODE, bool ELL, bool DUAL, bool PF>
 __global__ void __launch_bounds__(32 * warp_kernel_warps(DUAL), 6 * 8 / warp_kernel_warps(DUAL))
 spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
@@ -128,6 +130,7 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
                UpdParams up, ScalarDual sd, const RunState* __restrict__ st, uint32_t t_off) {
     constexpr int WW = warp_kernel_warps(DUAL);
     __shared__ float4 gred[DUAL ? WW : 1][32];
+    __shared__ long long adv[DUAL ? WW : 1][32][4];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ridx = blockIdx.x * WW + warp;
     const bool active = 4 * (blockIdx.y * 32 + lane) < B;
@@ -135,6 +138,7 @@ spmm_step_warp(int n_rows, const int32_t* __restrict__ row_list, int B,
     if (DUAL) {
         float4 gs = make_float4(0.f, 0.f, 0.f, 0.f);
         const float4 mu = ldg4(sd.mu + 4 * c4);
+        if (sd.advance && blockIdx.x == 0) scalar_dual_advance<WW>(adv, warp, lane, active, c4, sd);   // block-uniform: mu^{t+1} for this chunk's restarts
         if (ridx < n_rows) {                                 // warp-uniform
             const int row = row_list ? __ldg(row_list + ridx) : ridx;
             const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
@@ -249,6 +253,7 @@ spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chu
                 const float* __restrict__ x, float* __restrict__ y, float* __restrict__ xn,
                 UpdParams up, ScalarDual sd, const RunState* __restrict__ st, uint32_t t_off, int slice) {
     __shared__ float4 red[WARPS][32];
+    __shared__ long long adv[DUAL ? WARPS : 1][32][4];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int ridx = blockIdx.x / chunks, chunk = blockIdx.x % chunks;
     const int row = row_list ? __ldg(row_list + ridx) : ridx;
@@ -256,6 +261,7 @@ spmm_step_split(int n_rows, const int32_t* __restrict__ row_list, int B, int chu
     const int c4 = active ? chunk * 32 + lane : B / 4 - 1;
     const char* xb = reinterpret_cast<const char*>(x + 4 * c4);
     const int start = __ldg(rowptr + row), end = __ldg(rowptr + row + 1);
+    if (DUAL && sd.advance && ridx == 0) scalar_dual_advance<WARPS>(adv, warp, lane, active, c4, sd);   // block-uniform: mu^{t+1} for this chunk's restarts
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int base = start + slice * warp; base < end; base += slice * WARPS) {
         const float4 part = gather_row(col, val2, base, min(base + slice, end), xb, 4u * (uint32_t)B, lane);
@@ -689,6 +695,24 @@ spmm_value(int n, int B, int rows_per_block, const int32_t* __restrict__ rowptr,
         }
 }
 
+// PDBO-s, start of a run: S^0 = sum_i g(x_i^0) per restart into the fixed-point accumulators, block sums of 8 rows like the
+// step kernels' (ScalarDual in gda_internal.cuh)
+template <int GFUN>
+__global__ void __launch_bounds__(THREADS)
+dual_init_kernel(int n, int B, const float* __restrict__ x, UpdParams up, ScalarDual sd) {
+    __shared__ float4 gred[WARPS][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int row = blockIdx.x * WARPS + warp;
+    const bool active = 4 * (blockIdx.y * 32 + lane) < B;
+    const int c4 = active ? blockIdx.y * 32 + lane : B / 4 - 1;
+    float4 gs = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (row < n && active) {
+        const float4 xv = ldg4(x + (size_t)row * B + 4 * c4);
+        gs = make_float4(gda_g<GFUN>(xv.x, up), gda_g<GFUN>(xv.y, up), gda_g<GFUN>(xv.z, up), gda_g<GFUN>(xv.w, up));
+    }
+    scalar_dual_finish<WARPS>(gs, gred, warp, lane, active, c4, blockIdx.x, sd);
+}
+
 template <int MODE, bool DUAL>
 gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, float* xn, const UpdParams& up,
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
@@ -742,12 +766,14 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     }
     if (p->n_heavy > 0) {
         const unsigned grid = (unsigned)(p->n_heavy * chunks);
+        ScalarDual sdh = sd;
+        if (n_light > 0) sdh.advance = 0;                     // the launch above closes the multiplier update
         if (up.gfun == GDA_G_QUADRATIC)
             spmm_step_split<GDA_G_QUADRATIC, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off, 32);
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sdh, st, t_off, 32);
         else
             spmm_step_split<GDA_G_ENTROPY, MODE, DUAL><<<grid, THREADS, 0, s>>>(p->n_heavy, p->d_heavy_rows, B, chunks, p->d_rowptr,
-                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sd, st, t_off, 32);
+                p->d_col, p->d_val2, p->d_cprime, x, y, xn, up, sdh, st, t_off, 32);
         if (launches) ++*launches;
     }
     GDA_CUDA_TRY(cudaGetLastError());
@@ -777,6 +803,20 @@ gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, floa
                        const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s, int64_t* launches) {
     if (sd.mu) return launch_step<0, true>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
     return launch_step<0, false>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
+}
+
+gda_status sparse_dual_init(gda_problem* p, int32_t B, const float* x, int32_t gfun, unsigned long long* gacc, cudaStream_t s,
+                            int64_t* launches) {
+    UpdParams up{};
+    up.gfun = gfun;
+    ScalarDual sd;
+    sd.gacc_next = gacc; sd.B = B;
+    const dim3 grid((unsigned)((p->n + WARPS - 1) / WARPS), (unsigned)((B / 4 + 31) / 32));
+    if (gfun == GDA_G_QUADRATIC) dual_init_kernel<GDA_G_QUADRATIC><<<grid, THREADS, 0, s>>>(p->n, B, x, up, sd);
+    else dual_init_kernel<GDA_G_ENTROPY><<<grid, THREADS, 0, s>>>(p->n, B, x, up, sd);
+    if (launches) ++*launches;
+    GDA_CUDA_TRY(cudaGetLastError());
+    return GDA_OK;
 }
 
 gda_status sparse_grad(gda_problem* p, int32_t B, const float* x, float* G, cudaStream_t s) {
