@@ -196,3 +196,22 @@ def test_mis_ones_and_host_run_at_B_10(api, oracle):
     rh = P.run_host(X0, h.lambda0, prm)
     assert np.array_equal(rh["obj"], obj) and np.array_equal(rh["x_bin"], xb) and rh["best_restart"] == int(np.argmin(obj))
     P.destroy()
+
+
+@pytest.mark.parametrize("kind,B", [("slab", 20002), ("stream", 40003), ("maxsat", 30001)], ids=lambda v: str(v))
+def test_large_odd_batches(api, oracle, kind, B):
+    """Tens of thousands of restarts, not a multiple of anything: hundreds of 128-restart chunks, a ragged last one."""
+    w, path = workload(kind, B)
+    h, n = w.hyper, w.problem.n
+    OP = oracle_problem(w.problem)
+    P = create_problem(api, w, sparse_path=path)
+    X0 = wl.x0_uniform(n, B, 3)
+    sel = np.r_[0:40, B - 40:B]                                # the first and the last restarts through the oracle
+    r1 = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+    ref = oracle.run(OP, np.ascontiguousarray(X0[:, sel]), f32(h.lambda0), **okw(h, iters=1, eval_every=1))
+    assert np.abs(r1["x"].cpu().numpy()[:, sel] - ref["x"]).max() <= TOL_STEP
+    r = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=120, eval_every=50))
+    obj, xb = r["obj"].cpu().numpy(), r["x_bin"].cpu().numpy()
+    assert np.array_equal(obj[sel], oracle.F_binary(OP, np.ascontiguousarray(xb[:, sel])))
+    assert int(r["best_restart"].item()) == int(np.argmin(obj))
+    P.destroy()
