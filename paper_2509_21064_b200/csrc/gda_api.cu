@@ -721,7 +721,7 @@ static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const flo
         if (p->kind == GDA_KIND_DENSE)
             GDA_TRY(dense_make_operand(p, ws.ld, ws.x[0], ws.zt[0], /*hat=*/0, s, &p->last_launches));
         if (p->kind == GDA_KIND_SPARSE && prm->dual == GDA_DUAL_SCALAR)      // S^0 for the pipelined multiplier update (parity 0)
-            GDA_TRY(sparse_dual_init(p, ws.ld, ws.x[0], prm->gfun, ws.gacc, s, &p->last_launches));
+            GDA_TRY(sparse_dual_init(p, ws.ld, ws.x[0], prm->gfun, prm->log_eps, ws.gacc, s, &p->last_launches));
         if (p->kind == GDA_KIND_KCUT)                       // run_init put the logits in z; x[0] = SoftMax(z)
             GDA_TRY(kcut_softmax(p, ws.ld, ws.z, ws.x[0], s, &p->last_launches));
     } else {

@@ -244,7 +244,7 @@ gda_status gsum_reduce(int32_t B, const float* gpart, int32_t n_gpart, float bet
                        cudaStream_t s, int64_t* launches);
 gda_status mu_init(int32_t B, const float* l0, float l0_scalar, float* mu, cudaStream_t s, int64_t* launches);
 // PDBO-s, sparse / MaxSAT: mu_out[b] = mu_in[b] + beta * (sum of the ways of gacc[.][b]) / 2^32; clears gacc
-gda_status sparse_dual_init(gda_problem* p, int32_t B, const float* x, int32_t gfun, unsigned long long* gacc, cudaStream_t s,
+gda_status sparse_dual_init(gda_problem* p, int32_t B, const float* x, int32_t gfun, float log_eps, unsigned long long* gacc, cudaStream_t s,
                             int64_t* launches);      // S^0 = sum_i g(x_i^0) into the accumulators (start of a PDBO-s run)
 
 // ---------------------------------------------------------------------------------------------------

@@ -805,10 +805,10 @@ gda_status sparse_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     return launch_step<0, false>(p, B, x, y, xn, up, sd, st, t_off, s, launches);
 }
 
-gda_status sparse_dual_init(gda_problem* p, int32_t B, const float* x, int32_t gfun, unsigned long long* gacc, cudaStream_t s,
+gda_status sparse_dual_init(gda_problem* p, int32_t B, const float* x, int32_t gfun, float log_eps, unsigned long long* gacc, cudaStream_t s,
                             int64_t* launches) {
     UpdParams up{};
-    up.gfun = gfun;
+    up.gfun = gfun; up.log_eps = log_eps;                      // the entropy g clamps at log_eps (reading R4)
     ScalarDual sd;
     sd.gacc_next = gacc; sd.B = B;
     const dim3 grid((unsigned)((p->n + WARPS - 1) / WARPS), (unsigned)((B / 4 + 31) / 32));

@@ -742,6 +742,29 @@ def test_pdbo_s_row_grouping_is_bit_identical(api):
         assert torch.equal(a, b)
 
 
+@pytest.mark.parametrize("kind", ["sparse", "maxsat"])
+def test_pdbo_s_entropy_from_exact_binary_points(api, oracle, kind):
+    """The sum of g over the START point seeds the multiplier pipeline (dual_init kernels): with the entropy g and coordinates
+    at exactly 0 and 1 it must use the clamp of reading R4 (0 ln 0 = 0), not ln 0."""
+    w = wl.pdbo_s_variant(wl.config(3, B=132, n_scale=0.05) if kind == "sparse" else wl.config(5, B=132, n_scale=0.05))
+    h = w.hyper
+    h.gfun = 1
+    n, B = w.problem.n, w.B
+    OP = oracle_problem(w.problem)
+    P = create_problem(api, w, sparse_path="stream" if kind == "sparse" else None)
+    X0 = wl.x0_uniform(n, B, 5)
+    X0[:, :8] = np.round(X0[:, :8])                              # whole restarts at binary points
+    X0[::3, 8:16] = 0.0
+    for iters in (1, 3):
+        r = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=iters, eval_every=iters), want_final=True)
+        ref = oracle.run(OP, X0, f32(h.lambda0), **okw(h, iters=iters, eval_every=iters))
+        xg, mg = r["x"].cpu().numpy(), r["lam"].cpu().numpy()
+        assert np.isfinite(xg).all() and np.isfinite(mg).all()
+        assert np.abs(xg - ref["x"]).max() <= TOL_STEP * iters
+        assert (np.abs(mg - ref["y"]) <= mu_tolerance(h, n, ref["y"]) * iters).all()
+    P.destroy()
+
+
 def test_pdbo_s_heavy_rows_and_argument_checks(api, oracle):
     Pw = star_plus_isolated(700, 5)                             # row-split kernel + empty rows
     OP = oracle_problem(Pw)
