@@ -11,6 +11,7 @@
 #include "gda_internal.cuh"
 
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -876,6 +877,41 @@ gda_status sparse_build_slab(gda_problem* p, const std::vector<int32_t>& rowptr,
     std::vector<int32_t> order(n);
     for (int i = 0; i < n; ++i) order[i] = i;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return rowptr[a + 1] - rowptr[a] > rowptr[b + 1] - rowptr[b]; });
+    // 0. which rows share a quad.  A quad's schedule is at least as long as its longest row AND as the largest number of
+    //    entries its four rows have in one column class (col mod 4: every pass serves each class once), and with random
+    //    columns the second bound is the larger one (48-entry rows: about 55).  So inside windows of 128 rows of similar
+    //    degree the quads are put together greedily such that the class sums stay level.
+    {
+        std::vector<std::array<int, 4>> cls(n);
+        for (int i = 0; i < n; ++i) {
+            cls[i] = {0, 0, 0, 0};
+            for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) if (val2[k] != 0.0f) ++cls[i][col[k] & 3];
+        }
+        constexpr int WINDOW = 128;          // config 2, us per step: no balancing 8.48, windows of 16 / 32 / 64 / 128 / 256 / 800 rows 8.21 / 8.24 / 8.15 / 8.09 / 8.22 / 8.79
+        std::vector<int32_t> balanced;
+        balanced.reserve(n);
+        for (int w0 = 0; w0 < n; w0 += WINDOW) {
+            std::vector<int32_t> pool(order.begin() + w0, order.begin() + std::min(n, w0 + WINDOW));
+            while (!pool.empty()) {
+                std::array<int, 4> sum = cls[pool[0]];
+                balanced.push_back(pool[0]);
+                pool.erase(pool.begin());
+                for (int j = 1; j < 4 && !pool.empty(); ++j) {
+                    size_t best = 0; long best_score = -1;
+                    for (size_t q = 0; q < pool.size(); ++q) {
+                        long mx = 0, sq = 0;
+                        for (int c = 0; c < 4; ++c) { const long v = sum[c] + cls[pool[q]][c]; mx = std::max(mx, v); sq += v * v; }
+                        const long score = mx * 1000000L + sq;
+                        if (best_score < 0 || score < best_score) { best_score = score; best = q; }
+                    }
+                    for (int c = 0; c < 4; ++c) sum[c] += cls[pool[best]][c];
+                    balanced.push_back(pool[best]);
+                    pool.erase(pool.begin() + best);
+                }
+            }
+        }
+        order.swap(balanced);
+    }
     // 1. quads of four rows of similar degree.  The four rows of a quad share every LDS.128 pass: order their entries
     //    such that the four columns of a pass differ mod 4 (one 32-byte row of x per bank group).  Greedy: per pass, the
     //    assignment of distinct classes to the rows that uses up the most entries, ties to the largest remaining
