@@ -184,6 +184,40 @@ gda_status gda_score(gda_problem* p, int32_t B, const float* x, double* obj, voi
 gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, const float* lambda, float lambda_scalar,
                           int32_t gfun, float log_eps, double* out, void* stream);
 
+/* ---- scoring without any allocation -------------------------------------------------------------------
+ * gda_score_qubo_csr_static: obj[b] = F(x_hat_b) = x_hat^T Q x_hat + c^T x_hat, x_hat = [X[:,b] > 1/2] (the
+ * rounding and scoring step S5, reading R5) -- the result gda_score gives on a gda_create_qubo_csr handle,
+ * for callers that must not allocate device memory.
+ *
+ * Who that is.  A gda_problem handle is cudaMalloc'd memory (problem copy, iterates, a table of partial sums).  A host
+ * application that gave its whole HBM to its own pool at start-up, that runs under a latency bound (cudaMalloc / cudaFree may
+ * synchronise the whole device and so stall every stream of the process), or that may only touch buffers it was handed,
+ * cannot create one.  This entry point needs no handle: the problem is passed as the CSR the caller already keeps on the
+ * device, and the partial-sum table lives in a fixed 4 MiB array inside the library's image (GDA_STATIC_SCRATCH_BYTES; a
+ * file-scope __device__ array in csrc/gda_static.cu).  It calls no cudaMalloc, cudaFree or other allocating routine.
+ *
+ * Arguments -- ALL pointers are DEVICE memory of the current device, owned by the caller, nothing is copied or kept:
+ *   rowptr int32 [n+1], col int32 [rowptr[n]], val fp32 [rowptr[n]]: Q in CSR, every stored entry (i, j, Q_ij) counted once,
+ *          so a symmetric Q has both directions stored; diagonal entries are allowed (x_hat_i^2 = x_hat_i);
+ *   c      fp32 [n] or NULL (= 0);   x fp32 [n][B] row-major, any B >= 1 (no alignment needed);   obj double [B], written.
+ *   The CSR is NOT validated (that would need a copy to the host): rowptr must be non-decreasing from 0 and every column in
+ *   [0, n).  Sums are taken in fp64 in CSR order: exact for integer coefficients.
+ * Limits and sharing:
+ *   - B <= GDA_STATIC_SCORE_MAX_B (4096), any n > 0.  More restarts: GDA_ERR_UNSUPPORTED (score them in slices of <= 4096).
+ *   - every GPU that loads the library holds the 4 MiB until the process exits;
+ *   - the array is shared by ALL calls on a GPU.  Calls on one stream are ordered and fine; two calls that overlap on the
+ *     GPU (different streams or threads) race on it and return wrong objectives without an error -- serialise them.  It keeps
+ *     the previous call's contents; each call overwrites every entry it reads, so nothing needs clearing in between.
+ *   - the FIRST call on each GPU looks the array's device address up (cudaGetSymbolAddress, with that GPU current) and may
+ *     trigger the load of the module: make it once at start-up, before any stream capture begins.
+ *   - the device that `stream` belongs to must be the current device.  Asynchronous on `stream` like gda_score.
+ * INVALID_ARG: null pointer (c excepted), n <= 0, B <= 0, a pointer that is not device (or managed) memory.
+ * UNSUPPORTED: B > GDA_STATIC_SCORE_MAX_B.  ERR_CUDA: no usable device, or a failed CUDA call. */
+#define GDA_STATIC_SCORE_MAX_B 4096
+#define GDA_STATIC_SCRATCH_BYTES (4 * 1024 * 1024)
+gda_status gda_score_qubo_csr_static(int32_t n, const int32_t* rowptr, const int32_t* col, const float* val,
+                                     const float* c, int32_t B, const float* x, double* obj, void* stream);
+
 /* ---- queries ------------------------------------------------------------------------------------------ */
 typedef struct {
     int32_t kind;        /* 0 sparse QUBO, 1 dense QUBO, 2 MaxSAT, 3 Max-k-Cut                          */

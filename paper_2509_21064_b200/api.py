@@ -48,7 +48,8 @@ class Info(C.Structure):
 
 
 EXPORTS = ["gda_create_qubo_csr", "gda_create_qubo_dense", "gda_create_maxsat", "gda_create_maxkcut", "gda_destroy", "gda_run",
-           "gda_run_host", "gda_grad", "gda_score", "gda_lagrangian", "gda_get_info", "gda_last_error", "gda_version"]
+           "gda_run_host", "gda_grad", "gda_score", "gda_lagrangian", "gda_score_qubo_csr_static", "gda_get_info",
+           "gda_last_error", "gda_version"]
 
 
 def lib():
@@ -71,6 +72,7 @@ def lib():
         L.gda_grad.argtypes = [vp, i32, vp, vp, vp]
         L.gda_score.argtypes = [vp, i32, vp, vp, vp]
         L.gda_lagrangian.argtypes = [vp, i32, vp, vp, f32, i32, f32, vp, vp]
+        L.gda_score_qubo_csr_static.argtypes = [i32, vp, vp, vp, vp, i32, vp, vp, vp]
         L.gda_get_info.argtypes = [vp, C.POINTER(Info)]
         L.gda_last_error.restype = C.c_char_p
         L.gda_version.restype = C.c_char_p
@@ -260,6 +262,29 @@ class Problem:
         inf = Info()
         _check(lib().gda_get_info(self._h, C.byref(inf)))
         return inf
+
+
+STATIC_SCORE_MAX_B = 4096
+
+
+def score_qubo_csr_static(n, rowptr, col, val, c, x, obj, stream=None):
+    """gda_score_qubo_csr_static: obj[b] = F([x[:, b] > 1/2]) of the QUBO given as DEVICE CSR tensors, for callers that must
+    not allocate device memory (a host process whose pool owns all of the HBM, a loop that cannot afford cudaMalloc's
+    device-wide synchronisation, code restricted to the buffers it was handed).  No handle, and nothing is allocated on the
+    way -- not by the library (its partial sums live in a fixed 4 MiB array inside its image) and not here: every tensor,
+    the output `obj` (float64 [B]) included, is the caller's.  rowptr / col int32, val / c float32 (c may be None),
+    x float32 [n][B] with B <= STATIC_SCORE_MAX_B.  One array per GPU serves all calls: calls on different streams or
+    threads that overlap on the GPU race on it; calls on one stream are ordered.  The first call on a GPU does the one-time
+    address look-up and should happen at start-up, outside any stream capture."""
+    import torch
+    for t, dt in ((rowptr, torch.int32), (col, torch.int32), (val, torch.float32), (x, torch.float32), (obj, torch.float64)):
+        assert t.is_cuda and t.dtype == dt and t.is_contiguous()
+    assert c is None or (c.is_cuda and c.dtype == torch.float32 and c.is_contiguous() and c.numel() == n)
+    assert rowptr.numel() == n + 1 and x.dim() == 2 and x.shape[0] == n and obj.numel() == x.shape[1]
+    s = torch.cuda.current_stream(x.device).cuda_stream if stream is None else stream
+    _check(lib().gda_score_qubo_csr_static(n, rowptr.data_ptr(), col.data_ptr(), val.data_ptr(),
+                                           None if c is None else c.data_ptr(), x.shape[1], x.data_ptr(), obj.data_ptr(), s))
+    return obj
 
 
 def create_from_workload(P) -> Problem:

@@ -12,7 +12,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "lib" / "libgda_b200.so"
-SOURCES = ["gda_api.cu", "gda_sparse.cu", "gda_maxsat.cu", "gda_eval.cu", "gda_dense.cu", "gda_kcut.cu"]
+SOURCES = ["gda_api.cu", "gda_sparse.cu", "gda_maxsat.cu", "gda_eval.cu", "gda_dense.cu", "gda_kcut.cu", "gda_static.cu"]
 NVCC_FLAGS = ["-t", "0", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 

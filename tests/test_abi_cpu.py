@@ -104,6 +104,23 @@ def test_no_cpu_fallback_without_a_device(L):
     assert e.value.status == 3 and "no CPU fallback" in str(e.value)
 
 
+def test_static_score_checks_sizes_before_the_device(L):
+    """gda_score_qubo_csr_static (the entry point that allocates nothing): sizes beyond its fixed scratch array and null
+    pointers are refused before any CUDA call, with a message that names the limit."""
+    text = (ROOT / "include" / "gda.h").read_text()
+    assert int(re.search(r"#define GDA_STATIC_SCORE_MAX_B (\d+)", text).group(1)) == api.STATIC_SCORE_MAX_B
+    one = C.c_void_p(256)                                         # never dereferenced: the checks below fail first
+    f = L.gda_score_qubo_csr_static
+    assert f(5, one, one, one, None, api.STATIC_SCORE_MAX_B + 1, one, one, None) == 4
+    assert b"GDA_STATIC_SCORE_MAX_B = 4096" in L.gda_last_error()
+    assert f(0, one, one, one, None, 8, one, one, None) == 1
+    assert f(5, one, one, one, None, 0, one, one, None) == 1
+    assert f(5, None, one, one, None, 8, one, one, None) == 1
+    assert f(5, one, one, one, None, 8, one, None, None) == 1
+    if not has_gpu():                                             # valid sizes, no device: loud failure, no CPU path
+        assert f(5, one, one, one, None, 8, one, one, None) == 3
+
+
 def test_product_path_does_not_import_the_oracle():
     pkg = ROOT / "paper_2509_21064_b200"
     for f in list(pkg.rglob("*.py")) + list(pkg.rglob("*.cu")) + list(pkg.rglob("*.cuh")):
