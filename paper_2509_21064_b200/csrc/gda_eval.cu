@@ -273,7 +273,7 @@ count_ones_kernel(int n, int B, int ld, const uint8_t* __restrict__ x_bin, int32
         for (int q = 0; q < 4; ++q) {
             int t = 0;
             for (int k = 0; k < 32; ++k) t += red[k][lane][q];
-            ones[c + q] = t;
+            if (c + q < B) ones[c + q] = t;                  // the caller's buffer is [B]: padding restarts are not stored
         }
 }
 

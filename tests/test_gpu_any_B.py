@@ -215,3 +215,47 @@ def test_large_odd_batches(api, oracle, kind, B):
     assert np.array_equal(obj[sel], oracle.F_binary(OP, np.ascontiguousarray(xb[:, sel])))
     assert int(r["best_restart"].item()) == int(np.argmin(obj))
     P.destroy()
+
+
+@pytest.mark.parametrize("B", [1, 10, 13])
+@pytest.mark.parametrize("kind", ["slab", "stream", "maxsat", "dense"])
+def test_outputs_stay_inside_the_callers_buffers(api, kind, B):
+    """Every output of gda_run is documented as [B] or [n][B]: with B not a multiple of 4 the padding restarts must not be
+    stored.  Each output is a slice in the middle of a larger buffer filled with a sentinel; the bytes on both sides must be
+    untouched afterwards (torch rounds allocations up to 512 bytes, so an overrun of a tensor of its own goes unnoticed:
+    count_ones_kernel once wrote ones[B .. 4 ceil(B/4))."""
+    import ctypes as C
+    if kind == "dense":
+        w, path = wl.config(4, B=B, n_exact=300), None
+    else:
+        w, path = workload(kind, B)
+    h, n = w.hyper, w.problem.n
+    P = create_problem(api, w, sparse_path=path)
+    x0 = dev(wl.x0_uniform(n, B, w.x0_seed))
+    PAD = 64
+
+    def guarded(numel, dtype, sentinel):
+        buf = torch.full((numel + 2 * PAD,), sentinel, dtype=dtype, device="cuda")
+        return buf, buf[PAD:PAD + numel]
+
+    bufs = dict(x_bin=guarded(n * B, torch.uint8, 0xAB), obj=guarded(B, torch.float64, -7.25), best_restart=guarded(1, torch.int32, -77),
+                x_final=guarded(n * B, torch.float32, -7.25), lambda_final=guarded(n * B, torch.float32, -7.25),
+                best_obj=guarded(1, torch.float64, -7.25), ones=guarded(B, torch.int32, -77),
+                trace_best=guarded(8, torch.float64, -7.25), trace_ns=guarded(8, torch.int64, -77))
+    ex = api.Extra()
+    ex.x_final, ex.lambda_final, ex.best_obj = (bufs[k][1].data_ptr() for k in ("x_final", "lambda_final", "best_obj"))
+    ex.ones, ex.trace_best, ex.trace_ns, ex.trace_cap = bufs["ones"][1].data_ptr(), bufs["trace_best"][1].data_ptr(), bufs["trace_ns"][1].data_ptr(), 8
+    prm = api.params_from_hyper(h, iters=30, eval_every=7)
+    st = api.lib().gda_run(P._h, B, x0.data_ptr(), None, float(h.lambda0), C.byref(prm), bufs["x_bin"][1].data_ptr(),
+                           bufs["obj"][1].data_ptr(), bufs["best_restart"][1].data_ptr(), C.byref(ex),
+                           torch.cuda.current_stream().cuda_stream)
+    assert st == 0, api.lib().gda_last_error()
+    torch.cuda.synchronize()
+    for name, (buf, view) in bufs.items():
+        sentinel = buf[0].item()
+        assert (buf[:PAD] == sentinel).all() and (buf[PAD + view.numel():] == sentinel).all(), name
+    xb = bufs["x_bin"][1].view(n, B)
+    assert (xb <= 1).all() and torch.equal(bufs["ones"][1], xb.sum(dim=0).to(torch.int32))
+    rescored = P.score(xb.float())
+    assert torch.equal(rescored, bufs["obj"][1]) if kind != "dense" else torch.allclose(rescored, bufs["obj"][1], rtol=1e-5, atol=1e-2)
+    P.destroy()
