@@ -393,13 +393,13 @@ spmm_chunk_slab(const SlabArgs a) {
         float4 xv = make_float4(0.f, 0.f, 0.f, 0.f), yv = xv;
         if (b0 + 4 * qq < a.B) {
             const size_t off = (size_t)row * a.B + b0 + 4 * qq;
-            xv = ldg4(a.x_in + off);
-            if (!DUAL) yv = ldg4(a.y + off);
+            xv = __ldcg(reinterpret_cast<const float4*>(a.x_in + off));       // not ld.global.nc: this kernel writes x (x_out may alias
+            if (!DUAL) yv = __ldcg(reinterpret_cast<const float4*>(a.y + off));   // x_in), y and mu back, so they are not read-only for it
         }
         reinterpret_cast<float4*>(xa)[e] = xv;
         if (!DUAL) reinterpret_cast<float4*>(ys)[e] = yv;
     }
-    if (DUAL && threadIdx.x < SLAB_S) s_mu[threadIdx.x] = b0 + (int)threadIdx.x < a.B ? __ldg(a.mu_in + b0 + threadIdx.x) : 0.0f;
+    if (DUAL && threadIdx.x < SLAB_S) s_mu[threadIdx.x] = b0 + (int)threadIdx.x < a.B ? __ldcg(a.mu_in + b0 + threadIdx.x) : 0.0f;
     for (int e = threadIdx.x; e < a.n; e += blockDim.x) cps[e] = __ldg(a.cprime + e);
     if (COMPACT) {
         for (int e = threadIdx.x; e < a.n_pass * SLAB_ROWS; e += blockDim.x) cst[e] = __ldg(a.ent16 + e);
