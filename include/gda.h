@@ -133,7 +133,10 @@ typedef struct {
     double* best_obj;     /* [1]    obj[best_restart]                                                   */
     double* trace_best;   /* [trace_cap] min over restarts of the best objective after evaluation k     */
     uint64_t* trace_ns;   /* [trace_cap] GPU globaltimer (ns) when evaluation k finished                */
-    int32_t trace_cap;    /* entries available in the two trace arrays (evaluations beyond it are dropped) */
+    int32_t trace_cap;    /* entries available in the two trace arrays (evaluations beyond it are dropped).  The arrays   *
+                           * receive the evaluations of THIS call, entry 0 = its first one, also when the call resumes *
+                           * an earlier run; one call records at most 4096 evaluations, later ones are not traced, and  *
+                           * entries past the call's last evaluation are left as the caller had them                   */
     int32_t* ones;        /* [B]    number of ones in x_bin[:, b].  With obj it decides feasibility where the     *
                            *        objective is a penalised count, e.g. MIS as a QUBO:      *
                            *        F = -|S| + lam * (edges inside S), so S is independent iff obj[b] == -ones[b] */
@@ -148,7 +151,8 @@ typedef struct {
  *               objective seen at any evaluation (R5)
  *   obj         DEVICE double [B]: F(x_bin[:,b]) -- exact integers when all coefficients are integers
  *   best_restart DEVICE int32 [1]: argmin_b obj[b], ties -> lowest b (R6)
- * UNSUPPORTED: n * B >= 2^30 elements (after the dense path's padding; times k for Max-k-Cut).
+ * UNSUPPORTED: n * B >= 2^30 elements, counted on the padded workspace (B rounded up to a multiple of 4, sometimes 8; dense
+ * problems: n to a multiple of 256 and B to a multiple of 128; times k for Max-k-Cut) -- the message prints those sizes.
  * INVALID_ARG: null required pointer, B <= 0, alpha <= 0, beta < 0 or non-finite, delta outside
  * [0, 1/2), eval_every <= 0, iters < 0, unknown gfun or dual, log_eps outside (0, 1/2) with the entropy g;
  * a resumed run (x0 == NULL) whose `dual` differs from the run it continues.                              */

@@ -692,7 +692,9 @@ static gda_status check_run_args(const gda_problem* p, int32_t B, const float* x
         return GDA_ERR_UNSUPPORTED;
     }
     if ((int64_t)p->n_pad * (int64_t)lead_dim(p, B) * (p->kind == GDA_KIND_KCUT ? p->kparts : 1) >= ((int64_t)1 << 30)) {
-        gda_set_error("gda_run: n * B must be below 2^30 (got %lld): kernels use 32-bit byte offsets into X", (long long)p->n * B);
+        gda_set_error("gda_run: the padded state, %d rows x %d restarts%s, must stay below 2^30 elements (got %lld for n = %d, B = %d): "
+                      "kernels use 32-bit byte offsets into X", p->n_pad, lead_dim(p, B), p->kind == GDA_KIND_KCUT ? " x k parts" : "",
+                      (long long)p->n_pad * lead_dim(p, B) * (p->kind == GDA_KIND_KCUT ? p->kparts : 1), p->n, B);
         return GDA_ERR_UNSUPPORTED;
     }
     return GDA_OK;
@@ -709,7 +711,6 @@ static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const flo
     cudaStream_t user, s;
     GDA_TRY(pick_stream(p, stream, &user, &s));
     Workspace& ws = p->ws;
-    const size_t elems = (size_t)p->n * B;
     p->last_launches = 0; p->last_step_launches = 0;
 
     int parity = 0;
@@ -726,6 +727,10 @@ static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const flo
             GDA_TRY(kcut_softmax(p, ws.ld, ws.z, ws.x[0], s, &p->last_launches));
     } else {
         parity = ws.parity;      // resume: iterates, duals, best-so-far and the iteration counter stay as they are
+        // ... but the internal trace starts over: this call's evaluations land at entry 0 and are what the caller's trace
+        // arrays receive, however many evaluations the runs before it recorded (the buffer holds TRACE_CAP per call)
+        GDA_CUDA_TRY(cudaMemsetAsync(&ws.state->n_eval, 0, sizeof(uint32_t), s));
+        ws.n_eval_host = 0;
     }
     const int32_t full = prm->iters / prm->eval_every, rem = prm->iters % prm->eval_every;
     const int32_t n_eval = std::max(1, full + (rem > 0 ? 1 : 0)), trace_off = ws.n_eval_host;
@@ -754,7 +759,7 @@ static gda_status run_impl(gda_problem* p, int32_t B, const float* x0, const flo
             GDA_TRY(copy_out(extra->lambda_final, (size_t)B, ws.y, ld, n, sizeof(float), s));
         if (extra->ones) GDA_TRY(eval_count_ones(p, B, ws.x_bin, extra->ones, s, &p->last_launches));
         if (extra->best_obj) GDA_CUDA_TRY(cudaMemcpyAsync(extra->best_obj, ws.best_val, sizeof(double), cudaMemcpyDeviceToDevice, s));
-        // THIS call's evaluations: a resumed run appends to the trace of the run it continues (n_eval is not reset)
+        // THIS call's evaluations (the internal trace restarts at every call, resumed or not: trace_off == 0)
         const int32_t cnt = std::min(std::min(n_eval, extra->trace_cap), ws.trace_cap - trace_off);
         if (extra->trace_best && cnt > 0) GDA_CUDA_TRY(cudaMemcpyAsync(extra->trace_best, ws.trace_best + trace_off, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToDevice, s));
         if (extra->trace_ns && cnt > 0) GDA_CUDA_TRY(cudaMemcpyAsync(extra->trace_ns, ws.trace_ns + trace_off, (size_t)cnt * sizeof(uint64_t), cudaMemcpyDeviceToDevice, s));

@@ -469,6 +469,30 @@ def test_resumed_run_returns_its_own_slice_of_the_trace(api):
     P.destroy()
 
 
+def test_trace_of_a_resumed_run_after_more_evaluations_than_the_internal_buffer_holds(api):
+    """The library keeps 4096 trace entries per CALL: a resumed run starts its trace over, so its evaluations reach the
+    caller's arrays however many evaluations came before (they once stayed unwritten when the runs before had filled
+    the buffer), and a dense-problem size beyond the limit is refused with the padded sizes in the message."""
+    w = wl.config(1)
+    P = create_problem(api, w)
+    n, B, h = w.problem.n, w.B, w.hyper
+    first = P.run(dev(wl.x0_uniform(n, B, 7)), h.lambda0, api.params_from_hyper(h, iters=4100, eval_every=1), trace_cap=8)
+    assert not np.isnan(first["trace_best"].cpu().numpy()).any()
+    for _ in range(2):                                           # two resumed calls: each gets its own 3 evaluations
+        tb = torch.full((8,), float("nan"), dtype=torch.float64, device="cuda")
+        tn = torch.zeros(8, dtype=torch.int64, device="cuda")
+        ex = api.Extra()
+        ex.trace_best, ex.trace_ns, ex.trace_cap = tb.data_ptr(), tn.data_ptr(), 8
+        prm = api.params_from_hyper(h, iters=3, eval_every=1)
+        api._check(api.lib().gda_run(P._h, B, None, None, 0.0, api.C.byref(prm), first["x_bin"].data_ptr(), first["obj"].data_ptr(),
+                                     first["best_restart"].data_ptr(), api.C.byref(ex), torch.cuda.current_stream().cuda_stream))
+        torch.cuda.synchronize()
+        got = tb.cpu().numpy()
+        assert got[2] == first["obj"].min().item() and (np.diff(got[:3]) <= 0).all() and np.isnan(got[3:]).all()
+        assert (np.diff(tn.cpu().numpy()[:3]) > 0).all() and tn.cpu().numpy()[0] > first["trace_ns"].cpu().numpy()[7]
+    P.destroy()
+
+
 def test_two_handles_from_two_threads(api, oracle):
     """include/gda.h only forbids sharing ONE handle: two handles driven from two host threads at the same time
     (first-call kernel configuration included) give the results of the serial runs."""
