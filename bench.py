@@ -71,19 +71,53 @@ def algorithmic_work(w: wl.Workload):
 # clocks
 # ------------------------------------------------------------------------------------------------
 class ClockSampler:
+    """SM clock and clock-event reasons DURING a measurement.  NVML polled from a thread every ~2 ms (a secondary workload is
+    timed for a few hundred ms, so every record has well over 10 samples); `nvidia-smi -lms 20` if NVML cannot be loaded."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    PERIOD_S = 0.002
 
     def __init__(self, gpu_index: int):
         self.gpu, self.rows, self.proc = gpu_index, [], None
+        self.sm, self.smax, self.reasons, self.power = [], 0.0, set(), []
+        self._stop, self._thread, self.source = threading.Event(), None, None
+
+    def _nvml_loop(self, nv, handle):
+        bits = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown, "hw_thermal_slowdown": nv.nvmlClocksEventReasonHwThermalSlowdown,
+                "sw_thermal_slowdown": nv.nvmlClocksEventReasonSwThermalSlowdown, "sw_power_cap": nv.nvmlClocksEventReasonSwPowerCap}
+        while not self._stop.is_set():
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(handle, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(handle))
+                for name, bit in bits.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(handle) / 1e3)
+            except Exception:
+                pass
+            time.sleep(self.PERIOD_S)
 
     def start(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[self.gpu]) if vis and all(v.strip().isdigit() for v in vis.split(",")) else self.gpu
+            handle = nv.nvmlDeviceGetHandleByIndex(phys)
+            self.smax = float(nv.nvmlDeviceGetMaxClockInfo(handle, nv.NVML_CLOCK_SM))
+            self._thread = threading.Thread(target=self._nvml_loop, args=(nv, handle), daemon=True)
+            self._thread.start()
+            self.source = "nvml"
+            return
+        except Exception:
+            self._thread = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
                                           "-lms", "20", "-i", str(self.gpu)], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
+            self.source = "nvidia-smi"
         except Exception:
             self.proc = None
 
@@ -92,13 +126,16 @@ class ClockSampler:
             self.rows.append([c.strip() for c in line.split(",")])
 
     def stop(self):
+        if self._thread:
+            self._stop.set()
+            self._thread.join(timeout=1)
         if self.proc:
             self.proc.terminate()
             try:
                 self.proc.wait(timeout=2)
             except Exception:
                 self.proc.kill()
-        sm, smax, reasons = [], 0.0, set()
+        sm, smax, reasons = list(self.sm), self.smax, set(self.reasons)
         for r in self.rows:
             try:
                 sm.append(float(r[1]))
@@ -110,7 +147,8 @@ class ClockSampler:
                     reasons.add(name)
         busy = [v for v in sm if v > 0]
         return dict(sm_mhz=statistics.median(busy) if busy else None, sm_max_mhz=smax or None,
-                    reasons=sorted(reasons), samples=len(sm))
+                    reasons=sorted(reasons), samples=len(sm), source=self.source,
+                    power_w_max=max(self.power) if self.power else None)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -303,7 +341,10 @@ def roofline_block(w: wl.Workload, peaks, t_step_mean, t_step_median, t_eval):
     else:
         basis = (f"algorithmic bytes / step-kernel time against the measured HBM copy peak; the state ({state_bytes(w) / 1e6:.1f} MB) exceeds "
                  f"the 126 MB L2, so the step streams from HBM")
-    return {"bound": work["bound"], "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
+    extra = {}
+    if work["bound"] == "tensor":       # the timed loop is short (well under a second): the burst peak applies as well -- both are quoted
+        extra = {"peak_burst": peaks["bf16_tflops"], "frac_burst": achieved / peaks["bf16_tflops"]}
+    return {"bound": work["bound"], "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak, **extra,
             "traffic": rec.get("bytes"), "l2_to_sm_bytes": rec.get("l2_to_sm_bytes"), "traffic_source": rec.get("source"),
             "peak_source": peaks["source"], "kernel": rec.get("kernel", "step kernel (gradient + fused update)"),
             "us_per_launch": t_kernel * 1e6, "us_per_launch_median": t_kernel_med * 1e6,
@@ -342,9 +383,10 @@ class Session:
             dist.barrier()
             self.torch.cuda.synchronize(self.dev)
 
-    def measure(self, w: wl.Workload, K: int, W: int, peaks, full: bool):
+    def measure(self, w: wl.Workload, K: int, W: int, peaks, full: bool, min_seconds: float = 0.0):
         """K timed steps (flushed L2), the evaluation alone, clocks; with full=True also the whole run, the trace and
-        the end-to-end numbers through gda_run_host."""
+        the end-to-end numbers through gda_run_host.  min_seconds > 0 raises K (up to 400) until the timed steps alone keep
+        the GPU busy for that long, so that the clock record of a short workload has enough samples under load."""
         torch = self.torch
         from paper_2509_21064_b200 import api, multirank
         h, B, n = w.hyper, w.B, w.problem.n
@@ -354,13 +396,21 @@ class Session:
         stream, flush = self.stream, self.flush
         prm_step = api.params_from_hyper(h, iters=h.eval_every)
         prm0 = api.params_from_hyper(h, iters=0)
-        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
         res = {}
         with torch.cuda.stream(stream):
             out = P.run(x0, h.lambda0, prm_step)                          # warm-up: captures the graph, warms clocks
             for _ in range(W - 1):
                 P.resume(prm_step, out)
             self.sync_all()
+            if min_seconds > 0:
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                P.resume(prm_step, out)
+                e1.record(stream)
+                self.sync_all()
+                K = int(min(400, max(K, np.ceil(min_seconds * 1e3 / max(e0.elapsed_time(e1), 1e-3)))))
+            res["K"] = K
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
             sampler = ClockSampler(self.local_rank)
             sampler.start()
             out = P.run(x0, h.lambda0, prm0)
@@ -428,13 +478,39 @@ class Session:
         return res
 
 
+def workload_tag(w: wl.Workload) -> str:
+    return w.name + ("_pdbo_s" if getattr(w.hyper, "dual", 0) and "pdbo_s" not in w.name else "")
+
+
 def secondary_line(w: wl.Workload, r, K):
-    """One entry of `secondary`: the same measurement (K flushed steps, CUDA events) on another workload."""
+    """One entry of `secondary`: the same measurement (K flushed steps, CUDA events) on another workload.  Numbers only: the
+    prose of the roofline block (basis, sources) stays on the headline."""
     t = sum(r["step_ms"]) / 1e3
-    return {"workload": w.name, "kind": w.kind, "n": w.problem.n, "B": w.B, "steps": K,
+    roof = {k: v for k, v in r["roofline"].items() if not isinstance(v, str) or k in ("bound", "unit")}
+    if "on_chip" in roof:
+        roof["on_chip"] = {k: v for k, v in roof["on_chip"].items() if k != "basis"}
+    return {"workload": workload_tag(w), "kind": w.kind, "n": w.problem.n, "B": w.B, "steps": K,
             "value": w.B * w.hyper.eval_every * K / t, "unit": "restart-iters/s", "ms_per_step": 1e3 * t / K,
-            "ms_per_step_median": statistics.median(r["step_ms"]), "roofline": r["roofline"], "clocks": r["clocks"],
+            "ms_per_step_median": statistics.median(r["step_ms"]), "roofline": roof, "clocks": r["clocks"],
             "best_objective": r["best_flushed"], "gpu_launches": r["launches"]}
+
+
+def summary_entry(w: wl.Workload, r):
+    """[workload, B, us per GDA iteration (mean, median), bound, fraction of that bound's peak, SM MHz (median under load),
+    clock samples, clock-event reasons] -- one short list per workload; `summary` is the LAST key of the JSON line."""
+    roof, ck = r["roofline"], r["clocks"] or {}
+    bound, frac = roof["bound"], roof["frac"]
+    if "on_chip" in roof:                       # slab kernel: shared-memory bound
+        bound, frac = roof["on_chip"]["bound"], roof["on_chip"]["frac"]
+    elif "l2" in roof:                          # L2-resident state: the measured L2 -> SM ceiling is the honest one
+        bound, frac = "l2", roof["l2"]["frac"]
+    e = [workload_tag(w), w.B, round(roof["us_per_launch"], 2), round(roof["us_per_launch_median"], 2), bound, round(frac, 3),
+         ck.get("sm_mhz"), ck.get("samples"), ck.get("reasons")]
+    if roof["bound"] == "tensor":
+        e += [{"frac_sustained": round(roof["frac"], 3), "frac_burst": round(roof["frac_burst"], 3)}]
+    elif bound != "hbm":
+        e += [{"hbm_algorithmic_frac": round(roof["frac"], 3)}]
+    return e
 
 
 def run_ours(args, w: wl.Workload):
@@ -471,16 +547,18 @@ def run_ours(args, w: wl.Workload):
     P.destroy()
 
     # ---- secondary workloads, same process, same method (default headline run on one GPU only) ----
-    secondary = []
+    secondary, summary = [], []
     if world == 1 and not args.no_secondary and args.config == HEADLINE_CONFIG and not (args.mis or args.maxkcut or args.pdbo_s or args.B):
         Ks = max(5, min(K, args.secondary_steps))
         # the configs of BASELINE.json, config 3's graph at the paper's largest batch (HBM-streaming), PDBO-s, and two of the
         # paper's own small-batch settings (Max-k-SAT and MIS run B = 10: Table 6, 1040-1048 Table 13)
-        for sw in (wl.config(3, B=1024), wl.config(4), wl.config(5), wl.config(2), wl.config(1), wl.pdbo_s_variant(wl.config(3)),
-                   wl.pdbo_s_variant(wl.config(2)), wl.config(5, B=10), wl.mis(10000, 100, B=10)):
-            rs = S.measure(sw, Ks, 3, peaks, full=False)
+        # (ordered so that the BASELINE.json configs close the line: a log tail that is cut short still holds them)
+        for sw in (wl.mis(10000, 100, B=10), wl.config(5, B=10), wl.pdbo_s_variant(wl.config(2)), wl.pdbo_s_variant(wl.config(3)),
+                   wl.config(1), wl.config(3, B=1024), wl.config(2), wl.config(5), wl.config(4)):
+            rs = S.measure(sw, Ks, 3, peaks, full=False, min_seconds=args.secondary_seconds)
             rs["P"].destroy()
-            secondary.append(secondary_line(sw, rs, Ks))
+            secondary.append(secondary_line(sw, rs, rs["K"]))
+            summary.append(summary_entry(sw, rs))
 
     iters_per_step = h.eval_every
     units = world * B * iters_per_step * K
@@ -522,7 +600,10 @@ def run_ours(args, w: wl.Workload):
             line["secondary"] = secondary
         if cpu:
             line["cpu_baseline"] = cpu
-        print(json.dumps(line))
+        # LAST key, compact: one entry per workload, the headline closing the list
+        line["summary_fields"] = "workload,B,us_per_iter_mean,us_per_iter_median,bound,frac,sm_mhz_median,clock_samples,reasons[,more]"
+        line["summary"] = summary + [summary_entry(w, r)]
+        print(json.dumps(line, separators=(",", ":")))
     if world > 1:
         dist.destroy_process_group()
 
@@ -537,7 +618,9 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the secondary workloads of the default run")
-    ap.add_argument("--secondary-steps", type=int, default=20, help="timed steps per secondary workload")
+    ap.add_argument("--secondary-steps", type=int, default=20, help="timed steps per secondary workload (at least)")
+    ap.add_argument("--secondary-seconds", type=float, default=0.25,
+                    help="a secondary workload is timed for at least this long (more steps, up to 400), for its clock record")
     ap.add_argument("--B", type=int, default=None)
     ap.add_argument("--pdbo-s", action="store_true", help="run the PDBO-s ablation (one multiplier per restart, PAPER.md:630-648)")
     ap.add_argument("--maxkcut", default=None, metavar="N,M,K", help="instead of --config: Max-K-Cut on G(N, M) (PAPER.md:784-828)")
