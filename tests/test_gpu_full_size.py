@@ -151,3 +151,109 @@ def test_mis_on_a_3_regular_graph_against_the_papers_table_13(api):
     assert best > val[("PIGNN", 10000, 3)] and best > val[("Gurobi", 10000, 3)]
     assert best >= 0.97 * val[("PDBO", 10000, 3)]
     P.destroy()
+
+
+# ------------------------------------------------------------------------------------------------
+# the "next" rows of SURVEY.md 8(f) at the sizes that are timed (round 2 tested them at toy sizes only)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("idx", [3, 5])
+def test_pdbo_s_at_full_size_on_sampled_restarts(api, oracle, idx):
+    """PDBO-s (reading R14) on configs 3 and 5 at full size: the streaming sparse path has 2 500 blocks
+    adding into 32 accumulator ways per restart and walks 20 000 rows in adjacency-grouped order; the MaxSAT path reduces
+    1 250 partial rows.  One step on sampled columns against the oracle (a column's multiplier needs the sum of g over ALL
+    its n variables), then the launch configuration bench.py times with exact objectives of the returned points."""
+    w = wl.pdbo_s_variant(wl.config(idx))
+    Pw, h, B, n = w.problem, w.hyper, w.B, w.problem.n
+    OP = oracle_problem(Pw)
+    P = api.create_from_workload(Pw)
+    X0 = wl.x0_uniform(n, B, w.x0_seed)
+    x0 = torch.from_numpy(X0).cuda()
+    cols = np.array([0, 1, B // 3, B // 2 + 1, B - 2, B - 1], dtype=np.int32)
+    csel = torch.from_numpy(cols).long().cuda()
+    mu0 = np.linspace(0.5 * h.lambda0, h.lambda0, B).astype(np.float32)           # a different multiplier per restart
+    for steps in (1, 3):                                                          # 3: the pipelined multiplier update has run twice
+        r = P.run(x0, torch.from_numpy(mu0).cuda(), api.params_from_hyper(h, iters=steps, eval_every=steps), want_final=True)
+        ref = oracle.run(OP, X0[:, cols], mu0[cols], col_ids=cols, nthreads=4, **okw(h, iters=steps, eval_every=steps))
+        assert np.abs(r["x"][:, csel].cpu().numpy() - ref["x"]).max() <= 1e-5 * steps
+        mu_tol = 1e-5 * np.maximum(1.0, np.abs(ref["y"])) + 1e-6 * f32(h.beta) * n * steps
+        assert (np.abs(r["lam"][csel].cpu().numpy() - ref["y"]) <= mu_tol).all()
+    r = P.run(x0, h.lambda0, api.params_from_hyper(h, iters=h.eval_every), want_final=True)
+    P.resume(api.params_from_hyper(h, iters=h.eval_every), r)
+    torch.cuda.synchronize()
+    obj = r["obj"].cpu().numpy()
+    assert np.array_equal(obj[cols], oracle.F_binary(OP, r["x_bin"][:, csel].cpu().numpy()))
+    assert int(r["best_restart"].item()) == int(np.argmin(obj))
+    assert bool(((r["x"] >= 0) & (r["x"] <= 1)).all()) and bool((r["lam"] <= h.lambda0 + 1e-6).all())   # mu is non-increasing (g <= 0)
+    P.destroy()
+
+
+def test_max3cut_at_the_timed_size_on_sampled_restarts(api):
+    """Max-3-Cut on G(20 000, 40 000) at B = 128, the shape profiles/r1_kcut_n20000.md times: one step of
+    the logits on sampled columns against the k-cut oracle, exact objectives of the returned labels."""
+    from oracle import kcut
+    w = wl.maxkcut(20000, 40000, 3, B=128)
+    Pw, h, B, n, k = w.problem, w.hyper, w.B, w.problem.n, w.problem.k
+    OK = kcut.Problem(n, k, Pw.rowptr, Pw.col, Pw.val.astype(np.float64))
+    P = api.create_from_workload(Pw)
+    Z0 = wl.z0_uniform(k, n, B, w.x0_seed)
+    z0 = torch.from_numpy(Z0).cuda()
+    cols = np.array([0, 1, B // 3, B // 2 + 1, B - 2, B - 1], dtype=np.int32)
+    csel = torch.from_numpy(cols).long().cuda()
+    kw = dict(alpha=f32(h.alpha), beta=f32(h.beta), gfun=h.gfun, log_eps=f32(h.log_eps))
+    r1 = P.run(z0, h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+    ref = kcut.run(OK, np.ascontiguousarray(Z0[:, :, cols]), f32(h.lambda0), iters=1, eval_every=1, **kw)
+    zg, yg = r1["x"][:, :, csel].cpu().numpy(), r1["lam"][:, csel].cpu().numpy()
+    assert (np.abs(zg - ref["z"]) <= 1e-5 * np.maximum(1.0, np.abs(ref["z"]))).all()
+    assert (np.abs(yg - ref["y"]) <= 1e-5 * np.maximum(1.0, np.abs(ref["y"]))).all()
+    r = P.run(z0, h.lambda0, api.params_from_hyper(h, iters=200, eval_every=100))
+    obj, lab = r["obj"].cpu().numpy(), r["x_bin"][:, csel].cpu().numpy()
+    assert lab.max() < k and np.array_equal(obj[cols], kcut.objective(OK, lab))
+    assert int(r["best_restart"].item()) == int(np.argmin(obj))
+    total = float(Pw.val.sum())
+    assert ((total - obj) / 2 > 0.6 * 40000).all()                # sanity only: a random 3-partition already cuts 2/3 of the edges
+    P.destroy()
+
+
+def test_mis_at_the_papers_largest_setting(api, oracle):
+    """MIS as a QUBO on a random 100-regular graph with 5 * 10^4 vertices at B = 10, the largest row of Table 13
+    (PAPER.md:1030-1048): one step against the oracle, exact objective, cardinality and the feasibility rule by the edge list."""
+    w = wl.mis(50000, 100, B=10, iters=400)
+    Pw, h, B, n = w.problem, w.hyper, w.B, w.problem.n
+    OP = oracle_problem(Pw)
+    P = api.create_from_workload(Pw)
+    X0 = wl.x0_uniform(n, B, w.x0_seed)
+    r1 = P.run(torch.from_numpy(X0).cuda(), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+    ref = oracle.run(OP, X0, f32(h.lambda0), nthreads=8, **okw(h, iters=1, eval_every=1))
+    assert np.abs(r1["x"].cpu().numpy() - ref["x"]).max() <= 1e-5
+    r = P.run(torch.from_numpy(X0).cuda(), h.lambda0, api.params_from_hyper(h), want_ones=True)
+    obj, xb, ones = r["obj"].cpu().numpy(), r["x_bin"].cpu().numpy(), r["ones"].cpu().numpy()
+    E = Pw.edges
+    inside = (xb[E[:, 0]] & xb[E[:, 1]]).sum(axis=0)
+    assert np.array_equal(obj, oracle.F_binary(OP, xb)) and np.array_equal(ones, xb.sum(axis=0))
+    assert np.array_equal(obj, -ones + 4.0 * inside) and np.array_equal(obj == -ones, inside == 0)
+    assert int(r["best_restart"].item()) == int(np.argmin(obj))
+    P.destroy()
+
+
+def test_evaluation_schedule_gives_the_oracles_objectives_on_a_short_run(api, oracle):
+    """Reading R5 itself: evaluations after every `eval_every` steps AND after the last one, best-so-far per restart.  On a
+    short integral run (config 1, delta = 0, 60 steps, eval_every = 7: evaluations at t = 7, 14, ..., 56 and 60) the fp32 and
+    fp64 trajectories still round to the same points, so the GPU's per-restart best objectives must EQUAL the oracle's (a
+    schedule that skipped the ragged last evaluation, or kept the last instead of the best value, would differ)."""
+    # config 3 (scaled): the convex start pulls every coordinate towards 1/2 during the first few hundred steps (DESIGN.md R3), so
+    # at t <= 60 more coordinates sit within rounding error of the threshold and a few restarts round differently: 90 % there
+    for idx, scale, share in ((1, 1.0, 0.99), (3, 0.05, 0.90)):
+        w = wl.config(idx, n_scale=scale)
+        Pw, h, B = w.problem, w.hyper, w.B
+        OP = oracle_problem(Pw)
+        P = api.create_from_workload(Pw)
+        X0 = wl.x0_uniform(Pw.n, B, w.x0_seed)
+        r = P.run(torch.from_numpy(X0).cuda(), h.lambda0, api.params_from_hyper(h, iters=60, eval_every=7, delta=0.0), trace_cap=16)
+        ref = oracle.run(OP, X0, f32(h.lambda0), **okw(h, iters=60, eval_every=7, delta=0.0))
+        obj = r["obj"].cpu().numpy()
+        assert (obj == ref["obj"]).mean() >= share, (w.name, (obj == ref["obj"]).mean())
+        assert np.array_equal(obj, oracle.F_binary(OP, r["x_bin"].cpu().numpy()))
+        tb = r["trace_best"].cpu().numpy()
+        assert not np.isnan(tb[:9]).any() and np.isnan(tb[9:]).all()          # 8 full chunks + the ragged last one = 9 evaluations
+        assert tb[8] == obj.min() and (np.diff(tb[:9]) <= 0).all()
+        P.destroy()
