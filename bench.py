@@ -319,6 +319,25 @@ def ncu_record(w: wl.Workload) -> dict:
     return rec if rec.get("B", w.B) == w.B else {}          # a capture at another batch size says nothing about this one
 
 
+def l2_block(w: wl.Workload, rec: dict, t_kernel: float):
+    """L2 roofline of a step kernel whose state is L2-resident: the bytes ncu saw cross the L2 <-> SM boundary per launch
+    (profiles/ncu_traffic.json) / the kernel's duration, against the measured ceiling in profiles/measured_l2.json (the
+    probe and its access shapes: profiles/l2_peak.md).  `shape_floor` is a kernel with this workload's access shape and no
+    arithmetic, timed by the same probe: frac_of_shape_floor = its time / this kernel's time."""
+    f = ROOT / "profiles" / "measured_l2.json"
+    if not f.exists() or not rec.get("l2_to_sm_bytes"):
+        return None
+    m = json.loads(f.read_text())
+    nbytes = rec["l2_to_sm_bytes"] + rec.get("sm_to_l2_bytes", 0)
+    out = {"bytes_per_launch": nbytes, "achieved": nbytes / t_kernel / 1e12, "peak": m["l2_peak_tbps"], "unit": "TB/s",
+           "frac": nbytes / t_kernel / 1e12 / m["l2_peak_tbps"], "peak_source": "profiles/measured_l2.json"}
+    floor = m.get("shape_floor", {}).get(f"{w.name}_B{w.B}")
+    if floor:
+        out["shape_floor_us"] = floor["us"]
+        out["frac_of_shape_floor"] = floor["us"] * 1e-6 / t_kernel
+    return out
+
+
 def roofline_block(w: wl.Workload, peaks, t_step_mean, t_step_median, t_eval):
     """roofline of the step kernel: algorithmic work per launch / its average duration, the duration being
     (one captured chunk - one evaluation) / eval_every from CUDA events (it includes the graph's launch gaps)."""
@@ -342,6 +361,10 @@ def roofline_block(w: wl.Workload, peaks, t_step_mean, t_step_median, t_eval):
         basis = (f"algorithmic bytes / step-kernel time against the measured HBM copy peak; the state ({state_bytes(w) / 1e6:.1f} MB) exceeds "
                  f"the 126 MB L2, so the step streams from HBM")
     extra = {}
+    if work["bound"] == "hbm" and resident and not getattr(w.hyper, "dual", 0):
+        l2 = l2_block(w, rec, t_kernel)
+        if l2:
+            extra["l2"] = l2
     if work["bound"] == "tensor":       # the timed loop is short (well under a second): the burst peak applies as well -- both are quoted
         extra = {"peak_burst": peaks["bf16_tflops"], "frac_burst": achieved / peaks["bf16_tflops"]}
     return {"bound": work["bound"], "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak, **extra,
