@@ -222,6 +222,25 @@ gda_status gda_lagrangian(gda_problem* p, int32_t B, const float* x, const float
 gda_status gda_score_qubo_csr_static(int32_t n, const int32_t* rowptr, const int32_t* col, const float* val,
                                      const float* c, int32_t B, const float* x, double* obj, void* stream);
 
+/* ---- launch options, per handle -----------------------------------------------------------------------
+ * The library picks its launch path from the sizes (cost models in csrc/); these switches override a choice for ONE handle,
+ * for tests and A/B timing.  No result changes beyond rounding order (the tests compare the paths bit for bit where the
+ * arithmetic is the same).  There is no process-wide state: no environment variable is read by the library.  A change takes
+ * effect at the next call on the handle (the graphs it has captured are dropped); like every call on a handle it must not
+ * run concurrently with another call on the same handle.  INVALID_ARG: null handle, unknown key, value out of range. */
+typedef enum {
+    GDA_OPT_SPARSE_PATH = 0,    /* sparse QUBO: 0 cost model (default), 1 slab kernel (state in shared memory, whole chunk in one
+                                   launch) whenever the instance fits it, 2 streaming kernels (one launch per step)          */
+    GDA_OPT_SPLIT_ALL_ROWS = 1, /* sparse QUBO, Max-k-Cut: -1 by the rule (default), 0 a warp per row, 1 every row split      */
+    GDA_OPT_NARROW_SPLIT = 2,   /* sparse QUBO, B <= 64: 1 lane groups share long rows (default), 0 one group per row         */
+    GDA_OPT_MAXSAT_NARROW = 3,  /* MaxSAT, B <= 64: 1 lane groups share the slots of a variable (default), 0 off               */
+    GDA_OPT_DENSE_SHAPE = 4,    /* dense QUBO: -1 the cluster shape the cost model picks (default); 0 one CTA per tile, 1 CTA
+                                   pairs, 2 clusters of 2 pairs, 3 clusters of 4 pairs -- at most this shape, sizes permitting */
+    GDA_OPT_GRAPHS = 5,         /* 1 replay CUDA graphs of whole chunks (default), 0 enqueue the same kernels directly         */
+    GDA_OPT_ROW_GROUPING = 6    /* sparse PDBO-s step: 1 rows walked grouped by adjacency (default), 0 in index order          */
+} gda_option;
+gda_status gda_set_option(gda_problem* p, int32_t key, int32_t value);
+
 /* ---- queries ------------------------------------------------------------------------------------------ */
 typedef struct {
     int32_t kind;        /* 0 sparse QUBO, 1 dense QUBO, 2 MaxSAT, 3 Max-k-Cut                          */

@@ -22,6 +22,9 @@ STATUS = {0: "GDA_OK", 1: "GDA_ERR_INVALID_ARG", 2: "GDA_ERR_ALLOC", 3: "GDA_ERR
 G_QUADRATIC, G_ENTROPY = 0, 1
 DUAL_PER_VARIABLE, DUAL_SCALAR = 0, 1
 DENSE_BF16 = 1
+# gda_option keys of gda_set_option (per-handle launch options)
+OPT_SPARSE_PATH, OPT_SPLIT_ALL_ROWS, OPT_NARROW_SPLIT, OPT_MAXSAT_NARROW, OPT_DENSE_SHAPE, OPT_GRAPHS, OPT_ROW_GROUPING = range(7)
+SPARSE_PATH = {"auto": 0, "slab": 1, "stream": 2}
 
 
 class GdaError(RuntimeError):
@@ -48,7 +51,7 @@ class Info(C.Structure):
 
 
 EXPORTS = ["gda_create_qubo_csr", "gda_create_qubo_dense", "gda_create_maxsat", "gda_create_maxkcut", "gda_destroy", "gda_run",
-           "gda_run_host", "gda_grad", "gda_score", "gda_lagrangian", "gda_score_qubo_csr_static", "gda_get_info",
+           "gda_run_host", "gda_grad", "gda_score", "gda_lagrangian", "gda_score_qubo_csr_static", "gda_set_option", "gda_get_info",
            "gda_last_error", "gda_version"]
 
 
@@ -73,6 +76,7 @@ def lib():
         L.gda_score.argtypes = [vp, i32, vp, vp, vp]
         L.gda_lagrangian.argtypes = [vp, i32, vp, vp, f32, i32, f32, vp, vp]
         L.gda_score_qubo_csr_static.argtypes = [i32, vp, vp, vp, vp, i32, vp, vp, vp]
+        L.gda_set_option.argtypes = [vp, i32, i32]
         L.gda_get_info.argtypes = [vp, C.POINTER(Info)]
         L.gda_last_error.restype = C.c_char_p
         L.gda_version.restype = C.c_char_p
@@ -137,6 +141,11 @@ class Problem:
         h = C.c_void_p()
         _check(lib().gda_create_maxkcut(n, k, _hp(rowptr), _hp(col), _hp(val), C.byref(h)))
         return Problem(h.value, n, k)
+
+    def set_option(self, key: int, value: int) -> "Problem":
+        """gda_set_option: a launch option of THIS handle (OPT_* keys above); takes effect at the next call."""
+        _check(lib().gda_set_option(self._h, key, value))
+        return self
 
     def destroy(self):
         if self._h:

@@ -141,11 +141,6 @@ static bool locality_order(int n, const std::vector<int32_t>& rowptr, const std:
     return true;
 }
 
-static bool locality_disabled() {
-    const char* e = getenv("GDA_SPARSE_LOCALITY");
-    return e && e[0] == '0';
-}
-
 extern "C" gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, const int32_t* col, const float* val,
                                           const float* c, gda_problem** out) {
     if (out) *out = nullptr;
@@ -222,7 +217,7 @@ extern "C" gda_status gda_create_qubo_csr(int32_t n, const int32_t* rowptr, cons
         if (st == GDA_OK) st = upload(&p->d_light_rows, light);
     }
     std::vector<int32_t> local;
-    if (st == GDA_OK && !locality_disabled() && locality_order(n, h_rowptr, h_col, light, &local)) st = upload(&p->d_local_rows, local);
+    if (st == GDA_OK && locality_order(n, h_rowptr, h_col, light, &local)) st = upload(&p->d_local_rows, local);
     if (st == GDA_OK) st = sparse_build_slab(p, h_rowptr, h_col, h_val2);
     if (st == GDA_OK && (int64_t)h_col.size() <= 8 * (int64_t)n) {
         // packed records for rows of degree <= 8 (one 64-byte load replaces rowptr -> col/val): 8 columns then 8
@@ -626,14 +621,9 @@ static gda_params canonical_params(const gda_problem* p, const gda_params& in) {
     return c;
 }
 
-static bool graphs_disabled() {
-    const char* e = getenv("GDA_NO_GRAPH");
-    return e && e[0] && e[0] != '0';
-}
-
 static gda_status launch_chunk(gda_problem* p, int32_t B, int32_t len, int32_t parity, const gda_params& prm,
                                cudaStream_t s) {
-    if (graphs_disabled() || len == 0) {
+    if (!p->opt_graphs || len == 0) {                         // GDA_OPT_GRAPHS
         return enqueue_chunk(p, B, len, parity, prm, s, &p->last_launches, &p->last_step_launches);
     }
     GraphKey key;
@@ -869,6 +859,33 @@ extern "C" gda_status gda_score(gda_problem* p, int32_t B, const float* x, doubl
     }
     GDA_TRY(score_reduce(p, B, ws.ld, ws.partial, n_part, obj, s));
     return join_stream(p, user, s);
+}
+
+// Per-handle launch options (tests, A/B timing).  Every choice below is read when a chunk is enqueued, i.e. also when a
+// graph is captured, so a change drops the handle's cached graphs: the next chunk is captured with the new choice.
+extern "C" gda_status gda_set_option(gda_problem* p, int32_t key, int32_t value) {
+    GDA_REQUIRE(p != nullptr, "gda_set_option: null handle");
+    int32_t* slot = nullptr;
+    int32_t lo = 0, hi = 1;
+    switch (key) {
+        case GDA_OPT_SPARSE_PATH: slot = &p->slab_mode; lo = 0; hi = 2; break;
+        case GDA_OPT_SPLIT_ALL_ROWS: slot = &p->opt_split_all; lo = -1; hi = 1; break;
+        case GDA_OPT_NARROW_SPLIT: slot = &p->opt_narrow_split; break;
+        case GDA_OPT_MAXSAT_NARROW: slot = &p->opt_maxsat_narrow; break;
+        case GDA_OPT_DENSE_SHAPE: slot = &p->opt_dense_shape; lo = -1; hi = 3; break;
+        case GDA_OPT_GRAPHS: slot = &p->opt_graphs; break;
+        case GDA_OPT_ROW_GROUPING: slot = &p->opt_row_grouping; break;
+        default: break;
+    }
+    GDA_REQUIRE(slot != nullptr, "gda_set_option: unknown option %d", key);
+    GDA_REQUIRE(value >= lo && value <= hi, "gda_set_option: option %d takes values in [%d, %d] (got %d)", key, lo, hi, value);
+    if (key == GDA_OPT_SPARSE_PATH) value = value == 2 ? -1 : value;      // stored as 1 slab / -1 stream / 0 cost model
+    if (*slot != value) {
+        *slot = value;
+        DeviceGuard guard(p->device);
+        drop_graphs(p);
+    }
+    return GDA_OK;
 }
 
 extern "C" gda_status gda_get_info(const gda_problem* p, gda_info* info) {

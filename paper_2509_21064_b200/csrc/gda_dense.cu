@@ -586,7 +586,6 @@ struct DenseHost {
     int32_t z_B = 0;
     // co-resident clusters per kernel variant (1 CTA per SM), see configure_variant
     int max_clusters[4 * 2 * 4] = {};
-    int forced_shape = -1;              // GDA_DENSE_SHAPE (read at create)
 };
 
 // The launch shapes: single CTAs, pairs, two pairs (1 x 2) and four pairs (2 x 2) per cluster.
@@ -655,12 +654,12 @@ gda_status launch_variant(gda_problem* p, const CUtensorMap& ta, const CUtensorM
     return GDA_OK;
 }
 
-// GDA_DENSE_SHAPE=0..3 forces a launch shape the sizes allow (tests, A/B timing); default: the largest cluster that fits
+// GDA_OPT_DENSE_SHAPE = 0..3 forces a launch shape the sizes allow (tests, A/B timing); default: the largest cluster that fits
 template <int MODE, int GFUN>
 gda_status launch_gemm(gda_problem* p, const CUtensorMap& ta, const CUtensorMap& tzo, const DenseArgs& a, cudaStream_t s) {
     DenseHost* h = static_cast<DenseHost*>(p->tmap_Q);
     int shape = a.B % (BM * 2) != 0 ? 0 : a.n % (BN * 2) != 0 ? 1 : a.B % (BM * 4) != 0 ? 2 : 3;
-    if (shape == 3 && h->forced_shape < 0) {
+    if (shape == 3 && p->opt_dense_shape < 0) {
         // Clusters of 8 move a third less operand data per tile (measured on config 4: 30 us per round against 34 us)
         // but only 15 of them are co-resident on a B200 (120 SMs) against 33 clusters of 4: take them only when the
         // round count does not eat the gain (config 4: 64 units -> 5 rounds x 30 us against 4 x 34 us: clusters of 4).
@@ -669,7 +668,7 @@ gda_status launch_gemm(gda_problem* p, const CUtensorMap& ta, const CUtensorMap&
         const long rounds8 = (units8 + mc[3] - 1) / mc[3], rounds4 = (units4 + mc[2] - 1) / mc[2];
         if (15 * rounds8 >= 17 * rounds4) shape = 2;
     }
-    if (h->forced_shape >= 0 && h->forced_shape < shape) shape = h->forced_shape;
+    if (p->opt_dense_shape >= 0 && p->opt_dense_shape < shape) shape = p->opt_dense_shape;
     switch (shape) {
         case 0: return launch_variant<MODE, GFUN, 1, 1, 1>(p, ta, h->tmap_q, tzo, a, s);
         case 1: return launch_variant<MODE, GFUN, 2, 1, 1>(p, ta, h->tmap_q, tzo, a, s);
@@ -725,7 +724,6 @@ gda_status dense_prepare(gda_problem* p, const float* Q, const float* c) {
     GDA_CUDA_TRY(cudaMemcpy(p->d_cprime, cp.data(), np * sizeof(float), cudaMemcpyHostToDevice));
     DenseHost* h = new DenseHost();
     p->tmap_Q = h;
-    if (const char* e = getenv("GDA_DENSE_SHAPE")) if (e[0] >= '0' && e[0] <= '3') h->forced_shape = e[0] - '0';
     GDA_TRY(configure_all(p));
     return make_tmap(&h->tmap_q, p->d_Qbf, (uint64_t)np, (uint64_t)np, BBOX);
 }

@@ -146,7 +146,14 @@ struct gda_problem {
     int2* d_slab_ent = nullptr; int32_t* d_slab_goff = nullptr; int32_t* d_slab_grow = nullptr;
     int32_t slab_groups = 0, slab_slots = 0; int64_t slab_real = 0;
     uint16_t* d_slab_ent16 = nullptr; uint32_t slab_cbits = 0; int32_t slab_passes = 0;   // compact form (one |val2|), else null
-    int32_t slab_mode = 0;               // GDA_SPARSE_PATH at create: 1 "slab" always, -1 "stream" never, 0 by the cost model
+    int32_t slab_mode = 0;               // GDA_OPT_SPARSE_PATH: 1 "slab" always, -1 "stream" never, 0 by the cost model
+    // the other per-handle options of gda_set_option (include/gda.h); a change drops the cached graphs
+    int32_t opt_split_all = -1;          // GDA_OPT_SPLIT_ALL_ROWS: -1 by the rule, 0 rows whole, 1 every row through the row-split kernel
+    int32_t opt_narrow_split = 1;        // GDA_OPT_NARROW_SPLIT: lane groups share long rows in the narrow sparse step
+    int32_t opt_maxsat_narrow = 1;       // GDA_OPT_MAXSAT_NARROW: slot groups in the MaxSAT step for B <= 64
+    int32_t opt_dense_shape = -1;        // GDA_OPT_DENSE_SHAPE: -1 the largest cluster shape that pays, 0..3 at most this shape
+    int32_t opt_graphs = 1;              // GDA_OPT_GRAPHS: replay captured chunks (1) or enqueue the kernels directly (0)
+    int32_t opt_row_grouping = 1;        // GDA_OPT_ROW_GROUPING: PDBO-s sparse step walks the rows grouped by adjacency
     int32_t* d_ell = nullptr;            // [n][16] packed low-degree rows: 8 cols + 8 val2 (see gda_sparse.cu); nullptr = not built
     // dense QUBO: Q_off in bf16 [n][n] (zero diagonal), r0 = Q_off 1 (row sums) for the centred operand
     __nv_bfloat16* d_Qbf = nullptr; float* d_rowsum = nullptr;

@@ -250,8 +250,7 @@ template <int GFUN>
 void launch_k(gda_problem* p, int32_t B, dim3 grid, const float* x, float* z, float* y, float* xn, const UpdParams& up,
               cudaStream_t s) {
     // few warps that each walk a long row: split the rows (the rule of the sparse QUBO path, gda_sparse.cu)
-    const char* e = getenv("GDA_SPARSE_SPLIT_ALL");
-    const bool split = e && e[0] ? e[0] == '1'
+    const bool split = p->opt_split_all >= 0 ? p->opt_split_all == 1      // GDA_OPT_SPLIT_ALL_ROWS
                                  : (int64_t)p->n * grid.y < (int64_t)p->num_sms * 12 && p->nnz >= 16 * (int64_t)p->n;
 #define KCUT_CASE(K) case K: if (split) kcut_step_kernel<GFUN, K, true><<<dim3((unsigned)p->n, grid.y), 32 * SPLIT_WARPS, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, x, z, y, xn, up); \
                              else kcut_step_kernel<GFUN, K><<<grid, 32 * SW, 0, s>>>(p->n, B, p->d_rowptr, p->d_col, p->d_val2, x, z, y, xn, up); break;

@@ -235,11 +235,6 @@ maxsat_value(int m, int B, int clauses_per_block, const int32_t* __restrict__ cp
         }
 }
 
-static bool maxsat_narrow_disabled() {
-    const char* e = getenv("GDA_MAXSAT_NARROW");
-    return e && e[0] == '0';
-}
-
 template <int GFUN, int MODE, bool DUAL>
 void launch_kw(gda_problem* p, int32_t B, dim3 grid, const float* x, float* y, float* xn,
                const UpdParams& up, const ScalarDual& sd, const RunState* st, uint32_t t_off, cudaStream_t s) {
@@ -252,7 +247,7 @@ void launch_kw(gda_problem* p, int32_t B, dim3 grid, const float* x, float* y, f
     // records hold ENC_PAD when clauses are shorter than kmax -- and ALWAYS when kmax == 1 (kw is then 1 with no other literal)
     const bool pad = p->kmin != p->kmax || p->kmax == 1;
     // few restarts: slot groups (gather_var); B <= 64 is one 128-restart chunk, so grid.y == 1
-    const bool narrow = MODE == 0 && !DUAL && B <= 64 && p->kw <= 4 && !maxsat_narrow_disabled();
+    const bool narrow = MODE == 0 && !DUAL && B <= 64 && p->kw <= 4 && p->opt_maxsat_narrow;   // GDA_OPT_MAXSAT_NARROW
     int lanes = 1;
     while (4 * lanes < B) lanes <<= 1;
     switch (p->kw) {

@@ -28,15 +28,13 @@ constexpr int THREADS = WARPS * 32;
 // Config 2's graph (n = 800, degree 48) through the streaming kernels, us per step: B = 100 8.66 with a warp per row, 4.38 with
 // the rows split; B = 256 8.72 / 6.58; B = 512 9.10 / 11.21; B = 1024 12.08 / 20.37 (the slab kernel: 8.4 at any B).
 static bool split_all_rows(const gda_problem* p, int32_t B) {
-    const char* e = getenv("GDA_SPARSE_SPLIT_ALL");
-    if (e && e[0]) return e[0] == '1';
+    if (p->opt_split_all >= 0) return p->opt_split_all == 1;      // GDA_OPT_SPLIT_ALL_ROWS
     const int64_t chunks = (B / 4 + 31) / 32;
     return B > 32 && (int64_t)p->n * chunks < (int64_t)p->num_sms * 12 && p->nnz >= 16 * (int64_t)p->n;   // B <= 32: the narrow kernel splits rows itself
 }
 // narrow kernel (B <= 64): lane groups per row, as many as give every group about two batches of four entries of an average row
 static int narrow_split_log2(const gda_problem* p, int32_t B) {
-    const char* e = getenv("GDA_NARROW_SPLIT");
-    if (e && e[0] == '0') return 0;
+    if (!p->opt_narrow_split) return 0;                           // GDA_OPT_NARROW_SPLIT
     int G = 1, split_log2 = 0;
     while (4 * G < B) G <<= 1;
     while ((G << (split_log2 + 1)) <= 32 && (8 << (split_log2 + 1)) <= p->nnz / std::max(p->n, 1)) ++split_log2;
@@ -753,7 +751,7 @@ gda_status launch_step(gda_problem* p, int32_t B, const float* x, float* y, floa
     const bool pf = MODE == 0 && !DUAL && 12.0 * (double)p->n * (double)B > 0.8 * (double)p->l2_bytes;   // the streaming switch (see spmm_step_warp)
     if (n_light > 0) {
         const dim3 grid((unsigned)light_blocks, (unsigned)chunks);
-        const int32_t* row_list = (DUAL && p->d_local_rows) ? p->d_local_rows : p->d_light_rows;   // PDBO-s: rows grouped by adjacency
+        const int32_t* row_list = (DUAL && p->d_local_rows && p->opt_row_grouping) ? p->d_local_rows : p->d_light_rows;   // PDBO-s: rows grouped by adjacency
 #define GDA_SP_ARGS n_light, row_list, B, p->d_rowptr, p->d_col, p->d_val2, p->d_ell, p->d_cprime, x, y, xn, up, sd, st, t_off
 #define GDA_SP_PF(G, E) do { if (pf) spmm_step_warp<G, MODE, E, DUAL, (MODE == 0 && !DUAL)><<<grid, WTHREADS, 0, s>>>(GDA_SP_ARGS); \
                              else spmm_step_warp<G, MODE, E, DUAL, false><<<grid, WTHREADS, 0, s>>>(GDA_SP_ARGS); } while (0)
@@ -1026,7 +1024,6 @@ gda_status sparse_build_slab(gda_problem* p, const std::vector<int32_t>& rowptr,
     GDA_CUDA_TRY(cudaMemcpy(p->d_slab_goff, goff.data(), goff.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
     GDA_CUDA_TRY(cudaMalloc((void**)&p->d_slab_grow, grow.size() * sizeof(int32_t)));
     GDA_CUDA_TRY(cudaMemcpy(p->d_slab_grow, grow.data(), grow.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
-    if (const char* e = getenv("GDA_SPARSE_PATH")) p->slab_mode = !strcmp(e, "slab") ? 1 : !strcmp(e, "stream") ? -1 : 0;
     return GDA_OK;
 }
 

@@ -26,14 +26,11 @@ def hyper_kwargs(h, **over):
 
 def create_problem(api, w_or_problem, sparse_path=None):
     """gda_create_* for a workload (or a bare problem container).  `sparse_path` = "slab" | "stream" (or
-    workload.extra["sparse_path"]) forces the sparse launch path through GDA_SPARSE_PATH, which the library reads at
-    create; None leaves the choice to its cost model."""
-    import os
+    workload.extra["sparse_path"]) forces the sparse launch path of THIS handle (gda_set_option, GDA_OPT_SPARSE_PATH);
+    None leaves the choice to the library's cost model."""
     problem = getattr(w_or_problem, "problem", w_or_problem)
     path = sparse_path or getattr(w_or_problem, "extra", {}).get("sparse_path")
+    P = api.create_from_workload(problem)
     if path:
-        os.environ["GDA_SPARSE_PATH"] = path
-    try:
-        return api.create_from_workload(problem)
-    finally:
-        os.environ.pop("GDA_SPARSE_PATH", None)
+        P.set_option(api.OPT_SPARSE_PATH, api.SPARSE_PATH[path])
+    return P

@@ -94,6 +94,7 @@ def test_invalid_arguments_are_rejected_before_the_device(L):
     h = C.c_void_p(123)
     assert L.gda_create_qubo_csr(4, None, None, None, None, C.byref(h)) == 1 and h.value is None   # out set to NULL
     L.gda_destroy(None)                                           # NULL-safe
+    assert L.gda_set_option(None, api.OPT_GRAPHS, 0) == 1 and b"null handle" in L.gda_last_error()
 
 
 @pytest.mark.skipif(has_gpu(), reason="only meaningful on a box without a GPU")

@@ -66,14 +66,11 @@ IDS = [v[0] for v in VARIANTS]
 
 
 def create(api, name, problem):
-    """gda_create_qubo_dense; GDA_DENSE_SHAPE (read at create) forces the cluster-of-8 launch shape where asked."""
-    import os
+    """gda_create_qubo_dense; GDA_OPT_DENSE_SHAPE = 3 forces the cluster-of-8 launch shape on this handle where asked."""
+    P = api.create_from_workload(problem)
     if name == "cluster8_units":
-        os.environ["GDA_DENSE_SHAPE"] = "3"
-    try:
-        return api.create_from_workload(problem)
-    finally:
-        os.environ.pop("GDA_DENSE_SHAPE", None)
+        P.set_option(api.OPT_DENSE_SHAPE, 3)
+    return P
 
 
 def sample_columns(B, k=24):

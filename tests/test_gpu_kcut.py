@@ -69,7 +69,7 @@ def test_teacher_forced_steps(api, w):
 
 @pytest.mark.parametrize("w", CASES, ids=lambda w: w.name)
 def test_rows_split_across_the_warps_of_a_block(api, w):
-    """kcut_step_kernel<.., SPLIT>: a block of 8 warps per node (slices of 8 neighbours); forced with GDA_SPARSE_SPLIT_ALL=1,
+    """kcut_step_kernel<.., SPLIT>: a block of 8 warps per node (slices of 8 neighbours); forced with GDA_OPT_SPLIT_ALL_ROWS = 1,
     read at every launch.  One step against the oracle and against the warp-per-node kernel, exact objectives after a run."""
     import os
     Pw, h = w.problem, w.hyper
@@ -79,13 +79,10 @@ def test_rows_split_across_the_warps_of_a_block(api, w):
     Z0 = wl.z0_uniform(k, n, B, w.x0_seed)
     out = {}
     for sw in ("1", "0"):
-        os.environ["GDA_SPARSE_SPLIT_ALL"] = sw
-        try:
-            r1 = P.run(dev(Z0), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
-            r = P.run(dev(Z0), h.lambda0, api.params_from_hyper(h, iters=230, eval_every=50))
-            torch.cuda.synchronize()
-        finally:
-            os.environ.pop("GDA_SPARSE_SPLIT_ALL", None)
+        P.set_option(api.OPT_SPLIT_ALL_ROWS, int(sw))
+        r1 = P.run(dev(Z0), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
+        r = P.run(dev(Z0), h.lambda0, api.params_from_hyper(h, iters=230, eval_every=50))
+        torch.cuda.synchronize()
         ref = kcut.run(OP, Z0, f32(h.lambda0), **okw(h, iters=1, eval_every=1))
         assert (np.abs(r1["x"].cpu().numpy() - ref["z"]) <= TOL_STEP * np.maximum(1.0, np.abs(ref["z"]))).all()
         assert (np.abs(r1["lam"].cpu().numpy() - ref["y"]) <= TOL_STEP * np.maximum(1.0, np.abs(ref["y"]))).all()

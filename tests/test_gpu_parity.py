@@ -329,8 +329,7 @@ def test_sparse_edge_cases(api, oracle, case, path):
 def test_all_rows_through_the_row_split_kernel(api, oracle, case, B, dual):
     """Few warps that each walk a long row are bound by the latency of that walk (config 2's graph at the paper's B = 100:
     800 warps); the launcher then sends EVERY row through the row-split kernel with slices of 8 entries
-    (split_all_rows in gda_sparse.cu; forced here with GDA_SPARSE_SPLIT_ALL=1, which is read at every launch)."""
-    import os
+    (split_all_rows in gda_sparse.cu; forced here with GDA_OPT_SPLIT_ALL_ROWS = 1 on the handle)."""
     if case == "cfg2":
         w = wl.config(2, B=B, n_scale=0.5)
         Pw, h = w.problem, w.hyper
@@ -343,9 +342,9 @@ def test_all_rows_through_the_row_split_kernel(api, oracle, case, B, dual):
     OP = oracle_problem(Pw)
     n = Pw.n
     X0 = wl.x0_uniform(n, B, 17)
-    os.environ["GDA_SPARSE_SPLIT_ALL"] = "1"
-    try:
+    if True:
         P = create_problem(api, Pw, sparse_path="stream")
+        P.set_option(api.OPT_SPLIT_ALL_ROWS, 1)
         r1 = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
         ref = oracle.run(OP, X0, f32(h.lambda0), **okw(h, iters=1, eval_every=1))
         assert np.abs(r1["x"].cpu().numpy() - ref["x"]).max() <= TOL_STEP
@@ -357,11 +356,9 @@ def test_all_rows_through_the_row_split_kernel(api, oracle, case, B, dual):
         assert np.array_equal(obj, Fref) if case != "general_float" else np.allclose(obj, Fref, rtol=1e-6, atol=1e-5)
         G = P.grad(dev(X0)).cpu().numpy()
         assert grad_rel_err(G, oracle.grad(OP, X0.astype(np.float64))) <= TOL_STEP
-        os.environ["GDA_SPARSE_SPLIT_ALL"] = "0"                 # the same run with a warp per row: same objective values
+        P.set_option(api.OPT_SPLIT_ALL_ROWS, 0)                  # the same run with a warp per row: same objective values
         r0 = P.run(dev(X0), h.lambda0, api.params_from_hyper(h, iters=1, eval_every=1), want_final=True)
         assert np.abs(r0["x"].cpu().numpy() - r1["x"].cpu().numpy()).max() <= 2 * TOL_STEP
-    finally:
-        os.environ.pop("GDA_SPARSE_SPLIT_ALL", None)
     P.destroy()
 
 
@@ -495,14 +492,18 @@ def test_trace_of_a_resumed_run_after_more_evaluations_than_the_internal_buffer_
 
 def test_two_handles_from_two_threads(api, oracle):
     """include/gda.h only forbids sharing ONE handle: two handles driven from two host threads at the same time
-    (first-call kernel configuration included) give the results of the serial runs."""
+    (first-call kernel configuration included) give the results of the serial runs.  Launch options are per handle
+    (gda_set_option; the library reads no environment variable): the two handles of the SAME sparse instance are forced onto
+    different paths at the same time, one through the slab kernel (one launch per chunk), one through the streaming kernels."""
     import threading
     ws = [wl.config(1), wl.config(4, B=128, n_scale=0.0625), wl.config(1), wl.config(4, B=256, n_scale=0.125)]
+    paths = ["slab", None, "stream", None]
+    step_launches = [None] * len(ws)
     prms = [api.params_from_hyper(w.hyper, iters=120, eval_every=40) for w in ws]
     x0s = [dev(wl.x0_uniform(w.problem.n, w.B, w.x0_seed)) for w in ws]
     serial = []
-    for w, prm, x0 in zip(ws, prms, x0s):
-        P = create_problem(api, w)
+    for w, prm, x0, path in zip(ws, prms, x0s, paths):
+        P = create_problem(api, w, sparse_path=path)
         serial.append(P.run(x0, w.hyper.lambda0, prm)["obj"].cpu().numpy())
         P.destroy()
     results, errors = [None] * len(ws), []
@@ -511,10 +512,11 @@ def test_two_handles_from_two_threads(api, oracle):
         try:
             s = torch.cuda.Stream()
             with torch.cuda.stream(s):
-                P = api.create_from_workload(ws[k].problem)
+                P = create_problem(api, ws[k], sparse_path=paths[k])
                 for _ in range(3):
                     r = P.run(x0s[k], ws[k].hyper.lambda0, prms[k])
                 s.synchronize()
+                step_launches[k] = P.info().last_run_step_launches
                 results[k] = r["obj"].cpu().numpy()
                 P.destroy()
         except Exception as e:      # noqa: BLE001
@@ -527,12 +529,12 @@ def test_two_handles_from_two_threads(api, oracle):
     assert not errors, errors
     for a, b in zip(results, serial):
         assert np.array_equal(a, b)
+    assert step_launches[0] == 3 and step_launches[2] == 120    # 3 chunks of 40 steps: one slab launch each / one launch per step
 
 
 @pytest.mark.parametrize("kind", ["sparse_stream", "sparse_slab", "maxsat", "dense"])
 def test_run_without_cuda_graphs_is_bit_identical(api, kind):
-    """GDA_NO_GRAPH=1 (read at every chunk) enqueues the same kernels directly instead of replaying a captured graph."""
-    import os
+    """GDA_OPT_GRAPHS = 0 enqueues the same kernels directly instead of replaying a captured graph."""
     w = {"sparse_stream": wl.config(3, B=132, n_scale=0.05), "sparse_slab": wl.config(2, B=64, n_scale=0.25),
          "maxsat": wl.config(5, B=64, n_scale=0.05), "dense": wl.config(4, B=128, n_scale=0.0625)}[kind]
     P = create_problem(api, w, sparse_path="stream" if kind == "sparse_stream" else None)
@@ -540,12 +542,9 @@ def test_run_without_cuda_graphs_is_bit_identical(api, kind):
     prm = api.params_from_hyper(w.hyper, iters=230, eval_every=50)
     a = P.run(x0, w.hyper.lambda0, prm, want_final=True)
     xa, oa, ba = a["x"].clone(), a["obj"].clone(), a["x_bin"].clone()
-    os.environ["GDA_NO_GRAPH"] = "1"
-    try:
-        b = P.run(x0, w.hyper.lambda0, prm, want_final=True)
-        torch.cuda.synchronize()
-    finally:
-        os.environ.pop("GDA_NO_GRAPH", None)
+    P.set_option(api.OPT_GRAPHS, 0)
+    b = P.run(x0, w.hyper.lambda0, prm, want_final=True)
+    torch.cuda.synchronize()
     assert torch.equal(b["x"], xa) and torch.equal(b["obj"], oa) and torch.equal(b["x_bin"], ba)
     P.destroy()
 
@@ -743,8 +742,8 @@ def test_pdbo_s_free_running_and_full_run(api, oracle, w):
 
 
 def test_pdbo_s_row_grouping_is_bit_identical(api):
-    """The PDBO-s step kernel walks the rows grouped by adjacency (locality_order in gda_api.cu; GDA_SPARSE_LOCALITY=0, read
-    at create, switches the list off).  Which rows share a block changes nothing that is computed: the sums of g are exact
+    """The PDBO-s step kernel walks the rows grouped by adjacency (locality_order in gda_api.cu; GDA_OPT_ROW_GROUPING = 0
+    switches the list off for a handle).  Which rows share a block changes nothing that is computed: the sums of g are exact
     integers (fixed point), so iterates, multipliers and objectives agree bit for bit."""
     import os
     w = wl.pdbo_s_variant(wl.config(3, B=260, n_scale=0.2))
@@ -752,12 +751,9 @@ def test_pdbo_s_row_grouping_is_bit_identical(api):
     x0 = dev(wl.x0_uniform(w.problem.n, w.B, w.x0_seed))
     prm = api.params_from_hyper(h, iters=230, eval_every=50)
     res = []
-    for sw in ("1", "0"):
-        os.environ["GDA_SPARSE_LOCALITY"] = sw
-        try:
-            P = create_problem(api, w, sparse_path="stream")
-        finally:
-            os.environ.pop("GDA_SPARSE_LOCALITY", None)
+    for sw in (1, 0):
+        P = create_problem(api, w, sparse_path="stream")
+        P.set_option(api.OPT_ROW_GROUPING, sw)
         r = P.run(x0, h.lambda0, prm, want_final=True)
         torch.cuda.synchronize()
         res.append((r["x"].clone(), r["lam"].clone(), r["obj"].clone(), r["x_bin"].clone()))
