@@ -21,6 +21,9 @@ constexpr int THREADS = WARPS * 32;
 // step with 8 warps, 39.75 with 4, 39.35 with 2); PDBO-s: 8, one gpart row per block of 8 variables
 __host__ __device__ constexpr int step_warps(bool dual) { return dual ? WARPS : 2; }
 constexpr int SCORE_CLAUSES = 128;
+#ifndef GDA_MS_SLOTS_PER_BATCH
+#define GDA_MS_SLOTS_PER_BATCH 2
+#endif
 
 // Slot records hold each OTHER literal encoded as  enc = var | (positive ? 0x80000000 : 0);  ENC_PAD marks padding.
 // p_l(x) = off + sgn * x with (off, sgn) = (1, -1) for a positive literal and (0, +1) for a negated one.
@@ -54,7 +57,7 @@ __device__ __forceinline__ float4 gather_var(const float* __restrict__ coef, con
 #pragma unroll
             for (int q = 0; q < KW; ++q) my_o[q] = (s < end) ? __ldg(others + (size_t)s * KW + q) : (int)ENC_PAD;
             const int cnt = min(32, end - base);
-            constexpr int U = 2;                                  // slots per batch: U*KW independent 512 B gathers in flight
+            constexpr int U = GDA_MS_SLOTS_PER_BATCH;             // slots per batch: U*KW independent 512 B gathers in flight
             for (int u0 = 0; u0 < cnt; u0 += U * ngrp) {
                 float cf[U]; int l[U][KW > 0 ? KW : 1]; float4 t[U][KW > 0 ? KW : 1];
 #pragma unroll
